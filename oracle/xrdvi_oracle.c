@@ -1,0 +1,456 @@
+/*
+ * xrdvi_oracle.c -- plain, slow, fp64 CPU oracle for the ELBO-and-gradient hot path of
+ * "Rapid, Comprehensive Search of Crystalline Phases from X-ray Diffraction in Seconds via
+ * GPU-Accelerated Bayesian Variational Inference" (arXiv 2501.09308; PAPER.md).
+ *
+ * THIS IS TEST INFRASTRUCTURE, NOT THE PRODUCT.  Only tests/, __graft_entry__.smoke() and the
+ * cpu_baseline / --impl reference legs of bench.py may load it.  It shares no code, header,
+ * table or pre/post-processing with the CUDA path (paper_2501_09308_b200/csrc); it is written
+ * from the paper and the readings listed in DESIGN.md ("Readings"), one loop per sum in the
+ * paper, no blocking, no fusion, no reordering.
+ *
+ * What follows which passage:
+ *   profile   f = S_F + B, S_F = sum_k h_k C_k, C_k = sum_m I_m V, V = (1-r) G + r L,
+ *             rho_mk = p_m + mu_k                         PAPER.md:204-232 (A3-A8)
+ *   G, L      bodies missing from PAPER.md -> unit-area FWHM forms (reading R1)
+ *   window    static integer window |i - j_m| <= n_c       (reading R16; W<=0 -> dense)
+ *   ll        Gaussian, known sigma_n                      (reading R3; paper: Poisson A12-A16)
+ *   priors    h~Exp(lambda_h) eq.(3); mu~N(0,0.03), w~Gam(3,rate), r~U(0,1)
+ *             PAPER.md:274 (B.2); rate reading of "scale" (R12)
+ *   q         mean-field Gaussian in unconstrained space, eq.(10) PAPER.md:131 (R6)
+ *   ELBO      eq.(7) PAPER.md:111 as MC mean + analytic entropy (R7), pathwise gradient (R8)
+ *   optimiser Adam ascent, "1000 optimization steps" PAPER.md:138 (R10)
+ *   inclusion closed form from (m, l), 1 % area threshold PAPER.md:140 (R15)
+ *   draws     Philox4x32-10, counter (iter, s, k, inst), key (seed_lo, seed_hi) (R18)
+ *
+ * Pins (tests/test_oracle_pins.py): unit area and half-height of G/L/V, normal/Cauchy pdf
+ * special cases, zero-inclusion, shift and dummy-peak invariances, linearity in h, direct
+ * normal log-pdf, closed-form prior-only ELBO, Philox known-answer vectors, central finite
+ * differences of the fixed-draw ELBO, first Adam step, brute force over 2^K subsets.
+ * Unpinned: the absolute ELBO as a bound on ln p(Y) ("parity unpinned" for that reading only).
+ *
+ * Layouts: state[P][R][2][K][4] doubles: [0]=m (variational mean), [1]=l (log sigma);
+ * the 4 latent classes are ordered (h, mu, w, r) in unconstrained space zeta:
+ *   h = exp(zeta_h), mu = zeta_mu, w = exp(zeta_w), r = 1/(1+exp(-zeta_r)).
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+typedef struct {
+    double lambda_h;       /* <=0: auto 1/eta_h per pattern (R13)            */
+    double mu_sigma;       /* 0.03                                           */
+    double w_shape, w_rate;
+    double noise_sigma;    /* <=0: auto 0.01*max(y-B) per pattern (R4)       */
+    double window_W, fwhm_ref;
+    double incl_tau;
+    double lr, beta1, beta2, adam_eps;
+    double init_log_sigma;
+    int32_t n_patterns, n_restarts;
+} orc_hyper;
+
+typedef struct {
+    int64_t N;
+    int32_t K;
+    int64_t M;
+    int32_t P, R;
+    double *x;             /* [N]                                            */
+    double *y, *B;         /* [P][N]                                         */
+    int64_t *ofs;          /* [K+1]                                          */
+    double *pos, *inten;   /* [M]                                            */
+    int64_t *jm;           /* [M] nearest grid index (may lie outside [0,N)) */
+    int64_t n_c;           /* window half width in points; <0 -> dense       */
+    double delta;          /* grid step                                      */
+    double *sigma_n;       /* [P]                                            */
+    double *lambda_h;      /* [P]                                            */
+    double *eta_h;         /* [P]                                            */
+    orc_hyper hy;
+} orc_problem;
+
+/* ------------------------------------------------------------------ Philox4x32-10 (R18) */
+static void mulhilo(uint32_t a, uint32_t b, uint32_t *hi, uint32_t *lo) {
+    uint64_t p = (uint64_t)a * (uint64_t)b;
+    *hi = (uint32_t)(p >> 32);
+    *lo = (uint32_t)p;
+}
+
+void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]) {
+    uint32_t c0 = ctr[0], c1 = ctr[1], c2 = ctr[2], c3 = ctr[3];
+    uint32_t k0 = key[0], k1 = key[1];
+    for (int round = 0; round < 10; ++round) {
+        uint32_t hi0, lo0, hi1, lo1;
+        mulhilo(0xD2511F53u, c0, &hi0, &lo0);
+        mulhilo(0xCD9E8D57u, c2, &hi1, &lo1);
+        uint32_t n0 = hi1 ^ c1 ^ k0;
+        uint32_t n1 = lo1;
+        uint32_t n2 = hi0 ^ c3 ^ k1;
+        uint32_t n3 = lo0;
+        c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+        k0 += 0x9E3779B9u;
+        k1 += 0xBB67AE85u;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+/* u = ((word >> 9) + 1/2) 2^-23 in (0,1): exact in fp32 and fp64. */
+static double uniform23(uint32_t w) { return ((double)(w >> 9) + 0.5) * (1.0 / 8388608.0); }
+
+/* The four standard normals of (iteration, draw s, phase k, instance inst):
+ * (eps_h, eps_mu) = BoxMuller(u0,u1), (eps_w, eps_r) = BoxMuller(u2,u3). */
+void orc_eps(uint64_t seed, uint64_t iteration, uint32_t inst, uint32_t s, uint32_t k, double eps[4]) {
+    uint32_t ctr[4] = {(uint32_t)iteration, s, k, inst};
+    uint32_t key[2] = {(uint32_t)seed, (uint32_t)(seed >> 32)};
+    uint32_t w[4];
+    orc_philox4x32_10(ctr, key, w);
+    double u0 = uniform23(w[0]), u1 = uniform23(w[1]), u2 = uniform23(w[2]), u3 = uniform23(w[3]);
+    double r0 = sqrt(-2.0 * log(u0)), r1 = sqrt(-2.0 * log(u2));
+    eps[0] = r0 * cos(2.0 * M_PI * u1);
+    eps[1] = r0 * sin(2.0 * M_PI * u1);
+    eps[2] = r1 * cos(2.0 * M_PI * u3);
+    eps[3] = r1 * sin(2.0 * M_PI * u3);
+}
+
+/* ------------------------------------------------------------------ problem set-up */
+void orc_destroy(orc_problem *q) {
+    if (!q) return;
+    free(q->x); free(q->y); free(q->B); free(q->ofs); free(q->pos); free(q->inten);
+    free(q->jm); free(q->sigma_n); free(q->lambda_h); free(q->eta_h);
+    free(q);
+}
+
+static void *dup_mem(const void *src, size_t bytes) {
+    void *p = malloc(bytes ? bytes : 1);
+    if (src && bytes) memcpy(p, src, bytes);
+    return p;
+}
+
+orc_problem *orc_create(const double *x, int64_t N, const double *y, const double *B, int32_t K,
+                        const int64_t *ofs, const double *pos, const double *inten,
+                        const orc_hyper *hy) {
+    orc_problem *q = (orc_problem *)calloc(1, sizeof(orc_problem));
+    q->hy = *hy;
+    q->N = N; q->K = K; q->M = ofs[K];
+    q->P = hy->n_patterns > 0 ? hy->n_patterns : 1;
+    q->R = hy->n_restarts > 0 ? hy->n_restarts : 1;
+    q->x = (double *)dup_mem(x, sizeof(double) * N);
+    q->y = (double *)dup_mem(y, sizeof(double) * N * q->P);
+    if (B) q->B = (double *)dup_mem(B, sizeof(double) * N * q->P);
+    else   q->B = (double *)calloc((size_t)(N * q->P), sizeof(double));
+    q->ofs = (int64_t *)dup_mem(ofs, sizeof(int64_t) * (K + 1));
+    q->pos = (double *)dup_mem(pos, sizeof(double) * q->M);
+    q->inten = (double *)dup_mem(inten, sizeof(double) * q->M);
+    q->jm = (int64_t *)malloc(sizeof(int64_t) * (q->M ? q->M : 1));
+    q->delta = (x[N - 1] - x[0]) / (double)(N - 1);
+    /* R16: j_m = floor((p_m - x_0)/Delta + 1/2); n_c = ceil(W fwhm_ref / Delta - 1e-9)
+     * (the 1e-9 keeps an exact ratio such as 1.5/0.02 = 75 from rounding up to 76) */
+    for (int64_t m = 0; m < q->M; ++m) q->jm[m] = (int64_t)floor((pos[m] - x[0]) / q->delta + 0.5);
+    if (hy->window_W > 0.0) q->n_c = (int64_t)ceil(hy->window_W * hy->fwhm_ref / q->delta - 1e-9);
+    else q->n_c = -1;
+    q->sigma_n = (double *)malloc(sizeof(double) * q->P);
+    q->lambda_h = (double *)malloc(sizeof(double) * q->P);
+    q->eta_h = (double *)malloc(sizeof(double) * q->P);
+    double imax = 0.0;
+    for (int64_t m = 0; m < q->M; ++m) if (inten[m] > imax) imax = inten[m];
+    for (int32_t p = 0; p < q->P; ++p) {
+        double smax = -INFINITY;                           /* eta = max(Y - B) */
+        for (int64_t i = 0; i < N; ++i) {
+            double v = q->y[p * N + i] - q->B[p * N + i];
+            if (v > smax) smax = v;
+        }
+        q->sigma_n[p] = hy->noise_sigma > 0.0 ? hy->noise_sigma : 0.01 * smax;            /* R4  */
+        q->eta_h[p] = smax * hy->fwhm_ref / (imax > 0.0 ? imax : 1.0);                    /* R13 */
+        q->lambda_h[p] = hy->lambda_h > 0.0 ? hy->lambda_h : 1.0 / q->eta_h[p];
+    }
+    return q;
+}
+
+int64_t orc_window_halfwidth(const orc_problem *q) { return q->n_c; }
+double orc_sigma_n(const orc_problem *q, int32_t pat) { return q->sigma_n[pat]; }
+double orc_lambda_h(const orc_problem *q, int32_t pat) { return q->lambda_h[pat]; }
+
+/* R16: pair (m,i) is in the model iff |i - j_m| <= n_c and 0 <= i < N (dense: every i).
+ * The loops below run i over exactly that index range. */
+static void window(const orc_problem *q, int64_t m, int64_t *i_lo, int64_t *i_hi) {
+    if (q->n_c < 0) { *i_lo = 0; *i_hi = q->N - 1; return; }
+    *i_lo = q->jm[m] - q->n_c; if (*i_lo < 0) *i_lo = 0;
+    *i_hi = q->jm[m] + q->n_c; if (*i_hi > q->N - 1) *i_hi = q->N - 1;
+}
+
+/* number of in-window (m,i) pairs per instance (the metric's unit) */
+int64_t orc_pair_count(const orc_problem *q) {
+    int64_t n = 0;
+    for (int64_t m = 0; m < q->M; ++m)
+        for (int64_t i = 0; i < q->N; ++i)
+            if (q->n_c < 0 || llabs(i - q->jm[m]) <= q->n_c) ++n;
+    return n;
+}
+
+/* ------------------------------------------------------------------ peak shapes (R1) */
+static const double LN2 = 0.69314718055994530942;
+
+double orc_gauss(double x, double rho, double w) {           /* unit area, FWHM w */
+    double t = (x - rho) / w;
+    return (2.0 / w) * sqrt(LN2 / M_PI) * exp(-4.0 * LN2 * t * t);
+}
+double orc_lorentz(double x, double rho, double w) {         /* unit area, FWHM w */
+    double t = (x - rho) / w;
+    return (2.0 / (M_PI * w)) / (1.0 + 4.0 * t * t);
+}
+double orc_pseudo_voigt(double x, double rho, double w, double r) {   /* A7 PAPER.md:226 */
+    return (1.0 - r) * orc_gauss(x, rho, w) + r * orc_lorentz(x, rho, w);
+}
+
+static void constrain(const double zeta[4], double *h, double *mu, double *w, double *r) {
+    *h = exp(zeta[0]);
+    *mu = zeta[1];
+    *w = exp(zeta[2]);
+    *r = 1.0 / (1.0 + exp(-zeta[3]));
+}
+
+/* ------------------------------------------------------------------ forward model */
+/* f_i = B_i + sum_k h_k sum_m I_m V(x_i; p_m + mu_k, w_k, r_k), pairs restricted to the window */
+void orc_profile(const orc_problem *q, int32_t pat, const double *zeta /*[K][4]*/, double *f /*[N]*/) {
+    const int64_t N = q->N;
+    for (int64_t i = 0; i < N; ++i) f[i] = q->B[pat * N + i];
+    for (int32_t k = 0; k < q->K; ++k) {
+        double h, mu, w, r;
+        constrain(zeta + 4 * k, &h, &mu, &w, &r);
+        for (int64_t m = q->ofs[k]; m < q->ofs[k + 1]; ++m) {
+            double rho = q->pos[m] + mu;                                  /* A8 */
+            int64_t i_lo, i_hi;
+            window(q, m, &i_lo, &i_hi);
+            for (int64_t i = i_lo; i <= i_hi; ++i) {
+                f[i] += h * q->inten[m] * orc_pseudo_voigt(q->x[i], rho, w, r);
+            }
+        }
+    }
+}
+
+/* ll = -1/2 sum_i ((y_i - f_i)/sigma_n)^2 - N ln sigma_n - (N/2) ln 2 pi */
+double orc_loglik(const orc_problem *q, int32_t pat, const double *f) {
+    const int64_t N = q->N;
+    double sn = q->sigma_n[pat], acc = 0.0;
+    for (int64_t i = 0; i < N; ++i) {
+        double z = (q->y[pat * N + i] - f[i]) / sn;
+        acc += z * z;
+    }
+    return -0.5 * acc - (double)N * log(sn) - 0.5 * (double)N * log(2.0 * M_PI);
+}
+
+/* log p(Phi) + log |d Phi / d zeta|  summed over phases */
+double orc_logprior_jac(const orc_problem *q, int32_t pat, const double *zeta) {
+    const orc_hyper *hy = &q->hy;
+    double lam = q->lambda_h[pat], acc = 0.0;
+    for (int32_t k = 0; k < q->K; ++k) {
+        double h, mu, w, r;
+        constrain(zeta + 4 * k, &h, &mu, &w, &r);
+        acc += log(lam) - lam * h + zeta[4 * k + 0];                                  /* eq.(3) + J */
+        acc += -0.5 * (mu / hy->mu_sigma) * (mu / hy->mu_sigma) - log(hy->mu_sigma * sqrt(2.0 * M_PI));
+        acc += hy->w_shape * log(hy->w_rate) - lgamma(hy->w_shape)
+             + (hy->w_shape - 1.0) * zeta[4 * k + 2] - hy->w_rate * w + zeta[4 * k + 2]; /* eq.(1) + J */
+        acc += log(r) + log(1.0 - r);                                                  /* U(0,1): 0 + J */
+    }
+    return acc;
+}
+
+/* ll, lpJ and the analytic gradient of (ll + lpJ) wrt zeta[K][4]; f_out optional */
+void orc_logjoint_grad(const orc_problem *q, int32_t pat, const double *zeta, double *ll_out,
+                       double *lpj_out, double *g /*[K][4]*/, double *f_out /*[N] or NULL*/) {
+    const int64_t N = q->N;
+    const orc_hyper *hy = &q->hy;
+    double *f = f_out ? f_out : (double *)malloc(sizeof(double) * N);
+    orc_profile(q, pat, zeta, f);
+    *ll_out = orc_loglik(q, pat, f);
+    *lpj_out = orc_logprior_jac(q, pat, zeta);
+    double sn = q->sigma_n[pat], lam = q->lambda_h[pat];
+    const double aG = 2.0 * sqrt(LN2 / M_PI), aL = 2.0 / M_PI;
+    for (int32_t k = 0; k < q->K; ++k) {
+        double h, mu, w, r;
+        constrain(zeta + 4 * k, &h, &mu, &w, &r);
+        double dh = 0.0, dmu = 0.0, dw = 0.0, dr = 0.0;
+        for (int64_t m = q->ofs[k]; m < q->ofs[k + 1]; ++m) {
+            double I = q->inten[m], rho = q->pos[m] + mu;
+            int64_t i_lo, i_hi;
+            window(q, m, &i_lo, &i_hi);
+            for (int64_t i = i_lo; i <= i_hi; ++i) {
+                double e = (q->y[pat * N + i] - f[i]) / (sn * sn);          /* d ll / d f_i */
+                double t = (q->x[i] - rho) / w;
+                double G = exp(-4.0 * LN2 * t * t), L = 1.0 / (1.0 + 4.0 * t * t);
+                double Gn = (aG / w) * G, Ln = (aL / w) * L;                 /* unit-area values */
+                double V = (1.0 - r) * Gn + r * Ln;
+                /* dV/dt: dG/dt = -8 ln2 t G ; dL/dt = -8 t L^2 */
+                double dVdt = (1.0 - r) * (aG / w) * (-8.0 * LN2 * t * G) + r * (aL / w) * (-8.0 * t * L * L);
+                dh += e * I * V;
+                dr += e * I * h * (Ln - Gn);
+                dmu += e * I * h * dVdt * (-1.0 / w);                        /* dt/dmu = -1/w  */
+                dw += e * I * h * (-V / w + dVdt * (-t / w));                /* d(1/w)/dw, dt/dw = -t/w */
+            }
+        }
+        g[4 * k + 0] = dh * h + (1.0 - lam * h);
+        g[4 * k + 1] = dmu + (-mu / (hy->mu_sigma * hy->mu_sigma));
+        g[4 * k + 2] = dw * w + (hy->w_shape - hy->w_rate * w);
+        g[4 * k + 3] = dr * r * (1.0 - r) + (1.0 - 2.0 * r);
+    }
+    if (!f_out) free(f);
+}
+
+/* ------------------------------------------------------------------ ELBO and its gradient */
+/* state [P][R][2][K][4]; elbo [P][R]; grad [P][R][2][K][4]; optional per-instance outputs:
+ * ll_out [P][R][S], f_out [n_f][N] = profiles of the first n_f sample-instances (pat,rst,s order) */
+void orc_elbo_grad(const orc_problem *q, const double *state, int32_t S, uint64_t seed,
+                   uint64_t iteration, double *elbo, double *grad, double *ll_out, double *f_out,
+                   int64_t n_f) {
+    const int32_t K = q->K, P = q->P, R = q->R;
+    const int64_t N = q->N;
+    const int64_t T = (int64_t)P * R * S;
+    double *gz_all = (double *)malloc(sizeof(double) * (size_t)T * K * 4);
+    double *eps_all = (double *)malloc(sizeof(double) * (size_t)T * K * 4);
+    double *lj_all = (double *)malloc(sizeof(double) * (size_t)T * 2);
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int64_t t = 0; t < T; ++t) {
+        int32_t s = (int32_t)(t % S);
+        int32_t inst = (int32_t)(t / S);          /* inst = pat*R + rst */
+        int32_t pat = inst / R;
+        const double *m = state + (size_t)inst * 2 * K * 4, *l = m + (size_t)K * 4;
+        double *zeta = (double *)malloc(sizeof(double) * K * 4);
+        double *eps = eps_all + (size_t)t * K * 4;
+        for (int32_t k = 0; k < K; ++k) {
+            orc_eps(seed, iteration, (uint32_t)inst, (uint32_t)s, (uint32_t)k, eps + 4 * k);
+            for (int c = 0; c < 4; ++c) zeta[4 * k + c] = m[4 * k + c] + exp(l[4 * k + c]) * eps[4 * k + c];
+        }
+        double *fbuf = (f_out && t < n_f) ? f_out + (size_t)t * N : NULL;
+        orc_logjoint_grad(q, pat, zeta, &lj_all[2 * t], &lj_all[2 * t + 1], gz_all + (size_t)t * K * 4, fbuf);
+        if (ll_out) ll_out[t] = lj_all[2 * t];
+        free(zeta);
+    }
+    for (int32_t inst = 0; inst < P * R; ++inst) {
+        const double *l = state + (size_t)inst * 2 * K * 4 + (size_t)K * 4;
+        double *gm = grad + (size_t)inst * 2 * K * 4, *gl = gm + (size_t)K * 4;
+        double acc = 0.0;
+        for (int j = 0; j < 4 * K; ++j) { gm[j] = 0.0; gl[j] = 0.0; }
+        for (int32_t s = 0; s < S; ++s) {
+            int64_t t = (int64_t)inst * S + s;
+            acc += lj_all[2 * t] + lj_all[2 * t + 1];
+            for (int j = 0; j < 4 * K; ++j) {
+                double gz = gz_all[(size_t)t * K * 4 + j];
+                gm[j] += gz;
+                gl[j] += gz * eps_all[(size_t)t * K * 4 + j] * exp(l[j]);
+            }
+        }
+        double ent = 0.0;
+        for (int j = 0; j < 4 * K; ++j) {
+            gm[j] /= (double)S;
+            gl[j] = gl[j] / (double)S + 1.0;
+            ent += l[j] + 0.5 * log(2.0 * M_PI * M_E);
+        }
+        elbo[inst] = acc / (double)S + ent;
+    }
+    free(gz_all); free(eps_all); free(lj_all);
+}
+
+/* ------------------------------------------------------------------ optimiser (R10, R11) */
+/* Adam ascent with bias correction on every entry of state; l clamped to [-12, 2]. step >= 1. */
+void orc_adam_step(const orc_problem *q, double *state, const double *grad, double *mom1, double *mom2,
+                   int64_t step) {
+    const orc_hyper *hy = &q->hy;
+    const int64_t per = 2 * (int64_t)q->K * 4, total = per * q->P * q->R;
+    double bc1 = 1.0 - pow(hy->beta1, (double)step), bc2 = 1.0 - pow(hy->beta2, (double)step);
+    for (int64_t j = 0; j < total; ++j) {
+        mom1[j] = hy->beta1 * mom1[j] + (1.0 - hy->beta1) * grad[j];
+        mom2[j] = hy->beta2 * mom2[j] + (1.0 - hy->beta2) * grad[j] * grad[j];
+        double mh = mom1[j] / bc1, vh = mom2[j] / bc2;
+        state[j] += hy->lr * mh / (sqrt(vh) + hy->adam_eps);
+        int is_l = (j % per) >= per / 2;
+        if (is_l) {
+            if (state[j] < -12.0) state[j] = -12.0;
+            if (state[j] > 2.0) state[j] = 2.0;
+        }
+    }
+}
+
+/* R11: m_h = ln(eta_h/K), m_mu = 0, m_w = ln(alpha_w/lambda_w), m_r = 0, l = init_log_sigma;
+ * restart r > 0: m += (0.5, 0.01, 0.2, 0.5) * eps_init, eps_init = normals of Philox
+ * ctr = (0xFFFFFFFF, r, k, pat) under the given seed. */
+void orc_init_state(const orc_problem *q, uint64_t seed, double *state) {
+    const int32_t K = q->K;
+    static const double jit[4] = {0.5, 0.01, 0.2, 0.5};
+    for (int32_t pat = 0; pat < q->P; ++pat)
+        for (int32_t rst = 0; rst < q->R; ++rst) {
+            double *m = state + (size_t)(pat * q->R + rst) * 2 * K * 4, *l = m + (size_t)K * 4;
+            for (int32_t k = 0; k < K; ++k) {
+                m[4 * k + 0] = log(q->eta_h[pat] / (double)K);
+                m[4 * k + 1] = 0.0;
+                m[4 * k + 2] = log(q->hy.w_shape / q->hy.w_rate);
+                m[4 * k + 3] = 0.0;
+                if (rst > 0) {
+                    double e[4];
+                    uint32_t ctr[4] = {0xFFFFFFFFu, (uint32_t)rst, (uint32_t)k, (uint32_t)pat};
+                    uint32_t key[2] = {(uint32_t)seed, (uint32_t)(seed >> 32)};
+                    uint32_t wd[4];
+                    orc_philox4x32_10(ctr, key, wd);
+                    double u0 = uniform23(wd[0]), u1 = uniform23(wd[1]), u2 = uniform23(wd[2]), u3 = uniform23(wd[3]);
+                    double r0 = sqrt(-2.0 * log(u0)), r1 = sqrt(-2.0 * log(u2));
+                    e[0] = r0 * cos(2.0 * M_PI * u1); e[1] = r0 * sin(2.0 * M_PI * u1);
+                    e[2] = r1 * cos(2.0 * M_PI * u3); e[3] = r1 * sin(2.0 * M_PI * u3);
+                    for (int c = 0; c < 4; ++c) m[4 * k + c] += jit[c] * e[c];
+                }
+                for (int c = 0; c < 4; ++c) l[4 * k + c] = q->hy.init_log_sigma;
+            }
+        }
+}
+
+/* iterations of (elbo_grad at Philox iteration first_step+j, Adam step first_step+j), j=0.. ;
+ * first_step >= 1.  mom1/mom2 carried by the caller (zeros at first_step == 1). */
+void orc_fit(const orc_problem *q, double *state, double *mom1, double *mom2, int32_t iterations,
+             int32_t S, uint64_t seed, int64_t first_step, double *elbo_trace /*[iterations][P][R] or NULL*/) {
+    const int64_t per = 2 * (int64_t)q->K * 4, total = per * q->P * q->R;
+    double *grad = (double *)malloc(sizeof(double) * total);
+    double *elbo = (double *)malloc(sizeof(double) * q->P * q->R);
+    for (int32_t it = 0; it < iterations; ++it) {
+        int64_t step = first_step + it;
+        orc_elbo_grad(q, state, S, seed, (uint64_t)step, elbo, grad, NULL, NULL, 0);
+        if (elbo_trace) memcpy(elbo_trace + (size_t)it * q->P * q->R, elbo, sizeof(double) * q->P * q->R);
+        orc_adam_step(q, state, grad, mom1, mom2, step);
+    }
+    free(grad); free(elbo);
+}
+
+/* ------------------------------------------------------------------ read-out (R15) */
+static double normal_cdf(double z) { return 0.5 * erfc(-z / sqrt(2.0)); }
+
+/* A_k = sum_m I_m; Tbar = sum_j A_j exp(m_hj + s_hj^2/2);
+ * P_incl(k) = Phi((m_hk - ln(tau Tbar / A_k)) / s_hk); area_ratio = A_k E[h_k] / Tbar */
+void orc_inclusion(const orc_problem *q, const double *state, double *incl /*[P][R][K]*/,
+                   double *area_ratio /*[P][R][K] or NULL*/) {
+    const int32_t K = q->K;
+    for (int32_t inst = 0; inst < q->P * q->R; ++inst) {
+        const double *m = state + (size_t)inst * 2 * K * 4, *l = m + (size_t)K * 4;
+        double Tbar = 0.0;
+        for (int32_t k = 0; k < K; ++k) {
+            double A = 0.0;
+            for (int64_t mm = q->ofs[k]; mm < q->ofs[k + 1]; ++mm) A += q->inten[mm];
+            double s = exp(l[4 * k]);
+            Tbar += A * exp(m[4 * k] + 0.5 * s * s);
+        }
+        for (int32_t k = 0; k < K; ++k) {
+            double A = 0.0;
+            for (int64_t mm = q->ofs[k]; mm < q->ofs[k + 1]; ++mm) A += q->inten[mm];
+            double s = exp(l[4 * k]);
+            incl[(size_t)inst * K + k] = normal_cdf((m[4 * k] - log(q->hy.incl_tau * Tbar / A)) / s);
+            if (area_ratio) area_ratio[(size_t)inst * K + k] = A * exp(m[4 * k] + 0.5 * s * s) / Tbar;
+        }
+    }
+}
+
+int orc_num_threads(void) {
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
