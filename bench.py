@@ -1,0 +1,276 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the ELBO-and-gradient hot path (BASELINE.json metric).
+
+A *step* is one pass of the whole hot path over one batch of synthetic input: one optimisation
+iteration of the variational fit (Philox draws -> transform -> forward profile + residual ->
+backward six sums -> chain rule + reduction over draws -> Adam), i.e. one replay of the CUDA Graph
+xrdvi_fit runs.  Workload: config 1 of BASELINE.json (K=50 candidates = 2^50 combinations,
+N=4001, S=256 draws) unless --config says otherwise.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl ours|reference]
+
+One JSON line on stdout (rank 0).  `value` = peak.point pair evaluations per second (forward +
+backward of one in-window (peak, grid point) pair of one draw count as ONE evaluation), whole job.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import pathlib
+import statistics
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = pathlib.Path(__file__).resolve().parent
+sys.path.insert(0, str(ROOT))
+
+METRIC = "ELBO+grad peak-point evals/s"
+UNIT = "pair-evals/s"
+L2_FLUSH_BYTES = 256 << 20          # > 126 MB L2
+REF_DRAWS = 16                      # draws per step of the oracle arm (bounded sample)
+# Plain-formulation issue model of one pair: forward 5 FP32 + 2 MUFU,
+# backward 14 FP32 + 2 MUFU + 1/4 LDG.128; MUFU 16 lanes/SM/clk, FP32 128 lanes/SM/clk, 4 issue/SM/clk.
+PIPE = {"forward": dict(fp32=5, mufu=2, other=0.0), "backward": dict(fp32=14, mufu=2, other=0.25)}
+
+
+def alu_peak_pairs_per_s(kernel: str, n_sm: int, f_hz: float) -> float:
+    c = PIPE[kernel]
+    clk_per_pair = max(c["fp32"] / 128.0, c["mufu"] / 16.0, (c["fp32"] + c["mufu"] + c["other"]) / 128.0)
+    return n_sm * f_hz / clk_per_pair
+
+
+class ClockSampler:
+    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.tmp = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.proc = None
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--query-gpu={self.FIELDS}", "--format=csv,noheader,nounits", "-lms", "100",
+                 "-i", str(index)], stdout=self.tmp, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.proc = None
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        self.tmp.flush()
+        rows = [ln.strip().split(", ") for ln in open(self.tmp.name) if ln.strip()]
+        os.unlink(self.tmp.name)
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+            except (ValueError, IndexError):
+                continue
+            for nm, v in zip(names, r[3:7]):
+                if v.strip().lower() == "active":
+                    reasons.add(nm)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(mx), "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def measured_peaks() -> dict:
+    p = ROOT / "MEASURED_PEAKS.json"
+    if p.exists():
+        try:
+            return json.loads(p.read_text())
+        except Exception:
+            pass
+    return {}
+
+
+def run_reference(args, rank: int) -> None:
+    """Oracle arm: the fp64 CPU oracle, as it stands, on the host cores (rank 0 only)."""
+    if rank != 0:
+        return
+    from oracle import xrdvi_oracle as orc
+    from paper_2501_09308_b200 import synth
+    wl = synth.make_workload(args.config, n_patterns=1 if args.config == 3 else None,
+                             n_restarts=1 if args.config == 2 else None)
+    o = orc.from_workload(wl)
+    S = min(wl.S, REF_DRAWS)
+    pairs = o.pair_count()
+    st = o.init_state()
+    mom = None
+    st, mom, _ = o.fit(st, args.warmup, S, seed=1, first_step=1, mom=mom)
+    t0 = time.perf_counter()
+    st, mom, _ = o.fit(st, args.steps, S, seed=1, first_step=1 + args.warmup, mom=mom)
+    dt = time.perf_counter() - t0
+    value = pairs * S * args.steps / dt
+    cores = orc.num_threads()
+    sample = f"{S} of {wl.S} draws per step, 1 pattern x 1 restart, all {wl.K} phases and {wl.N} points"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"config{args.config}: K={wl.K} N={wl.N} M={wl.M} draws/step={S}",
+                   "pairs_per_instance": pairs},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+def run_ours(args, rank: int, local_rank: int, world: int) -> None:
+    import torch
+    from paper_2501_09308_b200 import Xrdvi, synth
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the hot path has no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist_mod
+        dist_mod.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+        dist = dist_mod
+
+    # weak scaling: every rank fits its own replica (own restart seed) of the same workload; the path
+    # shards over independent (pattern, restart) instances with no data-path collective.
+    wl = synth.make_workload(args.config)
+    gpu = Xrdvi.from_workload(wl, device=local_rank)
+    gpu.reset_state(seed=rank)
+    S, T = wl.S, wl.P * wl.R * wl.S
+    pairs = gpu.pair_count
+    gpu.bench_steps(max(args.warmup, 1), S=S, seed=1 + rank, l2_flush_bytes=L2_FLUSH_BYTES)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    barrier()
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+    ms = gpu.bench_steps(args.steps, S=S, seed=1 + rank, l2_flush_bytes=L2_FLUSH_BYTES)
+    barrier()
+    t_ms = float(ms.astype(np.float64).sum())
+    if dist is not None:
+        tt = torch.tensor([t_ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        t_ms = float(tt.item())
+    # per-kernel device times, measured live on the launching stream (CUDA events inside the library)
+    tk = gpu.time_kernels(S=S, seed=1 + rank, reps=30)
+    clocks = sampler.stop() if sampler else None
+
+    # end to end through the C ABI with HOST buffers: create (H2D of the pattern and peak tables) +
+    # fit + read-back of the variational parameters and inclusion probabilities, host wall clock.
+    barrier()
+    t0 = time.perf_counter()
+    gpu2 = Xrdvi.from_workload(wl, device=local_rank)
+    gpu2.reset_state(seed=rank)
+    st, inc, _ = gpu2.fit(args.steps, S=S, seed=1 + rank)
+    e2e_s = time.perf_counter() - t0
+    if dist is not None:
+        tt = torch.tensor([e2e_s], device="cuda", dtype=torch.float64)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        e2e_s = float(tt.item())
+    h2d = 8 * (wl.two_theta.size + wl.y.size + wl.background.size + wl.peak_pos.size + wl.peak_int.size
+               + wl.peak_ofs.size)
+    d2h = st.nbytes + inc.nbytes
+    gpu2.close()
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    value = pairs * T * args.steps * world / (t_ms * 1e-3)
+    props = torch.cuda.get_device_properties(local_rank)
+    n_sm = props.multi_processor_count
+    peaks = measured_peaks()
+    f_max = 1e6 * float(peaks.get("sm_max_mhz", 1965.0))
+    dom = "backward" if tk["ms_backward"] >= tk["ms_forward"] else "forward"
+    dom_ms = tk["ms_" + dom]
+    achieved = pairs * T / (dom_ms * 1e-3)
+    peak = alu_peak_pairs_per_s(dom, n_sm, f_max)
+    roofline = {
+        "bound": "alu", "kernel": dom + "_kernel", "achieved": achieved / 1e9, "peak": peak / 1e9,
+        "unit": "Gpair/s", "frac": achieved / peak, "traffic": None,
+        "peak_source": f"derived: {n_sm} SMs x {f_max / 1e6:.0f} MHz (MEASURED_PEAKS sm_max_mhz) / "
+                       f"max(fp32/128, mufu/16, issue/128) clk per pair, plain formulation (DESIGN.md)",
+        "ms_forward": tk["ms_forward"], "ms_backward": tk["ms_backward"], "ms_iteration_unfused": tk["ms_iteration"],
+        "frac_fwd_bwd_vs_R_plain": (pairs * T / ((tk["ms_forward"] + tk["ms_backward"]) * 1e-3)) / (n_sm * f_max * 4.0),
+    }
+    if clocks and clocks.get("sm_mhz"):
+        roofline["frac_at_achieved_clock"] = achieved / alu_peak_pairs_per_s(dom, n_sm, 1e6 * clocks["sm_mhz"])
+
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        from oracle import xrdvi_oracle as orc
+        wl1 = wl if (wl.P == 1 and wl.R == 1) else synth.make_workload(args.config, n_patterns=1, n_restarts=1)
+        o = orc.from_workload(wl1)
+        Sc = min(wl1.S, 256)
+        st0 = o.init_state()
+        o.elbo_grad(st0, min(Sc, 16), 1, 1)
+        reps, t0 = 0, time.perf_counter()
+        while True:
+            o.elbo_grad(st0, Sc, 1, 1 + reps)
+            reps += 1
+            if time.perf_counter() - t0 > 10.0 or reps >= 50:
+                break
+        dt = time.perf_counter() - t0
+        cpu = {"value": o.pair_count() * Sc * reps / dt, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle",
+               "sample": f"{reps} ELBO+gradient evaluations of {Sc} draws (1 pattern x 1 restart) of config {args.config}"}
+
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": t_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic",
+        "config": {"workload": f"config{args.config}: K={wl.K} (2^{wl.K} combinations) N={wl.N} M={wl.M} "
+                               f"P={wl.P} R={wl.R} S={wl.S}, window +-{gpu.n_c} points",
+                   "pairs_per_instance": pairs, "instances_per_step": T,
+                   "l2": f"flushed between timed steps ({L2_FLUSH_BYTES >> 20} MiB memset outside the event brackets)",
+                   "parallelism": f"replicas x{world} (independent restarts, no collective)"},
+        "fit_wall_s": e2e_s, "fit_iterations": args.steps,
+        "e2e": {"value": pairs * T * args.steps * world / e2e_s, "unit": UNIT,
+                "h2d_bytes_per_step": h2d / args.steps, "d2h_bytes_per_step": d2h / args.steps,
+                "covers": "xrdvi_create (host fp64 preprocessing + H2D) + xrdvi_fit + D2H of parameters and "
+                          "inclusion probabilities; inputs are uploaded once per fit"},
+        "gpu_launches": 6 * args.steps,
+        "roofline": roofline,
+        "cpu_baseline": cpu,
+        "clocks": clocks,
+    }
+    print(json.dumps(out))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main() -> None:
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=2000)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--config", type=int, default=1)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.impl == "reference":
+        run_reference(args, rank)
+    else:
+        run_ours(args, rank, local_rank, world)
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,162 @@
+/*
+ * xrdvi.h -- C ABI of the B200-native ELBO-and-gradient hot path of
+ * "Rapid, Comprehensive Search of Crystalline Phases from X-ray Diffraction in Seconds via
+ * GPU-Accelerated Bayesian Variational Inference" (arXiv 2501.09308).
+ *
+ * Citations are PAPER.md:<line> (the paper's text) and DESIGN.md "Readings" R<n> (how a silent,
+ * ambiguous or garbled passage is read; the same table binds the fp64 oracle).
+ *
+ * Problem statement (A1-A2): measured pattern D = {(x_i, y_i)}, i < N, and a
+ * candidate set F = {F_k}, k < K, F_k = {(p_m, I_m)}, m < M_k (ragged).  Profile model
+ * (A3-A8):
+ *     f(x_i) = B(x_i) + sum_k h_k sum_m I_m [ (1-r_k) G(x_i; p_m+mu_k, w_k) + r_k L(x_i; p_m+mu_k, w_k) ]
+ * with unit-area, FWHM-parameterised G and L (R1), a static +-n_c-point window per peak (R16), Gaussian
+ * noise of known sigma_n (R3), priors h~Exp(lambda_h) (eq.3), mu~N(0,mu_sigma),
+ * w~Gam(w_shape, rate w_rate), r~U(0,1) (B.2), and a mean-field Gaussian q (eq.10,
+ * PAPER.md:131) over the unconstrained latents zeta = (ln h, mu, ln w, logit r) (R6).
+ *
+ * General rules
+ *  - Every function returns 0 (XRDVI_OK) or a negative XRDVI_E_* code; on failure outputs are
+ *    untouched and xrdvi_last_error() (thread-local) describes the failure.  No exception or abort
+ *    crosses this boundary.  There is NO CPU fallback: without a CUDA device of compute capability
+ *    10.x every call fails with XRDVI_E_NOT_SM100 / XRDVI_E_CUDA.
+ *  - Pointers are HOST pointers unless the parameter says "device".  The caller owns every array;
+ *    inputs are copied during the call and never retained; outputs are written to caller memory.
+ *  - All device work is enqueued on the stream given at create; calls that return host outputs
+ *    synchronise that stream before returning.  Calls on one handle are not thread-safe.
+ *  - Results are bitwise reproducible for equal inputs (all reductions have a fixed order).
+ *
+ * Layout of variational parameters ("state"): float [P][R][2][K][4]; [..][0] = m (mean), [..][1] =
+ * l = log sigma; the last axis is the latent class (h, mu, w, r).  An "instance" is inst = pat*R + rst.
+ */
+#ifndef XRDVI_H
+#define XRDVI_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct xrdvi xrdvi; /* opaque; one per problem (P patterns x R restarts) */
+
+enum {
+    XRDVI_OK = 0,
+    XRDVI_E_INVALID_ARG = -1,
+    XRDVI_E_UNSORTED_GRID = -2,      /* 2theta not strictly increasing                      */
+    XRDVI_E_NONUNIFORM_GRID = -3,    /* 2theta not uniform to 1e-6 of the step (this build)  */
+    XRDVI_E_EMPTY_PHASE = -4,        /* a phase with M_k = 0                                 */
+    XRDVI_E_WORKSPACE_TOO_SMALL = -5,
+    XRDVI_E_CUDA = -6,
+    XRDVI_E_NOT_SM100 = -7
+};
+
+/* Hyper-parameters (POD, versioned by .size = sizeof(xrdvi_hyper)).  xrdvi_default_hyper fills the
+ * paper's values (B.2; threshold PAPER.md:140) and the DESIGN.md readings.          */
+typedef struct {
+    uint32_t size;
+    uint32_t _pad;
+    double lambda_h;       /* rate of the Exp prior on h (eq.3).  <=0: auto 1/eta_h per pattern,
+                              eta_h = max(y-B) * fwhm_ref / max(I) (R13)                          */
+    double mu_sigma;       /* 0.03 deg (B.2)                                                      */
+    double w_shape;        /* 3   (B.2)                                                           */
+    double w_rate;         /* 100 (B.2; lambda is a RATE, R12)                                     */
+    double noise_sigma;    /* Gaussian sigma_n.  <=0: auto 0.01 * max(y-B) per pattern (R4)       */
+    double window_W;       /* static cutoff c = window_W * fwhm_ref (deg).  <=0: dense (R16)      */
+    double fwhm_ref;       /* 0.15 deg                                                            */
+    double incl_tau;       /* 0.01: area-ratio threshold (R15)                      */
+    double lr, beta1, beta2, adam_eps; /* Adam ascent: 0.1, 0.9, 0.999, 1e-8 (R10)                */
+    double init_log_sigma; /* ln 0.1 (R11)                                                        */
+    int32_t n_patterns;    /* P >= 1                                                              */
+    int32_t n_restarts;    /* R >= 1                                                              */
+    int32_t likelihood;    /* 0 Gaussian (only value accepted by this build)                      */
+    int32_t _pad2;
+} xrdvi_hyper;
+
+void xrdvi_default_hyper(xrdvi_hyper* hyp);
+
+/* Bytes of device workspace xrdvi_create needs for draws up to S_max per (pattern, restart).
+ * Depends only on the sizes (an upper bound over peak positions).  0 on invalid arguments.      */
+size_t xrdvi_workspace_bytes(int64_t N, int32_t K, int64_t M, int32_t S_max, const xrdvi_hyper* hyp);
+
+/* Build a problem.
+ *  two_theta [N]     strictly increasing, uniform grid (deg)
+ *  y [P][N]          observed intensities;  background [P][N] or NULL (-> 0) (R5: B is an input)
+ *  peak_ofs [K+1]    CSR offsets into peak_pos / peak_int ([M], M = peak_ofs[K]); any order inside
+ *                    a phase; peaks with no in-window grid point are dropped (R16)
+ *  device, cuda_stream   CUDA device ordinal and a cudaStream_t (0 = legacy default stream)
+ *  workspace         DEVICE pointer, >= xrdvi_workspace_bytes(...) bytes, 256-byte aligned, owned by
+ *                    the caller and kept alive until xrdvi_destroy
+ * Preprocessing (sorting, grid-index encoding j_m/delta_m, window tables) is done on the host in
+ * fp64; the state is initialised as xrdvi_reset_state(h, 0).                                       */
+int xrdvi_create(const double* two_theta, int64_t N, const double* y, const double* background,
+                 int32_t K, const int64_t* peak_ofs, const double* peak_pos, const double* peak_int,
+                 const xrdvi_hyper* hyp, int32_t S_max, int device, void* cuda_stream,
+                 void* workspace, size_t workspace_bytes, xrdvi** out);
+
+void xrdvi_destroy(xrdvi* h);
+
+/* In-window (m,i) pairs per sample-instance: the unit of the throughput metric.                    */
+int64_t xrdvi_pair_count(const xrdvi* h);
+/* Window half-width n_c in grid points (N for dense).                                              */
+int64_t xrdvi_window_halfwidth(const xrdvi* h);
+
+/* (Re)initialise the variational state (R11), zero the Adam moments and the step counter.
+ * Restart r > 0 is jittered with Philox counter (0xFFFFFFFF, r, k, pat) under `seed`.              */
+int xrdvi_reset_state(xrdvi* h, uint64_t seed);
+/* Copy the state out / in: var_params float [P][R][2][K][4].  set_state also zeroes the Adam
+ * moments and sets the step counter to `step` (number of completed optimisation steps).            */
+int xrdvi_get_state(xrdvi* h, float* var_params, int64_t* step);
+int xrdvi_set_state(xrdvi* h, const float* var_params, int64_t step);
+
+/* One ELBO-and-gradient evaluation (eq.7 PAPER.md:111 as a Monte-Carlo mean over S reparameterised
+ * draws + analytic entropy, R7/R8):
+ *  var_params   float [P][R][2][K][4] or NULL (use the internal state; it is not modified)
+ *  S            draws per (pattern, restart), 1 <= S <= S_max
+ *  seed, iteration   Philox4x32-10 key and counter word 0; draw (s, k, inst) uses counter
+ *               (iteration, s, k, inst) (R18)
+ *  elbo         double [P][R];   grad  float [P][R][2][K][4] = d ELBO / d (m, l); either may be NULL */
+int xrdvi_elbo_grad(xrdvi* h, const float* var_params, int32_t S, uint64_t seed, uint64_t iteration,
+                    double* elbo, float* grad);
+
+/* `iterations` Adam-ascent steps from the internal state, each one a replay of a CUDA
+ * Graph (draw -> forward -> backward -> chain/reduce -> update); step t uses Philox iteration t, t
+ * continuing from the state's step counter + 1.  Outputs (each may be NULL, nothing is copied then):
+ *  var_params_out float [P][R][2][K][4]; incl_prob double [P][R][K] (R15);
+ *  elbo_trace double [iterations][P][R] (only the last 4096 iterations are kept; older rows = NaN)  */
+int xrdvi_fit(xrdvi* h, int32_t iterations, int32_t S, uint64_t seed, float* var_params_out,
+              double* incl_prob, double* elbo_trace);
+
+/* Posterior inclusion probability and area ratio per phase from the internal state (R15):
+ * incl_prob, area_ratio double [P][R][K], either may be NULL.                                      */
+int xrdvi_inclusion(xrdvi* h, double* incl_prob, double* area_ratio);
+
+/* Debug read-back of the forward pass for parity tests: runs draw + forward at (var_params or
+ * internal state, S, seed, iteration) and returns, for the first n sample-instances in
+ * (pat, rst, s) order, the profile f float [n][N] (including B) and ll double [n]; f or ll may be NULL. */
+int xrdvi_debug_profile(xrdvi* h, const float* var_params, int32_t S, uint64_t seed,
+                        uint64_t iteration, int64_t n, float* f, double* ll);
+
+/* Debug read-back of the draw kernel: eps float [n][K][4] for the first n sample-instances.        */
+int xrdvi_debug_draws(xrdvi* h, int32_t S, uint64_t seed, uint64_t iteration, int64_t n, float* eps,
+                      uint32_t* raw_words /* [n][K][4] or NULL */);
+
+/* Mean CUDA-event time (ms) of the kernels of the last xrdvi_fit call: total per iteration and the
+ * share measured separately for the forward and backward kernels by xrdvi_time_kernels.            */
+int xrdvi_time_kernels(xrdvi* h, int32_t S, uint64_t seed, int32_t reps, float* ms_forward,
+                       float* ms_backward, float* ms_iteration);
+
+/* Measurement: `steps` optimisation steps (graph replays, exactly as xrdvi_fit runs them), each one
+ * bracketed by its own pair of CUDA events on the handle's stream; between two steps, outside the
+ * brackets, `l2_flush_bytes` of device memory are overwritten (0 = no flush) so that every step starts
+ * with a cold L2.  ms_steps float [steps] receives the per-step device times.  The state advances.   */
+int xrdvi_bench_steps(xrdvi* h, int32_t steps, int32_t S, uint64_t seed, size_t l2_flush_bytes,
+                      float* ms_steps);
+
+const char* xrdvi_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* XRDVI_H */

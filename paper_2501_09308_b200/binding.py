@@ -1,0 +1,234 @@
+"""Thin Python binding of the C ABI in include/xrdvi.h (argument marshalling only).
+
+Every step of the hot path runs in the CUDA kernels of libxrdvi.so.  PyTorch is used for the
+device workspace (one uint8 tensor) and the CUDA stream, nothing else.  There is no CPU
+fallback: a missing library or a missing sm_100 device raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import pathlib
+
+import numpy as np
+
+_PKG = pathlib.Path(__file__).resolve().parent
+_LIB_PATH = _PKG / "libxrdvi.so"
+
+EXPORTS = (
+    "xrdvi_default_hyper", "xrdvi_workspace_bytes", "xrdvi_create", "xrdvi_destroy", "xrdvi_pair_count",
+    "xrdvi_window_halfwidth", "xrdvi_reset_state", "xrdvi_get_state", "xrdvi_set_state", "xrdvi_elbo_grad",
+    "xrdvi_fit", "xrdvi_inclusion", "xrdvi_debug_profile", "xrdvi_debug_draws", "xrdvi_time_kernels",
+    "xrdvi_bench_steps", "xrdvi_last_error",
+)
+
+
+class XrdviError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"xrdvi error {code}: {msg}")
+        self.code = code
+
+
+class Hyper(C.Structure):
+    """Mirror of ``xrdvi_hyper`` (include/xrdvi.h)."""
+    _fields_ = [
+        ("size", C.c_uint32), ("_pad", C.c_uint32),
+        ("lambda_h", C.c_double), ("mu_sigma", C.c_double), ("w_shape", C.c_double), ("w_rate", C.c_double),
+        ("noise_sigma", C.c_double), ("window_W", C.c_double), ("fwhm_ref", C.c_double),
+        ("incl_tau", C.c_double), ("lr", C.c_double), ("beta1", C.c_double), ("beta2", C.c_double),
+        ("adam_eps", C.c_double), ("init_log_sigma", C.c_double),
+        ("n_patterns", C.c_int32), ("n_restarts", C.c_int32), ("likelihood", C.c_int32), ("_pad2", C.c_int32),
+    ]
+
+
+_lib = None
+
+
+def load_library():
+    """dlopen libxrdvi.so (built in-tree by paper_2501_09308_b200.build); fails loudly if absent."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not _LIB_PATH.exists():
+        raise XrdviError(-100, f"{_LIB_PATH} not built; run `python -m paper_2501_09308_b200.build` "
+                               "(there is no CPU fallback)")
+    L = C.CDLL(str(_LIB_PATH))
+    vp, fp, dp = C.c_void_p, C.POINTER(C.c_float), C.POINTER(C.c_double)
+    L.xrdvi_default_hyper.argtypes = [C.POINTER(Hyper)]
+    L.xrdvi_default_hyper.restype = None
+    L.xrdvi_workspace_bytes.argtypes = [C.c_int64, C.c_int32, C.c_int64, C.c_int32, C.POINTER(Hyper)]
+    L.xrdvi_workspace_bytes.restype = C.c_size_t
+    L.xrdvi_create.argtypes = [dp, C.c_int64, dp, dp, C.c_int32, C.POINTER(C.c_int64), dp, dp, C.POINTER(Hyper),
+                               C.c_int32, C.c_int, vp, vp, C.c_size_t, C.POINTER(vp)]
+    L.xrdvi_destroy.argtypes = [vp]
+    L.xrdvi_destroy.restype = None
+    L.xrdvi_pair_count.argtypes = [vp]
+    L.xrdvi_pair_count.restype = C.c_int64
+    L.xrdvi_window_halfwidth.argtypes = [vp]
+    L.xrdvi_window_halfwidth.restype = C.c_int64
+    L.xrdvi_reset_state.argtypes = [vp, C.c_uint64]
+    L.xrdvi_get_state.argtypes = [vp, fp, C.POINTER(C.c_int64)]
+    L.xrdvi_set_state.argtypes = [vp, fp, C.c_int64]
+    L.xrdvi_elbo_grad.argtypes = [vp, fp, C.c_int32, C.c_uint64, C.c_uint64, dp, fp]
+    L.xrdvi_fit.argtypes = [vp, C.c_int32, C.c_int32, C.c_uint64, fp, dp, dp]
+    L.xrdvi_inclusion.argtypes = [vp, dp, dp]
+    L.xrdvi_debug_profile.argtypes = [vp, fp, C.c_int32, C.c_uint64, C.c_uint64, C.c_int64, fp, dp]
+    L.xrdvi_debug_draws.argtypes = [vp, C.c_int32, C.c_uint64, C.c_uint64, C.c_int64, fp, C.POINTER(C.c_uint32)]
+    L.xrdvi_time_kernels.argtypes = [vp, C.c_int32, C.c_uint64, C.c_int32, fp, fp, fp]
+    L.xrdvi_bench_steps.argtypes = [vp, C.c_int32, C.c_int32, C.c_uint64, C.c_size_t, fp]
+    L.xrdvi_last_error.restype = C.c_char_p
+    _lib = L
+    return L
+
+
+def default_hyper(**overrides) -> Hyper:
+    hy = Hyper()
+    load_library().xrdvi_default_hyper(C.byref(hy))
+    for k, v in overrides.items():
+        if k.startswith("_") or k == "size" or not hasattr(hy, k):
+            raise TypeError(f"unknown hyper-parameter {k!r}")
+        setattr(hy, k, v)
+    return hy
+
+
+def _check(rc):
+    if rc != 0:
+        raise XrdviError(rc, load_library().xrdvi_last_error().decode())
+
+
+def _f(a):
+    return a.ctypes.data_as(C.POINTER(C.c_float)) if a is not None else None
+
+
+def _d(a):
+    return a.ctypes.data_as(C.POINTER(C.c_double)) if a is not None else None
+
+
+class Xrdvi:
+    """One problem: P patterns x R restarts over a shared candidate library (xrdvi_create)."""
+
+    def __init__(self, two_theta, y, background, peak_ofs, peak_pos, peak_int, S_max, device=0, **hyper):
+        import torch  # device memory and stream only
+
+        L = load_library()
+        if not torch.cuda.is_available():
+            raise XrdviError(-6, "no CUDA device: the xrdvi hot path has no CPU fallback")
+        self.hyper = default_hyper(**hyper)
+        self.P, self.R = int(self.hyper.n_patterns), int(self.hyper.n_restarts)
+        x = np.ascontiguousarray(two_theta, dtype=np.float64)
+        self.N = int(x.shape[0])
+        yy = np.ascontiguousarray(np.asarray(y, dtype=np.float64).reshape(self.P, self.N))
+        bg = None if background is None else np.ascontiguousarray(
+            np.asarray(background, dtype=np.float64).reshape(self.P, self.N))
+        ofs = np.ascontiguousarray(peak_ofs, dtype=np.int64)
+        pos = np.ascontiguousarray(peak_pos, dtype=np.float64)
+        inten = np.ascontiguousarray(peak_int, dtype=np.float64)
+        self.K, self.M, self.S_max = int(ofs.shape[0] - 1), int(pos.shape[0]), int(S_max)
+        nbytes = int(L.xrdvi_workspace_bytes(self.N, self.K, self.M, self.S_max, C.byref(self.hyper)))
+        if nbytes == 0:
+            raise XrdviError(-1, "xrdvi_workspace_bytes: invalid sizes")
+        self.device = torch.device("cuda", device)
+        self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+        self.stream = torch.cuda.Stream(device=self.device)   # non-default: CUDA Graph capture needs it
+        self._h = C.c_void_p()
+        _check(L.xrdvi_create(_d(x), self.N, _d(yy), _d(bg), self.K, ofs.ctypes.data_as(C.POINTER(C.c_int64)),
+                              _d(pos), _d(inten), C.byref(self.hyper), self.S_max, device,
+                              C.c_void_p(self.stream.cuda_stream), C.c_void_p(self.workspace.data_ptr()),
+                              nbytes, C.byref(self._h)))
+        self.workspace_bytes = nbytes
+
+    @classmethod
+    def from_workload(cls, wl, S_max=None, device=0, **overrides):
+        hp = dict(wl.hyper)
+        hp.update(overrides)
+        return cls(wl.two_theta, wl.y, wl.background, wl.peak_ofs, wl.peak_pos, wl.peak_int,
+                   S_max=wl.S if S_max is None else S_max, device=device, **hp)
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            load_library().xrdvi_destroy(self._h)
+            self._h = C.c_void_p()
+        self.workspace = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ---- queries ---------------------------------------------------------------
+    @property
+    def pair_count(self) -> int:
+        return int(load_library().xrdvi_pair_count(self._h))
+
+    @property
+    def n_c(self) -> int:
+        return int(load_library().xrdvi_window_halfwidth(self._h))
+
+    def _state_shape(self):
+        return (self.P, self.R, 2, self.K, 4)
+
+    # ---- state -----------------------------------------------------------------
+    def reset_state(self, seed=0):
+        _check(load_library().xrdvi_reset_state(self._h, int(seed)))
+
+    def get_state(self):
+        st = np.empty(self._state_shape(), dtype=np.float32)
+        step = C.c_int64()
+        _check(load_library().xrdvi_get_state(self._h, _f(st), C.byref(step)))
+        return st, int(step.value)
+
+    def set_state(self, state, step=0):
+        st = np.ascontiguousarray(state, dtype=np.float32).reshape(self._state_shape())
+        _check(load_library().xrdvi_set_state(self._h, _f(st), int(step)))
+
+    # ---- hot path --------------------------------------------------------------
+    def elbo_grad(self, state=None, S=None, seed=0, iteration=0):
+        S = self.S_max if S is None else int(S)
+        st = None if state is None else np.ascontiguousarray(state, dtype=np.float32).reshape(self._state_shape())
+        elbo = np.empty((self.P, self.R), dtype=np.float64)
+        grad = np.empty(self._state_shape(), dtype=np.float32)
+        _check(load_library().xrdvi_elbo_grad(self._h, _f(st), S, int(seed), int(iteration), _d(elbo), _f(grad)))
+        return elbo, grad
+
+    def fit(self, iterations, S=None, seed=0, want_state=True, want_incl=True, want_trace=False):
+        S = self.S_max if S is None else int(S)
+        st = np.empty(self._state_shape(), dtype=np.float32) if want_state else None
+        inc = np.empty((self.P, self.R, self.K), dtype=np.float64) if want_incl else None
+        tr = np.empty((int(iterations), self.P, self.R), dtype=np.float64) if want_trace else None
+        _check(load_library().xrdvi_fit(self._h, int(iterations), S, int(seed), _f(st), _d(inc), _d(tr)))
+        return st, inc, tr
+
+    def inclusion(self):
+        inc = np.empty((self.P, self.R, self.K), dtype=np.float64)
+        ar = np.empty_like(inc)
+        _check(load_library().xrdvi_inclusion(self._h, _d(inc), _d(ar)))
+        return inc, ar
+
+    # ---- debug / measurement ---------------------------------------------------
+    def debug_profile(self, n, state=None, S=None, seed=0, iteration=0, want_f=True):
+        S = self.S_max if S is None else int(S)
+        st = None if state is None else np.ascontiguousarray(state, dtype=np.float32).reshape(self._state_shape())
+        f = np.empty((int(n), self.N), dtype=np.float32) if want_f else None
+        ll = np.empty(int(n), dtype=np.float64)
+        _check(load_library().xrdvi_debug_profile(self._h, _f(st), S, int(seed), int(iteration), int(n), _f(f), _d(ll)))
+        return f, ll
+
+    def debug_draws(self, n, S=None, seed=0, iteration=0):
+        S = self.S_max if S is None else int(S)
+        eps = np.empty((int(n), self.K, 4), dtype=np.float32)
+        raw = np.empty((int(n), self.K, 4), dtype=np.uint32)
+        _check(load_library().xrdvi_debug_draws(self._h, S, int(seed), int(iteration), int(n), _f(eps),
+                                                raw.ctypes.data_as(C.POINTER(C.c_uint32))))
+        return eps, raw
+
+    def time_kernels(self, S=None, seed=0, reps=20):
+        S = self.S_max if S is None else int(S)
+        a, b, c = C.c_float(), C.c_float(), C.c_float()
+        _check(load_library().xrdvi_time_kernels(self._h, S, int(seed), int(reps), C.byref(a), C.byref(b), C.byref(c)))
+        return dict(ms_forward=a.value, ms_backward=b.value, ms_iteration=c.value)
+
+    def bench_steps(self, steps, S=None, seed=0, l2_flush_bytes=0):
+        S = self.S_max if S is None else int(S)
+        ms = np.empty(int(steps), dtype=np.float32)
+        _check(load_library().xrdvi_bench_steps(self._h, int(steps), S, int(seed), int(l2_flush_bytes), _f(ms)))
+        return ms

@@ -1,0 +1,31 @@
+"""Compile the CUDA library (C ABI of include/xrdvi.h) for sm_100a, in-tree.
+
+``python -m paper_2501_09308_b200.build`` or ``__graft_entry__.build()``.  nvcc cross-compiles
+without a GPU; the resulting paper_2501_09308_b200/libxrdvi.so travels with the tree.
+"""
+from __future__ import annotations
+
+import pathlib
+import subprocess
+
+PKG = pathlib.Path(__file__).resolve().parent
+CSRC = PKG / "csrc"
+LIB = PKG / "libxrdvi.so"
+SOURCES = [CSRC / "xrdvi.cu"]
+DEPS = SOURCES + [CSRC / "xrdvi_kernels.cuh", PKG.parent / "include" / "xrdvi.h"]
+
+NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
+              "-Xcompiler", "-fPIC", "-shared", "-cudart", "static"]
+
+
+def build(force: bool = False, verbose: bool = False) -> pathlib.Path:
+    if not force and LIB.exists() and all(LIB.stat().st_mtime >= p.stat().st_mtime for p in DEPS):
+        return LIB
+    cmd = ["nvcc", *NVCC_FLAGS, *(["-Xptxas", "-v"] if verbose else []), "-o", str(LIB), *map(str, SOURCES)]
+    subprocess.run(cmd, check=True)
+    return LIB
+
+
+if __name__ == "__main__":
+    import sys
+    print(build(force=True, verbose="-v" in sys.argv))

@@ -1,0 +1,81 @@
+"""CPU-side checks of the boundary: the library loads, exports every symbol include/xrdvi.h
+declares, the hyper struct mirrors the header, and argument validation fails loudly (no GPU needed)."""
+import ctypes as C
+import pathlib
+import re
+
+import numpy as np
+import pytest
+
+from paper_2501_09308_b200 import binding, build
+
+ROOT = pathlib.Path(__file__).resolve().parents[1]
+
+
+@pytest.fixture(scope="module")
+def lib():
+    build.build()
+    return binding.load_library()
+
+
+def test_every_declared_symbol_is_exported(lib):
+    header = (ROOT / "include" / "xrdvi.h").read_text()
+    header = re.sub(r"/\*.*?\*/", "", header, flags=re.S)
+    declared = set(re.findall(r"\b(xrdvi_[a-z_]+)\s*\(", header))
+    assert declared == set(binding.EXPORTS)
+    for name in declared:
+        assert hasattr(lib, name), name
+
+
+def test_hyper_struct_mirrors_header(lib):
+    hy = binding.default_hyper()
+    assert hy.size == C.sizeof(binding.Hyper)
+    assert (hy.mu_sigma, hy.w_shape, hy.w_rate) == (0.03, 3.0, 100.0)          # PAPER.md:274 (B.2)
+    assert hy.incl_tau == 0.01
+    assert (hy.lr, hy.beta1, hy.beta2, hy.adam_eps) == (0.1, 0.9, 0.999, 1e-8)
+    assert hy.init_log_sigma == pytest.approx(np.log(0.1))
+    assert (hy.n_patterns, hy.n_restarts, hy.likelihood) == (1, 1, 0)
+
+
+def test_workspace_bytes(lib):
+    hy = binding.default_hyper()
+    small = lib.xrdvi_workspace_bytes(1001, 6, 120, 16, C.byref(hy))
+    big = lib.xrdvi_workspace_bytes(4001, 50, 4500, 256, C.byref(hy))
+    assert 0 < small < big < 1 << 30
+    assert lib.xrdvi_workspace_bytes(1, 6, 120, 16, C.byref(hy)) == 0
+    hy.size = 3
+    assert lib.xrdvi_workspace_bytes(1001, 6, 120, 16, C.byref(hy)) == 0
+
+
+def test_create_rejects_bad_arguments_before_touching_cuda(lib):
+    hy = binding.default_hyper()
+    x = np.linspace(10, 80, 101)
+    y = np.ones(101)
+    ofs = np.array([0, 2, 4], dtype=np.int64)
+    pos = np.array([20.0, 30.0, 40.0, 50.0])
+    inten = np.array([1.0, 2.0, 3.0, 4.0])
+    out = C.c_void_p()
+    dp = lambda a: a.ctypes.data_as(C.POINTER(C.c_double))  # noqa: E731
+    ip = lambda a: a.ctypes.data_as(C.POINTER(C.c_int64))   # noqa: E731
+
+    def create(x=x, ofs=ofs, inten=inten, hy=hy):
+        return lib.xrdvi_create(dp(x), len(x), dp(y), None, 2, ip(ofs), dp(pos), dp(inten), C.byref(hy), 16, 0,
+                                None, C.c_void_p(256), 1 << 20, C.byref(out))
+
+    xs = x.copy(); xs[5] = xs[4]
+    assert create(x=xs) == -2 and b"increasing" in lib.xrdvi_last_error()
+    xn = x.copy(); xn[7] += 0.01
+    assert create(x=xn) == -3
+    assert create(ofs=np.array([0, 0, 4], dtype=np.int64)) == -4
+    assert create(inten=np.array([1.0, -2.0, 3.0, 4.0])) == -1
+    hb = binding.default_hyper(likelihood=1)
+    assert create(hy=hb) == -1
+    assert out.value is None
+
+
+def test_no_cpu_fallback_without_device():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    with pytest.raises(binding.XrdviError):
+        binding.Xrdvi(np.linspace(0, 1, 11), np.ones(11), None, [0, 1], [0.5], [1.0], S_max=4)

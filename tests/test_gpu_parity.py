@@ -1,0 +1,201 @@
+"""Parity of the CUDA path (through the C ABI) against the fp64 oracle on the same seeded inputs
+and the same Philox draws.  Tolerances are north_star's: profile / ll / ELBO relative 1e-4,
+gradients relative 1e-3 (class-normalised, SURVEY.md 8(c) "Parity metrics"), inclusion 0.02 absolute."""
+import math
+
+import numpy as np
+import pytest
+
+from oracle import xrdvi_oracle as orc
+from paper_2501_09308_b200 import Xrdvi, synth
+
+pytestmark = pytest.mark.gpu
+
+TOL_PROFILE = 1e-4
+TOL_ELBO = 1e-4
+TOL_GRAD = 1e-3
+TOL_INCL = 0.02
+
+
+def class_errors(g_gpu, g_ref):
+    """max_k |g_gpu - g_ref| / max_k |g_ref| per (pattern, restart, m|l, class)."""
+    err = np.abs(g_gpu.astype(np.float64) - g_ref).max(axis=3)
+    ref = np.abs(g_ref).max(axis=3)
+    return err / ref
+
+
+def check_eval(gpu, o, state, S, seed, iteration, n_prof=4):
+    elbo_r, grad_r, ll_r, f_r = o.elbo_grad(state.astype(np.float64), S, seed, iteration, want_ll=True,
+                                            n_profiles=n_prof)
+    f_g, ll_g = gpu.debug_profile(n_prof, state=state, S=S, seed=seed, iteration=iteration)
+    for t in range(n_prof):
+        assert np.abs(f_g[t] - f_r[t]).max() / np.abs(f_r[t]).max() <= TOL_PROFILE
+    ll_flat = ll_r.reshape(-1)
+    np.testing.assert_allclose(ll_g, ll_flat[:n_prof], rtol=TOL_ELBO)
+    elbo_g, grad_g = gpu.elbo_grad(state=state, S=S, seed=seed, iteration=iteration)
+    np.testing.assert_allclose(elbo_g, elbo_r, rtol=TOL_ELBO)
+    ce = class_errors(grad_g, grad_r)
+    assert ce.max() <= TOL_GRAD, ce
+    return ce.max()
+
+
+# --------------------------------------------------------------------------- a-1 draws
+def test_philox_words_bit_exact_and_normals():
+    wl = synth.make_workload(0, n_restarts=2)
+    gpu = Xrdvi.from_workload(wl, S_max=40)
+    seed, it, S = (7 << 32) | 12345, 77, 40
+    eps, raw = gpu.debug_draws(2 * S, S=S, seed=seed, iteration=it)
+    for t in (0, 1, 17, 39, 40, 79):
+        inst, s = divmod(t, S)
+        for k in range(wl.K):
+            ref = orc.philox4x32_10([it, s, k, inst], [seed & 0xFFFFFFFF, seed >> 32])
+            assert [int(v) for v in raw[t, k]] == ref                      # bit-exact integer work
+            np.testing.assert_allclose(eps[t, k], orc.eps(seed, it, inst, s, k), rtol=0, atol=4e-6)
+    # published known-answer vector through the device generator: counter (it=0,s=0,k=0,inst=0), key 0
+    eps0, raw0 = gpu.debug_draws(1, S=S, seed=0, iteration=0)
+    assert [int(v) for v in raw0[0, 0]] == [0x6627E8D5, 0xE169C58D, 0xBC57AC4C, 0x9B00DBD8]
+
+
+# --------------------------------------------------------------------------- configs
+def test_config0_all_states():
+    wl = synth.make_workload(0)
+    o = orc.from_workload(wl)
+    gpu = Xrdvi.from_workload(wl)
+    assert gpu.pair_count == o.pair_count() and gpu.n_c == o.n_c
+    st0, step = gpu.get_state()
+    assert step == 0
+    np.testing.assert_allclose(st0, o.init_state(), rtol=1e-6)
+    check_eval(gpu, o, st0, wl.S, seed=3, iteration=1, n_prof=16)
+    gpu.fit(50, seed=3)
+    st50, step = gpu.get_state()
+    assert step == 50
+    check_eval(gpu, o, st50, wl.S, seed=3, iteration=51, n_prof=16)
+    gpu.fit(450, seed=3)
+    st500, _ = gpu.get_state()
+    check_eval(gpu, o, st500, wl.S, seed=3, iteration=501, n_prof=16)
+
+
+def test_config0_fit_inclusion_parity():
+    wl = synth.make_workload(0)
+    o = orc.from_workload(wl)
+    gpu = Xrdvi.from_workload(wl)
+    st_g, inc_g, tr_g = gpu.fit(500, seed=11, want_trace=True)
+    st_r, _, tr_r = o.fit(o.init_state(), 500, wl.S, seed=11, want_trace=True)
+    inc_r = o.inclusion(st_r)
+    assert np.abs(inc_g - inc_r).max() <= TOL_INCL
+    # the first steps follow the oracle closely (before fp32/fp64 trajectories drift apart)
+    np.testing.assert_allclose(tr_g[:3], tr_r[:3], rtol=TOL_ELBO)
+    # identified parameters of the planted phases agree
+    for k in wl.true_phases[0]:
+        np.testing.assert_allclose(st_g[0, 0, 0, k, :3], st_r[0, 0, 0, k, :3], atol=0.02)
+    inc2, area = gpu.inclusion()
+    np.testing.assert_array_equal(inc2, inc_g)
+    assert area.sum() == pytest.approx(1.0, rel=1e-9)
+
+
+def test_single_adam_step_matches_oracle():
+    wl = synth.make_workload(0)
+    o = orc.from_workload(wl)
+    gpu = Xrdvi.from_workload(wl)
+    st_g, _, _ = gpu.fit(1, seed=5)
+    st_r, _, _ = o.fit(o.init_state(), 1, wl.S, seed=5)
+    np.testing.assert_allclose(st_g, st_r, atol=2e-5)
+    st_g2, _, _ = gpu.fit(2, seed=5)                              # steps 2 and 3 continue the counter
+    st_r3, _, _ = o.fit(o.init_state(), 3, wl.S, seed=5)
+    np.testing.assert_allclose(st_g2, st_r3, atol=2e-3)
+
+
+def test_config1_reduced_draws():
+    wl = synth.make_workload(1, S=64)
+    o = orc.from_workload(wl)
+    gpu = Xrdvi.from_workload(wl)
+    assert gpu.pair_count == o.pair_count()
+    st0, _ = gpu.get_state()
+    check_eval(gpu, o, st0, 64, seed=1, iteration=1)
+    gpu.fit(50, seed=1)
+    st50, _ = gpu.get_state()
+    check_eval(gpu, o, st50, 64, seed=1, iteration=51)
+    gpu.fit(250, seed=1)
+    st300, _ = gpu.get_state()
+    check_eval(gpu, o, st300, 64, seed=1, iteration=301)
+
+
+def test_config2_restarts_batched():
+    wl = synth.make_workload(2, n_restarts=3, S=32)
+    o = orc.from_workload(wl)
+    gpu = Xrdvi.from_workload(wl)
+    gpu.reset_state(seed=9)
+    st0, _ = gpu.get_state()
+    np.testing.assert_allclose(st0, o.init_state(seed=9), rtol=2e-6, atol=2e-7)
+    assert np.abs(st0[0, 1, 0] - st0[0, 0, 0]).min() > 0          # restarts are jittered
+    check_eval(gpu, o, st0, 32, seed=2, iteration=4, n_prof=2)
+
+
+def test_config3_patterns_batched():
+    wl = synth.make_workload(3, n_patterns=3, S=32)
+    o = orc.from_workload(wl)
+    gpu = Xrdvi.from_workload(wl)
+    st = synth.random_state(wl.K, 3, 1, seed=4)
+    st[:, :, 0, :, 0] += np.log(1.0 / np.array([o.lambda_h(p) for p in range(3)]))[:, None, None] - 2.0
+    elbo_r, grad_r, ll_r = o.elbo_grad(st.astype(np.float64), 32, 8, 3, want_ll=True)
+    elbo_g, grad_g = gpu.elbo_grad(state=st, S=32, seed=8, iteration=3)
+    np.testing.assert_allclose(elbo_g, elbo_r, rtol=TOL_ELBO)
+    assert class_errors(grad_g, grad_r).max() <= TOL_GRAD
+    f_g, ll_g = gpu.debug_profile(96, state=st, S=32, seed=8, iteration=3, want_f=False)
+    np.testing.assert_allclose(ll_g, ll_r.reshape(-1), rtol=TOL_ELBO)
+
+
+def test_config4_reduced_library():
+    wl = synth.make_workload(4, K=60, S=8)
+    o = orc.from_workload(wl)
+    gpu = Xrdvi.from_workload(wl)
+    assert gpu.n_c == 400 and gpu.pair_count == o.pair_count()
+    st0, _ = gpu.get_state()
+    check_eval(gpu, o, st0, 8, seed=6, iteration=2, n_prof=2)
+    st = synth.random_state(wl.K, 1, 1, seed=12)
+    st[:, :, 0, :, 0] += math.log(1.0 / o.lambda_h()) - 3.0
+    st[:, :, 0, :, 2] = np.log(np.random.default_rng(0).uniform(0.03, 0.3, wl.K))
+    check_eval(gpu, o, st, 8, seed=6, iteration=2, n_prof=2)
+
+
+# --------------------------------------------------------------------------- edge cases
+def test_dense_mode_ragged_sizes_and_out_of_range_peaks():
+    rng = np.random.default_rng(5)
+    N = 203                                                        # not a multiple of 4 or 8
+    x = 20.0 + 0.02 * np.arange(N)
+    ofs = np.array([0, 3, 4, 9], dtype=np.int64)
+    pos = np.array([19.0, 21.0, 23.9, 22.5, 10.0, 20.01, 24.05, 24.06, 30.0])   # some outside the grid
+    inten = rng.uniform(1, 100, 9)
+    y = rng.uniform(0, 30, N)
+    for W in (0.0, 3.0):
+        hp = dict(window_W=W, fwhm_ref=0.1, noise_sigma=1.5, lambda_h=0.5, w_rate=30.0)
+        o = orc.Oracle(x, y, None, ofs, pos, inten, **hp)
+        gpu = Xrdvi(x, y, None, ofs, pos, inten, S_max=5, **hp)
+        assert gpu.pair_count == o.pair_count()
+        st = synth.random_state(3, 1, 1, seed=1)
+        st[:, :, 0, :, 0] += 2.0
+        check_eval(gpu, o, st, 5, seed=1, iteration=0, n_prof=5)
+        gpu.close()
+
+
+def test_results_are_bitwise_reproducible():
+    wl = synth.make_workload(1, S=64)
+    outs = []
+    for _ in range(2):
+        gpu = Xrdvi.from_workload(wl)
+        st, inc, tr = gpu.fit(20, seed=3, want_trace=True)
+        e, g = gpu.elbo_grad(S=64, seed=3, iteration=99)
+        outs.append((st, inc, tr, e, g))
+        gpu.close()
+    for a, b in zip(outs[0], outs[1]):
+        np.testing.assert_array_equal(a, b)
+
+
+def test_error_paths_on_device():
+    wl = synth.make_workload(0)
+    gpu = Xrdvi.from_workload(wl)
+    from paper_2501_09308_b200 import XrdviError
+    with pytest.raises(XrdviError):
+        gpu.elbo_grad(S=wl.S + 64)
+    with pytest.raises(XrdviError):
+        gpu.fit(-1)
