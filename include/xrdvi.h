@@ -154,6 +154,13 @@ int xrdvi_time_kernels(xrdvi* h, int32_t S, uint64_t seed, int32_t reps, float* 
 int xrdvi_bench_steps(xrdvi* h, int32_t steps, int32_t S, uint64_t seed, size_t l2_flush_bytes,
                       float* ms_steps);
 
+/* Measurement: per-SM, per-clock rates of the pipes that bound the path (microbenchmark, DESIGN.md
+ * "Roofline").  rates float [9]: lane-operations per SM clock of [0] FFMA, [1] FFMA2 (2 FMAs per lane),
+ * [2] MUFU.EX2, [3] MUFU.RCP, [4] the plain forward instruction mix (5 FP32 : 2 MUFU), [5] the plain
+ * backward mix (14 FP32 : 2 MUFU), [6] 7 FFMA2 : 2 MUFU, [7] EX2 and RCP chains run together (MUFU
+ * operations per clock); [8] = SM clock (MHz) during the run.                                       */
+int xrdvi_pipe_rates(int device, float* rates);
+
 const char* xrdvi_last_error(void);
 
 #ifdef __cplusplus

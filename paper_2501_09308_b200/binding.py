@@ -18,7 +18,7 @@ EXPORTS = (
     "xrdvi_default_hyper", "xrdvi_workspace_bytes", "xrdvi_create", "xrdvi_destroy", "xrdvi_pair_count",
     "xrdvi_window_halfwidth", "xrdvi_reset_state", "xrdvi_get_state", "xrdvi_set_state", "xrdvi_elbo_grad",
     "xrdvi_fit", "xrdvi_inclusion", "xrdvi_debug_profile", "xrdvi_debug_draws", "xrdvi_time_kernels",
-    "xrdvi_bench_steps", "xrdvi_last_error",
+    "xrdvi_bench_steps", "xrdvi_pipe_rates", "xrdvi_last_error",
 )
 
 
@@ -75,6 +75,7 @@ def load_library():
     L.xrdvi_debug_draws.argtypes = [vp, C.c_int32, C.c_uint64, C.c_uint64, C.c_int64, fp, C.POINTER(C.c_uint32)]
     L.xrdvi_time_kernels.argtypes = [vp, C.c_int32, C.c_uint64, C.c_int32, fp, fp, fp]
     L.xrdvi_bench_steps.argtypes = [vp, C.c_int32, C.c_int32, C.c_uint64, C.c_size_t, fp]
+    L.xrdvi_pipe_rates.argtypes = [C.c_int, fp]
     L.xrdvi_last_error.restype = C.c_char_p
     _lib = L
     return L
@@ -101,6 +102,14 @@ def _f(a):
 
 def _d(a):
     return a.ctypes.data_as(C.POINTER(C.c_double)) if a is not None else None
+
+
+def pipe_rates(device=0) -> dict:
+    """Measured per-SM per-clock pipe rates (xrdvi_pipe_rates)."""
+    r = np.zeros(9, dtype=np.float32)
+    _check(load_library().xrdvi_pipe_rates(int(device), _f(r)))
+    names = ("ffma", "ffma2", "mufu_ex2", "mufu_rcp", "mix_forward", "mix_backward", "mix_ffma2", "mufu_ex2_rcp", "sm_mhz")
+    return {k: float(v) for k, v in zip(names, r)}
 
 
 class Xrdvi:

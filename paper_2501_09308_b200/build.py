@@ -11,7 +11,7 @@ import subprocess
 PKG = pathlib.Path(__file__).resolve().parent
 CSRC = PKG / "csrc"
 LIB = PKG / "libxrdvi.so"
-SOURCES = [CSRC / "xrdvi.cu"]
+SOURCES = [CSRC / "xrdvi.cu", CSRC / "pipe_rates.cu"]
 DEPS = SOURCES + [CSRC / "xrdvi_kernels.cuh", PKG.parent / "include" / "xrdvi.h"]
 
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",

@@ -257,8 +257,14 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
     const int P = pl.P;
     long long n_c;
     if (hyp->window_W > 0.0) n_c = static_cast<long long>(std::ceil(hyp->window_W * hyp->fwhm_ref / delta - 1e-9));
-    else n_c = N;  // dense: every point is inside every window
-    if (n_c > N) n_c = N;
+    else {         // dense: every point is inside every window, wherever the peak lies
+        n_c = N;
+        for (int64_t m = 0; m < M; ++m) {
+            const long long j = static_cast<long long>(std::floor((pos[m] - x[0]) / delta + 0.5));
+            n_c = std::max<long long>(n_c, std::max<long long>(std::llabs(j), std::llabs(N - 1 - j)) + 1);
+        }
+    }
+    if (n_c > (1ll << 30)) return fail(XRDVI_E_INVALID_ARG, "peak positions too far from the grid");
     struct HP { long long j; double d; double I; int k; };
     std::vector<HP> kept;
     kept.reserve(M);
