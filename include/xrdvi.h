@@ -77,8 +77,11 @@ typedef struct {
 void xrdvi_default_hyper(xrdvi_hyper* hyp);
 
 /* Bytes of device workspace xrdvi_create needs for draws up to S_max per (pattern, restart).
- * Depends only on the sizes (an upper bound over peak positions).  0 on invalid arguments.      */
-size_t xrdvi_workspace_bytes(int64_t N, int32_t K, int64_t M, int32_t S_max, const xrdvi_hyper* hyp);
+ * two_theta_step = (two_theta[N-1] - two_theta[0]) / (N-1), the grid step in degrees (it fixes the window
+ * half-width n_c, R16).  Depends only on the sizes (an upper bound over peak positions).  0 on invalid
+ * arguments.                                                                                       */
+size_t xrdvi_workspace_bytes(int64_t N, int32_t K, int64_t M, int32_t S_max, double two_theta_step,
+                             const xrdvi_hyper* hyp);
 
 /* Build a problem.
  *  two_theta [N]     strictly increasing, uniform grid (deg)
@@ -121,8 +124,9 @@ int xrdvi_elbo_grad(xrdvi* h, const float* var_params, int32_t S, uint64_t seed,
                     double* elbo, float* grad);
 
 /* `iterations` Adam-ascent steps from the internal state, each one a replay of a CUDA
- * Graph (draw -> forward -> backward -> chain/reduce -> update); step t uses Philox iteration t, t
- * continuing from the state's step counter + 1.  Outputs (each may be NULL, nothing is copied then):
+ * Graph; step t uses Philox iteration t, t
+ * continuing from the state's step counter + 1 (the graph holds two kernels: the fused profile/residual/
+ * backward kernel and the reduce + Adam + next-draw kernel).  Outputs (each may be NULL, nothing is copied then):
  *  var_params_out float [P][R][2][K][4]; incl_prob double [P][R][K] (R15);
  *  elbo_trace double [iterations][P][R] (only the last 4096 iterations are kept; older rows = NaN)  */
 int xrdvi_fit(xrdvi* h, int32_t iterations, int32_t S, uint64_t seed, float* var_params_out,
@@ -138,14 +142,18 @@ int xrdvi_inclusion(xrdvi* h, double* incl_prob, double* area_ratio);
 int xrdvi_debug_profile(xrdvi* h, const float* var_params, int32_t S, uint64_t seed,
                         uint64_t iteration, int64_t n, float* f, double* ll);
 
-/* Debug read-back of the draw kernel: eps float [n][K][4] for the first n sample-instances.        */
+/* Debug read-back of the draw kernel (a-1, a-2) at the internal state: eps float [n][K][4] for the first n
+ * sample-instances; raw_words uint32 [n][K][4] (the Philox output) or NULL; core_halfwidth int32 [n][K]
+ * or NULL: the Gaussian-core half-width n_g in grid points of the 32-draw group the instance belongs to
+ * (outside |i - j_m| <= n_g the kernels evaluate only the Lorentzian).          */
 int xrdvi_debug_draws(xrdvi* h, int32_t S, uint64_t seed, uint64_t iteration, int64_t n, float* eps,
-                      uint32_t* raw_words /* [n][K][4] or NULL */);
+                      uint32_t* raw_words, int32_t* core_halfwidth);
 
-/* Mean CUDA-event time (ms) of the kernels of the last xrdvi_fit call: total per iteration and the
- * share measured separately for the forward and backward kernels by xrdvi_time_kernels.            */
-int xrdvi_time_kernels(xrdvi* h, int32_t S, uint64_t seed, int32_t reps, float* ms_forward,
-                       float* ms_backward, float* ms_iteration);
+/* Measurement: mean CUDA-event times (ms) over `reps` repetitions (after one warm-up) of the kernels of one
+ * evaluation at the internal state, launched one by one on the handle's stream: ms float [4] =
+ * [0] elbo_tile_kernel (fused profile + residual + backward), [1] its forward-only instantiation (profile +
+ * residual), [2] update_draw_kernel without the update, [3] draw + tile + update together.          */
+int xrdvi_time_kernels(xrdvi* h, int32_t S, uint64_t seed, int32_t reps, float* ms);
 
 /* Measurement: `steps` optimisation steps (graph replays, exactly as xrdvi_fit runs them), each one
  * bracketed by its own pair of CUDA events on the handle's stream; between two steps, outside the

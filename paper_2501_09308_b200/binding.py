@@ -55,7 +55,7 @@ def load_library():
     vp, fp, dp = C.c_void_p, C.POINTER(C.c_float), C.POINTER(C.c_double)
     L.xrdvi_default_hyper.argtypes = [C.POINTER(Hyper)]
     L.xrdvi_default_hyper.restype = None
-    L.xrdvi_workspace_bytes.argtypes = [C.c_int64, C.c_int32, C.c_int64, C.c_int32, C.POINTER(Hyper)]
+    L.xrdvi_workspace_bytes.argtypes = [C.c_int64, C.c_int32, C.c_int64, C.c_int32, C.c_double, C.POINTER(Hyper)]
     L.xrdvi_workspace_bytes.restype = C.c_size_t
     L.xrdvi_create.argtypes = [dp, C.c_int64, dp, dp, C.c_int32, C.POINTER(C.c_int64), dp, dp, C.POINTER(Hyper),
                                C.c_int32, C.c_int, vp, vp, C.c_size_t, C.POINTER(vp)]
@@ -72,8 +72,9 @@ def load_library():
     L.xrdvi_fit.argtypes = [vp, C.c_int32, C.c_int32, C.c_uint64, fp, dp, dp]
     L.xrdvi_inclusion.argtypes = [vp, dp, dp]
     L.xrdvi_debug_profile.argtypes = [vp, fp, C.c_int32, C.c_uint64, C.c_uint64, C.c_int64, fp, dp]
-    L.xrdvi_debug_draws.argtypes = [vp, C.c_int32, C.c_uint64, C.c_uint64, C.c_int64, fp, C.POINTER(C.c_uint32)]
-    L.xrdvi_time_kernels.argtypes = [vp, C.c_int32, C.c_uint64, C.c_int32, fp, fp, fp]
+    L.xrdvi_debug_draws.argtypes = [vp, C.c_int32, C.c_uint64, C.c_uint64, C.c_int64, fp, C.POINTER(C.c_uint32),
+                                    C.POINTER(C.c_int32)]
+    L.xrdvi_time_kernels.argtypes = [vp, C.c_int32, C.c_uint64, C.c_int32, fp]
     L.xrdvi_bench_steps.argtypes = [vp, C.c_int32, C.c_int32, C.c_uint64, C.c_size_t, fp]
     L.xrdvi_pipe_rates.argtypes = [C.c_int, fp]
     L.xrdvi_last_error.restype = C.c_char_p
@@ -132,7 +133,8 @@ class Xrdvi:
         pos = np.ascontiguousarray(peak_pos, dtype=np.float64)
         inten = np.ascontiguousarray(peak_int, dtype=np.float64)
         self.K, self.M, self.S_max = int(ofs.shape[0] - 1), int(pos.shape[0]), int(S_max)
-        nbytes = int(L.xrdvi_workspace_bytes(self.N, self.K, self.M, self.S_max, C.byref(self.hyper)))
+        step = float((x[-1] - x[0]) / (self.N - 1)) if self.N > 1 else 0.0
+        nbytes = int(L.xrdvi_workspace_bytes(self.N, self.K, self.M, self.S_max, step, C.byref(self.hyper)))
         if nbytes == 0:
             raise XrdviError(-1, "xrdvi_workspace_bytes: invalid sizes")
         self.device = torch.device("cuda", device)
@@ -222,19 +224,22 @@ class Xrdvi:
         _check(load_library().xrdvi_debug_profile(self._h, _f(st), S, int(seed), int(iteration), int(n), _f(f), _d(ll)))
         return f, ll
 
-    def debug_draws(self, n, S=None, seed=0, iteration=0):
+    def debug_draws(self, n, S=None, seed=0, iteration=0, want_core=False):
         S = self.S_max if S is None else int(S)
         eps = np.empty((int(n), self.K, 4), dtype=np.float32)
         raw = np.empty((int(n), self.K, 4), dtype=np.uint32)
-        _check(load_library().xrdvi_debug_draws(self._h, S, int(seed), int(iteration), int(n), _f(eps),
-                                                raw.ctypes.data_as(C.POINTER(C.c_uint32))))
-        return eps, raw
+        core = np.empty((int(n), self.K), dtype=np.int32) if want_core else None
+        _check(load_library().xrdvi_debug_draws(
+            self._h, S, int(seed), int(iteration), int(n), _f(eps), raw.ctypes.data_as(C.POINTER(C.c_uint32)),
+            core.ctypes.data_as(C.POINTER(C.c_int32)) if want_core else None))
+        return (eps, raw, core) if want_core else (eps, raw)
 
     def time_kernels(self, S=None, seed=0, reps=20):
         S = self.S_max if S is None else int(S)
-        a, b, c = C.c_float(), C.c_float(), C.c_float()
-        _check(load_library().xrdvi_time_kernels(self._h, S, int(seed), int(reps), C.byref(a), C.byref(b), C.byref(c)))
-        return dict(ms_forward=a.value, ms_backward=b.value, ms_iteration=c.value)
+        ms = np.zeros(4, dtype=np.float32)
+        _check(load_library().xrdvi_time_kernels(self._h, S, int(seed), int(reps), _f(ms)))
+        return dict(ms_tile=float(ms[0]), ms_tile_forward_only=float(ms[1]), ms_update=float(ms[2]),
+                    ms_iteration=float(ms[3]))
 
     def bench_steps(self, steps, S=None, seed=0, l2_flush_bytes=0):
         S = self.S_max if S is None else int(S)

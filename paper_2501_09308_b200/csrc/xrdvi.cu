@@ -7,8 +7,10 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <limits>
+#include <numeric>
 #include <string>
 #include <vector>
 
@@ -33,18 +35,37 @@ int fail(int code, const std::string& msg) {
 size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
 
 struct Plan {   // workspace carve; identical arithmetic in workspace_bytes and create
-    int P, R, PR, S_pad, gpi_max, G_max, NQ, ntile, K;
-    int unit_peaks;    // target peaks per backward unit
-    int units_cap;     // upper bound on the number of units
-    long long M;
+    int P, R, PR, S_pad, gpi_max, G_max, K;
+    int W, SP, n_seg, n_tile;
+    long long M, n_c, bwd_cap, slots_cap;
     size_t total;
-    size_t o_yb, o_bg, o_pkf, o_tile, o_pkb, o_units, o_uofs, o_pat, o_area, o_mh0;
-    size_t o_var, o_vartmp, o_mom1, o_mom2, o_grad, o_elbo, o_elbok, o_llt, o_trace, o_ctl;
-    size_t o_lat, o_eps, o_e, o_llpart, o_sums, o_dbg;
+    size_t o_yb, o_bg, o_pkf, o_tile, o_pkb, o_wrng, o_sord, o_sofs, o_sids, o_pat, o_area, o_mh0;
+    size_t o_var, o_vartmp, o_mom1, o_mom2, o_grad, o_elbo, o_elbok, o_llt, o_trace, o_done, o_ctl;
+    size_t o_lat, o_eps, o_rr, o_ng, o_llpart, o_part8, o_dbg;
 };
 
-bool make_plan(int64_t N, int32_t K, int64_t M, int32_t S_max, const xrdvi_hyper* hyp, Plan* pl) {
-    if (N < 2 || K < 1 || M < 1 || S_max < 1 || !hyp) return false;
+// window half-width in grid points (R16); dense (W <= 0) is represented by n_c = -1 here
+long long window_points(const xrdvi_hyper* hyp, double step) {
+    if (!(hyp->window_W > 0.0)) return -1;
+    return static_cast<long long>(std::ceil(hyp->window_W * hyp->fwhm_ref / step - 1e-9));
+}
+
+// warps per CTA of elbo_tile_kernel (segment = 16 W points): as large as still gives >= 8 CTAs per SM
+int choose_seg_warps(int64_t N, int G_max) {
+    if (const char* e = std::getenv("XRDVI_SEG_WARPS")) {   // tuning knob for sweeps
+        const int w = std::atoi(e);
+        if (w == 1 || w == 2 || w == 4 || w == 8) return w;
+    }
+    const long long target = 148ll * 8;
+    for (int w : {4, 2}) {
+        const long long n_seg = (N + 16 * w - 1) / (16 * w);
+        if (n_seg * G_max >= target) return w;
+    }
+    return 2;
+}
+
+bool make_plan(int64_t N, int32_t K, int64_t M, int32_t S_max, double step, const xrdvi_hyper* hyp, Plan* pl) {
+    if (N < 2 || K < 1 || M < 1 || S_max < 1 || !hyp || !(step > 0.0)) return false;
     if (N > (1 << 28) || M > (1ll << 30) || K > (1 << 24)) return false;
     Plan p{};
     p.P = std::max(1, hyp->n_patterns);
@@ -56,22 +77,29 @@ bool make_plan(int64_t N, int32_t K, int64_t M, int32_t S_max, const xrdvi_hyper
     p.gpi_max = p.S_pad / 32;
     p.G_max = p.PR * p.gpi_max;
     if (p.G_max > 65535 || p.PR > 65535) return false;  // grid.y limit
-    p.NQ = static_cast<int>((N + 3) / 4);
-    p.ntile = static_cast<int>((N + kFwdP - 1) / kFwdP);
-    // backward units: enough warps to fill 148 SMs x 16 warps, at least one unit per phase
-    const long long want = std::max<long long>(K, (148ll * 16 + p.G_max - 1) / p.G_max);
-    p.unit_peaks = static_cast<int>(std::max<long long>(4, (M + want - 1) / want));
-    p.units_cap = static_cast<int>(M / p.unit_peaks + K + 1);
+    p.W = choose_seg_warps(N, p.G_max);
+    p.SP = kPT * p.W;
+    p.n_seg = static_cast<int>((N + p.SP - 1) / p.SP);
+    p.n_tile = static_cast<int>((N + kPT - 1) / kPT);
+    p.n_c = window_points(hyp, step);
+    // entries of the per-segment phase-major lists: a peak appears once per segment its window touches
+    const long long per_peak = p.n_c < 0 ? p.n_seg : std::min<long long>(p.n_seg, (2 * p.n_c + p.SP) / p.SP + 1);
+    p.bwd_cap = M * per_peak;
+    p.slots_cap = std::min<long long>(static_cast<long long>(p.n_seg) * (K + p.W), p.bwd_cap + static_cast<long long>(p.n_seg) * p.W);
+    if (p.bwd_cap > (1ll << 31) - 1 || p.slots_cap > (1ll << 31) - 1) return false;
     size_t o = 0;
     auto take = [&](size_t bytes) { size_t r = o; o = align_up(o + bytes); return r; };
     const size_t var_b = sizeof(float) * p.PR * 8 * static_cast<size_t>(K);
+    const size_t gk32 = static_cast<size_t>(p.G_max) * K * 32;
     p.o_yb = take(sizeof(float) * p.P * N);
     p.o_bg = take(sizeof(float) * p.P * N);
     p.o_pkf = take(sizeof(PeakRec) * M);
-    p.o_tile = take(sizeof(int2) * p.ntile);
-    p.o_pkb = take(sizeof(PeakRec) * M);
-    p.o_units = take(sizeof(int4) * p.units_cap);
-    p.o_uofs = take(sizeof(int) * (K + 1));
+    p.o_tile = take(sizeof(int2) * p.n_tile);
+    p.o_pkb = take(sizeof(PeakRec) * std::max<long long>(p.bwd_cap, 1));
+    p.o_wrng = take(sizeof(int4) * static_cast<size_t>(p.n_seg) * p.W);
+    p.o_sord = take(sizeof(int) * p.n_seg);
+    p.o_sofs = take(sizeof(int) * (K + 1));
+    p.o_sids = take(sizeof(int) * std::max<long long>(p.slots_cap, 1));
     p.o_pat = take(sizeof(PatConst) * p.P);
     p.o_area = take(sizeof(double) * K);
     p.o_mh0 = take(sizeof(float) * p.P);
@@ -81,15 +109,17 @@ bool make_plan(int64_t N, int32_t K, int64_t M, int32_t S_max, const xrdvi_hyper
     p.o_mom2 = take(var_b);
     p.o_grad = take(var_b);
     p.o_elbo = take(sizeof(double) * p.PR);
-    p.o_elbok = take(sizeof(double) * p.PR * K);
+    p.o_elbok = take(sizeof(double) * p.PR * (K + 1));
     p.o_llt = take(sizeof(double) * p.PR * p.S_pad);
     p.o_trace = take(sizeof(double) * kTraceCap * p.PR);
+    p.o_done = take(sizeof(unsigned int) * p.PR);
     p.o_ctl = take(sizeof(Ctl));
-    p.o_lat = take(sizeof(float4) * static_cast<size_t>(p.G_max) * K * 32);
-    p.o_eps = take(sizeof(float4) * static_cast<size_t>(p.G_max) * K * 32);
-    p.o_e = take(sizeof(float4) * static_cast<size_t>(p.G_max) * p.NQ * 32);
-    p.o_llpart = take(sizeof(float) * static_cast<size_t>(p.G_max) * p.ntile * 32);
-    p.o_sums = take(sizeof(float) * static_cast<size_t>(p.G_max) * p.units_cap * 6 * 32);
+    p.o_lat = take(sizeof(float4) * gk32);
+    p.o_eps = take(sizeof(float4) * gk32);
+    p.o_rr = take(sizeof(float) * gk32);
+    p.o_ng = take(sizeof(int) * static_cast<size_t>(p.G_max) * K);
+    p.o_llpart = take(sizeof(float) * static_cast<size_t>(p.G_max) * p.n_seg * 32);
+    p.o_part8 = take(sizeof(float) * static_cast<size_t>(p.G_max) * std::max<long long>(p.slots_cap, 1) * 8);
     p.o_dbg = take(sizeof(double) * (2 * static_cast<size_t>(p.PR) * K + 64));
     p.total = o;
     *pl = p;
@@ -125,29 +155,50 @@ void set_S(xrdvi* h, int S) {
     h->dev.G = h->plan.PR * h->dev.gpi;
 }
 
-// enqueue the kernels of one evaluation (and optionally the Adam update) on the stream
-int enqueue_iteration(xrdvi* h, const float* var, int do_update, float* f_dbg, long long n_dbg,
-                      uint4* raw_out, bool forward_only) {
-    const Dev& d = h->dev;
-    cudaStream_t st = h->stream;
-    draw_transform_kernel<<<dim3((d.K + 3) / 4, d.G), 128, 0, st>>>(d, var, raw_out);
-    forward_kernel<<<dim3((d.ntile + kFwdWarps - 1) / kFwdWarps, d.G), 32 * kFwdWarps, 0, st>>>(d, f_dbg, n_dbg);
-    if (!forward_only) {
-        backward_kernel<<<dim3((d.n_units + kBwdWarps - 1) / kBwdWarps, d.G), 32 * kBwdWarps, 0, st>>>(d);
-        chain_reduce_kernel<<<dim3(d.K, d.PR), kChainThreads, 0, st>>>(d, var);
+template <bool BWD>
+void launch_tile(const Dev& d, cudaStream_t st, float* f_dbg, long long n_dbg) {
+    const dim3 grid(d.n_seg, d.G);
+    switch (d.W) {
+        case 1: elbo_tile_kernel<1, BWD><<<grid, 32, 0, st>>>(d, f_dbg, n_dbg); break;
+        case 2: elbo_tile_kernel<2, BWD><<<grid, 64, 0, st>>>(d, f_dbg, n_dbg); break;
+        case 4: elbo_tile_kernel<4, BWD><<<grid, 128, 0, st>>>(d, f_dbg, n_dbg); break;
+        default: elbo_tile_kernel<8, BWD><<<grid, 256, 0, st>>>(d, f_dbg, n_dbg); break;
     }
-    finalize_update_kernel<<<d.PR, kFinThreads, 0, st>>>(d, var, do_update);
-    if (do_update) bump_step_kernel<<<1, 1, 0, st>>>(d.ctl);
+}
+
+void launch_draw(const Dev& d, cudaStream_t st, const float* var, uint4* raw_out) {
+    draw_transform_kernel<<<dim3((d.K + 3) / 4, d.G), 128, 0, st>>>(d, var, raw_out);
+}
+
+// one optimisation step as the graph replays it: fused profile/residual/backward, then reduce + Adam +
+// the draws of the next step.  The draws of the FIRST step come from launch_draw.
+int enqueue_step(xrdvi* h) {
+    const Dev& d = h->dev;
+    launch_tile<true>(d, h->stream, nullptr, 0);
+    update_draw_kernel<<<dim3(d.K + 1, d.PR), kUpdThreads, 0, h->stream>>>(d, d.var, 1);
+    CU(cudaGetLastError());
+    return XRDVI_OK;
+}
+
+// one evaluation at `var` without touching the state: draw -> tile -> reduce
+int enqueue_eval(xrdvi* h, const float* var, float* f_dbg, long long n_dbg, bool forward_only) {
+    const Dev& d = h->dev;
+    launch_draw(d, h->stream, var, nullptr);
+    if (forward_only) launch_tile<false>(d, h->stream, f_dbg, n_dbg);
+    else launch_tile<true>(d, h->stream, f_dbg, n_dbg);
+    // forward_only leaves stale partials in part8: the gradient output of this launch is not used then
+    update_draw_kernel<<<dim3(d.K + 1, d.PR), kUpdThreads, 0, h->stream>>>(d, var, 0);
     CU(cudaGetLastError());
     return XRDVI_OK;
 }
 
 int write_ctl(xrdvi* h, uint64_t seed, long long step, long long trace_base, long long it_override) {
-    Ctl c;
+    Ctl c{};
     c.seed = seed;
     c.step = step;
     c.trace_base = trace_base;
     c.iteration_override = it_override;
+    c.done_total = 0;
     CU(cudaMemcpyAsync(h->dev.ctl, &c, sizeof(Ctl), cudaMemcpyHostToDevice, h->stream));
     CU(cudaStreamSynchronize(h->stream));  // c lives on this stack frame
     return XRDVI_OK;
@@ -165,7 +216,7 @@ int ensure_graph(xrdvi* h, int S) {
     set_S(h, S);
     cudaGraph_t graph = nullptr;
     CU(cudaStreamBeginCapture(h->stream, cudaStreamCaptureModeThreadLocal));
-    int rc = enqueue_iteration(h, h->dev.var, 1, nullptr, 0, nullptr, false);
+    int rc = enqueue_step(h);
     cudaError_t e = cudaStreamEndCapture(h->stream, &graph);
     if (rc != XRDVI_OK) { if (graph) cudaGraphDestroy(graph); return rc; }
     if (e != cudaSuccess) return fail(XRDVI_E_CUDA, std::string("cudaStreamEndCapture: ") + cudaGetErrorString(e));
@@ -173,6 +224,18 @@ int ensure_graph(xrdvi* h, int S) {
     cudaGraphDestroy(graph);
     if (e != cudaSuccess) return fail(XRDVI_E_CUDA, std::string("cudaGraphInstantiate: ") + cudaGetErrorString(e));
     h->graph_S = S;
+    return XRDVI_OK;
+}
+
+// start of a run of optimisation steps: control block, then the draws of step step0 + 1
+int begin_steps(xrdvi* h, int S, uint64_t seed) {
+    int rc = ensure_graph(h, S);
+    if (rc) return rc;
+    set_S(h, S);
+    rc = write_ctl(h, seed, h->step_host, h->step_host, -1);
+    if (rc) return rc;
+    launch_draw(h->dev, h->stream, h->dev.var, nullptr);
+    CU(cudaGetLastError());
     return XRDVI_OK;
 }
 
@@ -204,10 +267,11 @@ void xrdvi_default_hyper(xrdvi_hyper* hy) {
     hy->likelihood = 0;
 }
 
-size_t xrdvi_workspace_bytes(int64_t N, int32_t K, int64_t M, int32_t S_max, const xrdvi_hyper* hyp) {
+size_t xrdvi_workspace_bytes(int64_t N, int32_t K, int64_t M, int32_t S_max, double two_theta_step,
+                             const xrdvi_hyper* hyp) {
     Plan pl;
     if (!hyp || hyp->size != sizeof(xrdvi_hyper)) return 0;
-    if (!make_plan(N, K, M, S_max, hyp, &pl)) return 0;
+    if (!make_plan(N, K, M, S_max, two_theta_step, hyp, &pl)) return 0;
     return pl.total;
 }
 
@@ -249,15 +313,14 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
     CU(cudaSetDevice(device));
 
     Plan pl;
-    if (!make_plan(N, K, M, S_max, hyp, &pl)) return fail(XRDVI_E_INVALID_ARG, "sizes out of range");
+    if (!make_plan(N, K, M, S_max, delta, hyp, &pl)) return fail(XRDVI_E_INVALID_ARG, "sizes out of range");
     if (workspace_bytes < pl.total) return fail(XRDVI_E_WORKSPACE_TOO_SMALL, "workspace too small: need " + std::to_string(pl.total));
     if (reinterpret_cast<uintptr_t>(workspace) % 256) return fail(XRDVI_E_INVALID_ARG, "workspace not 256-byte aligned");
 
     // ---- fp64 preprocessing (R16) ----------------------------------------------------------------
-    const int P = pl.P;
-    long long n_c;
-    if (hyp->window_W > 0.0) n_c = static_cast<long long>(std::ceil(hyp->window_W * hyp->fwhm_ref / delta - 1e-9));
-    else {         // dense: every point is inside every window, wherever the peak lies
+    const int P = pl.P, W = pl.W, SP = pl.SP;
+    long long n_c = pl.n_c;
+    if (n_c < 0) {     // dense: every point is inside every window, wherever the peak lies
         n_c = N;
         for (int64_t m = 0; m < M; ++m) {
             const long long j = static_cast<long long>(std::floor((pos[m] - x[0]) / delta + 0.5));
@@ -286,46 +349,81 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
     for (int k = 0; k < K; ++k)
         if (!(area[k] > 0.0)) return fail(XRDVI_E_EMPTY_PHASE, "phase " + std::to_string(k) + " has zero total intensity");
 
-    // forward table: sorted by j (stable in (j, k, original order)); tile ranges by binary search
+    // phase-1 table: sorted by j (stable in (j, k, original order)); 16-point tile ranges by binary search
     std::vector<HP> fw = kept;
     std::stable_sort(fw.begin(), fw.end(), [](const HP& a, const HP& b) { return a.j < b.j; });
-    std::vector<PeakRec> pk_fwd(std::max(Mv, 1)), pk_bwd(std::max(Mv, 1));
-    for (int m = 0; m < Mv; ++m)
-        pk_fwd[m] = {static_cast<int>(fw[m].j), static_cast<float>(fw[m].d), static_cast<float>(fw[m].I), fw[m].k};
-    std::vector<int2> tile_rng(pl.ntile);
-    for (int t = 0; t < pl.ntile; ++t) {
-        const long long i0 = static_cast<long long>(t) * kFwdP;
-        const long long jlo = i0 - n_c, jhi = i0 + kFwdP - 1 + n_c;
+    auto rec = [](const HP& p) {
+        return PeakRec{static_cast<int>(p.j), static_cast<float>(p.d), static_cast<float>(p.I), p.k};
+    };
+    std::vector<PeakRec> pk_fwd(std::max(Mv, 1));
+    for (int m = 0; m < Mv; ++m) pk_fwd[m] = rec(fw[m]);
+    auto j_range = [&](long long jlo, long long jhi) {
         auto a = std::lower_bound(fw.begin(), fw.end(), jlo, [](const HP& p, long long v) { return p.j < v; });
         auto b = std::upper_bound(fw.begin(), fw.end(), jhi, [](long long v, const HP& p) { return v < p.j; });
-        tile_rng[t] = make_int2(static_cast<int>(a - fw.begin()), static_cast<int>(b - fw.begin()));
+        return make_int2(static_cast<int>(a - fw.begin()), static_cast<int>(b - fw.begin()));
+    };
+    std::vector<int2> tile_rng(pl.n_tile);
+    for (int t = 0; t < pl.n_tile; ++t) {
+        const long long i0 = static_cast<long long>(t) * kPT;
+        tile_rng[t] = j_range(i0 - n_c, std::min<long long>(i0 + kPT - 1, N - 1) + n_c);
     }
-    // backward table: phase-major (kept is already phase-major), split into units of ~unit_peaks peaks
-    std::vector<int4> units;
-    std::vector<int> unit_ofs(K + 1, 0);
+
+    // phase-2 tables: per segment, the peaks whose window reaches it, phase-major; W contiguous warp
+    // ranges balanced by clipped pair count; one output slot per (segment, warp, phase run)
+    std::vector<PeakRec> pk_bwd;
+    pk_bwd.reserve(static_cast<size_t>(std::min<long long>(pl.bwd_cap, 1ll << 24)));
+    std::vector<int4> warp_rng(static_cast<size_t>(pl.n_seg) * W);
+    std::vector<long long> seg_work(pl.n_seg, 0);
+    std::vector<int> slot_phase;
+    long long pairs_check = 0;
     {
-        int m = 0;
-        for (int k = 0; k < K; ++k) {
-            int m_end = m;
-            while (m_end < Mv && kept[m_end].k == k) ++m_end;
-            const int cnt = m_end - m;
-            unit_ofs[k] = static_cast<int>(units.size());
-            if (cnt > 0) {
-                const int nu = (cnt + pl.unit_peaks - 1) / pl.unit_peaks;
-                for (int u = 0; u < nu; ++u) {
-                    const int a = m + static_cast<int>(static_cast<long long>(cnt) * u / nu);
-                    const int b = m + static_cast<int>(static_cast<long long>(cnt) * (u + 1) / nu);
-                    units.push_back(make_int4(k, a, b, 0));
-                }
+        std::vector<HP> sl;
+        std::vector<long long> wgt;
+        for (int s = 0; s < pl.n_seg; ++s) {
+            const long long s0 = static_cast<long long>(s) * SP, s1 = std::min<long long>(s0 + SP - 1, N - 1);
+            const int2 r = j_range(s0 - n_c, s1 + n_c);
+            sl.assign(fw.begin() + r.x, fw.begin() + r.y);
+            std::stable_sort(sl.begin(), sl.end(), [](const HP& a, const HP& b) { return a.k < b.k; });
+            wgt.resize(sl.size());
+            long long tot = 0;
+            for (size_t q = 0; q < sl.size(); ++q) {
+                const long long lo = std::max(s0, sl[q].j - n_c), hi = std::min(s1, sl[q].j + n_c);
+                wgt[q] = hi - lo + 1;   // >= 1 by construction of the range
+                tot += wgt[q];
             }
-            m = m_end;
+            seg_work[s] = tot;
+            pairs_check += tot;
+            const int base = static_cast<int>(pk_bwd.size());
+            for (const HP& p : sl) pk_bwd.push_back(rec(p));
+            size_t q = 0;
+            long long cum = 0;
+            for (int w = 0; w < W; ++w) {
+                const size_t q0 = q;
+                const long long goal = tot * (w + 1) / W;
+                if (w == W - 1) q = sl.size();
+                else while (q < sl.size() && cum + wgt[q] <= goal) { cum += wgt[q]; ++q; }
+                const int slot0 = static_cast<int>(slot_phase.size());
+                for (size_t t = q0; t < q; ++t)
+                    if (t == q0 || sl[t].k != sl[t - 1].k) slot_phase.push_back(sl[t].k);
+                warp_rng[static_cast<size_t>(s) * W + w] = make_int4(base + static_cast<int>(q0), base + static_cast<int>(q), slot0, 0);
+            }
         }
-        unit_ofs[K] = static_cast<int>(units.size());
-        for (int q = 0; q < Mv; ++q)
-            pk_bwd[q] = {static_cast<int>(kept[q].j), static_cast<float>(kept[q].d), static_cast<float>(kept[q].I), kept[q].k};
     }
-    if (static_cast<int>(units.size()) > pl.units_cap) return fail(XRDVI_E_INVALID_ARG, "internal: unit bound exceeded");
-    if (units.empty()) units.push_back(make_int4(0, 0, 0, 0));
+    if (pairs_check != pairs) return fail(XRDVI_E_INVALID_ARG, "internal: segment tables do not cover every pair once");
+    const int n_slots = static_cast<int>(slot_phase.size());
+    if (static_cast<long long>(pk_bwd.size()) > pl.bwd_cap || n_slots > pl.slots_cap)
+        return fail(XRDVI_E_INVALID_ARG, "internal: table bound exceeded");
+    std::vector<int> slot_ofs(K + 1, 0), slot_ids(std::max(n_slots, 1));
+    for (int s = 0; s < n_slots; ++s) ++slot_ofs[slot_phase[s] + 1];
+    for (int k = 0; k < K; ++k) slot_ofs[k + 1] += slot_ofs[k];
+    {
+        std::vector<int> fill(slot_ofs.begin(), slot_ofs.end() - 1);
+        for (int s = 0; s < n_slots; ++s) slot_ids[fill[slot_phase[s]]++] = s;   // increasing slot id per phase
+    }
+    std::vector<int> seg_order(pl.n_seg);
+    std::iota(seg_order.begin(), seg_order.end(), 0);
+    std::stable_sort(seg_order.begin(), seg_order.end(), [&](int a, int b) { return seg_work[a] > seg_work[b]; });
+    if (pk_bwd.empty()) pk_bwd.push_back(PeakRec{0, 0.f, 0.f, 0});
 
     // observed data and per-pattern constants
     std::vector<float> yb(static_cast<size_t>(P) * N), bgf(static_cast<size_t>(P) * N);
@@ -366,9 +464,12 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
     h->m_w0 = static_cast<float>(std::log(hyp->w_shape / hyp->w_rate));
     Dev& d = h->dev;
     char* w = h->ws;
-    d.N = static_cast<int>(N); d.NQ = pl.NQ; d.K = K; d.P = pl.P; d.R = pl.R; d.PR = pl.PR;
-    d.n_c = static_cast<int>(n_c); d.ntile = pl.ntile; d.n_units = static_cast<int>(units.size()); d.Mv = Mv;
+    d.N = static_cast<int>(N); d.K = K; d.P = pl.P; d.R = pl.R; d.PR = pl.PR;
+    d.n_c = static_cast<int>(n_c); d.SP = SP; d.W = W; d.n_seg = pl.n_seg; d.n_tile = pl.n_tile;
+    d.n_slots = std::max(n_slots, 1); d.Mv = Mv;
     d.delta = static_cast<float>(delta);
+    d.gcut = static_cast<float>(static_cast<double>(kGaussCut) / (2.0 * delta));
+    d.inv_delta = static_cast<float>(1.0 / delta);
     d.mu_inv_var = static_cast<float>(1.0 / (hyp->mu_sigma * hyp->mu_sigma));
     d.mu_logc = static_cast<float>(-std::log(hyp->mu_sigma * std::sqrt(2.0 * M_PI)));
     d.w_shape = static_cast<float>(hyp->w_shape);
@@ -381,8 +482,10 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
     d.pk_fwd = reinterpret_cast<PeakRec*>(w + pl.o_pkf);
     d.tile_rng = reinterpret_cast<int2*>(w + pl.o_tile);
     d.pk_bwd = reinterpret_cast<PeakRec*>(w + pl.o_pkb);
-    d.units = reinterpret_cast<int4*>(w + pl.o_units);
-    d.unit_ofs = reinterpret_cast<int*>(w + pl.o_uofs);
+    d.warp_rng = reinterpret_cast<int4*>(w + pl.o_wrng);
+    d.seg_order = reinterpret_cast<int*>(w + pl.o_sord);
+    d.slot_ofs = reinterpret_cast<int*>(w + pl.o_sofs);
+    d.slot_ids = reinterpret_cast<int*>(w + pl.o_sids);
     d.pat = reinterpret_cast<PatConst*>(w + pl.o_pat);
     d.area = reinterpret_cast<double*>(w + pl.o_area);
     d.var = reinterpret_cast<float*>(w + pl.o_var);
@@ -393,12 +496,14 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
     d.elbo_k = reinterpret_cast<double*>(w + pl.o_elbok);
     d.ll_t = reinterpret_cast<double*>(w + pl.o_llt);
     d.trace = reinterpret_cast<double*>(w + pl.o_trace);
+    d.done_inst = reinterpret_cast<unsigned int*>(w + pl.o_done);
     d.ctl = reinterpret_cast<Ctl*>(w + pl.o_ctl);
     d.lat = reinterpret_cast<float4*>(w + pl.o_lat);
     d.eps = reinterpret_cast<float4*>(w + pl.o_eps);
-    d.e = reinterpret_cast<float4*>(w + pl.o_e);
+    d.rr = reinterpret_cast<float*>(w + pl.o_rr);
+    d.ng = reinterpret_cast<int*>(w + pl.o_ng);
     d.llpart = reinterpret_cast<float*>(w + pl.o_llpart);
-    d.sums = reinterpret_cast<float*>(w + pl.o_sums);
+    d.part8 = reinterpret_cast<float*>(w + pl.o_part8);
     set_S(h, S_max);
 
     cudaStream_t st = h->stream;
@@ -409,15 +514,18 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
     auto chk = [&](cudaError_t e) { if (ce == cudaSuccess) ce = e; };
     chk(up(pl.o_yb, yb.data(), sizeof(float) * yb.size()));
     chk(up(pl.o_bg, bgf.data(), sizeof(float) * bgf.size()));
-    chk(up(pl.o_pkf, pk_fwd.data(), sizeof(PeakRec) * std::max(Mv, 1)));
+    chk(up(pl.o_pkf, pk_fwd.data(), sizeof(PeakRec) * pk_fwd.size()));
     chk(up(pl.o_tile, tile_rng.data(), sizeof(int2) * tile_rng.size()));
-    chk(up(pl.o_pkb, pk_bwd.data(), sizeof(PeakRec) * std::max(Mv, 1)));
-    chk(up(pl.o_units, units.data(), sizeof(int4) * units.size()));
-    chk(up(pl.o_uofs, unit_ofs.data(), sizeof(int) * unit_ofs.size()));
+    chk(up(pl.o_pkb, pk_bwd.data(), sizeof(PeakRec) * pk_bwd.size()));
+    chk(up(pl.o_wrng, warp_rng.data(), sizeof(int4) * warp_rng.size()));
+    chk(up(pl.o_sord, seg_order.data(), sizeof(int) * seg_order.size()));
+    chk(up(pl.o_sofs, slot_ofs.data(), sizeof(int) * slot_ofs.size()));
+    chk(up(pl.o_sids, slot_ids.data(), sizeof(int) * slot_ids.size()));
     chk(up(pl.o_pat, pat.data(), sizeof(PatConst) * pat.size()));
     chk(up(pl.o_area, area.data(), sizeof(double) * area.size()));
     chk(up(pl.o_mh0, m_h0.data(), sizeof(float) * m_h0.size()));
     chk(cudaMemsetAsync(w + pl.o_trace, 0xFF, sizeof(double) * kTraceCap * pl.PR, st));
+    chk(cudaMemsetAsync(w + pl.o_part8, 0, sizeof(float) * static_cast<size_t>(pl.G_max) * d.n_slots * 8, st));
     chk(cudaStreamSynchronize(st));  // host staging vectors go out of scope below
     for (auto& e : h->ev) chk(cudaEventCreate(&e));
     if (ce != cudaSuccess) {
@@ -472,23 +580,30 @@ int xrdvi_set_state(xrdvi* h, const float* var_params, int64_t step) {
     return write_ctl(h, 0, step, step, -1);
 }
 
-int xrdvi_elbo_grad(xrdvi* h, const float* var_params, int32_t S, uint64_t seed, uint64_t iteration,
-                    double* elbo, float* grad) {
+// shared prologue of the evaluation entry points: stage var_params (or use the state), set S and the
+// Philox iteration
+static int begin_eval(xrdvi* h, const float* var_params, int32_t S, uint64_t seed, uint64_t iteration, const float** var) {
     int rc = check_S(h, S);
     if (rc) return rc;
     CU(cudaSetDevice(h->device));
-    const size_t b = sizeof(float) * h->plan.PR * 8 * h->K;
-    const float* var = h->dev.var;
+    *var = h->dev.var;
     if (var_params) {
         float* tmp = reinterpret_cast<float*>(h->ws + h->plan.o_vartmp);
-        CU(cudaMemcpyAsync(tmp, var_params, b, cudaMemcpyHostToDevice, h->stream));
-        var = tmp;
+        CU(cudaMemcpyAsync(tmp, var_params, sizeof(float) * h->plan.PR * 8 * h->K, cudaMemcpyHostToDevice, h->stream));
+        *var = tmp;
     }
     set_S(h, S);
-    rc = write_ctl(h, seed, h->step_host, h->step_host, static_cast<long long>(iteration & 0xFFFFFFFFull));
+    return write_ctl(h, seed, h->step_host, h->step_host, static_cast<long long>(iteration & 0xFFFFFFFFull));
+}
+
+int xrdvi_elbo_grad(xrdvi* h, const float* var_params, int32_t S, uint64_t seed, uint64_t iteration,
+                    double* elbo, float* grad) {
+    const float* var = nullptr;
+    int rc = begin_eval(h, var_params, S, seed, iteration, &var);
     if (rc) return rc;
-    rc = enqueue_iteration(h, var, 0, nullptr, 0, nullptr, false);
+    rc = enqueue_eval(h, var, nullptr, 0, false);
     if (rc) return rc;
+    const size_t b = sizeof(float) * h->plan.PR * 8 * h->K;
     std::vector<double> el(elbo ? h->plan.PR : 0);
     std::vector<float> gr(grad ? h->plan.PR * 8 * static_cast<size_t>(h->K) : 0);
     if (elbo) CU(cudaMemcpyAsync(el.data(), h->dev.elbo, sizeof(double) * h->plan.PR, cudaMemcpyDeviceToHost, h->stream));
@@ -504,14 +619,12 @@ int xrdvi_fit(xrdvi* h, int32_t iterations, int32_t S, uint64_t seed, float* var
     if (rc) return rc;
     if (iterations < 0) return fail(XRDVI_E_INVALID_ARG, "iterations < 0");
     CU(cudaSetDevice(h->device));
-    rc = ensure_graph(h, S);
-    if (rc) return rc;
-    set_S(h, S);
-    const long long step0 = h->step_host;
-    rc = write_ctl(h, seed, step0, step0, -1);
-    if (rc) return rc;
-    for (int it = 0; it < iterations; ++it) CU(cudaGraphLaunch(h->graph_exec, h->stream));
-    h->step_host = step0 + iterations;
+    if (iterations > 0) {
+        rc = begin_steps(h, S, seed);
+        if (rc) return rc;
+        for (int it = 0; it < iterations; ++it) CU(cudaGraphLaunch(h->graph_exec, h->stream));
+        h->step_host += iterations;
+    }
     const int PR = h->plan.PR;
     std::vector<float> vo(var_out ? PR * 8 * static_cast<size_t>(h->K) : 0);
     std::vector<double> inc(incl ? PR * static_cast<size_t>(h->K) : 0);
@@ -559,24 +672,14 @@ int xrdvi_inclusion(xrdvi* h, double* incl, double* ratio) {
 
 int xrdvi_debug_profile(xrdvi* h, const float* var_params, int32_t S, uint64_t seed, uint64_t iteration,
                         int64_t n, float* f, double* ll) {
-    int rc = check_S(h, S);
+    const float* var = nullptr;
+    int rc = begin_eval(h, var_params, S, seed, iteration, &var);
     if (rc) return rc;
-    CU(cudaSetDevice(h->device));
     const long long T = static_cast<long long>(h->plan.PR) * S;
     if (n < 0 || n > T) return fail(XRDVI_E_INVALID_ARG, "n out of range");
-    const size_t b = sizeof(float) * h->plan.PR * 8 * h->K;
-    const float* var = h->dev.var;
-    if (var_params) {
-        float* tmp = reinterpret_cast<float*>(h->ws + h->plan.o_vartmp);
-        CU(cudaMemcpyAsync(tmp, var_params, b, cudaMemcpyHostToDevice, h->stream));
-        var = tmp;
-    }
-    set_S(h, S);
-    rc = write_ctl(h, seed, h->step_host, h->step_host, static_cast<long long>(iteration & 0xFFFFFFFFull));
-    if (rc) return rc;
     float* f_dev = nullptr;
     if (f && n > 0) CU(cudaMalloc(&f_dev, sizeof(float) * n * h->N));  // debug path only
-    rc = enqueue_iteration(h, var, 0, f_dev, n, nullptr, true);
+    rc = enqueue_eval(h, var, f_dev, n, true);
     if (rc) { cudaFree(f_dev); return rc; }
     std::vector<double> llh(static_cast<size_t>(h->plan.PR) * h->plan.S_pad);
     cudaError_t e = cudaMemcpyAsync(llh.data(), h->dev.ll_t, sizeof(double) * llh.size(), cudaMemcpyDeviceToHost, h->stream);
@@ -591,25 +694,25 @@ int xrdvi_debug_profile(xrdvi* h, const float* var_params, int32_t S, uint64_t s
     return XRDVI_OK;
 }
 
-int xrdvi_debug_draws(xrdvi* h, int32_t S, uint64_t seed, uint64_t iteration, int64_t n, float* eps, uint32_t* raw) {
-    int rc = check_S(h, S);
+int xrdvi_debug_draws(xrdvi* h, int32_t S, uint64_t seed, uint64_t iteration, int64_t n, float* eps, uint32_t* raw,
+                      int32_t* core_halfwidth) {
+    const float* var = nullptr;
+    int rc = begin_eval(h, nullptr, S, seed, iteration, &var);
     if (rc) return rc;
-    CU(cudaSetDevice(h->device));
     const long long T = static_cast<long long>(h->plan.PR) * S;
     if (n < 0 || n > T || !eps) return fail(XRDVI_E_INVALID_ARG, "n out of range or eps NULL");
-    set_S(h, S);
-    rc = write_ctl(h, seed, h->step_host, h->step_host, static_cast<long long>(iteration & 0xFFFFFFFFull));
-    if (rc) return rc;
     const Dev& d = h->dev;
     const size_t cnt = static_cast<size_t>(d.G) * d.K * 32;
     uint4* raw_dev = nullptr;
     CU(cudaMalloc(&raw_dev, sizeof(uint4) * cnt));  // debug path only
-    draw_transform_kernel<<<dim3((d.K + 3) / 4, d.G), 128, 0, h->stream>>>(d, d.var, raw_dev);
+    launch_draw(d, h->stream, var, raw_dev);
     std::vector<float4> eh(cnt);
     std::vector<uint4> rh(cnt);
+    std::vector<int> ngh(static_cast<size_t>(d.G) * d.K);
     cudaError_t e = cudaGetLastError();
     if (e == cudaSuccess) e = cudaMemcpyAsync(eh.data(), d.eps, sizeof(float4) * cnt, cudaMemcpyDeviceToHost, h->stream);
     if (e == cudaSuccess) e = cudaMemcpyAsync(rh.data(), raw_dev, sizeof(uint4) * cnt, cudaMemcpyDeviceToHost, h->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(ngh.data(), d.ng, sizeof(int) * ngh.size(), cudaMemcpyDeviceToHost, h->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
     cudaFree(raw_dev);
     if (e != cudaSuccess) return fail(XRDVI_E_CUDA, std::string("debug_draws: ") + cudaGetErrorString(e));
@@ -620,45 +723,47 @@ int xrdvi_debug_draws(xrdvi* h, int32_t S, uint64_t seed, uint64_t iteration, in
             const size_t o = (static_cast<size_t>(g) * d.K + k) * 32 + lane;
             std::memcpy(eps + (static_cast<size_t>(t) * d.K + k) * 4, &eh[o], sizeof(float4));
             if (raw) std::memcpy(raw + (static_cast<size_t>(t) * d.K + k) * 4, &rh[o], sizeof(uint4));
+            if (core_halfwidth) core_halfwidth[static_cast<size_t>(t) * d.K + k] = ngh[static_cast<size_t>(g) * d.K + k];
         }
     }
     return XRDVI_OK;
 }
 
-int xrdvi_time_kernels(xrdvi* h, int32_t S, uint64_t seed, int32_t reps, float* ms_fwd, float* ms_bwd, float* ms_iter) {
+int xrdvi_time_kernels(xrdvi* h, int32_t S, uint64_t seed, int32_t reps, float* ms /* [4] */) {
     int rc = check_S(h, S);
     if (rc) return rc;
-    if (reps < 1) return fail(XRDVI_E_INVALID_ARG, "reps < 1");
+    if (reps < 1 || !ms) return fail(XRDVI_E_INVALID_ARG, "reps < 1 or ms NULL");
     CU(cudaSetDevice(h->device));
     set_S(h, S);
     rc = write_ctl(h, seed, h->step_host, h->step_host, -1);
     if (rc) return rc;
     const Dev& d = h->dev;
     cudaStream_t st = h->stream;
-    double tf = 0.0, tb = 0.0, ti = 0.0;
+    double tt = 0.0, tf = 0.0, tu = 0.0, ti = 0.0;
     for (int r = 0; r < reps + 1; ++r) {   // first pass is a warm-up
         CU(cudaEventRecord(h->ev[0], st));
-        draw_transform_kernel<<<dim3((d.K + 3) / 4, d.G), 128, 0, st>>>(d, d.var, nullptr);
+        launch_draw(d, st, d.var, nullptr);
         CU(cudaEventRecord(h->ev[1], st));
-        forward_kernel<<<dim3((d.ntile + kFwdWarps - 1) / kFwdWarps, d.G), 32 * kFwdWarps, 0, st>>>(d, nullptr, 0);
+        launch_tile<true>(d, st, nullptr, 0);
         CU(cudaEventRecord(h->ev[2], st));
-        backward_kernel<<<dim3((d.n_units + kBwdWarps - 1) / kBwdWarps, d.G), 32 * kBwdWarps, 0, st>>>(d);
+        update_draw_kernel<<<dim3(d.K + 1, d.PR), kUpdThreads, 0, st>>>(d, d.var, 0);
         CU(cudaEventRecord(h->ev[3], st));
-        chain_reduce_kernel<<<dim3(d.K, d.PR), kChainThreads, 0, st>>>(d, d.var);
-        finalize_update_kernel<<<d.PR, kFinThreads, 0, st>>>(d, d.var, 0);
+        launch_tile<false>(d, st, nullptr, 0);
         CU(cudaEventRecord(h->ev[4], st));
         CU(cudaGetLastError());
         CU(cudaStreamSynchronize(st));
         if (r == 0) continue;
-        float a = 0, b = 0, c = 0;
+        float a = 0, b = 0, c = 0, e = 0;
         CU(cudaEventElapsedTime(&a, h->ev[1], h->ev[2]));
         CU(cudaEventElapsedTime(&b, h->ev[2], h->ev[3]));
-        CU(cudaEventElapsedTime(&c, h->ev[0], h->ev[4]));
-        tf += a; tb += b; ti += c;
+        CU(cudaEventElapsedTime(&c, h->ev[3], h->ev[4]));
+        CU(cudaEventElapsedTime(&e, h->ev[0], h->ev[3]));
+        tt += a; tu += b; tf += c; ti += e;
     }
-    if (ms_fwd) *ms_fwd = static_cast<float>(tf / reps);
-    if (ms_bwd) *ms_bwd = static_cast<float>(tb / reps);
-    if (ms_iter) *ms_iter = static_cast<float>(ti / reps);
+    ms[0] = static_cast<float>(tt / reps);
+    ms[1] = static_cast<float>(tf / reps);
+    ms[2] = static_cast<float>(tu / reps);
+    ms[3] = static_cast<float>(ti / reps);
     return XRDVI_OK;
 }
 
@@ -667,10 +772,7 @@ int xrdvi_bench_steps(xrdvi* h, int32_t steps, int32_t S, uint64_t seed, size_t 
     if (rc) return rc;
     if (steps < 1 || !ms_steps) return fail(XRDVI_E_INVALID_ARG, "steps < 1 or ms_steps NULL");
     CU(cudaSetDevice(h->device));
-    rc = ensure_graph(h, S);
-    if (rc) return rc;
-    set_S(h, S);
-    rc = write_ctl(h, seed, h->step_host, h->step_host, -1);
+    rc = begin_steps(h, S, seed);
     if (rc) return rc;
     void* flush = nullptr;
     if (flush_bytes) CU(cudaMalloc(&flush, flush_bytes));  // measurement path only

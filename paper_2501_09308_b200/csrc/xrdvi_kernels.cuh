@@ -1,24 +1,43 @@
 // xrdvi_kernels.cuh -- sm_100a kernels of the ELBO-and-gradient hot path.
 //
 // Data-parallel axes: a *sample-instance* t = (pattern, restart, draw s) lives in one LANE; 32
-// consecutive draws of one (pattern, restart) form a *group* g, so every warp works on one 2theta tile
-// (forward) or one peak chunk (backward) for 32 draws at once: peak records and observed data are
-// warp-uniform (broadcast loads), latents are lane-private, all global traffic is 128-byte coalesced.
+// consecutive draws of one (pattern, restart) form a *group* g, so every warp works on one run of grid
+// points for 32 draws at once: peak records and observed data are warp-uniform (broadcast loads),
+// latents are lane-private, all global traffic is 128-byte coalesced.
+//
+// One optimisation step is two kernels:
+//   elbo_tile_kernel   (a-3, a-4, a-5, a-6 likelihood part) one CTA per (2theta segment, group):
+//                      phase 1 synthesises the profile on the segment from every peak whose window
+//                      reaches it and leaves the residual e = (y - f)/sigma_n^2 in SHARED memory;
+//                      phase 2 walks the same peaks phase-major, accumulates the six backward sums
+//                      over the segment, applies the chain rule and reduces over the 32 draws with
+//                      warp shuffles (fixed tree) to 8 floats per (segment, warp, phase-run, group).
+//   update_draw_kernel (a-6 prior part, a-7, a-8, a-1, a-2) one CTA per (phase, instance): fixed-order
+//                      reduction of the partials and of the per-draw prior terms, ELBO, Adam ascent
+//                      on the 8 variational parameters of the phase, then the Philox draws and the
+//                      transform for the NEXT step.
 //
 // Coordinates: t' = 2 (x_i - p_m - mu) / w, so that  G = exp(-4 ln2 t^2) = 2^(-t'^2)  and
 // L = 1/(1+4t^2) = 1/(1+t'^2)  (PAPER.md:221-232 with the unit-area FWHM shapes, reading R1).  A peak is
 // stored as (j_m, delta_m) with p_m = x_{j_m} + delta_m computed in fp64 at create, so
 // t' = (i - j_m) * (Delta*2/w) + (-delta_m - mu) * 2/w  has no fp32 cancellation at high angles.
+//
+// Instruction diet: the FP32 FMA pipe (128 lanes/SM/clk) and the MUFU pipe (16
+// lanes/SM/clk, shared by ex2 and rcp) bound the path.  Two measures cut the MUFU work of the plain
+// formulation (2 MUFU per pair and pass):
+//   * Gaussian core / Lorentz tail: 2^(-t'^2) < 2^-24 for |t'| > 4.9, so outside a per-(group, phase)
+//     core half-width n_g (from the largest sampled w and |mu| of the 32 draws) only L is evaluated;
+//   * shared reciprocal: 1/ua and 1/ub of two neighbouring points come from ONE rcp(ua*ub).
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
 
 namespace xrdvi_dev {
 
-constexpr int kFwdP = 8;        // grid points per thread in the forward kernel
-constexpr int kFwdWarps = 4;    // warps (= tiles) per forward block
-constexpr int kBwdWarps = 4;    // warps (= peak units) per backward block
+constexpr int kPT = 16;         // grid points per thread in phase 1 (one warp = one 16-point tile)
 constexpr int kTraceCap = 4096; // iterations of ELBO trace kept on the device
+constexpr int kUpdThreads = 256;
+constexpr float kGaussCut = 4.9f;   // |t'| beyond which 2^(-t'^2) < 2^-24 is dropped
 
 constexpr float kAG = 0.93943727869965132f;  // 2 sqrt(ln2/pi)
 constexpr float kAL = 0.63661977236758134f;  // 2/pi
@@ -44,13 +63,17 @@ struct Ctl {       // device-resident control block (so that graph replays need 
     long long step;        // completed optimisation steps
     long long trace_base;  // step index of trace row 0
     long long iteration_override;  // >= 0: Philox iteration for elbo_grad/debug; < 0: use step + 1
+    unsigned int done_total;       // instances whose last CTA has finished (update_draw_kernel)
+    unsigned int pad;
 };
 
 struct Dev {
     // sizes
-    int N, NQ, K, P, R, PR, n_c, ntile, n_units, Mv;
+    int N, K, P, R, PR, n_c, SP, n_seg, n_tile, n_slots, Mv, W;
     int S, gpi, G;       // draws, groups per instance, groups (run-time)
     float delta;         // grid step (deg)
+    float gcut;          // kGaussCut / (2 Delta): core half-width in points per unit of w
+    float inv_delta;
     // priors / optimiser
     float mu_inv_var, mu_logc, w_shape, w_rate, w_logc;
     float lr, beta1, beta2, adam_eps;
@@ -58,10 +81,12 @@ struct Dev {
     const float* yb;          // [P][N]  y - B
     const float* bg;          // [P][N]
     const PeakRec* pk_fwd;    // [Mv] sorted by j
-    const int2* tile_rng;     // [ntile] peak range [x,y) of each forward tile
-    const PeakRec* pk_bwd;    // [Mv] phase-major
-    const int4* units;        // [n_units] (k, m0, m1, -)
-    const int* unit_ofs;      // [K+1] units of phase k
+    const int2* tile_rng;     // [n_tile] peak range [x,y) in pk_fwd of each 16-point tile
+    const PeakRec* pk_bwd;    // per-segment phase-major peak lists, concatenated
+    const int4* warp_rng;     // [n_seg][W]: (m0, m1) range in pk_bwd of the warp, .z = its first slot
+    const int* seg_order;     // [n_seg] segments by decreasing work (LPT dispatch order)
+    const int* slot_ofs;      // [K+1] CSR: slots of phase k
+    const int* slot_ids;      // [n_slots]
     const PatConst* pat;      // [P]
     const double* area;       // [K] A_k = sum_m I_m
     // state
@@ -70,16 +95,18 @@ struct Dev {
     float* mom2;
     float* grad;              // [PR][2][K][4]
     double* elbo;             // [PR]
-    double* elbo_k;           // [PR][K]
+    double* elbo_k;           // [PR][K+1]  per-phase ELBO terms; [K] = mean log-likelihood
     double* ll_t;             // [PR][S_pad]
     double* trace;            // [kTraceCap][PR]
+    unsigned int* done_inst;  // [PR] CTAs of the instance that have finished
     Ctl* ctl;
     // per-iteration buffers
     float4* lat;              // [G][K][32]  (2/w, -mu*2/w, h(1-r)aG/w, h r aL/w)
     float4* eps;              // [G][K][32]
-    float4* e;                // [G][NQ][32] residual e_i = (y_i - f_i)/sigma_n^2, 4 points per float4
-    float* llpart;            // [G][ntile][32] sum over the tile of ((y-f)/sigma_n)^2
-    float* sums;              // [G][n_units][6][32]
+    float* rr;                // [G][K][32]  r
+    int* ng;                  // [G][K]      Gaussian core half-width in grid points
+    float* llpart;            // [G][n_seg][32] sum over the segment of ((y-f)/sigma_n)^2
+    float* part8;             // [G][n_slots][8] (g_h, g_mu, g_w, g_r, g_h eps_h, ...) summed over 32 draws
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -123,12 +150,12 @@ __device__ __forceinline__ float4 normals_from_words(uint4 w) {
 struct Phys { float zh, zw, zr, h, mu, w, r; };
 
 // zeta = m + exp(l) * eps; h = exp(zeta_h), mu = zeta_mu, w = exp(zeta_w), r = sigmoid(zeta_r)  (R6)
-__device__ __forceinline__ Phys transform(const float4 m, const float4 l, const float4 ep) {
+__device__ __forceinline__ Phys transform(const float4 m, const float4 sg, const float4 ep) {
     Phys q;
-    q.zh = fmaf(expf(l.x), ep.x, m.x);
-    q.mu = fmaf(expf(l.y), ep.y, m.y);
-    q.zw = fmaf(expf(l.z), ep.z, m.z);
-    q.zr = fmaf(expf(l.w), ep.w, m.w);
+    q.zh = fmaf(sg.x, ep.x, m.x);
+    q.mu = fmaf(sg.y, ep.y, m.y);
+    q.zw = fmaf(sg.z, ep.z, m.z);
+    q.zr = fmaf(sg.w, ep.w, m.w);
     q.h = expf(q.zh);
     q.w = expf(q.zw);
     q.r = 1.0f / (1.0f + expf(-q.zr));
@@ -140,8 +167,43 @@ __device__ __forceinline__ long long philox_iteration(const Ctl* ctl) {
     return o >= 0 ? o : ctl->step + 1;
 }
 
-// ------------------------------------------------------------------------------------------------
-// a-1 + a-2: draws and transform.  grid (ceil(K/4), G), block 128: thread = (phase k, lane).
+// a-1 + a-2 for one (instance, phase k, draw s): Philox draw, transform, latent record.  Must be called by
+// all 32 lanes of a warp whose lanes hold consecutive draws of one group (the core half-width n_g is a
+// warp maximum).
+__device__ __forceinline__ void draw_one(const Dev& d, int inst, int k, int s, unsigned it, unsigned long long seed,
+                                         const float4 m, const float4 l, uint4* __restrict__ raw_out) {
+    const int lane = threadIdx.x & 31;
+    const int g = inst * d.gpi + (s >> 5);
+    const uint4 words = philox4x32_10(make_uint4(it, static_cast<unsigned>(s), static_cast<unsigned>(k),
+                                                 static_cast<unsigned>(inst)),
+                                      make_uint2(static_cast<unsigned>(seed), static_cast<unsigned>(seed >> 32)));
+    const float4 ep = normals_from_words(words);
+    const float4 sg = make_float4(expf(l.x), expf(l.y), expf(l.z), expf(l.w));
+    const Phys q = transform(m, sg, ep);
+    // 1/w is capped at 5e7 (w >= 2e-8 deg: far outside the model's regime) so that the shared reciprocal
+    // rcp(ua ub) of two points can never see an overflowed product
+    const float iw = fminf(1.0f / q.w, 5.0e7f);
+    const float iw2 = 2.0f * iw;
+    float4 lt = make_float4(iw2, -q.mu * iw2, q.h * (1.0f - q.r) * kAG * iw, q.h * q.r * kAL * iw);
+    // Gaussian core half-width in grid points for this draw: |t'| <= kGaussCut  <=>
+    // |i - j| <= kGaussCut w / (2 Delta) + |delta_m + mu| / Delta; |delta_m| <= Delta/2, +1 for rounding
+    float reach = fmaf(d.gcut, q.w, fabsf(q.mu) * d.inv_delta) + 1.5f;
+    if (s >= d.S) {  // padding lanes contribute nothing
+        lt = make_float4(1.0f, 0.0f, 0.0f, 0.0f);
+        reach = 0.0f;
+    }
+    if (!(reach < 1.0e9f)) reach = 1.0e9f;  // also catches NaN
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) reach = fmaxf(reach, __shfl_xor_sync(0xffffffffu, reach, o));
+    const size_t o = (static_cast<size_t>(g) * d.K + k) * 32 + lane;
+    d.lat[o] = lt;
+    d.eps[o] = ep;
+    d.rr[o] = q.r;
+    if (lane == 0) d.ng[static_cast<size_t>(g) * d.K + k] = static_cast<int>(reach) + 1;
+    if (raw_out) raw_out[o] = words;
+}
+
+// Stand-alone draw kernel (first step of a fit, xrdvi_elbo_grad, debug).  grid (ceil(K/4), G), block 128.
 __global__ void __launch_bounds__(128) draw_transform_kernel(const Dev d, const float* __restrict__ var,
                                                               uint4* __restrict__ raw_out) {
     const int lane = threadIdx.x & 31;
@@ -150,164 +212,342 @@ __global__ void __launch_bounds__(128) draw_transform_kernel(const Dev d, const 
     if (k >= d.K) return;
     const int inst = g / d.gpi;
     const int s = (g - inst * d.gpi) * 32 + lane;
-    const unsigned long long seed = d.ctl->seed;
-    const unsigned it = static_cast<unsigned>(philox_iteration(d.ctl));
-    const uint4 words = philox4x32_10(make_uint4(it, static_cast<unsigned>(s), static_cast<unsigned>(k),
-                                                 static_cast<unsigned>(inst)),
-                                      make_uint2(static_cast<unsigned>(seed), static_cast<unsigned>(seed >> 32)));
-    const float4 ep = normals_from_words(words);
     const float4 m = *reinterpret_cast<const float4*>(var + (static_cast<size_t>(inst) * 2 * d.K + k) * 4);
     const float4 l = *reinterpret_cast<const float4*>(var + (static_cast<size_t>(inst) * 2 * d.K + d.K + k) * 4);
-    const Phys q = transform(m, l, ep);
-    const float iw = 1.0f / q.w;
-    const float iw2 = 2.0f * iw;
-    float4 lt = make_float4(iw2, -q.mu * iw2, q.h * (1.0f - q.r) * kAG * iw, q.h * q.r * kAL * iw);
-    if (s >= d.S) lt = make_float4(1.0f, 0.0f, 0.0f, 0.0f);  // padding lanes contribute nothing
-    const size_t o = (static_cast<size_t>(g) * d.K + k) * 32 + lane;
-    d.lat[o] = lt;
-    d.eps[o] = ep;
-    if (raw_out) raw_out[o] = words;
+    draw_one(d, inst, k, s, static_cast<unsigned>(philox_iteration(d.ctl)), d.ctl->seed, m, l, raw_out);
 }
 
 // ------------------------------------------------------------------------------------------------
-// a-3 + a-4: fused profile + residual.  grid (ceil(ntile/kFwdWarps), G), block 32*kFwdWarps.
-// Warp = one tile of kFwdP consecutive grid points for the 32 draws of group g.
-__global__ void __launch_bounds__(32 * kFwdWarps) forward_kernel(const Dev d, float* __restrict__ f_dbg,
-                                                                  long long n_dbg) {
+// Phase-1 building blocks (profile).  acc[p] += I_m [ c_G 2^(-t'^2) + c_L / (1 + t'^2) ].
+// Two neighbouring points share one reciprocal: 1/ua = ub * rcp(ua ub).
+template <bool CORE>
+__device__ __forceinline__ void fwd_pair(float ta, float tb, float cg, float cl, float& acca, float& accb) {
+    const float ua = fmaf(ta, ta, 1.0f), ub = fmaf(tb, tb, 1.0f);
+    const float rc = rcp_approx(ua * ub) * cl;
+    acca = fmaf(rc, ub, acca);
+    accb = fmaf(rc, ua, accb);
+    if (CORE) {
+        acca = fmaf(cg, ex2_approx(-(ta * ta)), acca);
+        accb = fmaf(cg, ex2_approx(-(tb * tb)), accb);
+    }
+}
+
+// One quad (4 points, first point index p0 of the tile) with per-point window masks.
+template <bool CORE>
+__device__ __forceinline__ void fwd_quad_masked(float t0, float step, int p0, int p_lo, int p_hi, float cg, float cl,
+                                                float& a0, float& a1, float& a2, float& a3) {
+    float v[4] = {0.f, 0.f, 0.f, 0.f};
+    const float ta = fmaf(static_cast<float>(p0), step, t0), tb = fmaf(static_cast<float>(p0 + 1), step, t0);
+    const float tc = fmaf(static_cast<float>(p0 + 2), step, t0), td = fmaf(static_cast<float>(p0 + 3), step, t0);
+    fwd_pair<CORE>(ta, tb, cg, cl, v[0], v[1]);
+    fwd_pair<CORE>(tc, td, cg, cl, v[2], v[3]);
+    a0 += (p0 + 0 >= p_lo && p0 + 0 <= p_hi) ? v[0] : 0.0f;
+    a1 += (p0 + 1 >= p_lo && p0 + 1 <= p_hi) ? v[1] : 0.0f;
+    a2 += (p0 + 2 >= p_lo && p0 + 2 <= p_hi) ? v[2] : 0.0f;
+    a3 += (p0 + 3 >= p_lo && p0 + 3 <= p_hi) ? v[3] : 0.0f;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Phase-2 building blocks (six sums in t' units):
+//   a1 = sum e L, a2 = sum e G, a3 = sum e L^2 t', a4 = sum e G t', a5 = sum e L^2, a6 = sum e G t'^2
+struct Acc6 { float a1, a2, a3, a4, a5, a6; };
+
+template <bool CORE>
+__device__ __forceinline__ void bwd_pair(float ea, float eb, float ta, float tb, Acc6& a) {
+    const float ua = fmaf(ta, ta, 1.0f), ub = fmaf(tb, tb, 1.0f);
+    const float r = rcp_approx(ua * ub);
+    const float La = r * ub, Lb = r * ua;
+    const float xa = ea * La, xb = eb * Lb;
+    a.a1 += xa + xb;
+    const float pa = xa * La, pb = xb * Lb;
+    a.a5 += pa + pb;
+    a.a3 = fmaf(pa, ta, fmaf(pb, tb, a.a3));
+    if (CORE) {
+        const float za = ea * ex2_approx(-(ta * ta)), zb = eb * ex2_approx(-(tb * tb));
+        a.a2 += za + zb;
+        const float zta = za * ta, ztb = zb * tb;
+        a.a4 += zta + ztb;
+        a.a6 = fmaf(zta, ta, fmaf(ztb, tb, a.a6));
+    }
+}
+
+template <bool CORE>
+__device__ __forceinline__ void bwd_quad(const float4 e4, float tq, float step, Acc6& a) {
+    const float t1 = tq + step, t2 = fmaf(2.0f, step, tq), t3 = fmaf(3.0f, step, tq);
+    bwd_pair<CORE>(e4.x, e4.y, tq, t1, a);
+    bwd_pair<CORE>(e4.z, e4.w, t2, t3, a);
+}
+
+// Fixed-tree reduction of 8 per-lane values over the 32 lanes; lane c < 8 returns the total of v[c].
+// Rounds 1-3 halve the number of values each lane carries (transpose-reduce), rounds 4-5 are plain
+// butterflies: 9 shuffles instead of 40.
+__device__ __forceinline__ float warp_reduce8(float (&v)[8]) {
     const int lane = threadIdx.x & 31;
-    const int tile = blockIdx.x * kFwdWarps + (threadIdx.x >> 5);
+    float w4[4], w2[2];
+    {
+        const bool up = lane & 16;
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const float send = up ? v[i] : v[i + 4];
+            const float keep = up ? v[i + 4] : v[i];
+            w4[i] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
+        }
+    }
+    {
+        const bool up = lane & 8;
+#pragma unroll
+        for (int i = 0; i < 2; ++i) {
+            const float send = up ? w4[i] : w4[i + 2];
+            const float keep = up ? w4[i + 2] : w4[i];
+            w2[i] = keep + __shfl_xor_sync(0xffffffffu, send, 8);
+        }
+    }
+    float w1;
+    {
+        const bool up = lane & 4;
+        const float send = up ? w2[0] : w2[1];
+        const float keep = up ? w2[1] : w2[0];
+        w1 = keep + __shfl_xor_sync(0xffffffffu, send, 4);
+    }
+    w1 += __shfl_xor_sync(0xffffffffu, w1, 2);
+    w1 += __shfl_xor_sync(0xffffffffu, w1, 1);
+    // a lane now holds the total of value c = 4*bit4 + 2*bit3 + bit2 of its lane index; move it to lane c
+    const int src = ((lane & 4) ? 16 : 0) | ((lane & 2) ? 8 : 0) | ((lane & 1) ? 4 : 0);
+    return __shfl_sync(0xffffffffu, w1, src);
+}
+
+// ------------------------------------------------------------------------------------------------
+// a-3 .. a-6 (likelihood part): fused profile + residual + backward.
+// grid (n_seg, G), block 32*W; segment = 16*W consecutive grid points; warp w owns tile 16*w.. in phase 1
+// and the peak range warp_rng[seg][w] of the segment's phase-major list in phase 2.
+template <int W, bool BWD>
+__global__ void __launch_bounds__(32 * W) elbo_tile_kernel(const Dev d, float* __restrict__ f_dbg, long long n_dbg) {
+    __shared__ float4 e_s[4 * W][32];
+    __shared__ float ss_s[W][32];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int seg = d.seg_order[blockIdx.x];
     const int g = blockIdx.y;
-    if (tile >= d.ntile) return;
-    const int i0 = tile * kFwdP;
-    const int2 rng = d.tile_rng[tile];
+    const int seg0 = seg * (kPT * W);
+    const int i0 = seg0 + kPT * w;
     const float4* __restrict__ lat = d.lat + static_cast<size_t>(g) * d.K * 32 + lane;
-    const int full_lo = i0 + kFwdP - 1 - d.n_c, full_hi = i0 + d.n_c;
+    const int* __restrict__ ngk = d.ng + static_cast<size_t>(g) * d.K;
+    const int inst = g / d.gpi;
+    const int pat = inst / d.R;
+    const PatConst pc = d.pat[pat];
 
-    float acc[kFwdP];
+    // ---------------- phase 1: profile on the 16 points of this warp ----------------
+    float acc[kPT];
 #pragma unroll
-    for (int p = 0; p < kFwdP; ++p) acc[p] = 0.0f;
+    for (int p = 0; p < kPT; ++p) acc[p] = 0.0f;
 
-    for (int m = rng.x; m < rng.y; ++m) {
-        const PeakRec pk = d.pk_fwd[m];
-        const float4 lt = lat[static_cast<size_t>(pk.k) * 32];
-        const float step = d.delta * lt.x;
-        const float tc = fmaf(-pk.delta, lt.x, lt.y);
-        const float t0 = fmaf(static_cast<float>(i0 - pk.j), step, tc);
-        const float cg = pk.inten * lt.z, cl = pk.inten * lt.w;
-        if (pk.j >= full_lo && pk.j <= full_hi) {  // window covers the whole tile (warp-uniform)
-#pragma unroll
-            for (int p = 0; p < kFwdP; ++p) {
-                const float t = fmaf(static_cast<float>(p), step, t0);
-                const float q = t * t;
-                acc[p] = fmaf(cg, ex2_approx(-q), acc[p]);
-                acc[p] = fmaf(cl, rcp_approx(1.0f + q), acc[p]);
+    if (i0 < d.N) {
+        const int2 rng = d.tile_rng[i0 / kPT];
+        const int n_c = d.n_c;
+        PeakRec pk_n;
+        float4 lt_n;
+        int ng_n = 0;
+        if (rng.x < rng.y) {
+            pk_n = d.pk_fwd[rng.x];
+            lt_n = lat[static_cast<size_t>(pk_n.k) * 32];
+            ng_n = ngk[pk_n.k];
+        }
+        for (int m = rng.x; m < rng.y; ++m) {
+            const PeakRec pk = pk_n;
+            const float4 lt = lt_n;
+            const int ngc = ng_n;
+            if (m + 1 < rng.y) {  // prefetch the next peak and its latents
+                pk_n = d.pk_fwd[m + 1];
+                lt_n = lat[static_cast<size_t>(pk_n.k) * 32];
+                ng_n = ngk[pk_n.k];
             }
-        } else {
+            const float step = d.delta * lt.x;
+            const float tc = fmaf(-pk.delta, lt.x, lt.y);
+            const int dj = pk.j - i0;                         // peak centre in tile coordinates
+            const float t0 = fmaf(static_cast<float>(-dj), step, tc);
+            const float cl = pk.inten * lt.w;
+            const int p_lo = dj - n_c, p_hi = dj + n_c;       // in-window points of the tile: p_lo <= p <= p_hi
+            const bool full = (p_lo <= 0) && (p_hi >= kPT - 1);
+            const bool core_any = (dj + ngc >= 0) && (dj - ngc <= kPT - 1);
+            if (full && !core_any) {  // whole tile inside the window and on the Lorentz tail (warp-uniform)
 #pragma unroll
-            for (int p = 0; p < kFwdP; ++p) {
-                const int dn = i0 + p - pk.j;
-                const bool in = (dn >= -d.n_c) && (dn <= d.n_c);
-                const float t = fmaf(static_cast<float>(p), step, t0);
-                const float q = t * t;
-                const float v = fmaf(cg, ex2_approx(-q), cl * rcp_approx(1.0f + q));
-                acc[p] += in ? v : 0.0f;
+                for (int p = 0; p < kPT; p += 2) {
+                    const float ta = fmaf(static_cast<float>(p), step, t0);
+                    const float tb = fmaf(static_cast<float>(p + 1), step, t0);
+                    fwd_pair<false>(ta, tb, 0.0f, cl, acc[p], acc[p + 1]);
+                }
+            } else {
+                const float cg = pk.inten * lt.z;
+#pragma unroll
+                for (int q = 0; q < kPT / 4; ++q) {
+                    const int qlo = 4 * q, qhi = 4 * q + 3;
+                    if (qhi < p_lo || qlo > p_hi) continue;                 // quad outside the window
+                    const bool qfull = (qlo >= p_lo) && (qhi <= p_hi);
+                    const bool qcore = (dj + ngc >= qlo) && (dj - ngc <= qhi);
+                    if (qfull) {
+                        const float ta = fmaf(static_cast<float>(qlo), step, t0);
+                        const float tb = fmaf(static_cast<float>(qlo + 1), step, t0);
+                        const float tcq = fmaf(static_cast<float>(qlo + 2), step, t0);
+                        const float td = fmaf(static_cast<float>(qlo + 3), step, t0);
+                        if (qcore) {
+                            fwd_pair<true>(ta, tb, cg, cl, acc[qlo], acc[qlo + 1]);
+                            fwd_pair<true>(tcq, td, cg, cl, acc[qlo + 2], acc[qlo + 3]);
+                        } else {
+                            fwd_pair<false>(ta, tb, cg, cl, acc[qlo], acc[qlo + 1]);
+                            fwd_pair<false>(tcq, td, cg, cl, acc[qlo + 2], acc[qlo + 3]);
+                        }
+                    } else if (qcore) {
+                        fwd_quad_masked<true>(t0, step, qlo, p_lo, p_hi, cg, cl, acc[qlo], acc[qlo + 1], acc[qlo + 2], acc[qlo + 3]);
+                    } else {
+                        fwd_quad_masked<false>(t0, step, qlo, p_lo, p_hi, cg, cl, acc[qlo], acc[qlo + 1], acc[qlo + 2], acc[qlo + 3]);
+                    }
+                }
             }
         }
     }
 
-    // epilogue: residual, e = (y - f)/sigma_n^2, partial sum of ((y - f)/sigma_n)^2
-    const int inst = g / d.gpi;
-    const int pat = inst / d.R;
-    const PatConst pc = d.pat[pat];
-    const float* __restrict__ yb = d.yb + static_cast<size_t>(pat) * d.N;
-    float ev[kFwdP];
-    float ss = 0.0f;
+    // residual, e = (y - f)/sigma_n^2, partial sum of ((y - f)/sigma_n)^2
+    {
+        const float* __restrict__ yb = d.yb + static_cast<size_t>(pat) * d.N;
+        float ev[kPT];
+        float ss = 0.0f;
 #pragma unroll
-    for (int p = 0; p < kFwdP; ++p) {
-        const int i = i0 + p;
-        float r = 0.0f;
-        if (i < d.N) r = yb[i] - acc[p];
-        const float z = r * pc.inv_sn;
-        ss = fmaf(z, z, ss);
-        ev[p] = r * pc.inv_sn2;
+        for (int p = 0; p < kPT; ++p) {
+            const int i = i0 + p;
+            float r = 0.0f;
+            if (i < d.N) r = yb[i] - acc[p];
+            const float z = r * pc.inv_sn;
+            ss = fmaf(z, z, ss);
+            ev[p] = r * pc.inv_sn2;
+        }
+        if (BWD) {
+#pragma unroll
+            for (int v = 0; v < kPT / 4; ++v)
+                e_s[4 * w + v][lane] = make_float4(ev[4 * v], ev[4 * v + 1], ev[4 * v + 2], ev[4 * v + 3]);
+        }
+        ss_s[w][lane] = ss;
     }
-    float4* __restrict__ eo = d.e + (static_cast<size_t>(g) * d.NQ + (i0 >> 2)) * 32 + lane;
-#pragma unroll
-    for (int v = 0; v < kFwdP / 4; ++v)
-        if ((i0 >> 2) + v < d.NQ) eo[static_cast<size_t>(v) * 32] = make_float4(ev[4 * v], ev[4 * v + 1], ev[4 * v + 2], ev[4 * v + 3]);
-    d.llpart[(static_cast<size_t>(g) * d.ntile + tile) * 32 + lane] = ss;
-
-    if (f_dbg) {  // debug read-back of the profile (parity tests); warp-uniform branch
+    if (f_dbg && i0 < d.N) {  // debug read-back of the profile (parity tests); warp-uniform branch
         const int s = (g - inst * d.gpi) * 32 + lane;
         const long long t = static_cast<long long>(inst) * d.S + s;
         if (s < d.S && t < n_dbg) {
             const float* __restrict__ bg = d.bg + static_cast<size_t>(pat) * d.N;
 #pragma unroll
-            for (int p = 0; p < kFwdP; ++p)
+            for (int p = 0; p < kPT; ++p)
                 if (i0 + p < d.N) f_dbg[t * d.N + i0 + p] = acc[p] + bg[i0 + p];
         }
     }
-}
-
-// ------------------------------------------------------------------------------------------------
-// a-5: backward six sums.  grid (ceil(n_units/kBwdWarps), G), block 32*kBwdWarps.
-// Warp = one unit (a chunk of peaks of one phase) for the 32 draws of group g.  Sums in t' units:
-//   B1 = sum e I L, B2 = sum e I G, B3 = sum e I L^2 t', B4 = sum e I G t', B5 = sum e I L^2, B6 = sum e I G t'^2
-__global__ void __launch_bounds__(32 * kBwdWarps) backward_kernel(const Dev d) {
-    const int lane = threadIdx.x & 31;
-    const int unit = blockIdx.x * kBwdWarps + (threadIdx.x >> 5);
-    const int g = blockIdx.y;
-    if (unit >= d.n_units) return;
-    const int4 un = d.units[unit];
-    const float4 lt = d.lat[(static_cast<size_t>(g) * d.K + un.x) * 32 + lane];
-    const float step = d.delta * lt.x;
-    const float4* __restrict__ eg = d.e + static_cast<size_t>(g) * d.NQ * 32 + lane;
-
-    float B1 = 0.f, B2 = 0.f, B3 = 0.f, B4 = 0.f, B5 = 0.f, B6 = 0.f;
-    for (int m = un.y; m < un.z; ++m) {
-        const PeakRec pk = d.pk_bwd[m];
-        const int lo = max(0, pk.j - d.n_c), hi = min(d.N - 1, pk.j + d.n_c);
-        const int q0 = lo >> 2, q1 = hi >> 2;
-        const float tc = fmaf(-pk.delta, lt.x, lt.y);
-        float a1 = 0.f, a2 = 0.f, a3 = 0.f, a4 = 0.f, a5 = 0.f, a6 = 0.f;
-        for (int q = q0; q <= q1; ++q) {
-            float4 e4 = eg[static_cast<size_t>(q) * 32];
-            if (q == q0 || q == q1) {  // ragged ends of the window (warp-uniform)
-                const int ib = q * 4;
-                if (ib + 0 < lo || ib + 0 > hi) e4.x = 0.f;
-                if (ib + 1 < lo || ib + 1 > hi) e4.y = 0.f;
-                if (ib + 2 < lo || ib + 2 > hi) e4.z = 0.f;
-                if (ib + 3 < lo || ib + 3 > hi) e4.w = 0.f;
-            }
-            const float tq = fmaf(static_cast<float>(q * 4 - pk.j), step, tc);
-            const float ee[4] = {e4.x, e4.y, e4.z, e4.w};
+    __syncthreads();
+    if (w == 0) {  // fixed-order sum over the warps of the segment
+        float ss = ss_s[0][lane];
 #pragma unroll
-            for (int c = 0; c < 4; ++c) {
-                const float t = fmaf(static_cast<float>(c), step, tq);
-                const float qq = t * t;
-                const float G = ex2_approx(-qq);
-                const float L = rcp_approx(1.0f + qq);
-                const float x = ee[c] * L;
-                a1 += x;
-                const float y = x * L;
-                a5 += y;
-                a3 = fmaf(y, t, a3);
-                const float z = ee[c] * G;
-                a2 += z;
-                const float zt = z * t;
-                a4 += zt;
-                a6 = fmaf(zt, t, a6);
+        for (int v = 1; v < W; ++v) ss += ss_s[v][lane];
+        d.llpart[(static_cast<size_t>(g) * d.n_seg + seg) * 32 + lane] = ss;
+    }
+    if (!BWD) return;
+
+    // ---------------- phase 2: six sums over the segment, chain rule, reduction over the draws ----------------
+    const int4 wr = d.warp_rng[seg * W + w];
+    if (wr.x >= wr.y) return;
+    const int seg_hi = min(seg0 + kPT * W - 1, d.N - 1);
+    const float4* __restrict__ epsg = d.eps + static_cast<size_t>(g) * d.K * 32 + lane;
+    const float* __restrict__ rrg = d.rr + static_cast<size_t>(g) * d.K * 32 + lane;
+    float* __restrict__ part = d.part8 + static_cast<size_t>(g) * d.n_slots * 8;
+    int slot = wr.z;
+    int cur_k = -1;
+    float4 lt = make_float4(0.f, 0.f, 0.f, 0.f);
+    float step = 0.0f;
+    int ngc = 0;
+    float B1 = 0.f, B2 = 0.f, B3 = 0.f, B4 = 0.f, B5 = 0.f, B6 = 0.f;
+
+    auto flush = [&]() {
+        // chain rule for the likelihood part (per draw), then sum over the 32 draws of the group
+        const float4 ep = epsg[static_cast<size_t>(cur_k) * 32];
+        const float r = rrg[static_cast<size_t>(cur_k) * 32];
+        const float cG = lt.z, cL = lt.w;
+        float v[8];
+        v[0] = fmaf(cL, B1, cG * B2);
+        v[1] = lt.x * (2.0f * cL * B3 + (2.0f * kLn2) * cG * B4);
+        v[2] = -(cL * (2.0f * B5 - B1) + cG * (B2 - (2.0f * kLn2) * B6));
+        v[3] = (1.0f - r) * cL * B1 - r * cG * B2;
+        v[4] = v[0] * ep.x; v[5] = v[1] * ep.y; v[6] = v[2] * ep.z; v[7] = v[3] * ep.w;
+        const float tot = warp_reduce8(v);
+        if (lane < 8) part[static_cast<size_t>(slot) * 8 + lane] = tot;
+    };
+
+    PeakRec pk_n = d.pk_bwd[wr.x];
+    for (int m = wr.x; m < wr.y; ++m) {
+        const PeakRec pk = pk_n;
+        if (m + 1 < wr.y) pk_n = d.pk_bwd[m + 1];
+        if (pk.k != cur_k) {   // new phase run (warp-uniform)
+            if (cur_k >= 0) { flush(); ++slot; }
+            cur_k = pk.k;
+            lt = lat[static_cast<size_t>(cur_k) * 32];
+            step = d.delta * lt.x;
+            ngc = ngk[cur_k];
+            B1 = B2 = B3 = B4 = B5 = B6 = 0.f;
+        }
+        const int lo = max(seg0, pk.j - d.n_c), hi = min(seg_hi, pk.j + d.n_c);   // lo <= hi by construction
+        const float tc = fmaf(-pk.delta, lt.x, lt.y);
+        const float tseg = fmaf(static_cast<float>(seg0 - pk.j), step, tc);       // t' at the first point of the segment
+        const float step4 = 4.0f * step;
+        int ql = (lo - seg0) >> 2, qh = (hi - seg0) >> 2;                         // local quads [ql, qh]
+        const int c_lo = pk.j - ngc, c_hi = pk.j + ngc;                           // Gaussian core [c_lo, c_hi]
+        Acc6 a = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+        // ragged window ends: quads whose points are partly outside [lo, hi] get their e zeroed there
+        const bool rag_lo = (lo & 3) != 0, rag_hi = ((hi + 1) & 3) != 0;
+        if (rag_lo || (rag_hi && ql == qh)) {
+            float4 e4 = e_s[ql][lane];
+            const int ib = seg0 + 4 * ql;
+            if (ib + 0 < lo || ib + 0 > hi) e4.x = 0.f;
+            if (ib + 1 < lo || ib + 1 > hi) e4.y = 0.f;
+            if (ib + 2 < lo || ib + 2 > hi) e4.z = 0.f;
+            if (ib + 3 < lo || ib + 3 > hi) e4.w = 0.f;
+            const float tq = fmaf(static_cast<float>(4 * ql), step, tseg);
+            if (ib + 3 >= c_lo && ib <= c_hi) bwd_quad<true>(e4, tq, step, a);
+            else bwd_quad<false>(e4, tq, step, a);
+            ++ql;
+        }
+        if (rag_hi && ql <= qh) {
+            float4 e4 = e_s[qh][lane];
+            const int ib = seg0 + 4 * qh;
+            if (ib + 1 > hi) e4.y = 0.f;
+            if (ib + 2 > hi) e4.z = 0.f;
+            if (ib + 3 > hi) e4.w = 0.f;
+            const float tq = fmaf(static_cast<float>(4 * qh), step, tseg);
+            if (ib + 3 >= c_lo && ib <= c_hi) bwd_quad<true>(e4, tq, step, a);
+            else bwd_quad<false>(e4, tq, step, a);
+            --qh;
+        }
+        if (ql <= qh) {
+            // split [ql, qh] into tail | core | tail at quad granularity
+            int qc0 = (max(c_lo, seg0) - seg0) >> 2, qc1 = (min(c_hi, seg_hi) - seg0) >> 2;
+            if (c_hi < seg0 + 4 * ql || c_lo > seg0 + 4 * qh + 3) { qc0 = qh + 1; qc1 = qh; }  // no core quad
+            qc0 = max(qc0, ql);
+            qc1 = min(qc1, qh);
+            float tq = fmaf(static_cast<float>(4 * ql), step, tseg);
+            int q = ql;
+            for (; q < qc0; ++q) {
+                bwd_quad<false>(e_s[q][lane], tq, step, a);
+                tq += step4;
+            }
+            for (; q <= qc1; ++q) {
+                bwd_quad<true>(e_s[q][lane], tq, step, a);
+                tq += step4;
+            }
+            if (qc1 >= qc0) tq = fmaf(static_cast<float>(4 * q), step, tseg);   // re-anchor after the core
+            for (; q <= qh; ++q) {
+                bwd_quad<false>(e_s[q][lane], tq, step, a);
+                tq += step4;
             }
         }
-        B1 = fmaf(pk.inten, a1, B1);
-        B2 = fmaf(pk.inten, a2, B2);
-        B3 = fmaf(pk.inten, a3, B3);
-        B4 = fmaf(pk.inten, a4, B4);
-        B5 = fmaf(pk.inten, a5, B5);
-        B6 = fmaf(pk.inten, a6, B6);
+        B1 = fmaf(pk.inten, a.a1, B1);
+        B2 = fmaf(pk.inten, a.a2, B2);
+        B3 = fmaf(pk.inten, a.a3, B3);
+        B4 = fmaf(pk.inten, a.a4, B4);
+        B5 = fmaf(pk.inten, a.a5, B5);
+        B6 = fmaf(pk.inten, a.a6, B6);
     }
-    float* __restrict__ so = d.sums + (static_cast<size_t>(g) * d.n_units + unit) * 6 * 32 + lane;
-    so[0] = B1; so[32] = B2; so[64] = B3; so[96] = B4; so[128] = B5; so[160] = B6;
+    flush();
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -334,117 +574,145 @@ __device__ __forceinline__ void block_reduce(double (&v)[NV], double* smem /* [N
     __syncthreads();
 }
 
-// a-6 + a-7: chain rule, prior/Jacobian gradient, mean over the S draws.
-// grid (K, PR), block 128: threads stride over the draws of instance inst for phase k.
-constexpr int kChainThreads = 128;
-__global__ void __launch_bounds__(kChainThreads) chain_reduce_kernel(const Dev d, const float* __restrict__ var) {
-    __shared__ double red[(kChainThreads / 32) * 9];
+// a-6 (prior part) + a-7 + a-8 + next a-1/a-2.  grid (K + 1, PR), block 256.
+//  blockIdx.x = k < K : reduce the part8 slots of phase k and the per-draw prior/Jacobian terms over the S
+//                       draws of instance blockIdx.y -> grad; Adam ascent on the 8 parameters of (inst, k);
+//                       draws + transform of the next step for (inst, k, all s)          (do_update)
+//  blockIdx.x = K     : log-likelihood per draw (sum of llpart over the segments) and its mean
+//  The last CTA of an instance to finish (atomic ticket; the SUM itself has a fixed order) assembles the
+//  ELBO; the last instance bumps the step counter.
+__global__ void __launch_bounds__(kUpdThreads) update_draw_kernel(const Dev d, const float* __restrict__ var_in,
+                                                                  int do_update) {
+    __shared__ double red[(kUpdThreads / 32) * 9];
+    __shared__ float new_ml[8];
+    __shared__ double tot_s[8];
+    __shared__ unsigned int ticket_s;
     const int k = blockIdx.x, inst = blockIdx.y;
     const int pat = inst / d.R;
     const PatConst pc = d.pat[pat];
-    const float4 m = *reinterpret_cast<const float4*>(var + (static_cast<size_t>(inst) * 2 * d.K + k) * 4);
-    const float4 l = *reinterpret_cast<const float4*>(var + (static_cast<size_t>(inst) * 2 * d.K + d.K + k) * 4);
-    const float sg[4] = {expf(l.x), expf(l.y), expf(l.z), expf(l.w)};
-    const int u0 = d.unit_ofs[k], u1 = d.unit_ofs[k + 1];
-    double v[9];
-#pragma unroll
-    for (int i = 0; i < 9; ++i) v[i] = 0.0;
+    const long long step = d.ctl->step;           // completed steps; this is step + 1
+    const unsigned long long seed = d.ctl->seed;
+    const double inv_s = 1.0 / static_cast<double>(d.S);
 
-    for (int s = threadIdx.x; s < d.S; s += kChainThreads) {
-        const int g = inst * d.gpi + (s >> 5), lane = s & 31;
-        float B[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-        for (int u = u0; u < u1; ++u) {
-            const float* __restrict__ sp = d.sums + (static_cast<size_t>(g) * d.n_units + u) * 6 * 32 + lane;
-#pragma unroll
-            for (int c = 0; c < 6; ++c) B[c] += sp[c * 32];
+    if (k == d.K) {
+        double v[1] = {0.0};
+        for (int s = threadIdx.x; s < d.S; s += kUpdThreads) {
+            const int g = inst * d.gpi + (s >> 5), lane = s & 31;
+            const float* __restrict__ lp = d.llpart + static_cast<size_t>(g) * d.n_seg * 32 + lane;
+            double a = 0.0;
+            for (int t = 0; t < d.n_seg; ++t) a += static_cast<double>(lp[static_cast<size_t>(t) * 32]);
+            const double ll = -0.5 * a + pc.ll_const;
+            d.ll_t[static_cast<size_t>(inst) * d.gpi * 32 + s] = ll;
+            v[0] += ll;
         }
-        const float4 ep = d.eps[(static_cast<size_t>(g) * d.K + k) * 32 + lane];
-        const Phys q = transform(m, l, ep);
-        const float iw = 1.0f / q.w;
-        const float cLp = q.r * kAL * iw, cGp = (1.0f - q.r) * kAG * iw;
-        const float dh = cLp * B[0] + cGp * B[1];
-        const float dr = q.h * iw * (kAL * B[0] - kAG * B[1]);
-        const float dmu = q.h * iw * (4.0f * cLp * B[2] + 4.0f * kLn2 * cGp * B[3]);
-        const float dw = -q.h * iw * (cLp * (2.0f * B[4] - B[0]) + cGp * (B[1] - 2.0f * kLn2 * B[5]));
-        const float gz[4] = {fmaf(dh, q.h, 1.0f - pc.lambda_h * q.h),
-                             dmu - q.mu * d.mu_inv_var,
-                             fmaf(dw, q.w, d.w_shape - d.w_rate * q.w),
-                             fmaf(dr, q.r * (1.0f - q.r), 1.0f - 2.0f * q.r)};
-        const float az = fabsf(q.zr);
-        const float lp = (pc.log_lambda_h - pc.lambda_h * q.h + q.zh)
-                       + (-0.5f * q.mu * q.mu * d.mu_inv_var + d.mu_logc)
-                       + (d.w_logc + d.w_shape * q.zw - d.w_rate * q.w)
-                       - (az + 2.0f * log1pf(expf(-az)));
-        const float e4[4] = {ep.x, ep.y, ep.z, ep.w};
+        block_reduce<1, kUpdThreads / 32>(v, red);
+        if (threadIdx.x == 0) d.elbo_k[static_cast<size_t>(inst) * (d.K + 1) + d.K] = v[0] * inv_s;
+    } else {
+        const float4 m = *reinterpret_cast<const float4*>(var_in + (static_cast<size_t>(inst) * 2 * d.K + k) * 4);
+        const float4 l = *reinterpret_cast<const float4*>(var_in + (static_cast<size_t>(inst) * 2 * d.K + d.K + k) * 4);
+        const float4 sg = make_float4(expf(l.x), expf(l.y), expf(l.z), expf(l.w));
+        double v[9];
 #pragma unroll
-        for (int c = 0; c < 4; ++c) {
-            v[c] += static_cast<double>(gz[c]);
-            v[4 + c] += static_cast<double>(gz[c] * e4[c] * sg[c]);
+        for (int i = 0; i < 9; ++i) v[i] = 0.0;
+        // likelihood part: partials of phase k, all groups of the instance
+        const int s0 = d.slot_ofs[k], s1 = d.slot_ofs[k + 1];
+        const int n_sl = s1 - s0;
+        for (int idx = threadIdx.x; idx < n_sl * d.gpi; idx += kUpdThreads) {
+            const int gi = idx / n_sl, sl = d.slot_ids[s0 + (idx - gi * n_sl)];
+            const float4* __restrict__ pp = reinterpret_cast<const float4*>(
+                d.part8 + (static_cast<size_t>(inst * d.gpi + gi) * d.n_slots + sl) * 8);
+            const float4 a = pp[0], b = pp[1];
+            v[0] += a.x; v[1] += a.y; v[2] += a.z; v[3] += a.w;
+            v[4] += b.x; v[5] += b.y; v[6] += b.z; v[7] += b.w;
         }
-        v[8] += static_cast<double>(lp);
+        // prior + Jacobian part, per draw
+        for (int s = threadIdx.x; s < d.S; s += kUpdThreads) {
+            const int g = inst * d.gpi + (s >> 5), lane = s & 31;
+            const float4 ep = d.eps[(static_cast<size_t>(g) * d.K + k) * 32 + lane];
+            const Phys q = transform(m, sg, ep);
+            const float gz[4] = {1.0f - pc.lambda_h * q.h, -q.mu * d.mu_inv_var,
+                                 d.w_shape - d.w_rate * q.w, 1.0f - 2.0f * q.r};
+            const float az = fabsf(q.zr);
+            const float lp = (pc.log_lambda_h - pc.lambda_h * q.h + q.zh)
+                           + (-0.5f * q.mu * q.mu * d.mu_inv_var + d.mu_logc)
+                           + (d.w_logc + d.w_shape * q.zw - d.w_rate * q.w)
+                           - (az + 2.0f * log1pf(expf(-az)));
+            const float e4[4] = {ep.x, ep.y, ep.z, ep.w};
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+                v[c] += static_cast<double>(gz[c]);
+                v[4 + c] += static_cast<double>(gz[c] * e4[c]);
+            }
+            v[8] += static_cast<double>(lp);
+        }
+        block_reduce<9, kUpdThreads / 32>(v, red);
+        if (threadIdx.x == 0) {
+#pragma unroll
+            for (int i = 0; i < 8; ++i) tot_s[i] = v[i];
+        }
+        __syncthreads();
+        if (threadIdx.x < 8) {
+            const int c = threadIdx.x & 3;
+            const bool is_l = threadIdx.x >= 4;
+            const float sgc = c == 0 ? sg.x : c == 1 ? sg.y : c == 2 ? sg.z : sg.w;
+            const double tot = tot_s[threadIdx.x];
+            const double gd = is_l ? tot * inv_s * static_cast<double>(sgc) + 1.0 : tot * inv_s;
+            const float gj = static_cast<float>(gd);
+            const size_t o = (static_cast<size_t>(inst) * 2 * d.K + (is_l ? d.K : 0) + k) * 4 + c;
+            d.grad[o] = gj;
+            float x = var_in[o];
+            if (do_update) {   // Adam ascent, bias-corrected (R10); l clamped to [-12, 2]
+                const float stepf = static_cast<float>(step + 1);
+                const float bc1 = 1.0f - powf(d.beta1, stepf);
+                const float bc2 = 1.0f - powf(d.beta2, stepf);
+                const float m1 = d.beta1 * d.mom1[o] + (1.0f - d.beta1) * gj;
+                const float m2 = d.beta2 * d.mom2[o] + (1.0f - d.beta2) * gj * gj;
+                d.mom1[o] = m1;
+                d.mom2[o] = m2;
+                x += d.lr * (m1 / bc1) / (sqrtf(m2 / bc2) + d.adam_eps);
+                if (is_l) x = fminf(fmaxf(x, -12.0f), 2.0f);
+                d.var[o] = x;
+            }
+            new_ml[threadIdx.x] = x;
+        }
+        if (threadIdx.x == 0)  // mean log prior + Jacobian of the phase, plus its entropy sum_c (l_c + 1/2 ln 2 pi e)
+            d.elbo_k[static_cast<size_t>(inst) * (d.K + 1) + k] =
+                v[8] * inv_s + (static_cast<double>(l.x) + static_cast<double>(l.y) + static_cast<double>(l.z) +
+                                static_cast<double>(l.w)) + 4.0 * 1.4189385332046727;
+        if (do_update) {       // draws of the next step from the updated parameters
+            __syncthreads();
+            const float4 mn = make_float4(new_ml[0], new_ml[1], new_ml[2], new_ml[3]);
+            const float4 ln = make_float4(new_ml[4], new_ml[5], new_ml[6], new_ml[7]);
+            const unsigned it = static_cast<unsigned>(step + 2);
+            const int s_pad = d.gpi * 32;
+            for (int s = threadIdx.x; s < s_pad; s += kUpdThreads) draw_one(d, inst, k, s, it, seed, mn, ln, nullptr);
+        }
     }
-    block_reduce<9, kChainThreads / 32>(v, red);
-    if (threadIdx.x < 4) {
-        const double inv_s = 1.0 / static_cast<double>(d.S);
-        const int c = threadIdx.x;
-        d.grad[(static_cast<size_t>(inst) * 2 * d.K + k) * 4 + c] = static_cast<float>(v[c] * inv_s);
-        d.grad[(static_cast<size_t>(inst) * 2 * d.K + d.K + k) * 4 + c] = static_cast<float>(v[4 + c] * inv_s + 1.0);
-        if (c == 0) d.elbo_k[static_cast<size_t>(inst) * d.K + k] = v[8] * inv_s;
+
+    // ---- ELBO assembly by the last CTA of the instance (fixed summation order) ----
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) ticket_s = atomicAdd(&d.done_inst[inst], 1u);
+    __syncthreads();
+    if (ticket_s != static_cast<unsigned>(d.K)) return;
+    if (threadIdx.x != 0) return;
+    __threadfence();
+    d.done_inst[inst] = 0u;
+    const volatile double* ek = d.elbo_k + static_cast<size_t>(inst) * (d.K + 1);
+    double el = ek[d.K];
+    for (int kk = 0; kk < d.K; ++kk) el += ek[kk];
+    d.elbo[inst] = el;
+    if (do_update) {
+        const long long row = step - d.ctl->trace_base;
+        if (row >= 0) d.trace[static_cast<size_t>(row % kTraceCap) * d.PR + inst] = el;
+    }
+    __threadfence();
+    const unsigned int t2 = atomicAdd(&d.ctl->done_total, 1u);
+    if (t2 == static_cast<unsigned>(d.PR - 1)) {
+        d.ctl->done_total = 0u;
+        if (do_update) d.ctl->step = step + 1;
     }
 }
-
-// a-7 (ELBO) + a-8 (Adam ascent).  grid PR, block 256.
-constexpr int kFinThreads = 256;
-__global__ void __launch_bounds__(kFinThreads) finalize_update_kernel(const Dev d, const float* __restrict__ var_in,
-                                                                      int do_update) {
-    __shared__ double red[(kFinThreads / 32) * 1];
-    const int inst = blockIdx.x;
-    const int pat = inst / d.R;
-    const PatConst pc = d.pat[pat];
-    double v[1] = {0.0};
-    for (int s = threadIdx.x; s < d.S; s += kFinThreads) {
-        const int g = inst * d.gpi + (s >> 5), lane = s & 31;
-        const float* __restrict__ lp = d.llpart + static_cast<size_t>(g) * d.ntile * 32 + lane;
-        double a = 0.0;
-        for (int t = 0; t < d.ntile; ++t) a += static_cast<double>(lp[static_cast<size_t>(t) * 32]);
-        const double ll = -0.5 * a + pc.ll_const;
-        d.ll_t[static_cast<size_t>(inst) * d.gpi * 32 + s] = ll;
-        v[0] += ll;
-    }
-    block_reduce<1, kFinThreads / 32>(v, red);
-    const long long step = d.ctl->step + 1;
-    if (threadIdx.x == 0) {
-        double el = v[0] / static_cast<double>(d.S);
-        for (int k = 0; k < d.K; ++k) el += d.elbo_k[static_cast<size_t>(inst) * d.K + k];
-        const float* l = var_in + (static_cast<size_t>(inst) * 2 * d.K + d.K) * 4;
-        double ent = 0.0;
-        for (int j = 0; j < 4 * d.K; ++j) ent += static_cast<double>(l[j]) + 1.4189385332046727;  // 1/2 ln(2 pi e)
-        el += ent;
-        d.elbo[inst] = el;
-        if (do_update) {
-            const long long row = step - 1 - d.ctl->trace_base;
-            if (row >= 0) d.trace[static_cast<size_t>(row % kTraceCap) * d.PR + inst] = el;
-        }
-    }
-    if (!do_update) return;
-    __syncthreads();  // thread 0 has read l for the entropy before anyone overwrites it
-    const float bc1 = 1.0f - powf(d.beta1, static_cast<float>(step));
-    const float bc2 = 1.0f - powf(d.beta2, static_cast<float>(step));
-    const int per = 8 * d.K;
-    for (int j = threadIdx.x; j < per; j += kFinThreads) {
-        const size_t o = static_cast<size_t>(inst) * per + j;
-        const float gj = d.grad[o];
-        const float m1 = d.beta1 * d.mom1[o] + (1.0f - d.beta1) * gj;
-        const float m2 = d.beta2 * d.mom2[o] + (1.0f - d.beta2) * gj * gj;
-        d.mom1[o] = m1;
-        d.mom2[o] = m2;
-        float x = d.var[o] + d.lr * (m1 / bc1) / (sqrtf(m2 / bc2) + d.adam_eps);
-        if (j >= per / 2) x = fminf(fmaxf(x, -12.0f), 2.0f);
-        d.var[o] = x;
-    }
-}
-
-__global__ void bump_step_kernel(Ctl* ctl) { ctl->step += 1; }
 
 // a-10: inclusion probability and area ratio (R15), fp64.  grid PR, block 128.
 __global__ void __launch_bounds__(128) inclusion_kernel(const Dev d, double tau, double* __restrict__ incl,
@@ -492,6 +760,7 @@ __global__ void __launch_bounds__(128) init_state_kernel(const Dev d, const floa
         d.mom1[static_cast<size_t>(inst) * per + j] = 0.0f;
         d.mom2[static_cast<size_t>(inst) * per + j] = 0.0f;
     }
+    if (threadIdx.x == 0) d.done_inst[inst] = 0u;
 }
 
 }  // namespace xrdvi_dev

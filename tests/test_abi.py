@@ -39,12 +39,20 @@ def test_hyper_struct_mirrors_header(lib):
 
 def test_workspace_bytes(lib):
     hy = binding.default_hyper()
-    small = lib.xrdvi_workspace_bytes(1001, 6, 120, 16, C.byref(hy))
-    big = lib.xrdvi_workspace_bytes(4001, 50, 4500, 256, C.byref(hy))
+    small = lib.xrdvi_workspace_bytes(1001, 6, 120, 16, 0.07, C.byref(hy))
+    big = lib.xrdvi_workspace_bytes(4001, 50, 4500, 256, 0.02, C.byref(hy))
     assert 0 < small < big < 1 << 30
-    assert lib.xrdvi_workspace_bytes(1, 6, 120, 16, C.byref(hy)) == 0
+    # the high-throughput configs stay far below the 180 GB of one B200
+    hy3 = binding.default_hyper(n_patterns=1024)
+    assert lib.xrdvi_workspace_bytes(4001, 50, 4500, 128, 0.02, C.byref(hy3)) < 8 << 30
+    hy4 = binding.default_hyper(window_W=20.0, fwhm_ref=0.3)
+    assert lib.xrdvi_workspace_bytes(8001, 1000, 175000, 256, 0.015, C.byref(hy4)) < 8 << 30
+    dense = binding.default_hyper(window_W=0.0)
+    assert lib.xrdvi_workspace_bytes(1001, 6, 120, 16, 0.07, C.byref(dense)) > small
+    assert lib.xrdvi_workspace_bytes(1, 6, 120, 16, 0.07, C.byref(hy)) == 0
+    assert lib.xrdvi_workspace_bytes(1001, 6, 120, 16, 0.0, C.byref(hy)) == 0
     hy.size = 3
-    assert lib.xrdvi_workspace_bytes(1001, 6, 120, 16, C.byref(hy)) == 0
+    assert lib.xrdvi_workspace_bytes(1001, 6, 120, 16, 0.07, C.byref(hy)) == 0
 
 
 def test_create_rejects_bad_arguments_before_touching_cuda(lib):
