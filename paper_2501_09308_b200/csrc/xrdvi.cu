@@ -36,7 +36,7 @@ size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
 
 struct Plan {   // workspace carve; identical arithmetic in workspace_bytes and create
     int P, R, PR, S_pad, gpi_max, G_max, K;
-    int W, SP, n_seg, n_tile;
+    int TW, PS, NW, SP, n_seg, n_tile;
     long long M, n_c, bwd_cap, slots_cap;
     size_t total;
     size_t o_yb, o_bg, o_pkf, o_tile, o_pkb, o_wrng, o_sord, o_sofs, o_sids, o_pat, o_area, o_mh0;
@@ -50,18 +50,22 @@ long long window_points(const xrdvi_hyper* hyp, double step) {
     return static_cast<long long>(std::ceil(hyp->window_W * hyp->fwhm_ref / step - 1e-9));
 }
 
-// warps per CTA of elbo_tile_kernel (segment = 16 W points): as large as still gives >= 8 CTAs per SM
-int choose_seg_warps(int64_t N, int G_max) {
-    if (const char* e = std::getenv("XRDVI_SEG_WARPS")) {   // tuning knob for sweeps
-        const int w = std::atoi(e);
-        if (w == 1 || w == 2 || w == 4 || w == 8) return w;
+// CTA shape of elbo_tile_kernel: TW tiles of 16 points per segment, PS shares of each tile's peak list
+// (TW * PS warps).  Many groups: long segments, no split.  Few groups (config 1: 8): short segments and a
+// split peak list, so that the 148 SMs still see several warps per scheduler.
+void choose_shape(int64_t N, int G_max, int* TW, int* PS) {
+    if (const char* e = std::getenv("XRDVI_TILE_SHAPE")) {   // tuning knob for sweeps: "TWxPS"
+        int a = 0, b = 0;
+        if (std::sscanf(e, "%dx%d", &a, &b) == 2 && (a == 1 || a == 2 || a == 4) && (b == 1 || b == 2 || b == 4)) {
+            *TW = a; *PS = b;
+            return;
+        }
     }
-    const long long target = 148ll * 8;
-    for (int w : {4, 2}) {
-        const long long n_seg = (N + 16 * w - 1) / (16 * w);
-        if (n_seg * G_max >= target) return w;
-    }
-    return 2;
+    const long long tiles = (N + 15) / 16 * static_cast<long long>(G_max);   // warps at PS = 1
+    const long long want = 148ll * 4 * 8;                                     // 8 warps per scheduler
+    if (tiles >= want) { *TW = 4; *PS = 1; }
+    else if (2 * tiles >= want) { *TW = 2; *PS = 2; }
+    else { *TW = 2; *PS = 4; }
 }
 
 bool make_plan(int64_t N, int32_t K, int64_t M, int32_t S_max, double step, const xrdvi_hyper* hyp, Plan* pl) {
@@ -77,15 +81,16 @@ bool make_plan(int64_t N, int32_t K, int64_t M, int32_t S_max, double step, cons
     p.gpi_max = p.S_pad / 32;
     p.G_max = p.PR * p.gpi_max;
     if (p.G_max > 65535 || p.PR > 65535) return false;  // grid.y limit
-    p.W = choose_seg_warps(N, p.G_max);
-    p.SP = kPT * p.W;
+    choose_shape(N, p.G_max, &p.TW, &p.PS);
+    p.NW = p.TW * p.PS;
+    p.SP = kPT * p.TW;
     p.n_seg = static_cast<int>((N + p.SP - 1) / p.SP);
     p.n_tile = static_cast<int>((N + kPT - 1) / kPT);
     p.n_c = window_points(hyp, step);
     // entries of the per-segment phase-major lists: a peak appears once per segment its window touches
     const long long per_peak = p.n_c < 0 ? p.n_seg : std::min<long long>(p.n_seg, (2 * p.n_c + p.SP) / p.SP + 1);
     p.bwd_cap = M * per_peak;
-    p.slots_cap = std::min<long long>(static_cast<long long>(p.n_seg) * (K + p.W), p.bwd_cap + static_cast<long long>(p.n_seg) * p.W);
+    p.slots_cap = std::min<long long>(static_cast<long long>(p.n_seg) * (K + p.NW), p.bwd_cap + static_cast<long long>(p.n_seg) * p.NW);
     if (p.bwd_cap > (1ll << 31) - 1 || p.slots_cap > (1ll << 31) - 1) return false;
     size_t o = 0;
     auto take = [&](size_t bytes) { size_t r = o; o = align_up(o + bytes); return r; };
@@ -94,9 +99,9 @@ bool make_plan(int64_t N, int32_t K, int64_t M, int32_t S_max, double step, cons
     p.o_yb = take(sizeof(float) * p.P * N);
     p.o_bg = take(sizeof(float) * p.P * N);
     p.o_pkf = take(sizeof(PeakRec) * M);
-    p.o_tile = take(sizeof(int2) * p.n_tile);
+    p.o_tile = take(sizeof(int4) * p.n_tile);
     p.o_pkb = take(sizeof(PeakRec) * std::max<long long>(p.bwd_cap, 1));
-    p.o_wrng = take(sizeof(int4) * static_cast<size_t>(p.n_seg) * p.W);
+    p.o_wrng = take(sizeof(int4) * static_cast<size_t>(p.n_seg) * p.NW);
     p.o_sord = take(sizeof(int) * p.n_seg);
     p.o_sofs = take(sizeof(int) * (K + 1));
     p.o_sids = take(sizeof(int) * std::max<long long>(p.slots_cap, 1));
@@ -158,12 +163,17 @@ void set_S(xrdvi* h, int S) {
 template <bool BWD>
 void launch_tile(const Dev& d, cudaStream_t st, float* f_dbg, long long n_dbg) {
     const dim3 grid(d.n_seg, d.G);
-    switch (d.W) {
-        case 1: elbo_tile_kernel<1, BWD><<<grid, 32, 0, st>>>(d, f_dbg, n_dbg); break;
-        case 2: elbo_tile_kernel<2, BWD><<<grid, 64, 0, st>>>(d, f_dbg, n_dbg); break;
-        case 4: elbo_tile_kernel<4, BWD><<<grid, 128, 0, st>>>(d, f_dbg, n_dbg); break;
-        default: elbo_tile_kernel<8, BWD><<<grid, 256, 0, st>>>(d, f_dbg, n_dbg); break;
+#define XRDVI_TILE_CASE(TW_, PS_)                                                                           \
+    case TW_ * 8 + PS_:                                                                                    \
+        elbo_tile_kernel<TW_, PS_, BWD><<<grid, 32 * TW_ * PS_, 0, st>>>(d, f_dbg, n_dbg);                 \
+        break;
+    switch (d.TW * 8 + d.PS) {
+        XRDVI_TILE_CASE(1, 1) XRDVI_TILE_CASE(1, 2) XRDVI_TILE_CASE(1, 4)
+        XRDVI_TILE_CASE(2, 1) XRDVI_TILE_CASE(2, 2) XRDVI_TILE_CASE(2, 4)
+        XRDVI_TILE_CASE(4, 1) XRDVI_TILE_CASE(4, 2) XRDVI_TILE_CASE(4, 4)
+        default: break;
     }
+#undef XRDVI_TILE_CASE
 }
 
 void launch_draw(const Dev& d, cudaStream_t st, const float* var, uint4* raw_out) {
@@ -318,7 +328,7 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
     if (reinterpret_cast<uintptr_t>(workspace) % 256) return fail(XRDVI_E_INVALID_ARG, "workspace not 256-byte aligned");
 
     // ---- fp64 preprocessing (R16) ----------------------------------------------------------------
-    const int P = pl.P, W = pl.W, SP = pl.SP;
+    const int P = pl.P, W = pl.NW, SP = pl.SP;
     long long n_c = pl.n_c;
     if (n_c < 0) {     // dense: every point is inside every window, wherever the peak lies
         n_c = N;
@@ -362,10 +372,14 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
         auto b = std::upper_bound(fw.begin(), fw.end(), jhi, [](long long v, const HP& p) { return v < p.j; });
         return make_int2(static_cast<int>(a - fw.begin()), static_cast<int>(b - fw.begin()));
     };
-    std::vector<int2> tile_rng(pl.n_tile);
+    std::vector<int4> tile_rng(pl.n_tile);
     for (int t = 0; t < pl.n_tile; ++t) {
-        const long long i0 = static_cast<long long>(t) * kPT;
-        tile_rng[t] = j_range(i0 - n_c, std::min<long long>(i0 + kPT - 1, N - 1) + n_c);
+        const long long i0 = static_cast<long long>(t) * kPT, i1 = i0 + kPT - 1;
+        const int2 all = j_range(i0 - n_c, std::min<long long>(i1, N - 1) + n_c);   // window reaches a tile point < N
+        int2 full = j_range(i1 - n_c, i0 + n_c);                                   // window covers all 16 points
+        full.x = std::min(std::max(full.x, all.x), all.y);
+        full.y = std::min(std::max(full.y, full.x), all.y);
+        tile_rng[t] = make_int4(all.x, full.x, full.y, all.y);
     }
 
     // phase-2 tables: per segment, the peaks whose window reaches it, phase-major; W contiguous warp
@@ -465,7 +479,7 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
     Dev& d = h->dev;
     char* w = h->ws;
     d.N = static_cast<int>(N); d.K = K; d.P = pl.P; d.R = pl.R; d.PR = pl.PR;
-    d.n_c = static_cast<int>(n_c); d.SP = SP; d.W = W; d.n_seg = pl.n_seg; d.n_tile = pl.n_tile;
+    d.n_c = static_cast<int>(n_c); d.SP = SP; d.TW = pl.TW; d.PS = pl.PS; d.n_seg = pl.n_seg; d.n_tile = pl.n_tile;
     d.n_slots = std::max(n_slots, 1); d.Mv = Mv;
     d.delta = static_cast<float>(delta);
     d.gcut = static_cast<float>(static_cast<double>(kGaussCut) / (2.0 * delta));
@@ -480,7 +494,7 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
     d.yb = reinterpret_cast<float*>(w + pl.o_yb);
     d.bg = reinterpret_cast<float*>(w + pl.o_bg);
     d.pk_fwd = reinterpret_cast<PeakRec*>(w + pl.o_pkf);
-    d.tile_rng = reinterpret_cast<int2*>(w + pl.o_tile);
+    d.tile_rng = reinterpret_cast<int4*>(w + pl.o_tile);
     d.pk_bwd = reinterpret_cast<PeakRec*>(w + pl.o_pkb);
     d.warp_rng = reinterpret_cast<int4*>(w + pl.o_wrng);
     d.seg_order = reinterpret_cast<int*>(w + pl.o_sord);
@@ -515,7 +529,7 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
     chk(up(pl.o_yb, yb.data(), sizeof(float) * yb.size()));
     chk(up(pl.o_bg, bgf.data(), sizeof(float) * bgf.size()));
     chk(up(pl.o_pkf, pk_fwd.data(), sizeof(PeakRec) * pk_fwd.size()));
-    chk(up(pl.o_tile, tile_rng.data(), sizeof(int2) * tile_rng.size()));
+    chk(up(pl.o_tile, tile_rng.data(), sizeof(int4) * tile_rng.size()));
     chk(up(pl.o_pkb, pk_bwd.data(), sizeof(PeakRec) * pk_bwd.size()));
     chk(up(pl.o_wrng, warp_rng.data(), sizeof(int4) * warp_rng.size()));
     chk(up(pl.o_sord, seg_order.data(), sizeof(int) * seg_order.size()));

@@ -69,7 +69,7 @@ struct Ctl {       // device-resident control block (so that graph replays need 
 
 struct Dev {
     // sizes
-    int N, K, P, R, PR, n_c, SP, n_seg, n_tile, n_slots, Mv, W;
+    int N, K, P, R, PR, n_c, SP, n_seg, n_tile, n_slots, Mv, TW, PS;
     int S, gpi, G;       // draws, groups per instance, groups (run-time)
     float delta;         // grid step (deg)
     float gcut;          // kGaussCut / (2 Delta): core half-width in points per unit of w
@@ -81,9 +81,10 @@ struct Dev {
     const float* yb;          // [P][N]  y - B
     const float* bg;          // [P][N]
     const PeakRec* pk_fwd;    // [Mv] sorted by j
-    const int2* tile_rng;     // [n_tile] peak range [x,y) in pk_fwd of each 16-point tile
+    const int4* tile_rng;     // [n_tile] peak ranges in pk_fwd of each 16-point tile: [x,w) reaches the tile,
+                              //          [y,z) covers all 16 points with its window
     const PeakRec* pk_bwd;    // per-segment phase-major peak lists, concatenated
-    const int4* warp_rng;     // [n_seg][W]: (m0, m1) range in pk_bwd of the warp, .z = its first slot
+    const int4* warp_rng;     // [n_seg][TW*PS]: (m0, m1) range in pk_bwd of the warp, .z = its first slot
     const int* seg_order;     // [n_seg] segments by decreasing work (LPT dispatch order)
     const int* slot_ofs;      // [K+1] CSR: slots of phase k
     const int* slot_ids;      // [n_slots]
@@ -232,19 +233,55 @@ __device__ __forceinline__ void fwd_pair(float ta, float tb, float cg, float cl,
     }
 }
 
-// One quad (4 points, first point index p0 of the tile) with per-point window masks.
-template <bool CORE>
-__device__ __forceinline__ void fwd_quad_masked(float t0, float step, int p0, int p_lo, int p_hi, float cg, float cl,
-                                                float& a0, float& a1, float& a2, float& a3) {
-    float v[4] = {0.f, 0.f, 0.f, 0.f};
-    const float ta = fmaf(static_cast<float>(p0), step, t0), tb = fmaf(static_cast<float>(p0 + 1), step, t0);
-    const float tc = fmaf(static_cast<float>(p0 + 2), step, t0), td = fmaf(static_cast<float>(p0 + 3), step, t0);
-    fwd_pair<CORE>(ta, tb, cg, cl, v[0], v[1]);
-    fwd_pair<CORE>(tc, td, cg, cl, v[2], v[3]);
-    a0 += (p0 + 0 >= p_lo && p0 + 0 <= p_hi) ? v[0] : 0.0f;
-    a1 += (p0 + 1 >= p_lo && p0 + 1 <= p_hi) ? v[1] : 0.0f;
-    a2 += (p0 + 2 >= p_lo && p0 + 2 <= p_hi) ? v[2] : 0.0f;
-    a3 += (p0 + 3 >= p_lo && p0 + 3 <= p_hi) ? v[3] : 0.0f;
+// One peak on the 16 points of a tile.  MASK: only points p_lo <= p <= p_hi are inside the peak's window.
+template <bool CORE, bool MASK>
+__device__ __forceinline__ void fwd_tile(float t0, float step, float cg, float cl, int p_lo, int p_hi, float (&acc)[kPT]) {
+    const unsigned span = static_cast<unsigned>(p_hi - p_lo);
+#pragma unroll
+    for (int p = 0; p < kPT; p += 2) {
+        const float ta = fmaf(static_cast<float>(p), step, t0);
+        const float tb = fmaf(static_cast<float>(p + 1), step, t0);
+        if (MASK) {
+            float va = 0.0f, vb = 0.0f;
+            fwd_pair<CORE>(ta, tb, cg, cl, va, vb);
+            acc[p] += (static_cast<unsigned>(p - p_lo) <= span) ? va : 0.0f;
+            acc[p + 1] += (static_cast<unsigned>(p + 1 - p_lo) <= span) ? vb : 0.0f;
+        } else {
+            fwd_pair<CORE>(ta, tb, cg, cl, acc[p], acc[p + 1]);
+        }
+    }
+}
+
+// Loop of phase 1 over the peaks [m0, m1) of pk_fwd for the tile starting at grid point i0.
+template <bool MASK>
+__device__ __forceinline__ void fwd_peaks(const Dev& d, const float4* __restrict__ lat, const int* __restrict__ ngk,
+                                          int m0, int m1, int i0, float (&acc)[kPT]) {
+    if (m0 >= m1) return;
+    const int n_c = d.n_c;
+    PeakRec pk_n = d.pk_fwd[m0];
+    float4 lt_n = lat[static_cast<size_t>(pk_n.k) * 32];
+    int ng_n = ngk[pk_n.k];
+    for (int m = m0; m < m1; ++m) {
+        const PeakRec pk = pk_n;
+        const float4 lt = lt_n;
+        const int ngc = ng_n;
+        if (m + 1 < m1) {  // prefetch the next peak and its latents
+            pk_n = d.pk_fwd[m + 1];
+            lt_n = lat[static_cast<size_t>(pk_n.k) * 32];
+            ng_n = ngk[pk_n.k];
+        }
+        const float step = d.delta * lt.x;
+        const float tc = fmaf(-pk.delta, lt.x, lt.y);
+        const int dj = pk.j - i0;                         // peak centre in tile coordinates
+        const float t0 = fmaf(static_cast<float>(-dj), step, tc);
+        const float cl = pk.inten * lt.w;
+        const int p_lo = dj - n_c, p_hi = dj + n_c;       // in-window points of the tile: p_lo <= p <= p_hi
+        // Gaussian core |p - dj| <= n_g touches the tile?  (warp-uniform)
+        if (static_cast<unsigned>(dj + ngc) <= static_cast<unsigned>(kPT - 1 + 2 * ngc))
+            fwd_tile<true, MASK>(t0, step, pk.inten * lt.z, cl, p_lo, p_hi, acc);
+        else
+            fwd_tile<false, MASK>(t0, step, 0.0f, cl, p_lo, p_hi, acc);
+    }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -318,95 +355,59 @@ __device__ __forceinline__ float warp_reduce8(float (&v)[8]) {
 
 // ------------------------------------------------------------------------------------------------
 // a-3 .. a-6 (likelihood part): fused profile + residual + backward.
-// grid (n_seg, G), block 32*W; segment = 16*W consecutive grid points; warp w owns tile 16*w.. in phase 1
-// and the peak range warp_rng[seg][w] of the segment's phase-major list in phase 2.
-template <int W, bool BWD>
-__global__ void __launch_bounds__(32 * W) elbo_tile_kernel(const Dev d, float* __restrict__ f_dbg, long long n_dbg) {
-    __shared__ float4 e_s[4 * W][32];
-    __shared__ float ss_s[W][32];
+// grid (n_seg, G), block 32*TW*PS; segment = 16*TW consecutive grid points.  Phase 1: warp w owns tile
+// (w % TW) of the segment and share (w / TW) of the PS equal shares of that tile's peak list; the PS partial
+// profiles are summed through shared memory in a fixed order.  Phase 2: warp w owns the peak range
+// warp_rng[seg][w] of the segment's phase-major list.
+template <int TW, int PS, bool BWD>
+__global__ void __launch_bounds__(32 * TW * PS) elbo_tile_kernel(const Dev d, float* __restrict__ f_dbg, long long n_dbg) {
+    constexpr int NW = TW * PS;
+    __shared__ float4 e_s[4 * TW][32];
+    __shared__ float ss_s[TW][32];
+    __shared__ float acc_s[PS > 1 ? (PS - 1) * TW * kPT : 1][32];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int tw = w % TW, ps = w / TW;
     const int seg = d.seg_order[blockIdx.x];
     const int g = blockIdx.y;
-    const int seg0 = seg * (kPT * W);
-    const int i0 = seg0 + kPT * w;
+    const int seg0 = seg * (kPT * TW);
+    const int i0 = seg0 + kPT * tw;
     const float4* __restrict__ lat = d.lat + static_cast<size_t>(g) * d.K * 32 + lane;
     const int* __restrict__ ngk = d.ng + static_cast<size_t>(g) * d.K;
     const int inst = g / d.gpi;
     const int pat = inst / d.R;
     const PatConst pc = d.pat[pat];
 
-    // ---------------- phase 1: profile on the 16 points of this warp ----------------
+    // ---------------- phase 1: profile on the 16 points of this warp's tile ----------------
     float acc[kPT];
 #pragma unroll
     for (int p = 0; p < kPT; ++p) acc[p] = 0.0f;
 
     if (i0 < d.N) {
-        const int2 rng = d.tile_rng[i0 / kPT];
-        const int n_c = d.n_c;
-        PeakRec pk_n;
-        float4 lt_n;
-        int ng_n = 0;
-        if (rng.x < rng.y) {
-            pk_n = d.pk_fwd[rng.x];
-            lt_n = lat[static_cast<size_t>(pk_n.k) * 32];
-            ng_n = ngk[pk_n.k];
+        // tile_rng = (lo, full_lo, full_hi, hi): [lo, full_lo) and [full_hi, hi) reach only part of the tile
+        const int4 rng = d.tile_rng[i0 / kPT];
+        const int n = rng.w - rng.x;
+        const int a = rng.x + static_cast<int>(static_cast<long long>(n) * ps / PS);
+        const int b = rng.x + static_cast<int>(static_cast<long long>(n) * (ps + 1) / PS);
+        fwd_peaks<true>(d, lat, ngk, a, min(b, rng.y), i0, acc);
+        fwd_peaks<false>(d, lat, ngk, max(a, rng.y), min(b, rng.z), i0, acc);
+        fwd_peaks<true>(d, lat, ngk, max(a, rng.z), b, i0, acc);
+    }
+    if (PS > 1) {   // sum the PS partial profiles of the tile: shares 1.. in order onto share 0
+        if (ps > 0) {
+#pragma unroll
+            for (int p = 0; p < kPT; ++p) acc_s[((ps - 1) * TW + tw) * kPT + p][lane] = acc[p];
         }
-        for (int m = rng.x; m < rng.y; ++m) {
-            const PeakRec pk = pk_n;
-            const float4 lt = lt_n;
-            const int ngc = ng_n;
-            if (m + 1 < rng.y) {  // prefetch the next peak and its latents
-                pk_n = d.pk_fwd[m + 1];
-                lt_n = lat[static_cast<size_t>(pk_n.k) * 32];
-                ng_n = ngk[pk_n.k];
-            }
-            const float step = d.delta * lt.x;
-            const float tc = fmaf(-pk.delta, lt.x, lt.y);
-            const int dj = pk.j - i0;                         // peak centre in tile coordinates
-            const float t0 = fmaf(static_cast<float>(-dj), step, tc);
-            const float cl = pk.inten * lt.w;
-            const int p_lo = dj - n_c, p_hi = dj + n_c;       // in-window points of the tile: p_lo <= p <= p_hi
-            const bool full = (p_lo <= 0) && (p_hi >= kPT - 1);
-            const bool core_any = (dj + ngc >= 0) && (dj - ngc <= kPT - 1);
-            if (full && !core_any) {  // whole tile inside the window and on the Lorentz tail (warp-uniform)
+        __syncthreads();
+        if (ps == 0) {
 #pragma unroll
-                for (int p = 0; p < kPT; p += 2) {
-                    const float ta = fmaf(static_cast<float>(p), step, t0);
-                    const float tb = fmaf(static_cast<float>(p + 1), step, t0);
-                    fwd_pair<false>(ta, tb, 0.0f, cl, acc[p], acc[p + 1]);
-                }
-            } else {
-                const float cg = pk.inten * lt.z;
+            for (int q = 1; q < PS; ++q)
 #pragma unroll
-                for (int q = 0; q < kPT / 4; ++q) {
-                    const int qlo = 4 * q, qhi = 4 * q + 3;
-                    if (qhi < p_lo || qlo > p_hi) continue;                 // quad outside the window
-                    const bool qfull = (qlo >= p_lo) && (qhi <= p_hi);
-                    const bool qcore = (dj + ngc >= qlo) && (dj - ngc <= qhi);
-                    if (qfull) {
-                        const float ta = fmaf(static_cast<float>(qlo), step, t0);
-                        const float tb = fmaf(static_cast<float>(qlo + 1), step, t0);
-                        const float tcq = fmaf(static_cast<float>(qlo + 2), step, t0);
-                        const float td = fmaf(static_cast<float>(qlo + 3), step, t0);
-                        if (qcore) {
-                            fwd_pair<true>(ta, tb, cg, cl, acc[qlo], acc[qlo + 1]);
-                            fwd_pair<true>(tcq, td, cg, cl, acc[qlo + 2], acc[qlo + 3]);
-                        } else {
-                            fwd_pair<false>(ta, tb, cg, cl, acc[qlo], acc[qlo + 1]);
-                            fwd_pair<false>(tcq, td, cg, cl, acc[qlo + 2], acc[qlo + 3]);
-                        }
-                    } else if (qcore) {
-                        fwd_quad_masked<true>(t0, step, qlo, p_lo, p_hi, cg, cl, acc[qlo], acc[qlo + 1], acc[qlo + 2], acc[qlo + 3]);
-                    } else {
-                        fwd_quad_masked<false>(t0, step, qlo, p_lo, p_hi, cg, cl, acc[qlo], acc[qlo + 1], acc[qlo + 2], acc[qlo + 3]);
-                    }
-                }
-            }
+                for (int p = 0; p < kPT; ++p) acc[p] += acc_s[((q - 1) * TW + tw) * kPT + p][lane];
         }
     }
 
     // residual, e = (y - f)/sigma_n^2, partial sum of ((y - f)/sigma_n)^2
-    {
+    if (ps == 0) {
         const float* __restrict__ yb = d.yb + static_cast<size_t>(pat) * d.N;
         float ev[kPT];
         float ss = 0.0f;
@@ -422,33 +423,33 @@ __global__ void __launch_bounds__(32 * W) elbo_tile_kernel(const Dev d, float* _
         if (BWD) {
 #pragma unroll
             for (int v = 0; v < kPT / 4; ++v)
-                e_s[4 * w + v][lane] = make_float4(ev[4 * v], ev[4 * v + 1], ev[4 * v + 2], ev[4 * v + 3]);
+                e_s[4 * tw + v][lane] = make_float4(ev[4 * v], ev[4 * v + 1], ev[4 * v + 2], ev[4 * v + 3]);
         }
-        ss_s[w][lane] = ss;
-    }
-    if (f_dbg && i0 < d.N) {  // debug read-back of the profile (parity tests); warp-uniform branch
-        const int s = (g - inst * d.gpi) * 32 + lane;
-        const long long t = static_cast<long long>(inst) * d.S + s;
-        if (s < d.S && t < n_dbg) {
-            const float* __restrict__ bg = d.bg + static_cast<size_t>(pat) * d.N;
+        ss_s[tw][lane] = ss;
+        if (f_dbg && i0 < d.N) {  // debug read-back of the profile (parity tests); warp-uniform branch
+            const int s = (g - inst * d.gpi) * 32 + lane;
+            const long long t = static_cast<long long>(inst) * d.S + s;
+            if (s < d.S && t < n_dbg) {
+                const float* __restrict__ bg = d.bg + static_cast<size_t>(pat) * d.N;
 #pragma unroll
-            for (int p = 0; p < kPT; ++p)
-                if (i0 + p < d.N) f_dbg[t * d.N + i0 + p] = acc[p] + bg[i0 + p];
+                for (int p = 0; p < kPT; ++p)
+                    if (i0 + p < d.N) f_dbg[t * d.N + i0 + p] = acc[p] + bg[i0 + p];
+            }
         }
     }
     __syncthreads();
-    if (w == 0) {  // fixed-order sum over the warps of the segment
+    if (w == 0) {  // fixed-order sum over the tiles of the segment
         float ss = ss_s[0][lane];
 #pragma unroll
-        for (int v = 1; v < W; ++v) ss += ss_s[v][lane];
+        for (int v = 1; v < TW; ++v) ss += ss_s[v][lane];
         d.llpart[(static_cast<size_t>(g) * d.n_seg + seg) * 32 + lane] = ss;
     }
     if (!BWD) return;
 
     // ---------------- phase 2: six sums over the segment, chain rule, reduction over the draws ----------------
-    const int4 wr = d.warp_rng[seg * W + w];
+    const int4 wr = d.warp_rng[seg * NW + w];
     if (wr.x >= wr.y) return;
-    const int seg_hi = min(seg0 + kPT * W - 1, d.N - 1);
+    const int seg_hi = min(seg0 + kPT * TW - 1, d.N - 1);
     const float4* __restrict__ epsg = d.eps + static_cast<size_t>(g) * d.K * 32 + lane;
     const float* __restrict__ rrg = d.rr + static_cast<size_t>(g) * d.K * 32 + lane;
     float* __restrict__ part = d.part8 + static_cast<size_t>(g) * d.n_slots * 8;
