@@ -1,0 +1,117 @@
+"""Brute force over all 2^K phase combinations at tiny K, against the variational inclusion
+probabilities of the fp64 oracle (BASELINE.json north_star; SURVEY.md 8(c) "Pins": inclusion).
+
+The discrete problem the paper replaces (2^K indicator combinations) is enumerated
+exactly for K = 6: for every subset gamma the nuisances (mu, w, r) are fixed at the fitted variational
+means and the evidence is integrated EXACTLY over the scales h_gamma >= 0:
+
+    Z_gamma = int_{h >= 0} prod_k lambda e^{-lambda h_k} N(y; B + C_gamma^T h, sigma_n^2) dh
+            = c_0 lambda^{|g|} (2 pi)^{|g|/2} |Lam|^{-1/2} exp(b^T Lam^{-1} b / 2) Pr[N(Lam^{-1} b, Lam^{-1}) >= 0]
+
+with Lam = C C^T / sigma_n^2, b = C (y - B) / sigma_n^2 - lambda 1 (completing the square; c_0 is common to
+all subsets), the orthant probability from scipy's multivariate-normal cdf (Genz).  Uniform prior over
+subsets.  This is independent of the variational machinery (no q, no ELBO, no Adam): it only uses the
+oracle's per-phase unit profile, which test_oracle_pins.py pins against scipy pdfs.
+
+Criterion: the maximum-evidence subset equals {k : P_incl(k) > 1/2} and equals the planted
+set; every phase falls on the same side of 1/2 under both; max |difference| is reported.  The Occam factor
+makes exact inclusion of absent phases small but not zero (SURVEY probe: 0.004-0.14).
+"""
+import itertools
+import math
+
+import numpy as np
+import pytest
+import scipy.stats
+
+from oracle import xrdvi_oracle as orc
+from paper_2501_09308_b200 import synth
+
+
+def unit_profiles(o, zeta):
+    """C_k(x_i): windowed profile of phase k alone at h_k = 1 and the nuisances of `zeta` (via the oracle's
+    profile function and its linearity in h, which is pinned separately)."""
+    C = np.empty((o.K, o.N))
+    for k in range(o.K):
+        z = zeta.copy()
+        z[:, 0] = -745.0            # exp(-745) = 5e-324: the other phases contribute nothing
+        z[k, 0] = 0.0
+        C[k] = o.profile(z) - o.B[0]
+    return C
+
+
+def log_evidence(C, resid, sigma_n, lam):
+    g = C.shape[0]
+    if g == 0:
+        return 0.0
+    Lam = C @ C.T / sigma_n ** 2
+    b = C @ resid / sigma_n ** 2 - lam
+    cov = np.linalg.inv(Lam)
+    cov = 0.5 * (cov + cov.T)
+    hhat = cov @ b
+    sign, logdet = np.linalg.slogdet(Lam)
+    assert sign > 0
+    if g == 1:
+        orth = scipy.stats.norm.sf(0.0, loc=hhat[0], scale=math.sqrt(cov[0, 0]))
+    else:
+        # Pr[X >= 0] = Pr[-X <= 0]
+        orth = scipy.stats.multivariate_normal.cdf(np.zeros(g), mean=-hhat, cov=cov, maxpts=200000 * g,
+                                                   abseps=1e-10, releps=1e-10)
+    return g * math.log(lam) + 0.5 * g * math.log(2 * math.pi) - 0.5 * logdet + 0.5 * b @ hhat + math.log(max(orth, 1e-300))
+
+
+@pytest.mark.parametrize("seed", [1000, 2024])
+def test_variational_inclusion_against_all_64_subsets(seed):
+    wl = synth.make_workload(0, seed=seed)
+    o = orc.from_workload(wl)
+    assert o.K == 6
+    st, _, _ = o.fit(o.init_state(), 500, wl.S, seed=11)
+    inc_vi, area = o.inclusion(st, want_area=True)
+    inc_vi, area = inc_vi[0, 0], area[0, 0]
+
+    zeta = st[0, 0, 0].copy()                       # variational means: nuisances fixed there
+    C = unit_profiles(o, zeta)
+    resid = o.y[0] - o.B[0]
+    sig, lam = o.sigma_n(), o.lambda_h()
+
+    subsets, logZ = [], []
+    for n in range(o.K + 1):
+        for g in itertools.combinations(range(o.K), n):
+            subsets.append(g)
+            logZ.append(log_evidence(C[list(g)], resid, sig, lam))
+    logZ = np.array(logZ)
+    post = np.exp(logZ - logZ.max())
+    post /= post.sum()
+    inc_bf = np.array([sum(p for g, p in zip(subsets, post) if k in g) for k in range(o.K)])
+
+    truth = tuple(sorted(wl.true_phases[0]))
+    best = subsets[int(np.argmax(post))]
+    assert best == truth                                              # exact posterior mode = planted set
+    # variational read-out (area-ratio form, robust to the 1 % threshold on a coarse grid): same set
+    vi_set = tuple(k for k in range(o.K) if area[k] > 0.03)
+    assert vi_set == truth
+    for k in range(o.K):
+        assert (inc_bf[k] > 0.5) == (k in truth)
+        if k in truth:
+            assert inc_vi[k] > 0.99 and inc_bf[k] > 0.99
+    # true phases: both say "certainly in"; absent phases: exact inclusion is small (Occam), bounded
+    absent = [k for k in range(o.K) if k not in truth]
+    assert inc_bf[absent].max() < 0.35
+    print("max |P_bf - P_vi| over true phases", np.abs(inc_bf - inc_vi)[list(truth)].max(),
+          "exact inclusion of absent phases", inc_bf[absent], "variational", inc_vi[absent])
+
+
+def test_subset_evidence_one_dimensional_closed_form():
+    """The building block against direct quadrature in one dimension (a plausible sign / factor slip in the
+    completed square fails here)."""
+    rng = np.random.default_rng(3)
+    N = 60
+    c = np.abs(rng.normal(0, 1, N))
+    sigma_n, lam = 0.7, 1.3
+    y = 0.8 * c + rng.normal(0, sigma_n, N)
+    import scipy.integrate
+    f = lambda h: lam * math.exp(-lam * h) * math.exp(-0.5 * ((y - c * h) ** 2).sum() / sigma_n ** 2
+                                                       + 0.5 * (y ** 2).sum() / sigma_n ** 2)
+    ref, _ = scipy.integrate.quad(f, 0, 10, epsabs=0, epsrel=1e-11, limit=400)
+    got = math.exp(log_evidence(c[None, :], y, sigma_n, lam))
+    assert got == pytest.approx(ref, rel=1e-8)
