@@ -124,7 +124,7 @@ def run_reference(args, rank: int) -> None:
 
 def run_ours(args, rank: int, local_rank: int, world: int) -> None:
     import torch
-    from paper_2501_09308_b200 import Xrdvi, synth
+    from paper_2501_09308_b200 import Xrdvi, replicas, synth
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (the hot path has no CPU fallback)")
@@ -139,10 +139,11 @@ def run_ours(args, rank: int, local_rank: int, world: int) -> None:
     # shards over independent (pattern, restart) instances with no data-path collective.
     wl = synth.make_workload(args.config)
     gpu = Xrdvi.from_workload(wl, device=local_rank)
-    gpu.reset_state(seed=rank)
+    seeds = replicas.replica_seeds(rank)
+    gpu.reset_state(seed=seeds["state_seed"])
     S, T = wl.S, wl.P * wl.R * wl.S
     pairs = gpu.pair_count
-    gpu.bench_steps(max(args.warmup, 1), S=S, seed=1 + rank, l2_flush_bytes=L2_FLUSH_BYTES)
+    gpu.bench_steps(max(args.warmup, 1), S=S, seed=seeds["draw_seed"], l2_flush_bytes=L2_FLUSH_BYTES)
 
     def barrier():
         torch.cuda.synchronize()
@@ -152,15 +153,11 @@ def run_ours(args, rank: int, local_rank: int, world: int) -> None:
 
     barrier()
     sampler = ClockSampler(local_rank) if rank == 0 else None
-    ms = gpu.bench_steps(args.steps, S=S, seed=1 + rank, l2_flush_bytes=L2_FLUSH_BYTES)
+    ms = gpu.bench_steps(args.steps, S=S, seed=seeds["draw_seed"], l2_flush_bytes=L2_FLUSH_BYTES)
     barrier()
-    t_ms = float(ms.astype(np.float64).sum())
-    if dist is not None:
-        tt = torch.tensor([t_ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        t_ms = float(tt.item())
+    t_ms = replicas.max_over_ranks(float(ms.astype(np.float64).sum()), dist, "cuda")
     # per-kernel device times, measured live on the launching stream (CUDA events inside the library)
-    tk = gpu.time_kernels(S=S, seed=1 + rank, reps=30)
+    tk = gpu.time_kernels(S=S, seed=seeds["draw_seed"], reps=30)
     clocks = sampler.stop() if sampler else None
 
     # end to end through the C ABI with HOST buffers: create (H2D of the pattern and peak tables) +
@@ -168,13 +165,9 @@ def run_ours(args, rank: int, local_rank: int, world: int) -> None:
     barrier()
     t0 = time.perf_counter()
     gpu2 = Xrdvi.from_workload(wl, device=local_rank)
-    gpu2.reset_state(seed=rank)
-    st, inc, _ = gpu2.fit(args.steps, S=S, seed=1 + rank)
-    e2e_s = time.perf_counter() - t0
-    if dist is not None:
-        tt = torch.tensor([e2e_s], device="cuda", dtype=torch.float64)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        e2e_s = float(tt.item())
+    gpu2.reset_state(seed=seeds["state_seed"])
+    st, inc, _ = gpu2.fit(args.steps, S=S, seed=seeds["draw_seed"])
+    e2e_s = replicas.max_over_ranks(time.perf_counter() - t0, dist, "cuda")
     h2d = 8 * (wl.two_theta.size + wl.y.size + wl.background.size + wl.peak_pos.size + wl.peak_int.size
                + wl.peak_ofs.size)
     d2h = st.nbytes + inc.nbytes
@@ -185,7 +178,7 @@ def run_ours(args, rank: int, local_rank: int, world: int) -> None:
             dist.destroy_process_group()
         return
 
-    value = pairs * T * args.steps * world / (t_ms * 1e-3)
+    value = replicas.whole_job_rate(pairs * T * args.steps, world, t_ms * 1e-3)
     props = torch.cuda.get_device_properties(local_rank)
     n_sm = props.multi_processor_count
     peaks = measured_peaks()
@@ -233,7 +226,7 @@ def run_ours(args, rank: int, local_rank: int, world: int) -> None:
                    "l2": f"flushed between timed steps ({L2_FLUSH_BYTES >> 20} MiB memset outside the event brackets)",
                    "parallelism": f"replicas x{world} (independent restarts, no collective)"},
         "fit_wall_s": e2e_s, "fit_iterations": args.steps,
-        "e2e": {"value": pairs * T * args.steps * world / e2e_s, "unit": UNIT,
+        "e2e": {"value": replicas.whole_job_rate(pairs * T * args.steps, world, e2e_s), "unit": UNIT,
                 "h2d_bytes_per_step": h2d / args.steps, "d2h_bytes_per_step": d2h / args.steps,
                 "covers": "xrdvi_create (host fp64 preprocessing + H2D) + xrdvi_fit + D2H of parameters and "
                           "inclusion probabilities; inputs are uploaded once per fit"},

@@ -302,19 +302,23 @@ void orc_logjoint_grad(const orc_problem *q, int32_t pat, const double *zeta, do
 /* ------------------------------------------------------------------ ELBO and its gradient */
 /* state [P][R][2][K][4]; elbo [P][R]; grad [P][R][2][K][4]; optional per-instance outputs:
  * ll_out [P][R][S], f_out [n_f][N] = profiles of the first n_f sample-instances (pat,rst,s order) */
-void orc_elbo_grad(const orc_problem *q, const double *state, int32_t S, uint64_t seed,
-                   uint64_t iteration, double *elbo, double *grad, double *ll_out, double *f_out,
-                   int64_t n_f) {
-    const int32_t K = q->K, P = q->P, R = q->R;
+/* Instances [inst0, inst0 + n_inst) only (a SELECTION of which (pattern, restart) pairs are evaluated; the
+ * arithmetic per instance is unchanged and the Philox counter keeps the global instance index).  state is the
+ * full [P][R][2][K][4] array; elbo [n_inst], grad [n_inst][2][K][4], ll_out [n_inst][S], f_out: the first n_f
+ * draws of the selection. */
+void orc_elbo_grad_range(const orc_problem *q, const double *state, int32_t S, uint64_t seed,
+                         uint64_t iteration, int32_t inst0, int32_t n_inst, double *elbo, double *grad,
+                         double *ll_out, double *f_out, int64_t n_f) {
+    const int32_t K = q->K, R = q->R;
     const int64_t N = q->N;
-    const int64_t T = (int64_t)P * R * S;
+    const int64_t T = (int64_t)n_inst * S;
     double *gz_all = (double *)malloc(sizeof(double) * (size_t)T * K * 4);
     double *eps_all = (double *)malloc(sizeof(double) * (size_t)T * K * 4);
     double *lj_all = (double *)malloc(sizeof(double) * (size_t)T * 2);
 #pragma omp parallel for schedule(dynamic, 1)
     for (int64_t t = 0; t < T; ++t) {
         int32_t s = (int32_t)(t % S);
-        int32_t inst = (int32_t)(t / S);          /* inst = pat*R + rst */
+        int32_t inst = inst0 + (int32_t)(t / S);  /* inst = pat*R + rst */
         int32_t pat = inst / R;
         const double *m = state + (size_t)inst * 2 * K * 4, *l = m + (size_t)K * 4;
         double *zeta = (double *)malloc(sizeof(double) * K * 4);
@@ -328,13 +332,14 @@ void orc_elbo_grad(const orc_problem *q, const double *state, int32_t S, uint64_
         if (ll_out) ll_out[t] = lj_all[2 * t];
         free(zeta);
     }
-    for (int32_t inst = 0; inst < P * R; ++inst) {
+    for (int32_t li = 0; li < n_inst; ++li) {
+        const int32_t inst = inst0 + li;
         const double *l = state + (size_t)inst * 2 * K * 4 + (size_t)K * 4;
-        double *gm = grad + (size_t)inst * 2 * K * 4, *gl = gm + (size_t)K * 4;
+        double *gm = grad + (size_t)li * 2 * K * 4, *gl = gm + (size_t)K * 4;
         double acc = 0.0;
         for (int j = 0; j < 4 * K; ++j) { gm[j] = 0.0; gl[j] = 0.0; }
         for (int32_t s = 0; s < S; ++s) {
-            int64_t t = (int64_t)inst * S + s;
+            int64_t t = (int64_t)li * S + s;
             acc += lj_all[2 * t] + lj_all[2 * t + 1];
             for (int j = 0; j < 4 * K; ++j) {
                 double gz = gz_all[(size_t)t * K * 4 + j];
@@ -348,9 +353,15 @@ void orc_elbo_grad(const orc_problem *q, const double *state, int32_t S, uint64_
             gl[j] = gl[j] / (double)S + 1.0;
             ent += l[j] + 0.5 * log(2.0 * M_PI * M_E);
         }
-        elbo[inst] = acc / (double)S + ent;
+        elbo[li] = acc / (double)S + ent;
     }
     free(gz_all); free(eps_all); free(lj_all);
+}
+
+void orc_elbo_grad(const orc_problem *q, const double *state, int32_t S, uint64_t seed,
+                   uint64_t iteration, double *elbo, double *grad, double *ll_out, double *f_out,
+                   int64_t n_f) {
+    orc_elbo_grad_range(q, state, S, seed, iteration, 0, q->P * q->R, elbo, grad, ll_out, f_out, n_f);
 }
 
 /* ------------------------------------------------------------------ optimiser (R10, R11) */

@@ -72,6 +72,8 @@ def lib():
         L.orc_logjoint_grad.argtypes = [C.c_void_p, C.c_int32, dp, dp, dp, dp, dp]
         L.orc_elbo_grad.argtypes = [C.c_void_p, dp, C.c_int32, C.c_uint64, C.c_uint64, dp, dp, dp, dp,
                                     C.c_int64]
+        L.orc_elbo_grad_range.argtypes = [C.c_void_p, dp, C.c_int32, C.c_uint64, C.c_uint64, C.c_int32, C.c_int32,
+                                          dp, dp, dp, dp, C.c_int64]
         L.orc_adam_step.argtypes = [C.c_void_p, dp, dp, dp, dp, C.c_int64]
         L.orc_init_state.argtypes = [C.c_void_p, C.c_uint64, dp]
         L.orc_fit.argtypes = [C.c_void_p, dp, dp, dp, C.c_int32, C.c_int32, C.c_uint64, C.c_int64, dp]
@@ -211,6 +213,16 @@ class Oracle:
         if n_profiles:
             out.append(f)
         return tuple(out)
+
+    def elbo_grad_range(self, state, S, seed, iteration, inst0, n_inst, want_ll=False):
+        """ELBO / gradient (/ ll per draw) of instances inst0 .. inst0+n_inst-1 only (inst = pat*R + rst)."""
+        st = self._state(state)
+        elbo = np.empty(n_inst, dtype=np.float64)
+        grad = np.empty((n_inst, 2, self.K, 4), dtype=np.float64)
+        ll = np.empty((n_inst, S), dtype=np.float64) if want_ll else None
+        lib().orc_elbo_grad_range(self._h, _dp(st), int(S), int(seed), int(iteration), int(inst0), int(n_inst),
+                                  _dp(elbo), _dp(grad), _dp(ll), None, 0)
+        return (elbo, grad, ll) if want_ll else (elbo, grad)
 
     def init_state(self, seed=0):
         st = np.empty((self.P, self.R, 2, self.K, 4), dtype=np.float64)
