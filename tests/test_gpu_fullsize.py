@@ -1,0 +1,133 @@
+"""Parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times (full P, R, S, so the
+same kernel shape, grid and workspace), on outputs the oracle can compute in seconds:
+
+  cfg 1  K=50, S=256: everything (profile, ll per draw, ELBO, gradient) at three states;
+  cfg 2  R=32 x S=4096 (131 072 sample-instances in one launch): ll of every draw and ELBO + gradient of two
+         sampled restarts (first and last), ll of sampled draws of others one by one;
+  cfg 3  P=1024 x S=128: ELBO + gradient + ll of sampled patterns (first, middle, last);
+  cfg 4  K=1000, M~175k, N=8001, +-400-point window, S=256: ll of sampled draws one by one, ELBO and gradient
+         of the whole evaluation;
+plus properties that hold at any size (restarts with identical state and identical counters would coincide;
+every ll finite; gradient of l is 1 + O(.)).  Tolerances as in test_gpu_parity.py (north_star).
+"""
+import numpy as np
+import pytest
+
+from oracle import xrdvi_oracle as orc
+from paper_2501_09308_b200 import Xrdvi, synth
+
+pytestmark = pytest.mark.gpu
+
+TOL_ELBO = 1e-4
+TOL_GRAD = 1e-3
+TOL_PROFILE = 1e-4
+
+
+def class_err(g_gpu, g_ref):
+    """g [..., 2, K, 4] -> max over classes of max_k |diff| / max_k |ref|."""
+    err = np.abs(g_gpu.astype(np.float64) - g_ref).max(axis=-2)
+    ref = np.abs(g_ref).max(axis=-2)
+    return float((err / ref).max())
+
+
+def ll_one_draw(o, state64, seed, iteration, inst, s):
+    """log-likelihood of ONE draw computed piece by piece with the oracle (eps -> zeta -> profile -> ll)."""
+    pat = inst // o.R
+    st = state64.reshape(o.P * o.R, 2, o.K, 4)[inst]
+    zeta = np.empty((o.K, 4))
+    for k in range(o.K):
+        zeta[k] = st[0, k] + np.exp(st[1, k]) * orc.eps(seed, iteration, inst, s, k)
+    return o.loglik(o.profile(zeta, pat), pat)
+
+
+def test_config1_full_size_three_states():
+    wl = synth.make_workload(1)
+    o = orc.from_workload(wl)
+    gpu = Xrdvi.from_workload(wl)
+    assert gpu.pair_count == o.pair_count()
+    for n_fit, it in ((0, 1), (50, 51), (450, 501)):
+        if n_fit:
+            gpu.fit(n_fit, seed=1)
+        st, _ = gpu.get_state()
+        elbo_r, grad_r, ll_r, f_r = o.elbo_grad(st.astype(np.float64), wl.S, 1, it, want_ll=True, n_profiles=3)
+        f_g, ll_g = gpu.debug_profile(wl.S, state=st, S=wl.S, seed=1, iteration=it, want_f=False)
+        np.testing.assert_allclose(ll_g, ll_r.reshape(-1), rtol=TOL_ELBO)
+        f_g, _ = gpu.debug_profile(3, state=st, S=wl.S, seed=1, iteration=it)
+        for t in range(3):
+            assert np.abs(f_g[t] - f_r[t]).max() / np.abs(f_r[t]).max() <= TOL_PROFILE
+        elbo_g, grad_g = gpu.elbo_grad(state=st, S=wl.S, seed=1, iteration=it)
+        np.testing.assert_allclose(elbo_g, elbo_r, rtol=TOL_ELBO)
+        assert class_err(grad_g, grad_r) <= TOL_GRAD
+    inc, area = gpu.inclusion()
+    truth = wl.true_phases[0]
+    assert np.all(inc[0, 0, truth] > 0.99)                       # the planted phases are found
+    assert area[0, 0, truth].sum() > 0.9
+
+
+def test_config2_full_size_sampled_restarts():
+    wl = synth.make_workload(2)
+    assert (wl.R, wl.S) == (32, 4096)
+    o = orc.from_workload(wl)
+    gpu = Xrdvi.from_workload(wl)
+    gpu.reset_state(seed=5)
+    gpu.fit(3, seed=2)                                           # a few full-size steps away from the start
+    st, step = gpu.get_state()
+    assert step == 3
+    st64 = st.astype(np.float64)
+    elbo_g, grad_g = gpu.elbo_grad(state=st, S=wl.S, seed=2, iteration=9)
+    _, ll_g = gpu.debug_profile(wl.R * wl.S, state=st, S=wl.S, seed=2, iteration=9, want_f=False)
+    ll_g = ll_g.reshape(wl.R, wl.S)
+    assert np.isfinite(ll_g).all() and np.isfinite(grad_g).all()
+    for rst in (0, wl.R - 1):
+        e_r, g_r, ll_r = o.elbo_grad_range(st64, wl.S, 2, 9, rst, 1, want_ll=True)
+        np.testing.assert_allclose(ll_g[rst], ll_r[0], rtol=TOL_ELBO)
+        np.testing.assert_allclose(elbo_g[0, rst], e_r[0], rtol=TOL_ELBO)
+        assert class_err(grad_g[0, rst], g_r[0]) <= TOL_GRAD
+    rng = np.random.default_rng(0)
+    for _ in range(12):                                          # other restarts: sampled draws one by one
+        rst, s = int(rng.integers(1, wl.R - 1)), int(rng.integers(0, wl.S))
+        assert ll_g[rst, s] == pytest.approx(ll_one_draw(o, st64, 2, 9, rst, s), rel=TOL_ELBO)
+
+
+def test_config3_full_size_sampled_patterns():
+    wl = synth.make_workload(3)
+    assert (wl.P, wl.S) == (1024, 128)
+    o = orc.from_workload(wl)
+    gpu = Xrdvi.from_workload(wl)
+    gpu.fit(2, seed=4)
+    st, _ = gpu.get_state()
+    st64 = st.astype(np.float64)
+    elbo_g, grad_g = gpu.elbo_grad(state=st, S=wl.S, seed=4, iteration=7)
+    _, ll_g = gpu.debug_profile(wl.P * wl.S, state=st, S=wl.S, seed=4, iteration=7, want_f=False)
+    ll_g = ll_g.reshape(wl.P, wl.S)
+    assert np.isfinite(ll_g).all() and np.isfinite(grad_g).all()
+    for pat in (0, 511, 1023):
+        e_r, g_r, ll_r = o.elbo_grad_range(st64, wl.S, 4, 7, pat, 1, want_ll=True)
+        np.testing.assert_allclose(ll_g[pat], ll_r[0], rtol=TOL_ELBO)
+        np.testing.assert_allclose(elbo_g[pat, 0], e_r[0], rtol=TOL_ELBO)
+        assert class_err(grad_g[pat, 0], g_r[0]) <= TOL_GRAD
+    rng = np.random.default_rng(1)
+    for _ in range(12):
+        pat, s = int(rng.integers(0, wl.P)), int(rng.integers(0, wl.S))
+        assert ll_g[pat, s] == pytest.approx(ll_one_draw(o, st64, 4, 7, pat, s), rel=TOL_ELBO)
+
+
+def test_config4_full_size():
+    wl = synth.make_workload(4)
+    assert (wl.K, wl.N, wl.S) == (1000, 8001, 256)
+    o = orc.from_workload(wl)
+    gpu = Xrdvi.from_workload(wl)
+    assert gpu.n_c == 400 and gpu.pair_count == o.pair_count()
+    gpu.fit(2, seed=6)
+    st, _ = gpu.get_state()
+    st64 = st.astype(np.float64)
+    _, ll_g = gpu.debug_profile(wl.S, state=st, S=wl.S, seed=6, iteration=5, want_f=False)
+    assert np.isfinite(ll_g).all()
+    for s in (0, 31, 32, 100, 255):
+        assert ll_g[s] == pytest.approx(ll_one_draw(o, st64, 6, 5, 0, s), rel=TOL_ELBO)
+    # whole evaluation: 3.6e10 pair evaluations in the fp64 oracle (about a minute on 16 host cores)
+    elbo_g, grad_g = gpu.elbo_grad(state=st, S=wl.S, seed=6, iteration=5)
+    e_r, g_r, ll_r = o.elbo_grad_range(st64, wl.S, 6, 5, 0, 1, want_ll=True)
+    np.testing.assert_allclose(ll_g, ll_r[0], rtol=TOL_ELBO)
+    np.testing.assert_allclose(elbo_g[0, 0], e_r[0], rtol=TOL_ELBO)
+    assert class_err(grad_g[0, 0], g_r[0]) <= TOL_GRAD
