@@ -37,9 +37,9 @@ size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
 struct Plan {   // workspace carve; identical arithmetic in workspace_bytes and create
     int P, R, PR, S_pad, gpi_max, G_max, K;
     int TW, PS, NW, SP, n_seg, n_tile;
-    long long M, n_c, bwd_cap, slots_cap;
+    long long M, n_c, tile_cap, slots_cap;
     size_t total;
-    size_t o_yb, o_bg, o_pkf, o_tile, o_pkb, o_wrng, o_sord, o_sofs, o_sids, o_pat, o_area, o_mh0;
+    size_t o_yb, o_bg, o_pkt, o_runs, o_srng, o_sord, o_sofs, o_sids, o_pat, o_area, o_mh0;
     size_t o_var, o_vartmp, o_mom1, o_mom2, o_grad, o_elbo, o_elbok, o_llt, o_trace, o_done, o_ctl;
     size_t o_lat, o_eps, o_rr, o_ng, o_llpart, o_part8, o_dbg;
 };
@@ -51,21 +51,22 @@ long long window_points(const xrdvi_hyper* hyp, double step) {
 }
 
 // CTA shape of elbo_tile_kernel: TW tiles of 16 points per segment, PS shares of each tile's peak list
-// (TW * PS warps).  Many groups: long segments, no split.  Few groups (config 1: 8): short segments and a
-// split peak list, so that the 148 SMs still see several warps per scheduler.
+// (TW * PS warps).  Many groups: no split.  Few groups (config 1: 8): split peak lists, so that the 148 SMs
+// still see several warps per scheduler.
 void choose_shape(int64_t N, int G_max, int* TW, int* PS) {
     if (const char* e = std::getenv("XRDVI_TILE_SHAPE")) {   // tuning knob for sweeps: "TWxPS"
         int a = 0, b = 0;
-        if (std::sscanf(e, "%dx%d", &a, &b) == 2 && (a == 1 || a == 2 || a == 4) && (b == 1 || b == 2 || b == 4)) {
+        if (std::sscanf(e, "%dx%d", &a, &b) == 2 && (a == 1 || a == 2 || a == 4) && (b == 1 || b == 2 || b == 4 || b == 8) && a * b <= 16) {
             *TW = a; *PS = b;
             return;
         }
     }
+    // measured on B200 (profiles/r1_v3_shape_sweep.md): one tile per CTA is best everywhere; few tile-warps
+    // (configs 1 and 4: 2008 / 4008) want the peak lists split four ways, many (configs 2, 3: 1e6) no split
     const long long tiles = (N + 15) / 16 * static_cast<long long>(G_max);   // warps at PS = 1
-    const long long want = 148ll * 4 * 8;                                     // 8 warps per scheduler
-    if (tiles >= want) { *TW = 4; *PS = 1; }
-    else if (2 * tiles >= want) { *TW = 2; *PS = 2; }
-    else { *TW = 2; *PS = 4; }
+    const long long resident = 148ll * 24;                                    // warps the GPU holds at 80 registers
+    *TW = 1;
+    *PS = tiles >= 8 * resident ? 1 : 4;
 }
 
 bool make_plan(int64_t N, int32_t K, int64_t M, int32_t S_max, double step, const xrdvi_hyper* hyp, Plan* pl) {
@@ -87,21 +88,20 @@ bool make_plan(int64_t N, int32_t K, int64_t M, int32_t S_max, double step, cons
     p.n_seg = static_cast<int>((N + p.SP - 1) / p.SP);
     p.n_tile = static_cast<int>((N + kPT - 1) / kPT);
     p.n_c = window_points(hyp, step);
-    // entries of the per-segment phase-major lists: a peak appears once per segment its window touches
-    const long long per_peak = p.n_c < 0 ? p.n_seg : std::min<long long>(p.n_seg, (2 * p.n_c + p.SP) / p.SP + 1);
-    p.bwd_cap = M * per_peak;
-    p.slots_cap = std::min<long long>(static_cast<long long>(p.n_seg) * (K + p.NW), p.bwd_cap + static_cast<long long>(p.n_seg) * p.NW);
-    if (p.bwd_cap > (1ll << 31) - 1 || p.slots_cap > (1ll << 31) - 1) return false;
+    // entries of the per-tile phase-major lists: a peak appears once per 16-point tile its window touches
+    const long long per_peak = p.n_c < 0 ? p.n_tile : std::min<long long>(p.n_tile, (2 * p.n_c + kPT) / kPT + 1);
+    p.tile_cap = M * per_peak;
+    p.slots_cap = std::min<long long>(static_cast<long long>(p.n_tile) * K, p.tile_cap);   // one slot per (tile, phase)
+    if (p.tile_cap > (1ll << 31) - 1 || p.slots_cap > (1ll << 31) - 1) return false;
     size_t o = 0;
     auto take = [&](size_t bytes) { size_t r = o; o = align_up(o + bytes); return r; };
     const size_t var_b = sizeof(float) * p.PR * 8 * static_cast<size_t>(K);
     const size_t gk32 = static_cast<size_t>(p.G_max) * K * 32;
     p.o_yb = take(sizeof(float) * p.P * N);
     p.o_bg = take(sizeof(float) * p.P * N);
-    p.o_pkf = take(sizeof(PeakRec) * M);
-    p.o_tile = take(sizeof(int4) * p.n_tile);
-    p.o_pkb = take(sizeof(PeakRec) * std::max<long long>(p.bwd_cap, 1));
-    p.o_wrng = take(sizeof(int4) * static_cast<size_t>(p.n_seg) * p.NW);
+    p.o_pkt = take(sizeof(PeakRec) * (p.tile_cap + 1));
+    p.o_runs = take(sizeof(int4) * (p.slots_cap + 1));
+    p.o_srng = take(sizeof(int2) * static_cast<size_t>(p.n_tile) * p.PS);
     p.o_sord = take(sizeof(int) * p.n_seg);
     p.o_sofs = take(sizeof(int) * (K + 1));
     p.o_sids = take(sizeof(int) * std::max<long long>(p.slots_cap, 1));
@@ -164,12 +164,12 @@ template <bool BWD>
 void launch_tile(const Dev& d, cudaStream_t st, float* f_dbg, long long n_dbg) {
     const dim3 grid(d.n_seg, d.G);
 #define XRDVI_TILE_CASE(TW_, PS_)                                                                           \
-    case TW_ * 8 + PS_:                                                                                    \
+    case TW_ * 16 + PS_:                                                                                    \
         elbo_tile_kernel<TW_, PS_, BWD><<<grid, 32 * TW_ * PS_, 0, st>>>(d, f_dbg, n_dbg);                 \
         break;
-    switch (d.TW * 8 + d.PS) {
-        XRDVI_TILE_CASE(1, 1) XRDVI_TILE_CASE(1, 2) XRDVI_TILE_CASE(1, 4)
-        XRDVI_TILE_CASE(2, 1) XRDVI_TILE_CASE(2, 2) XRDVI_TILE_CASE(2, 4)
+    switch (d.TW * 16 + d.PS) {
+        XRDVI_TILE_CASE(1, 1) XRDVI_TILE_CASE(1, 2) XRDVI_TILE_CASE(1, 4) XRDVI_TILE_CASE(1, 8)
+        XRDVI_TILE_CASE(2, 1) XRDVI_TILE_CASE(2, 2) XRDVI_TILE_CASE(2, 4) XRDVI_TILE_CASE(2, 8)
         XRDVI_TILE_CASE(4, 1) XRDVI_TILE_CASE(4, 2) XRDVI_TILE_CASE(4, 4)
         default: break;
     }
@@ -328,7 +328,7 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
     if (reinterpret_cast<uintptr_t>(workspace) % 256) return fail(XRDVI_E_INVALID_ARG, "workspace not 256-byte aligned");
 
     // ---- fp64 preprocessing (R16) ----------------------------------------------------------------
-    const int P = pl.P, W = pl.NW, SP = pl.SP;
+    const int P = pl.P, SP = pl.SP;
     long long n_c = pl.n_c;
     if (n_c < 0) {     // dense: every point is inside every window, wherever the peak lies
         n_c = N;
@@ -359,73 +359,73 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
     for (int k = 0; k < K; ++k)
         if (!(area[k] > 0.0)) return fail(XRDVI_E_EMPTY_PHASE, "phase " + std::to_string(k) + " has zero total intensity");
 
-    // phase-1 table: sorted by j (stable in (j, k, original order)); 16-point tile ranges by binary search
+    // per-tile phase-major lists: the peaks whose window reaches the tile, stable-sorted by phase; PS
+    // contiguous shares split at phase boundaries and balanced by clipped pair count; one output slot per
+    // (tile, phase present in the tile)
     std::vector<HP> fw = kept;
     std::stable_sort(fw.begin(), fw.end(), [](const HP& a, const HP& b) { return a.j < b.j; });
-    auto rec = [](const HP& p) {
-        return PeakRec{static_cast<int>(p.j), static_cast<float>(p.d), static_cast<float>(p.I), p.k};
-    };
-    std::vector<PeakRec> pk_fwd(std::max(Mv, 1));
-    for (int m = 0; m < Mv; ++m) pk_fwd[m] = rec(fw[m]);
     auto j_range = [&](long long jlo, long long jhi) {
         auto a = std::lower_bound(fw.begin(), fw.end(), jlo, [](const HP& p, long long v) { return p.j < v; });
         auto b = std::upper_bound(fw.begin(), fw.end(), jhi, [](long long v, const HP& p) { return v < p.j; });
         return make_int2(static_cast<int>(a - fw.begin()), static_cast<int>(b - fw.begin()));
     };
-    std::vector<int4> tile_rng(pl.n_tile);
-    for (int t = 0; t < pl.n_tile; ++t) {
-        const long long i0 = static_cast<long long>(t) * kPT, i1 = i0 + kPT - 1;
-        const int2 all = j_range(i0 - n_c, std::min<long long>(i1, N - 1) + n_c);   // window reaches a tile point < N
-        int2 full = j_range(i1 - n_c, i0 + n_c);                                   // window covers all 16 points
-        full.x = std::min(std::max(full.x, all.x), all.y);
-        full.y = std::min(std::max(full.y, full.x), all.y);
-        tile_rng[t] = make_int4(all.x, full.x, full.y, all.y);
-    }
-
-    // phase-2 tables: per segment, the peaks whose window reaches it, phase-major; W contiguous warp
-    // ranges balanced by clipped pair count; one output slot per (segment, warp, phase run)
-    std::vector<PeakRec> pk_bwd;
-    pk_bwd.reserve(static_cast<size_t>(std::min<long long>(pl.bwd_cap, 1ll << 24)));
-    std::vector<int4> warp_rng(static_cast<size_t>(pl.n_seg) * W);
+    const int PSn = pl.PS, TWn = pl.TW;
+    std::vector<PeakRec> pk_tile;
+    pk_tile.reserve(static_cast<size_t>(std::min<long long>(pl.tile_cap, 1ll << 24)));
+    std::vector<int4> run_tab;                                  // (m0, m1, phase, 0); index = output slot
+    std::vector<int2> share_rng(static_cast<size_t>(pl.n_tile) * PSn);
     std::vector<long long> seg_work(pl.n_seg, 0);
     std::vector<int> slot_phase;
     long long pairs_check = 0;
     {
-        std::vector<HP> sl;
-        std::vector<long long> wgt;
-        for (int s = 0; s < pl.n_seg; ++s) {
-            const long long s0 = static_cast<long long>(s) * SP, s1 = std::min<long long>(s0 + SP - 1, N - 1);
-            const int2 r = j_range(s0 - n_c, s1 + n_c);
-            sl.assign(fw.begin() + r.x, fw.begin() + r.y);
-            std::stable_sort(sl.begin(), sl.end(), [](const HP& a, const HP& b) { return a.k < b.k; });
-            wgt.resize(sl.size());
+        std::vector<HP> tl;
+        std::vector<long long> run_w;      // clipped pair count per phase run
+        std::vector<int> run_end;          // end index (exclusive) of each phase run in tl
+        for (int t = 0; t < pl.n_tile; ++t) {
+            const long long i0 = static_cast<long long>(t) * kPT, i1 = std::min<long long>(i0 + kPT - 1, N - 1);
+            const int2 r = j_range(i0 - n_c, i1 + n_c);
+            tl.assign(fw.begin() + r.x, fw.begin() + r.y);
+            std::stable_sort(tl.begin(), tl.end(), [](const HP& a, const HP& b) { return a.k < b.k; });
+            run_w.clear();
+            run_end.clear();
             long long tot = 0;
-            for (size_t q = 0; q < sl.size(); ++q) {
-                const long long lo = std::max(s0, sl[q].j - n_c), hi = std::min(s1, sl[q].j + n_c);
-                wgt[q] = hi - lo + 1;   // >= 1 by construction of the range
-                tot += wgt[q];
+            for (size_t q = 0; q < tl.size(); ++q) {
+                const long long lo = std::max(i0, tl[q].j - n_c), hi = std::min(i1, tl[q].j + n_c);
+                const long long wq = hi - lo + 1;   // >= 1 by construction of the range
+                if (q == 0 || tl[q].k != tl[q - 1].k) { run_w.push_back(0); run_end.push_back(0); }
+                run_w.back() += wq;
+                run_end.back() = static_cast<int>(q + 1);
+                tot += wq;
             }
-            seg_work[s] = tot;
+            seg_work[t / TWn] += tot;
             pairs_check += tot;
-            const int base = static_cast<int>(pk_bwd.size());
-            for (const HP& p : sl) pk_bwd.push_back(rec(p));
-            size_t q = 0;
+            const int base = static_cast<int>(pk_tile.size());
+            for (const HP& p : tl) {
+                const long long dj = p.j - i0;
+                const bool full = (i1 - i0 == kPT - 1) && dj - n_c <= 0 && dj + n_c >= kPT - 1;
+                pk_tile.push_back(PeakRec{static_cast<int>(dj), static_cast<float>(p.d), static_cast<float>(p.I), full ? 1 : 0});
+            }
+            const int run_base = static_cast<int>(run_tab.size());
+            for (size_t rr = 0; rr < run_w.size(); ++rr) {
+                const int q0 = rr ? run_end[rr - 1] : 0;
+                run_tab.push_back(make_int4(base + q0, base + run_end[rr], tl[q0].k, 0));
+                slot_phase.push_back(tl[q0].k);
+            }
+            size_t run = 0;
             long long cum = 0;
-            for (int w = 0; w < W; ++w) {
-                const size_t q0 = q;
-                const long long goal = tot * (w + 1) / W;
-                if (w == W - 1) q = sl.size();
-                else while (q < sl.size() && cum + wgt[q] <= goal) { cum += wgt[q]; ++q; }
-                const int slot0 = static_cast<int>(slot_phase.size());
-                for (size_t t = q0; t < q; ++t)
-                    if (t == q0 || sl[t].k != sl[t - 1].k) slot_phase.push_back(sl[t].k);
-                warp_rng[static_cast<size_t>(s) * W + w] = make_int4(base + static_cast<int>(q0), base + static_cast<int>(q), slot0, 0);
+            for (int w = 0; w < PSn; ++w) {
+                const size_t run0 = run;
+                const long long goal = tot * (w + 1) / PSn;
+                if (w == PSn - 1) run = run_w.size();
+                else while (run < run_w.size() && cum + run_w[run] <= goal) { cum += run_w[run]; ++run; }
+                share_rng[static_cast<size_t>(t) * PSn + w] =
+                    make_int2(run_base + static_cast<int>(run0), run_base + static_cast<int>(run));
             }
         }
     }
-    if (pairs_check != pairs) return fail(XRDVI_E_INVALID_ARG, "internal: segment tables do not cover every pair once");
+    if (pairs_check != pairs) return fail(XRDVI_E_INVALID_ARG, "internal: tile tables do not cover every pair once");
     const int n_slots = static_cast<int>(slot_phase.size());
-    if (static_cast<long long>(pk_bwd.size()) > pl.bwd_cap || n_slots > pl.slots_cap)
+    if (static_cast<long long>(pk_tile.size()) > pl.tile_cap + 1 || n_slots > pl.slots_cap)
         return fail(XRDVI_E_INVALID_ARG, "internal: table bound exceeded");
     std::vector<int> slot_ofs(K + 1, 0), slot_ids(std::max(n_slots, 1));
     for (int s = 0; s < n_slots; ++s) ++slot_ofs[slot_phase[s] + 1];
@@ -437,7 +437,8 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
     std::vector<int> seg_order(pl.n_seg);
     std::iota(seg_order.begin(), seg_order.end(), 0);
     std::stable_sort(seg_order.begin(), seg_order.end(), [&](int a, int b) { return seg_work[a] > seg_work[b]; });
-    if (pk_bwd.empty()) pk_bwd.push_back(PeakRec{0, 0.f, 0.f, 0});
+    pk_tile.push_back(PeakRec{0, 0.f, 0.f, 0});       // padding entries: the kernel prefetches one record and
+    run_tab.push_back(make_int4(0, 0, 0, 0));         // one run header past the end of every share
 
     // observed data and per-pattern constants
     std::vector<float> yb(static_cast<size_t>(P) * N), bgf(static_cast<size_t>(P) * N);
@@ -493,10 +494,9 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
     d.beta2 = static_cast<float>(hyp->beta2); d.adam_eps = static_cast<float>(hyp->adam_eps);
     d.yb = reinterpret_cast<float*>(w + pl.o_yb);
     d.bg = reinterpret_cast<float*>(w + pl.o_bg);
-    d.pk_fwd = reinterpret_cast<PeakRec*>(w + pl.o_pkf);
-    d.tile_rng = reinterpret_cast<int4*>(w + pl.o_tile);
-    d.pk_bwd = reinterpret_cast<PeakRec*>(w + pl.o_pkb);
-    d.warp_rng = reinterpret_cast<int4*>(w + pl.o_wrng);
+    d.pk_tile = reinterpret_cast<PeakRec*>(w + pl.o_pkt);
+    d.run_tab = reinterpret_cast<int4*>(w + pl.o_runs);
+    d.share_rng = reinterpret_cast<int2*>(w + pl.o_srng);
     d.seg_order = reinterpret_cast<int*>(w + pl.o_sord);
     d.slot_ofs = reinterpret_cast<int*>(w + pl.o_sofs);
     d.slot_ids = reinterpret_cast<int*>(w + pl.o_sids);
@@ -528,10 +528,9 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
     auto chk = [&](cudaError_t e) { if (ce == cudaSuccess) ce = e; };
     chk(up(pl.o_yb, yb.data(), sizeof(float) * yb.size()));
     chk(up(pl.o_bg, bgf.data(), sizeof(float) * bgf.size()));
-    chk(up(pl.o_pkf, pk_fwd.data(), sizeof(PeakRec) * pk_fwd.size()));
-    chk(up(pl.o_tile, tile_rng.data(), sizeof(int4) * tile_rng.size()));
-    chk(up(pl.o_pkb, pk_bwd.data(), sizeof(PeakRec) * pk_bwd.size()));
-    chk(up(pl.o_wrng, warp_rng.data(), sizeof(int4) * warp_rng.size()));
+    chk(up(pl.o_pkt, pk_tile.data(), sizeof(PeakRec) * pk_tile.size()));
+    chk(up(pl.o_runs, run_tab.data(), sizeof(int4) * run_tab.size()));
+    chk(up(pl.o_srng, share_rng.data(), sizeof(int2) * share_rng.size()));
     chk(up(pl.o_sord, seg_order.data(), sizeof(int) * seg_order.size()));
     chk(up(pl.o_sofs, slot_ofs.data(), sizeof(int) * slot_ofs.size()));
     chk(up(pl.o_sids, slot_ids.data(), sizeof(int) * slot_ids.size()));

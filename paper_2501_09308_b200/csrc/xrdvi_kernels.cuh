@@ -6,12 +6,15 @@
 // latents are lane-private, all global traffic is 128-byte coalesced.
 //
 // One optimisation step is two kernels:
-//   elbo_tile_kernel   (a-3, a-4, a-5, a-6 likelihood part) one CTA per (2theta segment, group):
-//                      phase 1 synthesises the profile on the segment from every peak whose window
-//                      reaches it and leaves the residual e = (y - f)/sigma_n^2 in SHARED memory;
-//                      phase 2 walks the same peaks phase-major, accumulates the six backward sums
-//                      over the segment, applies the chain rule and reduces over the 32 draws with
-//                      warp shuffles (fixed tree) to 8 floats per (segment, warp, phase-run, group).
+//   elbo_tile_kernel   (a-3, a-4, a-5, a-6 likelihood part) one CTA per (TW consecutive 16-point tiles, group).
+//                      Every tile has a static, PHASE-MAJOR list of the peaks whose window reaches it, split at
+//                      phase boundaries into PS shares; warp (tile, share) walks its share twice:
+//                      phase 1 synthesises the profile of the tile in 16 registers per lane (the PS partial
+//                      profiles are summed through shared memory), the residual e = (y - f)/sigma_n^2 goes
+//                      back to all shares through shared memory and then lives in REGISTERS;
+//                      phase 2 accumulates the six backward sums of each peak over the 16 points, folds them
+//                      per phase, applies the chain rule and reduces over the 32 draws with warp shuffles
+//                      (fixed tree) to 8 floats per (tile, phase, group).
 //   update_draw_kernel (a-6 prior part, a-7, a-8, a-1, a-2) one CTA per (phase, instance): fixed-order
 //                      reduction of the partials and of the per-draw prior terms, ELBO, Adam ascent
 //                      on the 8 variational parameters of the phase, then the Philox draws and the
@@ -22,12 +25,15 @@
 // stored as (j_m, delta_m) with p_m = x_{j_m} + delta_m computed in fp64 at create, so
 // t' = (i - j_m) * (Delta*2/w) + (-delta_m - mu) * 2/w  has no fp32 cancellation at high angles.
 //
-// Instruction diet: the FP32 FMA pipe (128 lanes/SM/clk) and the MUFU pipe (16
-// lanes/SM/clk, shared by ex2 and rcp) bound the path.  Two measures cut the MUFU work of the plain
-// formulation (2 MUFU per pair and pass):
+// Instruction diet: the path is bound by SM issue slots (4 warp-instructions per
+// clock), then by the MUFU pipe (16 lanes/SM/clk, shared by ex2 and rcp).  Measures:
 //   * Gaussian core / Lorentz tail: 2^(-t'^2) < 2^-24 for |t'| > 4.9, so outside a per-(group, phase)
 //     core half-width n_g (from the largest sampled w and |mu| of the 32 draws) only L is evaluated;
-//   * shared reciprocal: 1/ua and 1/ub of two neighbouring points come from ONE rcp(ua*ub).
+//   * shared reciprocal: 1/ua and 1/ub of two neighbouring points come from ONE rcp(ua*ub);
+//   * (peak, tile) pairs whose 16 points are all in-window and all tail take a branch-free unrolled body;
+//     the others are processed quad by quad (out-of-window quads skipped, partial quads masked);
+//   * backward first moments use t' = t0 + p*step: sum e L^2 t' = t0 sum e L^2 + step sum (p e) L^2 with
+//     p*e held in registers, so the inner loop needs no multiplication by t'.
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
@@ -43,11 +49,11 @@ constexpr float kAG = 0.93943727869965132f;  // 2 sqrt(ln2/pi)
 constexpr float kAL = 0.63661977236758134f;  // 2/pi
 constexpr float kLn2 = 0.69314718055994531f;
 
-struct PeakRec {   // 16 bytes
-    int j;         // nearest grid index of the peak (may lie outside [0,N))
-    float delta;   // p_m - x_j  (|delta| <= Delta/2), fp64-computed
+struct PeakRec {   // 16 bytes; one record per (peak, 16-point tile its window reaches)
+    int dj;        // nearest grid index j_m of the peak minus the first grid index of the tile
+    float delta;   // p_m - x_{j_m}  (|delta| <= Delta/2), fp64-computed
     float inten;   // I_m
-    int k;         // phase
+    int full;      // 1: all 16 points of the tile exist and lie inside the peak's window
 };
 
 struct PatConst {  // per observed pattern
@@ -80,12 +86,11 @@ struct Dev {
     // static tables
     const float* yb;          // [P][N]  y - B
     const float* bg;          // [P][N]
-    const PeakRec* pk_fwd;    // [Mv] sorted by j
-    const int4* tile_rng;     // [n_tile] peak ranges in pk_fwd of each 16-point tile: [x,w) reaches the tile,
-                              //          [y,z) covers all 16 points with its window
-    const PeakRec* pk_bwd;    // per-segment phase-major peak lists, concatenated
-    const int4* warp_rng;     // [n_seg][TW*PS]: (m0, m1) range in pk_bwd of the warp, .z = its first slot
-    const int* seg_order;     // [n_seg] segments by decreasing work (LPT dispatch order)
+    const PeakRec* pk_tile;   // per-tile phase-major peak lists, concatenated (+1 padding record)
+    const int4* run_tab;      // [n_slots + 1] phase runs of the tile lists: (m0, m1) range in pk_tile, .z = phase;
+                              //               the run index is also the output slot in part8
+    const int2* share_rng;    // [n_tile][PS]: range of runs of the share
+    const int* seg_order;     // [n_seg] segments (TW tiles) by decreasing work (LPT dispatch order)
     const int* slot_ofs;      // [K+1] CSR: slots of phase k
     const int* slot_ids;      // [n_slots]
     const PatConst* pat;      // [P]
@@ -221,98 +226,118 @@ __global__ void __launch_bounds__(128) draw_transform_kernel(const Dev d, const 
 // ------------------------------------------------------------------------------------------------
 // Phase-1 building blocks (profile).  acc[p] += I_m [ c_G 2^(-t'^2) + c_L / (1 + t'^2) ].
 // Two neighbouring points share one reciprocal: 1/ua = ub * rcp(ua ub).
+// The Gaussian uses u = 1 + t'^2 as well: 2^(-t'^2) = 2 * 2^(-u), the factor 2 is folded into cg2 = 2 c_G.
 template <bool CORE>
-__device__ __forceinline__ void fwd_pair(float ta, float tb, float cg, float cl, float& acca, float& accb) {
+__device__ __forceinline__ void fwd_pair(float ta, float tb, float cg2, float cl, float& acca, float& accb) {
     const float ua = fmaf(ta, ta, 1.0f), ub = fmaf(tb, tb, 1.0f);
     const float rc = rcp_approx(ua * ub) * cl;
     acca = fmaf(rc, ub, acca);
     accb = fmaf(rc, ua, accb);
     if (CORE) {
-        acca = fmaf(cg, ex2_approx(-(ta * ta)), acca);
-        accb = fmaf(cg, ex2_approx(-(tb * tb)), accb);
+        acca = fmaf(cg2, ex2_approx(-ua), acca);
+        accb = fmaf(cg2, ex2_approx(-ub), accb);
     }
 }
 
-// One peak on the 16 points of a tile.  MASK: only points p_lo <= p <= p_hi are inside the peak's window.
-template <bool CORE, bool MASK>
-__device__ __forceinline__ void fwd_tile(float t0, float step, float cg, float cl, int p_lo, int p_hi, float (&acc)[kPT]) {
-    const unsigned span = static_cast<unsigned>(p_hi - p_lo);
-#pragma unroll
-    for (int p = 0; p < kPT; p += 2) {
-        const float ta = fmaf(static_cast<float>(p), step, t0);
-        const float tb = fmaf(static_cast<float>(p + 1), step, t0);
-        if (MASK) {
-            float va = 0.0f, vb = 0.0f;
-            fwd_pair<CORE>(ta, tb, cg, cl, va, vb);
-            acc[p] += (static_cast<unsigned>(p - p_lo) <= span) ? va : 0.0f;
-            acc[p + 1] += (static_cast<unsigned>(p + 1 - p_lo) <= span) ? vb : 0.0f;
+// same with per-point coefficients (window-edge quads: the coefficient of an out-of-window point is 0)
+template <bool CORE>
+__device__ __forceinline__ void fwd_pair_masked(float ta, float tb, float cga, float cgb, float cla, float clb,
+                                                float& acca, float& accb) {
+    const float ua = fmaf(ta, ta, 1.0f), ub = fmaf(tb, tb, 1.0f);
+    const float rc = rcp_approx(ua * ub);
+    acca = fmaf(rc * ub, cla, acca);
+    accb = fmaf(rc * ua, clb, accb);
+    if (CORE) {
+        acca = fmaf(cga, ex2_approx(-ua), acca);
+        accb = fmaf(cgb, ex2_approx(-ub), accb);
+    }
+}
+
+// Per-(peak, tile) geometry in tile coordinates (warp-uniform): in-window points p_lo <= p <= p_hi, Gaussian
+// core c_lo <= p <= c_hi.
+struct PeakGeo { int p_lo, p_hi, c_lo, c_hi; };
+
+// One quad (points 4Q .. 4Q+3) of the generic path of phase 1.
+template <int Q>
+__device__ __forceinline__ void fwd_quad_generic(const PeakGeo& g, float t0, float step, float cg, float cl,
+                                                 float (&acc)[kPT]) {
+    const int lo = max(g.p_lo, 4 * Q), hi = min(g.p_hi, 4 * Q + 3);
+    if (lo > hi) return;                                   // quad outside the window
+    const bool core = g.c_hi >= 4 * Q && g.c_lo <= 4 * Q + 3;
+    const float t_0 = fmaf(static_cast<float>(4 * Q), step, t0), t_1 = fmaf(static_cast<float>(4 * Q + 1), step, t0);
+    const float t_2 = fmaf(static_cast<float>(4 * Q + 2), step, t0), t_3 = fmaf(static_cast<float>(4 * Q + 3), step, t0);
+    if (hi - lo == 3) {
+        if (core) {
+            fwd_pair<true>(t_0, t_1, cg, cl, acc[4 * Q], acc[4 * Q + 1]);
+            fwd_pair<true>(t_2, t_3, cg, cl, acc[4 * Q + 2], acc[4 * Q + 3]);
         } else {
-            fwd_pair<CORE>(ta, tb, cg, cl, acc[p], acc[p + 1]);
+            fwd_pair<false>(t_0, t_1, cg, cl, acc[4 * Q], acc[4 * Q + 1]);
+            fwd_pair<false>(t_2, t_3, cg, cl, acc[4 * Q + 2], acc[4 * Q + 3]);
         }
-    }
-}
-
-// Loop of phase 1 over the peaks [m0, m1) of pk_fwd for the tile starting at grid point i0.
-template <bool MASK>
-__device__ __forceinline__ void fwd_peaks(const Dev& d, const float4* __restrict__ lat, const int* __restrict__ ngk,
-                                          int m0, int m1, int i0, float (&acc)[kPT]) {
-    if (m0 >= m1) return;
-    const int n_c = d.n_c;
-    PeakRec pk_n = d.pk_fwd[m0];
-    float4 lt_n = lat[static_cast<size_t>(pk_n.k) * 32];
-    int ng_n = ngk[pk_n.k];
-    for (int m = m0; m < m1; ++m) {
-        const PeakRec pk = pk_n;
-        const float4 lt = lt_n;
-        const int ngc = ng_n;
-        if (m + 1 < m1) {  // prefetch the next peak and its latents
-            pk_n = d.pk_fwd[m + 1];
-            lt_n = lat[static_cast<size_t>(pk_n.k) * 32];
-            ng_n = ngk[pk_n.k];
+    } else {
+        const unsigned span = static_cast<unsigned>(hi - lo);
+        const bool m0 = static_cast<unsigned>(4 * Q - lo) <= span, m1 = static_cast<unsigned>(4 * Q + 1 - lo) <= span;
+        const bool m2 = static_cast<unsigned>(4 * Q + 2 - lo) <= span, m3 = static_cast<unsigned>(4 * Q + 3 - lo) <= span;
+        if (core) {
+            fwd_pair_masked<true>(t_0, t_1, m0 ? cg : 0.f, m1 ? cg : 0.f, m0 ? cl : 0.f, m1 ? cl : 0.f, acc[4 * Q], acc[4 * Q + 1]);
+            fwd_pair_masked<true>(t_2, t_3, m2 ? cg : 0.f, m3 ? cg : 0.f, m2 ? cl : 0.f, m3 ? cl : 0.f, acc[4 * Q + 2], acc[4 * Q + 3]);
+        } else {
+            fwd_pair_masked<false>(t_0, t_1, 0.f, 0.f, m0 ? cl : 0.f, m1 ? cl : 0.f, acc[4 * Q], acc[4 * Q + 1]);
+            fwd_pair_masked<false>(t_2, t_3, 0.f, 0.f, m2 ? cl : 0.f, m3 ? cl : 0.f, acc[4 * Q + 2], acc[4 * Q + 3]);
         }
-        const float step = d.delta * lt.x;
-        const float tc = fmaf(-pk.delta, lt.x, lt.y);
-        const int dj = pk.j - i0;                         // peak centre in tile coordinates
-        const float t0 = fmaf(static_cast<float>(-dj), step, tc);
-        const float cl = pk.inten * lt.w;
-        const int p_lo = dj - n_c, p_hi = dj + n_c;       // in-window points of the tile: p_lo <= p <= p_hi
-        // Gaussian core |p - dj| <= n_g touches the tile?  (warp-uniform)
-        if (static_cast<unsigned>(dj + ngc) <= static_cast<unsigned>(kPT - 1 + 2 * ngc))
-            fwd_tile<true, MASK>(t0, step, pk.inten * lt.z, cl, p_lo, p_hi, acc);
-        else
-            fwd_tile<false, MASK>(t0, step, 0.0f, cl, p_lo, p_hi, acc);
     }
 }
 
 // ------------------------------------------------------------------------------------------------
-// Phase-2 building blocks (six sums in t' units):
-//   a1 = sum e L, a2 = sum e G, a3 = sum e L^2 t', a4 = sum e G t', a5 = sum e L^2, a6 = sum e G t'^2
-struct Acc6 { float a1, a2, a3, a4, a5, a6; };
+// Phase-2 building blocks.  Per (peak, tile) with t'_p = t0 + p step, e_p the residual and pe_p = p e_p:
+//   a1 = sum e L, a5 = sum e L^2, a3p = sum pe L^2      (Lorentz part, every in-window point)
+//   a2 = sum e g, a4p = sum pe g, a6u = sum e u g       (Gaussian part, core points only; g = 2^(-u) = G/2,
+//                                                        u = 1 + t'^2)
+// and then  sum e L^2 t' = t0 a5 + step a3p,  sum e G = 2 a2,  sum e G t' = 2 (t0 a2 + step a4p),
+// sum e G t'^2 = 2 (a6u - a2).
+struct Acc6 { float a1, a2, a3p, a4p, a5, a6u; };
 
 template <bool CORE>
-__device__ __forceinline__ void bwd_pair(float ea, float eb, float ta, float tb, Acc6& a) {
+__device__ __forceinline__ void bwd_pair(float ea, float eb, float pea, float peb, float ta, float tb, Acc6& a) {
     const float ua = fmaf(ta, ta, 1.0f), ub = fmaf(tb, tb, 1.0f);
     const float r = rcp_approx(ua * ub);
     const float La = r * ub, Lb = r * ua;
-    const float xa = ea * La, xb = eb * Lb;
-    a.a1 += xa + xb;
-    const float pa = xa * La, pb = xb * Lb;
-    a.a5 += pa + pb;
-    a.a3 = fmaf(pa, ta, fmaf(pb, tb, a.a3));
+    const float La2 = La * La, Lb2 = Lb * Lb;
+    a.a1 = fmaf(ea, La, fmaf(eb, Lb, a.a1));
+    a.a5 = fmaf(ea, La2, fmaf(eb, Lb2, a.a5));
+    a.a3p = fmaf(pea, La2, fmaf(peb, Lb2, a.a3p));
     if (CORE) {
-        const float za = ea * ex2_approx(-(ta * ta)), zb = eb * ex2_approx(-(tb * tb));
-        a.a2 += za + zb;
-        const float zta = za * ta, ztb = zb * tb;
-        a.a4 += zta + ztb;
-        a.a6 = fmaf(zta, ta, fmaf(ztb, tb, a.a6));
+        const float ga = ex2_approx(-ua), gb = ex2_approx(-ub);
+        a.a2 = fmaf(ea, ga, fmaf(eb, gb, a.a2));
+        a.a4p = fmaf(pea, ga, fmaf(peb, gb, a.a4p));
+        a.a6u = fmaf(ea * ua, ga, fmaf(eb * ub, gb, a.a6u));
     }
 }
 
-template <bool CORE>
-__device__ __forceinline__ void bwd_quad(const float4 e4, float tq, float step, Acc6& a) {
-    const float t1 = tq + step, t2 = fmaf(2.0f, step, tq), t3 = fmaf(3.0f, step, tq);
-    bwd_pair<CORE>(e4.x, e4.y, tq, t1, a);
-    bwd_pair<CORE>(e4.z, e4.w, t2, t3, a);
+template <int Q>
+__device__ __forceinline__ void bwd_quad_generic(const PeakGeo& g, float t0, float step, const float (&e)[kPT],
+                                                 const float (&pe)[kPT], Acc6& a) {
+    const int lo = max(g.p_lo, 4 * Q), hi = min(g.p_hi, 4 * Q + 3);
+    if (lo > hi) return;
+    const bool core = g.c_hi >= 4 * Q && g.c_lo <= 4 * Q + 3;
+    const float t_0 = fmaf(static_cast<float>(4 * Q), step, t0), t_1 = fmaf(static_cast<float>(4 * Q + 1), step, t0);
+    const float t_2 = fmaf(static_cast<float>(4 * Q + 2), step, t0), t_3 = fmaf(static_cast<float>(4 * Q + 3), step, t0);
+    float e0 = e[4 * Q], e1 = e[4 * Q + 1], e2 = e[4 * Q + 2], e3 = e[4 * Q + 3];
+    float q0 = pe[4 * Q], q1 = pe[4 * Q + 1], q2 = pe[4 * Q + 2], q3 = pe[4 * Q + 3];
+    if (hi - lo != 3) {   // partial quad: out-of-window points get a zero residual
+        const unsigned span = static_cast<unsigned>(hi - lo);
+        if (static_cast<unsigned>(4 * Q - lo) > span) { e0 = 0.f; q0 = 0.f; }
+        if (static_cast<unsigned>(4 * Q + 1 - lo) > span) { e1 = 0.f; q1 = 0.f; }
+        if (static_cast<unsigned>(4 * Q + 2 - lo) > span) { e2 = 0.f; q2 = 0.f; }
+        if (static_cast<unsigned>(4 * Q + 3 - lo) > span) { e3 = 0.f; q3 = 0.f; }
+    }
+    if (core) {
+        bwd_pair<true>(e0, e1, q0, q1, t_0, t_1, a);
+        bwd_pair<true>(e2, e3, q2, q3, t_2, t_3, a);
+    } else {
+        bwd_pair<false>(e0, e1, q0, q1, t_0, t_1, a);
+        bwd_pair<false>(e2, e3, q2, q3, t_2, t_3, a);
+    }
 }
 
 // Fixed-tree reduction of 8 per-lane values over the 32 lanes; lane c < 8 returns the total of v[c].
@@ -353,44 +378,98 @@ __device__ __forceinline__ float warp_reduce8(float (&v)[8]) {
     return __shfl_sync(0xffffffffu, w1, src);
 }
 
+// Warp-uniform geometry of a window-edge (peak, tile) pair in tile coordinates.
+__device__ __forceinline__ PeakGeo edge_geo(int dj, int ngc, int n_c, int plim) {
+    PeakGeo g;
+    g.p_lo = dj - n_c;
+    g.p_hi = min(dj + n_c, plim);
+    g.c_lo = dj - ngc;
+    g.c_hi = dj + ngc;
+    return g;
+}
+
 // ------------------------------------------------------------------------------------------------
 // a-3 .. a-6 (likelihood part): fused profile + residual + backward.
-// grid (n_seg, G), block 32*TW*PS; segment = 16*TW consecutive grid points.  Phase 1: warp w owns tile
-// (w % TW) of the segment and share (w / TW) of the PS equal shares of that tile's peak list; the PS partial
-// profiles are summed through shared memory in a fixed order.  Phase 2: warp w owns the peak range
-// warp_rng[seg][w] of the segment's phase-major list.
+// grid (n_seg, G), block 32*TW*PS; segment = TW consecutive 16-point tiles.  Warp w owns tile (w % TW) of the
+// segment and share (w / TW) of that tile's phase runs, in BOTH phases.  A run = the peaks of one phase that
+// reach the tile; its header carries the phase, so the per-phase latents are loaded once per run (prefetched one
+// run ahead) and the run index is the output slot of phase 2.
+#ifndef XRDVI_TILE_WARPS_PER_SM
+#define XRDVI_TILE_WARPS_PER_SM 24          // register budget: 65536 / (32 * 24) = 85 -> 80 registers per thread
+#endif
 template <int TW, int PS, bool BWD>
-__global__ void __launch_bounds__(32 * TW * PS) elbo_tile_kernel(const Dev d, float* __restrict__ f_dbg, long long n_dbg) {
-    constexpr int NW = TW * PS;
-    __shared__ float4 e_s[4 * TW][32];
+__global__ void __launch_bounds__(32 * TW * PS, XRDVI_TILE_WARPS_PER_SM / (TW * PS) > 0 ? XRDVI_TILE_WARPS_PER_SM / (TW * PS) : 1)
+elbo_tile_kernel(const Dev d, float* __restrict__ f_dbg, long long n_dbg) {
+    __shared__ float4 e_s[TW][kPT / 4][32];
     __shared__ float ss_s[TW][32];
     __shared__ float acc_s[PS > 1 ? (PS - 1) * TW * kPT : 1][32];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const int tw = w % TW, ps = w / TW;
     const int seg = d.seg_order[blockIdx.x];
     const int g = blockIdx.y;
-    const int seg0 = seg * (kPT * TW);
-    const int i0 = seg0 + kPT * tw;
+    const int tile = seg * TW + tw;
+    const int i0 = tile * kPT;
+    const bool live = tile < d.n_tile;                      // the last segment may have fewer than TW tiles
+    const int plim = min(kPT - 1, d.N - 1 - i0);            // last valid point of the tile
+    const int n_c = d.n_c;
     const float4* __restrict__ lat = d.lat + static_cast<size_t>(g) * d.K * 32 + lane;
     const int* __restrict__ ngk = d.ng + static_cast<size_t>(g) * d.K;
+    const PeakRec* __restrict__ pkt = d.pk_tile;
+    const int4* __restrict__ runs = d.run_tab;
     const int inst = g / d.gpi;
     const int pat = inst / d.R;
     const PatConst pc = d.pat[pat];
+    int2 rng = make_int2(0, 0);
+    if (live) rng = d.share_rng[tile * PS + ps];
 
     // ---------------- phase 1: profile on the 16 points of this warp's tile ----------------
     float acc[kPT];
 #pragma unroll
     for (int p = 0; p < kPT; ++p) acc[p] = 0.0f;
 
-    if (i0 < d.N) {
-        // tile_rng = (lo, full_lo, full_hi, hi): [lo, full_lo) and [full_hi, hi) reach only part of the tile
-        const int4 rng = d.tile_rng[i0 / kPT];
-        const int n = rng.w - rng.x;
-        const int a = rng.x + static_cast<int>(static_cast<long long>(n) * ps / PS);
-        const int b = rng.x + static_cast<int>(static_cast<long long>(n) * (ps + 1) / PS);
-        fwd_peaks<true>(d, lat, ngk, a, min(b, rng.y), i0, acc);
-        fwd_peaks<false>(d, lat, ngk, max(a, rng.y), min(b, rng.z), i0, acc);
-        fwd_peaks<true>(d, lat, ngk, max(a, rng.z), b, i0, acc);
+    if (rng.x < rng.y) {
+        int4 run_n = runs[rng.x];
+        float4 lt_n = lat[static_cast<size_t>(run_n.z) * 32];
+        int ng_n = ngk[run_n.z];
+        for (int r = rng.x; r < rng.y; ++r) {
+            const int4 run = run_n;
+            const float4 lt = lt_n;
+            const int ngc = ng_n;
+            run_n = runs[r + 1];                            // run_tab and pk_tile carry one padding entry
+            lt_n = lat[static_cast<size_t>(run_n.z) * 32];
+            ng_n = ngk[run_n.z];
+            const float step = d.delta * lt.x;
+            const unsigned core_span = static_cast<unsigned>(kPT - 1 + 2 * ngc);
+            PeakRec pk_n = pkt[run.x];
+            for (int m = run.x; m < run.y; ++m) {
+                const PeakRec pk = pk_n;
+                pk_n = pkt[m + 1];
+                const float t0 = fmaf(static_cast<float>(-pk.dj), step, fmaf(-pk.delta, lt.x, lt.y));
+                const float cl = pk.inten * lt.w;
+                const bool core = static_cast<unsigned>(pk.dj + ngc) <= core_span;   // Gaussian core touches the tile
+                if (pk.full) {   // branch-free bodies: Lorentz tail only, or tail + Gaussian on all 16 points
+                    if (!core) {
+#pragma unroll
+                        for (int p = 0; p < kPT; p += 2)
+                            fwd_pair<false>(fmaf(static_cast<float>(p), step, t0), fmaf(static_cast<float>(p + 1), step, t0),
+                                            0.0f, cl, acc[p], acc[p + 1]);
+                    } else {
+                        const float cg2 = 2.0f * pk.inten * lt.z;
+#pragma unroll
+                        for (int p = 0; p < kPT; p += 2)
+                            fwd_pair<true>(fmaf(static_cast<float>(p), step, t0), fmaf(static_cast<float>(p + 1), step, t0),
+                                           cg2, cl, acc[p], acc[p + 1]);
+                    }
+                } else {         // window edge: quad by quad
+                    const PeakGeo geo = edge_geo(pk.dj, ngc, n_c, plim);
+                    const float cg2 = 2.0f * pk.inten * lt.z;
+                    fwd_quad_generic<0>(geo, t0, step, cg2, cl, acc);
+                    fwd_quad_generic<1>(geo, t0, step, cg2, cl, acc);
+                    fwd_quad_generic<2>(geo, t0, step, cg2, cl, acc);
+                    fwd_quad_generic<3>(geo, t0, step, cg2, cl, acc);
+                }
+            }
+        }
     }
     if (PS > 1) {   // sum the PS partial profiles of the tile: shares 1.. in order onto share 0
         if (ps > 0) {
@@ -406,16 +485,15 @@ __global__ void __launch_bounds__(32 * TW * PS) elbo_tile_kernel(const Dev d, fl
         }
     }
 
-    // residual, e = (y - f)/sigma_n^2, partial sum of ((y - f)/sigma_n)^2
+    // residual e = (y - f)/sigma_n^2 (0 beyond the grid), partial sum of ((y - f)/sigma_n)^2
     if (ps == 0) {
         const float* __restrict__ yb = d.yb + static_cast<size_t>(pat) * d.N;
         float ev[kPT];
         float ss = 0.0f;
 #pragma unroll
         for (int p = 0; p < kPT; ++p) {
-            const int i = i0 + p;
             float r = 0.0f;
-            if (i < d.N) r = yb[i] - acc[p];
+            if (p <= plim) r = yb[i0 + p] - acc[p];         // plim < 0 for a dead tile
             const float z = r * pc.inv_sn;
             ss = fmaf(z, z, ss);
             ev[p] = r * pc.inv_sn2;
@@ -423,17 +501,17 @@ __global__ void __launch_bounds__(32 * TW * PS) elbo_tile_kernel(const Dev d, fl
         if (BWD) {
 #pragma unroll
             for (int v = 0; v < kPT / 4; ++v)
-                e_s[4 * tw + v][lane] = make_float4(ev[4 * v], ev[4 * v + 1], ev[4 * v + 2], ev[4 * v + 3]);
+                e_s[tw][v][lane] = make_float4(ev[4 * v], ev[4 * v + 1], ev[4 * v + 2], ev[4 * v + 3]);
         }
         ss_s[tw][lane] = ss;
-        if (f_dbg && i0 < d.N) {  // debug read-back of the profile (parity tests); warp-uniform branch
+        if (f_dbg && live) {  // debug read-back of the profile (parity tests); warp-uniform branch
             const int s = (g - inst * d.gpi) * 32 + lane;
             const long long t = static_cast<long long>(inst) * d.S + s;
             if (s < d.S && t < n_dbg) {
                 const float* __restrict__ bg = d.bg + static_cast<size_t>(pat) * d.N;
 #pragma unroll
                 for (int p = 0; p < kPT; ++p)
-                    if (i0 + p < d.N) f_dbg[t * d.N + i0 + p] = acc[p] + bg[i0 + p];
+                    if (p <= plim) f_dbg[t * d.N + i0 + p] = acc[p] + bg[i0 + p];
             }
         }
     }
@@ -445,110 +523,88 @@ __global__ void __launch_bounds__(32 * TW * PS) elbo_tile_kernel(const Dev d, fl
         d.llpart[(static_cast<size_t>(g) * d.n_seg + seg) * 32 + lane] = ss;
     }
     if (!BWD) return;
+    if (rng.x >= rng.y) return;
 
-    // ---------------- phase 2: six sums over the segment, chain rule, reduction over the draws ----------------
-    const int4 wr = d.warp_rng[seg * NW + w];
-    if (wr.x >= wr.y) return;
-    const int seg_hi = min(seg0 + kPT * TW - 1, d.N - 1);
+    // ---------------- phase 2: six sums per phase run over the tile, chain rule, reduction over the draws ----------------
+    float e[kPT], pe[kPT];
+#pragma unroll
+    for (int v = 0; v < kPT / 4; ++v) {
+        const float4 t = e_s[tw][v][lane];
+        e[4 * v] = t.x; e[4 * v + 1] = t.y; e[4 * v + 2] = t.z; e[4 * v + 3] = t.w;
+    }
+#pragma unroll
+    for (int p = 0; p < kPT; ++p) pe[p] = static_cast<float>(p) * e[p];
+
     const float4* __restrict__ epsg = d.eps + static_cast<size_t>(g) * d.K * 32 + lane;
     const float* __restrict__ rrg = d.rr + static_cast<size_t>(g) * d.K * 32 + lane;
     float* __restrict__ part = d.part8 + static_cast<size_t>(g) * d.n_slots * 8;
-    int slot = wr.z;
-    int cur_k = -1;
-    float4 lt = make_float4(0.f, 0.f, 0.f, 0.f);
-    float step = 0.0f;
-    int ngc = 0;
-    float B1 = 0.f, B2 = 0.f, B3 = 0.f, B4 = 0.f, B5 = 0.f, B6 = 0.f;
 
-    auto flush = [&]() {
+    int4 run_n = runs[rng.x];
+    float4 lt_n = lat[static_cast<size_t>(run_n.z) * 32];
+    int ng_n = ngk[run_n.z];
+    for (int r = rng.x; r < rng.y; ++r) {
+        const int4 run = run_n;
+        const float4 lt = lt_n;
+        const int ngc = ng_n;
+        run_n = runs[r + 1];
+        lt_n = lat[static_cast<size_t>(run_n.z) * 32];
+        ng_n = ngk[run_n.z];
+        // loads of the flush, issued early
+        const float4 ep = epsg[static_cast<size_t>(run.z) * 32];
+        const float rmix = rrg[static_cast<size_t>(run.z) * 32];
+        const float step = d.delta * lt.x;
+        const unsigned core_span = static_cast<unsigned>(kPT - 1 + 2 * ngc);
+        // sums over the peaks of the run, I_m folded in:
+        //   B1 = sum I e L, B3 = sum I e L^2 t', B5 = sum I e L^2; B2 = sum I e G, B4 = sum I e G t', B6 = sum I e G t'^2
+        float B1 = 0.f, B2 = 0.f, B3 = 0.f, B4 = 0.f, B5 = 0.f, B6 = 0.f;
+        PeakRec pk_n = pkt[run.x];
+        for (int m = run.x; m < run.y; ++m) {
+            const PeakRec pk = pk_n;
+            pk_n = pkt[m + 1];
+            const float t0 = fmaf(static_cast<float>(-pk.dj), step, fmaf(-pk.delta, lt.x, lt.y));
+            const bool core = static_cast<unsigned>(pk.dj + ngc) <= core_span;
+            Acc6 a = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+            if (pk.full && !core) {
+#pragma unroll
+                for (int p = 0; p < kPT; p += 2)
+                    bwd_pair<false>(e[p], e[p + 1], pe[p], pe[p + 1], fmaf(static_cast<float>(p), step, t0),
+                                    fmaf(static_cast<float>(p + 1), step, t0), a);
+                B1 = fmaf(pk.inten, a.a1, B1);
+                B3 = fmaf(pk.inten, fmaf(t0, a.a5, step * a.a3p), B3);
+                B5 = fmaf(pk.inten, a.a5, B5);
+            } else {
+                if (pk.full) {
+#pragma unroll
+                    for (int p = 0; p < kPT; p += 2)
+                        bwd_pair<true>(e[p], e[p + 1], pe[p], pe[p + 1], fmaf(static_cast<float>(p), step, t0),
+                                       fmaf(static_cast<float>(p + 1), step, t0), a);
+                } else {
+                    const PeakGeo geo = edge_geo(pk.dj, ngc, n_c, plim);
+                    bwd_quad_generic<0>(geo, t0, step, e, pe, a);
+                    bwd_quad_generic<1>(geo, t0, step, e, pe, a);
+                    bwd_quad_generic<2>(geo, t0, step, e, pe, a);
+                    bwd_quad_generic<3>(geo, t0, step, e, pe, a);
+                }
+                const float i2 = 2.0f * pk.inten;           // g = G/2 in the Gaussian sums
+                B1 = fmaf(pk.inten, a.a1, B1);
+                B2 = fmaf(i2, a.a2, B2);
+                B3 = fmaf(pk.inten, fmaf(t0, a.a5, step * a.a3p), B3);
+                B4 = fmaf(i2, fmaf(t0, a.a2, step * a.a4p), B4);
+                B5 = fmaf(pk.inten, a.a5, B5);
+                B6 = fmaf(i2, a.a6u - a.a2, B6);
+            }
+        }
         // chain rule for the likelihood part (per draw), then sum over the 32 draws of the group
-        const float4 ep = epsg[static_cast<size_t>(cur_k) * 32];
-        const float r = rrg[static_cast<size_t>(cur_k) * 32];
         const float cG = lt.z, cL = lt.w;
         float v[8];
         v[0] = fmaf(cL, B1, cG * B2);
         v[1] = lt.x * (2.0f * cL * B3 + (2.0f * kLn2) * cG * B4);
         v[2] = -(cL * (2.0f * B5 - B1) + cG * (B2 - (2.0f * kLn2) * B6));
-        v[3] = (1.0f - r) * cL * B1 - r * cG * B2;
+        v[3] = (1.0f - rmix) * cL * B1 - rmix * cG * B2;
         v[4] = v[0] * ep.x; v[5] = v[1] * ep.y; v[6] = v[2] * ep.z; v[7] = v[3] * ep.w;
         const float tot = warp_reduce8(v);
-        if (lane < 8) part[static_cast<size_t>(slot) * 8 + lane] = tot;
-    };
-
-    PeakRec pk_n = d.pk_bwd[wr.x];
-    for (int m = wr.x; m < wr.y; ++m) {
-        const PeakRec pk = pk_n;
-        if (m + 1 < wr.y) pk_n = d.pk_bwd[m + 1];
-        if (pk.k != cur_k) {   // new phase run (warp-uniform)
-            if (cur_k >= 0) { flush(); ++slot; }
-            cur_k = pk.k;
-            lt = lat[static_cast<size_t>(cur_k) * 32];
-            step = d.delta * lt.x;
-            ngc = ngk[cur_k];
-            B1 = B2 = B3 = B4 = B5 = B6 = 0.f;
-        }
-        const int lo = max(seg0, pk.j - d.n_c), hi = min(seg_hi, pk.j + d.n_c);   // lo <= hi by construction
-        const float tc = fmaf(-pk.delta, lt.x, lt.y);
-        const float tseg = fmaf(static_cast<float>(seg0 - pk.j), step, tc);       // t' at the first point of the segment
-        const float step4 = 4.0f * step;
-        int ql = (lo - seg0) >> 2, qh = (hi - seg0) >> 2;                         // local quads [ql, qh]
-        const int c_lo = pk.j - ngc, c_hi = pk.j + ngc;                           // Gaussian core [c_lo, c_hi]
-        Acc6 a = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-        // ragged window ends: quads whose points are partly outside [lo, hi] get their e zeroed there
-        const bool rag_lo = (lo & 3) != 0, rag_hi = ((hi + 1) & 3) != 0;
-        if (rag_lo || (rag_hi && ql == qh)) {
-            float4 e4 = e_s[ql][lane];
-            const int ib = seg0 + 4 * ql;
-            if (ib + 0 < lo || ib + 0 > hi) e4.x = 0.f;
-            if (ib + 1 < lo || ib + 1 > hi) e4.y = 0.f;
-            if (ib + 2 < lo || ib + 2 > hi) e4.z = 0.f;
-            if (ib + 3 < lo || ib + 3 > hi) e4.w = 0.f;
-            const float tq = fmaf(static_cast<float>(4 * ql), step, tseg);
-            if (ib + 3 >= c_lo && ib <= c_hi) bwd_quad<true>(e4, tq, step, a);
-            else bwd_quad<false>(e4, tq, step, a);
-            ++ql;
-        }
-        if (rag_hi && ql <= qh) {
-            float4 e4 = e_s[qh][lane];
-            const int ib = seg0 + 4 * qh;
-            if (ib + 1 > hi) e4.y = 0.f;
-            if (ib + 2 > hi) e4.z = 0.f;
-            if (ib + 3 > hi) e4.w = 0.f;
-            const float tq = fmaf(static_cast<float>(4 * qh), step, tseg);
-            if (ib + 3 >= c_lo && ib <= c_hi) bwd_quad<true>(e4, tq, step, a);
-            else bwd_quad<false>(e4, tq, step, a);
-            --qh;
-        }
-        if (ql <= qh) {
-            // split [ql, qh] into tail | core | tail at quad granularity
-            int qc0 = (max(c_lo, seg0) - seg0) >> 2, qc1 = (min(c_hi, seg_hi) - seg0) >> 2;
-            if (c_hi < seg0 + 4 * ql || c_lo > seg0 + 4 * qh + 3) { qc0 = qh + 1; qc1 = qh; }  // no core quad
-            qc0 = max(qc0, ql);
-            qc1 = min(qc1, qh);
-            float tq = fmaf(static_cast<float>(4 * ql), step, tseg);
-            int q = ql;
-            for (; q < qc0; ++q) {
-                bwd_quad<false>(e_s[q][lane], tq, step, a);
-                tq += step4;
-            }
-            for (; q <= qc1; ++q) {
-                bwd_quad<true>(e_s[q][lane], tq, step, a);
-                tq += step4;
-            }
-            if (qc1 >= qc0) tq = fmaf(static_cast<float>(4 * q), step, tseg);   // re-anchor after the core
-            for (; q <= qh; ++q) {
-                bwd_quad<false>(e_s[q][lane], tq, step, a);
-                tq += step4;
-            }
-        }
-        B1 = fmaf(pk.inten, a.a1, B1);
-        B2 = fmaf(pk.inten, a.a2, B2);
-        B3 = fmaf(pk.inten, a.a3, B3);
-        B4 = fmaf(pk.inten, a.a4, B4);
-        B5 = fmaf(pk.inten, a.a5, B5);
-        B6 = fmaf(pk.inten, a.a6, B6);
+        if (lane < 8) part[static_cast<size_t>(r) * 8 + lane] = tot;
     }
-    flush();
 }
 
 // ------------------------------------------------------------------------------------------------
