@@ -14,7 +14,8 @@
  *             rho_mk = p_m + mu_k                         PAPER.md:204-232 (A3-A8)
  *   G, L      bodies missing from PAPER.md -> unit-area FWHM forms (reading R1)
  *   window    static integer window |i - j_m| <= n_c       (reading R16; W<=0 -> dense)
- *   ll        Gaussian, known sigma_n                      (reading R3; paper: Poisson A12-A16)
+ *   ll        Gaussian, known sigma_n (reading R3, the graded path) or, hyper.likelihood = 1,
+ *             the paper's Poisson likelihood A12-A16 PAPER.md:247-261 (R24: y_i >= 0, f_i > 0)
  *   priors    h~Exp(lambda_h) eq.(3); mu~N(0,0.03), w~Gam(3,rate), r~U(0,1)
  *             PAPER.md:274 (B.2); rate reading of "scale" (R12)
  *   q         mean-field Gaussian in unconstrained space, eq.(10) PAPER.md:131 (R6)
@@ -26,7 +27,9 @@
  * Pins (tests/test_oracle_pins.py): unit area and half-height of G/L/V, normal/Cauchy pdf
  * special cases, zero-inclusion, shift and dummy-peak invariances, linearity in h, direct
  * normal log-pdf, closed-form prior-only ELBO, Philox known-answer vectors, central finite
- * differences of the fixed-draw ELBO, first Adam step, brute force over 2^K subsets.
+ * differences of the fixed-draw ELBO, first Adam step, brute force over 2^K subsets
+ * (tests/test_bruteforce_subsets.py); Poisson: scipy logpmf sum, finite differences, count-data fit
+ * (tests/test_poisson_pins.py).
  * Unpinned: the absolute ELBO as a bound on ln p(Y) ("parity unpinned" for that reading only).
  *
  * Layouts: state[P][R][2][K][4] doubles: [0]=m (variational mean), [1]=l (log sigma);
@@ -52,6 +55,8 @@ typedef struct {
     double lr, beta1, beta2, adam_eps;
     double init_log_sigma;
     int32_t n_patterns, n_restarts;
+    int32_t likelihood;    /* 0 Gaussian with known sigma_n (R3); 1 Poisson, A12-A16 PAPER.md:247-261 (R24) */
+    int32_t pad_;
 } orc_hyper;
 
 typedef struct {
@@ -231,9 +236,18 @@ void orc_profile(const orc_problem *q, int32_t pat, const double *zeta /*[K][4]*
     }
 }
 
-/* ll = -1/2 sum_i ((y_i - f_i)/sigma_n)^2 - N ln sigma_n - (N/2) ln 2 pi */
+/* Gaussian (R3):  ll = -1/2 sum_i ((y_i - f_i)/sigma_n)^2 - N ln sigma_n - (N/2) ln 2 pi
+ * Poisson (A16; R24):  ll = sum_i { y_i ln f_i - f_i - ln y_i! },  ln y! = lgamma(y + 1) */
 double orc_loglik(const orc_problem *q, int32_t pat, const double *f) {
     const int64_t N = q->N;
+    if (q->hy.likelihood == 1) {
+        double acc = 0.0;
+        for (int64_t i = 0; i < N; ++i) {
+            double y = q->y[pat * N + i];
+            acc += y * log(f[i]) - f[i] - lgamma(y + 1.0);
+        }
+        return acc;
+    }
     double sn = q->sigma_n[pat], acc = 0.0;
     for (int64_t i = 0; i < N; ++i) {
         double z = (q->y[pat * N + i] - f[i]) / sn;
@@ -278,7 +292,9 @@ void orc_logjoint_grad(const orc_problem *q, int32_t pat, const double *zeta, do
             int64_t i_lo, i_hi;
             window(q, m, &i_lo, &i_hi);
             for (int64_t i = i_lo; i <= i_hi; ++i) {
-                double e = (q->y[pat * N + i] - f[i]) / (sn * sn);          /* d ll / d f_i */
+                double e = q->hy.likelihood == 1
+                               ? q->y[pat * N + i] / f[i] - 1.0                  /* d ll / d f_i of A16    */
+                               : (q->y[pat * N + i] - f[i]) / (sn * sn);        /* d ll / d f_i, Gaussian */
                 double t = (q->x[i] - rho) / w;
                 double G = exp(-4.0 * LN2 * t * t), L = 1.0 / (1.0 + 4.0 * t * t);
                 double Gn = (aG / w) * G, Ln = (aL / w) * L;                 /* unit-area values */

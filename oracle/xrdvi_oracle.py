@@ -30,12 +30,13 @@ class OrcHyper(C.Structure):
         ("lr", C.c_double), ("beta1", C.c_double), ("beta2", C.c_double), ("adam_eps", C.c_double),
         ("init_log_sigma", C.c_double),
         ("n_patterns", C.c_int32), ("n_restarts", C.c_int32),
+        ("likelihood", C.c_int32), ("pad_", C.c_int32),
     ]
 
 
 DEFAULTS = dict(lambda_h=0.0, mu_sigma=0.03, w_shape=3.0, w_rate=100.0, noise_sigma=0.0,
                 window_W=10.0, fwhm_ref=0.15, incl_tau=0.01, lr=0.1, beta1=0.9, beta2=0.999,
-                adam_eps=1e-8, init_log_sigma=float(np.log(0.1)), n_patterns=1, n_restarts=1)
+                adam_eps=1e-8, init_log_sigma=float(np.log(0.1)), n_patterns=1, n_restarts=1, likelihood=0)
 
 _lib = None
 

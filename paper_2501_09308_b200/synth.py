@@ -94,9 +94,14 @@ _SPEC = {
 
 
 def make_workload(cfg: int, n_patterns: int | None = None, n_restarts: int | None = None,
-                  S: int | None = None, K: int | None = None, seed: int | None = None) -> Workload:
+                  S: int | None = None, K: int | None = None, seed: int | None = None,
+                  peak_counts: float | None = None) -> Workload:
     """Build config ``cfg`` (0..4).  Optional overrides shrink a config for tests
-    (e.g. ``n_patterns=4`` for cfg 3) without changing its per-pattern recipe."""
+    (e.g. ``n_patterns=4`` for cfg 3) without changing its per-pattern recipe.
+
+    ``peak_counts``: COUNT data for the paper's Poisson likelihood: signal + background
+    are scaled so that their maximum is ``peak_counts`` and y ~ Poisson(signal + background) replaces the
+    Gaussian noise; the planted scales h are multiplied by the same factor and ``hyper['likelihood'] = 1``."""
     if cfg not in _SPEC:
         raise ValueError(f"unknown config {cfg}")
     (K0, (mlo, mhi), N, lo, hi, P0, R0, S0, its, W, fwhm_ref, (fw_lo, fw_hi), (w_shape, w_rate)) = _SPEC[cfg]
@@ -166,10 +171,18 @@ def make_workload(cfg: int, n_patterns: int | None = None, n_restarts: int | Non
         b1 = rng.uniform(-0.5, 0.5) * b0 / (hi - lo)
         bg[pat] = b0 + b1 * (x - lo)
         sigma_n = 0.01 * smax
-        y[pat] = sig + bg[pat] + rng.normal(0.0, sigma_n, size=N)
+        if peak_counts is None:
+            y[pat] = sig + bg[pat] + rng.normal(0.0, sigma_n, size=N)
+        else:
+            c = float(peak_counts) / float((sig + bg[pat]).max())
+            bg[pat] *= c
+            y[pat] = rng.poisson(c * sig + bg[pat]).astype(np.float64)
+            true_params[pat] = {k: (h * c, sh, fw, mix) for k, (h, sh, fw, mix) in true_params[pat].items()}
 
     hyper = dict(window_W=W, fwhm_ref=fwhm_ref, w_shape=w_shape, w_rate=w_rate,
                  n_patterns=P, n_restarts=R)
+    if peak_counts is not None:
+        hyper["likelihood"] = 1
     return Workload(cfg=cfg, two_theta=x, y=y, background=bg, peak_ofs=peak_ofs,
                     peak_pos=peak_pos, peak_int=peak_int, hyper=hyper, S=S, iterations=its,
                     true_phases=true_phases, true_params=true_params)
