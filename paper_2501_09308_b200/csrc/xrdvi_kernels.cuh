@@ -61,7 +61,9 @@ struct PatConst {  // per observed pattern
     float inv_sn2;     // 1/sigma_n^2
     float lambda_h;    // rate of the Exp prior
     float log_lambda_h;
-    double ll_const;   // -N ln sigma_n - N/2 ln 2pi
+    double ll_const;   // Gaussian: -N ln sigma_n - N/2 ln 2pi;  Poisson: sum_i (y ln y - y - ln y!)
+    float ll_scale;    // ll = ll_scale * (sum of llpart) + ll_const: -1/2 (Gaussian), 1 (Poisson)
+    float pad;
 };
 
 struct Ctl {       // device-resident control block (so that graph replays need no new arguments)
@@ -77,6 +79,7 @@ struct Dev {
     // sizes
     int N, K, P, R, PR, n_c, SP, n_seg, n_tile, n_slots, Mv, TW, PS;
     int S, gpi, G;       // draws, groups per instance, groups (run-time)
+    int likelihood;      // 0 Gaussian with known sigma_n (R3), 1 Poisson (A12-A16; R24)
     float delta;         // grid step (deg)
     float gcut;          // kGaussCut / (2 Delta): core half-width in points per unit of w
     float inv_delta;
@@ -485,18 +488,40 @@ elbo_tile_kernel(const Dev d, float* __restrict__ f_dbg, long long n_dbg) {
         }
     }
 
-    // residual e = (y - f)/sigma_n^2 (0 beyond the grid), partial sum of ((y - f)/sigma_n)^2
+    // residual e = d ll / d f (0 beyond the grid) and the tile's part of ll:
+    //   Gaussian (R3):  e = (y - f)/sigma_n^2,  part = sum ((y - f)/sigma_n)^2            (ll = -1/2 sum + const)
+    //   Poisson (A16):  e = y/f - 1,            part = sum y ln(f/y) + (y - f)  (-f if y = 0)   (ll = sum + const)
     if (ps == 0) {
         const float* __restrict__ yb = d.yb + static_cast<size_t>(pat) * d.N;
         float ev[kPT];
         float ss = 0.0f;
+        if (d.likelihood == 0) {
 #pragma unroll
-        for (int p = 0; p < kPT; ++p) {
-            float r = 0.0f;
-            if (p <= plim) r = yb[i0 + p] - acc[p];         // plim < 0 for a dead tile
-            const float z = r * pc.inv_sn;
-            ss = fmaf(z, z, ss);
-            ev[p] = r * pc.inv_sn2;
+            for (int p = 0; p < kPT; ++p) {
+                float r = 0.0f;
+                if (p <= plim) r = yb[i0 + p] - acc[p];         // plim < 0 for a dead tile
+                const float z = r * pc.inv_sn;
+                ss = fmaf(z, z, ss);
+                ev[p] = r * pc.inv_sn2;
+            }
+        } else {
+            const float* __restrict__ bgp = d.bg + static_cast<size_t>(pat) * d.N;
+#pragma unroll
+            for (int p = 0; p < kPT; ++p) {
+                ev[p] = 0.0f;
+                if (p <= plim) {
+                    const float b = bgp[i0 + p], ymb = yb[i0 + p];
+                    const float yv = ymb + b, f = acc[p] + b;   // y and f = S_F + B (A3)
+                    const float diff = ymb - acc[p];            // y - f
+                    ev[p] = diff / f;
+                    if (yv > 0.0f) {
+                        const float x = -diff / yv;             // f/y - 1
+                        ss = fmaf(yv, log1pf(x) - x, ss);
+                    } else {
+                        ss -= f;
+                    }
+                }
+            }
         }
         if (BWD) {
 #pragma unroll
@@ -658,7 +683,7 @@ __global__ void __launch_bounds__(kUpdThreads) update_draw_kernel(const Dev d, c
             const float* __restrict__ lp = d.llpart + static_cast<size_t>(g) * d.n_seg * 32 + lane;
             double a = 0.0;
             for (int t = 0; t < d.n_seg; ++t) a += static_cast<double>(lp[static_cast<size_t>(t) * 32]);
-            const double ll = -0.5 * a + pc.ll_const;
+            const double ll = static_cast<double>(pc.ll_scale) * a + pc.ll_const;
             d.ll_t[static_cast<size_t>(inst) * d.gpi * 32 + s] = ll;
             v[0] += ll;
         }

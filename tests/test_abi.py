@@ -76,7 +76,7 @@ def test_create_rejects_bad_arguments_before_touching_cuda(lib):
     assert create(x=xn) == -3
     assert create(ofs=np.array([0, 0, 4], dtype=np.int64)) == -4
     assert create(inten=np.array([1.0, -2.0, 3.0, 4.0])) == -1
-    hb = binding.default_hyper(likelihood=1)
+    hb = binding.default_hyper(likelihood=2)          # 0 Gaussian and 1 Poisson are the only likelihoods
     assert create(hy=hb) == -1
     assert out.value is None
 

@@ -199,3 +199,45 @@ def test_error_paths_on_device():
         gpu.elbo_grad(S=wl.S + 64)
     with pytest.raises(XrdviError):
         gpu.fit(-1)
+
+
+# --------------------------------------------------------------------------- Poisson likelihood (A12-A16)
+def test_poisson_config0_all_states_and_fit():
+    wl = synth.make_workload(0, peak_counts=2.0e4)
+    o = orc.from_workload(wl)
+    gpu = Xrdvi.from_workload(wl)
+    st0, _ = gpu.get_state()
+    np.testing.assert_allclose(st0, o.init_state(), rtol=1e-6)
+    check_eval(gpu, o, st0, wl.S, seed=3, iteration=1, n_prof=16)
+    st_g, inc_g, tr_g = gpu.fit(500, seed=3, want_trace=True)
+    check_eval(gpu, o, st_g, wl.S, seed=3, iteration=501, n_prof=16)
+    st_r, _, tr_r = o.fit(o.init_state(), 500, wl.S, seed=3, want_trace=True)
+    np.testing.assert_allclose(tr_g[:3], tr_r[:3], rtol=TOL_ELBO)
+    assert np.abs(inc_g - o.inclusion(st_r)).max() <= TOL_INCL
+    for k in wl.true_phases[0]:
+        np.testing.assert_allclose(st_g[0, 0, 0, k, :3], st_r[0, 0, 0, k, :3], atol=0.02)
+
+
+def test_poisson_config1_reduced_draws_and_zero_counts():
+    wl = synth.make_workload(1, S=64, peak_counts=300.0)          # low counts: many y = 0 points
+    assert (wl.y == 0).sum() > 10
+    o = orc.from_workload(wl)
+    gpu = Xrdvi.from_workload(wl)
+    st0, _ = gpu.get_state()
+    check_eval(gpu, o, st0, 64, seed=1, iteration=1)
+    gpu.fit(100, seed=1)
+    st, _ = gpu.get_state()
+    check_eval(gpu, o, st, 64, seed=1, iteration=101)
+
+
+def test_poisson_rejects_non_positive_background():
+    from paper_2501_09308_b200 import XrdviError
+    wl = synth.make_workload(0, peak_counts=1.0e3)
+    bg = wl.background.copy()
+    bg[0, 17] = 0.0
+    with pytest.raises(XrdviError):
+        Xrdvi(wl.two_theta, wl.y, bg, wl.peak_ofs, wl.peak_pos, wl.peak_int, S_max=4, **wl.hyper)
+    y = wl.y.copy()
+    y[0, 5] = -1.0
+    with pytest.raises(XrdviError):
+        Xrdvi(wl.two_theta, y, wl.background, wl.peak_ofs, wl.peak_pos, wl.peak_int, S_max=4, **wl.hyper)
