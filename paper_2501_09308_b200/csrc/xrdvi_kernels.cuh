@@ -49,7 +49,7 @@ constexpr float kAG = 0.93943727869965132f;  // 2 sqrt(ln2/pi)
 constexpr float kAL = 0.63661977236758134f;  // 2/pi
 constexpr float kLn2 = 0.69314718055994531f;
 
-struct PeakRec {   // 16 bytes; one record per (peak, 16-point tile its window reaches)
+struct __align__(16) PeakRec {   // 16 bytes (one LDG.128); one record per (peak, 16-point tile its window reaches)
     int dj;        // nearest grid index j_m of the peak minus the first grid index of the tile
     float delta;   // p_m - x_{j_m}  (|delta| <= Delta/2), fp64-computed
     float inten;   // I_m
@@ -443,10 +443,9 @@ elbo_tile_kernel(const Dev d, float* __restrict__ f_dbg, long long n_dbg) {
             ng_n = ngk[run_n.z];
             const float step = d.delta * lt.x;
             const unsigned core_span = static_cast<unsigned>(kPT - 1 + 2 * ngc);
-            PeakRec pk_n = pkt[run.x];
+#pragma unroll 1
             for (int m = run.x; m < run.y; ++m) {
-                const PeakRec pk = pk_n;
-                pk_n = pkt[m + 1];
+                const PeakRec pk = pkt[m];
                 const float t0 = fmaf(static_cast<float>(-pk.dj), step, fmaf(-pk.delta, lt.x, lt.y));
                 const float cl = pk.inten * lt.w;
                 const bool core = static_cast<unsigned>(pk.dj + ngc) <= core_span;   // Gaussian core touches the tile
@@ -582,10 +581,9 @@ elbo_tile_kernel(const Dev d, float* __restrict__ f_dbg, long long n_dbg) {
         // sums over the peaks of the run, I_m folded in:
         //   B1 = sum I e L, B3 = sum I e L^2 t', B5 = sum I e L^2; B2 = sum I e G, B4 = sum I e G t', B6 = sum I e G t'^2
         float B1 = 0.f, B2 = 0.f, B3 = 0.f, B4 = 0.f, B5 = 0.f, B6 = 0.f;
-        PeakRec pk_n = pkt[run.x];
+#pragma unroll 1
         for (int m = run.x; m < run.y; ++m) {
-            const PeakRec pk = pk_n;
-            pk_n = pkt[m + 1];
+            const PeakRec pk = pkt[m];
             const float t0 = fmaf(static_cast<float>(-pk.dj), step, fmaf(-pk.delta, lt.x, lt.y));
             const bool core = static_cast<unsigned>(pk.dj + ngc) <= core_span;
             Acc6 a = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
