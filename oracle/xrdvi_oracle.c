@@ -20,7 +20,8 @@
  *             PAPER.md:274 (B.2); rate reading of "scale" (R12)
  *   q         mean-field Gaussian in unconstrained space, eq.(10) PAPER.md:131 (R6)
  *   ELBO      eq.(7) PAPER.md:111 as MC mean + analytic entropy (R7), pathwise gradient (R8)
- *   optimiser Adam ascent, "1000 optimization steps" PAPER.md:138 (R10)
+ *   optimiser Adam ascent, "1000 optimization steps" PAPER.md:138 (R10); hyper.optimizer = 1:
+ *             natural-gradient ascent (R25; north_star names both)
  *   inclusion closed form from (m, l), 1 % area threshold PAPER.md:140 (R15)
  *   draws     Philox4x32-10, counter (iter, s, k, inst), key (seed_lo, seed_hi) (R18)
  *
@@ -56,7 +57,7 @@ typedef struct {
     double init_log_sigma;
     int32_t n_patterns, n_restarts;
     int32_t likelihood;    /* 0 Gaussian with known sigma_n (R3); 1 Poisson, A12-A16 PAPER.md:247-261 (R24) */
-    int32_t pad_;
+    int32_t optimizer;     /* 0 Adam (R10); 1 natural-gradient ascent of the mean-field Gaussian (R25)       */
 } orc_hyper;
 
 typedef struct {
@@ -400,6 +401,25 @@ void orc_adam_step(const orc_problem *q, double *state, const double *grad, doub
     }
 }
 
+/* R25: natural-gradient ascent.  The Fisher information of q = N(m, sigma^2) in the coordinates
+ * (m, l = ln sigma) is diag(1/sigma^2, 2), so one step is
+ *     m <- m + lr sigma^2 dELBO/dm,     l <- l + lr (dELBO/dl) / 2,   l clamped to [-12, 2],
+ * with sigma taken BEFORE the step.  No moments, no bias correction. */
+void orc_natgrad_step(const orc_problem *q, double *state, const double *grad) {
+    const int64_t half = (int64_t)q->K * 4, per = 2 * half;
+    for (int32_t inst = 0; inst < q->P * q->R; ++inst) {
+        double *m = state + (size_t)inst * per, *l = m + half;
+        const double *gm = grad + (size_t)inst * per, *gl = gm + half;
+        for (int64_t j = 0; j < half; ++j) {
+            double sigma = exp(l[j]);
+            m[j] += q->hy.lr * sigma * sigma * gm[j];
+            l[j] += q->hy.lr * 0.5 * gl[j];
+            if (l[j] < -12.0) l[j] = -12.0;
+            if (l[j] > 2.0) l[j] = 2.0;
+        }
+    }
+}
+
 /* R11: m_h = ln(eta_h/K), m_mu = 0, m_w = ln(alpha_w/lambda_w), m_r = 0, l = init_log_sigma;
  * restart r > 0: m += (0.5, 0.01, 0.2, 0.5) * eps_init, eps_init = normals of Philox
  * ctr = (0xFFFFFFFF, r, k, pat) under the given seed. */
@@ -442,7 +462,8 @@ void orc_fit(const orc_problem *q, double *state, double *mom1, double *mom2, in
         int64_t step = first_step + it;
         orc_elbo_grad(q, state, S, seed, (uint64_t)step, elbo, grad, NULL, NULL, 0);
         if (elbo_trace) memcpy(elbo_trace + (size_t)it * q->P * q->R, elbo, sizeof(double) * q->P * q->R);
-        orc_adam_step(q, state, grad, mom1, mom2, step);
+        if (q->hy.optimizer == 1) orc_natgrad_step(q, state, grad);
+        else orc_adam_step(q, state, grad, mom1, mom2, step);
     }
     free(grad); free(elbo);
 }

@@ -30,13 +30,13 @@ class OrcHyper(C.Structure):
         ("lr", C.c_double), ("beta1", C.c_double), ("beta2", C.c_double), ("adam_eps", C.c_double),
         ("init_log_sigma", C.c_double),
         ("n_patterns", C.c_int32), ("n_restarts", C.c_int32),
-        ("likelihood", C.c_int32), ("pad_", C.c_int32),
+        ("likelihood", C.c_int32), ("optimizer", C.c_int32),
     ]
 
 
 DEFAULTS = dict(lambda_h=0.0, mu_sigma=0.03, w_shape=3.0, w_rate=100.0, noise_sigma=0.0,
                 window_W=10.0, fwhm_ref=0.15, incl_tau=0.01, lr=0.1, beta1=0.9, beta2=0.999,
-                adam_eps=1e-8, init_log_sigma=float(np.log(0.1)), n_patterns=1, n_restarts=1, likelihood=0)
+                adam_eps=1e-8, init_log_sigma=float(np.log(0.1)), n_patterns=1, n_restarts=1, likelihood=0, optimizer=0)
 
 _lib = None
 
@@ -76,6 +76,7 @@ def lib():
         L.orc_elbo_grad_range.argtypes = [C.c_void_p, dp, C.c_int32, C.c_uint64, C.c_uint64, C.c_int32, C.c_int32,
                                           dp, dp, dp, dp, C.c_int64]
         L.orc_adam_step.argtypes = [C.c_void_p, dp, dp, dp, dp, C.c_int64]
+        L.orc_natgrad_step.argtypes = [C.c_void_p, dp, dp]
         L.orc_init_state.argtypes = [C.c_void_p, C.c_uint64, dp]
         L.orc_fit.argtypes = [C.c_void_p, dp, dp, dp, C.c_int32, C.c_int32, C.c_uint64, C.c_int64, dp]
         L.orc_inclusion.argtypes = [C.c_void_p, dp, dp, dp]
@@ -234,6 +235,12 @@ class Oracle:
         st = self._state(state).copy()
         g = np.ascontiguousarray(grad, dtype=np.float64)
         lib().orc_adam_step(self._h, _dp(st), _dp(g), _dp(mom1), _dp(mom2), int(step))
+        return st
+
+    def natgrad_step(self, state, grad):
+        st = self._state(state).copy()
+        g = np.ascontiguousarray(grad, dtype=np.float64)
+        lib().orc_natgrad_step(self._h, _dp(st), _dp(g))
         return st
 
     def fit(self, state, iterations, S, seed, first_step=1, mom=None, want_trace=False):
