@@ -73,7 +73,9 @@ typedef struct {
     int32_t likelihood;    /* 0 Gaussian with known sigma_n (R3, the graded path); 1 Poisson, the paper's
                               A12-A16: ll = sum y ln f - f - ln y!; needs y >= 0 and
                               background > 0 everywhere (R24), noise_sigma is ignored                */
-    int32_t _pad2;
+    int32_t optimizer;     /* 0 Adam ascent (R10); 1 natural-gradient ascent of the mean-field Gaussian:
+                              m += lr sigma^2 dELBO/dm, l += lr (dELBO/dl)/2, l clamped to [-12, 2] (R25);
+                              plain steps, no trust region: needs a small lr (0.01 at config 0)             */
 } xrdvi_hyper;
 
 void xrdvi_default_hyper(xrdvi_hyper* hyp);
@@ -125,7 +127,7 @@ int xrdvi_set_state(xrdvi* h, const float* var_params, int64_t step);
 int xrdvi_elbo_grad(xrdvi* h, const float* var_params, int32_t S, uint64_t seed, uint64_t iteration,
                     double* elbo, float* grad);
 
-/* `iterations` Adam-ascent steps from the internal state, each one a replay of a CUDA
+/* `iterations` ascent steps (Adam, or natural gradient if hyper.optimizer = 1) from the internal state, each one a replay of a CUDA
  * Graph; step t uses Philox iteration t, t
  * continuing from the state's step counter + 1 (the graph holds two kernels: the fused profile/residual/
  * backward kernel and the reduce + Adam + next-draw kernel).  Outputs (each may be NULL, nothing is copied then):

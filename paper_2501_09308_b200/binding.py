@@ -36,7 +36,7 @@ class Hyper(C.Structure):
         ("noise_sigma", C.c_double), ("window_W", C.c_double), ("fwhm_ref", C.c_double),
         ("incl_tau", C.c_double), ("lr", C.c_double), ("beta1", C.c_double), ("beta2", C.c_double),
         ("adam_eps", C.c_double), ("init_log_sigma", C.c_double),
-        ("n_patterns", C.c_int32), ("n_restarts", C.c_int32), ("likelihood", C.c_int32), ("_pad2", C.c_int32),
+        ("n_patterns", C.c_int32), ("n_restarts", C.c_int32), ("likelihood", C.c_int32), ("optimizer", C.c_int32),
     ]
 
 

@@ -275,6 +275,7 @@ void xrdvi_default_hyper(xrdvi_hyper* hy) {
     hy->n_patterns = 1;
     hy->n_restarts = 1;
     hy->likelihood = 0;
+    hy->optimizer = 0;
 }
 
 size_t xrdvi_workspace_bytes(int64_t N, int32_t K, int64_t M, int32_t S_max, double two_theta_step,
@@ -294,6 +295,8 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
     if (hyp->size != sizeof(xrdvi_hyper)) return fail(XRDVI_E_INVALID_ARG, "xrdvi_hyper.size mismatch");
     if (hyp->likelihood != 0 && hyp->likelihood != 1)
         return fail(XRDVI_E_INVALID_ARG, "likelihood must be 0 (Gaussian) or 1 (Poisson)");
+    if (hyp->optimizer != 0 && hyp->optimizer != 1)
+        return fail(XRDVI_E_INVALID_ARG, "optimizer must be 0 (Adam) or 1 (natural gradient)");
     if (N < 2 || K < 1 || S_max < 1) return fail(XRDVI_E_INVALID_ARG, "N >= 2, K >= 1, S_max >= 1 required");
     if (hyp->n_patterns < 1 || hyp->n_restarts < 1) return fail(XRDVI_E_INVALID_ARG, "P, R >= 1 required");
     if (!(hyp->mu_sigma > 0) || !(hyp->w_shape > 0) || !(hyp->w_rate > 0) || !(hyp->fwhm_ref > 0) ||
@@ -496,6 +499,7 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
     d.n_c = static_cast<int>(n_c); d.SP = SP; d.TW = pl.TW; d.PS = pl.PS; d.n_seg = pl.n_seg; d.n_tile = pl.n_tile;
     d.n_slots = std::max(n_slots, 1); d.Mv = Mv;
     d.likelihood = hyp->likelihood;
+    d.optimizer = hyp->optimizer;
     d.delta = static_cast<float>(delta);
     d.gcut = static_cast<float>(static_cast<double>(kGaussCut) / (2.0 * delta));
     d.inv_delta = static_cast<float>(1.0 / delta);

@@ -80,6 +80,7 @@ struct Dev {
     int N, K, P, R, PR, n_c, SP, n_seg, n_tile, n_slots, Mv, TW, PS;
     int S, gpi, G;       // draws, groups per instance, groups (run-time)
     int likelihood;      // 0 Gaussian with known sigma_n (R3), 1 Poisson (A12-A16; R24)
+    int optimizer;       // 0 Adam (R10), 1 natural gradient (R25)
     float delta;         // grid step (deg)
     float gcut;          // kGaussCut / (2 Delta): core half-width in points per unit of w
     float inv_delta;
@@ -741,15 +742,19 @@ __global__ void __launch_bounds__(kUpdThreads) update_draw_kernel(const Dev d, c
             const size_t o = (static_cast<size_t>(inst) * 2 * d.K + (is_l ? d.K : 0) + k) * 4 + c;
             d.grad[o] = gj;
             float x = var_in[o];
-            if (do_update) {   // Adam ascent, bias-corrected (R10); l clamped to [-12, 2]
-                const float stepf = static_cast<float>(step + 1);
-                const float bc1 = 1.0f - powf(d.beta1, stepf);
-                const float bc2 = 1.0f - powf(d.beta2, stepf);
-                const float m1 = d.beta1 * d.mom1[o] + (1.0f - d.beta1) * gj;
-                const float m2 = d.beta2 * d.mom2[o] + (1.0f - d.beta2) * gj * gj;
-                d.mom1[o] = m1;
-                d.mom2[o] = m2;
-                x += d.lr * (m1 / bc1) / (sqrtf(m2 / bc2) + d.adam_eps);
+            if (do_update) {   // l clamped to [-12, 2]
+                if (d.optimizer == 1) {   // natural-gradient ascent: Fisher metric diag(1/sigma^2, 2) (R25)
+                    x += d.lr * (is_l ? 0.5f * gj : sgc * sgc * gj);
+                } else {                  // Adam ascent, bias-corrected (R10)
+                    const float stepf = static_cast<float>(step + 1);
+                    const float bc1 = 1.0f - powf(d.beta1, stepf);
+                    const float bc2 = 1.0f - powf(d.beta2, stepf);
+                    const float m1 = d.beta1 * d.mom1[o] + (1.0f - d.beta1) * gj;
+                    const float m2 = d.beta2 * d.mom2[o] + (1.0f - d.beta2) * gj * gj;
+                    d.mom1[o] = m1;
+                    d.mom2[o] = m2;
+                    x += d.lr * (m1 / bc1) / (sqrtf(m2 / bc2) + d.adam_eps);
+                }
                 if (is_l) x = fminf(fmaxf(x, -12.0f), 2.0f);
                 d.var[o] = x;
             }

@@ -34,7 +34,7 @@ def test_hyper_struct_mirrors_header(lib):
     assert hy.incl_tau == 0.01
     assert (hy.lr, hy.beta1, hy.beta2, hy.adam_eps) == (0.1, 0.9, 0.999, 1e-8)
     assert hy.init_log_sigma == pytest.approx(np.log(0.1))
-    assert (hy.n_patterns, hy.n_restarts, hy.likelihood) == (1, 1, 0)
+    assert (hy.n_patterns, hy.n_restarts, hy.likelihood, hy.optimizer) == (1, 1, 0, 0)
 
 
 def test_workspace_bytes(lib):

@@ -241,3 +241,22 @@ def test_poisson_rejects_non_positive_background():
     y[0, 5] = -1.0
     with pytest.raises(XrdviError):
         Xrdvi(wl.two_theta, y, wl.background, wl.peak_ofs, wl.peak_pos, wl.peak_int, S_max=4, **wl.hyper)
+
+
+# --------------------------------------------------------------------------- natural-gradient update (R25)
+def test_natural_gradient_steps_match_oracle():
+    wl = synth.make_workload(0)
+    o = orc.from_workload(wl, optimizer=1, lr=0.01)
+    gpu = Xrdvi.from_workload(wl, optimizer=1, lr=0.01)
+    st_g, _, tr_g = gpu.fit(1, seed=5, want_trace=True)
+    st_r, _, tr_r = o.fit(o.init_state(), 1, wl.S, seed=5, want_trace=True)
+    np.testing.assert_allclose(st_g, st_r, rtol=1e-4, atol=2e-5)
+    st_g, inc_g, tr_g = gpu.fit(199, seed=5, want_trace=True)            # steps 2..200 continue the counter
+    st_r, _, tr_r = o.fit(o.init_state(), 200, wl.S, seed=5, want_trace=True)
+    np.testing.assert_allclose(tr_g[:3, 0, 0], tr_r[1:4, 0, 0], rtol=TOL_ELBO)
+    assert tr_g[-20:].mean() > tr_r[:20].mean() + 100.0                   # the ELBO rises
+    assert np.abs(inc_g - o.inclusion(st_r)).max() <= TOL_INCL
+    check_eval(gpu, o, st_g, wl.S, seed=5, iteration=201)
+    from paper_2501_09308_b200 import XrdviError
+    with pytest.raises(XrdviError):
+        Xrdvi.from_workload(wl, optimizer=2)
