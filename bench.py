@@ -90,6 +90,18 @@ def measured_peaks() -> dict:
     return {}
 
 
+def measured_traffic(kernel: str, cfg: int):
+    """DRAM bytes per launch of `kernel` from the committed ncu capture (profiles/), or None."""
+    p = ROOT / "profiles" / "r1_v3_traffic.txt"
+    if not p.exists():
+        return None
+    for ln in p.read_text().splitlines():
+        t = ln.split()
+        if len(t) == 3 and not ln.startswith("#") and t[0] == kernel and t[1] == str(cfg):
+            return int(t[2])
+    return None
+
+
 def run_reference(args, rank: int) -> None:
     """Oracle arm: the fp64 CPU oracle, as it stands, on the host cores (rank 0 only)."""
     if rank != 0:
@@ -130,7 +142,7 @@ def run_ours(args, rank: int, local_rank: int, world: int) -> None:
         raise SystemExit("bench.py: no CUDA device (the hot path has no CPU fallback)")
     torch.cuda.set_device(local_rank)
     dist = None
-    if world > 1:
+    if world > 1 or ("RANK" in os.environ and "MASTER_ADDR" in os.environ):   # launched by torchrun (any N)
         import torch.distributed as dist_mod
         dist_mod.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
         dist = dist_mod
@@ -189,7 +201,8 @@ def run_ours(args, rank: int, local_rank: int, world: int) -> None:
     r_plain = n_sm * f_max * 16.0 / 4.0          # plain formulation: 4 MUFU per pair (2 per pass), 16 MUFU lanes/SM/clk
     roofline = {
         "bound": "alu", "kernel": "elbo_tile_kernel", "achieved": achieved / 1e9, "peak": r_plain / 1e9,
-        "unit": "Gpair/s", "frac": achieved / r_plain, "traffic": None,
+        "unit": "Gpair/s", "frac": achieved / r_plain, "traffic": measured_traffic("elbo_tile_kernel", args.config),
+        "traffic_source": "profiles/r1_v3_traffic.txt (ncu --set full, dram read + write bytes per launch)",
         "peak_source": f"derived: {n_sm} SMs x {f_max / 1e6:.0f} MHz (MEASURED_PEAKS sm_max_mhz) x 16 MUFU lanes / "
                        f"4 MUFU per pair (plain forward+backward formulation, DESIGN.md Roofline)",
         "ms_tile": tk["ms_tile"], "ms_tile_forward_only": tk["ms_tile_forward_only"], "ms_update": tk["ms_update"],

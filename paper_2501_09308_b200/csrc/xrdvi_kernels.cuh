@@ -680,8 +680,15 @@ __global__ void __launch_bounds__(kUpdThreads) update_draw_kernel(const Dev d, c
         for (int s = threadIdx.x; s < d.S; s += kUpdThreads) {
             const int g = inst * d.gpi + (s >> 5), lane = s & 31;
             const float* __restrict__ lp = d.llpart + static_cast<size_t>(g) * d.n_seg * 32 + lane;
-            double a = 0.0;
-            for (int t = 0; t < d.n_seg; ++t) a += static_cast<double>(lp[static_cast<size_t>(t) * 32]);
+            // eight interleaved partial sums (independent load/add chains), combined in a fixed order
+            double a8[8] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+            int t = 0;
+            for (; t + 8 <= d.n_seg; t += 8) {
+#pragma unroll
+                for (int j = 0; j < 8; ++j) a8[j] += static_cast<double>(lp[static_cast<size_t>(t + j) * 32]);
+            }
+            for (int j = 0; t < d.n_seg; ++t, ++j) a8[j] += static_cast<double>(lp[static_cast<size_t>(t) * 32]);
+            const double a = ((a8[0] + a8[1]) + (a8[2] + a8[3])) + ((a8[4] + a8[5]) + (a8[6] + a8[7]));
             const double ll = static_cast<double>(pc.ll_scale) * a + pc.ll_const;
             d.ll_t[static_cast<size_t>(inst) * d.gpi * 32 + s] = ll;
             v[0] += ll;
