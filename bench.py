@@ -180,6 +180,14 @@ def run_ours(args, rank: int, local_rank: int, world: int) -> None:
     gpu2.reset_state(seed=seeds["state_seed"])
     st, inc, _ = gpu2.fit(args.steps, S=S, seed=seeds["draw_seed"])
     e2e_s = replicas.max_over_ranks(time.perf_counter() - t0, dist, "cuda")
+    # the same through one xrdvi_elbo_grad call per step: H2D of the variational parameters, D2H of ELBO and
+    # gradient, and a stream synchronisation in EVERY step (the per-call cost a host-side optimiser would see)
+    n_calls = min(args.steps, 200)
+    barrier()
+    t0 = time.perf_counter()
+    for i in range(n_calls):
+        gpu2.elbo_grad(state=st, S=S, seed=seeds["draw_seed"], iteration=i + 1)
+    percall_s = replicas.max_over_ranks(time.perf_counter() - t0, dist, "cuda")
     h2d = 8 * (wl.two_theta.size + wl.y.size + wl.background.size + wl.peak_pos.size + wl.peak_int.size
                + wl.peak_ofs.size)
     d2h = st.nbytes + inc.nbytes
@@ -243,6 +251,10 @@ def run_ours(args, rank: int, local_rank: int, world: int) -> None:
                 "h2d_bytes_per_step": h2d / args.steps, "d2h_bytes_per_step": d2h / args.steps,
                 "covers": "xrdvi_create (host fp64 preprocessing + H2D) + xrdvi_fit + D2H of parameters and "
                           "inclusion probabilities; inputs are uploaded once per fit"},
+        "e2e_per_call": {"value": replicas.whole_job_rate(pairs * T * n_calls, world, percall_s), "unit": UNIT,
+                         "calls": n_calls, "h2d_bytes_per_step": int(st.nbytes), "d2h_bytes_per_step": int(st.nbytes + 8 * wl.P * wl.R),
+                         "covers": "one xrdvi_elbo_grad call per step with host buffers: H2D of the variational "
+                                   "parameters, draw + tile + reduce kernels, D2H of ELBO and gradient, stream sync"},
         "gpu_launches": 2 * args.steps + 1,
         "roofline": roofline,
         "cpu_baseline": cpu,

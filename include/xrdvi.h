@@ -140,6 +140,19 @@ int xrdvi_fit(xrdvi* h, int32_t iterations, int32_t S, uint64_t seed, float* var
  * incl_prob, area_ratio double [P][R][K], either may be NULL.                                      */
 int xrdvi_inclusion(xrdvi* h, double* incl_prob, double* area_ratio);
 
+/* Log-joint gradient service: log p(Y, Phi) + log |dPhi/dzeta| and its gradient at n
+ * caller-supplied points of the unconstrained latent space, for one pattern -- what a gradient-based sampler of the
+ * paper's model (the MCMC rows of Table 1) evaluates per leapfrog step.  The same
+ * profile / residual / backward kernels run on the points as on Monte-Carlo draws; no variational state is read
+ * or modified (the per-step draw buffers are overwritten).
+ *  zeta     float [n][K][4] = (ln h, mu, ln w, logit r) per phase (R6);  1 <= n <= S_max rounded up to 32
+ *  pattern  index of the observed pattern, 0 <= pattern < P
+ *  ll       double [n]: log-likelihood (Gaussian or Poisson, hyper.likelihood)
+ *  lpj      double [n]: log prior + log Jacobian;   grad float [n][K][4] = d (ll + lpj) / d zeta
+ *  ll, lpj, grad may each be NULL.                                                                           */
+int xrdvi_logjoint_grad(xrdvi* h, const float* zeta, int64_t n, int32_t pattern, double* ll, double* lpj,
+                        float* grad);
+
 /* Debug read-back of the forward pass for parity tests: runs draw + forward at (var_params or
  * internal state, S, seed, iteration) and returns, for the first n sample-instances in
  * (pat, rst, s) order, the profile f float [n][N] (including B) and ll double [n]; f or ll may be NULL. */

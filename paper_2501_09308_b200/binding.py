@@ -17,7 +17,7 @@ _LIB_PATH = _PKG / "libxrdvi.so"
 EXPORTS = (
     "xrdvi_default_hyper", "xrdvi_workspace_bytes", "xrdvi_create", "xrdvi_destroy", "xrdvi_pair_count",
     "xrdvi_window_halfwidth", "xrdvi_reset_state", "xrdvi_get_state", "xrdvi_set_state", "xrdvi_elbo_grad",
-    "xrdvi_fit", "xrdvi_inclusion", "xrdvi_debug_profile", "xrdvi_debug_draws", "xrdvi_time_kernels",
+    "xrdvi_fit", "xrdvi_inclusion", "xrdvi_logjoint_grad", "xrdvi_debug_profile", "xrdvi_debug_draws", "xrdvi_time_kernels",
     "xrdvi_bench_steps", "xrdvi_pipe_rates", "xrdvi_last_error",
 )
 
@@ -71,6 +71,7 @@ def load_library():
     L.xrdvi_elbo_grad.argtypes = [vp, fp, C.c_int32, C.c_uint64, C.c_uint64, dp, fp]
     L.xrdvi_fit.argtypes = [vp, C.c_int32, C.c_int32, C.c_uint64, fp, dp, dp]
     L.xrdvi_inclusion.argtypes = [vp, dp, dp]
+    L.xrdvi_logjoint_grad.argtypes = [vp, fp, C.c_int64, C.c_int32, dp, dp, fp]
     L.xrdvi_debug_profile.argtypes = [vp, fp, C.c_int32, C.c_uint64, C.c_uint64, C.c_int64, fp, dp]
     L.xrdvi_debug_draws.argtypes = [vp, C.c_int32, C.c_uint64, C.c_uint64, C.c_int64, fp, C.POINTER(C.c_uint32),
                                     C.POINTER(C.c_int32)]
@@ -208,6 +209,16 @@ class Xrdvi:
         tr = np.empty((int(iterations), self.P, self.R), dtype=np.float64) if want_trace else None
         _check(load_library().xrdvi_fit(self._h, int(iterations), S, int(seed), _f(st), _d(inc), _d(tr)))
         return st, inc, tr
+
+    def logjoint_grad(self, zeta, pattern=0):
+        """ll [n], log prior + log Jacobian [n], gradient [n][K][4] at the points zeta [n][K][4] (xrdvi_logjoint_grad)."""
+        z = np.ascontiguousarray(zeta, dtype=np.float32).reshape(-1, self.K, 4)
+        n = int(z.shape[0])
+        ll = np.empty(n, dtype=np.float64)
+        lpj = np.empty(n, dtype=np.float64)
+        g = np.empty((n, self.K, 4), dtype=np.float32)
+        _check(load_library().xrdvi_logjoint_grad(self._h, _f(z), n, int(pattern), _d(ll), _d(lpj), _f(g)))
+        return ll, lpj, g
 
     def inclusion(self):
         inc = np.empty((self.P, self.R, self.K), dtype=np.float64)

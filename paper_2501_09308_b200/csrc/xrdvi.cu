@@ -42,6 +42,8 @@ struct Plan {   // workspace carve; identical arithmetic in workspace_bytes and 
     size_t o_yb, o_bg, o_pkt, o_runs, o_srng, o_sord, o_sofs, o_sids, o_pat, o_area, o_mh0;
     size_t o_var, o_vartmp, o_mom1, o_mom2, o_grad, o_elbo, o_elbok, o_llt, o_trace, o_done, o_ctl;
     size_t o_lat, o_eps, o_rr, o_ng, o_llpart, o_part8, o_dbg;
+    size_t o_pd, o_lpk, o_zeta, o_gradz, o_lls;
+    int pd_groups;     // groups one launch of the log-joint gradient service handles
 };
 
 // window half-width in grid points (R16); dense (W <= 0) is represented by n_c = -1 here
@@ -126,6 +128,14 @@ bool make_plan(int64_t N, int32_t K, int64_t M, int32_t S_max, double step, cons
     p.o_llpart = take(sizeof(float) * static_cast<size_t>(p.G_max) * p.n_seg * 32);
     p.o_part8 = take(sizeof(float) * static_cast<size_t>(p.G_max) * std::max<long long>(p.slots_cap, 1) * 8);
     p.o_dbg = take(sizeof(double) * (2 * static_cast<size_t>(p.PR) * K + 64));
+    // log-joint gradient service: per-draw partials of at most 64 MiB worth of groups (at least one)
+    const size_t pd_group_bytes = sizeof(float) * 128 * static_cast<size_t>(std::max<long long>(p.slots_cap, 1));
+    p.pd_groups = static_cast<int>(std::min<size_t>(p.gpi_max, std::max<size_t>(1, (size_t(64) << 20) / pd_group_bytes)));
+    p.o_pd = take(pd_group_bytes * p.pd_groups);
+    p.o_lpk = take(sizeof(float) * 32 * static_cast<size_t>(K) * p.pd_groups);
+    p.o_zeta = take(sizeof(float4) * static_cast<size_t>(p.S_pad) * K);
+    p.o_gradz = take(sizeof(float4) * static_cast<size_t>(p.S_pad) * K);
+    p.o_lls = take(sizeof(double) * 2 * p.S_pad);
     p.total = o;
     *pl = p;
     return true;
@@ -536,6 +546,8 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
     d.ng = reinterpret_cast<int*>(w + pl.o_ng);
     d.llpart = reinterpret_cast<float*>(w + pl.o_llpart);
     d.part8 = reinterpret_cast<float*>(w + pl.o_part8);
+    d.pd = nullptr;
+    d.g_base = 0;
     set_S(h, S_max);
 
     cudaStream_t st = h->stream;
@@ -757,6 +769,47 @@ int xrdvi_debug_draws(xrdvi* h, int32_t S, uint64_t seed, uint64_t iteration, in
             if (core_halfwidth) core_halfwidth[static_cast<size_t>(t) * d.K + k] = ngh[static_cast<size_t>(g) * d.K + k];
         }
     }
+    return XRDVI_OK;
+}
+
+int xrdvi_logjoint_grad(xrdvi* h, const float* zeta, int64_t n, int32_t pattern, double* ll, double* lpj, float* grad) {
+    if (!h || !zeta) return fail(XRDVI_E_INVALID_ARG, "null handle or zeta");
+    if (n < 1 || n > h->plan.S_pad) return fail(XRDVI_E_INVALID_ARG, "n out of range [1, S_max rounded up to 32]");
+    if (pattern < 0 || pattern >= h->plan.P) return fail(XRDVI_E_INVALID_ARG, "pattern out of range");
+    CU(cudaSetDevice(h->device));
+    const int K = h->K;
+    const size_t zb = sizeof(float4) * static_cast<size_t>(n) * K;
+    float4* zeta_dev = reinterpret_cast<float4*>(h->ws + h->plan.o_zeta);
+    float4* grad_dev = reinterpret_cast<float4*>(h->ws + h->plan.o_gradz);
+    double* ll_dev = reinterpret_cast<double*>(h->ws + h->plan.o_lls);
+    double* lpj_dev = ll_dev + h->plan.S_pad;
+    float* lpk = reinterpret_cast<float*>(h->ws + h->plan.o_lpk);
+    cudaStream_t st = h->stream;
+    CU(cudaMemcpyAsync(zeta_dev, zeta, zb, cudaMemcpyHostToDevice, st));
+    set_S(h, static_cast<int>(n));                    // the n points take the place of the draws of one instance
+    const int gpi = h->dev.gpi;
+    const int inst = pattern * h->plan.R;             // restart 0 of the pattern: only its buffers are used
+    for (int c0 = 0; c0 < gpi; c0 += h->plan.pd_groups) {
+        const int ng = std::min(h->plan.pd_groups, gpi - c0);
+        Dev dd = h->dev;
+        dd.g_base = inst * gpi + c0;
+        dd.G = ng;
+        dd.pd = reinterpret_cast<float*>(h->ws + h->plan.o_pd);
+        zeta_latent_kernel<<<dim3((K + 3) / 4, ng), 128, 0, st>>>(dd, zeta_dev, static_cast<int>(n), c0);
+        launch_tile<true>(dd, st, nullptr, 0);
+        logjoint_grad_kernel<<<dim3(K, ng), 32, 0, st>>>(dd, zeta_dev, static_cast<int>(n), c0, pattern, grad_dev, lpk);
+        logjoint_scalar_kernel<<<ng, 32, 0, st>>>(dd, static_cast<int>(n), c0, pattern, lpk, ll_dev, lpj_dev);
+        CU(cudaGetLastError());
+    }
+    std::vector<double> llh(ll ? n : 0), lph(lpj ? n : 0);
+    std::vector<float> gh(grad ? static_cast<size_t>(n) * K * 4 : 0);
+    if (ll) CU(cudaMemcpyAsync(llh.data(), ll_dev, sizeof(double) * n, cudaMemcpyDeviceToHost, st));
+    if (lpj) CU(cudaMemcpyAsync(lph.data(), lpj_dev, sizeof(double) * n, cudaMemcpyDeviceToHost, st));
+    if (grad) CU(cudaMemcpyAsync(gh.data(), grad_dev, zb, cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    if (ll) std::memcpy(ll, llh.data(), sizeof(double) * n);
+    if (lpj) std::memcpy(lpj, lph.data(), sizeof(double) * n);
+    if (grad) std::memcpy(grad, gh.data(), zb);
     return XRDVI_OK;
 }
 

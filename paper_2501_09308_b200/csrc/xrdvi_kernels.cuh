@@ -117,6 +117,9 @@ struct Dev {
     int* ng;                  // [G][K]      Gaussian core half-width in grid points
     float* llpart;            // [G][n_seg][32] sum over the segment of ((y-f)/sigma_n)^2
     float* part8;             // [G][n_slots][8] (g_h, g_mu, g_w, g_r, g_h eps_h, ...) summed over 32 draws
+    // log-joint gradient service (xrdvi_logjoint_grad): per-draw output instead of the sum over the draws
+    float* pd;                // nullptr, or [gridDim.y][n_slots][4][32] d ll / d zeta per (run, class, draw)
+    int g_base;               // group of blockIdx.y = 0 in elbo_tile_kernel (0 except in the service)
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -177,19 +180,11 @@ __device__ __forceinline__ long long philox_iteration(const Ctl* ctl) {
     return o >= 0 ? o : ctl->step + 1;
 }
 
-// a-1 + a-2 for one (instance, phase k, draw s): Philox draw, transform, latent record.  Must be called by
-// all 32 lanes of a warp whose lanes hold consecutive draws of one group (the core half-width n_g is a
-// warp maximum).
-__device__ __forceinline__ void draw_one(const Dev& d, int inst, int k, int s, unsigned it, unsigned long long seed,
-                                         const float4 m, const float4 l, uint4* __restrict__ raw_out) {
+// a-2, second half: latent record, eps, r and the group's Gaussian-core half-width of phase k for the lane's
+// draw.  Must be called by all 32 lanes of a warp whose lanes hold consecutive draws of group g (the core
+// half-width n_g is a warp maximum); `valid` = false for padding lanes, which contribute nothing.
+__device__ __forceinline__ void emit_latent(const Dev& d, int g, int k, bool valid, const Phys& q, const float4 ep) {
     const int lane = threadIdx.x & 31;
-    const int g = inst * d.gpi + (s >> 5);
-    const uint4 words = philox4x32_10(make_uint4(it, static_cast<unsigned>(s), static_cast<unsigned>(k),
-                                                 static_cast<unsigned>(inst)),
-                                      make_uint2(static_cast<unsigned>(seed), static_cast<unsigned>(seed >> 32)));
-    const float4 ep = normals_from_words(words);
-    const float4 sg = make_float4(expf(l.x), expf(l.y), expf(l.z), expf(l.w));
-    const Phys q = transform(m, sg, ep);
     // 1/w is capped at 5e7 (w >= 2e-8 deg: far outside the model's regime) so that the shared reciprocal
     // rcp(ua ub) of two points can never see an overflowed product
     const float iw = fminf(1.0f / q.w, 5.0e7f);
@@ -198,7 +193,7 @@ __device__ __forceinline__ void draw_one(const Dev& d, int inst, int k, int s, u
     // Gaussian core half-width in grid points for this draw: |t'| <= kGaussCut  <=>
     // |i - j| <= kGaussCut w / (2 Delta) + |delta_m + mu| / Delta; |delta_m| <= Delta/2, +1 for rounding
     float reach = fmaf(d.gcut, q.w, fabsf(q.mu) * d.inv_delta) + 1.5f;
-    if (s >= d.S) {  // padding lanes contribute nothing
+    if (!valid) {
         lt = make_float4(1.0f, 0.0f, 0.0f, 0.0f);
         reach = 0.0f;
     }
@@ -210,7 +205,19 @@ __device__ __forceinline__ void draw_one(const Dev& d, int inst, int k, int s, u
     d.eps[o] = ep;
     d.rr[o] = q.r;
     if (lane == 0) d.ng[static_cast<size_t>(g) * d.K + k] = static_cast<int>(reach) + 1;
-    if (raw_out) raw_out[o] = words;
+}
+
+// a-1 + a-2 for one (instance, phase k, draw s): Philox draw, transform, latent record (all 32 lanes of a warp).
+__device__ __forceinline__ void draw_one(const Dev& d, int inst, int k, int s, unsigned it, unsigned long long seed,
+                                         const float4 m, const float4 l, uint4* __restrict__ raw_out) {
+    const int g = inst * d.gpi + (s >> 5);
+    const uint4 words = philox4x32_10(make_uint4(it, static_cast<unsigned>(s), static_cast<unsigned>(k),
+                                                 static_cast<unsigned>(inst)),
+                                      make_uint2(static_cast<unsigned>(seed), static_cast<unsigned>(seed >> 32)));
+    const float4 ep = normals_from_words(words);
+    const float4 sg = make_float4(expf(l.x), expf(l.y), expf(l.z), expf(l.w));
+    emit_latent(d, g, k, s < d.S, transform(m, sg, ep), ep);
+    if (raw_out) raw_out[(static_cast<size_t>(g) * d.K + k) * 32 + (threadIdx.x & 31)] = words;
 }
 
 // Stand-alone draw kernel (first step of a fit, xrdvi_elbo_grad, debug).  grid (ceil(K/4), G), block 128.
@@ -410,7 +417,7 @@ elbo_tile_kernel(const Dev d, float* __restrict__ f_dbg, long long n_dbg) {
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const int tw = w % TW, ps = w / TW;
     const int seg = d.seg_order[blockIdx.x];
-    const int g = blockIdx.y;
+    const int g = d.g_base + blockIdx.y;
     const int tile = seg * TW + tw;
     const int i0 = tile * kPT;
     const bool live = tile < d.n_tile;                      // the last segment may have fewer than TW tiles
@@ -625,6 +632,11 @@ elbo_tile_kernel(const Dev d, float* __restrict__ f_dbg, long long n_dbg) {
         v[1] = lt.x * (2.0f * cL * B3 + (2.0f * kLn2) * cG * B4);
         v[2] = -(cL * (2.0f * B5 - B1) + cG * (B2 - (2.0f * kLn2) * B6));
         v[3] = (1.0f - rmix) * cL * B1 - rmix * cG * B2;
+        if (d.pd) {   // gradient service: keep the draws apart
+            float* __restrict__ o = d.pd + (static_cast<size_t>(blockIdx.y) * d.n_slots + r) * 128 + lane;
+            o[0] = v[0]; o[32] = v[1]; o[64] = v[2]; o[96] = v[3];
+            continue;
+        }
         v[4] = v[0] * ep.x; v[5] = v[1] * ep.y; v[6] = v[2] * ep.z; v[7] = v[3] * ep.w;
         const float tot = warp_reduce8(v);
         if (lane < 8) part[static_cast<size_t>(r) * 8 + lane] = tot;
@@ -853,6 +865,68 @@ __global__ void __launch_bounds__(128) init_state_kernel(const Dev d, const floa
         d.mom2[static_cast<size_t>(inst) * per + j] = 0.0f;
     }
     if (threadIdx.x == 0) d.done_inst[inst] = 0u;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Log-joint gradient service (the gradient an HMC / MCMC sampler of the paper's Table 1 needs):
+// the caller supplies the unconstrained latents zeta [n][K][4] of n points; the tile kernel runs on them exactly
+// as on draws and leaves d ll / d zeta per draw in d.pd.
+
+// a-2 for supplied points.  grid (ceil(K/4), groups of this launch), block 128.  Point of lane:
+// s = (s_group0 + blockIdx.y) * 32 + lane.
+__global__ void __launch_bounds__(128) zeta_latent_kernel(const Dev d, const float4* __restrict__ zeta, int n, int s_group0) {
+    const int lane = threadIdx.x & 31;
+    const int k = blockIdx.x * 4 + (threadIdx.x >> 5);
+    if (k >= d.K) return;
+    const int s = (s_group0 + blockIdx.y) * 32 + lane;
+    const bool valid = s < n;
+    const float4 z = valid ? zeta[static_cast<size_t>(s) * d.K + k] : make_float4(0.f, 0.f, 0.f, 0.f);
+    const float4 zero = make_float4(0.f, 0.f, 0.f, 0.f);
+    emit_latent(d, d.g_base + blockIdx.y, k, valid, transform(z, zero, zero), zero);
+}
+
+// Sum of the per-run gradients of phase k over the tiles (fixed order) + prior and Jacobian part (a-6).
+// grid (K, groups of this launch), block 32 (lane = point).  Also the phase's log prior + log Jacobian -> lpk.
+__global__ void __launch_bounds__(32) logjoint_grad_kernel(const Dev d, const float4* __restrict__ zeta, int n, int s_group0,
+                                                           int pat, float4* __restrict__ grad, float* __restrict__ lpk) {
+    const int lane = threadIdx.x, k = blockIdx.x, gi = blockIdx.y;
+    const int s = (s_group0 + gi) * 32 + lane;
+    if (s >= n) return;
+    const PatConst pc = d.pat[pat];
+    double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+    for (int j = d.slot_ofs[k]; j < d.slot_ofs[k + 1]; ++j) {
+        const float* __restrict__ o = d.pd + (static_cast<size_t>(gi) * d.n_slots + d.slot_ids[j]) * 128 + lane;
+        a0 += static_cast<double>(o[0]); a1 += static_cast<double>(o[32]);
+        a2 += static_cast<double>(o[64]); a3 += static_cast<double>(o[96]);
+    }
+    const float4 zero = make_float4(0.f, 0.f, 0.f, 0.f);
+    const Phys q = transform(zeta[static_cast<size_t>(s) * d.K + k], zero, zero);
+    grad[static_cast<size_t>(s) * d.K + k] =
+        make_float4(static_cast<float>(a0 + static_cast<double>(1.0f - pc.lambda_h * q.h)),
+                    static_cast<float>(a1 + static_cast<double>(-q.mu * d.mu_inv_var)),
+                    static_cast<float>(a2 + static_cast<double>(d.w_shape - d.w_rate * q.w)),
+                    static_cast<float>(a3 + static_cast<double>(1.0f - 2.0f * q.r)));
+    const float az = fabsf(q.zr);
+    lpk[(static_cast<size_t>(gi) * d.K + k) * 32 + lane] =
+        (pc.log_lambda_h - pc.lambda_h * q.h + q.zh) + (-0.5f * q.mu * q.mu * d.mu_inv_var + d.mu_logc) +
+        (d.w_logc + d.w_shape * q.zw - d.w_rate * q.w) - (az + 2.0f * log1pf(expf(-az)));
+}
+
+// ll and log prior + log Jacobian per point.  grid (groups of this launch), block 32.
+__global__ void __launch_bounds__(32) logjoint_scalar_kernel(const Dev d, int n, int s_group0, int pat,
+                                                             const float* __restrict__ lpk, double* __restrict__ ll,
+                                                             double* __restrict__ lpj) {
+    const int lane = threadIdx.x, gi = blockIdx.x;
+    const int s = (s_group0 + gi) * 32 + lane;
+    if (s >= n) return;
+    const PatConst pc = d.pat[pat];
+    const float* __restrict__ lp = d.llpart + static_cast<size_t>(d.g_base + gi) * d.n_seg * 32 + lane;
+    double a = 0.0;
+    for (int t = 0; t < d.n_seg; ++t) a += static_cast<double>(lp[static_cast<size_t>(t) * 32]);
+    ll[s] = static_cast<double>(pc.ll_scale) * a + pc.ll_const;
+    double b = 0.0;
+    for (int k = 0; k < d.K; ++k) b += static_cast<double>(lpk[(static_cast<size_t>(gi) * d.K + k) * 32 + lane]);
+    lpj[s] = b;
 }
 
 }  // namespace xrdvi_dev

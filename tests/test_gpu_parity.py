@@ -260,3 +260,65 @@ def test_natural_gradient_steps_match_oracle():
     from paper_2501_09308_b200 import XrdviError
     with pytest.raises(XrdviError):
         Xrdvi.from_workload(wl, optimizer=2)
+
+
+# --------------------------------------------------------------------------- log-joint gradient service (NEXT-4)
+def check_logjoint(gpu, o, zeta, pat):
+    ll_g, lpj_g, g_g = gpu.logjoint_grad(zeta, pattern=pat)
+    for t in range(zeta.shape[0]):
+        ll_r, lpj_r, g_r = o.logjoint_grad(zeta[t].astype(np.float64), pat)
+        assert ll_g[t] == pytest.approx(ll_r, rel=TOL_ELBO)
+        assert lpj_g[t] == pytest.approx(lpj_r, rel=TOL_ELBO, abs=1e-3)
+        err = np.abs(g_g[t] - g_r).max(axis=0) / np.abs(g_r).max(axis=0)       # per latent class, over phases
+        assert err.max() <= TOL_GRAD, err
+
+
+def test_logjoint_gradient_service_matches_oracle():
+    wl = synth.make_workload(3, n_patterns=3, S=64)
+    o = orc.from_workload(wl)
+    gpu = Xrdvi.from_workload(wl)
+    rng = np.random.default_rng(3)
+    for pat, n in ((0, 1), (2, 37), (1, 64)):
+        st = synth.random_state(wl.K, n, 1, seed=20 + pat)[:, 0, 0]            # [n][K][4] points near a fit
+        st[:, :, 0] += math.log(1.0 / o.lambda_h(pat)) - 2.0 + rng.normal(0, 0.3, (n, wl.K))
+        ll_g, lpj_g, g_g = gpu.logjoint_grad(st, pattern=pat)
+        for t in sorted({0, n // 2, n - 1}):
+            ll_r, lpj_r, g_r = o.logjoint_grad(st[t].astype(np.float64), pat)
+            assert ll_g[t] == pytest.approx(ll_r, rel=TOL_ELBO)
+            assert lpj_g[t] == pytest.approx(lpj_r, rel=TOL_ELBO, abs=1e-3)
+            err = np.abs(g_g[t] - g_r).max(axis=0) / np.abs(g_r).max(axis=0)
+            assert err.max() <= TOL_GRAD, err
+    # the state of a fit is untouched by the service, and a fit still runs after it
+    st0, step = gpu.get_state()
+    gpu.logjoint_grad(synth.random_state(wl.K, 3, 1, seed=1)[:, 0, 0], pattern=0)
+    st1, _ = gpu.get_state()
+    np.testing.assert_array_equal(st0, st1)
+    gpu.fit(3, seed=2)
+    from paper_2501_09308_b200 import XrdviError
+    with pytest.raises(XrdviError):
+        gpu.logjoint_grad(np.zeros((65, wl.K, 4), np.float32))                 # n > S_max rounded up to 32
+    with pytest.raises(XrdviError):
+        gpu.logjoint_grad(np.zeros((1, wl.K, 4), np.float32), pattern=3)
+
+
+def test_logjoint_gradient_service_chunks_and_poisson():
+    wl = synth.make_workload(4, K=60, S=256)                                   # 4 groups per launch, 7 groups: 2 launches
+    o = orc.from_workload(wl)
+    gpu = Xrdvi.from_workload(wl)
+    n = 200
+    st = synth.random_state(wl.K, n, 1, seed=5)[:, 0, 0]
+    st[:, :, 0] += math.log(1.0 / o.lambda_h()) - 3.0
+    st[:, :, 2] = np.log(np.random.default_rng(1).uniform(0.03, 0.3, (n, wl.K)))
+    ll_g, lpj_g, g_g = gpu.logjoint_grad(st)
+    for t in (0, 31, 32, 127, 128, 199):
+        ll_r, lpj_r, g_r = o.logjoint_grad(st[t].astype(np.float64))
+        assert ll_g[t] == pytest.approx(ll_r, rel=TOL_ELBO)
+        assert lpj_g[t] == pytest.approx(lpj_r, rel=TOL_ELBO, abs=1e-3)
+        err = np.abs(g_g[t] - g_r).max(axis=0) / np.abs(g_r).max(axis=0)
+        assert err.max() <= TOL_GRAD, err
+    wlp = synth.make_workload(0, peak_counts=5.0e3)
+    op = orc.from_workload(wlp)
+    gp = Xrdvi.from_workload(wlp)
+    stp = synth.random_state(wlp.K, 9, 1, seed=8)[:, 0, 0]
+    stp[:, :, 0] += math.log(1.0 / op.lambda_h()) - 1.0
+    check_logjoint(gp, op, stp, 0)
