@@ -322,3 +322,29 @@ def test_logjoint_gradient_service_chunks_and_poisson():
     stp = synth.random_state(wlp.K, 9, 1, seed=8)[:, 0, 0]
     stp[:, :, 0] += math.log(1.0 / op.lambda_h()) - 1.0
     check_logjoint(gp, op, stp, 0)
+
+
+# --------------------------------------------------------------------------- extreme latents
+def test_extreme_widths_shifts_and_mixing():
+    """Very narrow and very wide peaks, shifts of many grid points, mixing at both ends, tiny and huge scales:
+    the Gaussian-core / Lorentz-tail split, the shared reciprocals and the grid-index coordinates must hold."""
+    wl = synth.make_workload(1, S=32, K=12)
+    o = orc.from_workload(wl)
+    gpu = Xrdvi.from_workload(wl)
+    K = wl.K
+    st = synth.random_state(K, 1, 1, seed=3)
+    st[0, 0, 0, :, 0] += math.log(1.0 / o.lambda_h()) - 2.0
+    # FWHM (deg) from half a grid step to twice the window; narrower peaks amplify the fp32 rounding of the
+    # sampled shift (3e-8 deg at |mu| = 0.5) by 2/w beyond 1e-4 of the peak height (DESIGN.md "Domain")
+    st[0, 0, 0, :, 2] = np.log([0.01, 0.015, 0.02, 0.05, 0.1, 0.2, 0.5, 1.0, 3.0, 0.03, 0.3, 0.08])
+    st[0, 0, 0, :, 1] = [0.5, -0.5, 0.3, -0.2, 0.0, 0.01, -0.01, 0.1, -0.1, 0.02, 0.0, 0.25]             # shift (deg)
+    st[0, 0, 0, :, 3] = [-20, 20, -8, 8, 0, 1, -1, 3, -3, 0.5, 15, -15]                                  # logit r
+    st[0, 0, 0, 3, 0] -= 12.0                                                                              # h tiny
+    st[0, 0, 0, 5, 0] += 3.0                                                                               # h large
+    st[0, 0, 1] = math.log(0.02)
+    st[0, 0, 1, :, 2] = math.log(0.3)                                                                      # wide spread of w inside a group
+    check_eval(gpu, o, st, 32, seed=4, iteration=2, n_prof=4)
+    ll_g, lpj_g, g_g = gpu.logjoint_grad(st[0, 0, 0][None])
+    ll_r, lpj_r, g_r = o.logjoint_grad(st[0, 0, 0].astype(np.float64))
+    assert ll_g[0] == pytest.approx(ll_r, rel=TOL_ELBO)
+    assert (np.abs(g_g[0] - g_r).max(axis=0) / np.abs(g_r).max(axis=0)).max() <= TOL_GRAD
