@@ -250,52 +250,34 @@ __device__ __forceinline__ void fwd_pair(float ta, float tb, float cg2, float cl
     }
 }
 
-// same with per-point coefficients (window-edge quads: the coefficient of an out-of-window point is 0)
-template <bool CORE>
-__device__ __forceinline__ void fwd_pair_masked(float ta, float tb, float cga, float cgb, float cla, float clb,
-                                                float& acca, float& accb) {
-    const float ua = fmaf(ta, ta, 1.0f), ub = fmaf(tb, tb, 1.0f);
-    const float rc = rcp_approx(ua * ub);
-    acca = fmaf(rc * ub, cla, acca);
-    accb = fmaf(rc * ua, clb, accb);
-    if (CORE) {
-        acca = fmaf(cga, ex2_approx(-ua), acca);
-        accb = fmaf(cgb, ex2_approx(-ub), accb);
-    }
-}
-
 // Per-(peak, tile) geometry in tile coordinates (warp-uniform): in-window points p_lo <= p <= p_hi, Gaussian
 // core c_lo <= p <= c_hi.
 struct PeakGeo { int p_lo, p_hi, c_lo, c_hi; };
 
-// One quad (points 4Q .. 4Q+3) of the generic path of phase 1.
+// One quad (points 4Q .. 4Q+3) of a window-edge (peak, tile) pair in phase 1: quads outside the window are
+// skipped, out-of-window points of a partial quad get a zero coefficient, the Gaussian is added if the core
+// touches the quad.  One compact body per quad (these pairs are 2 of ~10 per peak; code size matters more).
 template <int Q>
-__device__ __forceinline__ void fwd_quad_generic(const PeakGeo& g, float t0, float step, float cg, float cl,
+__device__ __forceinline__ void fwd_quad_generic(const PeakGeo& g, float t0, float step, float cg2, float cl,
                                                  float (&acc)[kPT]) {
     const int lo = max(g.p_lo, 4 * Q), hi = min(g.p_hi, 4 * Q + 3);
     if (lo > hi) return;                                   // quad outside the window
-    const bool core = g.c_hi >= 4 * Q && g.c_lo <= 4 * Q + 3;
-    const float t_0 = fmaf(static_cast<float>(4 * Q), step, t0), t_1 = fmaf(static_cast<float>(4 * Q + 1), step, t0);
-    const float t_2 = fmaf(static_cast<float>(4 * Q + 2), step, t0), t_3 = fmaf(static_cast<float>(4 * Q + 3), step, t0);
-    if (hi - lo == 3) {
-        if (core) {
-            fwd_pair<true>(t_0, t_1, cg, cl, acc[4 * Q], acc[4 * Q + 1]);
-            fwd_pair<true>(t_2, t_3, cg, cl, acc[4 * Q + 2], acc[4 * Q + 3]);
-        } else {
-            fwd_pair<false>(t_0, t_1, cg, cl, acc[4 * Q], acc[4 * Q + 1]);
-            fwd_pair<false>(t_2, t_3, cg, cl, acc[4 * Q + 2], acc[4 * Q + 3]);
-        }
-    } else {
-        const unsigned span = static_cast<unsigned>(hi - lo);
-        const bool m0 = static_cast<unsigned>(4 * Q - lo) <= span, m1 = static_cast<unsigned>(4 * Q + 1 - lo) <= span;
-        const bool m2 = static_cast<unsigned>(4 * Q + 2 - lo) <= span, m3 = static_cast<unsigned>(4 * Q + 3 - lo) <= span;
-        if (core) {
-            fwd_pair_masked<true>(t_0, t_1, m0 ? cg : 0.f, m1 ? cg : 0.f, m0 ? cl : 0.f, m1 ? cl : 0.f, acc[4 * Q], acc[4 * Q + 1]);
-            fwd_pair_masked<true>(t_2, t_3, m2 ? cg : 0.f, m3 ? cg : 0.f, m2 ? cl : 0.f, m3 ? cl : 0.f, acc[4 * Q + 2], acc[4 * Q + 3]);
-        } else {
-            fwd_pair_masked<false>(t_0, t_1, 0.f, 0.f, m0 ? cl : 0.f, m1 ? cl : 0.f, acc[4 * Q], acc[4 * Q + 1]);
-            fwd_pair_masked<false>(t_2, t_3, 0.f, 0.f, m2 ? cl : 0.f, m3 ? cl : 0.f, acc[4 * Q + 2], acc[4 * Q + 3]);
-        }
+    const unsigned span = static_cast<unsigned>(hi - lo);
+    float u[4], m[4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const float t = fmaf(static_cast<float>(4 * Q + i), step, t0);
+        u[i] = fmaf(t, t, 1.0f);
+        m[i] = static_cast<unsigned>(4 * Q + i - lo) <= span ? 1.0f : 0.0f;
+    }
+    const float r01 = rcp_approx(u[0] * u[1]) * cl, r23 = rcp_approx(u[2] * u[3]) * cl;
+    acc[4 * Q] = fmaf(r01 * u[1], m[0], acc[4 * Q]);
+    acc[4 * Q + 1] = fmaf(r01 * u[0], m[1], acc[4 * Q + 1]);
+    acc[4 * Q + 2] = fmaf(r23 * u[3], m[2], acc[4 * Q + 2]);
+    acc[4 * Q + 3] = fmaf(r23 * u[2], m[3], acc[4 * Q + 3]);
+    if (g.c_hi >= 4 * Q && g.c_lo <= 4 * Q + 3) {
+#pragma unroll
+        for (int i = 0; i < 4; ++i) acc[4 * Q + i] = fmaf(cg2 * m[i], ex2_approx(-u[i]), acc[4 * Q + i]);
     }
 }
 
@@ -330,24 +312,33 @@ __device__ __forceinline__ void bwd_quad_generic(const PeakGeo& g, float t0, flo
                                                  const float (&pe)[kPT], Acc6& a) {
     const int lo = max(g.p_lo, 4 * Q), hi = min(g.p_hi, 4 * Q + 3);
     if (lo > hi) return;
-    const bool core = g.c_hi >= 4 * Q && g.c_lo <= 4 * Q + 3;
-    const float t_0 = fmaf(static_cast<float>(4 * Q), step, t0), t_1 = fmaf(static_cast<float>(4 * Q + 1), step, t0);
-    const float t_2 = fmaf(static_cast<float>(4 * Q + 2), step, t0), t_3 = fmaf(static_cast<float>(4 * Q + 3), step, t0);
-    float e0 = e[4 * Q], e1 = e[4 * Q + 1], e2 = e[4 * Q + 2], e3 = e[4 * Q + 3];
-    float q0 = pe[4 * Q], q1 = pe[4 * Q + 1], q2 = pe[4 * Q + 2], q3 = pe[4 * Q + 3];
-    if (hi - lo != 3) {   // partial quad: out-of-window points get a zero residual
-        const unsigned span = static_cast<unsigned>(hi - lo);
-        if (static_cast<unsigned>(4 * Q - lo) > span) { e0 = 0.f; q0 = 0.f; }
-        if (static_cast<unsigned>(4 * Q + 1 - lo) > span) { e1 = 0.f; q1 = 0.f; }
-        if (static_cast<unsigned>(4 * Q + 2 - lo) > span) { e2 = 0.f; q2 = 0.f; }
-        if (static_cast<unsigned>(4 * Q + 3 - lo) > span) { e3 = 0.f; q3 = 0.f; }
+    const unsigned span = static_cast<unsigned>(hi - lo);
+    float u[4], ev[4], qv[4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const float t = fmaf(static_cast<float>(4 * Q + i), step, t0);
+        u[i] = fmaf(t, t, 1.0f);
+        const bool in = static_cast<unsigned>(4 * Q + i - lo) <= span;   // out-of-window points: zero residual
+        ev[i] = in ? e[4 * Q + i] : 0.0f;
+        qv[i] = in ? pe[4 * Q + i] : 0.0f;
     }
-    if (core) {
-        bwd_pair<true>(e0, e1, q0, q1, t_0, t_1, a);
-        bwd_pair<true>(e2, e3, q2, q3, t_2, t_3, a);
-    } else {
-        bwd_pair<false>(e0, e1, q0, q1, t_0, t_1, a);
-        bwd_pair<false>(e2, e3, q2, q3, t_2, t_3, a);
+    const float r01 = rcp_approx(u[0] * u[1]), r23 = rcp_approx(u[2] * u[3]);
+    const float L[4] = {r01 * u[1], r01 * u[0], r23 * u[3], r23 * u[2]};
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const float L2 = L[i] * L[i];
+        a.a1 = fmaf(ev[i], L[i], a.a1);
+        a.a5 = fmaf(ev[i], L2, a.a5);
+        a.a3p = fmaf(qv[i], L2, a.a3p);
+    }
+    if (g.c_hi >= 4 * Q && g.c_lo <= 4 * Q + 3) {
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const float gg = ex2_approx(-u[i]);
+            a.a2 = fmaf(ev[i], gg, a.a2);
+            a.a4p = fmaf(qv[i], gg, a.a4p);
+            a.a6u = fmaf(ev[i] * u[i], gg, a.a6u);
+        }
     }
 }
 
@@ -387,6 +378,24 @@ __device__ __forceinline__ float warp_reduce8(float (&v)[8]) {
     // a lane now holds the total of value c = 4*bit4 + 2*bit3 + bit2 of its lane index; move it to lane c
     const int src = ((lane & 4) ? 16 : 0) | ((lane & 2) ? 8 : 0) | ((lane & 1) ? 4 : 0);
     return __shfl_sync(0xffffffffu, w1, src);
+}
+
+// Poisson likelihood of one grid point (A12-A16; R24): y = (y - B) + B, f = S_F + B (A3);
+// returns (d ll / d f, the point's term of ll minus its f-independent part):
+//   e = y/f - 1,   term = y ln(f/y) + (y - f)   (-f if y = 0).
+// Kept out of line: it runs once per point and tile and would otherwise put ~1000 instructions (IEEE divisions,
+// log1pf) between the two hot phases of the kernel.
+__device__ __noinline__ float2 poisson_point(float ymb, float b, float s_f) {
+    const float yv = ymb + b, f = s_f + b;
+    const float diff = ymb - s_f;                           // y - f
+    float term;
+    if (yv > 0.0f) {
+        const float x = -diff / yv;                         // f/y - 1
+        term = yv * (log1pf(x) - x);
+    } else {
+        term = -f;
+    }
+    return make_float2(diff / f, term);
 }
 
 // Warp-uniform geometry of a window-edge (peak, tile) pair in tile coordinates.
@@ -517,16 +526,9 @@ elbo_tile_kernel(const Dev d, float* __restrict__ f_dbg, long long n_dbg) {
             for (int p = 0; p < kPT; ++p) {
                 ev[p] = 0.0f;
                 if (p <= plim) {
-                    const float b = bgp[i0 + p], ymb = yb[i0 + p];
-                    const float yv = ymb + b, f = acc[p] + b;   // y and f = S_F + B (A3)
-                    const float diff = ymb - acc[p];            // y - f
-                    ev[p] = diff / f;
-                    if (yv > 0.0f) {
-                        const float x = -diff / yv;             // f/y - 1
-                        ss = fmaf(yv, log1pf(x) - x, ss);
-                    } else {
-                        ss -= f;
-                    }
+                    const float2 ed = poisson_point(yb[i0 + p], bgp[i0 + p], acc[p]);
+                    ev[p] = ed.x;
+                    ss += ed.y;
                 }
             }
         }
