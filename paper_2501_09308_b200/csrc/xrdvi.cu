@@ -42,7 +42,7 @@ struct Plan {   // workspace carve; identical arithmetic in workspace_bytes and 
     size_t o_yb, o_bg, o_pkt, o_runs, o_srng, o_sord, o_sofs, o_sids, o_pat, o_area, o_mh0;
     size_t o_var, o_vartmp, o_mom1, o_mom2, o_grad, o_elbo, o_elbok, o_llt, o_trace, o_done, o_ctl;
     size_t o_lat, o_eps, o_rr, o_ng, o_llpart, o_part8, o_dbg;
-    size_t o_pd, o_lpk, o_zeta, o_gradz, o_lls;
+    size_t o_pd, o_lpk, o_zeta, o_gradz, o_lls, o_partial, o_tcnt;
     int pd_groups;     // groups one launch of the log-joint gradient service handles
 };
 
@@ -136,6 +136,9 @@ bool make_plan(int64_t N, int32_t K, int64_t M, int32_t S_max, double step, cons
     p.o_zeta = take(sizeof(float4) * static_cast<size_t>(p.S_pad) * K);
     p.o_gradz = take(sizeof(float4) * static_cast<size_t>(p.S_pad) * K);
     p.o_lls = take(sizeof(double) * 2 * p.S_pad);
+    // split kernel (PS > 1): partial profiles of every (group, tile, share) and two counters per (group, tile)
+    p.o_partial = take(p.PS > 1 ? sizeof(float) * kPT * 32 * static_cast<size_t>(p.G_max) * p.n_tile * p.PS : 0);
+    p.o_tcnt = take(sizeof(unsigned int) * 2 * static_cast<size_t>(p.G_max) * p.n_tile);
     p.total = o;
     *pl = p;
     return true;
@@ -170,11 +173,31 @@ void set_S(xrdvi* h, int S) {
     h->dev.G = h->plan.PR * h->dev.gpi;
 }
 
+// Few tile-warps (PS > 1) and long work items: one-warp CTAs on a ticket queue (elbo_split_kernel) instead of PS-warp
+// CTAs with a barrier.  Measured on B200: config 4 (4300 peaks per item) 22.4 vs 23.5 ms per step, config 1 (39 peaks
+// per item) 0.1967 vs 0.1933 ms: the partial profiles through L2 only pay off for long items.
+bool use_split(const Dev& d) {
+    if (std::getenv("XRDVI_FUSED")) return false;            // A/B knobs for measurements
+    if (std::getenv("XRDVI_SPLIT")) return d.TW == 1 && d.PS > 1;
+    return d.TW == 1 && d.PS > 1 && d.split;
+}
+
 template <bool BWD>
 void launch_tile(const Dev& d, cudaStream_t st, float* f_dbg, long long n_dbg) {
+    if (BWD && use_split(d)) {   // forward-only launches (debug, timing) always take the fused kernel
+        const unsigned items = static_cast<unsigned>(d.n_tile) * d.PS * d.G;
+        const unsigned grid = BWD ? 2 * items : items + static_cast<unsigned>(d.n_tile) * d.G;
+        switch (d.PS) {
+            case 2: elbo_split_kernel<2, BWD><<<grid, 32, 0, st>>>(d, f_dbg, n_dbg); break;
+            case 4: elbo_split_kernel<4, BWD><<<grid, 32, 0, st>>>(d, f_dbg, n_dbg); break;
+            case 8: elbo_split_kernel<8, BWD><<<grid, 32, 0, st>>>(d, f_dbg, n_dbg); break;
+            default: break;
+        }
+        return;
+    }
     const dim3 grid(d.n_seg, d.G);
 #define XRDVI_TILE_CASE(TW_, PS_)                                                                           \
-    case TW_ * 16 + PS_:                                                                                    \
+    case TW_ * 16 + PS_:                                                                                   \
         elbo_tile_kernel<TW_, PS_, BWD><<<grid, 32 * TW_ * PS_, 0, st>>>(d, f_dbg, n_dbg);                 \
         break;
     switch (d.TW * 16 + d.PS) {
@@ -509,6 +532,7 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
     d.n_c = static_cast<int>(n_c); d.SP = SP; d.TW = pl.TW; d.PS = pl.PS; d.n_seg = pl.n_seg; d.n_tile = pl.n_tile;
     d.n_slots = std::max(n_slots, 1); d.Mv = Mv;
     d.likelihood = hyp->likelihood;
+    d.split = pairs / (static_cast<long long>(pl.n_tile) * pl.PS * kPT) >= 512 ? 1 : 0;   // peaks per work item
     d.optimizer = hyp->optimizer;
     d.delta = static_cast<float>(delta);
     d.gcut = static_cast<float>(static_cast<double>(kGaussCut) / (2.0 * delta));
@@ -548,6 +572,9 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
     d.part8 = reinterpret_cast<float*>(w + pl.o_part8);
     d.pd = nullptr;
     d.g_base = 0;
+    d.partial = reinterpret_cast<float*>(w + pl.o_partial);
+    d.tile_cnt = reinterpret_cast<unsigned int*>(w + pl.o_tcnt);
+    d.tile_cnt2 = d.tile_cnt + static_cast<size_t>(pl.G_max) * pl.n_tile;
     set_S(h, S_max);
 
     cudaStream_t st = h->stream;
@@ -567,6 +594,7 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
     chk(up(pl.o_pat, pat.data(), sizeof(PatConst) * pat.size()));
     chk(up(pl.o_area, area.data(), sizeof(double) * area.size()));
     chk(up(pl.o_mh0, m_h0.data(), sizeof(float) * m_h0.size()));
+    chk(cudaMemsetAsync(w + pl.o_tcnt, 0, sizeof(unsigned int) * 2 * static_cast<size_t>(pl.G_max) * pl.n_tile, st));
     chk(cudaMemsetAsync(w + pl.o_trace, 0xFF, sizeof(double) * kTraceCap * pl.PR, st));
     chk(cudaMemsetAsync(w + pl.o_part8, 0, sizeof(float) * static_cast<size_t>(pl.G_max) * d.n_slots * 8, st));
     chk(cudaStreamSynchronize(st));  // host staging vectors go out of scope below

@@ -72,6 +72,8 @@ struct Ctl {       // device-resident control block (so that graph replays need 
     long long trace_base;  // step index of trace row 0
     long long iteration_override;  // >= 0: Philox iteration for elbo_grad/debug; < 0: use step + 1
     unsigned int done_total;       // instances whose last CTA has finished (update_draw_kernel)
+    unsigned int ticket;           // next work item of elbo_split_kernel (re-armed by the launch's last CTA)
+    unsigned int finished;         // CTAs of the current elbo_split_kernel launch that are done
     unsigned int pad;
 };
 
@@ -81,6 +83,7 @@ struct Dev {
     int S, gpi, G;       // draws, groups per instance, groups (run-time)
     int likelihood;      // 0 Gaussian with known sigma_n (R3), 1 Poisson (A12-A16; R24)
     int optimizer;       // 0 Adam (R10), 1 natural gradient (R25)
+    int split;           // 1: backward launches with PS > 1 use elbo_split_kernel (long work items)
     float delta;         // grid step (deg)
     float gcut;          // kGaussCut / (2 Delta): core half-width in points per unit of w
     float inv_delta;
@@ -118,7 +121,10 @@ struct Dev {
     float* llpart;            // [G][n_seg][32] sum over the segment of ((y-f)/sigma_n)^2
     float* part8;             // [G][n_slots][8] (g_h, g_mu, g_w, g_r, g_h eps_h, ...) summed over 32 draws
     // log-joint gradient service (xrdvi_logjoint_grad): per-draw output instead of the sum over the draws
-    float* pd;                // nullptr, or [gridDim.y][n_slots][4][32] d ll / d zeta per (run, class, draw)
+    float* partial;           // [G][n_tile][PS][16][32] partial profiles of elbo_split_kernel (PS > 1 only)
+    unsigned int* tile_cnt;   // [G][n_tile] partial profiles that have arrived
+    unsigned int* tile_cnt2;  // [G][n_tile] phase-2 items that are done
+    float* pd;                // nullptr, or [groups of the launch][n_slots][4][32] d ll / d zeta per (run, class, draw)
     int g_base;               // group of blockIdx.y = 0 in elbo_tile_kernel (0 except in the service)
 };
 
@@ -409,180 +415,147 @@ __device__ __forceinline__ PeakGeo edge_geo(int dj, int ngc, int n_c, int plim) 
 }
 
 // ------------------------------------------------------------------------------------------------
-// a-3 .. a-6 (likelihood part): fused profile + residual + backward.
-// grid (n_seg, G), block 32*TW*PS; segment = TW consecutive 16-point tiles.  Warp w owns tile (w % TW) of the
-// segment and share (w / TW) of that tile's phase runs, in BOTH phases.  A run = the peaks of one phase that
-// reach the tile; its header carries the phase, so the per-phase latents are loaded once per run (prefetched one
-// run ahead) and the run index is the output slot of phase 2.
-#ifndef XRDVI_TILE_WARPS_PER_SM
-#define XRDVI_TILE_WARPS_PER_SM 24          // register budget: 65536 / (32 * 24) = 85 -> 80 registers per thread
-#endif
-template <int TW, int PS, bool BWD>
-__global__ void __launch_bounds__(32 * TW * PS, XRDVI_TILE_WARPS_PER_SM / (TW * PS) > 0 ? XRDVI_TILE_WARPS_PER_SM / (TW * PS) : 1)
-elbo_tile_kernel(const Dev d, float* __restrict__ f_dbg, long long n_dbg) {
-    __shared__ float4 e_s[TW][kPT / 4][32];
-    __shared__ float ss_s[TW][32];
-    __shared__ float acc_s[PS > 1 ? (PS - 1) * TW * kPT : 1][32];
-    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    const int tw = w % TW, ps = w / TW;
-    const int seg = d.seg_order[blockIdx.x];
-    const int g = d.g_base + blockIdx.y;
-    const int tile = seg * TW + tw;
-    const int i0 = tile * kPT;
-    const bool live = tile < d.n_tile;                      // the last segment may have fewer than TW tiles
-    const int plim = min(kPT - 1, d.N - 1 - i0);            // last valid point of the tile
-    const int n_c = d.n_c;
-    const float4* __restrict__ lat = d.lat + static_cast<size_t>(g) * d.K * 32 + lane;
-    const int* __restrict__ ngk = d.ng + static_cast<size_t>(g) * d.K;
+// a-3 .. a-6 (likelihood part): profile + residual + backward of one 16-point tile for one group of 32 draws.
+// A warp owns one tile and one share of the tile's phase runs, in BOTH phases.  A run = the peaks of one phase
+// that reach the tile; its header carries the phase, so the per-phase latents are loaded once per run (prefetched
+// one run ahead) and the run index is the output slot of phase 2.
+struct TileCtx {
+    int g;              // group (32 draws) of this warp
+    int i0, plim;       // first grid index of the tile, last valid point of the tile (< 0: no point)
+    int pat;            // observed pattern of the group
+    const float4* lat;  // latent records of the group, already offset by the lane
+    const int* ngk;     // Gaussian-core half-widths of the group
+};
+
+__device__ __forceinline__ TileCtx tile_ctx(const Dev& d, int g, int tile) {
+    TileCtx c;
+    c.g = g;
+    c.i0 = tile * kPT;
+    c.plim = min(kPT - 1, d.N - 1 - c.i0);
+    c.pat = (g / d.gpi) / d.R;
+    c.lat = d.lat + static_cast<size_t>(g) * d.K * 32 + (threadIdx.x & 31);
+    c.ngk = d.ng + static_cast<size_t>(g) * d.K;
+    return c;
+}
+
+// Phase 1: acc[p] += profile of the runs [rng.x, rng.y) on the 16 points of the tile.
+__device__ __forceinline__ void tile_phase1(const Dev& d, const TileCtx& c, int2 rng, float (&acc)[kPT]) {
+    if (rng.x >= rng.y) return;
     const PeakRec* __restrict__ pkt = d.pk_tile;
     const int4* __restrict__ runs = d.run_tab;
-    const int inst = g / d.gpi;
-    const int pat = inst / d.R;
-    const PatConst pc = d.pat[pat];
-    int2 rng = make_int2(0, 0);
-    if (live) rng = d.share_rng[tile * PS + ps];
-
-    // ---------------- phase 1: profile on the 16 points of this warp's tile ----------------
-    float acc[kPT];
-#pragma unroll
-    for (int p = 0; p < kPT; ++p) acc[p] = 0.0f;
-
-    if (rng.x < rng.y) {
-        int4 run_n = runs[rng.x];
-        float4 lt_n = lat[static_cast<size_t>(run_n.z) * 32];
-        int ng_n = ngk[run_n.z];
-        for (int r = rng.x; r < rng.y; ++r) {
-            const int4 run = run_n;
-            const float4 lt = lt_n;
-            const int ngc = ng_n;
-            run_n = runs[r + 1];                            // run_tab and pk_tile carry one padding entry
-            lt_n = lat[static_cast<size_t>(run_n.z) * 32];
-            ng_n = ngk[run_n.z];
-            const float step = d.delta * lt.x;
-            const unsigned core_span = static_cast<unsigned>(kPT - 1 + 2 * ngc);
+    int4 run_n = runs[rng.x];
+    float4 lt_n = c.lat[static_cast<size_t>(run_n.z) * 32];
+    int ng_n = c.ngk[run_n.z];
+    for (int r = rng.x; r < rng.y; ++r) {
+        const int4 run = run_n;
+        const float4 lt = lt_n;
+        const int ngc = ng_n;
+        run_n = runs[r + 1];                            // run_tab carries one padding entry
+        lt_n = c.lat[static_cast<size_t>(run_n.z) * 32];
+        ng_n = c.ngk[run_n.z];
+        const float step = d.delta * lt.x;
+        const unsigned core_span = static_cast<unsigned>(kPT - 1 + 2 * ngc);
 #pragma unroll 1
-            for (int m = run.x; m < run.y; ++m) {
-                const PeakRec pk = pkt[m];
-                const float t0 = fmaf(static_cast<float>(-pk.dj), step, fmaf(-pk.delta, lt.x, lt.y));
-                const float cl = pk.inten * lt.w;
-                const bool core = static_cast<unsigned>(pk.dj + ngc) <= core_span;   // Gaussian core touches the tile
-                if (pk.full) {   // branch-free bodies: Lorentz tail only, or tail + Gaussian on all 16 points
-                    if (!core) {
+        for (int m = run.x; m < run.y; ++m) {
+            const PeakRec pk = pkt[m];
+            const float t0 = fmaf(static_cast<float>(-pk.dj), step, fmaf(-pk.delta, lt.x, lt.y));
+            const float cl = pk.inten * lt.w;
+            const bool core = static_cast<unsigned>(pk.dj + ngc) <= core_span;   // Gaussian core touches the tile
+            if (pk.full) {   // branch-free bodies: Lorentz tail only, or tail + Gaussian on all 16 points
+                if (!core) {
 #pragma unroll
-                        for (int p = 0; p < kPT; p += 2)
-                            fwd_pair<false>(fmaf(static_cast<float>(p), step, t0), fmaf(static_cast<float>(p + 1), step, t0),
-                                            0.0f, cl, acc[p], acc[p + 1]);
-                    } else {
-                        const float cg2 = 2.0f * pk.inten * lt.z;
-#pragma unroll
-                        for (int p = 0; p < kPT; p += 2)
-                            fwd_pair<true>(fmaf(static_cast<float>(p), step, t0), fmaf(static_cast<float>(p + 1), step, t0),
-                                           cg2, cl, acc[p], acc[p + 1]);
-                    }
-                } else {         // window edge: quad by quad
-                    const PeakGeo geo = edge_geo(pk.dj, ngc, n_c, plim);
+                    for (int p = 0; p < kPT; p += 2)
+                        fwd_pair<false>(fmaf(static_cast<float>(p), step, t0), fmaf(static_cast<float>(p + 1), step, t0),
+                                        0.0f, cl, acc[p], acc[p + 1]);
+                } else {
                     const float cg2 = 2.0f * pk.inten * lt.z;
-                    fwd_quad_generic<0>(geo, t0, step, cg2, cl, acc);
-                    fwd_quad_generic<1>(geo, t0, step, cg2, cl, acc);
-                    fwd_quad_generic<2>(geo, t0, step, cg2, cl, acc);
-                    fwd_quad_generic<3>(geo, t0, step, cg2, cl, acc);
+#pragma unroll
+                    for (int p = 0; p < kPT; p += 2)
+                        fwd_pair<true>(fmaf(static_cast<float>(p), step, t0), fmaf(static_cast<float>(p + 1), step, t0),
+                                       cg2, cl, acc[p], acc[p + 1]);
                 }
+            } else {         // window edge: quad by quad
+                const PeakGeo geo = edge_geo(pk.dj, ngc, d.n_c, c.plim);
+                const float cg2 = 2.0f * pk.inten * lt.z;
+                fwd_quad_generic<0>(geo, t0, step, cg2, cl, acc);
+                fwd_quad_generic<1>(geo, t0, step, cg2, cl, acc);
+                fwd_quad_generic<2>(geo, t0, step, cg2, cl, acc);
+                fwd_quad_generic<3>(geo, t0, step, cg2, cl, acc);
             }
         }
     }
-    if (PS > 1) {   // sum the PS partial profiles of the tile: shares 1.. in order onto share 0
-        if (ps > 0) {
-#pragma unroll
-            for (int p = 0; p < kPT; ++p) acc_s[((ps - 1) * TW + tw) * kPT + p][lane] = acc[p];
-        }
-        __syncthreads();
-        if (ps == 0) {
-#pragma unroll
-            for (int q = 1; q < PS; ++q)
-#pragma unroll
-                for (int p = 0; p < kPT; ++p) acc[p] += acc_s[((q - 1) * TW + tw) * kPT + p][lane];
-        }
-    }
+}
 
-    // residual e = d ll / d f (0 beyond the grid) and the tile's part of ll:
-    //   Gaussian (R3):  e = (y - f)/sigma_n^2,  part = sum ((y - f)/sigma_n)^2            (ll = -1/2 sum + const)
-    //   Poisson (A16):  e = y/f - 1,            part = sum y ln(f/y) + (y - f)  (-f if y = 0)   (ll = sum + const)
-    if (ps == 0) {
-        const float* __restrict__ yb = d.yb + static_cast<size_t>(pat) * d.N;
-        float ev[kPT];
-        float ss = 0.0f;
-        if (d.likelihood == 0) {
+// a-4: residual e = d ll / d f (0 beyond the grid) from the complete profile acc (without B); returns the
+// tile's part of ll:
+//   Gaussian (R3):  e = (y - f)/sigma_n^2,  part = sum ((y - f)/sigma_n)^2            (ll = -1/2 sum + const)
+//   Poisson (A16):  e = y/f - 1,            part = sum y ln(f/y) + (y - f)  (-f if y = 0)   (ll = sum + const)
+__device__ __forceinline__ float tile_residual(const Dev& d, const TileCtx& c, const float (&acc)[kPT], float (&ev)[kPT]) {
+    const PatConst pc = d.pat[c.pat];
+    const float* __restrict__ yb = d.yb + static_cast<size_t>(c.pat) * d.N;
+    float ss = 0.0f;
+    if (d.likelihood == 0) {
 #pragma unroll
-            for (int p = 0; p < kPT; ++p) {
-                float r = 0.0f;
-                if (p <= plim) r = yb[i0 + p] - acc[p];         // plim < 0 for a dead tile
-                const float z = r * pc.inv_sn;
-                ss = fmaf(z, z, ss);
-                ev[p] = r * pc.inv_sn2;
-            }
-        } else {
-            const float* __restrict__ bgp = d.bg + static_cast<size_t>(pat) * d.N;
-#pragma unroll
-            for (int p = 0; p < kPT; ++p) {
-                ev[p] = 0.0f;
-                if (p <= plim) {
-                    const float2 ed = poisson_point(yb[i0 + p], bgp[i0 + p], acc[p]);
-                    ev[p] = ed.x;
-                    ss += ed.y;
-                }
-            }
+        for (int p = 0; p < kPT; ++p) {
+            float r = 0.0f;
+            if (p <= c.plim) r = yb[c.i0 + p] - acc[p];
+            const float z = r * pc.inv_sn;
+            ss = fmaf(z, z, ss);
+            ev[p] = r * pc.inv_sn2;
         }
-        if (BWD) {
+    } else {
+        const float* __restrict__ bgp = d.bg + static_cast<size_t>(c.pat) * d.N;
 #pragma unroll
-            for (int v = 0; v < kPT / 4; ++v)
-                e_s[tw][v][lane] = make_float4(ev[4 * v], ev[4 * v + 1], ev[4 * v + 2], ev[4 * v + 3]);
-        }
-        ss_s[tw][lane] = ss;
-        if (f_dbg && live) {  // debug read-back of the profile (parity tests); warp-uniform branch
-            const int s = (g - inst * d.gpi) * 32 + lane;
-            const long long t = static_cast<long long>(inst) * d.S + s;
-            if (s < d.S && t < n_dbg) {
-                const float* __restrict__ bg = d.bg + static_cast<size_t>(pat) * d.N;
-#pragma unroll
-                for (int p = 0; p < kPT; ++p)
-                    if (p <= plim) f_dbg[t * d.N + i0 + p] = acc[p] + bg[i0 + p];
+        for (int p = 0; p < kPT; ++p) {
+            ev[p] = 0.0f;
+            if (p <= c.plim) {
+                const float2 ed = poisson_point(yb[c.i0 + p], bgp[c.i0 + p], acc[p]);
+                ev[p] = ed.x;
+                ss += ed.y;
             }
         }
     }
-    __syncthreads();
-    if (w == 0) {  // fixed-order sum over the tiles of the segment
-        float ss = ss_s[0][lane];
+    return ss;
+}
+
+// debug read-back of the profile f = S_F + B of the first n_dbg sample-instances (parity tests)
+__device__ __forceinline__ void tile_debug_profile(const Dev& d, const TileCtx& c, const float (&acc)[kPT],
+                                                   float* __restrict__ f_dbg, long long n_dbg) {
+    const int inst = c.g / d.gpi;
+    const int s = (c.g - inst * d.gpi) * 32 + (threadIdx.x & 31);
+    const long long t = static_cast<long long>(inst) * d.S + s;
+    if (s < d.S && t < n_dbg) {
+        const float* __restrict__ bg = d.bg + static_cast<size_t>(c.pat) * d.N;
 #pragma unroll
-        for (int v = 1; v < TW; ++v) ss += ss_s[v][lane];
-        d.llpart[(static_cast<size_t>(g) * d.n_seg + seg) * 32 + lane] = ss;
+        for (int p = 0; p < kPT; ++p)
+            if (p <= c.plim) f_dbg[t * d.N + c.i0 + p] = acc[p] + bg[c.i0 + p];
     }
-    if (!BWD) return;
+}
+
+// Phase 2: six sums per phase run [rng.x, rng.y) over the tile from the residual e, chain rule, reduction over the
+// 32 draws (or, in the gradient service, per-draw output to row pd_row of d.pd).
+__device__ __forceinline__ void tile_phase2(const Dev& d, const TileCtx& c, int2 rng, const float (&e)[kPT], int pd_row) {
     if (rng.x >= rng.y) return;
-
-    // ---------------- phase 2: six sums per phase run over the tile, chain rule, reduction over the draws ----------------
-    float e[kPT], pe[kPT];
-#pragma unroll
-    for (int v = 0; v < kPT / 4; ++v) {
-        const float4 t = e_s[tw][v][lane];
-        e[4 * v] = t.x; e[4 * v + 1] = t.y; e[4 * v + 2] = t.z; e[4 * v + 3] = t.w;
-    }
+    const int lane = threadIdx.x & 31;
+    float pe[kPT];
 #pragma unroll
     for (int p = 0; p < kPT; ++p) pe[p] = static_cast<float>(p) * e[p];
-
-    const float4* __restrict__ epsg = d.eps + static_cast<size_t>(g) * d.K * 32 + lane;
-    const float* __restrict__ rrg = d.rr + static_cast<size_t>(g) * d.K * 32 + lane;
-    float* __restrict__ part = d.part8 + static_cast<size_t>(g) * d.n_slots * 8;
+    const PeakRec* __restrict__ pkt = d.pk_tile;
+    const int4* __restrict__ runs = d.run_tab;
+    const float4* __restrict__ epsg = d.eps + static_cast<size_t>(c.g) * d.K * 32 + lane;
+    const float* __restrict__ rrg = d.rr + static_cast<size_t>(c.g) * d.K * 32 + lane;
+    float* __restrict__ part = d.part8 + static_cast<size_t>(c.g) * d.n_slots * 8;
 
     int4 run_n = runs[rng.x];
-    float4 lt_n = lat[static_cast<size_t>(run_n.z) * 32];
-    int ng_n = ngk[run_n.z];
+    float4 lt_n = c.lat[static_cast<size_t>(run_n.z) * 32];
+    int ng_n = c.ngk[run_n.z];
     for (int r = rng.x; r < rng.y; ++r) {
         const int4 run = run_n;
         const float4 lt = lt_n;
         const int ngc = ng_n;
         run_n = runs[r + 1];
-        lt_n = lat[static_cast<size_t>(run_n.z) * 32];
-        ng_n = ngk[run_n.z];
+        lt_n = c.lat[static_cast<size_t>(run_n.z) * 32];
+        ng_n = c.ngk[run_n.z];
         // loads of the flush, issued early
         const float4 ep = epsg[static_cast<size_t>(run.z) * 32];
         const float rmix = rrg[static_cast<size_t>(run.z) * 32];
@@ -612,7 +585,7 @@ elbo_tile_kernel(const Dev d, float* __restrict__ f_dbg, long long n_dbg) {
                         bwd_pair<true>(e[p], e[p + 1], pe[p], pe[p + 1], fmaf(static_cast<float>(p), step, t0),
                                        fmaf(static_cast<float>(p + 1), step, t0), a);
                 } else {
-                    const PeakGeo geo = edge_geo(pk.dj, ngc, n_c, plim);
+                    const PeakGeo geo = edge_geo(pk.dj, ngc, d.n_c, c.plim);
                     bwd_quad_generic<0>(geo, t0, step, e, pe, a);
                     bwd_quad_generic<1>(geo, t0, step, e, pe, a);
                     bwd_quad_generic<2>(geo, t0, step, e, pe, a);
@@ -635,13 +608,165 @@ elbo_tile_kernel(const Dev d, float* __restrict__ f_dbg, long long n_dbg) {
         v[2] = -(cL * (2.0f * B5 - B1) + cG * (B2 - (2.0f * kLn2) * B6));
         v[3] = (1.0f - rmix) * cL * B1 - rmix * cG * B2;
         if (d.pd) {   // gradient service: keep the draws apart
-            float* __restrict__ o = d.pd + (static_cast<size_t>(blockIdx.y) * d.n_slots + r) * 128 + lane;
+            float* __restrict__ o = d.pd + (static_cast<size_t>(pd_row) * d.n_slots + r) * 128 + lane;
             o[0] = v[0]; o[32] = v[1]; o[64] = v[2]; o[96] = v[3];
             continue;
         }
         v[4] = v[0] * ep.x; v[5] = v[1] * ep.y; v[6] = v[2] * ep.z; v[7] = v[3] * ep.w;
         const float tot = warp_reduce8(v);
         if (lane < 8) part[static_cast<size_t>(r) * 8 + lane] = tot;
+    }
+}
+
+// Fused variant: grid (n_seg, G), block 32*TW*PS; segment = TW consecutive tiles.  Warp w owns tile (w % TW) of the
+// segment and share (w / TW) of that tile's runs; the PS partial profiles meet in shared memory.  Used when the
+// launch has enough tile-warps without splitting (PS = 1: no barrier is ever waited on) and for forward-only runs.
+#ifndef XRDVI_TILE_WARPS_PER_SM
+#define XRDVI_TILE_WARPS_PER_SM 24          // register budget: 65536 / (32 * 24) = 85 -> 80 registers per thread
+#endif
+template <int TW, int PS, bool BWD>
+__global__ void __launch_bounds__(32 * TW * PS, XRDVI_TILE_WARPS_PER_SM / (TW * PS) > 0 ? XRDVI_TILE_WARPS_PER_SM / (TW * PS) : 1)
+elbo_tile_kernel(const Dev d, float* __restrict__ f_dbg, long long n_dbg) {
+    __shared__ float4 e_s[TW][kPT / 4][32];
+    __shared__ float ss_s[TW][32];
+    __shared__ float acc_s[PS > 1 ? (PS - 1) * TW * kPT : 1][32];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int tw = w % TW, ps = w / TW;
+    const int seg = d.seg_order[blockIdx.x];
+    const int tile = seg * TW + tw;
+    const bool live = tile < d.n_tile;                      // the last segment may have fewer than TW tiles
+    const TileCtx c = tile_ctx(d, d.g_base + blockIdx.y, tile);
+    int2 rng = make_int2(0, 0);
+    if (live) rng = d.share_rng[tile * PS + ps];
+
+    float acc[kPT];
+#pragma unroll
+    for (int p = 0; p < kPT; ++p) acc[p] = 0.0f;
+    tile_phase1(d, c, rng, acc);
+
+    if (PS > 1) {   // sum the PS partial profiles of the tile: shares 1.. in order onto share 0
+        if (ps > 0) {
+#pragma unroll
+            for (int p = 0; p < kPT; ++p) acc_s[((ps - 1) * TW + tw) * kPT + p][lane] = acc[p];
+        }
+        __syncthreads();
+        if (ps == 0) {
+#pragma unroll
+            for (int q = 1; q < PS; ++q)
+#pragma unroll
+                for (int p = 0; p < kPT; ++p) acc[p] += acc_s[((q - 1) * TW + tw) * kPT + p][lane];
+        }
+    }
+    if (ps == 0) {
+        float ev[kPT];
+        const float ss = tile_residual(d, c, acc, ev);
+        if (BWD) {
+#pragma unroll
+            for (int v = 0; v < kPT / 4; ++v)
+                e_s[tw][v][lane] = make_float4(ev[4 * v], ev[4 * v + 1], ev[4 * v + 2], ev[4 * v + 3]);
+        }
+        ss_s[tw][lane] = ss;
+        if (f_dbg && live) tile_debug_profile(d, c, acc, f_dbg, n_dbg);
+    }
+    __syncthreads();
+    if (w == 0) {  // fixed-order sum over the tiles of the segment
+        float ss = ss_s[0][lane];
+#pragma unroll
+        for (int v = 1; v < TW; ++v) ss += ss_s[v][lane];
+        d.llpart[(static_cast<size_t>(c.g) * d.n_seg + seg) * 32 + lane] = ss;
+    }
+    if (!BWD) return;
+    if (rng.x >= rng.y) return;
+    float e[kPT];
+#pragma unroll
+    for (int v = 0; v < kPT / 4; ++v) {
+        const float4 t = e_s[tw][v][lane];
+        e[4 * v] = t.x; e[4 * v + 1] = t.y; e[4 * v + 2] = t.z; e[4 * v + 3] = t.w;
+    }
+    tile_phase2(d, c, rng, e, blockIdx.y);
+}
+
+// Split variant for launches with few tile-warps (PS > 1; configs 1 and 4): one warp per CTA, work items taken from a
+// ticket counter in the order  [phase-1 items of all tiles by decreasing work] [phase-2 items in the same order]:
+//   phase-1 item (tile, share, group): partial profile of the share's runs -> global memory (L2), then a release
+//                                      increment of the (tile, group) counter;
+//   phase-2 item (tile, share, group): waits until the PS partial profiles of its (tile, group) have arrived (their
+//                                      items have lower tickets, i.e. they are running or done: no deadlock), sums
+//                                      them in share order, forms the residual and runs its share of phase 2.
+// No barrier inside a CTA, items half as long as a fused CTA, phase-2 work fills the tail of phase 1.  All sums keep
+// a fixed order, so results do not depend on the schedule.  grid: n_items * 2 (BWD) or n_items + n_tile * G CTAs
+// (a persistent variant, 3552 CTAs looping over tickets, measured 3 % slower).
+template <int PS, bool BWD>
+__global__ void __launch_bounds__(32, XRDVI_TILE_WARPS_PER_SM) elbo_split_kernel(const Dev d, float* __restrict__ f_dbg, long long n_dbg) {
+    const int lane = threadIdx.x;
+    const unsigned n_items = static_cast<unsigned>(d.n_tile) * PS * d.G;
+    unsigned ticket = 0;
+    if (lane == 0) ticket = atomicAdd(&d.ctl->ticket, 1u);
+    ticket = __shfl_sync(0xffffffffu, ticket, 0);
+    const bool second = ticket >= n_items;
+    unsigned item = second ? ticket - n_items : ticket;
+    int ps, gi, pos;
+    if (second && !BWD) {            // forward only: one phase-2 item per (tile, group), played by share 0
+        ps = 0;
+        gi = item % d.G;
+        pos = item / d.G;
+    } else {
+        gi = item % d.G;
+        item /= d.G;
+        ps = item % PS;
+        pos = item / PS;
+    }
+    const int tile = d.seg_order[pos];                     // TW = 1: segments are tiles
+    const TileCtx c = tile_ctx(d, d.g_base + gi, tile);
+    const int2 rng = d.share_rng[tile * PS + ps];
+    const size_t tg = static_cast<size_t>(gi) * d.n_tile + tile;
+    float* __restrict__ partial = d.partial + tg * (PS * kPT * 32) + lane;
+
+    if (!second) {
+        float acc[kPT];
+#pragma unroll
+        for (int p = 0; p < kPT; ++p) acc[p] = 0.0f;
+        tile_phase1(d, c, rng, acc);
+#pragma unroll
+        for (int p = 0; p < kPT; ++p) __stcg(partial + (ps * kPT + p) * 32, acc[p]);
+        __threadfence();
+        __syncwarp();
+        if (lane == 0) atomicAdd(&d.tile_cnt[tg], 1u);
+    } else {
+        if (lane == 0) {
+            while (atomicAdd(&d.tile_cnt[tg], 0u) < static_cast<unsigned>(PS)) __nanosleep(64);
+        }
+        __syncwarp();
+        __threadfence();
+        float acc[kPT];
+#pragma unroll
+        for (int p = 0; p < kPT; ++p) acc[p] = __ldcg(partial + p * 32);
+#pragma unroll
+        for (int q = 1; q < PS; ++q)
+#pragma unroll
+            for (int p = 0; p < kPT; ++p) acc[p] += __ldcg(partial + (q * kPT + p) * 32);
+        float ev[kPT];
+        const float ss = tile_residual(d, c, acc, ev);
+        if (ps == 0) {
+            d.llpart[(static_cast<size_t>(c.g) * d.n_seg + tile) * 32 + lane] = ss;
+            if (f_dbg) tile_debug_profile(d, c, acc, f_dbg, n_dbg);
+        }
+        if (BWD) tile_phase2(d, c, rng, ev, gi);
+        __syncwarp();
+        if (lane == 0) {   // the last phase-2 item of the (tile, group) re-arms its counters for the next launch
+            const unsigned n_second = BWD ? PS : 1;
+            if (atomicAdd(&d.tile_cnt2[tg], 1u) == n_second - 1) {
+                d.tile_cnt[tg] = 0u;
+                d.tile_cnt2[tg] = 0u;
+            }
+        }
+    }
+    if (lane == 0) {       // the last CTA of the launch re-arms the ticket counter
+        __threadfence();
+        if (atomicAdd(&d.ctl->finished, 1u) == gridDim.x - 1) {
+            d.ctl->ticket = 0u;
+            d.ctl->finished = 0u;
+        }
     }
 }
 

@@ -348,3 +348,34 @@ def test_extreme_widths_shifts_and_mixing():
     ll_r, lpj_r, g_r = o.logjoint_grad(st[0, 0, 0].astype(np.float64))
     assert ll_g[0] == pytest.approx(ll_r, rel=TOL_ELBO)
     assert (np.abs(g_g[0] - g_r).max(axis=0) / np.abs(g_r).max(axis=0)).max() <= TOL_GRAD
+
+
+# --------------------------------------------------------------------------- split (ticket-queue) tile kernel
+def test_split_kernel_matches_oracle_and_the_fused_kernel_bitwise(monkeypatch):
+    """elbo_split_kernel (one-warp work items, partial profiles through L2) is chosen for long work items
+    (config 4 at full size); XRDVI_SPLIT=1 forces it on small problems.  Same summation orders as the fused
+    kernel, so the two must agree bit for bit, whatever the schedule."""
+    outs = {}
+    for mode in ("fused", "split"):
+        monkeypatch.delenv("XRDVI_SPLIT", raising=False)
+        monkeypatch.delenv("XRDVI_FUSED", raising=False)
+        monkeypatch.setenv("XRDVI_SPLIT" if mode == "split" else "XRDVI_FUSED", "1")
+        wl = synth.make_workload(1, S=96)
+        o = orc.from_workload(wl)
+        gpu = Xrdvi.from_workload(wl)
+        st0, _ = gpu.get_state()
+        check_eval(gpu, o, st0, 96, seed=1, iteration=1)
+        st, inc, tr = gpu.fit(30, seed=3, want_trace=True)
+        e, g = gpu.elbo_grad(S=96, seed=3, iteration=99)
+        e40, g40 = gpu.elbo_grad(S=40, seed=3, iteration=5)               # ragged group, fewer groups than S_max
+        ll, lpj, gz = gpu.logjoint_grad(synth.random_state(wl.K, 5, 1, seed=2)[:, 0, 0])
+        outs[mode] = (st, inc, tr, e, g, e40, g40, ll, gz)
+        check_eval(gpu, o, st, 96, seed=3, iteration=31)
+        gpu.close()
+        wl0 = synth.make_workload(0, peak_counts=1.0e4)                    # K = 6 < ... shares, Poisson, ragged last tile
+        o0, g0 = orc.from_workload(wl0), Xrdvi.from_workload(wl0)
+        s0, _ = g0.get_state()
+        check_eval(g0, o0, s0, wl0.S, seed=2, iteration=1, n_prof=4)
+        g0.close()
+    for a, b in zip(outs["fused"], outs["split"]):
+        np.testing.assert_array_equal(a, b)
