@@ -131,3 +131,44 @@ def test_config4_full_size():
     np.testing.assert_allclose(ll_g, ll_r[0], rtol=TOL_ELBO)
     np.testing.assert_allclose(elbo_g[0, 0], e_r[0], rtol=TOL_ELBO)
     assert class_err(grad_g[0, 0], g_r[0]) <= TOL_GRAD
+
+
+def _fit_parity(iterations):
+    """Fit config 1 at full size (K=50, S=256) on both sides with the same draws; compare what is unique (R22):
+    inclusion probabilities (north_star: 0.02 absolute), area ratios and the identified parameters of the planted
+    phases."""
+    wl = synth.make_workload(1)
+    o = orc.from_workload(wl)
+    gpu = Xrdvi.from_workload(wl)
+    st_g, inc_g, tr_g = gpu.fit(iterations, seed=1, want_trace=True)
+    st_r, _, tr_r = o.fit(o.init_state(), iterations, wl.S, seed=1, want_trace=True)
+    inc_r, area_r = o.inclusion(st_r, want_area=True)
+    _, area_g = gpu.inclusion()
+    d_inc = float(np.abs(inc_g - inc_r).max())
+    assert d_inc <= 0.02, d_inc
+    assert np.abs(area_g - area_r).max() <= 0.01
+    np.testing.assert_allclose(tr_g[:3, 0, 0], tr_r[:3, 0, 0], rtol=TOL_ELBO)
+    # later the fp32 and fp64 trajectories decorrelate (R22) and the S-draw ELBO estimate fluctuates from step to
+    # step: the tails agree as distributions, not entry by entry
+    n_tail = min(200, iterations // 2)
+    spread = float(tr_r[-n_tail:].std())
+    assert abs(float(np.median(tr_g[-n_tail:])) - float(np.median(tr_r[-n_tail:]))) <= max(spread, 1e-3 * abs(float(tr_r[-1, 0, 0])))
+    for k in wl.true_phases[0]:
+        np.testing.assert_allclose(st_g[0, 0, 0, k, :3], st_r[0, 0, 0, k, :3], atol=0.02)
+    print(f"fit parity, {iterations} iterations: max |dP_incl| = {d_inc:.2e}, max |d area ratio| = "
+          f"{float(np.abs(area_g - area_r).max()):.2e}, ELBO tail median GPU {float(np.median(tr_g[-n_tail:])):.2f} "
+          f"oracle {float(np.median(tr_r[-n_tail:])):.2f} (spread {spread:.1f})")
+    return d_inc, inc_g, inc_r, wl
+
+
+def test_config1_full_size_fit_inclusion_parity_200_iterations():
+    _fit_parity(200)
+
+
+@pytest.mark.skipif(not __import__("os").environ.get("XRDVI_LONG"), reason="8 min of fp64 oracle: set XRDVI_LONG=1")
+def test_config1_full_fit_2000_iterations_inclusion_parity():
+    d_inc, inc_g, inc_r, wl = _fit_parity(2000)
+    truth = wl.true_phases[0]
+    print("max |dP_incl| =", d_inc, "planted", truth, "P_incl(GPU) planted", inc_g[0, 0, truth],
+          "largest absent", np.delete(inc_g[0, 0], truth).max())
+    assert np.all(inc_g[0, 0, truth] > 0.99)
