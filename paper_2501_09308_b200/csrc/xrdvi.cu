@@ -365,7 +365,7 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
     if (reinterpret_cast<uintptr_t>(workspace) % 256) return fail(XRDVI_E_INVALID_ARG, "workspace not 256-byte aligned");
 
     // ---- fp64 preprocessing (R16) ----------------------------------------------------------------
-    const int P = pl.P, SP = pl.SP;
+    const int P = pl.P;
     long long n_c = pl.n_c;
     if (n_c < 0) {     // dense: every point is inside every window, wherever the peak lies
         n_c = N;
@@ -392,7 +392,6 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
             const double xj = (j >= 0 && j < N) ? x[j] : x[0] + delta * static_cast<double>(j);
             kept.push_back({j, pos[m] - xj, inten[m], k});
         }
-    const int Mv = static_cast<int>(kept.size());
     for (int k = 0; k < K; ++k)
         if (!(area[k] > 0.0)) return fail(XRDVI_E_EMPTY_PHASE, "phase " + std::to_string(k) + " has zero total intensity");
 
@@ -529,8 +528,8 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
     Dev& d = h->dev;
     char* w = h->ws;
     d.N = static_cast<int>(N); d.K = K; d.P = pl.P; d.R = pl.R; d.PR = pl.PR;
-    d.n_c = static_cast<int>(n_c); d.SP = SP; d.TW = pl.TW; d.PS = pl.PS; d.n_seg = pl.n_seg; d.n_tile = pl.n_tile;
-    d.n_slots = std::max(n_slots, 1); d.Mv = Mv;
+    d.n_c = static_cast<int>(n_c); d.TW = pl.TW; d.PS = pl.PS; d.n_seg = pl.n_seg; d.n_tile = pl.n_tile;
+    d.n_slots = std::max(n_slots, 1);
     d.likelihood = hyp->likelihood;
     d.split = pairs / (static_cast<long long>(pl.n_tile) * pl.PS * kPT) >= 512 ? 1 : 0;   // peaks per work item
     d.optimizer = hyp->optimizer;

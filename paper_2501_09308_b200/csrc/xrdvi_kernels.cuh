@@ -15,6 +15,8 @@
 //                      phase 2 accumulates the six backward sums of each peak over the 16 points, folds them
 //                      per phase, applies the chain rule and reduces over the 32 draws with warp shuffles
 //                      (fixed tree) to 8 floats per (tile, phase, group).
+//   elbo_split_kernel  the same two phases as one-warp work items on a ticket queue, partial profiles through
+//                      L2 instead of a CTA barrier; chosen for launches with few tile-warps and long items.
 //   update_draw_kernel (a-6 prior part, a-7, a-8, a-1, a-2) one CTA per (phase, instance): fixed-order
 //                      reduction of the partials and of the per-draw prior terms, ELBO, Adam ascent
 //                      on the 8 variational parameters of the phase, then the Philox draws and the
@@ -79,7 +81,7 @@ struct Ctl {       // device-resident control block (so that graph replays need 
 
 struct Dev {
     // sizes
-    int N, K, P, R, PR, n_c, SP, n_seg, n_tile, n_slots, Mv, TW, PS;
+    int N, K, P, R, PR, n_c, n_seg, n_tile, n_slots, TW, PS;   // n_seg = ceil(n_tile / TW) segments of TW tiles
     int S, gpi, G;       // draws, groups per instance, groups (run-time)
     int likelihood;      // 0 Gaussian with known sigma_n (R3), 1 Poisson (A12-A16; R24)
     int optimizer;       // 0 Adam (R10), 1 natural gradient (R25)
@@ -118,7 +120,7 @@ struct Dev {
     float4* eps;              // [G][K][32]
     float* rr;                // [G][K][32]  r
     int* ng;                  // [G][K]      Gaussian core half-width in grid points
-    float* llpart;            // [G][n_seg][32] sum over the segment of ((y-f)/sigma_n)^2
+    float* llpart;            // [G][n_seg][32] the segment's part of ll (tile_residual), per draw
     float* part8;             // [G][n_slots][8] (g_h, g_mu, g_w, g_r, g_h eps_h, ...) summed over 32 draws
     // log-joint gradient service (xrdvi_logjoint_grad): per-draw output instead of the sum over the draws
     float* partial;           // [G][n_tile][PS][16][32] partial profiles of elbo_split_kernel (PS > 1 only)
