@@ -39,8 +39,8 @@ struct Plan {   // workspace carve; identical arithmetic in workspace_bytes and 
     int TW, PS, NW, SP, n_seg, n_tile;
     long long M, n_c, tile_cap, slots_cap;
     size_t total;
-    size_t o_yb, o_bg, o_pkt, o_runs, o_srng, o_sord, o_sofs, o_sids, o_pat, o_area, o_mh0;
-    size_t o_var, o_vartmp, o_mom1, o_mom2, o_grad, o_elbo, o_elbok, o_llt, o_trace, o_done, o_ctl;
+    size_t o_yb, o_bg, o_pkt, o_runs, o_srng, o_sord, o_sofs, o_pat, o_area, o_mh0;
+    size_t o_var, o_vartmp, o_mom1, o_mom2, o_grad, o_elbo, o_elbok, o_llt, o_trace, o_ctl;
     size_t o_lat, o_eps, o_rr, o_ng, o_llpart, o_part8, o_dbg;
     size_t o_pd, o_lpk, o_zeta, o_gradz, o_lls, o_partial, o_tcnt;
     int pd_groups;     // groups one launch of the log-joint gradient service handles
@@ -106,7 +106,6 @@ bool make_plan(int64_t N, int32_t K, int64_t M, int32_t S_max, double step, cons
     p.o_srng = take(sizeof(int2) * static_cast<size_t>(p.n_tile) * p.PS);
     p.o_sord = take(sizeof(int) * p.n_seg);
     p.o_sofs = take(sizeof(int) * (K + 1));
-    p.o_sids = take(sizeof(int) * std::max<long long>(p.slots_cap, 1));
     p.o_pat = take(sizeof(PatConst) * p.P);
     p.o_area = take(sizeof(double) * K);
     p.o_mh0 = take(sizeof(float) * p.P);
@@ -119,7 +118,6 @@ bool make_plan(int64_t N, int32_t K, int64_t M, int32_t S_max, double step, cons
     p.o_elbok = take(sizeof(double) * p.PR * (K + 1));
     p.o_llt = take(sizeof(double) * p.PR * p.S_pad);
     p.o_trace = take(sizeof(double) * kTraceCap * p.PR);
-    p.o_done = take(sizeof(unsigned int) * p.PR);
     p.o_ctl = take(sizeof(Ctl));
     p.o_lat = take(sizeof(float4) * gk32);
     p.o_eps = take(sizeof(float4) * gk32);
@@ -163,6 +161,7 @@ struct xrdvi {
     cudaGraphExec_t graph_exec = nullptr;
     int graph_S = -1;
     cudaEvent_t ev[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+
 };
 
 namespace {
@@ -217,8 +216,15 @@ void launch_draw(const Dev& d, cudaStream_t st, const float* var, uint4* raw_out
 // the draws of the next step.  The draws of the FIRST step come from launch_draw.
 int enqueue_step(xrdvi* h) {
     const Dev& d = h->dev;
-    launch_tile<true>(d, h->stream, nullptr, 0);
+    launch_tile<true>(d, h->stream, nullptr, 0);     // also assembles the previous step's ELBO and counts it
     update_draw_kernel<<<dim3(d.K + 1, d.PR), kUpdThreads, 0, h->stream>>>(d, d.var, 1);
+    CU(cudaGetLastError());
+    return XRDVI_OK;
+}
+
+// after the last step of a run (and after an evaluation): the pending ELBO assembly / step count
+int enqueue_finish(xrdvi* h) {
+    finish_step_kernel<<<1, 256, 0, h->stream>>>(h->dev);
     CU(cudaGetLastError());
     return XRDVI_OK;
 }
@@ -232,7 +238,7 @@ int enqueue_eval(xrdvi* h, const float* var, float* f_dbg, long long n_dbg, bool
     // forward_only leaves stale partials in part8: the gradient output of this launch is not used then
     update_draw_kernel<<<dim3(d.K + 1, d.PR), kUpdThreads, 0, h->stream>>>(d, var, 0);
     CU(cudaGetLastError());
-    return XRDVI_OK;
+    return enqueue_finish(h);
 }
 
 int write_ctl(xrdvi* h, uint64_t seed, long long step, long long trace_base, long long it_override) {
@@ -241,7 +247,6 @@ int write_ctl(xrdvi* h, uint64_t seed, long long step, long long trace_base, lon
     c.step = step;
     c.trace_base = trace_base;
     c.iteration_override = it_override;
-    c.done_total = 0;
     CU(cudaMemcpyAsync(h->dev.ctl, &c, sizeof(Ctl), cudaMemcpyHostToDevice, h->stream));
     CU(cudaStreamSynchronize(h->stream));  // c lives on this stack frame
     return XRDVI_OK;
@@ -463,12 +468,14 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
     const int n_slots = static_cast<int>(slot_phase.size());
     if (static_cast<long long>(pk_tile.size()) > pl.tile_cap + 1 || n_slots > pl.slots_cap)
         return fail(XRDVI_E_INVALID_ARG, "internal: table bound exceeded");
-    std::vector<int> slot_ofs(K + 1, 0), slot_ids(std::max(n_slots, 1));
+    // output slots numbered phase-major (the reduction over the tiles of a phase reads one contiguous range);
+    // within a phase in increasing tile order
+    std::vector<int> slot_ofs(K + 1, 0);
     for (int s = 0; s < n_slots; ++s) ++slot_ofs[slot_phase[s] + 1];
     for (int k = 0; k < K; ++k) slot_ofs[k + 1] += slot_ofs[k];
     {
         std::vector<int> fill(slot_ofs.begin(), slot_ofs.end() - 1);
-        for (int s = 0; s < n_slots; ++s) slot_ids[fill[slot_phase[s]]++] = s;   // increasing slot id per phase
+        for (int s = 0; s < n_slots; ++s) run_tab[s].w = fill[slot_phase[s]]++;
     }
     std::vector<int> seg_order(pl.n_seg);
     std::iota(seg_order.begin(), seg_order.end(), 0);
@@ -550,7 +557,6 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
     d.share_rng = reinterpret_cast<int2*>(w + pl.o_srng);
     d.seg_order = reinterpret_cast<int*>(w + pl.o_sord);
     d.slot_ofs = reinterpret_cast<int*>(w + pl.o_sofs);
-    d.slot_ids = reinterpret_cast<int*>(w + pl.o_sids);
     d.pat = reinterpret_cast<PatConst*>(w + pl.o_pat);
     d.area = reinterpret_cast<double*>(w + pl.o_area);
     d.var = reinterpret_cast<float*>(w + pl.o_var);
@@ -561,7 +567,6 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
     d.elbo_k = reinterpret_cast<double*>(w + pl.o_elbok);
     d.ll_t = reinterpret_cast<double*>(w + pl.o_llt);
     d.trace = reinterpret_cast<double*>(w + pl.o_trace);
-    d.done_inst = reinterpret_cast<unsigned int*>(w + pl.o_done);
     d.ctl = reinterpret_cast<Ctl*>(w + pl.o_ctl);
     d.lat = reinterpret_cast<float4*>(w + pl.o_lat);
     d.eps = reinterpret_cast<float4*>(w + pl.o_eps);
@@ -589,7 +594,6 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
     chk(up(pl.o_srng, share_rng.data(), sizeof(int2) * share_rng.size()));
     chk(up(pl.o_sord, seg_order.data(), sizeof(int) * seg_order.size()));
     chk(up(pl.o_sofs, slot_ofs.data(), sizeof(int) * slot_ofs.size()));
-    chk(up(pl.o_sids, slot_ids.data(), sizeof(int) * slot_ids.size()));
     chk(up(pl.o_pat, pat.data(), sizeof(PatConst) * pat.size()));
     chk(up(pl.o_area, area.data(), sizeof(double) * area.size()));
     chk(up(pl.o_mh0, m_h0.data(), sizeof(float) * m_h0.size()));
@@ -598,6 +602,7 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
     chk(cudaMemsetAsync(w + pl.o_part8, 0, sizeof(float) * static_cast<size_t>(pl.G_max) * d.n_slots * 8, st));
     chk(cudaStreamSynchronize(st));  // host staging vectors go out of scope below
     for (auto& e : h->ev) chk(cudaEventCreate(&e));
+
     if (ce != cudaSuccess) {
         delete h;
         return fail(XRDVI_E_CUDA, std::string("upload: ") + cudaGetErrorString(ce));
@@ -612,6 +617,7 @@ void xrdvi_destroy(xrdvi* h) {
     if (!h) return;
     if (h->graph_exec) cudaGraphExecDestroy(h->graph_exec);
     for (auto& e : h->ev) if (e) cudaEventDestroy(e);
+
     delete h;
 }
 
@@ -693,6 +699,8 @@ int xrdvi_fit(xrdvi* h, int32_t iterations, int32_t S, uint64_t seed, float* var
         rc = begin_steps(h, S, seed);
         if (rc) return rc;
         for (int it = 0; it < iterations; ++it) CU(cudaGraphLaunch(h->graph_exec, h->stream));
+        rc = enqueue_finish(h);
+        if (rc) return rc;
         h->step_host += iterations;
     }
     const int PR = h->plan.PR;
@@ -897,6 +905,7 @@ int xrdvi_bench_steps(xrdvi* h, int32_t steps, int32_t S, uint64_t seed, size_t 
         if (e == cudaSuccess) e = cudaEventRecord(ev[2 * i + 1], h->stream);
         if (e == cudaSuccess && flush) e = cudaMemsetAsync(flush, i & 0xFF, flush_bytes, h->stream);
     }
+    if (e == cudaSuccess) { finish_step_kernel<<<1, 256, 0, h->stream>>>(h->dev); e = cudaGetLastError(); }
     if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
     h->step_host += steps;
     for (int i = 0; i < steps && e == cudaSuccess; ++i) e = cudaEventElapsedTime(&ms_steps[i], ev[2 * i], ev[2 * i + 1]);

@@ -73,7 +73,7 @@ struct Ctl {       // device-resident control block (so that graph replays need 
     long long step;        // completed optimisation steps
     long long trace_base;  // step index of trace row 0
     long long iteration_override;  // >= 0: Philox iteration for elbo_grad/debug; < 0: use step + 1
-    unsigned int done_total;       // instances whose last CTA has finished (update_draw_kernel)
+    unsigned int pending;          // update_draw_kernel has run and finish_step has not: 1 evaluation, 2 step
     unsigned int ticket;           // next work item of elbo_split_kernel (re-armed by the launch's last CTA)
     unsigned int finished;         // CTAs of the current elbo_split_kernel launch that are done
     unsigned int pad;
@@ -96,12 +96,11 @@ struct Dev {
     const float* yb;          // [P][N]  y - B
     const float* bg;          // [P][N]
     const PeakRec* pk_tile;   // per-tile phase-major peak lists, concatenated (+1 padding record)
-    const int4* run_tab;      // [n_slots + 1] phase runs of the tile lists: (m0, m1) range in pk_tile, .z = phase;
-                              //               the run index is also the output slot in part8
+    const int4* run_tab;      // [n_slots + 1] phase runs of the tile lists: (m0, m1) range in pk_tile, .z = phase,
+                              //               .w = output slot in part8 (slots are numbered phase-major)
     const int2* share_rng;    // [n_tile][PS]: range of runs of the share
     const int* seg_order;     // [n_seg] segments (TW tiles) by decreasing work (LPT dispatch order)
-    const int* slot_ofs;      // [K+1] CSR: slots of phase k
-    const int* slot_ids;      // [n_slots]
+    const int* slot_ofs;      // [K+1] output slots of phase k: [slot_ofs[k], slot_ofs[k+1]), tiles in increasing order
     const PatConst* pat;      // [P]
     const double* area;       // [K] A_k = sum_m I_m
     // state
@@ -113,7 +112,6 @@ struct Dev {
     double* elbo_k;           // [PR][K+1]  per-phase ELBO terms; [K] = mean log-likelihood
     double* ll_t;             // [PR][S_pad]
     double* trace;            // [kTraceCap][PR]
-    unsigned int* done_inst;  // [PR] CTAs of the instance that have finished
     Ctl* ctl;
     // per-iteration buffers
     float4* lat;              // [G][K][32]  (2/w, -mu*2/w, h(1-r)aG/w, h r aL/w)
@@ -416,6 +414,32 @@ __device__ __forceinline__ PeakGeo edge_geo(int dj, int ngc, int n_c, int plim) 
     return g;
 }
 
+// a-7 (last part), as a device function: ELBO of every instance = mean log-likelihood + sum over the phases of (mean
+// log prior + log Jacobian + entropy), summed in phase order; trace row and step counter of an optimisation step.
+// Called by ALL threads of ONE CTA; does nothing unless an update_draw_kernel has run since the last call
+// (ctl->pending).  The tile kernel of the next step calls it (its last CTA in launch order): neither the tile
+// kernel nor this function needs the other's results, and the next update_draw_kernel starts after both.
+__device__ __forceinline__ void finish_step(const Dev& d) {
+    const unsigned int pending = d.ctl->pending;           // 0 nothing, 1 evaluation only, 2 optimisation step
+    if (pending == 0u) return;                             // uniform over the CTA
+    const long long step = d.ctl->step;
+    for (int inst = threadIdx.x; inst < d.PR; inst += blockDim.x) {
+        const double* __restrict__ ek = d.elbo_k + static_cast<size_t>(inst) * (d.K + 1);
+        double el = ek[d.K];
+        for (int kk = 0; kk < d.K; ++kk) el += ek[kk];
+        d.elbo[inst] = el;
+        if (pending == 2u) {
+            const long long row = step - d.ctl->trace_base;
+            if (row >= 0) d.trace[static_cast<size_t>(row % kTraceCap) * d.PR + inst] = el;
+        }
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        if (pending == 2u) d.ctl->step = step + 1;
+        d.ctl->pending = 0u;
+    }
+}
+
 // ------------------------------------------------------------------------------------------------
 // a-3 .. a-6 (likelihood part): profile + residual + backward of one 16-point tile for one group of 32 draws.
 // A warp owns one tile and one share of the tile's phase runs, in BOTH phases.  A run = the peaks of one phase
@@ -610,13 +634,13 @@ __device__ __forceinline__ void tile_phase2(const Dev& d, const TileCtx& c, int2
         v[2] = -(cL * (2.0f * B5 - B1) + cG * (B2 - (2.0f * kLn2) * B6));
         v[3] = (1.0f - rmix) * cL * B1 - rmix * cG * B2;
         if (d.pd) {   // gradient service: keep the draws apart
-            float* __restrict__ o = d.pd + (static_cast<size_t>(pd_row) * d.n_slots + r) * 128 + lane;
+            float* __restrict__ o = d.pd + (static_cast<size_t>(pd_row) * d.n_slots + run.w) * 128 + lane;
             o[0] = v[0]; o[32] = v[1]; o[64] = v[2]; o[96] = v[3];
             continue;
         }
         v[4] = v[0] * ep.x; v[5] = v[1] * ep.y; v[6] = v[2] * ep.z; v[7] = v[3] * ep.w;
         const float tot = warp_reduce8(v);
-        if (lane < 8) part[static_cast<size_t>(r) * 8 + lane] = tot;
+        if (lane < 8) part[static_cast<size_t>(run.w) * 8 + lane] = tot;
     }
 }
 
@@ -632,6 +656,7 @@ elbo_tile_kernel(const Dev d, float* __restrict__ f_dbg, long long n_dbg) {
     __shared__ float4 e_s[TW][kPT / 4][32];
     __shared__ float ss_s[TW][32];
     __shared__ float acc_s[PS > 1 ? (PS - 1) * TW * kPT : 1][32];
+    if (blockIdx.x == gridDim.x - 1 && blockIdx.y == gridDim.y - 1) finish_step(d);   // previous step's ELBO / count
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const int tw = w % TW, ps = w / TW;
     const int seg = d.seg_order[blockIdx.x];
@@ -701,6 +726,7 @@ elbo_tile_kernel(const Dev d, float* __restrict__ f_dbg, long long n_dbg) {
 template <int PS, bool BWD>
 __global__ void __launch_bounds__(32, XRDVI_TILE_WARPS_PER_SM) elbo_split_kernel(const Dev d, float* __restrict__ f_dbg, long long n_dbg) {
     const int lane = threadIdx.x;
+    if (blockIdx.x == gridDim.x - 1) finish_step(d);       // previous step's ELBO / count
     const unsigned n_items = static_cast<unsigned>(d.n_tile) * PS * d.G;
     unsigned ticket = 0;
     if (lane == 0) ticket = atomicAdd(&d.ctl->ticket, 1u);
@@ -801,14 +827,12 @@ __device__ __forceinline__ void block_reduce(double (&v)[NV], double* smem /* [N
 //                       draws of instance blockIdx.y -> grad; Adam ascent on the 8 parameters of (inst, k);
 //                       draws + transform of the next step for (inst, k, all s)          (do_update)
 //  blockIdx.x = K     : log-likelihood per draw (sum of llpart over the segments) and its mean
-//  The last CTA of an instance to finish (atomic ticket; the SUM itself has a fixed order) assembles the
-//  ELBO; the last instance bumps the step counter.
+//  The ELBO is assembled, and the step counted, by finish_step (next tile kernel, or finish_step_kernel).
 __global__ void __launch_bounds__(kUpdThreads) update_draw_kernel(const Dev d, const float* __restrict__ var_in,
                                                                   int do_update) {
     __shared__ double red[(kUpdThreads / 32) * 9];
     __shared__ float new_ml[8];
     __shared__ double tot_s[8];
-    __shared__ unsigned int ticket_s;
     const int k = blockIdx.x, inst = blockIdx.y;
     const int pat = inst / d.R;
     const PatConst pc = d.pat[pat];
@@ -847,7 +871,7 @@ __global__ void __launch_bounds__(kUpdThreads) update_draw_kernel(const Dev d, c
         const int s0 = d.slot_ofs[k], s1 = d.slot_ofs[k + 1];
         const int n_sl = s1 - s0;
         for (int idx = threadIdx.x; idx < n_sl * d.gpi; idx += kUpdThreads) {
-            const int gi = idx / n_sl, sl = d.slot_ids[s0 + (idx - gi * n_sl)];
+            const int gi = idx / n_sl, sl = s0 + (idx - gi * n_sl);
             const float4* __restrict__ pp = reinterpret_cast<const float4*>(
                 d.part8 + (static_cast<size_t>(inst * d.gpi + gi) * d.n_slots + sl) * 8);
             const float4 a = pp[0], b = pp[1];
@@ -922,30 +946,15 @@ __global__ void __launch_bounds__(kUpdThreads) update_draw_kernel(const Dev d, c
         }
     }
 
-    // ---- ELBO assembly by the last CTA of the instance (fixed summation order) ----
-    __threadfence();
-    __syncthreads();
-    if (threadIdx.x == 0) ticket_s = atomicAdd(&d.done_inst[inst], 1u);
-    __syncthreads();
-    if (ticket_s != static_cast<unsigned>(d.K)) return;
-    if (threadIdx.x != 0) return;
-    __threadfence();
-    d.done_inst[inst] = 0u;
-    const volatile double* ek = d.elbo_k + static_cast<size_t>(inst) * (d.K + 1);
-    double el = ek[d.K];
-    for (int kk = 0; kk < d.K; ++kk) el += ek[kk];
-    d.elbo[inst] = el;
-    if (do_update) {
-        const long long row = step - d.ctl->trace_base;
-        if (row >= 0) d.trace[static_cast<size_t>(row % kTraceCap) * d.PR + inst] = el;
-    }
-    __threadfence();
-    const unsigned int t2 = atomicAdd(&d.ctl->done_total, 1u);
-    if (t2 == static_cast<unsigned>(d.PR - 1)) {
-        d.ctl->done_total = 0u;
-        if (do_update) d.ctl->step = step + 1;
-    }
+    // The ELBO of the step is assembled from elbo_k by finish_step, which also counts the step: the NEXT step's
+    // tile kernel runs it, so this kernel ends without fences, tickets or a serial tail.
+    if (k == d.K && inst == 0 && threadIdx.x == 0) d.ctl->pending = do_update ? 2u : 1u;
 }
+
+// a-7 (last part): ELBO of every instance = mean log-likelihood + sum over the phases of (mean log prior + log
+// Jacobian + entropy), summed in phase order; trace row and step counter of an optimisation step.
+// grid 1, block 256: finish_step after the last step of a run and after single evaluations.
+__global__ void __launch_bounds__(256) finish_step_kernel(const Dev d) { finish_step(d); }
 
 // a-10: inclusion probability and area ratio (R15), fp64.  grid PR, block 128.
 __global__ void __launch_bounds__(128) inclusion_kernel(const Dev d, double tau, double* __restrict__ incl,
@@ -993,7 +1002,6 @@ __global__ void __launch_bounds__(128) init_state_kernel(const Dev d, const floa
         d.mom1[static_cast<size_t>(inst) * per + j] = 0.0f;
         d.mom2[static_cast<size_t>(inst) * per + j] = 0.0f;
     }
-    if (threadIdx.x == 0) d.done_inst[inst] = 0u;
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -1024,7 +1032,7 @@ __global__ void __launch_bounds__(32) logjoint_grad_kernel(const Dev d, const fl
     const PatConst pc = d.pat[pat];
     double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
     for (int j = d.slot_ofs[k]; j < d.slot_ofs[k + 1]; ++j) {
-        const float* __restrict__ o = d.pd + (static_cast<size_t>(gi) * d.n_slots + d.slot_ids[j]) * 128 + lane;
+        const float* __restrict__ o = d.pd + (static_cast<size_t>(gi) * d.n_slots + j) * 128 + lane;
         a0 += static_cast<double>(o[0]); a1 += static_cast<double>(o[32]);
         a2 += static_cast<double>(o[64]); a3 += static_cast<double>(o[96]);
     }
