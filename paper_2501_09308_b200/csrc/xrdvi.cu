@@ -158,7 +158,8 @@ struct xrdvi {
     float m_w0 = 0.f;
     long long step_host = 0;   // mirror of ctl.step
     // CUDA Graph of one optimisation step, keyed by S
-    cudaGraphExec_t graph_exec = nullptr;
+    cudaGraphExec_t graph_exec = nullptr;    // one step
+    cudaGraphExec_t graph_execU = nullptr;   // kUnroll steps: programmatic launches also across step boundaries
     int graph_S = -1;
     cudaEvent_t ev[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
 
@@ -175,6 +176,23 @@ void set_S(xrdvi* h, int S) {
 // Few tile-warps (PS > 1) and long work items: one-warp CTAs on a ticket queue (elbo_split_kernel) instead of PS-warp
 // CTAs with a barrier.  Measured on B200: config 4 (4300 peaks per item) 22.4 vs 23.5 ms per step, config 1 (39 peaks
 // per item) 0.1967 vs 0.1933 ms: the partial profiles through L2 only pay off for long items.
+// Launch with the programmatic-stream-serialization attribute (the kernel may begin while its predecessor drains; it
+// calls griddep_wait() before touching the predecessor's data).  pdl = false: a plain launch.
+template <typename... KArgs, typename... Args>
+void launch_k(void (*kernel)(KArgs...), dim3 grid, dim3 block, cudaStream_t st, bool pdl, Args... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = pdl ? 1 : 0;
+    cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
+}
+
 bool use_split(const Dev& d) {
     if (std::getenv("XRDVI_FUSED")) return false;            // A/B knobs for measurements
     if (std::getenv("XRDVI_SPLIT")) return d.TW == 1 && d.PS > 1;
@@ -182,22 +200,22 @@ bool use_split(const Dev& d) {
 }
 
 template <bool BWD>
-void launch_tile(const Dev& d, cudaStream_t st, float* f_dbg, long long n_dbg) {
+void launch_tile(const Dev& d, cudaStream_t st, float* f_dbg, long long n_dbg, bool pdl = false) {
     if (BWD && use_split(d)) {   // forward-only launches (debug, timing) always take the fused kernel
         const unsigned items = static_cast<unsigned>(d.n_tile) * d.PS * d.G;
         const unsigned grid = BWD ? 2 * items : items + static_cast<unsigned>(d.n_tile) * d.G;
         switch (d.PS) {
-            case 2: elbo_split_kernel<2, BWD><<<grid, 32, 0, st>>>(d, f_dbg, n_dbg); break;
-            case 4: elbo_split_kernel<4, BWD><<<grid, 32, 0, st>>>(d, f_dbg, n_dbg); break;
-            case 8: elbo_split_kernel<8, BWD><<<grid, 32, 0, st>>>(d, f_dbg, n_dbg); break;
+            case 2: launch_k(elbo_split_kernel<2, BWD>, dim3(grid), dim3(32), st, pdl, d, f_dbg, n_dbg); break;
+            case 4: launch_k(elbo_split_kernel<4, BWD>, dim3(grid), dim3(32), st, pdl, d, f_dbg, n_dbg); break;
+            case 8: launch_k(elbo_split_kernel<8, BWD>, dim3(grid), dim3(32), st, pdl, d, f_dbg, n_dbg); break;
             default: break;
         }
         return;
     }
     const dim3 grid(d.n_seg, d.G);
-#define XRDVI_TILE_CASE(TW_, PS_)                                                                           \
-    case TW_ * 16 + PS_:                                                                                   \
-        elbo_tile_kernel<TW_, PS_, BWD><<<grid, 32 * TW_ * PS_, 0, st>>>(d, f_dbg, n_dbg);                 \
+#define XRDVI_TILE_CASE(TW_, PS_)                                                                                \
+    case TW_ * 16 + PS_:                                                                                        \
+        launch_k(elbo_tile_kernel<TW_, PS_, BWD>, grid, dim3(32 * TW_ * PS_), st, pdl, d, f_dbg, n_dbg);         \
         break;
     switch (d.TW * 16 + d.PS) {
         XRDVI_TILE_CASE(1, 1) XRDVI_TILE_CASE(1, 2) XRDVI_TILE_CASE(1, 4) XRDVI_TILE_CASE(1, 8)
@@ -216,8 +234,11 @@ void launch_draw(const Dev& d, cudaStream_t st, const float* var, uint4* raw_out
 // the draws of the next step.  The draws of the FIRST step come from launch_draw.
 int enqueue_step(xrdvi* h) {
     const Dev& d = h->dev;
-    launch_tile<true>(d, h->stream, nullptr, 0);     // also assembles the previous step's ELBO and counts it
-    update_draw_kernel<<<dim3(d.K + 1, d.PR), kUpdThreads, 0, h->stream>>>(d, d.var, 1);
+    static const bool pdl = std::getenv("XRDVI_NO_PDL") == nullptr;    // A/B knob for measurements
+    // both kernels may start while their predecessor drains (programmatic dependent launch); each waits with
+    // griddep_wait() before it touches the predecessor's data
+    launch_tile<true>(d, h->stream, nullptr, 0, pdl);                  // also finishes the previous step (ELBO, count)
+    launch_k(update_draw_kernel, dim3(d.K + 1, d.PR), dim3(kUpdThreads), h->stream, pdl, d, static_cast<const float*>(d.var), 1);
     CU(cudaGetLastError());
     return XRDVI_OK;
 }
@@ -258,20 +279,41 @@ int check_S(xrdvi* h, int32_t S) {
     return XRDVI_OK;
 }
 
-int ensure_graph(xrdvi* h, int S) {
-    if (h->graph_exec && h->graph_S == S) return XRDVI_OK;
-    if (h->graph_exec) { cudaGraphExecDestroy(h->graph_exec); h->graph_exec = nullptr; }
-    set_S(h, S);
+constexpr int kUnroll = 8;   // steps per graph of the long graph
+
+int capture_steps(xrdvi* h, int n, cudaGraphExec_t* out) {
     cudaGraph_t graph = nullptr;
     CU(cudaStreamBeginCapture(h->stream, cudaStreamCaptureModeThreadLocal));
-    int rc = enqueue_step(h);
+    int rc = XRDVI_OK;
+    for (int i = 0; i < n && rc == XRDVI_OK; ++i) rc = enqueue_step(h);
     cudaError_t e = cudaStreamEndCapture(h->stream, &graph);
     if (rc != XRDVI_OK) { if (graph) cudaGraphDestroy(graph); return rc; }
     if (e != cudaSuccess) return fail(XRDVI_E_CUDA, std::string("cudaStreamEndCapture: ") + cudaGetErrorString(e));
-    e = cudaGraphInstantiate(&h->graph_exec, graph, 0);
+    e = cudaGraphInstantiate(out, graph, 0);
     cudaGraphDestroy(graph);
     if (e != cudaSuccess) return fail(XRDVI_E_CUDA, std::string("cudaGraphInstantiate: ") + cudaGetErrorString(e));
+    return XRDVI_OK;
+}
+
+int ensure_graph(xrdvi* h, int S) {
+    if (h->graph_exec && h->graph_execU && h->graph_S == S) return XRDVI_OK;
+    if (h->graph_exec) { cudaGraphExecDestroy(h->graph_exec); h->graph_exec = nullptr; }
+    if (h->graph_execU) { cudaGraphExecDestroy(h->graph_execU); h->graph_execU = nullptr; }
+    set_S(h, S);
+    int rc = capture_steps(h, 1, &h->graph_exec);
+    if (rc == XRDVI_OK) rc = capture_steps(h, kUnroll, &h->graph_execU);
+    if (rc != XRDVI_OK) return rc;
     h->graph_S = S;
+    return XRDVI_OK;
+}
+
+// `n` optimisation steps: as many kUnroll-step graphs as fit, single-step graphs for the rest
+int launch_steps(xrdvi* h, int n) {
+    static const bool no_unroll = std::getenv("XRDVI_NO_UNROLL") != nullptr;   // A/B knob for measurements
+    int i = 0;
+    if (!no_unroll)
+        for (; i + kUnroll <= n; i += kUnroll) CU(cudaGraphLaunch(h->graph_execU, h->stream));
+    for (; i < n; ++i) CU(cudaGraphLaunch(h->graph_exec, h->stream));
     return XRDVI_OK;
 }
 
@@ -616,6 +658,7 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
 void xrdvi_destroy(xrdvi* h) {
     if (!h) return;
     if (h->graph_exec) cudaGraphExecDestroy(h->graph_exec);
+    if (h->graph_execU) cudaGraphExecDestroy(h->graph_execU);
     for (auto& e : h->ev) if (e) cudaEventDestroy(e);
 
     delete h;
@@ -698,7 +741,8 @@ int xrdvi_fit(xrdvi* h, int32_t iterations, int32_t S, uint64_t seed, float* var
     if (iterations > 0) {
         rc = begin_steps(h, S, seed);
         if (rc) return rc;
-        for (int it = 0; it < iterations; ++it) CU(cudaGraphLaunch(h->graph_exec, h->stream));
+        rc = launch_steps(h, iterations);
+        if (rc) return rc;
         rc = enqueue_finish(h);
         if (rc) return rc;
         h->step_host += iterations;

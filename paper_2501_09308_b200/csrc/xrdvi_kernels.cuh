@@ -134,6 +134,13 @@ __device__ __forceinline__ float ex2_approx(float x) {
     asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
 }
+// Programmatic dependent launch (sm_90+): a kernel launched with the programmatic-serialization attribute may start
+// before its predecessor in the stream has finished; griddep_wait() blocks until the predecessor has completed and
+// its writes are visible (a no-op for a normal launch), griddep_launch_dependents() lets the successor start
+// launching.  Everything that reads or overwrites data of the predecessor comes after griddep_wait().
+__device__ __forceinline__ void griddep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void griddep_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
 __device__ __forceinline__ float rcp_approx(float x) {
     float y;
     asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
@@ -656,15 +663,17 @@ elbo_tile_kernel(const Dev d, float* __restrict__ f_dbg, long long n_dbg) {
     __shared__ float4 e_s[TW][kPT / 4][32];
     __shared__ float ss_s[TW][32];
     __shared__ float acc_s[PS > 1 ? (PS - 1) * TW * kPT : 1][32];
-    if (blockIdx.x == gridDim.x - 1 && blockIdx.y == gridDim.y - 1) finish_step(d);   // previous step's ELBO / count
+    griddep_launch_dependents();
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const int tw = w % TW, ps = w / TW;
-    const int seg = d.seg_order[blockIdx.x];
+    const int seg = d.seg_order[blockIdx.x];                // static tables: may be read before the predecessor is done
     const int tile = seg * TW + tw;
     const bool live = tile < d.n_tile;                      // the last segment may have fewer than TW tiles
     const TileCtx c = tile_ctx(d, d.g_base + blockIdx.y, tile);
     int2 rng = make_int2(0, 0);
     if (live) rng = d.share_rng[tile * PS + ps];
+    griddep_wait();                                         // latents, control block: written by the predecessor
+    if (blockIdx.x == gridDim.x - 1 && blockIdx.y == gridDim.y - 1) finish_step(d);   // previous step's ELBO / count
 
     float acc[kPT];
 #pragma unroll
@@ -726,6 +735,8 @@ elbo_tile_kernel(const Dev d, float* __restrict__ f_dbg, long long n_dbg) {
 template <int PS, bool BWD>
 __global__ void __launch_bounds__(32, XRDVI_TILE_WARPS_PER_SM) elbo_split_kernel(const Dev d, float* __restrict__ f_dbg, long long n_dbg) {
     const int lane = threadIdx.x;
+    griddep_launch_dependents();
+    griddep_wait();
     if (blockIdx.x == gridDim.x - 1) finish_step(d);       // previous step's ELBO / count
     const unsigned n_items = static_cast<unsigned>(d.n_tile) * PS * d.G;
     unsigned ticket = 0;
@@ -836,6 +847,8 @@ __global__ void __launch_bounds__(kUpdThreads) update_draw_kernel(const Dev d, c
     const int k = blockIdx.x, inst = blockIdx.y;
     const int pat = inst / d.R;
     const PatConst pc = d.pat[pat];
+    griddep_launch_dependents();
+    griddep_wait();                               // partials and step counter: written by the tile kernel
     const long long step = d.ctl->step;           // completed steps; this is step + 1
     const unsigned long long seed = d.ctl->seed;
     const double inv_s = 1.0 / static_cast<double>(d.S);
