@@ -115,3 +115,47 @@ def test_subset_evidence_one_dimensional_closed_form():
     ref, _ = scipy.integrate.quad(f, 0, 10, epsabs=0, epsrel=1e-11, limit=400)
     got = math.exp(log_evidence(c[None, :], y, sigma_n, lam))
     assert got == pytest.approx(ref, rel=1e-8)
+
+
+def test_elbo_is_a_lower_bound_on_the_exact_log_evidence():
+    """Pins the ABSOLUTE value of the ELBO (all normalising constants, Jacobians, entropy): with the nuisances
+    (mu, w, r) frozen (variational sd e^-12) the model has only the scales h, whose evidence is exact (the full-set
+    term of the 2^K enumeration above).  ELBO_h = ELBO - [log prior + log Jacobian + entropy of the frozen
+    coordinates] must not exceed ln Z_h, and after a fit the gap (= KL(q_h || posterior)) is a few nats."""
+    wl = synth.make_workload(0)
+    o = orc.from_workload(wl)
+    st, _, _ = o.fit(o.init_state(), 500, wl.S, seed=11)
+    st = st.copy()
+    st[0, 0, 1, :, 1:] = -12.0                                   # freeze mu, w, r at their variational means
+    zeta = st[0, 0, 0]
+    hy = o.hyper
+    frozen = 0.0
+    for k in range(o.K):
+        mu, zw, zr = zeta[k, 1], zeta[k, 2], zeta[k, 3]
+        w, r = math.exp(zw), 1.0 / (1.0 + math.exp(-zr))
+        frozen += scipy.stats.norm.logpdf(mu, 0.0, hy["mu_sigma"])                                   # B.2
+        frozen += scipy.stats.gamma.logpdf(w, hy["w_shape"], scale=1.0 / hy["w_rate"]) + zw          # + log |dw/dzeta|
+        frozen += scipy.stats.uniform.logpdf(r) + math.log(r) + math.log(1.0 - r)                    # + log |dr/dzeta|
+        frozen += 3 * (-12.0 + 0.5 * math.log(2 * math.pi * math.e))                                 # entropy of the 3
+    # exact log evidence over h >= 0 with the nuisances fixed: all K phases included
+    C = unit_profiles(o, zeta)
+    resid = o.y[0] - o.B[0]
+    sig, lam = o.sigma_n(), o.lambda_h()
+    ln_c0 = -0.5 * float(resid @ resid) / sig ** 2 - o.N * math.log(sig) - 0.5 * o.N * math.log(2 * math.pi)
+    ln_z = ln_c0 + log_evidence(C, resid, sig, lam)
+
+    S = 4096
+    vals = []
+    for it in range(4):                                          # four independent draws sets: mean and its error
+        elbo, _ = o.elbo_grad(st, S, 77, 100 + it)
+        vals.append(elbo[0, 0] - frozen)
+    elbo_h, se = float(np.mean(vals)), float(np.std(vals, ddof=1) / math.sqrt(len(vals)))
+    gap = ln_z - elbo_h
+    print(f"ln Z_h = {ln_z:.3f}, ELBO_h = {elbo_h:.3f} +- {se:.3f}, gap = {gap:.3f}")
+    assert gap > -4.0 * se - 1e-6                                # a lower bound ...
+    assert gap < 8.0                                             # ... and a tight one after the fit (KL of q_h)
+    # a deliberately bad q_h (shifted by one nat in every ln h) is a much worse bound, but still a bound
+    bad = st.copy()
+    bad[0, 0, 0, :, 0] += 1.0
+    elbo_bad = o.elbo_grad(bad, S, 77, 200)[0][0, 0] - frozen
+    assert elbo_bad < elbo_h - 10.0 and elbo_bad < ln_z
