@@ -379,3 +379,30 @@ def test_split_kernel_matches_oracle_and_the_fused_kernel_bitwise(monkeypatch):
         g0.close()
     for a, b in zip(outs["fused"], outs["split"]):
         np.testing.assert_array_equal(a, b)
+
+
+def test_two_handles_interleaved_and_resumed_fit():
+    """Handles are independent (own workspace, control block, graphs); a fit split into pieces (odd lengths, so
+    both the 8-step and the 1-step graph run) equals the fit in one piece, bit for bit."""
+    wl_a, wl_b = synth.make_workload(0), synth.make_workload(1, S=64, K=10)
+    ref = {}
+    for name, wl in (("a", wl_a), ("b", wl_b)):
+        g = Xrdvi.from_workload(wl)
+        ref[name] = g.fit(37, seed=9, want_trace=True)
+        g.close()
+    ga, gb = Xrdvi.from_workload(wl_a), Xrdvi.from_workload(wl_b)
+    tr_a, tr_b = [], []
+    for n in (5, 9, 16, 7):                                         # 37 steps in four pieces, alternating handles
+        sa, ia, ta = ga.fit(n, seed=9, want_trace=True)
+        gb.elbo_grad(S=64, seed=1, iteration=3)                     # an evaluation in between must not disturb b's fit
+        sb, ib, tb = gb.fit(n, seed=9, want_trace=True)
+        ga.logjoint_grad(synth.random_state(wl_a.K, 2, 1, seed=1)[:, 0, 0])
+        tr_a.append(ta)
+        tr_b.append(tb)
+    np.testing.assert_array_equal(sa, ref["a"][0])
+    np.testing.assert_array_equal(ia, ref["a"][1])
+    np.testing.assert_array_equal(np.concatenate(tr_a), ref["a"][2])
+    np.testing.assert_array_equal(sb, ref["b"][0])
+    np.testing.assert_array_equal(ib, ref["b"][1])
+    np.testing.assert_array_equal(np.concatenate(tr_b), ref["b"][2])
+    assert ga.get_state()[1] == 37 and gb.get_state()[1] == 37
