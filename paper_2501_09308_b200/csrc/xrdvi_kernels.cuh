@@ -248,6 +248,117 @@ __global__ void __launch_bounds__(128) draw_transform_kernel(const Dev d, const 
 }
 
 // ------------------------------------------------------------------------------------------------
+// Packed FP32x2 arithmetic (Blackwell: fma/mul/add.rn.f32x2 on 64-bit register pairs).  One instruction does two
+// IEEE single-precision operations: the same FP32 rate as FFMA, HALF the issue slots -- and the path is bound by
+// issue slots (profiles/).  A quad of grid points 4Q .. 4Q+3 is held as X = (4Q, 4Q+2), Y = (4Q+1, 4Q+3), so that
+// the two shared reciprocals of a quad, r = (1/(u_a u_b), 1/(u_c u_d)), give L_X = r * u_Y and L_Y = r * u_X without
+// any swap of register halves.
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pack2(float lo, float hi) {
+    f32x2 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void unpack2(f32x2 v, float& lo, float& hi) {
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) {
+    f32x2 d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) {
+    f32x2 d;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) {
+    f32x2 d;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ f32x2 rcp2(f32x2 v) {      // two MUFU.RCP on the halves
+    float lo, hi;
+    unpack2(v, lo, hi);
+    return pack2(rcp_approx(lo), rcp_approx(hi));
+}
+__device__ __forceinline__ f32x2 ex2neg2(f32x2 v) {   // (2^-lo, 2^-hi): two MUFU.EX2
+    float lo, hi;
+    unpack2(v, lo, hi);
+    return pack2(ex2_approx(-lo), ex2_approx(-hi));
+}
+
+// Per-(peak, tile) constants of the packed bodies: t' of the quad's X and Y points advance by 4 step per quad.
+struct Quad2 {
+    f32x2 tX, tY;     // t' at (0, 2) and (1, 3) of the current quad
+    f32x2 step4;      // (4 step, 4 step)
+};
+__device__ __forceinline__ Quad2 quad2_begin(float t0, float step) {
+    Quad2 q;
+    q.tX = pack2(t0, fmaf(2.0f, step, t0));
+    q.tY = pack2(t0 + step, fmaf(3.0f, step, t0));
+    const float s4 = 4.0f * step;
+    q.step4 = pack2(s4, s4);
+    return q;
+}
+
+// Phase 1, full tile: acc2[2Q] (X points) and acc2[2Q+1] (Y points) += I [c_L L (+ c_G G)].
+template <bool CORE>
+__device__ __forceinline__ void fwd_tile2(float t0, float step, float cg2, float cl, f32x2 (&acc2)[kPT / 2]) {
+    Quad2 q = quad2_begin(t0, step);
+    const f32x2 one2 = pack2(1.0f, 1.0f), cl2 = pack2(cl, cl), cg22 = pack2(cg2, cg2);
+#pragma unroll
+    for (int Q = 0; Q < kPT / 4; ++Q) {
+        const f32x2 uX = fma2(q.tX, q.tX, one2), uY = fma2(q.tY, q.tY, one2);
+        const f32x2 rc = mul2(rcp2(mul2(uX, uY)), cl2);
+        acc2[2 * Q] = fma2(rc, uY, acc2[2 * Q]);
+        acc2[2 * Q + 1] = fma2(rc, uX, acc2[2 * Q + 1]);
+        if (CORE) {
+            acc2[2 * Q] = fma2(cg22, ex2neg2(uX), acc2[2 * Q]);
+            acc2[2 * Q + 1] = fma2(cg22, ex2neg2(uY), acc2[2 * Q + 1]);
+        }
+        if (Q + 1 < kPT / 4) {
+            q.tX = add2(q.tX, q.step4);
+            q.tY = add2(q.tY, q.step4);
+        }
+    }
+}
+
+// Phase 2, full tile: the six sums of bwd_pair, each as a pair of partial sums (X points, Y points).
+struct Acc6x2 { f32x2 a1, a2, a3p, a4p, a5, a6u; };
+template <bool CORE>
+__device__ __forceinline__ void bwd_tile2(float t0, float step, const f32x2 (&e2)[kPT / 2], const f32x2 (&pe2)[kPT / 2],
+                                          Acc6x2& a) {
+    Quad2 q = quad2_begin(t0, step);
+    const f32x2 one2 = pack2(1.0f, 1.0f);
+#pragma unroll
+    for (int Q = 0; Q < kPT / 4; ++Q) {
+        const f32x2 uX = fma2(q.tX, q.tX, one2), uY = fma2(q.tY, q.tY, one2);
+        const f32x2 r = rcp2(mul2(uX, uY));
+        const f32x2 LX = mul2(r, uY), LY = mul2(r, uX);
+        const f32x2 L2X = mul2(LX, LX), L2Y = mul2(LY, LY);
+        a.a1 = fma2(e2[2 * Q], LX, fma2(e2[2 * Q + 1], LY, a.a1));
+        a.a5 = fma2(e2[2 * Q], L2X, fma2(e2[2 * Q + 1], L2Y, a.a5));
+        a.a3p = fma2(pe2[2 * Q], L2X, fma2(pe2[2 * Q + 1], L2Y, a.a3p));
+        if (CORE) {
+            const f32x2 gX = ex2neg2(uX), gY = ex2neg2(uY);
+            a.a2 = fma2(e2[2 * Q], gX, fma2(e2[2 * Q + 1], gY, a.a2));
+            a.a4p = fma2(pe2[2 * Q], gX, fma2(pe2[2 * Q + 1], gY, a.a4p));
+            a.a6u = fma2(mul2(e2[2 * Q], uX), gX, fma2(mul2(e2[2 * Q + 1], uY), gY, a.a6u));
+        }
+        if (Q + 1 < kPT / 4) {
+            q.tX = add2(q.tX, q.step4);
+            q.tY = add2(q.tY, q.step4);
+        }
+    }
+}
+__device__ __forceinline__ float hsum2(f32x2 v) {
+    float lo, hi;
+    unpack2(v, lo, hi);
+    return lo + hi;
+}
+
+// ------------------------------------------------------------------------------------------------
 // Phase-1 building blocks (profile).  acc[p] += I_m [ c_G 2^(-t'^2) + c_L / (1 + t'^2) ].
 // Two neighbouring points share one reciprocal: 1/ua = ub * rcp(ua ub).
 // The Gaussian uses u = 1 + t'^2 as well: 2^(-t'^2) = 2 * 2^(-u), the factor 2 is folded into cg2 = 2 c_G.
@@ -272,11 +383,13 @@ struct PeakGeo { int p_lo, p_hi, c_lo, c_hi; };
 // touches the quad.  One compact body per quad (these pairs are 2 of ~10 per peak; code size matters more).
 template <int Q>
 __device__ __forceinline__ void fwd_quad_generic(const PeakGeo& g, float t0, float step, float cg2, float cl,
-                                                 float (&acc)[kPT]) {
+                                                 f32x2& accX, f32x2& accY) {
     const int lo = max(g.p_lo, 4 * Q), hi = min(g.p_hi, 4 * Q + 3);
     if (lo > hi) return;                                   // quad outside the window
     const unsigned span = static_cast<unsigned>(hi - lo);
-    float u[4], m[4];
+    float u[4], m[4], a[4];
+    unpack2(accX, a[0], a[2]);
+    unpack2(accY, a[1], a[3]);
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
         const float t = fmaf(static_cast<float>(4 * Q + i), step, t0);
@@ -284,14 +397,16 @@ __device__ __forceinline__ void fwd_quad_generic(const PeakGeo& g, float t0, flo
         m[i] = static_cast<unsigned>(4 * Q + i - lo) <= span ? 1.0f : 0.0f;
     }
     const float r01 = rcp_approx(u[0] * u[1]) * cl, r23 = rcp_approx(u[2] * u[3]) * cl;
-    acc[4 * Q] = fmaf(r01 * u[1], m[0], acc[4 * Q]);
-    acc[4 * Q + 1] = fmaf(r01 * u[0], m[1], acc[4 * Q + 1]);
-    acc[4 * Q + 2] = fmaf(r23 * u[3], m[2], acc[4 * Q + 2]);
-    acc[4 * Q + 3] = fmaf(r23 * u[2], m[3], acc[4 * Q + 3]);
+    a[0] = fmaf(r01 * u[1], m[0], a[0]);
+    a[1] = fmaf(r01 * u[0], m[1], a[1]);
+    a[2] = fmaf(r23 * u[3], m[2], a[2]);
+    a[3] = fmaf(r23 * u[2], m[3], a[3]);
     if (g.c_hi >= 4 * Q && g.c_lo <= 4 * Q + 3) {
 #pragma unroll
-        for (int i = 0; i < 4; ++i) acc[4 * Q + i] = fmaf(cg2 * m[i], ex2_approx(-u[i]), acc[4 * Q + i]);
+        for (int i = 0; i < 4; ++i) a[i] = fmaf(cg2 * m[i], ex2_approx(-u[i]), a[i]);
     }
+    accX = pack2(a[0], a[2]);
+    accY = pack2(a[1], a[3]);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -321,19 +436,23 @@ __device__ __forceinline__ void bwd_pair(float ea, float eb, float pea, float pe
 }
 
 template <int Q>
-__device__ __forceinline__ void bwd_quad_generic(const PeakGeo& g, float t0, float step, const float (&e)[kPT],
-                                                 const float (&pe)[kPT], Acc6& a) {
+__device__ __forceinline__ void bwd_quad_generic(const PeakGeo& g, float t0, float step, f32x2 eX, f32x2 eY, f32x2 peX,
+                                                 f32x2 peY, Acc6& a) {
     const int lo = max(g.p_lo, 4 * Q), hi = min(g.p_hi, 4 * Q + 3);
     if (lo > hi) return;
     const unsigned span = static_cast<unsigned>(hi - lo);
     float u[4], ev[4], qv[4];
+    unpack2(eX, ev[0], ev[2]);
+    unpack2(eY, ev[1], ev[3]);
+    unpack2(peX, qv[0], qv[2]);
+    unpack2(peY, qv[1], qv[3]);
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
         const float t = fmaf(static_cast<float>(4 * Q + i), step, t0);
         u[i] = fmaf(t, t, 1.0f);
         const bool in = static_cast<unsigned>(4 * Q + i - lo) <= span;   // out-of-window points: zero residual
-        ev[i] = in ? e[4 * Q + i] : 0.0f;
-        qv[i] = in ? pe[4 * Q + i] : 0.0f;
+        ev[i] = in ? ev[i] : 0.0f;
+        qv[i] = in ? qv[i] : 0.0f;
     }
     const float r01 = rcp_approx(u[0] * u[1]), r23 = rcp_approx(u[2] * u[3]);
     const float L[4] = {r01 * u[1], r01 * u[0], r23 * u[3], r23 * u[2]};
@@ -392,6 +511,7 @@ __device__ __forceinline__ float warp_reduce8(float (&v)[8]) {
     const int src = ((lane & 4) ? 16 : 0) | ((lane & 2) ? 8 : 0) | ((lane & 1) ? 4 : 0);
     return __shfl_sync(0xffffffffu, w1, src);
 }
+
 
 // Poisson likelihood of one grid point (A12-A16; R24): y = (y - B) + B, f = S_F + B (A3);
 // returns (d ll / d f, the point's term of ll minus its f-independent part):
@@ -471,51 +591,54 @@ __device__ __forceinline__ TileCtx tile_ctx(const Dev& d, int g, int tile) {
     return c;
 }
 
-// Phase 1: acc[p] += profile of the runs [rng.x, rng.y) on the 16 points of the tile.
+// Phase 1: acc[p] = profile of the runs [rng.x, rng.y) on the 16 points of the tile (acc is overwritten).  The
+// accumulators live as packed pairs (quad Q: acc2[2Q] = points (4Q, 4Q+2), acc2[2Q+1] = points (4Q+1, 4Q+3)).
 __device__ __forceinline__ void tile_phase1(const Dev& d, const TileCtx& c, int2 rng, float (&acc)[kPT]) {
-    if (rng.x >= rng.y) return;
-    const PeakRec* __restrict__ pkt = d.pk_tile;
-    const int4* __restrict__ runs = d.run_tab;
-    int4 run_n = runs[rng.x];
-    float4 lt_n = c.lat[static_cast<size_t>(run_n.z) * 32];
-    int ng_n = c.ngk[run_n.z];
-    for (int r = rng.x; r < rng.y; ++r) {
-        const int4 run = run_n;
-        const float4 lt = lt_n;
-        const int ngc = ng_n;
-        run_n = runs[r + 1];                            // run_tab carries one padding entry
-        lt_n = c.lat[static_cast<size_t>(run_n.z) * 32];
-        ng_n = c.ngk[run_n.z];
-        const float step = d.delta * lt.x;
-        const unsigned core_span = static_cast<unsigned>(kPT - 1 + 2 * ngc);
+    f32x2 acc2[kPT / 2];
+#pragma unroll
+    for (int i = 0; i < kPT / 2; ++i) acc2[i] = 0ull;
+    if (rng.x < rng.y) {
+        const PeakRec* __restrict__ pkt = d.pk_tile;
+        const int4* __restrict__ runs = d.run_tab;
+        int4 run_n = runs[rng.x];
+        float4 lt_n = c.lat[static_cast<size_t>(run_n.z) * 32];
+        int ng_n = c.ngk[run_n.z];
+        for (int r = rng.x; r < rng.y; ++r) {
+            const int4 run = run_n;
+            const float4 lt = lt_n;
+            const int ngc = ng_n;
+            run_n = runs[r + 1];                            // run_tab carries one padding entry
+            lt_n = c.lat[static_cast<size_t>(run_n.z) * 32];
+            ng_n = c.ngk[run_n.z];
+            const float step = d.delta * lt.x;
+            const unsigned core_span = static_cast<unsigned>(kPT - 1 + 2 * ngc);
 #pragma unroll 1
-        for (int m = run.x; m < run.y; ++m) {
-            const PeakRec pk = pkt[m];
-            const float t0 = fmaf(static_cast<float>(-pk.dj), step, fmaf(-pk.delta, lt.x, lt.y));
-            const float cl = pk.inten * lt.w;
-            const bool core = static_cast<unsigned>(pk.dj + ngc) <= core_span;   // Gaussian core touches the tile
-            if (pk.full) {   // branch-free bodies: Lorentz tail only, or tail + Gaussian on all 16 points
-                if (!core) {
-#pragma unroll
-                    for (int p = 0; p < kPT; p += 2)
-                        fwd_pair<false>(fmaf(static_cast<float>(p), step, t0), fmaf(static_cast<float>(p + 1), step, t0),
-                                        0.0f, cl, acc[p], acc[p + 1]);
-                } else {
+            for (int m = run.x; m < run.y; ++m) {
+                const PeakRec pk = pkt[m];
+                const float t0 = fmaf(static_cast<float>(-pk.dj), step, fmaf(-pk.delta, lt.x, lt.y));
+                const float cl = pk.inten * lt.w;
+                const bool core = static_cast<unsigned>(pk.dj + ngc) <= core_span;   // Gaussian core touches the tile
+                if (pk.full) {   // branch-free bodies: Lorentz tail only, or tail + Gaussian on all 16 points
+                    if (!core) {
+                        fwd_tile2<false>(t0, step, 0.0f, cl, acc2);
+                    } else {
+                        fwd_tile2<true>(t0, step, 2.0f * pk.inten * lt.z, cl, acc2);
+                    }
+                } else {         // window edge: quad by quad
+                    const PeakGeo geo = edge_geo(pk.dj, ngc, d.n_c, c.plim);
                     const float cg2 = 2.0f * pk.inten * lt.z;
-#pragma unroll
-                    for (int p = 0; p < kPT; p += 2)
-                        fwd_pair<true>(fmaf(static_cast<float>(p), step, t0), fmaf(static_cast<float>(p + 1), step, t0),
-                                       cg2, cl, acc[p], acc[p + 1]);
+                    fwd_quad_generic<0>(geo, t0, step, cg2, cl, acc2[0], acc2[1]);
+                    fwd_quad_generic<1>(geo, t0, step, cg2, cl, acc2[2], acc2[3]);
+                    fwd_quad_generic<2>(geo, t0, step, cg2, cl, acc2[4], acc2[5]);
+                    fwd_quad_generic<3>(geo, t0, step, cg2, cl, acc2[6], acc2[7]);
                 }
-            } else {         // window edge: quad by quad
-                const PeakGeo geo = edge_geo(pk.dj, ngc, d.n_c, c.plim);
-                const float cg2 = 2.0f * pk.inten * lt.z;
-                fwd_quad_generic<0>(geo, t0, step, cg2, cl, acc);
-                fwd_quad_generic<1>(geo, t0, step, cg2, cl, acc);
-                fwd_quad_generic<2>(geo, t0, step, cg2, cl, acc);
-                fwd_quad_generic<3>(geo, t0, step, cg2, cl, acc);
             }
         }
+    }
+#pragma unroll
+    for (int Q = 0; Q < kPT / 4; ++Q) {
+        unpack2(acc2[2 * Q], acc[4 * Q], acc[4 * Q + 2]);
+        unpack2(acc2[2 * Q + 1], acc[4 * Q + 1], acc[4 * Q + 3]);
     }
 }
 
@@ -570,9 +693,14 @@ __device__ __forceinline__ void tile_debug_profile(const Dev& d, const TileCtx& 
 __device__ __forceinline__ void tile_phase2(const Dev& d, const TileCtx& c, int2 rng, const float (&e)[kPT], int pd_row) {
     if (rng.x >= rng.y) return;
     const int lane = threadIdx.x & 31;
-    float pe[kPT];
+    f32x2 e2[kPT / 2], pe2[kPT / 2];     // packed like the accumulators of phase 1; pe_p = p e_p
 #pragma unroll
-    for (int p = 0; p < kPT; ++p) pe[p] = static_cast<float>(p) * e[p];
+    for (int Q = 0; Q < kPT / 4; ++Q) {
+        e2[2 * Q] = pack2(e[4 * Q], e[4 * Q + 2]);
+        e2[2 * Q + 1] = pack2(e[4 * Q + 1], e[4 * Q + 3]);
+        pe2[2 * Q] = pack2(static_cast<float>(4 * Q) * e[4 * Q], static_cast<float>(4 * Q + 2) * e[4 * Q + 2]);
+        pe2[2 * Q + 1] = pack2(static_cast<float>(4 * Q + 1) * e[4 * Q + 1], static_cast<float>(4 * Q + 3) * e[4 * Q + 3]);
+    }
     const PeakRec* __restrict__ pkt = d.pk_tile;
     const int4* __restrict__ runs = d.run_tab;
     const float4* __restrict__ epsg = d.eps + static_cast<size_t>(c.g) * d.K * 32 + lane;
@@ -602,27 +730,26 @@ __device__ __forceinline__ void tile_phase2(const Dev& d, const TileCtx& c, int2
             const PeakRec pk = pkt[m];
             const float t0 = fmaf(static_cast<float>(-pk.dj), step, fmaf(-pk.delta, lt.x, lt.y));
             const bool core = static_cast<unsigned>(pk.dj + ngc) <= core_span;
-            Acc6 a = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
             if (pk.full && !core) {
-#pragma unroll
-                for (int p = 0; p < kPT; p += 2)
-                    bwd_pair<false>(e[p], e[p + 1], pe[p], pe[p + 1], fmaf(static_cast<float>(p), step, t0),
-                                    fmaf(static_cast<float>(p + 1), step, t0), a);
-                B1 = fmaf(pk.inten, a.a1, B1);
-                B3 = fmaf(pk.inten, fmaf(t0, a.a5, step * a.a3p), B3);
-                B5 = fmaf(pk.inten, a.a5, B5);
+                Acc6x2 a2 = {0ull, 0ull, 0ull, 0ull, 0ull, 0ull};
+                bwd_tile2<false>(t0, step, e2, pe2, a2);
+                const float a1 = hsum2(a2.a1), a5 = hsum2(a2.a5), a3p = hsum2(a2.a3p);
+                B1 = fmaf(pk.inten, a1, B1);
+                B3 = fmaf(pk.inten, fmaf(t0, a5, step * a3p), B3);
+                B5 = fmaf(pk.inten, a5, B5);
             } else {
+                Acc6 a = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
                 if (pk.full) {
-#pragma unroll
-                    for (int p = 0; p < kPT; p += 2)
-                        bwd_pair<true>(e[p], e[p + 1], pe[p], pe[p + 1], fmaf(static_cast<float>(p), step, t0),
-                                       fmaf(static_cast<float>(p + 1), step, t0), a);
+                    Acc6x2 a2 = {0ull, 0ull, 0ull, 0ull, 0ull, 0ull};
+                    bwd_tile2<true>(t0, step, e2, pe2, a2);
+                    a.a1 = hsum2(a2.a1); a.a2 = hsum2(a2.a2); a.a3p = hsum2(a2.a3p);
+                    a.a4p = hsum2(a2.a4p); a.a5 = hsum2(a2.a5); a.a6u = hsum2(a2.a6u);
                 } else {
                     const PeakGeo geo = edge_geo(pk.dj, ngc, d.n_c, c.plim);
-                    bwd_quad_generic<0>(geo, t0, step, e, pe, a);
-                    bwd_quad_generic<1>(geo, t0, step, e, pe, a);
-                    bwd_quad_generic<2>(geo, t0, step, e, pe, a);
-                    bwd_quad_generic<3>(geo, t0, step, e, pe, a);
+                    bwd_quad_generic<0>(geo, t0, step, e2[0], e2[1], pe2[0], pe2[1], a);
+                    bwd_quad_generic<1>(geo, t0, step, e2[2], e2[3], pe2[2], pe2[3], a);
+                    bwd_quad_generic<2>(geo, t0, step, e2[4], e2[5], pe2[4], pe2[5], a);
+                    bwd_quad_generic<3>(geo, t0, step, e2[6], e2[7], pe2[6], pe2[7], a);
                 }
                 const float i2 = 2.0f * pk.inten;           // g = G/2 in the Gaussian sums
                 B1 = fmaf(pk.inten, a.a1, B1);
