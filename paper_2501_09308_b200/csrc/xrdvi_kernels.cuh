@@ -784,8 +784,20 @@ __device__ __forceinline__ void tile_phase2(const Dev& d, const TileCtx& c, int2
 #ifndef XRDVI_TILE_WARPS_PER_SM
 #define XRDVI_TILE_WARPS_PER_SM 24          // register budget: 65536 / (32 * 24) = 85 -> 80 registers per thread
 #endif
+#ifndef XRDVI_TILE_WARPS_PER_SM_SHARED
+#define XRDVI_TILE_WARPS_PER_SM_SHARED 20   // CTAs with several warps (few-group launches): 96 registers, no spills
+#endif
+// Resident CTAs per SM the register budget is set for.  Launches with millions of one-warp CTAs (PS = 1) are
+// throughput-bound and want 24 warps per SM; the few-group launches (config 1: 2008 CTAs of 4 warps) are bound by the
+// latency of each warp's own instruction stream, where 96 registers without spills beat 80 with (measured 0.169 vs
+// 0.180 ms, profiles/).
+constexpr int tile_ctas_per_sm(int TW, int PS) {
+    const int warps = TW * PS;
+    const int budget = warps > 1 ? XRDVI_TILE_WARPS_PER_SM_SHARED : XRDVI_TILE_WARPS_PER_SM;
+    return budget / warps > 0 ? budget / warps : 1;
+}
 template <int TW, int PS, bool BWD>
-__global__ void __launch_bounds__(32 * TW * PS, XRDVI_TILE_WARPS_PER_SM / (TW * PS) > 0 ? XRDVI_TILE_WARPS_PER_SM / (TW * PS) : 1)
+__global__ void __launch_bounds__(32 * TW * PS, tile_ctas_per_sm(TW, PS))
 elbo_tile_kernel(const Dev d, float* __restrict__ f_dbg, long long n_dbg) {
     __shared__ float4 e_s[TW][kPT / 4][32];
     __shared__ float ss_s[TW][32];
