@@ -172,6 +172,16 @@ int xrdvi_debug_draws(xrdvi* h, int32_t S, uint64_t seed, uint64_t iteration, in
  * residual), [2] update_draw_kernel without the update, [3] draw + tile + update together.          */
 int xrdvi_time_kernels(xrdvi* h, int32_t S, uint64_t seed, int32_t reps, float* ms);
 
+/* Measurement: per-warp timeline of ONE launch of the fused profile / residual / backward kernel (a-3 .. a-7) at the
+ * internal state with S draws per instance, after two un-stamped warm-up launches.  Every warp (or, where the
+ * ticket-queue variant of the kernel is selected, every one-warp work item) writes four uint64 words:
+ *   [0] %globaltimer (ns) when it starts, [1] at the end of the profile phase, [2] when it is done,
+ *   [3] SM id (low 32 bits) | number of (peak, tile) records of its share (high 32 bits).
+ * rows uint64 [capacity][4] (host), *n_rows = rows written; XRDVI_E_INVALID_ARG if capacity is smaller than the
+ * number of warps of the launch.  The state is not modified (the per-step draw buffers are overwritten).  This is
+ * how profiles/ shows which part of a launch is full-occupancy work and which part is the drain of its last wave. */
+int xrdvi_debug_timeline(xrdvi* h, int32_t S, uint64_t seed, int64_t capacity, uint64_t* rows, int64_t* n_rows);
+
 /* Measurement: `steps` optimisation steps (graph replays, exactly as xrdvi_fit runs them), each one
  * bracketed by its own pair of CUDA events on the handle's stream; between two steps, outside the
  * brackets, `l2_flush_bytes` of device memory are overwritten (0 = no flush) so that every step starts

@@ -18,7 +18,7 @@ EXPORTS = (
     "xrdvi_default_hyper", "xrdvi_workspace_bytes", "xrdvi_create", "xrdvi_destroy", "xrdvi_pair_count",
     "xrdvi_window_halfwidth", "xrdvi_reset_state", "xrdvi_get_state", "xrdvi_set_state", "xrdvi_elbo_grad",
     "xrdvi_fit", "xrdvi_inclusion", "xrdvi_logjoint_grad", "xrdvi_debug_profile", "xrdvi_debug_draws", "xrdvi_time_kernels",
-    "xrdvi_bench_steps", "xrdvi_pipe_rates", "xrdvi_last_error",
+    "xrdvi_bench_steps", "xrdvi_debug_timeline", "xrdvi_pipe_rates", "xrdvi_last_error",
 )
 
 
@@ -77,6 +77,7 @@ def load_library():
                                     C.POINTER(C.c_int32)]
     L.xrdvi_time_kernels.argtypes = [vp, C.c_int32, C.c_uint64, C.c_int32, fp]
     L.xrdvi_bench_steps.argtypes = [vp, C.c_int32, C.c_int32, C.c_uint64, C.c_size_t, fp]
+    L.xrdvi_debug_timeline.argtypes = [vp, C.c_int32, C.c_uint64, C.c_int64, C.POINTER(C.c_uint64), C.POINTER(C.c_int64)]
     L.xrdvi_pipe_rates.argtypes = [C.c_int, fp]
     L.xrdvi_last_error.restype = C.c_char_p
     _lib = L
@@ -251,6 +252,15 @@ class Xrdvi:
         _check(load_library().xrdvi_time_kernels(self._h, S, int(seed), int(reps), _f(ms)))
         return dict(ms_tile=float(ms[0]), ms_tile_forward_only=float(ms[1]), ms_update=float(ms[2]),
                     ms_iteration=float(ms[3]))
+
+    def debug_timeline(self, S=None, seed=0, capacity=1 << 22):
+        """Per-warp (start, end of phase 1, end, SM id | records << 32) of one tile-kernel launch (xrdvi_debug_timeline)."""
+        S = self.S_max if S is None else int(S)
+        rows = np.zeros((int(capacity), 4), dtype=np.uint64)
+        n = C.c_int64(0)
+        _check(load_library().xrdvi_debug_timeline(self._h, S, int(seed), int(capacity),
+                                                   rows.ctypes.data_as(C.POINTER(C.c_uint64)), C.byref(n)))
+        return rows[: n.value]
 
     def bench_steps(self, steps, S=None, seed=0, l2_flush_bytes=0):
         S = self.S_max if S is None else int(S)

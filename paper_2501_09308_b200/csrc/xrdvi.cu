@@ -931,6 +931,37 @@ int xrdvi_time_kernels(xrdvi* h, int32_t S, uint64_t seed, int32_t reps, float* 
     return XRDVI_OK;
 }
 
+int xrdvi_debug_timeline(xrdvi* h, int32_t S, uint64_t seed, int64_t capacity, uint64_t* rows, int64_t* n_rows) {
+    int rc = check_S(h, S);
+    if (rc) return rc;
+    if (!rows || !n_rows || capacity < 1) return fail(XRDVI_E_INVALID_ARG, "rows / n_rows NULL or capacity < 1");
+    CU(cudaSetDevice(h->device));
+    set_S(h, S);
+    rc = write_ctl(h, seed, h->step_host, h->step_host, -1);
+    if (rc) return rc;
+    Dev d = h->dev;                                       // a copy with the stamp buffer attached
+    const long long warps = use_split(d) ? 2ll * d.n_tile * d.PS * d.G : static_cast<long long>(d.n_seg) * d.G * d.TW * d.PS;
+    if (warps > capacity) return fail(XRDVI_E_INVALID_ARG, "capacity < warps of the launch");
+    unsigned long long* buf = nullptr;
+    CU(cudaMalloc(&buf, sizeof(unsigned long long) * 4 * warps));   // measurement path only
+    cudaStream_t st = h->stream;
+    cudaError_t e = cudaSuccess;
+    for (int pass = 0; pass < 3 && e == cudaSuccess; ++pass) {       // two warm-up passes, the third is stamped
+        launch_draw(h->dev, st, h->dev.var, nullptr);
+        d.tl = pass == 2 ? buf : nullptr;
+        if (pass == 2) e = cudaMemsetAsync(buf, 0, sizeof(unsigned long long) * 4 * warps, st);
+        launch_tile<true>(d, st, nullptr, 0);
+        update_draw_kernel<<<dim3(d.K + 1, d.PR), kUpdThreads, 0, st>>>(h->dev, h->dev.var, 0);
+        if (e == cudaSuccess) e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaMemcpyAsync(rows, buf, sizeof(unsigned long long) * 4 * warps, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    cudaFree(buf);
+    if (e != cudaSuccess) return fail(XRDVI_E_CUDA, std::string("debug_timeline: ") + cudaGetErrorString(e));
+    *n_rows = warps;
+    return enqueue_finish(h) ? XRDVI_E_CUDA : XRDVI_OK;
+}
+
 int xrdvi_bench_steps(xrdvi* h, int32_t steps, int32_t S, uint64_t seed, size_t flush_bytes, float* ms_steps) {
     int rc = check_S(h, S);
     if (rc) return rc;

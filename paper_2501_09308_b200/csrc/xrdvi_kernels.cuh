@@ -126,6 +126,8 @@ struct Dev {
     unsigned int* tile_cnt2;  // [G][n_tile] phase-2 items that are done
     float* pd;                // nullptr, or [groups of the launch][n_slots][4][32] d ll / d zeta per (run, class, draw)
     int g_base;               // group of blockIdx.y = 0 in elbo_tile_kernel (0 except in the service)
+    // measurement (xrdvi_debug_timeline): nullptr, or [warps of the launch][4] = (start, end of phase 1, end, SM id | records << 32)
+    unsigned long long* tl;
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -139,6 +141,22 @@ __device__ __forceinline__ float ex2_approx(float x) {
 // its writes are visible (a no-op for a normal launch), griddep_launch_dependents() lets the successor start
 // launching.  Everything that reads or overwrites data of the predecessor comes after griddep_wait().
 __device__ __forceinline__ void griddep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+// Per-warp timeline stamps of the tile kernels (xrdvi_debug_timeline; d.tl == nullptr in every other launch, a
+// warp-uniform test on a kernel parameter).  Each stamp is stored at once, nothing stays live across the phases.
+__device__ __forceinline__ void tl_stamp(unsigned long long* tl, unsigned row, int col) {
+    if (tl && (threadIdx.x & 31) == 0) {
+        unsigned long long t;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+        tl[static_cast<size_t>(row) * 4 + col] = t;
+    }
+}
+__device__ __forceinline__ void tl_tag(unsigned long long* tl, unsigned row, int records) {
+    if (tl && (threadIdx.x & 31) == 0) {
+        unsigned sm;
+        asm volatile("mov.u32 %0, %%smid;" : "=r"(sm));
+        tl[static_cast<size_t>(row) * 4 + 3] = sm | (static_cast<unsigned long long>(records) << 32);
+    }
+}
 __device__ __forceinline__ void griddep_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 
 __device__ __forceinline__ float rcp_approx(float x) {
@@ -813,6 +831,9 @@ elbo_tile_kernel(const Dev d, float* __restrict__ f_dbg, long long n_dbg) {
     if (live) rng = d.share_rng[tile * PS + ps];
     griddep_wait();                                         // latents, control block: written by the predecessor
     if (blockIdx.x == gridDim.x - 1 && blockIdx.y == gridDim.y - 1) finish_step(d);   // previous step's ELBO / count
+    const unsigned tl_row = (blockIdx.y * gridDim.x + blockIdx.x) * (TW * PS) + w;
+    tl_stamp(d.tl, tl_row, 0);
+    if (d.tl) tl_tag(d.tl, tl_row, rng.x < rng.y ? d.run_tab[rng.y - 1].y - d.run_tab[rng.x].x : 0);
 
     float acc[kPT];
 #pragma unroll
@@ -850,8 +871,9 @@ elbo_tile_kernel(const Dev d, float* __restrict__ f_dbg, long long n_dbg) {
         for (int v = 1; v < TW; ++v) ss += ss_s[v][lane];
         d.llpart[(static_cast<size_t>(c.g) * d.n_seg + seg) * 32 + lane] = ss;
     }
+    tl_stamp(d.tl, tl_row, 1);
     if (!BWD) return;
-    if (rng.x >= rng.y) return;
+    if (rng.x >= rng.y) { tl_stamp(d.tl, tl_row, 2); return; }
     float e[kPT];
 #pragma unroll
     for (int v = 0; v < kPT / 4; ++v) {
@@ -859,6 +881,7 @@ elbo_tile_kernel(const Dev d, float* __restrict__ f_dbg, long long n_dbg) {
         e[4 * v] = t.x; e[4 * v + 1] = t.y; e[4 * v + 2] = t.z; e[4 * v + 3] = t.w;
     }
     tile_phase2(d, c, rng, e, blockIdx.y);
+    tl_stamp(d.tl, tl_row, 2);
 }
 
 // Split variant for launches with few tile-warps (PS > 1; configs 1 and 4): one warp per CTA, work items taken from a
@@ -882,6 +905,8 @@ __global__ void __launch_bounds__(32, XRDVI_TILE_WARPS_PER_SM) elbo_split_kernel
     if (lane == 0) ticket = atomicAdd(&d.ctl->ticket, 1u);
     ticket = __shfl_sync(0xffffffffu, ticket, 0);
     const bool second = ticket >= n_items;
+    tl_stamp(d.tl, ticket, 0);
+    if (second) tl_stamp(d.tl, ticket, 1);                 // a phase-2 item: no phase-1 part
     unsigned item = second ? ticket - n_items : ticket;
     int ps, gi, pos;
     if (second && !BWD) {            // forward only: one phase-2 item per (tile, group), played by share 0
@@ -897,6 +922,7 @@ __global__ void __launch_bounds__(32, XRDVI_TILE_WARPS_PER_SM) elbo_split_kernel
     const int tile = d.seg_order[pos];                     // TW = 1: segments are tiles
     const TileCtx c = tile_ctx(d, d.g_base + gi, tile);
     const int2 rng = d.share_rng[tile * PS + ps];
+    if (d.tl) tl_tag(d.tl, ticket, rng.x < rng.y ? d.run_tab[rng.y - 1].y - d.run_tab[rng.x].x : 0);
     const size_t tg = static_cast<size_t>(gi) * d.n_tile + tile;
     float* __restrict__ partial = d.partial + tg * (PS * kPT * 32) + lane;
 
@@ -910,6 +936,7 @@ __global__ void __launch_bounds__(32, XRDVI_TILE_WARPS_PER_SM) elbo_split_kernel
         __threadfence();
         __syncwarp();
         if (lane == 0) atomicAdd(&d.tile_cnt[tg], 1u);
+        tl_stamp(d.tl, ticket, 1);
     } else {
         if (lane == 0) {
             while (atomicAdd(&d.tile_cnt[tg], 0u) < static_cast<unsigned>(PS)) __nanosleep(64);
@@ -939,6 +966,7 @@ __global__ void __launch_bounds__(32, XRDVI_TILE_WARPS_PER_SM) elbo_split_kernel
             }
         }
     }
+    tl_stamp(d.tl, ticket, 2);
     if (lane == 0) {       // the last CTA of the launch re-arms the ticket counter
         __threadfence();
         if (atomicAdd(&d.ctl->finished, 1u) == gridDim.x - 1) {

@@ -406,3 +406,29 @@ def test_two_handles_interleaved_and_resumed_fit():
     np.testing.assert_array_equal(ib, ref["b"][1])
     np.testing.assert_array_equal(np.concatenate(tr_b), ref["b"][2])
     assert ga.get_state()[1] == 37 and gb.get_state()[1] == 37
+
+
+def test_debug_timeline_rows_are_consistent():
+    """xrdvi_debug_timeline: one row per warp of the launch, ordered stamps, SM ids of a B200, every record counted."""
+    from paper_2501_09308_b200 import XrdviError
+    wl = synth.make_workload(1, S=64)
+    g = Xrdvi.from_workload(wl)
+    before, _ = g.get_state()
+    rows = g.debug_timeline(seed=3)
+    after, _ = g.get_state()
+    assert np.array_equal(before, after)                       # the state is not touched
+    assert len(rows) > 0 and (rows[:, 0] > 0).all()
+    t0, t1, t2 = (rows[:, i].astype(np.int64) for i in range(3))
+    assert (t1 >= t0).all() and (t2 >= t1).all()
+    assert (t2.max() - t0.min()) < 50_000_000                  # one launch: far below 50 ms
+    sm = (rows[:, 3] & np.uint64(0xFFFFFFFF)).astype(np.int64)
+    assert sm.max() < 160 and len(np.unique(sm)) > 100
+    rec = (rows[:, 3] >> np.uint64(32)).astype(np.int64)
+    # every (peak, tile) record is owned by exactly one share per group: 2 groups here, and the records of a draw
+    # hold pair_count in-window pairs of at most 16 points each
+    groups = 2
+    assert rec.sum() % groups == 0
+    assert rec.sum() // groups * 16 >= g.pair_count
+    with pytest.raises(XrdviError):
+        g.debug_timeline(capacity=8)
+    g.close()
