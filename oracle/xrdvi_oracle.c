@@ -24,6 +24,8 @@
  *             natural-gradient ascent (R25; north_star names both)
  *   inclusion closed form from (m, l), 1 % area threshold PAPER.md:140 (R15)
  *   draws     Philox4x32-10, counter (iter, s, k, inst), key (seed_lo, seed_hi) (R18)
+ *   adaptive  per-phase window half-widths n_c,k <= n_c refreshed from the variational means
+ *             (reading R27; north_star's "problem-defined +-W FWHM cutoff")
  *
  * Pins (tests/test_oracle_pins.py): unit area and half-height of G/L/V, normal/Cauchy pdf
  * special cases, zero-inclusion, shift and dummy-peak invariances, linearity in h, direct
@@ -72,6 +74,7 @@ typedef struct {
     double *pos, *inten;   /* [M]                                            */
     int64_t *jm;           /* [M] nearest grid index (may lie outside [0,N)) */
     int64_t n_c;           /* window half width in points; <0 -> dense       */
+    int64_t *n_ck;         /* [K] per-phase half widths (R27), NULL -> n_c   */
     double delta;          /* grid step                                      */
     double *sigma_n;       /* [P]                                            */
     double *lambda_h;      /* [P]                                            */
@@ -126,7 +129,7 @@ void orc_eps(uint64_t seed, uint64_t iteration, uint32_t inst, uint32_t s, uint3
 void orc_destroy(orc_problem *q) {
     if (!q) return;
     free(q->x); free(q->y); free(q->B); free(q->ofs); free(q->pos); free(q->inten);
-    free(q->jm); free(q->sigma_n); free(q->lambda_h); free(q->eta_h);
+    free(q->jm); free(q->sigma_n); free(q->lambda_h); free(q->eta_h); free(q->n_ck);
     free(q);
 }
 
@@ -180,21 +183,60 @@ int64_t orc_window_halfwidth(const orc_problem *q) { return q->n_c; }
 double orc_sigma_n(const orc_problem *q, int32_t pat) { return q->sigma_n[pat]; }
 double orc_lambda_h(const orc_problem *q, int32_t pat) { return q->lambda_h[pat]; }
 
-/* R16: pair (m,i) is in the model iff |i - j_m| <= n_c and 0 <= i < N (dense: every i).
- * The loops below run i over exactly that index range. */
-static void window(const orc_problem *q, int64_t m, int64_t *i_lo, int64_t *i_hi) {
+/* R16: pair (m,i), m a peak of phase k, is in the model iff |i - j_m| <= n_c and 0 <= i < N (dense: every
+ * i).  R27: with per-phase half-widths set, n_c is replaced by n_c,k.  The loops below run i over exactly
+ * that index range. */
+static int64_t halfwidth(const orc_problem *q, int32_t k) { return q->n_ck ? q->n_ck[k] : q->n_c; }
+
+static void window(const orc_problem *q, int32_t k, int64_t m, int64_t *i_lo, int64_t *i_hi) {
     if (q->n_c < 0) { *i_lo = 0; *i_hi = q->N - 1; return; }
-    *i_lo = q->jm[m] - q->n_c; if (*i_lo < 0) *i_lo = 0;
-    *i_hi = q->jm[m] + q->n_c; if (*i_hi > q->N - 1) *i_hi = q->N - 1;
+    *i_lo = q->jm[m] - halfwidth(q, k); if (*i_lo < 0) *i_lo = 0;
+    *i_hi = q->jm[m] + halfwidth(q, k); if (*i_hi > q->N - 1) *i_hi = q->N - 1;
 }
 
 /* number of in-window (m,i) pairs per instance (the metric's unit) */
 int64_t orc_pair_count(const orc_problem *q) {
     int64_t n = 0;
-    for (int64_t m = 0; m < q->M; ++m)
-        for (int64_t i = 0; i < q->N; ++i)
-            if (q->n_c < 0 || llabs(i - q->jm[m]) <= q->n_c) ++n;
+    for (int32_t k = 0; k < q->K; ++k)
+        for (int64_t m = q->ofs[k]; m < q->ofs[k + 1]; ++m)
+            for (int64_t i = 0; i < q->N; ++i)
+                if (q->n_c < 0 || llabs(i - q->jm[m]) <= halfwidth(q, k)) ++n;
     return n;
+}
+
+/* R27: replace the static half-width by per-phase ones, 0 <= n_c,k <= n_c (NULL: back to the static window).
+ * Returns 0, or -1 if the problem is dense or a value is out of range (nothing changed then). */
+int orc_set_phase_windows(orc_problem *q, const int64_t *n_ck) {
+    if (!n_ck) { free(q->n_ck); q->n_ck = NULL; return 0; }
+    if (q->n_c < 0) return -1;
+    for (int32_t k = 0; k < q->K; ++k) if (n_ck[k] < 0 || n_ck[k] > q->n_c) return -1;
+    if (!q->n_ck) q->n_ck = (int64_t *)malloc(sizeof(int64_t) * q->K);
+    memcpy(q->n_ck, n_ck, sizeof(int64_t) * q->K);
+    return 0;
+}
+
+/* R27, the refresh rule: the window of phase k must hold +-W FWHM around the SHIFTED peak centre p_m + mu_k
+ * while staying centred on the table position j_m, with FWHM and shift at their variational means
+ * wbar = E_q[w_k] = exp(m_w + s_w^2/2), mubar = m_mu, the widest over the (pattern, restart) instances:
+ *   n_c,k = min( n_c, max( n_min, ceil( max_inst (W wbar + |mubar|) / Delta - 1e-9 ) ) ),
+ *   n_min = ceil(2 W - 1e-9)   (the half-width of a peak of FWHM 2 Delta: narrower peaks are not resolved
+ *                               by the grid and the window never shrinks below that). */
+void orc_adaptive_halfwidths(const orc_problem *q, const double *state, double W, int64_t *n_ck) {
+    const int32_t K = q->K;
+    const int64_t n_min = (int64_t)ceil(2.0 * W - 1e-9);
+    for (int32_t k = 0; k < K; ++k) {
+        double c = 0.0;
+        for (int32_t inst = 0; inst < q->P * q->R; ++inst) {
+            const double *m = state + (size_t)inst * 2 * K * 4, *l = m + (size_t)K * 4;
+            double s_w = exp(l[4 * k + 2]);
+            double ci = W * exp(m[4 * k + 2] + 0.5 * s_w * s_w) + fabs(m[4 * k + 1]);
+            if (ci > c) c = ci;
+        }
+        int64_t n = (int64_t)ceil(c / q->delta - 1e-9);
+        if (n < n_min) n = n_min;
+        if (n > q->n_c) n = q->n_c;
+        n_ck[k] = n;
+    }
 }
 
 /* ------------------------------------------------------------------ peak shapes (R1) */
@@ -230,7 +272,7 @@ void orc_profile(const orc_problem *q, int32_t pat, const double *zeta /*[K][4]*
         for (int64_t m = q->ofs[k]; m < q->ofs[k + 1]; ++m) {
             double rho = q->pos[m] + mu;                                  /* A8 */
             int64_t i_lo, i_hi;
-            window(q, m, &i_lo, &i_hi);
+            window(q, k, m, &i_lo, &i_hi);
             for (int64_t i = i_lo; i <= i_hi; ++i) {
                 f[i] += h * q->inten[m] * orc_pseudo_voigt(q->x[i], rho, w, r);
             }
@@ -292,7 +334,7 @@ void orc_logjoint_grad(const orc_problem *q, int32_t pat, const double *zeta, do
         for (int64_t m = q->ofs[k]; m < q->ofs[k + 1]; ++m) {
             double I = q->inten[m], rho = q->pos[m] + mu;
             int64_t i_lo, i_hi;
-            window(q, m, &i_lo, &i_hi);
+            window(q, k, m, &i_lo, &i_hi);
             for (int64_t i = i_lo; i <= i_hi; ++i) {
                 double e = q->hy.likelihood == 1
                                ? q->y[pat * N + i] / f[i] - 1.0                  /* d ll / d f_i of A16    */

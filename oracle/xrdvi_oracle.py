@@ -80,6 +80,9 @@ def lib():
         L.orc_init_state.argtypes = [C.c_void_p, C.c_uint64, dp]
         L.orc_fit.argtypes = [C.c_void_p, dp, dp, dp, C.c_int32, C.c_int32, C.c_uint64, C.c_int64, dp]
         L.orc_inclusion.argtypes = [C.c_void_p, dp, dp, dp]
+        L.orc_set_phase_windows.restype = C.c_int
+        L.orc_set_phase_windows.argtypes = [C.c_void_p, C.POINTER(C.c_int64)]
+        L.orc_adaptive_halfwidths.argtypes = [C.c_void_p, dp, C.c_double, C.POINTER(C.c_int64)]
         L.orc_num_threads.restype = C.c_int
         _lib = L
     return _lib
@@ -254,6 +257,37 @@ class Oracle:
         lib().orc_fit(self._h, _dp(st), _dp(m1), _dp(m2), int(iterations), int(S), int(seed),
                       int(first_step), _dp(tr))
         return st, (m1, m2), tr
+
+    # ---- adaptive windows (R27) ---------------------------------------------
+    def set_phase_windows(self, n_ck=None):
+        """Per-phase window half-widths (points), 0 <= n_ck[k] <= n_c; None restores the static window."""
+        if n_ck is None:
+            lib().orc_set_phase_windows(self._h, None)
+            return
+        a = np.ascontiguousarray(n_ck, dtype=np.int64).reshape(self.K)
+        if lib().orc_set_phase_windows(self._h, a.ctypes.data_as(C.POINTER(C.c_int64))) != 0:
+            raise ValueError("per-phase half-widths need a windowed problem and 0 <= n_ck <= n_c")
+
+    def adaptive_halfwidths(self, state, W):
+        st = self._state(state)
+        out = np.empty(self.K, dtype=np.int64)
+        lib().orc_adaptive_halfwidths(self._h, _dp(st), float(W), out.ctypes.data_as(C.POINTER(C.c_int64)))
+        return out
+
+    def fit_adaptive(self, state, iterations, S, seed, refresh_every, W):
+        """R27: `iterations` steps in pieces of `refresh_every`; after every piece but the last the per-phase
+        windows are refreshed from the current state.  Starts from the windows currently set.  Returns
+        (state, list of the half-width vectors set after each refresh)."""
+        st, mom, done, hist = self._state(state).copy(), None, 0, []
+        while done < iterations:
+            n = min(int(refresh_every), iterations - done)
+            st, mom, _ = self.fit(st, n, S, seed, first_step=done + 1, mom=mom)
+            done += n
+            if done < iterations:
+                nck = self.adaptive_halfwidths(st, W)
+                self.set_phase_windows(nck)
+                hist.append(nck)
+        return st, hist
 
     def inclusion(self, state, want_area=False):
         st = self._state(state)
