@@ -109,6 +109,32 @@ int64_t xrdvi_pair_count(const xrdvi* h);
 /* Window half-width n_c in grid points (N for dense).                                              */
 int64_t xrdvi_window_halfwidth(const xrdvi* h);
 
+/* ---- Per-phase (adaptive) windows: DESIGN.md reading R27 of north_star's "pseudo-Voigt truncated at a
+ * problem-defined +-W FWHM cutoff" (second half).  The paper evaluates every peak on
+ * the whole grid; the window is this build's model reading R16.
+ *
+ * xrdvi_set_phase_windows: replace the static half-width n_c by per-phase ones, n_ck int32 [K] HOST,
+ *   0 <= n_ck[k] <= n_c (the create-time window sizes the workspace); NULL restores the static window.  A pair
+ *   (m, i), m a peak of phase k, is in the model iff |i - j_m| <= n_ck[k] and 0 <= i < N.  Rebuilds the per-tile
+ *   tables on the host (integers only) and uploads them; variational state, Adam moments and step counter are
+ *   untouched; xrdvi_pair_count follows.  Synchronises the stream.  XRDVI_E_INVALID_ARG on a dense problem
+ *   (window_W <= 0) or an out-of-range value (nothing changed then).
+ * xrdvi_get_phase_windows: the half-widths in force, n_ck int32 [K] HOST (all n_c after create).
+ * xrdvi_adapt_windows: the refresh rule.  Reads the variational state and sets
+ *     n_ck[k] = min(n_c, max(ceil(2 W - 1e-9), ceil(max_inst(W E_q[w_k] + |E_q[mu_k]|) / Delta - 1e-9))),
+ *     E_q[w_k] = exp(m_w + sigma_w^2 / 2), E_q[mu_k] = m_mu, the maximum over the (pattern, restart) instances,
+ *   i.e. +-W FWHM around the shifted peak centre at the variational means, never narrower than the window of
+ *   a peak of FWHM 2 Delta.  fp64 on the host from the fp32 state.  n_ck_out int32 [K] HOST or NULL.
+ * xrdvi_fit_adaptive: `iterations` steps as xrdvi_fit, in pieces of `refresh_every` steps with
+ *   xrdvi_adapt_windows(h, W) between the pieces (not after the last).  Starts from the windows in force and
+ *   leaves the last refreshed ones in force.  Outputs as xrdvi_fit (host buffers, NULL to skip; elbo_trace
+ *   rows older than 4096 steps within a piece are NaN).                                                     */
+int xrdvi_set_phase_windows(xrdvi* h, const int32_t* n_ck);
+int xrdvi_get_phase_windows(const xrdvi* h, int32_t* n_ck);
+int xrdvi_adapt_windows(xrdvi* h, double W, int32_t* n_ck_out);
+int xrdvi_fit_adaptive(xrdvi* h, int32_t iterations, int32_t S, uint64_t seed, int32_t refresh_every, double W,
+                       float* var_params_out, double* incl_prob, double* elbo_trace);
+
 /* (Re)initialise the variational state (R11), zero the Adam moments and the step counter.
  * Restart r > 0 is jittered with Philox counter (0xFFFFFFFF, r, k, pat) under `seed`.              */
 int xrdvi_reset_state(xrdvi* h, uint64_t seed);

@@ -16,7 +16,8 @@ _LIB_PATH = _PKG / "libxrdvi.so"
 
 EXPORTS = (
     "xrdvi_default_hyper", "xrdvi_workspace_bytes", "xrdvi_create", "xrdvi_destroy", "xrdvi_pair_count",
-    "xrdvi_window_halfwidth", "xrdvi_reset_state", "xrdvi_get_state", "xrdvi_set_state", "xrdvi_elbo_grad",
+    "xrdvi_window_halfwidth", "xrdvi_set_phase_windows", "xrdvi_get_phase_windows", "xrdvi_adapt_windows",
+    "xrdvi_fit_adaptive", "xrdvi_reset_state", "xrdvi_get_state", "xrdvi_set_state", "xrdvi_elbo_grad",
     "xrdvi_fit", "xrdvi_inclusion", "xrdvi_logjoint_grad", "xrdvi_debug_profile", "xrdvi_debug_draws", "xrdvi_time_kernels",
     "xrdvi_bench_steps", "xrdvi_debug_timeline", "xrdvi_pipe_rates", "xrdvi_last_error",
 )
@@ -65,6 +66,11 @@ def load_library():
     L.xrdvi_pair_count.restype = C.c_int64
     L.xrdvi_window_halfwidth.argtypes = [vp]
     L.xrdvi_window_halfwidth.restype = C.c_int64
+    ip = C.POINTER(C.c_int32)
+    L.xrdvi_set_phase_windows.argtypes = [vp, ip]
+    L.xrdvi_get_phase_windows.argtypes = [vp, ip]
+    L.xrdvi_adapt_windows.argtypes = [vp, C.c_double, ip]
+    L.xrdvi_fit_adaptive.argtypes = [vp, C.c_int32, C.c_int32, C.c_uint64, C.c_int32, C.c_double, fp, dp, dp]
     L.xrdvi_reset_state.argtypes = [vp, C.c_uint64]
     L.xrdvi_get_state.argtypes = [vp, fp, C.POINTER(C.c_int64)]
     L.xrdvi_set_state.argtypes = [vp, fp, C.c_int64]
@@ -209,6 +215,32 @@ class Xrdvi:
         inc = np.empty((self.P, self.R, self.K), dtype=np.float64) if want_incl else None
         tr = np.empty((int(iterations), self.P, self.R), dtype=np.float64) if want_trace else None
         _check(load_library().xrdvi_fit(self._h, int(iterations), S, int(seed), _f(st), _d(inc), _d(tr)))
+        return st, inc, tr
+
+    # ---- per-phase (adaptive) windows, R27 ---------------------------------------
+    def set_phase_windows(self, n_ck=None):
+        a = None if n_ck is None else np.ascontiguousarray(n_ck, dtype=np.int32).reshape(self.K)
+        _check(load_library().xrdvi_set_phase_windows(
+            self._h, None if a is None else a.ctypes.data_as(C.POINTER(C.c_int32))))
+
+    def get_phase_windows(self):
+        a = np.empty(self.K, dtype=np.int32)
+        _check(load_library().xrdvi_get_phase_windows(self._h, a.ctypes.data_as(C.POINTER(C.c_int32))))
+        return a
+
+    def adapt_windows(self, W):
+        a = np.empty(self.K, dtype=np.int32)
+        _check(load_library().xrdvi_adapt_windows(self._h, float(W), a.ctypes.data_as(C.POINTER(C.c_int32))))
+        return a
+
+    def fit_adaptive(self, iterations, refresh_every, W, S=None, seed=0, want_state=True, want_incl=True,
+                     want_trace=False):
+        S = self.S_max if S is None else int(S)
+        st = np.empty(self._state_shape(), dtype=np.float32) if want_state else None
+        inc = np.empty((self.P, self.R, self.K), dtype=np.float64) if want_incl else None
+        tr = np.empty((int(iterations), self.P, self.R), dtype=np.float64) if want_trace else None
+        _check(load_library().xrdvi_fit_adaptive(self._h, int(iterations), S, int(seed), int(refresh_every),
+                                                 float(W), _f(st), _d(inc), _d(tr)))
         return st, inc, tr
 
     def logjoint_grad(self, zeta, pattern=0):

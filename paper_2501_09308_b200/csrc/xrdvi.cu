@@ -142,6 +142,124 @@ bool make_plan(int64_t N, int32_t K, int64_t M, int32_t S_max, double step, cons
     return true;
 }
 
+// ---- static tables (R16, R27) -----------------------------------------------------------------------
+struct HostPeak { long long j; double d; double I; int k; };   // nearest grid index, p_m - x_j, intensity, phase
+
+struct Tables {
+    std::vector<PeakRec> pk_tile;     // per-tile phase-major peak lists (+1 padding record)
+    std::vector<int4> run_tab;        // (m0, m1, phase, slot) per phase run (+1 padding header)
+    std::vector<int2> share_rng;      // [n_tile][PS] run ranges of the shares
+    std::vector<int> seg_order, slot_ofs;
+    int n_slots = 0;
+    long long pairs = 0;              // in-window (peak, point) pairs per draw
+};
+
+// Per-tile phase-major lists: the peaks whose window reaches the tile, stable-sorted by phase; PS contiguous shares
+// split at phase boundaries and balanced by clipped pair count; one output slot per (tile, phase present in the
+// tile).  `nck[k]` is the window half-width of phase k in points (the static n_c for every phase at create; per
+// phase after xrdvi_set_phase_windows, R27); peaks with no in-range grid point are dropped.  All in integers.
+const char* build_tables(const Plan& pl, int64_t N, int K, const std::vector<HostPeak>& all,
+                         const std::vector<long long>& nck, Tables* T) {
+    std::vector<HostPeak> fw;
+    fw.reserve(all.size());
+    long long pairs = 0;
+    for (const HostPeak& p : all) {
+        const long long lo = std::max<long long>(0, p.j - nck[p.k]), hi = std::min<long long>(N - 1, p.j + nck[p.k]);
+        if (lo > hi) continue;  // no in-range grid point
+        pairs += hi - lo + 1;
+        fw.push_back(p);
+    }
+    // (phase, grid index, input order) order: the order of the entries inside every tile list
+    std::stable_sort(fw.begin(), fw.end(), [](const HostPeak& a, const HostPeak& b) { return a.j < b.j; });
+    std::stable_sort(fw.begin(), fw.end(), [](const HostPeak& a, const HostPeak& b) { return a.k < b.k; });
+    const int PSn = pl.PS, TWn = pl.TW, n_tile = pl.n_tile;
+    auto tiles_of = [&](const HostPeak& p, int* t0, int* t1) {
+        const long long lo = std::max<long long>(0, p.j - nck[p.k]), hi = std::min<long long>(N - 1, p.j + nck[p.k]);
+        *t0 = static_cast<int>(lo / kPT);
+        *t1 = static_cast<int>(hi / kPT);
+    };
+    // pass 1: entries and phase runs per tile
+    std::vector<long long> ent_base(n_tile + 1, 0);
+    std::vector<int> run_base(n_tile + 1, 0), last_k(n_tile, -1);
+    for (const HostPeak& p : fw) {
+        int t0, t1;
+        tiles_of(p, &t0, &t1);
+        for (int t = t0; t <= t1; ++t) {
+            ++ent_base[t + 1];
+            if (last_k[t] != p.k) { last_k[t] = p.k; ++run_base[t + 1]; }
+        }
+    }
+    for (int t = 0; t < n_tile; ++t) { ent_base[t + 1] += ent_base[t]; run_base[t + 1] += run_base[t]; }
+    const long long n_ent = ent_base[n_tile];
+    const int n_runs = run_base[n_tile];
+    if (n_ent > pl.tile_cap || n_runs > pl.slots_cap) return "internal: table bound exceeded";
+    // pass 2: fill the lists, the run headers (m0, m1, phase, 0) and the clipped pair count of every run
+    T->pk_tile.assign(static_cast<size_t>(n_ent) + 1, PeakRec{0, 0.f, 0.f, 0});   // +1: the kernel prefetches one
+    T->run_tab.assign(static_cast<size_t>(n_runs) + 1, make_int4(0, 0, 0, 0));    // record / header past the end
+    T->share_rng.assign(static_cast<size_t>(n_tile) * PSn, make_int2(0, 0));
+    std::vector<long long> run_w(n_runs, 0), seg_work(pl.n_seg, 0);
+    std::vector<long long> ent_cur(ent_base.begin(), ent_base.end() - 1);
+    std::vector<int> run_cur(run_base.begin(), run_base.end() - 1);
+    std::fill(last_k.begin(), last_k.end(), -1);
+    long long pairs_check = 0;
+    for (const HostPeak& p : fw) {
+        int t0, t1;
+        tiles_of(p, &t0, &t1);
+        const long long n = nck[p.k];
+        for (int t = t0; t <= t1; ++t) {
+            const long long i0 = static_cast<long long>(t) * kPT, i1 = std::min<long long>(i0 + kPT - 1, N - 1);
+            const long long wq = std::min(i1, p.j + n) - std::max(i0, p.j - n) + 1;   // >= 1 by construction
+            const long long dj = p.j - i0;
+            const bool full = (i1 - i0 == kPT - 1) && dj - n <= 0 && dj + n >= kPT - 1;
+            const long long e = ent_cur[t]++;
+            T->pk_tile[e] = PeakRec{static_cast<int>(dj), static_cast<float>(p.d), static_cast<float>(p.I),
+                                    static_cast<int>(n << 1) | (full ? 1 : 0)};
+            if (last_k[t] != p.k) {
+                last_k[t] = p.k;
+                T->run_tab[run_cur[t]++] = make_int4(static_cast<int>(e), static_cast<int>(e), p.k, 0);
+            }
+            const int r = run_cur[t] - 1;
+            T->run_tab[r].y = static_cast<int>(e) + 1;
+            run_w[r] += wq;
+            seg_work[t / TWn] += wq;
+            pairs_check += wq;
+        }
+    }
+    // pass 3: PS contiguous shares per tile, split at phase boundaries, balanced by clipped pair count
+    std::vector<int> slot_phase(n_runs);
+    for (int r = 0; r < n_runs; ++r) slot_phase[r] = T->run_tab[r].z;
+    for (int t = 0; t < n_tile; ++t) {
+        long long tot = 0;
+        for (int r = run_base[t]; r < run_base[t + 1]; ++r) tot += run_w[r];
+        int run = run_base[t];
+        long long cum = 0;
+        for (int w = 0; w < PSn; ++w) {
+            const int run0 = run;
+            const long long goal = tot * (w + 1) / PSn;
+            if (w == PSn - 1) run = run_base[t + 1];
+            else while (run < run_base[t + 1] && cum + run_w[run] <= goal) { cum += run_w[run]; ++run; }
+            T->share_rng[static_cast<size_t>(t) * PSn + w] = make_int2(run0, run);
+        }
+    }
+    if (pairs_check != pairs) return "internal: tile tables do not cover every pair once";
+    const int n_slots = n_runs;
+    // output slots numbered phase-major (the reduction over the tiles of a phase reads one contiguous range);
+    // within a phase in increasing tile order
+    T->slot_ofs.assign(K + 1, 0);
+    for (int s = 0; s < n_slots; ++s) ++T->slot_ofs[slot_phase[s] + 1];
+    for (int k = 0; k < K; ++k) T->slot_ofs[k + 1] += T->slot_ofs[k];
+    {
+        std::vector<int> fill(T->slot_ofs.begin(), T->slot_ofs.end() - 1);
+        for (int s = 0; s < n_slots; ++s) T->run_tab[s].w = fill[slot_phase[s]]++;
+    }
+    T->seg_order.resize(pl.n_seg);
+    std::iota(T->seg_order.begin(), T->seg_order.end(), 0);
+    std::stable_sort(T->seg_order.begin(), T->seg_order.end(), [&](int a, int b) { return seg_work[a] > seg_work[b]; });
+    T->n_slots = n_slots;
+    T->pairs = pairs;
+    return nullptr;
+}
+
 }  // namespace
 
 struct xrdvi {
@@ -153,7 +271,11 @@ struct xrdvi {
     char* ws = nullptr;
     int64_t N = 0, M = 0, pairs = 0;
     int K = 0;
-    int n_c = 0;
+    int n_c = 0;               // create-time (static) half-width; the cap of the per-phase ones
+    bool windowed = false;     // hyper.window_W > 0
+    double delta = 0.0;        // grid step
+    std::vector<HostPeak> peaks;   // every input peak, CSR order (xrdvi_set_phase_windows rebuilds the tables from it)
+    std::vector<long long> n_ck;   // [K] half-width per phase in force (R27); all n_c after create
     std::vector<float> m_h0;   // per pattern initial m_h
     float m_w0 = 0.f;
     long long step_host = 0;   // mirror of ctl.step
@@ -171,6 +293,34 @@ void set_S(xrdvi* h, int S) {
     h->dev.S = S;
     h->dev.gpi = (S + 31) / 32;
     h->dev.G = h->plan.PR * h->dev.gpi;
+}
+
+// Upload a set of static tables and make them the ones in force.  The Dev block (kernel argument, held by value in
+// the captured graphs) does not change after create: `n_slots` is only the row stride of the backward's output
+// slots and stays at the create-time count (per-phase windows are never wider than the static one, so a later
+// table set has at most as many (tile, phase) runs), and the fused / ticket-queue choice is made once.  A refresh
+// therefore needs no graph re-capture.
+int install_tables(xrdvi* h, const Tables& T, const std::vector<long long>& nck, bool at_create) {
+    const Plan& pl = h->plan;
+    Dev& d = h->dev;
+    cudaStream_t st = h->stream;
+    char* w = h->ws;
+    if (!at_create && T.n_slots > d.n_slots) return fail(XRDVI_E_INVALID_ARG, "internal: more output slots than at create");
+    CU(cudaStreamSynchronize(st));   // nothing in flight may still read the old tables
+    CU(cudaMemcpyAsync(w + pl.o_pkt, T.pk_tile.data(), sizeof(PeakRec) * T.pk_tile.size(), cudaMemcpyHostToDevice, st));
+    CU(cudaMemcpyAsync(w + pl.o_runs, T.run_tab.data(), sizeof(int4) * T.run_tab.size(), cudaMemcpyHostToDevice, st));
+    CU(cudaMemcpyAsync(w + pl.o_srng, T.share_rng.data(), sizeof(int2) * T.share_rng.size(), cudaMemcpyHostToDevice, st));
+    CU(cudaMemcpyAsync(w + pl.o_sord, T.seg_order.data(), sizeof(int) * T.seg_order.size(), cudaMemcpyHostToDevice, st));
+    CU(cudaMemcpyAsync(w + pl.o_sofs, T.slot_ofs.data(), sizeof(int) * T.slot_ofs.size(), cudaMemcpyHostToDevice, st));
+    if (at_create) {
+        d.n_slots = std::max(T.n_slots, 1);
+        d.split = T.pairs / (static_cast<long long>(pl.n_tile) * pl.PS * kPT) >= 512 ? 1 : 0;   // peaks per work item
+        CU(cudaMemsetAsync(w + pl.o_part8, 0, sizeof(float) * static_cast<size_t>(pl.G_max) * d.n_slots * 8, st));
+    }
+    CU(cudaStreamSynchronize(st));   // T belongs to the caller
+    h->pairs = T.pairs;
+    h->n_ck = nck;
+    return XRDVI_OK;
 }
 
 // Few tile-warps (PS > 1) and long work items: one-warp CTAs on a ticket queue (elbo_split_kernel) instead of PS-warp
@@ -422,109 +572,24 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
             n_c = std::max<long long>(n_c, std::max<long long>(std::llabs(j), std::llabs(N - 1 - j)) + 1);
         }
     }
-    if (n_c > (1ll << 30)) return fail(XRDVI_E_INVALID_ARG, "peak positions too far from the grid");
-    struct HP { long long j; double d; double I; int k; };
-    std::vector<HP> kept;
-    kept.reserve(M);
+    if (n_c > (1ll << 29)) return fail(XRDVI_E_INVALID_ARG, "peak positions too far from the grid");
+    std::vector<HostPeak> all_peaks;
+    all_peaks.reserve(M);
     std::vector<double> area(K, 0.0);
     double imax = 0.0;
-    long long pairs = 0;
     for (int k = 0; k < K; ++k)
         for (int64_t m = ofs[k]; m < ofs[k + 1]; ++m) {
             area[k] += inten[m];
             imax = std::max(imax, inten[m]);
             const long long j = static_cast<long long>(std::floor((pos[m] - x[0]) / delta + 0.5));
-            const long long lo = std::max<long long>(0, j - n_c), hi = std::min<long long>(N - 1, j + n_c);
-            if (lo > hi) continue;  // no in-range grid point
-            pairs += hi - lo + 1;
             const double xj = (j >= 0 && j < N) ? x[j] : x[0] + delta * static_cast<double>(j);
-            kept.push_back({j, pos[m] - xj, inten[m], k});
+            all_peaks.push_back({j, pos[m] - xj, inten[m], k});
         }
     for (int k = 0; k < K; ++k)
         if (!(area[k] > 0.0)) return fail(XRDVI_E_EMPTY_PHASE, "phase " + std::to_string(k) + " has zero total intensity");
-
-    // per-tile phase-major lists: the peaks whose window reaches the tile, stable-sorted by phase; PS
-    // contiguous shares split at phase boundaries and balanced by clipped pair count; one output slot per
-    // (tile, phase present in the tile)
-    std::vector<HP> fw = kept;
-    std::stable_sort(fw.begin(), fw.end(), [](const HP& a, const HP& b) { return a.j < b.j; });
-    auto j_range = [&](long long jlo, long long jhi) {
-        auto a = std::lower_bound(fw.begin(), fw.end(), jlo, [](const HP& p, long long v) { return p.j < v; });
-        auto b = std::upper_bound(fw.begin(), fw.end(), jhi, [](long long v, const HP& p) { return v < p.j; });
-        return make_int2(static_cast<int>(a - fw.begin()), static_cast<int>(b - fw.begin()));
-    };
-    const int PSn = pl.PS, TWn = pl.TW;
-    std::vector<PeakRec> pk_tile;
-    pk_tile.reserve(static_cast<size_t>(std::min<long long>(pl.tile_cap, 1ll << 24)));
-    std::vector<int4> run_tab;                                  // (m0, m1, phase, 0); index = output slot
-    std::vector<int2> share_rng(static_cast<size_t>(pl.n_tile) * PSn);
-    std::vector<long long> seg_work(pl.n_seg, 0);
-    std::vector<int> slot_phase;
-    long long pairs_check = 0;
-    {
-        std::vector<HP> tl;
-        std::vector<long long> run_w;      // clipped pair count per phase run
-        std::vector<int> run_end;          // end index (exclusive) of each phase run in tl
-        for (int t = 0; t < pl.n_tile; ++t) {
-            const long long i0 = static_cast<long long>(t) * kPT, i1 = std::min<long long>(i0 + kPT - 1, N - 1);
-            const int2 r = j_range(i0 - n_c, i1 + n_c);
-            tl.assign(fw.begin() + r.x, fw.begin() + r.y);
-            std::stable_sort(tl.begin(), tl.end(), [](const HP& a, const HP& b) { return a.k < b.k; });
-            run_w.clear();
-            run_end.clear();
-            long long tot = 0;
-            for (size_t q = 0; q < tl.size(); ++q) {
-                const long long lo = std::max(i0, tl[q].j - n_c), hi = std::min(i1, tl[q].j + n_c);
-                const long long wq = hi - lo + 1;   // >= 1 by construction of the range
-                if (q == 0 || tl[q].k != tl[q - 1].k) { run_w.push_back(0); run_end.push_back(0); }
-                run_w.back() += wq;
-                run_end.back() = static_cast<int>(q + 1);
-                tot += wq;
-            }
-            seg_work[t / TWn] += tot;
-            pairs_check += tot;
-            const int base = static_cast<int>(pk_tile.size());
-            for (const HP& p : tl) {
-                const long long dj = p.j - i0;
-                const bool full = (i1 - i0 == kPT - 1) && dj - n_c <= 0 && dj + n_c >= kPT - 1;
-                pk_tile.push_back(PeakRec{static_cast<int>(dj), static_cast<float>(p.d), static_cast<float>(p.I), full ? 1 : 0});
-            }
-            const int run_base = static_cast<int>(run_tab.size());
-            for (size_t rr = 0; rr < run_w.size(); ++rr) {
-                const int q0 = rr ? run_end[rr - 1] : 0;
-                run_tab.push_back(make_int4(base + q0, base + run_end[rr], tl[q0].k, 0));
-                slot_phase.push_back(tl[q0].k);
-            }
-            size_t run = 0;
-            long long cum = 0;
-            for (int w = 0; w < PSn; ++w) {
-                const size_t run0 = run;
-                const long long goal = tot * (w + 1) / PSn;
-                if (w == PSn - 1) run = run_w.size();
-                else while (run < run_w.size() && cum + run_w[run] <= goal) { cum += run_w[run]; ++run; }
-                share_rng[static_cast<size_t>(t) * PSn + w] =
-                    make_int2(run_base + static_cast<int>(run0), run_base + static_cast<int>(run));
-            }
-        }
-    }
-    if (pairs_check != pairs) return fail(XRDVI_E_INVALID_ARG, "internal: tile tables do not cover every pair once");
-    const int n_slots = static_cast<int>(slot_phase.size());
-    if (static_cast<long long>(pk_tile.size()) > pl.tile_cap + 1 || n_slots > pl.slots_cap)
-        return fail(XRDVI_E_INVALID_ARG, "internal: table bound exceeded");
-    // output slots numbered phase-major (the reduction over the tiles of a phase reads one contiguous range);
-    // within a phase in increasing tile order
-    std::vector<int> slot_ofs(K + 1, 0);
-    for (int s = 0; s < n_slots; ++s) ++slot_ofs[slot_phase[s] + 1];
-    for (int k = 0; k < K; ++k) slot_ofs[k + 1] += slot_ofs[k];
-    {
-        std::vector<int> fill(slot_ofs.begin(), slot_ofs.end() - 1);
-        for (int s = 0; s < n_slots; ++s) run_tab[s].w = fill[slot_phase[s]]++;
-    }
-    std::vector<int> seg_order(pl.n_seg);
-    std::iota(seg_order.begin(), seg_order.end(), 0);
-    std::stable_sort(seg_order.begin(), seg_order.end(), [&](int a, int b) { return seg_work[a] > seg_work[b]; });
-    pk_tile.push_back(PeakRec{0, 0.f, 0.f, 0});       // padding entries: the kernel prefetches one record and
-    run_tab.push_back(make_int4(0, 0, 0, 0));         // one run header past the end of every share
+    const std::vector<long long> nck0(K, n_c);
+    Tables tabs;
+    if (const char* terr = build_tables(pl, N, K, all_peaks, nck0, &tabs)) return fail(XRDVI_E_INVALID_ARG, terr);
 
     // observed data and per-pattern constants
     std::vector<float> yb(static_cast<size_t>(P) * N), bgf(static_cast<size_t>(P) * N);
@@ -572,16 +637,17 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
     h->device = device;
     h->stream = static_cast<cudaStream_t>(cuda_stream);
     h->ws = static_cast<char*>(workspace);
-    h->N = N; h->M = M; h->K = K; h->pairs = pairs; h->n_c = static_cast<int>(n_c);
+    h->N = N; h->M = M; h->K = K; h->n_c = static_cast<int>(n_c);
+    h->windowed = pl.n_c >= 0;
+    h->delta = delta;
+    h->peaks = std::move(all_peaks);
     h->m_h0 = m_h0;
     h->m_w0 = static_cast<float>(std::log(hyp->w_shape / hyp->w_rate));
     Dev& d = h->dev;
     char* w = h->ws;
     d.N = static_cast<int>(N); d.K = K; d.P = pl.P; d.R = pl.R; d.PR = pl.PR;
     d.n_c = static_cast<int>(n_c); d.TW = pl.TW; d.PS = pl.PS; d.n_seg = pl.n_seg; d.n_tile = pl.n_tile;
-    d.n_slots = std::max(n_slots, 1);
     d.likelihood = hyp->likelihood;
-    d.split = pairs / (static_cast<long long>(pl.n_tile) * pl.PS * kPT) >= 512 ? 1 : 0;   // peaks per work item
     d.optimizer = hyp->optimizer;
     d.delta = static_cast<float>(delta);
     d.gcut = static_cast<float>(static_cast<double>(kGaussCut) / (2.0 * delta));
@@ -632,17 +698,11 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
     auto chk = [&](cudaError_t e) { if (ce == cudaSuccess) ce = e; };
     chk(up(pl.o_yb, yb.data(), sizeof(float) * yb.size()));
     chk(up(pl.o_bg, bgf.data(), sizeof(float) * bgf.size()));
-    chk(up(pl.o_pkt, pk_tile.data(), sizeof(PeakRec) * pk_tile.size()));
-    chk(up(pl.o_runs, run_tab.data(), sizeof(int4) * run_tab.size()));
-    chk(up(pl.o_srng, share_rng.data(), sizeof(int2) * share_rng.size()));
-    chk(up(pl.o_sord, seg_order.data(), sizeof(int) * seg_order.size()));
-    chk(up(pl.o_sofs, slot_ofs.data(), sizeof(int) * slot_ofs.size()));
     chk(up(pl.o_pat, pat.data(), sizeof(PatConst) * pat.size()));
     chk(up(pl.o_area, area.data(), sizeof(double) * area.size()));
     chk(up(pl.o_mh0, m_h0.data(), sizeof(float) * m_h0.size()));
     chk(cudaMemsetAsync(w + pl.o_tcnt, 0, sizeof(unsigned int) * 2 * static_cast<size_t>(pl.G_max) * pl.n_tile, st));
     chk(cudaMemsetAsync(w + pl.o_trace, 0xFF, sizeof(double) * kTraceCap * pl.PR, st));
-    chk(cudaMemsetAsync(w + pl.o_part8, 0, sizeof(float) * static_cast<size_t>(pl.G_max) * d.n_slots * 8, st));
     chk(cudaStreamSynchronize(st));  // host staging vectors go out of scope below
     for (auto& e : h->ev) chk(cudaEventCreate(&e));
 
@@ -650,7 +710,8 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
         delete h;
         return fail(XRDVI_E_CUDA, std::string("upload: ") + cudaGetErrorString(ce));
     }
-    int rc = xrdvi_reset_state(h, 0);
+    int rc = install_tables(h, tabs, nck0, true);
+    if (rc == XRDVI_OK) rc = xrdvi_reset_state(h, 0);
     if (rc != XRDVI_OK) { xrdvi_destroy(h); return rc; }
     *out = h;
     return XRDVI_OK;
@@ -667,6 +728,84 @@ void xrdvi_destroy(xrdvi* h) {
 
 int64_t xrdvi_pair_count(const xrdvi* h) { return h ? h->pairs : -1; }
 int64_t xrdvi_window_halfwidth(const xrdvi* h) { return h ? h->n_c : -1; }
+
+// ---- per-phase (adaptive) windows, R27 ---------------------------------------------------------------
+int xrdvi_set_phase_windows(xrdvi* h, const int32_t* n_ck) {
+    if (!h) return fail(XRDVI_E_INVALID_ARG, "null handle");
+    if (!h->windowed) return fail(XRDVI_E_INVALID_ARG, "per-phase windows need a windowed problem (window_W > 0)");
+    std::vector<long long> nck(h->K, h->n_c);
+    if (n_ck)
+        for (int k = 0; k < h->K; ++k) {
+            if (n_ck[k] < 0 || n_ck[k] > h->n_c)
+                return fail(XRDVI_E_INVALID_ARG, "half-width of phase " + std::to_string(k) + " outside [0, n_c]");
+            nck[k] = n_ck[k];
+        }
+    if (nck == h->n_ck) return XRDVI_OK;
+    CU(cudaSetDevice(h->device));
+    Tables tabs;
+    if (const char* terr = build_tables(h->plan, h->N, h->K, h->peaks, nck, &tabs)) return fail(XRDVI_E_INVALID_ARG, terr);
+    return install_tables(h, tabs, nck, false);
+}
+
+int xrdvi_get_phase_windows(const xrdvi* h, int32_t* n_ck) {
+    if (!h || !n_ck) return fail(XRDVI_E_INVALID_ARG, "null handle/output");
+    for (int k = 0; k < h->K; ++k) n_ck[k] = static_cast<int32_t>(h->n_ck[k]);
+    return XRDVI_OK;
+}
+
+int xrdvi_adapt_windows(xrdvi* h, double W, int32_t* n_ck_out) {
+    if (!h) return fail(XRDVI_E_INVALID_ARG, "null handle");
+    if (!h->windowed) return fail(XRDVI_E_INVALID_ARG, "per-phase windows need a windowed problem (window_W > 0)");
+    if (!(W > 0.0) || !std::isfinite(W)) return fail(XRDVI_E_INVALID_ARG, "W must be positive");
+    CU(cudaSetDevice(h->device));
+    const int K = h->K, PR = h->plan.PR;
+    std::vector<float> var(static_cast<size_t>(PR) * 8 * K);
+    CU(cudaMemcpyAsync(var.data(), h->dev.var, sizeof(float) * var.size(), cudaMemcpyDeviceToHost, h->stream));
+    CU(cudaStreamSynchronize(h->stream));
+    // the rule, in fp64 on the host from the fp32 state (this is table preprocessing, like create):
+    // cutoff_k = max over instances of W E_q[w_k] + |E_q[mu_k]|, E_q[w] = exp(m_w + sigma_w^2 / 2)
+    const long long n_min = static_cast<long long>(std::ceil(2.0 * W - 1e-9));
+    std::vector<int32_t> nck(K);
+    for (int k = 0; k < K; ++k) {
+        double cut = 0.0;
+        for (int i = 0; i < PR; ++i) {
+            const float* m = var.data() + static_cast<size_t>(i) * 8 * K;
+            const float* l = m + 4 * static_cast<size_t>(K);
+            const double sw = std::exp(static_cast<double>(l[4 * k + 2]));
+            const double ci = W * std::exp(static_cast<double>(m[4 * k + 2]) + 0.5 * sw * sw) +
+                              std::fabs(static_cast<double>(m[4 * k + 1]));
+            if (!std::isfinite(ci)) return fail(XRDVI_E_INVALID_ARG, "non-finite variational state");
+            cut = std::max(cut, ci);
+        }
+        long long n = static_cast<long long>(std::ceil(std::min(cut / h->delta, 4e9) - 1e-9));
+        n = std::min<long long>(std::max(n, n_min), h->n_c);
+        nck[k] = static_cast<int32_t>(n);
+    }
+    int rc = xrdvi_set_phase_windows(h, nck.data());
+    if (rc) return rc;
+    if (n_ck_out) std::memcpy(n_ck_out, nck.data(), sizeof(int32_t) * K);
+    return XRDVI_OK;
+}
+
+int xrdvi_fit_adaptive(xrdvi* h, int32_t iterations, int32_t S, uint64_t seed, int32_t refresh_every, double W,
+                       float* var_out, double* incl, double* trace) {
+    int rc = check_S(h, S);
+    if (rc) return rc;
+    if (iterations < 0 || refresh_every < 1) return fail(XRDVI_E_INVALID_ARG, "iterations >= 0 and refresh_every >= 1 required");
+    if (!h->windowed) return fail(XRDVI_E_INVALID_ARG, "per-phase windows need a windowed problem (window_W > 0)");
+    if (!(W > 0.0) || !std::isfinite(W)) return fail(XRDVI_E_INVALID_ARG, "W must be positive");
+    int done = 0;
+    while (iterations - done > refresh_every) {
+        rc = xrdvi_fit(h, refresh_every, S, seed, nullptr, nullptr,
+                       trace ? trace + static_cast<size_t>(done) * h->plan.PR : nullptr);
+        if (rc) return rc;
+        done += refresh_every;
+        rc = xrdvi_adapt_windows(h, W, nullptr);
+        if (rc) return rc;
+    }
+    return xrdvi_fit(h, iterations - done, S, seed, var_out, incl,
+                     trace ? trace + static_cast<size_t>(done) * h->plan.PR : nullptr);
+}
 
 int xrdvi_reset_state(xrdvi* h, uint64_t seed) {
     if (!h) return fail(XRDVI_E_INVALID_ARG, "null handle");

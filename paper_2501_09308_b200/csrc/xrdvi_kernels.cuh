@@ -55,7 +55,8 @@ struct __align__(16) PeakRec {   // 16 bytes (one LDG.128); one record per (peak
     int dj;        // nearest grid index j_m of the peak minus the first grid index of the tile
     float delta;   // p_m - x_{j_m}  (|delta| <= Delta/2), fp64-computed
     float inten;   // I_m
-    int full;      // 1: all 16 points of the tile exist and lie inside the peak's window
+    int full;      // bit 0: all 16 points of the tile exist and lie inside the peak's window; bits 1..30: the window
+                   // half-width n_c,k of the peak's phase in points (per-phase windows, R27; read by the edge bodies)
 };
 
 struct PatConst {  // per observed pattern
@@ -636,14 +637,14 @@ __device__ __forceinline__ void tile_phase1(const Dev& d, const TileCtx& c, int2
                 const float t0 = fmaf(static_cast<float>(-pk.dj), step, fmaf(-pk.delta, lt.x, lt.y));
                 const float cl = pk.inten * lt.w;
                 const bool core = static_cast<unsigned>(pk.dj + ngc) <= core_span;   // Gaussian core touches the tile
-                if (pk.full) {   // branch-free bodies: Lorentz tail only, or tail + Gaussian on all 16 points
+                if (pk.full & 1) {   // branch-free bodies: Lorentz tail only, or tail + Gaussian on all 16 points
                     if (!core) {
                         fwd_tile2<false>(t0, step, 0.0f, cl, acc2);
                     } else {
                         fwd_tile2<true>(t0, step, 2.0f * pk.inten * lt.z, cl, acc2);
                     }
                 } else {         // window edge: quad by quad
-                    const PeakGeo geo = edge_geo(pk.dj, ngc, d.n_c, c.plim);
+                    const PeakGeo geo = edge_geo(pk.dj, ngc, pk.full >> 1, c.plim);
                     const float cg2 = 2.0f * pk.inten * lt.z;
                     fwd_quad_generic<0>(geo, t0, step, cg2, cl, acc2[0], acc2[1]);
                     fwd_quad_generic<1>(geo, t0, step, cg2, cl, acc2[2], acc2[3]);
@@ -748,7 +749,7 @@ __device__ __forceinline__ void tile_phase2(const Dev& d, const TileCtx& c, int2
             const PeakRec pk = pkt[m];
             const float t0 = fmaf(static_cast<float>(-pk.dj), step, fmaf(-pk.delta, lt.x, lt.y));
             const bool core = static_cast<unsigned>(pk.dj + ngc) <= core_span;
-            if (pk.full && !core) {
+            if ((pk.full & 1) && !core) {
                 Acc6x2 a2 = {0ull, 0ull, 0ull, 0ull, 0ull, 0ull};
                 bwd_tile2<false>(t0, step, e2, pe2, a2);
                 const float a1 = hsum2(a2.a1), a5 = hsum2(a2.a5), a3p = hsum2(a2.a3p);
@@ -757,13 +758,13 @@ __device__ __forceinline__ void tile_phase2(const Dev& d, const TileCtx& c, int2
                 B5 = fmaf(pk.inten, a5, B5);
             } else {
                 Acc6 a = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-                if (pk.full) {
+                if (pk.full & 1) {
                     Acc6x2 a2 = {0ull, 0ull, 0ull, 0ull, 0ull, 0ull};
                     bwd_tile2<true>(t0, step, e2, pe2, a2);
                     a.a1 = hsum2(a2.a1); a.a2 = hsum2(a2.a2); a.a3p = hsum2(a2.a3p);
                     a.a4p = hsum2(a2.a4p); a.a5 = hsum2(a2.a5); a.a6u = hsum2(a2.a6u);
                 } else {
-                    const PeakGeo geo = edge_geo(pk.dj, ngc, d.n_c, c.plim);
+                    const PeakGeo geo = edge_geo(pk.dj, ngc, pk.full >> 1, c.plim);
                     bwd_quad_generic<0>(geo, t0, step, e2[0], e2[1], pe2[0], pe2[1], a);
                     bwd_quad_generic<1>(geo, t0, step, e2[2], e2[3], pe2[2], pe2[3], a);
                     bwd_quad_generic<2>(geo, t0, step, e2[4], e2[5], pe2[4], pe2[5], a);
