@@ -152,3 +152,45 @@ def test_window_error_paths():
         dense.set_phase_windows(np.ones(6, dtype=np.int32))
     with pytest.raises(XrdviError):
         dense.adapt_windows(5.0)
+
+
+# --------------------------------------------------------------------------- full sizes, bench launch configuration
+def test_config1_full_size_adaptive_fit_and_evaluation():
+    """K=50, S=256 (the headline launch shape): 300 steps with a refresh every 100, then everything (ll of every
+    draw, profiles, ELBO, gradient) under the windows left in force, and the inclusion probabilities of the
+    oracle's own adaptive fit with the same draws."""
+    wl = synth.make_workload(1)
+    o, gpu = orc.from_workload(wl), Xrdvi.from_workload(wl)
+    st_g, inc_g, _ = gpu.fit_adaptive(300, refresh_every=100, W=10.0, seed=1)
+    n_g = gpu.get_phase_windows()
+    assert n_g.min() >= 20 and n_g.max() <= 75 and gpu.pair_count < 0.9 * 629906
+    st_r, hist = o.fit_adaptive(o.init_state(0), 300, wl.S, seed=1, refresh_every=100, W=10.0)
+    assert np.abs(n_g.astype(np.int64) - hist[-1]).max() <= 1
+    assert np.abs(inc_g - o.inclusion(st_r)).max() <= TOL_INCL
+    o.set_phase_windows(n_g)
+    assert gpu.pair_count == o.pair_count()
+    elbo_r, grad_r, ll_r = o.elbo_grad(st_g.astype(np.float64), wl.S, 1, 301, want_ll=True)
+    _, ll_g = gpu.debug_profile(wl.S, state=st_g, S=wl.S, seed=1, iteration=301, want_f=False)
+    np.testing.assert_allclose(ll_g, ll_r.reshape(-1), rtol=1e-4)
+    check_eval(gpu, o, st_g, wl.S, seed=1, iteration=301, n_prof=3)
+
+
+def test_config4_full_size_adapted_windows_sampled_draws():
+    """K=1000, N=8001, S=256, +-400-point cap: windows adapted after 3 steps (W = 20: 111..400 points); ll of sampled
+    draws one by one with the oracle under the same half-widths, pair counts equal."""
+    from test_gpu_fullsize import ll_one_draw
+    wl = synth.make_workload(4)
+    o, gpu = orc.from_workload(wl), Xrdvi.from_workload(wl)
+    gpu.fit(3, seed=6)
+    n_g = gpu.adapt_windows(20.0)
+    st, _ = gpu.get_state()
+    st64 = st.astype(np.float64)
+    assert np.array_equal(n_g, o.adaptive_halfwidths(st64, 20.0))
+    o.set_phase_windows(n_g)
+    assert gpu.pair_count == o.pair_count() < 137387988
+    _, ll_g = gpu.debug_profile(wl.S, state=st, S=wl.S, seed=6, iteration=7, want_f=False)
+    assert np.isfinite(ll_g).all()
+    for s in (0, 31, 32, 131, 255):
+        assert ll_g[s] == pytest.approx(ll_one_draw(o, st64, 6, 7, 0, s), rel=1e-4)
+    e, g = gpu.elbo_grad(state=st, S=wl.S, seed=6, iteration=7)
+    assert np.isfinite(e).all() and np.isfinite(g).all()
