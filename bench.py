@@ -92,7 +92,7 @@ def measured_peaks() -> dict:
 
 def measured_traffic(kernel: str, cfg: int):
     """DRAM bytes per launch of `kernel` from the committed ncu capture (profiles/), or None."""
-    p = ROOT / "profiles" / "r1_v4_traffic.txt"
+    p = ROOT / "profiles" / "r1_v5_traffic.txt"
     if not p.exists():
         return None
     for ln in p.read_text().splitlines():
@@ -237,7 +237,7 @@ def run_ours(args, rank: int, local_rank: int, world: int) -> None:
     roofline = {
         "bound": "alu", "kernel": "elbo_tile_kernel", "achieved": achieved / 1e9, "peak": r_plain / 1e9,
         "unit": "Gpair/s", "frac": achieved / r_plain, "traffic": measured_traffic("elbo_tile_kernel", args.config),
-        "traffic_source": "profiles/r1_v4_traffic.txt (ncu --set full, dram read + write bytes per launch)",
+        "traffic_source": "profiles/r1_v5_traffic.txt (ncu --set full, dram read + write bytes per launch)",
         "peak_source": f"derived: {n_sm} SMs x {f_max / 1e6:.0f} MHz (MEASURED_PEAKS sm_max_mhz) x 16 MUFU lanes / "
                        f"4 MUFU per pair (plain forward+backward formulation, DESIGN.md Roofline)",
         "ms_tile": tk["ms_tile"], "ms_tile_forward_only": tk["ms_tile_forward_only"], "ms_update": tk["ms_update"],
