@@ -89,6 +89,7 @@ bool make_plan(int64_t N, int32_t K, int64_t M, int32_t S_max, double step, cons
     p.SP = kPT * p.TW;
     p.n_seg = static_cast<int>((N + p.SP - 1) / p.SP);
     p.n_tile = static_cast<int>((N + kPT - 1) / kPT);
+    if (p.n_seg > 65535) return false;                  // grid.y limit of elbo_tile_kernel
     p.n_c = window_points(hyp, step);
     // entries of the per-tile phase-major lists: a peak appears once per 16-point tile its window touches
     const long long per_peak = p.n_c < 0 ? p.n_tile : std::min<long long>(p.n_tile, (2 * p.n_c + kPT) / kPT + 1);
@@ -363,7 +364,7 @@ void launch_tile(const Dev& d, cudaStream_t st, float* f_dbg, long long n_dbg, b
         }
         return;
     }
-    const dim3 grid(d.n_seg, d.G);
+    const dim3 grid(d.G, d.n_seg);   // x = draw group (dispatched fastest), y = position in seg_order
 #define XRDVI_TILE_CASE(TW_, PS_)                                                                                \
     case TW_ * 16 + PS_:                                                                                        \
         launch_k(elbo_tile_kernel<TW_, PS_, BWD>, grid, dim3(32 * TW_ * PS_), st, pdl, d, f_dbg, n_dbg);         \
