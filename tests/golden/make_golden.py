@@ -15,6 +15,9 @@ from oracle import xrdvi_oracle as orc            # noqa: E402
 from paper_2501_09308_b200 import synth           # noqa: E402  (inputs only)
 
 
+PHASE_WINDOWS = (22, 9, 15, 4, 22, 11)     # per-phase half-widths of the "gauss_windows" case (R27)
+
+
 def cases():
     wl = synth.make_workload(0)
     o = orc.from_workload(wl)
@@ -27,6 +30,9 @@ def cases():
     yield "gauss_init", o, f32(st0), wl.S, 3, 1
     yield "gauss_rand", o, f32(st1), wl.S, 3, 7
     yield "poisson_init", op, f32(op.init_state()), wlp.S, 5, 2
+    ow = orc.from_workload(wl)
+    ow.set_phase_windows(PHASE_WINDOWS)
+    yield "gauss_windows", ow, f32(st1), wl.S, 9, 4
 
 
 def main():
