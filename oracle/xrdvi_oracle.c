@@ -23,6 +23,8 @@
  *   optimiser Adam ascent, "1000 optimization steps" PAPER.md:138 (R10); hyper.optimizer = 1:
  *             natural-gradient ascent (R25; north_star names both)
  *   inclusion closed form from (m, l), 1 % area threshold PAPER.md:140 (R15)
+ *   summary   marginals of q in the constrained parameters (mean, sd, 2.5/50/97.5 % quantiles; reading R28,
+ *             the Fig. 6 marginals, SURVEY 8(f) NEXT-4 second half); pins: tests/test_posterior_summary_pins.py
  *   draws     Philox4x32-10, counter (iter, s, k, inst), key (seed_lo, seed_hi) (R18)
  *   adaptive  per-phase window half-widths n_c,k <= n_c refreshed from the variational means
  *             (reading R27; north_star's "problem-defined +-W FWHM cutoff")
@@ -535,6 +537,63 @@ void orc_inclusion(const orc_problem *q, const double *state, double *incl /*[P]
             incl[(size_t)inst * K + k] = normal_cdf((m[4 * k] - log(q->hy.incl_tau * Tbar / A)) / s);
             if (area_ratio) area_ratio[(size_t)inst * K + k] = A * exp(m[4 * k] + 0.5 * s * s) / Tbar;
         }
+    }
+}
+
+/* ------------------------------------------------------------------ marginal summaries (R28)
+ * Marginals of the fitted q (eq.(10), the posterior marginals the paper plots in Fig. 6) in the
+ * constrained parameters of R6: zeta ~ N(m, s^2), s = exp(l);
+ *   h = exp(zeta_h), w = exp(zeta_w): log-normal; mu = zeta_mu: normal; r = sigmoid(zeta_r): logit-normal.
+ * out [P][R][K][4][5] = (mean, sd, 2.5 %, 50 %, 97.5 % quantile) per class (h, mu, w, r).
+ * Quantiles: g(m + s z_p) for the monotone map g, z_p found by bisection on the normal cdf.
+ * Mean / sd: closed forms for the (log-)normal; for r the integrals E[r^j] = int sigmoid(m + s z)^j phi(z) dz
+ * by composite Simpson, 48001 points on z in [-12, 12] (no closed form exists).                               */
+static double normal_quantile_bisect(double p) {
+    double lo = -40.0, hi = 40.0;
+    for (int it = 0; it < 200; ++it) {
+        double mid = 0.5 * (lo + hi);
+        if (normal_cdf(mid) < p) lo = mid; else hi = mid;
+    }
+    return 0.5 * (lo + hi);
+}
+
+static double sigmoid_d(double x) { return 1.0 / (1.0 + exp(-x)); }
+
+void orc_posterior_summary(const orc_problem *q, const double *state, double *out /*[P][R][K][4][5]*/) {
+    const int32_t K = q->K;
+    const double zq[3] = {normal_quantile_bisect(0.025), 0.0, normal_quantile_bisect(0.975)};
+    const int nint = 48000;                      /* Simpson intervals (even) */
+    const double za = -12.0, zb = 12.0, dz = (zb - za) / nint;
+    for (int32_t inst = 0; inst < q->P * q->R; ++inst) {
+        const double *m = state + (size_t)inst * 2 * K * 4, *l = m + (size_t)K * 4;
+        for (int32_t k = 0; k < K; ++k)
+            for (int c = 0; c < 4; ++c) {
+                const double mm = m[4 * k + c], s = exp(l[4 * k + c]);
+                double *o = out + (((size_t)inst * K + k) * 4 + c) * 5;
+                if (c == 0 || c == 2) {          /* log-normal */
+                    o[0] = exp(mm + 0.5 * s * s);
+                    o[1] = sqrt(expm1(s * s)) * exp(mm + 0.5 * s * s);
+                    for (int j = 0; j < 3; ++j) o[2 + j] = exp(mm + s * zq[j]);
+                } else if (c == 1) {             /* normal */
+                    o[0] = mm;
+                    o[1] = s;
+                    for (int j = 0; j < 3; ++j) o[2 + j] = mm + s * zq[j];
+                } else {                         /* logit-normal */
+                    double e1 = 0.0, e2 = 0.0;
+                    for (int i = 0; i <= nint; ++i) {
+                        const double z = za + dz * i;
+                        const double wgt = (i == 0 || i == nint) ? 1.0 : ((i & 1) ? 4.0 : 2.0);
+                        const double phi = exp(-0.5 * z * z) / sqrt(2.0 * M_PI);
+                        const double r = sigmoid_d(mm + s * z);
+                        e1 += wgt * r * phi;
+                        e2 += wgt * r * r * phi;
+                    }
+                    e1 *= dz / 3.0; e2 *= dz / 3.0;
+                    o[0] = e1;
+                    o[1] = sqrt(fmax(e2 - e1 * e1, 0.0));
+                    for (int j = 0; j < 3; ++j) o[2 + j] = sigmoid_d(mm + s * zq[j]);
+                }
+            }
     }
 }
 

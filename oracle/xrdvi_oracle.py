@@ -80,6 +80,7 @@ def lib():
         L.orc_init_state.argtypes = [C.c_void_p, C.c_uint64, dp]
         L.orc_fit.argtypes = [C.c_void_p, dp, dp, dp, C.c_int32, C.c_int32, C.c_uint64, C.c_int64, dp]
         L.orc_inclusion.argtypes = [C.c_void_p, dp, dp, dp]
+        L.orc_posterior_summary.argtypes = [C.c_void_p, dp, dp]
         L.orc_set_phase_windows.restype = C.c_int
         L.orc_set_phase_windows.argtypes = [C.c_void_p, C.POINTER(C.c_int64)]
         L.orc_adaptive_halfwidths.argtypes = [C.c_void_p, dp, C.c_double, C.POINTER(C.c_int64)]
@@ -295,6 +296,13 @@ class Oracle:
         ar = np.empty_like(inc) if want_area else None
         lib().orc_inclusion(self._h, _dp(st), _dp(inc), _dp(ar))
         return (inc, ar) if want_area else inc
+
+    def posterior_summary(self, state):
+        """Marginals of q in (h, mu, w, r): [P][R][K][4][5] = (mean, sd, q2.5, q50, q97.5) (reading R28)."""
+        st = self._state(state)
+        out = np.empty((self.P, self.R, self.K, 4, 5), dtype=np.float64)
+        lib().orc_posterior_summary(self._h, _dp(st), _dp(out))
+        return out
 
 
 def from_workload(wl, **overrides):
