@@ -546,8 +546,8 @@ void orc_inclusion(const orc_problem *q, const double *state, double *incl /*[P]
  *   h = exp(zeta_h), w = exp(zeta_w): log-normal; mu = zeta_mu: normal; r = sigmoid(zeta_r): logit-normal.
  * out [P][R][K][4][5] = (mean, sd, 2.5 %, 50 %, 97.5 % quantile) per class (h, mu, w, r).
  * Quantiles: g(m + s z_p) for the monotone map g, z_p found by bisection on the normal cdf.
- * Mean / sd: closed forms for the (log-)normal; for r the integrals E[r^j] = int sigmoid(m + s z)^j phi(z) dz
- * by composite Simpson, 48001 points on z in [-12, 12] (no closed form exists).                               */
+ * Mean / sd: closed forms for the (log-)normal; for r the integrals E[r] = int sigmoid(m + s z) phi(z) dz and
+ * Var[r] = int (sigmoid(m + s z) - E[r])^2 phi(z) dz by composite Simpson, 48001 points on z in [-12, 12] (no closed form exists).                               */
 static double normal_quantile_bisect(double p) {
     double lo = -40.0, hi = 40.0;
     for (int it = 0; it < 200; ++it) {
@@ -579,18 +579,20 @@ void orc_posterior_summary(const orc_problem *q, const double *state, double *ou
                     o[1] = s;
                     for (int j = 0; j < 3; ++j) o[2 + j] = mm + s * zq[j];
                 } else {                         /* logit-normal */
-                    double e1 = 0.0, e2 = 0.0;
-                    for (int i = 0; i <= nint; ++i) {
-                        const double z = za + dz * i;
-                        const double wgt = (i == 0 || i == nint) ? 1.0 : ((i & 1) ? 4.0 : 2.0);
-                        const double phi = exp(-0.5 * z * z) / sqrt(2.0 * M_PI);
-                        const double r = sigmoid_d(mm + s * z);
-                        e1 += wgt * r * phi;
-                        e2 += wgt * r * r * phi;
+                    double e1 = 0.0, e2 = 0.0;   /* E[r], then E[(r - E r)^2]: two passes, the definitions */
+                    for (int pass = 0; pass < 2; ++pass) {
+                        double acc = 0.0;
+                        for (int i = 0; i <= nint; ++i) {
+                            const double z = za + dz * i;
+                            const double wgt = (i == 0 || i == nint) ? 1.0 : ((i & 1) ? 4.0 : 2.0);
+                            const double phi = exp(-0.5 * z * z) / sqrt(2.0 * M_PI);
+                            const double r = sigmoid_d(mm + s * z);
+                            acc += wgt * (pass == 0 ? r : (r - e1) * (r - e1)) * phi;
+                        }
+                        if (pass == 0) e1 = acc * dz / 3.0; else e2 = acc * dz / 3.0;
                     }
-                    e1 *= dz / 3.0; e2 *= dz / 3.0;
                     o[0] = e1;
-                    o[1] = sqrt(fmax(e2 - e1 * e1, 0.0));
+                    o[1] = sqrt(e2);
                     for (int j = 0; j < 3; ++j) o[2 + j] = sigmoid_d(mm + s * zq[j]);
                 }
             }

@@ -64,6 +64,12 @@ def test_symmetry_small_sigma_limit_and_ordering(case):
     g = special.expit(m)
     assert out[0, 3, 0] == pytest.approx(g + 0.5 * 0.02 ** 2 * g * (1 - g) * (1 - 2 * g), abs=1e-8)
     assert out[0, 3, 1] == pytest.approx(0.02 * g * (1 - g), rel=2e-3)
+    tiny = st.copy()                                                 # sigma = e^-12 (the clamp of R10): no cancellation
+    tiny[0, 0, 1, :, 3] = -12.0
+    t = o.posterior_summary(tiny)[0, 0]
+    gk = special.expit(tiny[0, 0, 0, :, 3])
+    assert t[:, 3, 1] == pytest.approx(np.exp(-12.0) * gk * (1 - gk), rel=1e-6)
+    assert t[:, 3, 0] == pytest.approx(gk, abs=1e-11)
     assert np.all(out[..., 2] < out[..., 3]) and np.all(out[..., 3] < out[..., 4])
     assert np.all(out[..., 1] > 0)
     assert np.all(out[:, 3, 2:] > 0) and np.all(out[:, 3, 2:] < 1) and np.all(out[:, 3, 0] < 1)
