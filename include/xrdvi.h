@@ -166,6 +166,14 @@ int xrdvi_fit(xrdvi* h, int32_t iterations, int32_t S, uint64_t seed, float* var
  * incl_prob, area_ratio double [P][R][K], either may be NULL.                                      */
 int xrdvi_inclusion(xrdvi* h, double* incl_prob, double* area_ratio);
 
+/* Marginal summaries of the fitted q in the constrained parameters (R28; the posterior marginals of the
+ * paper's Fig. 6, SURVEY.md 8(f) NEXT-4 second half), from the internal state, computed on the device in fp64:
+ * zeta ~ N(m, sigma^2) (eq.(10)) pushed through the bijections of R6 -- h, w log-normal, mu normal,
+ * r logit-normal (mean / sd by quadrature).
+ *  summary  host double [P][R][K][4][5], classes (h, mu, w, r) x (mean, sd, 2.5 %, 50 %, 97.5 % quantile); owned by
+ *           the caller, must not be NULL (XRDVI_E_INVALID_ARG).  Synchronous on the handle's stream.          */
+int xrdvi_posterior_summary(xrdvi* h, double* summary);
+
 /* Log-joint gradient service: log p(Y, Phi) + log |dPhi/dzeta| and its gradient at n
  * caller-supplied points of the unconstrained latent space, for one pattern -- what a gradient-based sampler of the
  * paper's model (the MCMC rows of Table 1) evaluates per leapfrog step.  The same

@@ -18,7 +18,7 @@ EXPORTS = (
     "xrdvi_default_hyper", "xrdvi_workspace_bytes", "xrdvi_create", "xrdvi_destroy", "xrdvi_pair_count",
     "xrdvi_window_halfwidth", "xrdvi_set_phase_windows", "xrdvi_get_phase_windows", "xrdvi_adapt_windows",
     "xrdvi_fit_adaptive", "xrdvi_reset_state", "xrdvi_get_state", "xrdvi_set_state", "xrdvi_elbo_grad",
-    "xrdvi_fit", "xrdvi_inclusion", "xrdvi_logjoint_grad", "xrdvi_debug_profile", "xrdvi_debug_draws", "xrdvi_time_kernels",
+    "xrdvi_fit", "xrdvi_inclusion", "xrdvi_posterior_summary", "xrdvi_logjoint_grad", "xrdvi_debug_profile", "xrdvi_debug_draws", "xrdvi_time_kernels",
     "xrdvi_bench_steps", "xrdvi_debug_timeline", "xrdvi_pipe_rates", "xrdvi_last_error",
 )
 
@@ -77,6 +77,7 @@ def load_library():
     L.xrdvi_elbo_grad.argtypes = [vp, fp, C.c_int32, C.c_uint64, C.c_uint64, dp, fp]
     L.xrdvi_fit.argtypes = [vp, C.c_int32, C.c_int32, C.c_uint64, fp, dp, dp]
     L.xrdvi_inclusion.argtypes = [vp, dp, dp]
+    L.xrdvi_posterior_summary.argtypes = [vp, dp]
     L.xrdvi_logjoint_grad.argtypes = [vp, fp, C.c_int64, C.c_int32, dp, dp, fp]
     L.xrdvi_debug_profile.argtypes = [vp, fp, C.c_int32, C.c_uint64, C.c_uint64, C.c_int64, fp, dp]
     L.xrdvi_debug_draws.argtypes = [vp, C.c_int32, C.c_uint64, C.c_uint64, C.c_int64, fp, C.POINTER(C.c_uint32),
@@ -258,6 +259,11 @@ class Xrdvi:
         ar = np.empty_like(inc)
         _check(load_library().xrdvi_inclusion(self._h, _d(inc), _d(ar)))
         return inc, ar
+
+    def posterior_summary(self):
+        out = np.empty((self.P, self.R, self.K, 4, 5), dtype=np.float64)
+        _check(load_library().xrdvi_posterior_summary(self._h, _d(out)))
+        return out
 
     # ---- debug / measurement ---------------------------------------------------
     def debug_profile(self, n, state=None, S=None, seed=0, iteration=0, want_f=True):

@@ -42,7 +42,7 @@ struct Plan {   // workspace carve; identical arithmetic in workspace_bytes and 
     size_t o_yb, o_bg, o_pkt, o_runs, o_srng, o_sord, o_sofs, o_pat, o_area, o_mh0;
     size_t o_var, o_vartmp, o_mom1, o_mom2, o_grad, o_elbo, o_elbok, o_llt, o_trace, o_ctl;
     size_t o_lat, o_eps, o_rr, o_ng, o_llpart, o_part8, o_dbg;
-    size_t o_pd, o_lpk, o_zeta, o_gradz, o_lls, o_partial, o_tcnt;
+    size_t o_pd, o_lpk, o_zeta, o_gradz, o_lls, o_partial, o_tcnt, o_summ;
     int pd_groups;     // groups one launch of the log-joint gradient service handles
 };
 
@@ -63,7 +63,7 @@ void choose_shape(int64_t N, int G_max, int* TW, int* PS) {
             return;
         }
     }
-    // measured on B200 (profiles/r1_v3_shape_sweep.md): one tile per CTA is best everywhere; few tile-warps
+    // measured on B200 (profiles/r1_v5_shape_sweep.md): one tile per CTA is best everywhere; few tile-warps
     // (configs 1 and 4: 2008 / 4008) want the peak lists split four ways, many (configs 2, 3: 1e6) no split
     const long long tiles = (N + 15) / 16 * static_cast<long long>(G_max);   // warps at PS = 1
     const long long resident = 148ll * 24;                                    // warps the GPU holds at 80 registers
@@ -127,6 +127,7 @@ bool make_plan(int64_t N, int32_t K, int64_t M, int32_t S_max, double step, cons
     p.o_llpart = take(sizeof(float) * static_cast<size_t>(p.G_max) * p.n_seg * 32);
     p.o_part8 = take(sizeof(float) * static_cast<size_t>(p.G_max) * std::max<long long>(p.slots_cap, 1) * 8);
     p.o_dbg = take(sizeof(double) * (2 * static_cast<size_t>(p.PR) * K + 64));
+    p.o_summ = take(sizeof(double) * 20 * static_cast<size_t>(p.PR) * K);   // marginal summaries (R28)
     // log-joint gradient service: per-draw partials of at most 64 MiB worth of groups (at least one)
     const size_t pd_group_bytes = sizeof(float) * 128 * static_cast<size_t>(std::max<long long>(p.slots_cap, 1));
     p.pd_groups = static_cast<int>(std::min<size_t>(p.gpi_max, std::max<size_t>(1, (size_t(64) << 20) / pd_group_bytes)));
@@ -930,6 +931,19 @@ int xrdvi_inclusion(xrdvi* h, double* incl, double* ratio) {
     CU(cudaStreamSynchronize(h->stream));
     if (incl) std::memcpy(incl, buf.data(), sizeof(double) * n);
     if (ratio) std::memcpy(ratio, buf.data() + n, sizeof(double) * n);
+    return XRDVI_OK;
+}
+
+int xrdvi_posterior_summary(xrdvi* h, double* summary) {
+    if (!h) return fail(XRDVI_E_INVALID_ARG, "null handle");
+    if (!summary) return fail(XRDVI_E_INVALID_ARG, "summary is NULL");
+    CU(cudaSetDevice(h->device));
+    const size_t n = 20 * static_cast<size_t>(h->plan.PR) * h->K;
+    double* dev = reinterpret_cast<double*>(h->ws + h->plan.o_summ);
+    posterior_summary_kernel<<<dim3((4 * h->K + 127) / 128, h->plan.PR), 128, 0, h->stream>>>(h->dev, dev);
+    CU(cudaGetLastError());
+    CU(cudaMemcpyAsync(summary, dev, sizeof(double) * n, cudaMemcpyDeviceToHost, h->stream));
+    CU(cudaStreamSynchronize(h->stream));
     return XRDVI_OK;
 }
 

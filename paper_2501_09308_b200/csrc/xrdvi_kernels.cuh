@@ -1161,6 +1161,41 @@ __global__ void __launch_bounds__(128) inclusion_kernel(const Dev d, double tau,
     }
 }
 
+// Marginal summaries of q in the constrained parameters (R28; the paper's Fig. 6 marginals), fp64.
+// grid (ceil(4K / 128), PR), block 128: one thread per (phase, class).  out [PR][K][4][5] = mean, sd, 2.5 %, 50 %,
+// 97.5 % quantile.  h, w log-normal, mu normal (closed forms); r logit-normal: trapezoid rule on z in [-10, 10],
+// step 1/32, of (r - r0) and (r - r0)^2 against the normal density, r0 = sigmoid(m) (centred, so a narrow q does not
+// cancel).  The integrand is analytic in |Im z| < pi / sigma >= 0.42 (sigma <= e^2, R10): trapezoid error ~ e^-85.
+__global__ void __launch_bounds__(128) posterior_summary_kernel(const Dev d, double* __restrict__ out) {
+    const int idx = blockIdx.x * 128 + threadIdx.x;
+    if (idx >= 4 * d.K) return;
+    const int inst = blockIdx.y, c = idx & 3;
+    const float* mp = d.var + static_cast<size_t>(inst) * 8 * d.K;
+    const double m = static_cast<double>(mp[idx]);
+    const double s = exp(static_cast<double>(mp[4 * d.K + idx]));
+    const double z975 = 1.95996398454005423552;
+    double* o = out + (static_cast<size_t>(inst) * 4 * d.K + idx) * 5;
+    if (c == 1) {
+        o[0] = m; o[1] = s; o[2] = m - s * z975; o[3] = m; o[4] = m + s * z975;
+    } else if (c != 3) {
+        const double mean = exp(m + 0.5 * s * s);
+        o[0] = mean; o[1] = sqrt(expm1(s * s)) * mean;
+        o[2] = exp(m - s * z975); o[3] = exp(m); o[4] = exp(m + s * z975);
+    } else {
+        const double r0 = 1.0 / (1.0 + exp(-m));
+        double a0 = 0.0, a1 = 0.0, a2 = 0.0;
+        for (int i = -320; i <= 320; ++i) {
+            const double z = i * 0.03125;
+            const double ph = ((i == -320 || i == 320) ? 0.5 : 1.0) * exp(-0.5 * z * z);
+            const double dr = 1.0 / (1.0 + exp(-(m + s * z))) - r0;
+            a0 += ph; a1 += ph * dr; a2 += ph * dr * dr;
+        }
+        const double e1 = a1 / a0, e2 = a2 / a0;
+        o[0] = r0 + e1; o[1] = sqrt(fmax(e2 - e1 * e1, 0.0));
+        o[2] = 1.0 / (1.0 + exp(-(m - s * z975))); o[3] = r0; o[4] = 1.0 / (1.0 + exp(-(m + s * z975)));
+    }
+}
+
 // R11 initial state.  grid PR, block 128 over phases.
 __global__ void __launch_bounds__(128) init_state_kernel(const Dev d, const float* __restrict__ m_h0 /*[P]*/,
                                                          float m_w0, float init_log_sigma, unsigned long long seed) {
