@@ -58,7 +58,7 @@ long long window_points(const xrdvi_hyper* hyp, double step) {
 void choose_shape(int64_t N, int G_max, int* TW, int* PS) {
     if (const char* e = std::getenv("XRDVI_TILE_SHAPE")) {   // tuning knob for sweeps: "TWxPS"
         int a = 0, b = 0;
-        if (std::sscanf(e, "%dx%d", &a, &b) == 2 && (a == 1 || a == 2 || a == 4) && (b == 1 || b == 2 || b == 3 || b == 4 || b == 8) && a * b <= 16) {
+        if (std::sscanf(e, "%dx%d", &a, &b) == 2 && (a == 1 || a == 2 || a == 4) && (b == 1 || b == 2 || b == 3 || b == 4 || b == 5 || b == 6 || b == 8) && a * b <= 16) {
             *TW = a; *PS = b;
             return;
         }
@@ -360,6 +360,8 @@ void launch_tile(const Dev& d, cudaStream_t st, float* f_dbg, long long n_dbg, b
             case 3: launch_k(elbo_split_kernel<3, BWD>, dim3(grid), dim3(32), st, pdl, d, f_dbg, n_dbg); break;
             case 2: launch_k(elbo_split_kernel<2, BWD>, dim3(grid), dim3(32), st, pdl, d, f_dbg, n_dbg); break;
             case 4: launch_k(elbo_split_kernel<4, BWD>, dim3(grid), dim3(32), st, pdl, d, f_dbg, n_dbg); break;
+            case 5: launch_k(elbo_split_kernel<5, BWD>, dim3(grid), dim3(32), st, pdl, d, f_dbg, n_dbg); break;
+            case 6: launch_k(elbo_split_kernel<6, BWD>, dim3(grid), dim3(32), st, pdl, d, f_dbg, n_dbg); break;
             case 8: launch_k(elbo_split_kernel<8, BWD>, dim3(grid), dim3(32), st, pdl, d, f_dbg, n_dbg); break;
             default: break;
         }
@@ -371,7 +373,7 @@ void launch_tile(const Dev& d, cudaStream_t st, float* f_dbg, long long n_dbg, b
         launch_k(elbo_tile_kernel<TW_, PS_, BWD>, grid, dim3(32 * TW_ * PS_), st, pdl, d, f_dbg, n_dbg);         \
         break;
     switch (d.TW * 16 + d.PS) {
-        XRDVI_TILE_CASE(1, 1) XRDVI_TILE_CASE(1, 2) XRDVI_TILE_CASE(1, 3) XRDVI_TILE_CASE(1, 4) XRDVI_TILE_CASE(1, 8)
+        XRDVI_TILE_CASE(1, 1) XRDVI_TILE_CASE(1, 2) XRDVI_TILE_CASE(1, 3) XRDVI_TILE_CASE(1, 4) XRDVI_TILE_CASE(1, 5) XRDVI_TILE_CASE(1, 6) XRDVI_TILE_CASE(1, 8)
         XRDVI_TILE_CASE(2, 1) XRDVI_TILE_CASE(2, 2) XRDVI_TILE_CASE(2, 4) XRDVI_TILE_CASE(2, 8)
         XRDVI_TILE_CASE(4, 1) XRDVI_TILE_CASE(4, 2) XRDVI_TILE_CASE(4, 4)
         default: break;
