@@ -942,7 +942,7 @@ int xrdvi_posterior_summary(xrdvi* h, double* summary) {
     CU(cudaSetDevice(h->device));
     const size_t n = 20 * static_cast<size_t>(h->plan.PR) * h->K;
     double* dev = reinterpret_cast<double*>(h->ws + h->plan.o_summ);
-    posterior_summary_kernel<<<dim3((4 * h->K + 127) / 128, h->plan.PR), 128, 0, h->stream>>>(h->dev, dev);
+    posterior_summary_kernel<<<dim3((h->K + 3) / 4, h->plan.PR), 128, 0, h->stream>>>(h->dev, dev);
     CU(cudaGetLastError());
     CU(cudaMemcpyAsync(summary, dev, sizeof(double) * n, cudaMemcpyDeviceToHost, h->stream));
     CU(cudaStreamSynchronize(h->stream));
