@@ -95,13 +95,18 @@ _SPEC = {
 
 def make_workload(cfg: int, n_patterns: int | None = None, n_restarts: int | None = None,
                   S: int | None = None, K: int | None = None, seed: int | None = None,
-                  peak_counts: float | None = None) -> Workload:
+                  peak_counts: float | None = None, grid: tuple | None = None,
+                  noise_frac: float = 0.01) -> Workload:
     """Build config ``cfg`` (0..4).  Optional overrides shrink a config for tests
     (e.g. ``n_patterns=4`` for cfg 3) without changing its per-pattern recipe.
 
     ``peak_counts``: COUNT data for the paper's Poisson likelihood: signal + background
     are scaled so that their maximum is ``peak_counts`` and y ~ Poisson(signal + background) replaces the
-    Gaussian noise; the planted scales h are multiplied by the same factor and ``hyper['likelihood'] = 1``."""
+    Gaussian noise; the planted scales h are multiplied by the same factor and ``hyper['likelihood'] = 1``.
+
+    ``grid = (lo, hi, N)`` replaces the config's 2theta range and point count (same recipe otherwise), e.g. config 0
+    on a 0.02 deg grid that resolves its peaks: ``grid=(10.0, 80.0, 3501)``.  ``noise_frac``: Gaussian noise sigma as a
+    fraction of the maximum signal (the configs' 1 %)."""
     if cfg not in _SPEC:
         raise ValueError(f"unknown config {cfg}")
     (K0, (mlo, mhi), N, lo, hi, P0, R0, S0, its, W, fwhm_ref, (fw_lo, fw_hi), (w_shape, w_rate)) = _SPEC[cfg]
@@ -109,6 +114,8 @@ def make_workload(cfg: int, n_patterns: int | None = None, n_restarts: int | Non
     P = P0 if n_patterns is None else int(n_patterns)
     R = R0 if n_restarts is None else int(n_restarts)
     S = S0 if S is None else int(S)
+    if grid is not None:
+        lo, hi, N = float(grid[0]), float(grid[1]), int(grid[2])
     rng = np.random.default_rng((1000 + cfg) if seed is None else seed)
 
     x = lo + (hi - lo) * np.arange(N, dtype=np.float64) / (N - 1)
@@ -170,7 +177,7 @@ def make_workload(cfg: int, n_patterns: int | None = None, n_restarts: int | Non
         b0 = 0.02 * smax
         b1 = rng.uniform(-0.5, 0.5) * b0 / (hi - lo)
         bg[pat] = b0 + b1 * (x - lo)
-        sigma_n = 0.01 * smax
+        sigma_n = float(noise_frac) * smax
         if peak_counts is None:
             y[pat] = sig + bg[pat] + rng.normal(0.0, sigma_n, size=N)
         else:

@@ -14,9 +14,12 @@ subsets.  This is independent of the variational machinery (no q, no ELBO, no Ad
 oracle's per-phase unit profile, which test_oracle_pins.py pins against scipy pdfs.
 
 Criterion: the maximum-evidence subset equals {k : P_incl(k) > 1/2} and equals the planted
-set; every phase falls on the same side of 1/2 under both; max |difference| is reported.  The Occam factor
-makes exact inclusion of absent phases small but not zero (SURVEY probe: 0.004-0.14).
+set; every phase falls on the same side of 1/2 under both; max |difference| is bounded.  The Occam factor
+makes exact inclusion of absent phases small but not zero (measured here: 0.002-0.18).  The criterion is asserted on
+P_incl itself (the R15 read-out at incl_tau = 1 %) for a converged fit on a grid that resolves the peaks; what happens
+on config 0's own undersampled grid and after its own 500 iterations is DESIGN.md reading R29 and is asserted too.
 """
+import functools
 import itertools
 import math
 
@@ -60,20 +63,27 @@ def log_evidence(C, resid, sigma_n, lam):
     return g * math.log(lam) + 0.5 * g * math.log(2 * math.pi) - 0.5 * logdet + 0.5 * b @ hhat + math.log(max(orth, 1e-300))
 
 
-@pytest.mark.parametrize("seed", [1000, 2024])
-def test_variational_inclusion_against_all_64_subsets(seed):
-    wl = synth.make_workload(0, seed=seed)
+RESOLVED_GRID = (10.0, 80.0, 3501)      # config-0 recipe on a 0.02 deg grid that resolves the 0.05-0.15 deg peaks
+ITS_CONVERGED = 2000                     # absent-phase scales decay slowly under Adam (R29)
+
+
+@functools.lru_cache(maxsize=None)
+def fitted(seed, resolved, its):
+    wl = synth.make_workload(0, seed=seed, grid=RESOLVED_GRID if resolved else None)
     o = orc.from_workload(wl)
     assert o.K == 6
-    st, _, _ = o.fit(o.init_state(), 500, wl.S, seed=11)
-    inc_vi, area = o.inclusion(st, want_area=True)
-    inc_vi, area = inc_vi[0, 0], area[0, 0]
+    st, _, _ = o.fit(o.init_state(), its, wl.S, seed=11)
+    return wl, o, st
 
-    zeta = st[0, 0, 0].copy()                       # variational means: nuisances fixed there
+
+def exact_posterior(o, st):
+    """All 64 subsets with the nuisances at the variational means: exact inclusion probability of every phase,
+    the maximum-evidence subset, and the noise-limited ("detection-limit") area ratio of every phase, i.e. the
+    exact posterior sd of h_k in the full linear model times A_k over the fitted total area."""
+    zeta = st[0, 0, 0].copy()
     C = unit_profiles(o, zeta)
     resid = o.y[0] - o.B[0]
     sig, lam = o.sigma_n(), o.lambda_h()
-
     subsets, logZ = [], []
     for n in range(o.K + 1):
         for g in itertools.combinations(range(o.K), n):
@@ -83,22 +93,76 @@ def test_variational_inclusion_against_all_64_subsets(seed):
     post = np.exp(logZ - logZ.max())
     post /= post.sum()
     inc_bf = np.array([sum(p for g, p in zip(subsets, post) if k in g) for k in range(o.K)])
+    cov = np.linalg.inv(C @ C.T / sig ** 2)
+    hhat = cov @ (C @ resid / sig ** 2 - lam)
+    A = np.array([o.inten[o.ofs[k]:o.ofs[k + 1]].sum() for k in range(o.K)])
+    detlim = np.sqrt(np.diag(cov)) * A / (A * np.maximum(hhat, 0.0)).sum()
+    return inc_bf, subsets[int(np.argmax(post))], detlim
 
+
+@pytest.mark.parametrize("seed", [1000, 2024])
+def test_variational_inclusion_probability_against_all_64_subsets(seed):
+    """The pin north_star asks for, on P_incl ITSELF (R15 read-out at the model's own incl_tau = 1 %):
+    {k : P_incl(k) > 1/2} = maximum-evidence subset = planted set, every phase on the same side of 1/2 under the
+    exact posterior and under q, and the absent phases' probabilities close.  Instance: config-0 recipe on a grid that
+    resolves the peaks, fitted to convergence (R29)."""
+    wl, o, st = fitted(seed, True, ITS_CONVERGED)
+    inc_vi = o.inclusion(st)[0, 0]
+    inc_bf, best, detlim = exact_posterior(o, st)
     truth = tuple(sorted(wl.true_phases[0]))
-    best = subsets[int(np.argmax(post))]
+    absent = [k for k in range(o.K) if k not in truth]
+    tau = o.hyper["incl_tau"]
     assert best == truth                                              # exact posterior mode = planted set
-    # variational read-out (area-ratio form, robust to the 1 % threshold on a coarse grid): same set
-    vi_set = tuple(k for k in range(o.K) if area[k] > 0.03)
-    assert vi_set == truth
+    assert tuple(k for k in range(o.K) if inc_vi[k] > 0.5) == truth   # variational read-out: the same set
     for k in range(o.K):
-        assert (inc_bf[k] > 0.5) == (k in truth)
+        assert (inc_bf[k] > 0.5) == (inc_vi[k] > 0.5) == (k in truth)
+    assert np.abs(inc_bf - inc_vi)[list(truth)].max() < 1e-3          # true phases: both say "certainly in"
+    assert inc_vi[absent].max() < 0.15 and inc_bf[absent].max() < 0.25
+    assert np.abs(inc_bf - inc_vi)[absent].max() < 0.2                # Occam factor vs area threshold: close, not equal
+    assert detlim.max() < 0.75 * tau                                  # the instance is decidable at tau (R29)
+    print("absent phases: exact", inc_bf[absent], "variational", inc_vi[absent], "noise-limited area", detlim[absent])
+
+
+@pytest.mark.parametrize("seed", [1000, 2024])
+def test_inclusion_on_config0_grid_and_its_documented_exception(seed):
+    """Config 0 proper (0.07 deg grid, peaks of 0.05-0.15 deg FWHM undersampled): the noise-limited area of an absent
+    phase is 0.4-0.8 % of the total, i.e. comparable with tau = 1 %, so the area-ratio read-out R15 cannot decide every
+    absent phase (R29).  Rule asserted here: true phases are in under both; an absent phase is out under
+    both UNLESS its noise-limited area is >= 0.75 tau (seed 1000 has one such phase: P_incl = 0.52, exact 0.03)."""
+    wl, o, st = fitted(seed, False, ITS_CONVERGED)
+    inc_vi = o.inclusion(st)[0, 0]
+    inc_bf, best, detlim = exact_posterior(o, st)
+    truth = tuple(sorted(wl.true_phases[0]))
+    tau = o.hyper["incl_tau"]
+    assert best == truth
+    undecided = []
+    for k in range(o.K):
         if k in truth:
             assert inc_vi[k] > 0.99 and inc_bf[k] > 0.99
-    # true phases: both say "certainly in"; absent phases: exact inclusion is small (Occam), bounded
+            continue
+        assert inc_bf[k] < 0.35
+        if inc_vi[k] >= 0.5:
+            assert detlim[k] >= 0.75 * tau, (k, inc_vi[k], detlim[k])
+            undecided.append(k)
+        assert inc_vi[k] < 0.6                                         # never "certainly in"
+    assert len(undecided) == (1 if seed == 1000 else 0)
+    print("undecided absent phases", undecided, "variational", inc_vi, "exact", inc_bf, "noise-limited area", detlim)
+
+
+def test_absent_phases_have_not_converged_after_500_iterations():
+    """R29, first half: config 0's own 500 iterations leave the absent phases' scales above their noise limit -- their
+    area ratios are still falling (2.2 % -> 0.7 %, 1.9 % -> 1.2 % between 500 and 2000 steps at seed 1000), so at 500
+    steps P_incl of an absent phase can read 0.99.  The GPU-vs-oracle 0.02 gate at 500 steps compares such values."""
+    wl, o, st500 = fitted(1000, False, 500)
+    _, _, st2000 = fitted(1000, False, ITS_CONVERGED)
+    truth = sorted(wl.true_phases[0])
     absent = [k for k in range(o.K) if k not in truth]
-    assert inc_bf[absent].max() < 0.35
-    print("max |P_bf - P_vi| over true phases", np.abs(inc_bf - inc_vi)[list(truth)].max(),
-          "exact inclusion of absent phases", inc_bf[absent], "variational", inc_vi[absent])
+    inc500, area500 = (a[0, 0] for a in o.inclusion(st500, want_area=True))
+    inc2000, area2000 = (a[0, 0] for a in o.inclusion(st2000, want_area=True))
+    assert inc500[truth].min() > 0.99 and inc2000[truth].min() > 0.99
+    assert area500[absent].max() > 1.5 * area2000[absent].max()       # still shrinking
+    assert inc500[absent].max() > 0.9 and inc2000[absent].max() < 0.6
+    assert np.all(area2000[absent] < area500[absent] + 1e-3)
 
 
 def test_subset_evidence_one_dimensional_closed_form():
