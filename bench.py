@@ -32,7 +32,9 @@ sys.path.insert(0, str(ROOT))
 METRIC = "ELBO+grad peak-point evals/s"
 UNIT = "pair-evals/s"
 L2_FLUSH_BYTES = 256 << 20          # > 126 MB L2
+DOM_KERNEL = "elbo_tile_kernel"     # the dominant kernel of a step (roofline object)
 REF_DRAWS = 16                      # draws per step of the oracle arm (bounded sample)
+FULL_FIT_BUDGET_S = 30.0            # the whole-fit leg of the default run is skipped above this prediction
 # Plain-formulation issue model of one pair: forward 5 FP32 + 2 MUFU,
 # backward 14 FP32 + 2 MUFU + 1/4 LDG.128; MUFU 16 lanes/SM/clk, FP32 128 lanes/SM/clk, 4 issue/SM/clk.
 
@@ -90,16 +92,21 @@ def measured_peaks() -> dict:
     return {}
 
 
-def measured_traffic(kernel: str, cfg: int):
-    """DRAM bytes per launch of `kernel` from the committed ncu capture (profiles/), or None."""
-    p = ROOT / "profiles" / "r1_v5_traffic.txt"
+CAPTURE_FILE = "profiles/r2_capture_counters.txt"
+
+
+def captured_counters(kernel: str, cfg: int):
+    """(DRAM bytes per launch, warp instructions per launch) of `kernel` at config `cfg` from the committed
+    `ncu --set full` capture of THIS build (profiles/r2_capture_counters.txt: kernel, config, dram bytes, warp
+    instructions; written from the capture named in its header), or (None, None) when no capture exists."""
+    p = ROOT / CAPTURE_FILE
     if not p.exists():
-        return None
+        return None, None
     for ln in p.read_text().splitlines():
         t = ln.split()
-        if len(t) == 3 and not ln.startswith("#") and t[0] == kernel and t[1] == str(cfg):
-            return int(t[2])
-    return None
+        if len(t) == 4 and not ln.startswith("#") and t[0] == kernel and t[1] == str(cfg):
+            return int(t[2]), int(t[3])
+    return None, None
 
 
 def run_reference(args, rank: int) -> None:
@@ -170,7 +177,6 @@ def run_ours(args, rank: int, local_rank: int, world: int) -> None:
     t_ms = replicas.max_over_ranks(float(ms.astype(np.float64).sum()), dist, "cuda")
     # per-kernel device times, measured live on the launching stream (CUDA events inside the library)
     tk = gpu.time_kernels(S=S, seed=seeds["draw_seed"], reps=30)
-    clocks = sampler.stop() if sampler else None
 
     # end to end through the C ABI with HOST buffers: create (H2D of the pattern and peak tables) +
     # fit + read-back of the variational parameters and inclusion probabilities, host wall clock.
@@ -191,34 +197,58 @@ def run_ours(args, rank: int, local_rank: int, world: int) -> None:
     h2d = 8 * (wl.two_theta.size + wl.y.size + wl.background.size + wl.peak_pos.size + wl.peak_int.size
                + wl.peak_ofs.size)
     d2h = st.nbytes + inc.nbytes
-    # DESIGN.md R27: the same fit with the per-phase windows refreshed from the variational
-    # means every 250 steps; reported beside the headline numbers, never inside them
+    gpu2.close()
+
+    # The second half of BASELINE.json's metric -- wall-clock of the WHOLE fit of the config (config 1: K=50 =
+    # 2^50 combinations, 2000 iterations) -- measured independently of --steps: xrdvi_create + xrdvi_fit(all
+    # iterations) + read-back through the C ABI with host buffers, host wall clock, max over ranks.  Skipped (with
+    # the reason) only when the per-step time just measured predicts more than FULL_FIT_BUDGET_S seconds.
+    ms_step = float(ms.astype(np.float64).mean())
+    full = {"fit_iterations_full": int(wl.iterations), "fit_wall_s_full": None}
     adaptive = None
     W = float(wl.hyper.get("window_W", 0.0))
-    if W > 0 and args.steps >= 500:
-        gpu2.reset_state(seed=seeds["state_seed"])
+    predicted_s = ms_step * 1e-3 * wl.iterations
+    if predicted_s > FULL_FIT_BUDGET_S:
+        full["skipped"] = f"predicted {predicted_s:.0f} s > {FULL_FIT_BUDGET_S:.0f} s budget of the default run"
+    else:
         barrier()
         t0 = time.perf_counter()
-        gpu2.fit(args.steps, S=S, seed=seeds["draw_seed"])              # static fit on the existing handle (no create)
-        static_s = replicas.max_over_ranks(time.perf_counter() - t0, dist, "cuda")
-        gpu2.reset_state(seed=seeds["state_seed"])
+        gpu3 = Xrdvi.from_workload(wl, device=local_rank)
+        gpu3.reset_state(seed=seeds["state_seed"])
+        _, inc_full, _ = gpu3.fit(wl.iterations, S=S, seed=seeds["draw_seed"])
+        full["fit_wall_s_full"] = replicas.max_over_ranks(time.perf_counter() - t0, dist, "cuda")
+        full["covers"] = ("xrdvi_create (host fp64 preprocessing + H2D) + xrdvi_fit(all iterations) + D2H of "
+                          "parameters and inclusion probabilities, host wall clock")
+        gpu3.reset_state(seed=seeds["state_seed"])
         barrier()
         t0 = time.perf_counter()
-        _, inc_a, _ = gpu2.fit_adaptive(args.steps, 250, W, S=S, seed=seeds["draw_seed"])
-        ad_s = replicas.max_over_ranks(time.perf_counter() - t0, dist, "cuda")
-        ms_a = gpu2.bench_steps(min(args.steps, 20), S=S, seed=seeds["draw_seed"], l2_flush_bytes=L2_FLUSH_BYTES)
-        pairs_after = gpu2.pair_count
-        gpu2.set_phase_windows(None)
-        t0 = time.perf_counter()
-        gpu2.adapt_windows(W)                                           # one full refresh from the static tables
-        refresh_ms = 1e3 * (time.perf_counter() - t0)
-        adaptive = {"fit_wall_s": ad_s, "static_fit_wall_s": static_s, "fit_iterations": args.steps,
-                    "refresh_every": 250, "W": W, "refresh_ms": refresh_ms,
-                    "pairs_per_instance_after": pairs_after,
-                    "ms_per_step_after": float(ms_a.astype(np.float64).mean()),
-                    "max_abs_inclusion_diff_vs_static_fit": float(np.abs(inc_a - inc).max()),
-                    "covers": "xrdvi_fit_adaptive on an existing handle (no create), host wall clock"}
-    gpu2.close()
+        gpu3.fit(wl.iterations, S=S, seed=seeds["draw_seed"])           # the same fit on the existing handle (no create)
+        full["fit_wall_s_full_existing_handle"] = replicas.max_over_ranks(time.perf_counter() - t0, dist, "cuda")
+        truth = set(wl.true_phases[0])
+        full["planted_phases_recovered"] = bool(
+            set(int(k) for k in np.nonzero(inc_full[0, 0] > 0.5)[0]) == truth)
+        # DESIGN.md R27: the same fit with the per-phase windows refreshed from the
+        # variational means every 250 steps; reported beside the headline numbers, never inside them
+        if W > 0 and wl.iterations >= 500:
+            gpu3.reset_state(seed=seeds["state_seed"])
+            barrier()
+            t0 = time.perf_counter()
+            _, inc_a, _ = gpu3.fit_adaptive(wl.iterations, 250, W, S=S, seed=seeds["draw_seed"])
+            ad_s = replicas.max_over_ranks(time.perf_counter() - t0, dist, "cuda")
+            ms_a = gpu3.bench_steps(20, S=S, seed=seeds["draw_seed"], l2_flush_bytes=L2_FLUSH_BYTES)
+            pairs_after = gpu3.pair_count
+            gpu3.set_phase_windows(None)
+            t0 = time.perf_counter()
+            gpu3.adapt_windows(W)                                       # one full refresh from the static tables
+            refresh_ms = 1e3 * (time.perf_counter() - t0)
+            adaptive = {"fit_wall_s": ad_s, "static_fit_wall_s": full["fit_wall_s_full_existing_handle"],
+                        "fit_iterations": int(wl.iterations), "refresh_every": 250, "W": W, "refresh_ms": refresh_ms,
+                        "pairs_per_instance_after": pairs_after,
+                        "ms_per_step_after": float(ms_a.astype(np.float64).mean()),
+                        "max_abs_inclusion_diff_vs_static_fit": float(np.abs(inc_a - inc_full).max()),
+                        "covers": "xrdvi_fit_adaptive on an existing handle (no create), host wall clock"}
+        gpu3.close()
+    clocks = sampler.stop() if sampler else None
 
     if rank != 0:
         if dist is not None:
@@ -234,10 +264,17 @@ def run_ours(args, rank: int, local_rank: int, world: int) -> None:
     dom_ms = tk["ms_tile"]
     achieved = pairs * T / (dom_ms * 1e-3)
     r_plain = n_sm * f_max * 16.0 / 4.0          # plain formulation: 4 MUFU per pair (2 per pass), 16 MUFU lanes/SM/clk
+    traffic, warp_instr = captured_counters(DOM_KERNEL, args.config)
     roofline = {
-        "bound": "alu", "kernel": "elbo_tile_kernel", "achieved": achieved / 1e9, "peak": r_plain / 1e9,
-        "unit": "Gpair/s", "frac": achieved / r_plain, "traffic": measured_traffic("elbo_tile_kernel", args.config),
-        "traffic_source": "profiles/r1_v5_traffic.txt (ncu --set full, dram read + write bytes per launch)",
+        "bound": "alu", "kernel": DOM_KERNEL, "achieved": achieved / 1e9, "peak": r_plain / 1e9,
+        "unit": "Gpair/s", "frac": achieved / r_plain, "traffic": traffic,
+        "traffic_source": (f"{CAPTURE_FILE} (ncu --set full capture of this build: dram read + write bytes per launch)"
+                           if traffic is not None else f"null: no ncu capture of this build at config {args.config} "
+                                                       f"in {CAPTURE_FILE}"),
+        # distance of the kernel from the hardware's own bound for the instruction stream it actually executes:
+        # warp instructions per launch (same capture) / (SMs x 4 issue slots per clock x f_clk x kernel time)
+        "issue_frac": (warp_instr / (n_sm * 4.0 * f_max * dom_ms * 1e-3) if warp_instr else None),
+        "warp_instructions_per_launch": warp_instr,
         "peak_source": f"derived: {n_sm} SMs x {f_max / 1e6:.0f} MHz (MEASURED_PEAKS sm_max_mhz) x 16 MUFU lanes / "
                        f"4 MUFU per pair (plain forward+backward formulation, DESIGN.md Roofline)",
         "ms_tile": tk["ms_tile"], "ms_tile_forward_only": tk["ms_tile_forward_only"], "ms_update": tk["ms_update"],
@@ -274,6 +311,8 @@ def run_ours(args, rank: int, local_rank: int, world: int) -> None:
                    "l2": f"flushed between timed steps ({L2_FLUSH_BYTES >> 20} MiB memset outside the event brackets)",
                    "parallelism": f"replicas x{world} (independent restarts, no collective)"},
         "fit_wall_s": e2e_s, "fit_iterations": args.steps,
+        "fit_wall_s_full": full["fit_wall_s_full"], "fit_iterations_full": full["fit_iterations_full"],
+        "full_fit": full,
         "e2e": {"value": replicas.whole_job_rate(pairs * T * args.steps, world, e2e_s), "unit": UNIT,
                 "h2d_bytes_per_step": h2d / args.steps, "d2h_bytes_per_step": d2h / args.steps,
                 "covers": "xrdvi_create (host fp64 preprocessing + H2D) + xrdvi_fit + D2H of parameters and "
