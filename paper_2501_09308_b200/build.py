@@ -18,14 +18,18 @@ NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a",
               "-Xcompiler", "-fPIC", "-shared", "-cudart", "static"]
 
 
-def build(force: bool = False, verbose: bool = False) -> pathlib.Path:
+def build(force: bool = False, verbose: bool = False, tuning: bool = False, defines: tuple = ()) -> pathlib.Path:
+    """`tuning=True` (``--tuning``) compiles with -DXRDVI_TUNING: the measurement build, in which environment knobs
+    (kernel choice, chunks per warp, cost weights) steer the library for A/B runs.  The product build has none."""
     if not force and LIB.exists() and all(LIB.stat().st_mtime >= p.stat().st_mtime for p in DEPS):
         return LIB
-    cmd = ["nvcc", *NVCC_FLAGS, *(["-Xptxas", "-v"] if verbose else []), "-o", str(LIB), *map(str, SOURCES)]
+    extra = (["-DXRDVI_TUNING"] if tuning else []) + [f"-D{d}" for d in defines]
+    cmd = ["nvcc", *NVCC_FLAGS, *extra, *(["-Xptxas", "-v"] if verbose else []), "-o", str(LIB), *map(str, SOURCES)]
     subprocess.run(cmd, check=True)
     return LIB
 
 
 if __name__ == "__main__":
     import sys
-    print(build(force=True, verbose="-v" in sys.argv))
+    print(build(force=True, verbose="-v" in sys.argv, tuning="--tuning" in sys.argv,
+                defines=tuple(a[2:] for a in sys.argv[1:] if a.startswith("-D"))))

@@ -34,6 +34,7 @@ int fail(int code, const std::string& msg) {
 
 size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
 
+
 struct Plan {   // workspace carve; identical arithmetic in workspace_bytes and create
     int P, R, PR, S_pad, gpi_max, G_max, K;
     int TW, PS, NW, SP, n_seg, n_tile;
@@ -43,6 +44,7 @@ struct Plan {   // workspace carve; identical arithmetic in workspace_bytes and 
     size_t o_var, o_vartmp, o_mom1, o_mom2, o_grad, o_elbo, o_elbok, o_llt, o_trace, o_ctl;
     size_t o_lat, o_eps, o_rr, o_ng, o_llpart, o_part8, o_dbg;
     size_t o_pd, o_lpk, o_zeta, o_gradz, o_lls, o_partial, o_tcnt, o_summ;
+    size_t o_trng;
     int pd_groups;     // groups one launch of the log-joint gradient service handles
 };
 
@@ -139,6 +141,7 @@ bool make_plan(int64_t N, int32_t K, int64_t M, int32_t S_max, double step, cons
     // split kernel (PS > 1): partial profiles of every (group, tile, share) and two counters per (group, tile)
     p.o_partial = take(p.PS > 1 ? sizeof(float) * kPT * 32 * static_cast<size_t>(p.G_max) * p.n_tile * p.PS : 0);
     p.o_tcnt = take(sizeof(unsigned int) * 2 * static_cast<size_t>(p.G_max) * p.n_tile);
+    p.o_trng = take(sizeof(int2) * (static_cast<size_t>(p.n_tile) + 1));
     p.total = o;
     *pl = p;
     return true;
@@ -152,6 +155,8 @@ struct Tables {
     std::vector<int4> run_tab;        // (m0, m1, phase, slot) per phase run (+1 padding header)
     std::vector<int2> share_rng;      // [n_tile][PS] run ranges of the shares
     std::vector<int> seg_order, slot_ofs;
+    std::vector<int2> tile_rng;       // [n_tile + 1] (first run, first record) of every tile's lists
+    int max_tile_rec = 0, max_tile_runs = 0;
     int n_slots = 0;
     long long pairs = 0;              // in-window (peak, point) pairs per draw
 };
@@ -257,6 +262,15 @@ const char* build_tables(const Plan& pl, int64_t N, int K, const std::vector<Hos
     T->seg_order.resize(pl.n_seg);
     std::iota(T->seg_order.begin(), T->seg_order.end(), 0);
     std::stable_sort(T->seg_order.begin(), T->seg_order.end(), [&](int a, int b) { return seg_work[a] > seg_work[b]; });
+    T->tile_rng.resize(static_cast<size_t>(n_tile) + 1);
+    T->max_tile_rec = T->max_tile_runs = 0;
+    for (int t = 0; t <= n_tile; ++t) {
+        T->tile_rng[t] = make_int2(run_base[t], static_cast<int>(ent_base[t]));
+        if (t < n_tile) {
+            T->max_tile_rec = std::max(T->max_tile_rec, static_cast<int>(ent_base[t + 1] - ent_base[t]));
+            T->max_tile_runs = std::max(T->max_tile_runs, run_base[t + 1] - run_base[t]);
+        }
+    }
     T->n_slots = n_slots;
     T->pairs = pairs;
     return nullptr;
@@ -286,15 +300,15 @@ struct xrdvi {
     cudaGraphExec_t graph_execU = nullptr;   // kUnroll steps: programmatic launches also across step boundaries
     int graph_S = -1;
     cudaEvent_t ev[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
-
 };
 
 namespace {
 
-void set_S(xrdvi* h, int S) {
+int set_S(xrdvi* h, int S) {
     h->dev.S = S;
     h->dev.gpi = (S + 31) / 32;
     h->dev.G = h->plan.PR * h->dev.gpi;
+    return XRDVI_OK;
 }
 
 // Upload a set of static tables and make them the ones in force.  The Dev block (kernel argument, held by value in
@@ -314,9 +328,16 @@ int install_tables(xrdvi* h, const Tables& T, const std::vector<long long>& nck,
     CU(cudaMemcpyAsync(w + pl.o_srng, T.share_rng.data(), sizeof(int2) * T.share_rng.size(), cudaMemcpyHostToDevice, st));
     CU(cudaMemcpyAsync(w + pl.o_sord, T.seg_order.data(), sizeof(int) * T.seg_order.size(), cudaMemcpyHostToDevice, st));
     CU(cudaMemcpyAsync(w + pl.o_sofs, T.slot_ofs.data(), sizeof(int) * T.slot_ofs.size(), cudaMemcpyHostToDevice, st));
+    CU(cudaMemcpyAsync(w + pl.o_trng, T.tile_rng.data(), sizeof(int2) * T.tile_rng.size(), cudaMemcpyHostToDevice, st));
     if (at_create) {
         d.n_slots = std::max(T.n_slots, 1);
         d.split = T.pairs / (static_cast<long long>(pl.n_tile) * pl.PS * kPT) >= 512 ? 1 : 0;   // peaks per work item
+        // bulk-copy staging (TW = 1) needs every tile list to fit the shared-memory buffers; decided once (the per-phase
+        // windows of R27 only ever shrink the lists), because the Dev block is held by value in the captured graphs
+        d.stage = (pl.TW == 1 && T.max_tile_rec <= kStageRec && T.max_tile_runs <= kStageRun - 1) ? 1 : 0;
+#ifdef XRDVI_TUNING
+        if (std::getenv("XRDVI_NO_STAGE")) d.stage = 0;     // A/B knob of the measurement build
+#endif
         CU(cudaMemsetAsync(w + pl.o_part8, 0, sizeof(float) * static_cast<size_t>(pl.G_max) * d.n_slots * 8, st));
     }
     CU(cudaStreamSynchronize(st));   // T belongs to the caller
@@ -370,7 +391,10 @@ void launch_tile(const Dev& d, cudaStream_t st, float* f_dbg, long long n_dbg, b
     const dim3 grid(d.G, d.n_seg);   // x = draw group (dispatched fastest), y = position in seg_order
 #define XRDVI_TILE_CASE(TW_, PS_)                                                                                \
     case TW_ * 16 + PS_:                                                                                        \
-        launch_k(elbo_tile_kernel<TW_, PS_, BWD>, grid, dim3(32 * TW_ * PS_), st, pdl, d, f_dbg, n_dbg);         \
+        if (TW_ == 1 && d.stage)                                                                                \
+            launch_k(elbo_tile_kernel<1, PS_, BWD, true>, grid, dim3(32 * PS_), st, pdl, d, f_dbg, n_dbg);       \
+        else                                                                                                    \
+            launch_k(elbo_tile_kernel<TW_, PS_, BWD, false>, grid, dim3(32 * TW_ * PS_), st, pdl, d, f_dbg, n_dbg); \
         break;
     switch (d.TW * 16 + d.PS) {
         XRDVI_TILE_CASE(1, 1) XRDVI_TILE_CASE(1, 2) XRDVI_TILE_CASE(1, 3) XRDVI_TILE_CASE(1, 4) XRDVI_TILE_CASE(1, 5) XRDVI_TILE_CASE(1, 6) XRDVI_TILE_CASE(1, 8)
@@ -454,8 +478,8 @@ int ensure_graph(xrdvi* h, int S) {
     if (h->graph_exec && h->graph_execU && h->graph_S == S) return XRDVI_OK;
     if (h->graph_exec) { cudaGraphExecDestroy(h->graph_exec); h->graph_exec = nullptr; }
     if (h->graph_execU) { cudaGraphExecDestroy(h->graph_execU); h->graph_execU = nullptr; }
-    set_S(h, S);
-    int rc = capture_steps(h, 1, &h->graph_exec);
+    int rc = set_S(h, S);
+    if (rc == XRDVI_OK) rc = capture_steps(h, 1, &h->graph_exec);
     if (rc == XRDVI_OK) rc = capture_steps(h, kUnroll, &h->graph_execU);
     if (rc != XRDVI_OK) return rc;
     h->graph_S = S;
@@ -692,6 +716,8 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
     d.partial = reinterpret_cast<float*>(w + pl.o_partial);
     d.tile_cnt = reinterpret_cast<unsigned int*>(w + pl.o_tcnt);
     d.tile_cnt2 = d.tile_cnt + static_cast<size_t>(pl.G_max) * pl.n_tile;
+    d.tile_rng = reinterpret_cast<int2*>(w + pl.o_trng);
+    d.stage = 0;
     set_S(h, S_max);
 
     cudaStream_t st = h->stream;
@@ -855,7 +881,8 @@ static int begin_eval(xrdvi* h, const float* var_params, int32_t S, uint64_t see
         CU(cudaMemcpyAsync(tmp, var_params, sizeof(float) * h->plan.PR * 8 * h->K, cudaMemcpyHostToDevice, h->stream));
         *var = tmp;
     }
-    set_S(h, S);
+    rc = set_S(h, S);
+    if (rc) return rc;
     return write_ctl(h, seed, h->step_host, h->step_host, static_cast<long long>(iteration & 0xFFFFFFFFull));
 }
 
@@ -1054,7 +1081,8 @@ int xrdvi_time_kernels(xrdvi* h, int32_t S, uint64_t seed, int32_t reps, float* 
     if (rc) return rc;
     if (reps < 1 || !ms) return fail(XRDVI_E_INVALID_ARG, "reps < 1 or ms NULL");
     CU(cudaSetDevice(h->device));
-    set_S(h, S);
+    rc = set_S(h, S);
+    if (rc) return rc;
     rc = write_ctl(h, seed, h->step_host, h->step_host, -1);
     if (rc) return rc;
     const Dev& d = h->dev;
@@ -1092,7 +1120,8 @@ int xrdvi_debug_timeline(xrdvi* h, int32_t S, uint64_t seed, int64_t capacity, u
     if (rc) return rc;
     if (!rows || !n_rows || capacity < 1) return fail(XRDVI_E_INVALID_ARG, "rows / n_rows NULL or capacity < 1");
     CU(cudaSetDevice(h->device));
-    set_S(h, S);
+    rc = set_S(h, S);
+    if (rc) return rc;
     rc = write_ctl(h, seed, h->step_host, h->step_host, -1);
     if (rc) return rc;
     Dev d = h->dev;                                       // a copy with the stamp buffer attached

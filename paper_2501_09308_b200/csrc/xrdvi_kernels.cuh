@@ -127,6 +127,8 @@ struct Dev {
     unsigned int* tile_cnt2;  // [G][n_tile] phase-2 items that are done
     float* pd;                // nullptr, or [groups of the launch][n_slots][4][32] d ll / d zeta per (run, class, draw)
     int g_base;               // group of blockIdx.x = 0 in elbo_tile_kernel (0 except in the service)
+    const int2* tile_rng;     // [n_tile + 1] (first run, first record) of every tile's lists
+    int stage;                // 1: elbo_tile_kernel copies the tile's lists into shared memory (they fit: host check)
     // measurement (xrdvi_debug_timeline): nullptr, or [warps of the launch][4] = (start, end of phase 1, end, SM id | records << 32)
     unsigned long long* tl;
 };
@@ -587,6 +589,57 @@ __device__ __forceinline__ void finish_step(const Dev& d) {
 }
 
 // ------------------------------------------------------------------------------------------------
+// Where a warp reads the static per-tile tables from: global memory (warp-uniform LDG.128 broadcasts through L1/L2),
+// or the copy of the tile's lists that elbo_tile_kernel staged in shared memory with bulk asynchronous copies
+// (north_star: "per-tile peak windows ... staged through shared memory/TMA"; LDS.128 broadcasts).
+struct SrcGlobal {
+    const PeakRec* __restrict__ pkt;
+    const int4* __restrict__ runs;
+    __device__ __forceinline__ PeakRec rec(int m) const { return pkt[m]; }
+    __device__ __forceinline__ int4 run(int r) const { return runs[r]; }
+};
+struct SrcShared {   // shared-window byte addresses of record 0 / run 0 (i.e. already offset by the tile's first index)
+    unsigned rec0, run0;
+    __device__ __forceinline__ PeakRec rec(int m) const {
+        PeakRec v;
+        asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];"
+                     : "=r"(v.dj), "=f"(v.delta), "=f"(v.inten), "=r"(v.full) : "r"(rec0 + 16u * static_cast<unsigned>(m)));
+        return v;
+    }
+    __device__ __forceinline__ int4 run(int r) const {
+        int4 v;
+        asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];"
+                     : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(run0 + 16u * static_cast<unsigned>(r)));
+        return v;
+    }
+};
+
+// Bulk asynchronous copy global -> shared memory completed on an mbarrier (cp.async.bulk; SASS UBLKCP).
+constexpr int kStageRec = 224;   // records / run headers (incl. the one after the last run) a staged tile list may hold
+constexpr int kStageRun = 56;
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return static_cast<unsigned>(__cvta_generic_to_shared(p)); }
+__device__ __forceinline__ void mbar_init(unsigned mbar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(mbar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned mbar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mbar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(unsigned dst, const void* src, unsigned bytes, unsigned mbar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(dst), "l"(src), "r"(bytes), "r"(mbar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned mbar, unsigned parity) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tWAIT_%=:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra DONE_%=;\n\tbra WAIT_%=;\n\tDONE_%=:\n\t}"
+        ::"r"(mbar), "r"(parity) : "memory");
+}
+template <bool STAGE> struct TileSrc;
+template <> struct TileSrc<false> { typedef SrcGlobal type; };
+template <> struct TileSrc<true> { typedef SrcShared type; };
+
+// ------------------------------------------------------------------------------------------------
 // a-3 .. a-6 (likelihood part): profile + residual + backward of one 16-point tile for one group of 32 draws.
 // A warp owns one tile and one share of the tile's phase runs, in BOTH phases.  A run = the peaks of one phase
 // that reach the tile; its header carries the phase, so the per-phase latents are loaded once per run (prefetched
@@ -612,28 +665,27 @@ __device__ __forceinline__ TileCtx tile_ctx(const Dev& d, int g, int tile) {
 
 // Phase 1: acc[p] = profile of the runs [rng.x, rng.y) on the 16 points of the tile (acc is overwritten).  The
 // accumulators live as packed pairs (quad Q: acc2[2Q] = points (4Q, 4Q+2), acc2[2Q+1] = points (4Q+1, 4Q+3)).
-__device__ __forceinline__ void tile_phase1(const Dev& d, const TileCtx& c, int2 rng, float (&acc)[kPT]) {
+template <class Src>
+__device__ __forceinline__ void tile_phase1(const Dev& d, const Src& src, const TileCtx& c, int2 rng, float (&acc)[kPT]) {
     f32x2 acc2[kPT / 2];
 #pragma unroll
     for (int i = 0; i < kPT / 2; ++i) acc2[i] = 0ull;
     if (rng.x < rng.y) {
-        const PeakRec* __restrict__ pkt = d.pk_tile;
-        const int4* __restrict__ runs = d.run_tab;
-        int4 run_n = runs[rng.x];
+        int4 run_n = src.run(rng.x);
         float4 lt_n = c.lat[static_cast<size_t>(run_n.z) * 32];
         int ng_n = c.ngk[run_n.z];
         for (int r = rng.x; r < rng.y; ++r) {
             const int4 run = run_n;
             const float4 lt = lt_n;
             const int ngc = ng_n;
-            run_n = runs[r + 1];                            // run_tab carries one padding entry
+            run_n = src.run(r + 1);                         // run_tab carries one padding entry
             lt_n = c.lat[static_cast<size_t>(run_n.z) * 32];
             ng_n = c.ngk[run_n.z];
             const float step = d.delta * lt.x;
             const unsigned core_span = static_cast<unsigned>(kPT - 1 + 2 * ngc);
 #pragma unroll 1
             for (int m = run.x; m < run.y; ++m) {
-                const PeakRec pk = pkt[m];
+                const PeakRec pk = src.rec(m);
                 const float t0 = fmaf(static_cast<float>(-pk.dj), step, fmaf(-pk.delta, lt.x, lt.y));
                 const float cl = pk.inten * lt.w;
                 const bool core = static_cast<unsigned>(pk.dj + ngc) <= core_span;   // Gaussian core touches the tile
@@ -709,7 +761,9 @@ __device__ __forceinline__ void tile_debug_profile(const Dev& d, const TileCtx& 
 
 // Phase 2: six sums per phase run [rng.x, rng.y) over the tile from the residual e, chain rule, reduction over the
 // 32 draws (or, in the gradient service, per-draw output to row pd_row of d.pd).
-__device__ __forceinline__ void tile_phase2(const Dev& d, const TileCtx& c, int2 rng, const float (&e)[kPT], int pd_row) {
+template <class Src>
+__device__ __forceinline__ void tile_phase2(const Dev& d, const Src& src, const TileCtx& c, int2 rng, const float (&e)[kPT],
+                                            int pd_row) {
     if (rng.x >= rng.y) return;
     const int lane = threadIdx.x & 31;
     f32x2 e2[kPT / 2], pe2[kPT / 2];     // packed like the accumulators of phase 1; pe_p = p e_p
@@ -720,20 +774,18 @@ __device__ __forceinline__ void tile_phase2(const Dev& d, const TileCtx& c, int2
         pe2[2 * Q] = pack2(static_cast<float>(4 * Q) * e[4 * Q], static_cast<float>(4 * Q + 2) * e[4 * Q + 2]);
         pe2[2 * Q + 1] = pack2(static_cast<float>(4 * Q + 1) * e[4 * Q + 1], static_cast<float>(4 * Q + 3) * e[4 * Q + 3]);
     }
-    const PeakRec* __restrict__ pkt = d.pk_tile;
-    const int4* __restrict__ runs = d.run_tab;
     const float4* __restrict__ epsg = d.eps + static_cast<size_t>(c.g) * d.K * 32 + lane;
     const float* __restrict__ rrg = d.rr + static_cast<size_t>(c.g) * d.K * 32 + lane;
     float* __restrict__ part = d.part8 + static_cast<size_t>(c.g) * d.n_slots * 8;
 
-    int4 run_n = runs[rng.x];
+    int4 run_n = src.run(rng.x);
     float4 lt_n = c.lat[static_cast<size_t>(run_n.z) * 32];
     int ng_n = c.ngk[run_n.z];
     for (int r = rng.x; r < rng.y; ++r) {
         const int4 run = run_n;
         const float4 lt = lt_n;
         const int ngc = ng_n;
-        run_n = runs[r + 1];
+        run_n = src.run(r + 1);
         lt_n = c.lat[static_cast<size_t>(run_n.z) * 32];
         ng_n = c.ngk[run_n.z];
         // loads of the flush, issued early
@@ -746,7 +798,7 @@ __device__ __forceinline__ void tile_phase2(const Dev& d, const TileCtx& c, int2
         float B1 = 0.f, B2 = 0.f, B3 = 0.f, B4 = 0.f, B5 = 0.f, B6 = 0.f;
 #pragma unroll 1
         for (int m = run.x; m < run.y; ++m) {
-            const PeakRec pk = pkt[m];
+            const PeakRec pk = src.rec(m);
             const float t0 = fmaf(static_cast<float>(-pk.dj), step, fmaf(-pk.delta, lt.x, lt.y));
             const bool core = static_cast<unsigned>(pk.dj + ngc) <= core_span;
             if ((pk.full & 1) && !core) {
@@ -815,12 +867,20 @@ constexpr int tile_ctas_per_sm(int TW, int PS) {
     const int budget = warps > 1 ? XRDVI_TILE_WARPS_PER_SM_SHARED : XRDVI_TILE_WARPS_PER_SM;
     return budget / warps > 0 ? budget / warps : 1;
 }
-template <int TW, int PS, bool BWD>
+// STAGE (TW = 1): thread 0 copies the tile's record list and run headers into shared memory with two bulk asynchronous
+// copies completed on an mbarrier (north_star: "per-tile peak windows ... staged through shared memory/TMA"); the
+// tables are static, so the copies are issued BEFORE griddepcontrol.wait and overlap the predecessor kernel's drain.
+// All PS shares of the CTA then read records and run headers with LDS.128 broadcasts in both phases.
+template <int TW, int PS, bool BWD, bool STAGE>
 __global__ void __launch_bounds__(32 * TW * PS, tile_ctas_per_sm(TW, PS))
 elbo_tile_kernel(const Dev d, float* __restrict__ f_dbg, long long n_dbg) {
+    static_assert(!STAGE || TW == 1, "staging holds one tile list per CTA");
     __shared__ float4 e_s[TW][kPT / 4][32];
     __shared__ float ss_s[TW][32];
     __shared__ float acc_s[PS > 1 ? (PS - 1) * TW * kPT : 1][32];
+    __shared__ __align__(128) PeakRec rec_s[STAGE ? kStageRec : 1];
+    __shared__ __align__(16) int4 run_s[STAGE ? kStageRun : 1];
+    __shared__ __align__(8) unsigned long long mbar_s;
     griddep_launch_dependents();
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const int tw = w % TW, ps = w / TW;
@@ -829,9 +889,30 @@ elbo_tile_kernel(const Dev d, float* __restrict__ f_dbg, long long n_dbg) {
     const int seg = d.seg_order[blockIdx.y];                // static tables: may be read before the predecessor is done
     const int tile = seg * TW + tw;
     const bool live = tile < d.n_tile;                      // the last segment may have fewer than TW tiles
+    typename TileSrc<STAGE>::type src;
+    if constexpr (STAGE) {
+        const int2 t0 = d.tile_rng[tile], t1 = d.tile_rng[tile + 1];
+        const unsigned mb = smem_u32(&mbar_s);
+        if (threadIdx.x == 0) {
+            mbar_init(mb, 1);
+            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+            const unsigned rb = 16u * static_cast<unsigned>(t1.y - t0.y), hb = 16u * static_cast<unsigned>(t1.x - t0.x + 1);
+            mbar_expect_tx(mb, rb + hb);
+            if (rb) bulk_g2s(smem_u32(&rec_s[0]), d.pk_tile + t0.y, rb, mb);
+            bulk_g2s(smem_u32(&run_s[0]), d.run_tab + t0.x, hb, mb);      // + the header after the last run
+        }
+        src.rec0 = smem_u32(&rec_s[0]) - 16u * static_cast<unsigned>(t0.y);
+        src.run0 = smem_u32(&run_s[0]) - 16u * static_cast<unsigned>(t0.x);
+    } else {
+        src = SrcGlobal{d.pk_tile, d.run_tab};
+    }
     const TileCtx c = tile_ctx(d, d.g_base + blockIdx.x, tile);
     int2 rng = make_int2(0, 0);
     if (live) rng = d.share_rng[tile * PS + ps];
+    if constexpr (STAGE) {
+        if (PS > 1) __syncthreads();                        // the mbarrier is initialised before anybody polls it
+        mbar_wait(smem_u32(&mbar_s), 0u);
+    }
     griddep_wait();                                         // latents, control block: written by the predecessor
     if (blockIdx.x == gridDim.x - 1 && blockIdx.y == gridDim.y - 1) finish_step(d);   // previous step's ELBO / count
     const unsigned tl_row = (blockIdx.y * gridDim.x + blockIdx.x) * (TW * PS) + w;
@@ -841,7 +922,7 @@ elbo_tile_kernel(const Dev d, float* __restrict__ f_dbg, long long n_dbg) {
     float acc[kPT];
 #pragma unroll
     for (int p = 0; p < kPT; ++p) acc[p] = 0.0f;
-    tile_phase1(d, c, rng, acc);
+    tile_phase1(d, src, c, rng, acc);
 
     if (PS > 1) {   // sum the PS partial profiles of the tile: shares 1.. in order onto share 0
         if (ps > 0) {
@@ -883,7 +964,7 @@ elbo_tile_kernel(const Dev d, float* __restrict__ f_dbg, long long n_dbg) {
         const float4 t = e_s[tw][v][lane];
         e[4 * v] = t.x; e[4 * v + 1] = t.y; e[4 * v + 2] = t.z; e[4 * v + 3] = t.w;
     }
-    tile_phase2(d, c, rng, e, blockIdx.x);
+    tile_phase2(d, src, c, rng, e, blockIdx.x);
     tl_stamp(d.tl, tl_row, 2);
 }
 
@@ -933,7 +1014,7 @@ __global__ void __launch_bounds__(32, XRDVI_TILE_WARPS_PER_SM) elbo_split_kernel
         float acc[kPT];
 #pragma unroll
         for (int p = 0; p < kPT; ++p) acc[p] = 0.0f;
-        tile_phase1(d, c, rng, acc);
+        tile_phase1(d, SrcGlobal{d.pk_tile, d.run_tab}, c, rng, acc);
 #pragma unroll
         for (int p = 0; p < kPT; ++p) __stcg(partial + (ps * kPT + p) * 32, acc[p]);
         __threadfence();
@@ -959,7 +1040,7 @@ __global__ void __launch_bounds__(32, XRDVI_TILE_WARPS_PER_SM) elbo_split_kernel
             d.llpart[(static_cast<size_t>(c.g) * d.n_seg + tile) * 32 + lane] = ss;
             if (f_dbg) tile_debug_profile(d, c, acc, f_dbg, n_dbg);
         }
-        if (BWD) tile_phase2(d, c, rng, ev, gi);
+        if (BWD) tile_phase2(d, SrcGlobal{d.pk_tile, d.run_tab}, c, rng, ev, gi);
         __syncwarp();
         if (lane == 0) {   // the last phase-2 item of the (tile, group) re-arms its counters for the next launch
             const unsigned n_second = BWD ? PS : 1;
