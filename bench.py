@@ -154,12 +154,12 @@ def run_ours(args, rank: int, local_rank: int, world: int) -> None:
         dist_mod.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
         dist = dist_mod
 
-    # weak scaling: every rank fits its own replica (own restart seed) of the same workload; the path
+    # weak scaling: every rank fits its own replica (own jittered restart, own draw seed) of the same workload; the path
     # shards over independent (pattern, restart) instances with no data-path collective.
     wl = synth.make_workload(args.config)
     gpu = Xrdvi.from_workload(wl, device=local_rank)
     seeds = replicas.replica_seeds(rank)
-    gpu.reset_state(seed=seeds["state_seed"])
+    gpu.reset_state(seed=seeds["state_seed"], restart_offset=seeds["restart_offset"])
     S, T = wl.S, wl.P * wl.R * wl.S
     pairs = gpu.pair_count
     gpu.bench_steps(max(args.warmup, 1), S=S, seed=seeds["draw_seed"], l2_flush_bytes=L2_FLUSH_BYTES)
@@ -183,7 +183,7 @@ def run_ours(args, rank: int, local_rank: int, world: int) -> None:
     barrier()
     t0 = time.perf_counter()
     gpu2 = Xrdvi.from_workload(wl, device=local_rank)
-    gpu2.reset_state(seed=seeds["state_seed"])
+    gpu2.reset_state(seed=seeds["state_seed"], restart_offset=seeds["restart_offset"])
     st, inc, _ = gpu2.fit(args.steps, S=S, seed=seeds["draw_seed"])
     e2e_s = replicas.max_over_ranks(time.perf_counter() - t0, dist, "cuda")
     # the same through one xrdvi_elbo_grad call per step: H2D of the variational parameters, D2H of ELBO and
@@ -214,12 +214,12 @@ def run_ours(args, rank: int, local_rank: int, world: int) -> None:
         barrier()
         t0 = time.perf_counter()
         gpu3 = Xrdvi.from_workload(wl, device=local_rank)
-        gpu3.reset_state(seed=seeds["state_seed"])
+        gpu3.reset_state(seed=seeds["state_seed"], restart_offset=seeds["restart_offset"])
         _, inc_full, _ = gpu3.fit(wl.iterations, S=S, seed=seeds["draw_seed"])
         full["fit_wall_s_full"] = replicas.max_over_ranks(time.perf_counter() - t0, dist, "cuda")
         full["covers"] = ("xrdvi_create (host fp64 preprocessing + H2D) + xrdvi_fit(all iterations) + D2H of "
                           "parameters and inclusion probabilities, host wall clock")
-        gpu3.reset_state(seed=seeds["state_seed"])
+        gpu3.reset_state(seed=seeds["state_seed"], restart_offset=seeds["restart_offset"])
         barrier()
         t0 = time.perf_counter()
         gpu3.fit(wl.iterations, S=S, seed=seeds["draw_seed"])           # the same fit on the existing handle (no create)
@@ -230,7 +230,7 @@ def run_ours(args, rank: int, local_rank: int, world: int) -> None:
         # DESIGN.md R27: the same fit with the per-phase windows refreshed from the
         # variational means every 250 steps; reported beside the headline numbers, never inside them
         if W > 0 and wl.iterations >= 500:
-            gpu3.reset_state(seed=seeds["state_seed"])
+            gpu3.reset_state(seed=seeds["state_seed"], restart_offset=seeds["restart_offset"])
             barrier()
             t0 = time.perf_counter()
             _, inc_a, _ = gpu3.fit_adaptive(wl.iterations, 250, W, S=S, seed=seeds["draw_seed"])

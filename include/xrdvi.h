@@ -45,7 +45,7 @@ enum {
     XRDVI_OK = 0,
     XRDVI_E_INVALID_ARG = -1,
     XRDVI_E_UNSORTED_GRID = -2,      /* 2theta not strictly increasing                      */
-    XRDVI_E_NONUNIFORM_GRID = -3,    /* 2theta not uniform to 1e-6 of the step (this build)  */
+    XRDVI_E_NONUNIFORM_GRID = -3,    /* 2theta not uniform to 1e-6 of the step (R16: see xrdvi_create) */
     XRDVI_E_EMPTY_PHASE = -4,        /* a phase with M_k = 0                                 */
     XRDVI_E_WORKSPACE_TOO_SMALL = -5,
     XRDVI_E_CUDA = -6,
@@ -88,11 +88,16 @@ size_t xrdvi_workspace_bytes(int64_t N, int32_t K, int64_t M, int32_t S_max, dou
                              const xrdvi_hyper* hyp);
 
 /* Build a problem.
- *  two_theta [N]     strictly increasing, uniform grid (deg)
+ *  two_theta [N]     strictly increasing, uniform grid (deg): the peak encoding (nearest grid index + fp64 offset,
+ *                    R16) and the integer window need a constant step; a grid that departs from uniform by more
+ *                    than 1e-6 of the step is rejected with XRDVI_E_NONUNIFORM_GRID (the paper's grid is uniform,
+ *                    PAPER.md:84)
  *  y [P][N]          observed intensities;  background [P][N] or NULL (-> 0) (R5: B is an input)
  *  peak_ofs [K+1]    CSR offsets into peak_pos / peak_int ([M], M = peak_ofs[K]); any order inside
  *                    a phase; peaks with no in-window grid point are dropped (R16)
- *  device, cuda_stream   CUDA device ordinal and a cudaStream_t (0 = legacy default stream)
+ *  device, cuda_stream   CUDA device ordinal and a cudaStream_t the library enqueues all its work on.  It must be
+ *                    capturable into a CUDA Graph; NULL (the legacy default stream cannot be captured) makes
+ *                    xrdvi_create create a private non-blocking stream, destroyed by xrdvi_destroy
  *  workspace         DEVICE pointer, >= xrdvi_workspace_bytes(...) bytes, 256-byte aligned, owned by
  *                    the caller and kept alive until xrdvi_destroy
  * Preprocessing (sorting, grid-index encoding j_m/delta_m, window tables) is done on the host in
@@ -136,12 +141,25 @@ int xrdvi_fit_adaptive(xrdvi* h, int32_t iterations, int32_t S, uint64_t seed, i
                        float* var_params_out, double* incl_prob, double* elbo_trace);
 
 /* (Re)initialise the variational state (R11), zero the Adam moments and the step counter.
- * Restart r > 0 is jittered with Philox counter (0xFFFFFFFF, r, k, pat) under `seed`.              */
+ * Restart r > 0 is jittered with Philox counter (0xFFFFFFFF, r, k, pat) under `seed`.
+ * xrdvi_reset_state_restart: the same with the restart index shifted, r = rst + restart_offset >= 0 -- instance
+ * (pat, rst) starts where restart rst + restart_offset of a larger problem would (independent replicas of one
+ * problem on several GPUs: rank as the offset gives every replica its own jittered start).            */
 int xrdvi_reset_state(xrdvi* h, uint64_t seed);
-/* Copy the state out / in: var_params float [P][R][2][K][4].  set_state also zeroes the Adam
- * moments and sets the step counter to `step` (number of completed optimisation steps).            */
+int xrdvi_reset_state_restart(xrdvi* h, uint64_t seed, int32_t restart_offset);
+/* Copy the state out / in: var_params float [P][R][2][K][4].  set_state sets the step counter to `step` (number of
+ * completed optimisation steps; the next step draws with Philox iteration step + 1) and starts a FRESH Adam: the
+ * moments are zeroed and the bias correction restarts with them (first step after set_state = lr * sign(g)).
+ * To continue a fit exactly (checkpoint / resume), also carry the optimiser state:
+ * xrdvi_get_optimizer_state: mom1, mom2 float [P][R][2][K][4] (Adam's first / second moments; either may be NULL),
+ *   *adam_steps = steps the moments have accumulated (the exponent of the bias correction).
+ * xrdvi_set_optimizer_state: after xrdvi_set_state; 0 <= adam_steps <= step.  fit(n) + get_state +
+ *   get_optimizer_state, then set_state + set_optimizer_state + fit(m) on any handle of the same problem is bitwise
+ *   fit(n + m) (tested).                                                                              */
 int xrdvi_get_state(xrdvi* h, float* var_params, int64_t* step);
 int xrdvi_set_state(xrdvi* h, const float* var_params, int64_t step);
+int xrdvi_get_optimizer_state(xrdvi* h, float* mom1, float* mom2, int64_t* adam_steps);
+int xrdvi_set_optimizer_state(xrdvi* h, const float* mom1, const float* mom2, int64_t adam_steps);
 
 /* One ELBO-and-gradient evaluation (eq.7 PAPER.md:111 as a Monte-Carlo mean over S reparameterised
  * draws + analytic entropy, R7/R8):
@@ -186,49 +204,6 @@ int xrdvi_posterior_summary(xrdvi* h, double* summary);
  *  ll, lpj, grad may each be NULL.                                                                           */
 int xrdvi_logjoint_grad(xrdvi* h, const float* zeta, int64_t n, int32_t pattern, double* ll, double* lpj,
                         float* grad);
-
-/* Debug read-back of the forward pass for parity tests: runs draw + forward at (var_params or
- * internal state, S, seed, iteration) and returns, for the first n sample-instances in
- * (pat, rst, s) order, the profile f float [n][N] (including B) and ll double [n]; f or ll may be NULL. */
-int xrdvi_debug_profile(xrdvi* h, const float* var_params, int32_t S, uint64_t seed,
-                        uint64_t iteration, int64_t n, float* f, double* ll);
-
-/* Debug read-back of the draw kernel (a-1, a-2) at the internal state: eps float [n][K][4] for the first n
- * sample-instances; raw_words uint32 [n][K][4] (the Philox output) or NULL; core_halfwidth int32 [n][K]
- * or NULL: the Gaussian-core half-width n_g in grid points of the 32-draw group the instance belongs to
- * (outside |i - j_m| <= n_g the kernels evaluate only the Lorentzian).          */
-int xrdvi_debug_draws(xrdvi* h, int32_t S, uint64_t seed, uint64_t iteration, int64_t n, float* eps,
-                      uint32_t* raw_words, int32_t* core_halfwidth);
-
-/* Measurement: mean CUDA-event times (ms) over `reps` repetitions (after one warm-up) of the kernels of one
- * evaluation at the internal state, launched one by one on the handle's stream: ms float [4] =
- * [0] elbo_tile_kernel (fused profile + residual + backward), [1] its forward-only instantiation (profile +
- * residual), [2] update_draw_kernel without the update, [3] draw + tile + update together.          */
-int xrdvi_time_kernels(xrdvi* h, int32_t S, uint64_t seed, int32_t reps, float* ms);
-
-/* Measurement: per-warp timeline of ONE launch of the fused profile / residual / backward kernel (a-3 .. a-7) at the
- * internal state with S draws per instance, after two un-stamped warm-up launches.  Every warp (or, where the
- * ticket-queue variant of the kernel is selected, every one-warp work item) writes four uint64 words:
- *   [0] %globaltimer (ns) when it starts, [1] at the end of the profile phase, [2] when it is done,
- *   [3] SM id (low 32 bits) | number of (peak, tile) records of its share (high 32 bits).
- * rows uint64 [capacity][4] (host), *n_rows = rows written; XRDVI_E_INVALID_ARG if capacity is smaller than the
- * number of warps of the launch.  The state is not modified (the per-step draw buffers are overwritten).  This is
- * how profiles/ shows which part of a launch is full-occupancy work and which part is the drain of its last wave. */
-int xrdvi_debug_timeline(xrdvi* h, int32_t S, uint64_t seed, int64_t capacity, uint64_t* rows, int64_t* n_rows);
-
-/* Measurement: `steps` optimisation steps (graph replays, exactly as xrdvi_fit runs them), each one
- * bracketed by its own pair of CUDA events on the handle's stream; between two steps, outside the
- * brackets, `l2_flush_bytes` of device memory are overwritten (0 = no flush) so that every step starts
- * with a cold L2.  ms_steps float [steps] receives the per-step device times.  The state advances.   */
-int xrdvi_bench_steps(xrdvi* h, int32_t steps, int32_t S, uint64_t seed, size_t l2_flush_bytes,
-                      float* ms_steps);
-
-/* Measurement: per-SM, per-clock rates of the pipes that bound the path (microbenchmark, DESIGN.md
- * "Roofline").  rates float [9]: lane-operations per SM clock of [0] FFMA, [1] FFMA2 (2 FMAs per lane),
- * [2] MUFU.EX2, [3] MUFU.RCP, [4] the plain forward instruction mix (5 FP32 : 2 MUFU), [5] the plain
- * backward mix (14 FP32 : 2 MUFU), [6] 7 FFMA2 : 2 MUFU, [7] EX2 and RCP chains run together (MUFU
- * operations per clock); [8] = SM clock (MHz) during the run.                                       */
-int xrdvi_pipe_rates(int device, float* rates);
 
 const char* xrdvi_last_error(void);
 

@@ -14,12 +14,15 @@ import numpy as np
 _PKG = pathlib.Path(__file__).resolve().parent
 _LIB_PATH = _PKG / "libxrdvi.so"
 
-EXPORTS = (
+EXPORTS = (            # include/xrdvi.h: the product boundary
     "xrdvi_default_hyper", "xrdvi_workspace_bytes", "xrdvi_create", "xrdvi_destroy", "xrdvi_pair_count",
     "xrdvi_window_halfwidth", "xrdvi_set_phase_windows", "xrdvi_get_phase_windows", "xrdvi_adapt_windows",
-    "xrdvi_fit_adaptive", "xrdvi_reset_state", "xrdvi_get_state", "xrdvi_set_state", "xrdvi_elbo_grad",
-    "xrdvi_fit", "xrdvi_inclusion", "xrdvi_posterior_summary", "xrdvi_logjoint_grad", "xrdvi_debug_profile", "xrdvi_debug_draws", "xrdvi_time_kernels",
-    "xrdvi_bench_steps", "xrdvi_debug_timeline", "xrdvi_pipe_rates", "xrdvi_last_error",
+    "xrdvi_fit_adaptive", "xrdvi_reset_state", "xrdvi_reset_state_restart", "xrdvi_get_state", "xrdvi_set_state",
+    "xrdvi_get_optimizer_state", "xrdvi_set_optimizer_state", "xrdvi_elbo_grad",
+    "xrdvi_fit", "xrdvi_inclusion", "xrdvi_posterior_summary", "xrdvi_logjoint_grad", "xrdvi_last_error",
+)
+DEBUG_EXPORTS = (      # include/xrdvi_debug.h: read-backs for the parity tests, timing for bench.py and profiles/
+    "xrdvi_debug_profile", "xrdvi_debug_draws", "xrdvi_time_kernels", "xrdvi_bench_steps", "xrdvi_debug_timeline",
 )
 
 
@@ -72,6 +75,9 @@ def load_library():
     L.xrdvi_adapt_windows.argtypes = [vp, C.c_double, ip]
     L.xrdvi_fit_adaptive.argtypes = [vp, C.c_int32, C.c_int32, C.c_uint64, C.c_int32, C.c_double, fp, dp, dp]
     L.xrdvi_reset_state.argtypes = [vp, C.c_uint64]
+    L.xrdvi_reset_state_restart.argtypes = [vp, C.c_uint64, C.c_int32]
+    L.xrdvi_get_optimizer_state.argtypes = [vp, fp, fp, C.POINTER(C.c_int64)]
+    L.xrdvi_set_optimizer_state.argtypes = [vp, fp, fp, C.c_int64]
     L.xrdvi_get_state.argtypes = [vp, fp, C.POINTER(C.c_int64)]
     L.xrdvi_set_state.argtypes = [vp, fp, C.c_int64]
     L.xrdvi_elbo_grad.argtypes = [vp, fp, C.c_int32, C.c_uint64, C.c_uint64, dp, fp]
@@ -79,13 +85,13 @@ def load_library():
     L.xrdvi_inclusion.argtypes = [vp, dp, dp]
     L.xrdvi_posterior_summary.argtypes = [vp, dp]
     L.xrdvi_logjoint_grad.argtypes = [vp, fp, C.c_int64, C.c_int32, dp, dp, fp]
-    L.xrdvi_debug_profile.argtypes = [vp, fp, C.c_int32, C.c_uint64, C.c_uint64, C.c_int64, fp, dp]
+    L.xrdvi_debug_profile.argtypes = [vp, fp, C.c_int32, C.c_uint64, C.c_uint64, C.c_int64, fp, dp, vp, C.c_size_t]
     L.xrdvi_debug_draws.argtypes = [vp, C.c_int32, C.c_uint64, C.c_uint64, C.c_int64, fp, C.POINTER(C.c_uint32),
-                                    C.POINTER(C.c_int32)]
+                                    C.POINTER(C.c_int32), vp, C.c_size_t]
     L.xrdvi_time_kernels.argtypes = [vp, C.c_int32, C.c_uint64, C.c_int32, fp]
-    L.xrdvi_bench_steps.argtypes = [vp, C.c_int32, C.c_int32, C.c_uint64, C.c_size_t, fp]
-    L.xrdvi_debug_timeline.argtypes = [vp, C.c_int32, C.c_uint64, C.c_int64, C.POINTER(C.c_uint64), C.POINTER(C.c_int64)]
-    L.xrdvi_pipe_rates.argtypes = [C.c_int, fp]
+    L.xrdvi_bench_steps.argtypes = [vp, C.c_int32, C.c_int32, C.c_uint64, vp, C.c_size_t, fp]
+    L.xrdvi_debug_timeline.argtypes = [vp, C.c_int32, C.c_uint64, C.c_int64, C.POINTER(C.c_uint64), C.POINTER(C.c_int64),
+                                       vp, C.c_size_t]
     L.xrdvi_last_error.restype = C.c_char_p
     _lib = L
     return L
@@ -115,9 +121,17 @@ def _d(a):
 
 
 def pipe_rates(device=0) -> dict:
-    """Measured per-SM per-clock pipe rates (xrdvi_pipe_rates)."""
+    """Measured per-SM per-clock pipe rates (xrdvi_pipe_rates, include/xrdvi_measure.h): the microbenchmark lives in
+    its own library, libxrdvi_measure.so (`python -m paper_2501_09308_b200.build --measure`), loaded only here."""
+    path = _PKG / "libxrdvi_measure.so"
+    if not path.exists():
+        raise XrdviError(-100, f"{path} not built; run `python -m paper_2501_09308_b200.build --measure`")
+    M = C.CDLL(str(path))
+    M.xrdvi_pipe_rates.argtypes = [C.c_int, C.POINTER(C.c_float)]
     r = np.zeros(9, dtype=np.float32)
-    _check(load_library().xrdvi_pipe_rates(int(device), _f(r)))
+    rc = M.xrdvi_pipe_rates(int(device), _f(r))
+    if rc != 0:
+        raise XrdviError(rc, "xrdvi_pipe_rates failed")
     names = ("ffma", "ffma2", "mufu_ex2", "mufu_rcp", "mix_forward", "mix_backward", "mix_ffma2", "mufu_ex2_rcp", "sm_mhz")
     return {k: float(v) for k, v in zip(names, r)}
 
@@ -125,7 +139,8 @@ def pipe_rates(device=0) -> dict:
 class Xrdvi:
     """One problem: P patterns x R restarts over a shared candidate library (xrdvi_create)."""
 
-    def __init__(self, two_theta, y, background, peak_ofs, peak_pos, peak_int, S_max, device=0, **hyper):
+    def __init__(self, two_theta, y, background, peak_ofs, peak_pos, peak_int, S_max, device=0, library_stream=False,
+                 **hyper):
         import torch  # device memory and stream only
 
         L = load_library()
@@ -148,20 +163,22 @@ class Xrdvi:
             raise XrdviError(-1, "xrdvi_workspace_bytes: invalid sizes")
         self.device = torch.device("cuda", device)
         self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
-        self.stream = torch.cuda.Stream(device=self.device)   # non-default: CUDA Graph capture needs it
+        # a non-default stream (CUDA Graph capture needs one); library_stream=True passes NULL and lets xrdvi_create
+        # make its own
+        self.stream = None if library_stream else torch.cuda.Stream(device=self.device)
         self._h = C.c_void_p()
         _check(L.xrdvi_create(_d(x), self.N, _d(yy), _d(bg), self.K, ofs.ctypes.data_as(C.POINTER(C.c_int64)),
                               _d(pos), _d(inten), C.byref(self.hyper), self.S_max, device,
-                              C.c_void_p(self.stream.cuda_stream), C.c_void_p(self.workspace.data_ptr()),
-                              nbytes, C.byref(self._h)))
+                              C.c_void_p(self.stream.cuda_stream if self.stream is not None else 0),
+                              C.c_void_p(self.workspace.data_ptr()), nbytes, C.byref(self._h)))
         self.workspace_bytes = nbytes
 
     @classmethod
-    def from_workload(cls, wl, S_max=None, device=0, **overrides):
+    def from_workload(cls, wl, S_max=None, device=0, library_stream=False, **overrides):
         hp = dict(wl.hyper)
         hp.update(overrides)
         return cls(wl.two_theta, wl.y, wl.background, wl.peak_ofs, wl.peak_pos, wl.peak_int,
-                   S_max=wl.S if S_max is None else S_max, device=device, **hp)
+                   S_max=wl.S if S_max is None else S_max, device=device, library_stream=library_stream, **hp)
 
     def close(self):
         if getattr(self, "_h", None) is not None and self._h.value:
@@ -188,8 +205,20 @@ class Xrdvi:
         return (self.P, self.R, 2, self.K, 4)
 
     # ---- state -----------------------------------------------------------------
-    def reset_state(self, seed=0):
-        _check(load_library().xrdvi_reset_state(self._h, int(seed)))
+    def reset_state(self, seed=0, restart_offset=0):
+        _check(load_library().xrdvi_reset_state_restart(self._h, int(seed), int(restart_offset)))
+
+    def get_optimizer_state(self):
+        m1 = np.empty(self._state_shape(), dtype=np.float32)
+        m2 = np.empty(self._state_shape(), dtype=np.float32)
+        n = C.c_int64()
+        _check(load_library().xrdvi_get_optimizer_state(self._h, _f(m1), _f(m2), C.byref(n)))
+        return m1, m2, int(n.value)
+
+    def set_optimizer_state(self, mom1, mom2, adam_steps):
+        m1 = np.ascontiguousarray(mom1, dtype=np.float32).reshape(self._state_shape())
+        m2 = np.ascontiguousarray(mom2, dtype=np.float32).reshape(self._state_shape())
+        _check(load_library().xrdvi_set_optimizer_state(self._h, _f(m1), _f(m2), int(adam_steps)))
 
     def get_state(self):
         st = np.empty(self._state_shape(), dtype=np.float32)
@@ -265,13 +294,23 @@ class Xrdvi:
         _check(load_library().xrdvi_posterior_summary(self._h, _d(out)))
         return out
 
-    # ---- debug / measurement ---------------------------------------------------
+    # ---- debug / measurement (include/xrdvi_debug.h) -----------------------------
+    def _scratch(self, nbytes):
+        """A device scratch tensor for the debug / measurement calls (the library allocates nothing itself)."""
+        import torch
+        if nbytes <= 0:
+            return None, None, 0
+        t = torch.empty(int(nbytes), dtype=torch.uint8, device=self.device)
+        return t, C.c_void_p(t.data_ptr()), int(nbytes)
+
     def debug_profile(self, n, state=None, S=None, seed=0, iteration=0, want_f=True):
         S = self.S_max if S is None else int(S)
         st = None if state is None else np.ascontiguousarray(state, dtype=np.float32).reshape(self._state_shape())
         f = np.empty((int(n), self.N), dtype=np.float32) if want_f else None
         ll = np.empty(int(n), dtype=np.float64)
-        _check(load_library().xrdvi_debug_profile(self._h, _f(st), S, int(seed), int(iteration), int(n), _f(f), _d(ll)))
+        scratch, ptr, nb = self._scratch(4 * int(n) * self.N if want_f else 0)
+        _check(load_library().xrdvi_debug_profile(self._h, _f(st), S, int(seed), int(iteration), int(n), _f(f), _d(ll),
+                                                  ptr, nb))
         return f, ll
 
     def debug_draws(self, n, S=None, seed=0, iteration=0, want_core=False):
@@ -279,9 +318,10 @@ class Xrdvi:
         eps = np.empty((int(n), self.K, 4), dtype=np.float32)
         raw = np.empty((int(n), self.K, 4), dtype=np.uint32)
         core = np.empty((int(n), self.K), dtype=np.int32) if want_core else None
+        scratch, ptr, nb = self._scratch(16 * self.P * self.R * ((S + 31) // 32) * 32 * self.K)
         _check(load_library().xrdvi_debug_draws(
             self._h, S, int(seed), int(iteration), int(n), _f(eps), raw.ctypes.data_as(C.POINTER(C.c_uint32)),
-            core.ctypes.data_as(C.POINTER(C.c_int32)) if want_core else None))
+            core.ctypes.data_as(C.POINTER(C.c_int32)) if want_core else None, ptr, nb))
         return (eps, raw, core) if want_core else (eps, raw)
 
     def time_kernels(self, S=None, seed=0, reps=20):
@@ -296,12 +336,14 @@ class Xrdvi:
         S = self.S_max if S is None else int(S)
         rows = np.zeros((int(capacity), 4), dtype=np.uint64)
         n = C.c_int64(0)
+        scratch, ptr, nb = self._scratch(32 * int(capacity))
         _check(load_library().xrdvi_debug_timeline(self._h, S, int(seed), int(capacity),
-                                                   rows.ctypes.data_as(C.POINTER(C.c_uint64)), C.byref(n)))
+                                                   rows.ctypes.data_as(C.POINTER(C.c_uint64)), C.byref(n), ptr, nb))
         return rows[: n.value]
 
     def bench_steps(self, steps, S=None, seed=0, l2_flush_bytes=0):
         S = self.S_max if S is None else int(S)
         ms = np.empty(int(steps), dtype=np.float32)
-        _check(load_library().xrdvi_bench_steps(self._h, int(steps), S, int(seed), int(l2_flush_bytes), _f(ms)))
+        scratch, ptr, nb = self._scratch(int(l2_flush_bytes))
+        _check(load_library().xrdvi_bench_steps(self._h, int(steps), S, int(seed), ptr, nb, _f(ms)))
         return ms

@@ -11,8 +11,9 @@ import subprocess
 PKG = pathlib.Path(__file__).resolve().parent
 CSRC = PKG / "csrc"
 LIB = PKG / "libxrdvi.so"
-SOURCES = [CSRC / "xrdvi.cu", CSRC / "pipe_rates.cu"]
-DEPS = SOURCES + [CSRC / "xrdvi_kernels.cuh", PKG.parent / "include" / "xrdvi.h"]
+SOURCES = [CSRC / "xrdvi.cu"]
+DEPS = SOURCES + [CSRC / "xrdvi_kernels.cuh", PKG.parent / "include" / "xrdvi.h", PKG.parent / "include" / "xrdvi_debug.h"]
+MEASURE_LIB = PKG / "libxrdvi_measure.so"      # pipe-rate microbenchmark: its own library, never loaded by the product
 
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-shared", "-cudart", "static"]
@@ -29,7 +30,15 @@ def build(force: bool = False, verbose: bool = False, tuning: bool = False, defi
     return LIB
 
 
+def build_measure() -> pathlib.Path:
+    """nvcc the pipe-rate microbenchmark (csrc/pipe_rates.cu, include/xrdvi_measure.h) into libxrdvi_measure.so."""
+    subprocess.run(["nvcc", *NVCC_FLAGS, "-o", str(MEASURE_LIB), str(CSRC / "pipe_rates.cu")], check=True)
+    return MEASURE_LIB
+
+
 if __name__ == "__main__":
     import sys
+    if "--measure" in sys.argv:
+        print(build_measure())
     print(build(force=True, verbose="-v" in sys.argv, tuning="--tuning" in sys.argv,
                 defines=tuple(a[2:] for a in sys.argv[1:] if a.startswith("-D"))))

@@ -3,7 +3,9 @@
 // (DESIGN.md "Roofline").  One CTA of 1024 threads per SM; every thread runs `iters` rounds of 8
 // independent dependency chains of one instruction kind; cycles come from clock64() inside the kernel,
 // so the figures are per SM clock, independent of the clock frequency.
-#include "../../include/xrdvi.h"
+#include "../../include/xrdvi_measure.h"
+
+enum { XRDVI_OK = 0, XRDVI_E_INVALID_ARG = -1, XRDVI_E_CUDA = -6, XRDVI_E_NOT_SM100 = -7 };   // as include/xrdvi.h
 
 #include <cuda_runtime.h>
 #include <string>

@@ -2,6 +2,7 @@
 // There is no CPU fallback anywhere in this file: every compute step is a kernel in
 // xrdvi_kernels.cuh; the host only validates, sorts and encodes the static tables at create.
 #include "../../include/xrdvi.h"
+#include "../../include/xrdvi_debug.h"
 #include "xrdvi_kernels.cuh"
 
 #include <algorithm>
@@ -55,25 +56,30 @@ long long window_points(const xrdvi_hyper* hyp, double step) {
 }
 
 // CTA shape of elbo_tile_kernel: TW tiles of 16 points per segment, PS shares of each tile's peak list
-// (TW * PS warps).  Many groups: no split.  Few groups (config 1: 8): split peak lists, so that the 148 SMs
-// still see several warps per scheduler.
-void choose_shape(int64_t N, int G_max, int* TW, int* PS) {
-    if (const char* e = std::getenv("XRDVI_TILE_SHAPE")) {   // tuning knob for sweeps: "TWxPS"
+// (TW * PS warps).  Many groups: no split.  Few groups (config 1: 8): split peak lists, so that the SMs still see
+// several warps per scheduler.  n_sm <= 0 (xrdvi_workspace_bytes, which knows no device): the decision for 256 SMs, whose
+// workspace bounds that of every smaller device (PS = 4 needs more than PS = 1).
+void choose_shape(int64_t N, int G_max, int n_sm, int* TW, int* PS) {
+#ifdef XRDVI_TUNING
+    if (const char* e = std::getenv("XRDVI_TILE_SHAPE")) {   // sweep knob of the measurement build: "TWxPS"
         int a = 0, b = 0;
         if (std::sscanf(e, "%dx%d", &a, &b) == 2 && (a == 1 || a == 2 || a == 4) && (b == 1 || b == 2 || b == 3 || b == 4 || b == 5 || b == 6 || b == 8) && a * b <= 16) {
             *TW = a; *PS = b;
             return;
         }
     }
-    // measured on B200 (profiles/r1_v5_shape_sweep.md): one tile per CTA is best everywhere; few tile-warps
-    // (configs 1 and 4: 2008 / 4008) want the peak lists split four ways, many (configs 2, 3: 1e6) no split
+#endif
+    // measured on B200 (profiles/r1_v5_shape_sweep.md, repeated with staged lists in profiles/r2_*): one tile per CTA
+    // is best everywhere; launches with fewer than 8 tile-warps per resident warp slot (configs 1 and 4: 2008 / 4008)
+    // want the peak lists split four ways, the others (configs 2, 3: 1e6) no split
     const long long tiles = (N + 15) / 16 * static_cast<long long>(G_max);   // warps at PS = 1
-    const long long resident = 148ll * 24;                                    // warps the GPU holds at 80 registers
+    const int sms = (n_sm <= 0 || n_sm > 256) ? 256 : n_sm;                   // no device: the largest count the bound covers
+    const long long resident = static_cast<long long>(sms) * 24;              // warps the GPU holds at 80 registers
     *TW = 1;
     *PS = tiles >= 8 * resident ? 1 : 4;
 }
 
-bool make_plan(int64_t N, int32_t K, int64_t M, int32_t S_max, double step, const xrdvi_hyper* hyp, Plan* pl) {
+bool make_plan(int64_t N, int32_t K, int64_t M, int32_t S_max, double step, const xrdvi_hyper* hyp, int n_sm, Plan* pl) {
     if (N < 2 || K < 1 || M < 1 || S_max < 1 || !hyp || !(step > 0.0)) return false;
     if (N > (1 << 28) || M > (1ll << 30) || K > (1 << 24)) return false;
     Plan p{};
@@ -86,7 +92,7 @@ bool make_plan(int64_t N, int32_t K, int64_t M, int32_t S_max, double step, cons
     p.gpi_max = p.S_pad / 32;
     p.G_max = p.PR * p.gpi_max;
     if (p.G_max > 65535 || p.PR > 65535) return false;  // grid.y limit
-    choose_shape(N, p.G_max, &p.TW, &p.PS);
+    choose_shape(N, p.G_max, n_sm, &p.TW, &p.PS);
     p.NW = p.TW * p.PS;
     p.SP = kPT * p.TW;
     p.n_seg = static_cast<int>((N + p.SP - 1) / p.SP);
@@ -295,6 +301,8 @@ struct xrdvi {
     std::vector<float> m_h0;   // per pattern initial m_h
     float m_w0 = 0.f;
     long long step_host = 0;   // mirror of ctl.step
+    long long adam_t0 = 0;     // mirror of ctl.adam_t0 (step count at which the Adam moments were last zeroed)
+    bool own_stream = false;   // the stream was created by xrdvi_create (caller passed 0)
     // CUDA Graph of one optimisation step, keyed by S
     cudaGraphExec_t graph_exec = nullptr;    // one step
     cudaGraphExec_t graph_execU = nullptr;   // kUnroll steps: programmatic launches also across step boundaries
@@ -367,8 +375,10 @@ void launch_k(void (*kernel)(KArgs...), dim3 grid, dim3 block, cudaStream_t st, 
 }
 
 bool use_split(const Dev& d) {
-    if (std::getenv("XRDVI_FUSED")) return false;            // A/B knobs for measurements
+#ifdef XRDVI_TUNING
+    if (std::getenv("XRDVI_FUSED")) return false;            // A/B knobs of the measurement build
     if (std::getenv("XRDVI_SPLIT")) return d.TW == 1 && d.PS > 1;
+#endif
     return d.TW == 1 && d.PS > 1 && d.split;
 }
 
@@ -378,12 +388,14 @@ void launch_tile(const Dev& d, cudaStream_t st, float* f_dbg, long long n_dbg, b
         const unsigned items = static_cast<unsigned>(d.n_tile) * d.PS * d.G;
         const unsigned grid = BWD ? 2 * items : items + static_cast<unsigned>(d.n_tile) * d.G;
         switch (d.PS) {
+            case 4: launch_k(elbo_split_kernel<4, BWD>, dim3(grid), dim3(32), st, pdl, d, f_dbg, n_dbg); break;
+#ifdef XRDVI_TUNING
             case 3: launch_k(elbo_split_kernel<3, BWD>, dim3(grid), dim3(32), st, pdl, d, f_dbg, n_dbg); break;
             case 2: launch_k(elbo_split_kernel<2, BWD>, dim3(grid), dim3(32), st, pdl, d, f_dbg, n_dbg); break;
-            case 4: launch_k(elbo_split_kernel<4, BWD>, dim3(grid), dim3(32), st, pdl, d, f_dbg, n_dbg); break;
             case 5: launch_k(elbo_split_kernel<5, BWD>, dim3(grid), dim3(32), st, pdl, d, f_dbg, n_dbg); break;
             case 6: launch_k(elbo_split_kernel<6, BWD>, dim3(grid), dim3(32), st, pdl, d, f_dbg, n_dbg); break;
             case 8: launch_k(elbo_split_kernel<8, BWD>, dim3(grid), dim3(32), st, pdl, d, f_dbg, n_dbg); break;
+#endif
             default: break;
         }
         return;
@@ -397,9 +409,12 @@ void launch_tile(const Dev& d, cudaStream_t st, float* f_dbg, long long n_dbg, b
             launch_k(elbo_tile_kernel<TW_, PS_, BWD, false>, grid, dim3(32 * TW_ * PS_), st, pdl, d, f_dbg, n_dbg); \
         break;
     switch (d.TW * 16 + d.PS) {
-        XRDVI_TILE_CASE(1, 1) XRDVI_TILE_CASE(1, 2) XRDVI_TILE_CASE(1, 3) XRDVI_TILE_CASE(1, 4) XRDVI_TILE_CASE(1, 5) XRDVI_TILE_CASE(1, 6) XRDVI_TILE_CASE(1, 8)
+        XRDVI_TILE_CASE(1, 1) XRDVI_TILE_CASE(1, 4)      // the shapes choose_shape selects
+#ifdef XRDVI_TUNING
+        XRDVI_TILE_CASE(1, 2) XRDVI_TILE_CASE(1, 3) XRDVI_TILE_CASE(1, 5) XRDVI_TILE_CASE(1, 6) XRDVI_TILE_CASE(1, 8)
         XRDVI_TILE_CASE(2, 1) XRDVI_TILE_CASE(2, 2) XRDVI_TILE_CASE(2, 4) XRDVI_TILE_CASE(2, 8)
         XRDVI_TILE_CASE(4, 1) XRDVI_TILE_CASE(4, 2) XRDVI_TILE_CASE(4, 4)
+#endif
         default: break;
     }
 #undef XRDVI_TILE_CASE
@@ -413,7 +428,11 @@ void launch_draw(const Dev& d, cudaStream_t st, const float* var, uint4* raw_out
 // the draws of the next step.  The draws of the FIRST step come from launch_draw.
 int enqueue_step(xrdvi* h) {
     const Dev& d = h->dev;
-    static const bool pdl = std::getenv("XRDVI_NO_PDL") == nullptr;    // A/B knob for measurements
+#ifdef XRDVI_TUNING
+    static const bool pdl = std::getenv("XRDVI_NO_PDL") == nullptr;    // A/B knob of the measurement build
+#else
+    const bool pdl = true;
+#endif
     // both kernels may start while their predecessor drains (programmatic dependent launch); each waits with
     // griddep_wait() before it touches the predecessor's data
     launch_tile<true>(d, h->stream, nullptr, 0, pdl);                  // also finishes the previous step (ELBO, count)
@@ -447,6 +466,7 @@ int write_ctl(xrdvi* h, uint64_t seed, long long step, long long trace_base, lon
     c.step = step;
     c.trace_base = trace_base;
     c.iteration_override = it_override;
+    c.adam_t0 = h->adam_t0;
     CU(cudaMemcpyAsync(h->dev.ctl, &c, sizeof(Ctl), cudaMemcpyHostToDevice, h->stream));
     CU(cudaStreamSynchronize(h->stream));  // c lives on this stack frame
     return XRDVI_OK;
@@ -488,7 +508,11 @@ int ensure_graph(xrdvi* h, int S) {
 
 // `n` optimisation steps: as many kUnroll-step graphs as fit, single-step graphs for the rest
 int launch_steps(xrdvi* h, int n) {
-    static const bool no_unroll = std::getenv("XRDVI_NO_UNROLL") != nullptr;   // A/B knob for measurements
+#ifdef XRDVI_TUNING
+    static const bool no_unroll = std::getenv("XRDVI_NO_UNROLL") != nullptr;   // A/B knob of the measurement build
+#else
+    const bool no_unroll = false;
+#endif
     int i = 0;
     if (!no_unroll)
         for (; i + kUnroll <= n; i += kUnroll) CU(cudaGraphLaunch(h->graph_execU, h->stream));
@@ -541,7 +565,7 @@ size_t xrdvi_workspace_bytes(int64_t N, int32_t K, int64_t M, int32_t S_max, dou
                              const xrdvi_hyper* hyp) {
     Plan pl;
     if (!hyp || hyp->size != sizeof(xrdvi_hyper)) return 0;
-    if (!make_plan(N, K, M, S_max, two_theta_step, hyp, &pl)) return 0;
+    if (!make_plan(N, K, M, S_max, two_theta_step, hyp, 0, &pl)) return 0;
     return pl.total;
 }
 
@@ -586,7 +610,7 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
     CU(cudaSetDevice(device));
 
     Plan pl;
-    if (!make_plan(N, K, M, S_max, delta, hyp, &pl)) return fail(XRDVI_E_INVALID_ARG, "sizes out of range");
+    if (!make_plan(N, K, M, S_max, delta, hyp, prop.multiProcessorCount, &pl)) return fail(XRDVI_E_INVALID_ARG, "sizes out of range");
     if (workspace_bytes < pl.total) return fail(XRDVI_E_WORKSPACE_TOO_SMALL, "workspace too small: need " + std::to_string(pl.total));
     if (reinterpret_cast<uintptr_t>(workspace) % 256) return fail(XRDVI_E_INVALID_ARG, "workspace not 256-byte aligned");
 
@@ -664,6 +688,11 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
     h->hyp = *hyp;
     h->device = device;
     h->stream = static_cast<cudaStream_t>(cuda_stream);
+    if (!h->stream) {   // the legacy default stream cannot be captured into a CUDA Graph: use a private non-blocking stream
+        cudaError_t se = cudaStreamCreateWithFlags(&h->stream, cudaStreamNonBlocking);
+        if (se != cudaSuccess) { delete h; return fail(XRDVI_E_CUDA, std::string("cudaStreamCreateWithFlags: ") + cudaGetErrorString(se)); }
+        h->own_stream = true;
+    }
     h->ws = static_cast<char*>(workspace);
     h->N = N; h->M = M; h->K = K; h->n_c = static_cast<int>(n_c);
     h->windowed = pl.n_c >= 0;
@@ -752,7 +781,7 @@ void xrdvi_destroy(xrdvi* h) {
     if (h->graph_exec) cudaGraphExecDestroy(h->graph_exec);
     if (h->graph_execU) cudaGraphExecDestroy(h->graph_execU);
     for (auto& e : h->ev) if (e) cudaEventDestroy(e);
-
+    if (h->own_stream) { cudaStreamSynchronize(h->stream); cudaStreamDestroy(h->stream); }
     delete h;
 }
 
@@ -837,13 +866,18 @@ int xrdvi_fit_adaptive(xrdvi* h, int32_t iterations, int32_t S, uint64_t seed, i
                      trace ? trace + static_cast<size_t>(done) * h->plan.PR : nullptr);
 }
 
-int xrdvi_reset_state(xrdvi* h, uint64_t seed) {
+int xrdvi_reset_state(xrdvi* h, uint64_t seed) { return xrdvi_reset_state_restart(h, seed, 0); }
+
+int xrdvi_reset_state_restart(xrdvi* h, uint64_t seed, int32_t restart_offset) {
     if (!h) return fail(XRDVI_E_INVALID_ARG, "null handle");
+    if (restart_offset < 0 || restart_offset > (1 << 30)) return fail(XRDVI_E_INVALID_ARG, "restart_offset out of range");
     CU(cudaSetDevice(h->device));
     init_state_kernel<<<h->plan.PR, 128, 0, h->stream>>>(h->dev, reinterpret_cast<const float*>(h->ws + h->plan.o_mh0),
-                                                          h->m_w0, static_cast<float>(h->hyp.init_log_sigma), seed);
+                                                          h->m_w0, static_cast<float>(h->hyp.init_log_sigma), seed,
+                                                          restart_offset);
     CU(cudaGetLastError());
     h->step_host = 0;
+    h->adam_t0 = 0;
     return write_ctl(h, 0, 0, 0, -1);
 }
 
@@ -866,7 +900,30 @@ int xrdvi_set_state(xrdvi* h, const float* var_params, int64_t step) {
     CU(cudaMemsetAsync(h->dev.mom1, 0, b, h->stream));
     CU(cudaMemsetAsync(h->dev.mom2, 0, b, h->stream));
     h->step_host = step;
+    h->adam_t0 = step;               // fresh moments: the bias correction restarts with them
     return write_ctl(h, 0, step, step, -1);
+}
+
+int xrdvi_get_optimizer_state(xrdvi* h, float* mom1, float* mom2, int64_t* adam_steps) {
+    if (!h) return fail(XRDVI_E_INVALID_ARG, "null handle");
+    CU(cudaSetDevice(h->device));
+    const size_t b = sizeof(float) * h->plan.PR * 8 * h->K;
+    if (mom1) CU(cudaMemcpyAsync(mom1, h->dev.mom1, b, cudaMemcpyDeviceToHost, h->stream));
+    if (mom2) CU(cudaMemcpyAsync(mom2, h->dev.mom2, b, cudaMemcpyDeviceToHost, h->stream));
+    CU(cudaStreamSynchronize(h->stream));
+    if (adam_steps) *adam_steps = h->step_host - h->adam_t0;
+    return XRDVI_OK;
+}
+
+int xrdvi_set_optimizer_state(xrdvi* h, const float* mom1, const float* mom2, int64_t adam_steps) {
+    if (!h || !mom1 || !mom2) return fail(XRDVI_E_INVALID_ARG, "null handle/moments");
+    if (adam_steps < 0 || adam_steps > h->step_host) return fail(XRDVI_E_INVALID_ARG, "adam_steps outside [0, step]");
+    CU(cudaSetDevice(h->device));
+    const size_t b = sizeof(float) * h->plan.PR * 8 * h->K;
+    CU(cudaMemcpyAsync(h->dev.mom1, mom1, b, cudaMemcpyHostToDevice, h->stream));
+    CU(cudaMemcpyAsync(h->dev.mom2, mom2, b, cudaMemcpyHostToDevice, h->stream));
+    h->adam_t0 = h->step_host - adam_steps;
+    return write_ctl(h, 0, h->step_host, h->step_host, -1);   // synchronises: the host buffers may go
 }
 
 // shared prologue of the evaluation entry points: stage var_params (or use the state), set S and the
@@ -977,21 +1034,24 @@ int xrdvi_posterior_summary(xrdvi* h, double* summary) {
 }
 
 int xrdvi_debug_profile(xrdvi* h, const float* var_params, int32_t S, uint64_t seed, uint64_t iteration,
-                        int64_t n, float* f, double* ll) {
+                        int64_t n, float* f, double* ll, void* scratch, size_t scratch_bytes) {
     const float* var = nullptr;
     int rc = begin_eval(h, var_params, S, seed, iteration, &var);
     if (rc) return rc;
     const long long T = static_cast<long long>(h->plan.PR) * S;
     if (n < 0 || n > T) return fail(XRDVI_E_INVALID_ARG, "n out of range");
     float* f_dev = nullptr;
-    if (f && n > 0) CU(cudaMalloc(&f_dev, sizeof(float) * n * h->N));  // debug path only
+    if (f && n > 0) {
+        if (!scratch || scratch_bytes < sizeof(float) * static_cast<size_t>(n) * h->N)
+            return fail(XRDVI_E_WORKSPACE_TOO_SMALL, "debug_profile: scratch smaller than n * N floats");
+        f_dev = static_cast<float*>(scratch);
+    }
     rc = enqueue_eval(h, var, f_dev, n, true);
-    if (rc) { cudaFree(f_dev); return rc; }
+    if (rc) return rc;
     std::vector<double> llh(static_cast<size_t>(h->plan.PR) * h->plan.S_pad);
     cudaError_t e = cudaMemcpyAsync(llh.data(), h->dev.ll_t, sizeof(double) * llh.size(), cudaMemcpyDeviceToHost, h->stream);
     if (e == cudaSuccess && f_dev) e = cudaMemcpyAsync(f, f_dev, sizeof(float) * n * h->N, cudaMemcpyDeviceToHost, h->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
-    cudaFree(f_dev);
     if (e != cudaSuccess) return fail(XRDVI_E_CUDA, std::string("debug_profile: ") + cudaGetErrorString(e));
     if (ll) {
         const int gpi32 = h->dev.gpi * 32;
@@ -1001,7 +1061,7 @@ int xrdvi_debug_profile(xrdvi* h, const float* var_params, int32_t S, uint64_t s
 }
 
 int xrdvi_debug_draws(xrdvi* h, int32_t S, uint64_t seed, uint64_t iteration, int64_t n, float* eps, uint32_t* raw,
-                      int32_t* core_halfwidth) {
+                      int32_t* core_halfwidth, void* scratch, size_t scratch_bytes) {
     const float* var = nullptr;
     int rc = begin_eval(h, nullptr, S, seed, iteration, &var);
     if (rc) return rc;
@@ -1009,8 +1069,9 @@ int xrdvi_debug_draws(xrdvi* h, int32_t S, uint64_t seed, uint64_t iteration, in
     if (n < 0 || n > T || !eps) return fail(XRDVI_E_INVALID_ARG, "n out of range or eps NULL");
     const Dev& d = h->dev;
     const size_t cnt = static_cast<size_t>(d.G) * d.K * 32;
-    uint4* raw_dev = nullptr;
-    CU(cudaMalloc(&raw_dev, sizeof(uint4) * cnt));  // debug path only
+    if (!scratch || scratch_bytes < sizeof(uint4) * cnt)
+        return fail(XRDVI_E_WORKSPACE_TOO_SMALL, "debug_draws: scratch smaller than 16 bytes per (draw slot, phase)");
+    uint4* raw_dev = static_cast<uint4*>(scratch);
     launch_draw(d, h->stream, var, raw_dev);
     std::vector<float4> eh(cnt);
     std::vector<uint4> rh(cnt);
@@ -1020,7 +1081,6 @@ int xrdvi_debug_draws(xrdvi* h, int32_t S, uint64_t seed, uint64_t iteration, in
     if (e == cudaSuccess) e = cudaMemcpyAsync(rh.data(), raw_dev, sizeof(uint4) * cnt, cudaMemcpyDeviceToHost, h->stream);
     if (e == cudaSuccess) e = cudaMemcpyAsync(ngh.data(), d.ng, sizeof(int) * ngh.size(), cudaMemcpyDeviceToHost, h->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
-    cudaFree(raw_dev);
     if (e != cudaSuccess) return fail(XRDVI_E_CUDA, std::string("debug_draws: ") + cudaGetErrorString(e));
     for (long long t = 0; t < n; ++t) {
         const int inst = static_cast<int>(t / S), s = static_cast<int>(t % S);
@@ -1115,7 +1175,8 @@ int xrdvi_time_kernels(xrdvi* h, int32_t S, uint64_t seed, int32_t reps, float* 
     return XRDVI_OK;
 }
 
-int xrdvi_debug_timeline(xrdvi* h, int32_t S, uint64_t seed, int64_t capacity, uint64_t* rows, int64_t* n_rows) {
+int xrdvi_debug_timeline(xrdvi* h, int32_t S, uint64_t seed, int64_t capacity, uint64_t* rows, int64_t* n_rows,
+                         void* scratch, size_t scratch_bytes) {
     int rc = check_S(h, S);
     if (rc) return rc;
     if (!rows || !n_rows || capacity < 1) return fail(XRDVI_E_INVALID_ARG, "rows / n_rows NULL or capacity < 1");
@@ -1127,8 +1188,9 @@ int xrdvi_debug_timeline(xrdvi* h, int32_t S, uint64_t seed, int64_t capacity, u
     Dev d = h->dev;                                       // a copy with the stamp buffer attached
     const long long warps = use_split(d) ? 2ll * d.n_tile * d.PS * d.G : static_cast<long long>(d.n_seg) * d.G * d.TW * d.PS;
     if (warps > capacity) return fail(XRDVI_E_INVALID_ARG, "capacity < warps of the launch");
-    unsigned long long* buf = nullptr;
-    CU(cudaMalloc(&buf, sizeof(unsigned long long) * 4 * warps));   // measurement path only
+    if (!scratch || scratch_bytes < sizeof(unsigned long long) * 4 * static_cast<size_t>(warps))
+        return fail(XRDVI_E_WORKSPACE_TOO_SMALL, "debug_timeline: scratch smaller than 32 bytes per warp of the launch");
+    unsigned long long* buf = static_cast<unsigned long long*>(scratch);
     cudaStream_t st = h->stream;
     cudaError_t e = cudaSuccess;
     for (int pass = 0; pass < 3 && e == cudaSuccess; ++pass) {       // two warm-up passes, the third is stamped
@@ -1141,21 +1203,19 @@ int xrdvi_debug_timeline(xrdvi* h, int32_t S, uint64_t seed, int64_t capacity, u
     }
     if (e == cudaSuccess) e = cudaMemcpyAsync(rows, buf, sizeof(unsigned long long) * 4 * warps, cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-    cudaFree(buf);
     if (e != cudaSuccess) return fail(XRDVI_E_CUDA, std::string("debug_timeline: ") + cudaGetErrorString(e));
     *n_rows = warps;
     return enqueue_finish(h) ? XRDVI_E_CUDA : XRDVI_OK;
 }
 
-int xrdvi_bench_steps(xrdvi* h, int32_t steps, int32_t S, uint64_t seed, size_t flush_bytes, float* ms_steps) {
+int xrdvi_bench_steps(xrdvi* h, int32_t steps, int32_t S, uint64_t seed, void* flush, size_t flush_bytes, float* ms_steps) {
     int rc = check_S(h, S);
     if (rc) return rc;
     if (steps < 1 || !ms_steps) return fail(XRDVI_E_INVALID_ARG, "steps < 1 or ms_steps NULL");
     CU(cudaSetDevice(h->device));
     rc = begin_steps(h, S, seed);
     if (rc) return rc;
-    void* flush = nullptr;
-    if (flush_bytes) CU(cudaMalloc(&flush, flush_bytes));  // measurement path only
+    if (!flush) flush_bytes = 0;
     std::vector<cudaEvent_t> ev(2 * static_cast<size_t>(steps), nullptr);
     cudaError_t e = cudaSuccess;
     for (auto& x : ev) if (e == cudaSuccess) e = cudaEventCreate(&x);
@@ -1171,7 +1231,6 @@ int xrdvi_bench_steps(xrdvi* h, int32_t steps, int32_t S, uint64_t seed, size_t 
     h->step_host += steps;
     for (int i = 0; i < steps && e == cudaSuccess; ++i) e = cudaEventElapsedTime(&ms_steps[i], ev[2 * i], ev[2 * i + 1]);
     for (auto& x : ev) if (x) cudaEventDestroy(x);
-    if (flush) cudaFree(flush);
     if (e != cudaSuccess) return fail(XRDVI_E_CUDA, std::string("bench_steps: ") + cudaGetErrorString(e));
     return XRDVI_OK;
 }

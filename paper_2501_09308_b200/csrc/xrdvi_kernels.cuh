@@ -74,6 +74,7 @@ struct Ctl {       // device-resident control block (so that graph replays need 
     long long step;        // completed optimisation steps
     long long trace_base;  // step index of trace row 0
     long long iteration_override;  // >= 0: Philox iteration for elbo_grad/debug; < 0: use step + 1
+    long long adam_t0;             // step count at which the Adam moments were last zeroed: bias correction uses step + 1 - adam_t0
     unsigned int pending;          // update_draw_kernel has run and finish_step has not: 1 evaluation, 2 step
     unsigned int ticket;           // next work item of elbo_split_kernel (re-armed by the launch's last CTA)
     unsigned int finished;         // CTAs of the current elbo_split_kernel launch that are done
@@ -1112,6 +1113,13 @@ __global__ void __launch_bounds__(kUpdThreads) update_draw_kernel(const Dev d, c
             // eight interleaved partial sums (independent load/add chains), combined in a fixed order
             double a8[8] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
             int t = 0;
+            for (; t + 32 <= d.n_seg; t += 32) {           // 32 loads in flight, added in the order of the loop below
+                float x[32];
+#pragma unroll
+                for (int j = 0; j < 32; ++j) x[j] = lp[static_cast<size_t>(t + j) * 32];
+#pragma unroll
+                for (int j = 0; j < 32; ++j) a8[j & 7] += static_cast<double>(x[j]);
+            }
             for (; t + 8 <= d.n_seg; t += 8) {
 #pragma unroll
                 for (int j = 0; j < 8; ++j) a8[j] += static_cast<double>(lp[static_cast<size_t>(t + j) * 32]);
@@ -1134,13 +1142,28 @@ __global__ void __launch_bounds__(kUpdThreads) update_draw_kernel(const Dev d, c
         // likelihood part: partials of phase k, all groups of the instance
         const int s0 = d.slot_ofs[k], s1 = d.slot_ofs[k + 1];
         const int n_sl = s1 - s0;
-        for (int idx = threadIdx.x; idx < n_sl * d.gpi; idx += kUpdThreads) {
-            const int gi = idx / n_sl, sl = s0 + (idx - gi * n_sl);
-            const float4* __restrict__ pp = reinterpret_cast<const float4*>(
-                d.part8 + (static_cast<size_t>(inst * d.gpi + gi) * d.n_slots + sl) * 8);
-            const float4 a = pp[0], b = pp[1];
-            v[0] += a.x; v[1] += a.y; v[2] += a.z; v[3] += a.w;
-            v[4] += b.x; v[5] += b.y; v[6] += b.z; v[7] += b.w;
+        const int n_part = n_sl * d.gpi;
+        for (int idx0 = threadIdx.x; idx0 < n_part; idx0 += 4 * kUpdThreads) {   // four slots in flight per thread,
+            float4 a[4], b[4];                                                    // added in increasing slot order
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const int idx = idx0 + u * kUpdThreads;
+                a[u] = b[u] = make_float4(0.f, 0.f, 0.f, 0.f);
+                if (idx < n_part) {
+                    const int gi = idx / n_sl, sl = s0 + (idx - gi * n_sl);
+                    const float4* __restrict__ pp = reinterpret_cast<const float4*>(
+                        d.part8 + (static_cast<size_t>(inst * d.gpi + gi) * d.n_slots + sl) * 8);
+                    a[u] = pp[0];
+                    b[u] = pp[1];
+                }
+            }
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                if (idx0 + u * kUpdThreads < n_part) {
+                    v[0] += a[u].x; v[1] += a[u].y; v[2] += a[u].z; v[3] += a[u].w;
+                    v[4] += b[u].x; v[5] += b[u].y; v[6] += b[u].z; v[7] += b[u].w;
+                }
+            }
         }
         // prior + Jacobian part, per draw
         for (int s = threadIdx.x; s < d.S; s += kUpdThreads) {
@@ -1182,7 +1205,7 @@ __global__ void __launch_bounds__(kUpdThreads) update_draw_kernel(const Dev d, c
                 if (d.optimizer == 1) {   // natural-gradient ascent: Fisher metric diag(1/sigma^2, 2) (R25)
                     x += d.lr * (is_l ? 0.5f * gj : sgc * sgc * gj);
                 } else {                  // Adam ascent, bias-corrected (R10)
-                    const float stepf = static_cast<float>(step + 1);
+                    const float stepf = static_cast<float>(step + 1 - d.ctl->adam_t0);
                     const float bc1 = 1.0f - powf(d.beta1, stepf);
                     const float bc2 = 1.0f - powf(d.beta2, stepf);
                     const float m1 = d.beta1 * d.mom1[o] + (1.0f - d.beta1) * gj;
@@ -1294,9 +1317,10 @@ __global__ void __launch_bounds__(128) posterior_summary_kernel(const Dev d, dou
 
 // R11 initial state.  grid PR, block 128 over phases.
 __global__ void __launch_bounds__(128) init_state_kernel(const Dev d, const float* __restrict__ m_h0 /*[P]*/,
-                                                         float m_w0, float init_log_sigma, unsigned long long seed) {
+                                                         float m_w0, float init_log_sigma, unsigned long long seed,
+                                                         int restart_offset) {
     const int inst = blockIdx.x;
-    const int pat = inst / d.R, rst = inst - pat * d.R;
+    const int pat = inst / d.R, rst = inst - pat * d.R + restart_offset;   // the restart index the jitter is drawn for
     for (int k = threadIdx.x; k < d.K; k += 128) {
         float4 m = make_float4(m_h0[pat], 0.0f, m_w0, 0.0f);
         if (rst > 0) {

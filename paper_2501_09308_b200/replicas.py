@@ -9,11 +9,13 @@ from __future__ import annotations
 
 
 def replica_seeds(rank: int, base_seed: int = 1) -> dict:
-    """Seeds of replica `rank`: restart jitter (xrdvi_reset_state) and Philox key (xrdvi_fit).
-    Rank 0 with base_seed 1 reproduces the single-GPU run."""
+    """What makes replica `rank` its own restart: `restart_offset` = rank shifts the restart index the R11 jitter is
+    drawn for (xrdvi_reset_state_restart: rank > 0 starts from a jittered state even with one restart per handle),
+    `state_seed` keys that jitter, `draw_seed` is the Philox key of the fit (xrdvi_fit).  Rank 0 with base_seed 1
+    reproduces the single-GPU run (offset 0: no jitter)."""
     if rank < 0:
         raise ValueError("rank < 0")
-    return {"state_seed": int(rank), "draw_seed": int(base_seed) + int(rank)}
+    return {"state_seed": 0, "restart_offset": int(rank), "draw_seed": int(base_seed) + int(rank)}
 
 
 def max_over_ranks(value: float, dist=None, device=None) -> float:

@@ -351,34 +351,98 @@ def test_extreme_widths_shifts_and_mixing():
 
 
 # --------------------------------------------------------------------------- split (ticket-queue) tile kernel
-def test_split_kernel_matches_oracle_and_the_fused_kernel_bitwise(monkeypatch):
-    """elbo_split_kernel (one-warp work items, partial profiles through L2) is chosen for long work items
-    (config 4 at full size); XRDVI_SPLIT=1 forces it on small problems.  Same summation orders as the fused
-    kernel, so the two must agree bit for bit, whatever the schedule."""
-    outs = {}
-    for mode in ("fused", "split"):
-        monkeypatch.delenv("XRDVI_SPLIT", raising=False)
-        monkeypatch.delenv("XRDVI_FUSED", raising=False)
-        monkeypatch.setenv("XRDVI_SPLIT" if mode == "split" else "XRDVI_FUSED", "1")
-        wl = synth.make_workload(1, S=96)
-        o = orc.from_workload(wl)
+def test_split_kernel_on_long_work_items():
+    """elbo_split_kernel (one-warp work items, partial profiles through L2) is what the library selects when a share
+    of a tile's list holds >= 512 records (config 4 at full size).  Config 4 with K = 150 reaches that on a problem the
+    oracle finishes in seconds (668 records per share, window +-400 points); K = 60 (test_config4_reduced_library) and
+    config 1 take the fused kernel.  Parity at two states, determinism across two handles, Poisson."""
+    wl = synth.make_workload(4, K=150, S=8)
+    o = orc.from_workload(wl)
+    outs = []
+    for rep in range(2):
         gpu = Xrdvi.from_workload(wl)
+        assert gpu.pair_count == o.pair_count() and gpu.pair_count // (((wl.N + 15) // 16) * 4 * 16) >= 512
         st0, _ = gpu.get_state()
-        check_eval(gpu, o, st0, 96, seed=1, iteration=1)
-        st, inc, tr = gpu.fit(30, seed=3, want_trace=True)
-        e, g = gpu.elbo_grad(S=96, seed=3, iteration=99)
-        e40, g40 = gpu.elbo_grad(S=40, seed=3, iteration=5)               # ragged group, fewer groups than S_max
-        ll, lpj, gz = gpu.logjoint_grad(synth.random_state(wl.K, 5, 1, seed=2)[:, 0, 0])
-        outs[mode] = (st, inc, tr, e, g, e40, g40, ll, gz)
-        check_eval(gpu, o, st, 96, seed=3, iteration=31)
+        if rep == 0:
+            check_eval(gpu, o, st0, 8, seed=6, iteration=2, n_prof=2)
+        st, inc, tr = gpu.fit(12, seed=3, want_trace=True)
+        e, g = gpu.elbo_grad(S=8, seed=3, iteration=99)
+        e5, g5 = gpu.elbo_grad(S=5, seed=3, iteration=5)                  # ragged group
+        outs.append((st, inc, tr, e, g, e5, g5))
+        if rep == 0:
+            check_eval(gpu, o, st, 8, seed=3, iteration=13, n_prof=2)
         gpu.close()
-        wl0 = synth.make_workload(0, peak_counts=1.0e4)                    # K = 6 < ... shares, Poisson, ragged last tile
-        o0, g0 = orc.from_workload(wl0), Xrdvi.from_workload(wl0)
-        s0, _ = g0.get_state()
-        check_eval(g0, o0, s0, wl0.S, seed=2, iteration=1, n_prof=4)
-        g0.close()
-    for a, b in zip(outs["fused"], outs["split"]):
+    for a, b in zip(outs[0], outs[1]):
         np.testing.assert_array_equal(a, b)
+
+
+# --------------------------------------------------------------------------- checkpoint / resume, restarts, streams
+def test_checkpoint_resume_is_bitwise_the_uninterrupted_fit():
+    """fit(n) + get_state + get_optimizer_state, then set_state + set_optimizer_state + fit(m) on ANOTHER handle of
+    the same problem equals fit(n + m) bit for bit (set_state alone restarts Adam)."""
+    wl = synth.make_workload(1, S=64, K=10)
+    ref = Xrdvi.from_workload(wl)
+    st_ref, inc_ref, _ = ref.fit(37, seed=9)
+    a = Xrdvi.from_workload(wl)
+    a.fit(21, seed=9)
+    st, step = a.get_state()
+    m1, m2, adam_steps = a.get_optimizer_state()
+    assert step == 21 and adam_steps == 21 and np.abs(m2).max() > 0
+    b = Xrdvi.from_workload(wl)
+    b.set_state(st, step)
+    b.set_optimizer_state(m1, m2, adam_steps)
+    st_b, inc_b, _ = b.fit(16, seed=9)
+    np.testing.assert_array_equal(st_b, st_ref)
+    np.testing.assert_array_equal(inc_b, inc_ref)
+    from paper_2501_09308_b200 import XrdviError
+    with pytest.raises(XrdviError):
+        b.set_optimizer_state(m1, m2, 99)                         # more Adam steps than completed steps
+
+
+def test_set_state_alone_starts_a_fresh_adam():
+    """set_state zeroes the moments AND restarts the bias correction: the steps after it are the oracle's Adam steps
+    1, 2, ... from zero moments on the draws of iterations step + 1, step + 2, ..."""
+    wl = synth.make_workload(0)
+    o = orc.from_workload(wl)
+    gpu = Xrdvi.from_workload(wl)
+    gpu.fit(30, seed=5)
+    st, step = gpu.get_state()
+    gpu.set_state(st, step)
+    assert gpu.get_optimizer_state()[2] == 0
+    st_g, _, _ = gpu.fit(3, seed=5)
+    ref = st.astype(np.float64)
+    m1, m2 = np.zeros_like(ref), np.zeros_like(ref)
+    for it in range(3):
+        _, grad = o.elbo_grad(ref, wl.S, 5, step + 1 + it)
+        ref = o.adam_step(ref, grad, m1, m2, it + 1)
+    np.testing.assert_allclose(st_g, ref, atol=2e-3)
+    first = Xrdvi.from_workload(wl)
+    first.set_state(st, step)
+    st1, _, _ = first.fit(1, seed=5)
+    np.testing.assert_allclose(np.abs(st1 - st)[0, 0, 0], 0.1, rtol=2e-3)   # fresh Adam: first step = lr * sign(g)
+
+
+def test_restart_offset_draws_the_jitter_of_a_later_restart():
+    wl1, wl3 = synth.make_workload(0), synth.make_workload(0, n_restarts=3)
+    o3 = orc.from_workload(wl3)
+    gpu = Xrdvi.from_workload(wl1)
+    ref = o3.init_state(seed=9)
+    for off in (0, 1, 2):
+        gpu.reset_state(seed=9, restart_offset=off)
+        st, _ = gpu.get_state()
+        np.testing.assert_allclose(st[0, 0], ref[0, off], rtol=2e-6, atol=2e-7)
+    assert np.abs(ref[0, 2, 0] - ref[0, 0, 0]).min() > 0
+
+
+def test_library_owned_stream_when_null_is_passed():
+    """A C caller may pass stream 0: the legacy default stream cannot be captured into a CUDA Graph, so xrdvi_create
+    makes a private stream; results equal those on a caller-provided stream."""
+    wl = synth.make_workload(0)
+    a, b = Xrdvi.from_workload(wl), Xrdvi.from_workload(wl, library_stream=True)
+    ra, rb = a.fit(25, seed=4, want_trace=True), b.fit(25, seed=4, want_trace=True)
+    for x, y in zip(ra, rb):
+        np.testing.assert_array_equal(x, y)
+    b.close()
 
 
 def test_two_handles_interleaved_and_resumed_fit():

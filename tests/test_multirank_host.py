@@ -57,7 +57,8 @@ def test_two_rank_gloo_replica_logic(tmp_path):
     outs.sort(key=lambda o: o["rank"])
     assert [o["world"] for o in outs] == [2, 2]
     assert outs[0]["seeds"] != outs[1]["seeds"]                    # replicas are different restarts
-    assert outs[0]["seeds"] == {"state_seed": 0, "draw_seed": 1}   # rank 0 = the single-GPU run
+    assert outs[0]["seeds"] == {"state_seed": 0, "restart_offset": 0, "draw_seed": 1}   # rank 0 = the single-GPU run
+    assert outs[1]["seeds"]["restart_offset"] == 1                 # rank 1 starts from restart 1's jittered state
     assert outs[0]["t_max"] == outs[1]["t_max"] == 2.5             # max over ranks, on every rank
     assert outs[0]["rate"] == pytest.approx(2 * 1000.0 / 2.5)      # all ranks' units / slowest time
 
