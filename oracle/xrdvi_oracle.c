@@ -26,6 +26,9 @@
  *   summary   marginals of q in the constrained parameters (mean, sd, 2.5/50/97.5 % quantiles; reading R28,
  *             the Fig. 6 marginals, SURVEY 8(f) NEXT-4 second half); pins: tests/test_posterior_summary_pins.py
  *   draws     Philox4x32-10, counter (iter, s, k, inst), key (seed_lo, seed_hi) (R18)
+ *   asymmetry split width w A(x; alpha_k) on the high-angle side (A9/A10 PAPER.md:234-239), alpha_k ~ Norm(1, 0.2)
+ *             (B.2 PAPER.md:274), optional w_k sec(p_m / 2) (the sec of): reading R30, hyper.asymmetry /
+ *             hyper.width_sec; pins: tests/test_asymmetry_pins.py
  *   adaptive  per-phase window half-widths n_c,k <= n_c refreshed from the variational means
  *             (reading R27; north_star's "problem-defined +-W FWHM cutoff")
  *
@@ -38,9 +41,10 @@
  * The absolute ELBO (all constants, Jacobians, entropy) is pinned as a lower bound on the exact log evidence
  * over the scales h with the nuisances frozen, gap 1.8 nats after a fit (tests/test_bruteforce_subsets.py).
  *
- * Layouts: state[P][R][2][K][4] doubles: [0]=m (variational mean), [1]=l (log sigma);
- * the 4 latent classes are ordered (h, mu, w, r) in unconstrained space zeta:
- *   h = exp(zeta_h), mu = zeta_mu, w = exp(zeta_w), r = 1/(1+exp(-zeta_r)).
+ * Layouts: state[P][R][2][K][C] doubles: [0]=m (variational mean), [1]=l (log sigma);
+ * the C = 4 latent classes are ordered (h, mu, w, r) in unconstrained space zeta:
+ *   h = exp(zeta_h), mu = zeta_mu, w = exp(zeta_w), r = 1/(1+exp(-zeta_r));
+ * hyper.asymmetry = 1 (R30) adds a fifth, alpha = exp(zeta_alpha): C = 5.
  */
 #include <math.h>
 #include <stdint.h>
@@ -63,6 +67,9 @@ typedef struct {
     int32_t n_patterns, n_restarts;
     int32_t likelihood;    /* 0 Gaussian with known sigma_n (R3); 1 Poisson, A12-A16 PAPER.md:247-261 (R24) */
     int32_t optimizer;     /* 0 Adam (R10); 1 natural-gradient ascent of the mean-field Gaussian (R25)       */
+    int32_t asymmetry;     /* 1: fifth latent alpha_k, split width w A(x; alpha_k) (A9/A10 PAPER.md:234-239; R30)    */
+    int32_t width_sec;     /* 1: angle-dependent width w_k sec(p_m / 2) (the sec of; R30)               */
+    double alpha_mu, alpha_sigma;   /* prior alpha_k ~ Norm(1.00, 0.20), PAPER.md:274 (B.2)                          */
 } orc_hyper;
 
 typedef struct {
@@ -70,6 +77,7 @@ typedef struct {
     int32_t K;
     int64_t M;
     int32_t P, R;
+    int32_t C;             /* latent classes per phase: 4 (h, mu, w, r), 5 with the asymmetry alpha (R30) */
     double *x;             /* [N]                                            */
     double *y, *B;         /* [P][N]                                         */
     int64_t *ofs;          /* [K+1]                                          */
@@ -127,6 +135,16 @@ void orc_eps(uint64_t seed, uint64_t iteration, uint32_t inst, uint32_t s, uint3
     eps[3] = r1 * sin(2.0 * M_PI * u3);
 }
 
+/* R30: the normal of the fifth latent (asymmetry) of (iteration, s, k, inst): a second Philox call with bit 31 of the
+ * phase word set, eps_alpha = first Box-Muller output of its words (u0, u1). */
+double orc_eps_alpha(uint64_t seed, uint64_t iteration, uint32_t inst, uint32_t s, uint32_t k) {
+    uint32_t ctr[4] = {(uint32_t)iteration, s, k | 0x80000000u, inst};
+    uint32_t key[2] = {(uint32_t)seed, (uint32_t)(seed >> 32)};
+    uint32_t w[4];
+    orc_philox4x32_10(ctr, key, w);
+    return sqrt(-2.0 * log(uniform23(w[0]))) * cos(2.0 * M_PI * uniform23(w[1]));
+}
+
 /* ------------------------------------------------------------------ problem set-up */
 void orc_destroy(orc_problem *q) {
     if (!q) return;
@@ -147,6 +165,7 @@ orc_problem *orc_create(const double *x, int64_t N, const double *y, const doubl
     orc_problem *q = (orc_problem *)calloc(1, sizeof(orc_problem));
     q->hy = *hy;
     q->N = N; q->K = K; q->M = ofs[K];
+    q->C = hy->asymmetry ? 5 : 4;
     q->P = hy->n_patterns > 0 ? hy->n_patterns : 1;
     q->R = hy->n_restarts > 0 ? hy->n_restarts : 1;
     q->x = (double *)dup_mem(x, sizeof(double) * N);
@@ -184,6 +203,7 @@ orc_problem *orc_create(const double *x, int64_t N, const double *y, const doubl
 int64_t orc_window_halfwidth(const orc_problem *q) { return q->n_c; }
 double orc_sigma_n(const orc_problem *q, int32_t pat) { return q->sigma_n[pat]; }
 double orc_lambda_h(const orc_problem *q, int32_t pat) { return q->lambda_h[pat]; }
+int32_t orc_classes(const orc_problem *q) { return q->C; }
 
 /* R16: pair (m,i), m a peak of phase k, is in the model iff |i - j_m| <= n_c and 0 <= i < N (dense: every
  * i).  R27: with per-phase half-widths set, n_c is replaced by n_c,k.  The loops below run i over exactly
@@ -217,6 +237,8 @@ int orc_set_phase_windows(orc_problem *q, const int64_t *n_ck) {
     return 0;
 }
 
+static double sec_factor(const orc_problem *q, int64_t m);
+
 /* R27, the refresh rule: the window of phase k must hold +-W FWHM around the SHIFTED peak centre p_m + mu_k
  * while staying centred on the table position j_m, with FWHM and shift at their variational means
  * wbar = E_q[w_k] = exp(m_w + s_w^2/2), mubar = m_mu, the widest over the (pattern, restart) instances:
@@ -225,13 +247,21 @@ int orc_set_phase_windows(orc_problem *q, const int64_t *n_ck) {
  *                               by the grid and the window never shrinks below that). */
 void orc_adaptive_halfwidths(const orc_problem *q, const double *state, double W, int64_t *n_ck) {
     const int32_t K = q->K;
+    const int C = q->C;
     const int64_t n_min = (int64_t)ceil(2.0 * W - 1e-9);
     for (int32_t k = 0; k < K; ++k) {
         double c = 0.0;
+        double smax = 1.0;                   /* R30: the widest peak of the phase under the sec term */
+        for (int64_t m = q->ofs[k]; m < q->ofs[k + 1]; ++m) if (sec_factor(q, m) > smax) smax = sec_factor(q, m);
         for (int32_t inst = 0; inst < q->P * q->R; ++inst) {
-            const double *m = state + (size_t)inst * 2 * K * 4, *l = m + (size_t)K * 4;
-            double s_w = exp(l[4 * k + 2]);
-            double ci = W * exp(m[4 * k + 2] + 0.5 * s_w * s_w) + fabs(m[4 * k + 1]);
+            const double *m = state + (size_t)inst * 2 * K * C, *l = m + (size_t)K * C;
+            double s_w = exp(l[C * k + 2]);
+            double wbar = exp(m[C * k + 2] + 0.5 * s_w * s_w) * smax;
+            if (C == 5) {                    /* R30: the high-angle side is alpha times wider */
+                double s_a = exp(l[C * k + 4]), abar = exp(m[C * k + 4] + 0.5 * s_a * s_a);
+                if (abar > 1.0) wbar *= abar;
+            }
+            double ci = W * wbar + fabs(m[C * k + 1]);
             if (ci > c) c = ci;
         }
         int64_t n = (int64_t)ceil(c / q->delta - 1e-9);
@@ -256,27 +286,46 @@ double orc_pseudo_voigt(double x, double rho, double w, double r) {   /* A7 PAPE
     return (1.0 - r) * orc_gauss(x, rho, w) + r * orc_lorentz(x, rho, w);
 }
 
-static void constrain(const double zeta[4], double *h, double *mu, double *w, double *r) {
+/* R30 (A9/A10): split pseudo-Voigt.  A(x; alpha) = alpha for x >= rho, 1 for x < rho multiplies the
+ * WIDTH of the shape on the high-angle side; the height stays that of width w, so the shape is continuous at x = rho and
+ * its area is (1 + alpha) / 2.  alpha = 1 is orc_pseudo_voigt. */
+double orc_asym(double x, double rho, double alpha) { return x >= rho ? alpha : 1.0; }   /* A9 */
+double orc_pseudo_voigt_asym(double x, double rho, double w, double r, double alpha) {
+    double t = (x - rho) / (w * orc_asym(x, rho, alpha));
+    double G = (2.0 / w) * sqrt(LN2 / M_PI) * exp(-4.0 * LN2 * t * t);
+    double L = (2.0 / (M_PI * w)) / (1.0 + 4.0 * t * t);
+    return (1.0 - r) * G + r * L;
+}
+/* R30: angle-dependent width, w_mk = w_k sec(theta_m), theta_m = p_m / 2 (deg), at the table position */
+static double sec_factor(const orc_problem *q, int64_t m) {
+    return q->hy.width_sec ? 1.0 / cos(0.5 * q->pos[m] * M_PI / 180.0) : 1.0;
+}
+
+static void constrain(const orc_problem *q, const double *zeta, double *h, double *mu, double *w, double *r, double *alpha) {
     *h = exp(zeta[0]);
     *mu = zeta[1];
     *w = exp(zeta[2]);
     *r = 1.0 / (1.0 + exp(-zeta[3]));
+    *alpha = q->C == 5 ? exp(zeta[4]) : 1.0;
 }
 
 /* ------------------------------------------------------------------ forward model */
 /* f_i = B_i + sum_k h_k sum_m I_m V(x_i; p_m + mu_k, w_k, r_k), pairs restricted to the window */
-void orc_profile(const orc_problem *q, int32_t pat, const double *zeta /*[K][4]*/, double *f /*[N]*/) {
+void orc_profile(const orc_problem *q, int32_t pat, const double *zeta /*[K][C]*/, double *f /*[N]*/) {
     const int64_t N = q->N;
+    const int C = q->C;
     for (int64_t i = 0; i < N; ++i) f[i] = q->B[pat * N + i];
     for (int32_t k = 0; k < q->K; ++k) {
-        double h, mu, w, r;
-        constrain(zeta + 4 * k, &h, &mu, &w, &r);
+        double h, mu, w, r, alpha;
+        constrain(q, zeta + C * k, &h, &mu, &w, &r, &alpha);
         for (int64_t m = q->ofs[k]; m < q->ofs[k + 1]; ++m) {
             double rho = q->pos[m] + mu;                                  /* A8 */
+            double wm = w * sec_factor(q, m);                             /* R30; = w without the sec term */
             int64_t i_lo, i_hi;
             window(q, k, m, &i_lo, &i_hi);
             for (int64_t i = i_lo; i <= i_hi; ++i) {
-                f[i] += h * q->inten[m] * orc_pseudo_voigt(q->x[i], rho, w, r);
+                if (C == 5) f[i] += h * q->inten[m] * orc_pseudo_voigt_asym(q->x[i], rho, wm, r, alpha);
+                else        f[i] += h * q->inten[m] * orc_pseudo_voigt(q->x[i], rho, wm, r);
             }
         }
     }
@@ -306,14 +355,19 @@ double orc_loglik(const orc_problem *q, int32_t pat, const double *f) {
 double orc_logprior_jac(const orc_problem *q, int32_t pat, const double *zeta) {
     const orc_hyper *hy = &q->hy;
     double lam = q->lambda_h[pat], acc = 0.0;
+    const int C = q->C;
     for (int32_t k = 0; k < q->K; ++k) {
-        double h, mu, w, r;
-        constrain(zeta + 4 * k, &h, &mu, &w, &r);
-        acc += log(lam) - lam * h + zeta[4 * k + 0];                                  /* eq.(3) + J */
+        double h, mu, w, r, alpha;
+        constrain(q, zeta + C * k, &h, &mu, &w, &r, &alpha);
+        acc += log(lam) - lam * h + zeta[C * k + 0];                                  /* eq.(3) + J */
         acc += -0.5 * (mu / hy->mu_sigma) * (mu / hy->mu_sigma) - log(hy->mu_sigma * sqrt(2.0 * M_PI));
         acc += hy->w_shape * log(hy->w_rate) - lgamma(hy->w_shape)
-             + (hy->w_shape - 1.0) * zeta[4 * k + 2] - hy->w_rate * w + zeta[4 * k + 2]; /* eq.(1) + J */
+             + (hy->w_shape - 1.0) * zeta[C * k + 2] - hy->w_rate * w + zeta[C * k + 2]; /* eq.(1) + J */
         acc += log(r) + log(1.0 - r);                                                  /* U(0,1): 0 + J */
+        if (C == 5) {                      /* alpha ~ Norm(1, 0.2) (B.2 PAPER.md:274), alpha = exp(zeta): + J (R30) */
+            double z = (alpha - hy->alpha_mu) / hy->alpha_sigma;
+            acc += -0.5 * z * z - log(hy->alpha_sigma * sqrt(2.0 * M_PI)) + zeta[C * k + 4];
+        }
     }
     return acc;
 }
@@ -329,34 +383,40 @@ void orc_logjoint_grad(const orc_problem *q, int32_t pat, const double *zeta, do
     *lpj_out = orc_logprior_jac(q, pat, zeta);
     double sn = q->sigma_n[pat], lam = q->lambda_h[pat];
     const double aG = 2.0 * sqrt(LN2 / M_PI), aL = 2.0 / M_PI;
+    const int C = q->C;
     for (int32_t k = 0; k < q->K; ++k) {
-        double h, mu, w, r;
-        constrain(zeta + 4 * k, &h, &mu, &w, &r);
-        double dh = 0.0, dmu = 0.0, dw = 0.0, dr = 0.0;
+        double h, mu, w, r, alpha;
+        constrain(q, zeta + C * k, &h, &mu, &w, &r, &alpha);
+        double dh = 0.0, dmu = 0.0, dw = 0.0, dr = 0.0, dal = 0.0;
         for (int64_t m = q->ofs[k]; m < q->ofs[k + 1]; ++m) {
             double I = q->inten[m], rho = q->pos[m] + mu;
+            double sm = sec_factor(q, m), wm = w * sm;                       /* R30 */
             int64_t i_lo, i_hi;
             window(q, k, m, &i_lo, &i_hi);
             for (int64_t i = i_lo; i <= i_hi; ++i) {
                 double e = q->hy.likelihood == 1
                                ? q->y[pat * N + i] / f[i] - 1.0                  /* d ll / d f_i of A16    */
                                : (q->y[pat * N + i] - f[i]) / (sn * sn);        /* d ll / d f_i, Gaussian */
-                double t = (q->x[i] - rho) / w;
+                double A = orc_asym(q->x[i], rho, alpha);                        /* A9: 1 without asymmetry */
+                double t = (q->x[i] - rho) / (wm * A);
                 double G = exp(-4.0 * LN2 * t * t), L = 1.0 / (1.0 + 4.0 * t * t);
-                double Gn = (aG / w) * G, Ln = (aL / w) * L;                 /* unit-area values */
+                double Gn = (aG / wm) * G, Ln = (aL / wm) * L;               /* heights of width w_m (R30) */
                 double V = (1.0 - r) * Gn + r * Ln;
                 /* dV/dt: dG/dt = -8 ln2 t G ; dL/dt = -8 t L^2 */
-                double dVdt = (1.0 - r) * (aG / w) * (-8.0 * LN2 * t * G) + r * (aL / w) * (-8.0 * t * L * L);
+                double dVdt = (1.0 - r) * (aG / wm) * (-8.0 * LN2 * t * G) + r * (aL / wm) * (-8.0 * t * L * L);
                 dh += e * I * V;
                 dr += e * I * h * (Ln - Gn);
-                dmu += e * I * h * dVdt * (-1.0 / w);                        /* dt/dmu = -1/w  */
-                dw += e * I * h * (-V / w + dVdt * (-t / w));                /* d(1/w)/dw, dt/dw = -t/w */
+                dmu += e * I * h * dVdt * (-1.0 / (wm * A));                 /* dt/dmu = -1/(w_m A)  */
+                dw += e * I * h * (-V / w + dVdt * (-t / w));                /* d(1/w_m)/dw = -1/(w w_m), dt/dw = -t/w */
+                if (q->x[i] >= rho) dal += e * I * h * dVdt * (-t / alpha);  /* dt/dalpha = -t/alpha on the high side */
             }
         }
-        g[4 * k + 0] = dh * h + (1.0 - lam * h);
-        g[4 * k + 1] = dmu + (-mu / (hy->mu_sigma * hy->mu_sigma));
-        g[4 * k + 2] = dw * w + (hy->w_shape - hy->w_rate * w);
-        g[4 * k + 3] = dr * r * (1.0 - r) + (1.0 - 2.0 * r);
+        g[C * k + 0] = dh * h + (1.0 - lam * h);
+        g[C * k + 1] = dmu + (-mu / (hy->mu_sigma * hy->mu_sigma));
+        g[C * k + 2] = dw * w + (hy->w_shape - hy->w_rate * w);
+        g[C * k + 3] = dr * r * (1.0 - r) + (1.0 - 2.0 * r);
+        if (C == 5)
+            g[C * k + 4] = dal * alpha + (-(alpha - hy->alpha_mu) / (hy->alpha_sigma * hy->alpha_sigma)) * alpha + 1.0;
     }
     if (!f_out) free(f);
 }
@@ -372,45 +432,49 @@ void orc_elbo_grad_range(const orc_problem *q, const double *state, int32_t S, u
                          uint64_t iteration, int32_t inst0, int32_t n_inst, double *elbo, double *grad,
                          double *ll_out, double *f_out, int64_t n_f) {
     const int32_t K = q->K, R = q->R;
+    const int C = q->C;
     const int64_t N = q->N;
     const int64_t T = (int64_t)n_inst * S;
-    double *gz_all = (double *)malloc(sizeof(double) * (size_t)T * K * 4);
-    double *eps_all = (double *)malloc(sizeof(double) * (size_t)T * K * 4);
+    double *gz_all = (double *)malloc(sizeof(double) * (size_t)T * K * C);
+    double *eps_all = (double *)malloc(sizeof(double) * (size_t)T * K * C);
     double *lj_all = (double *)malloc(sizeof(double) * (size_t)T * 2);
 #pragma omp parallel for schedule(dynamic, 1)
     for (int64_t t = 0; t < T; ++t) {
         int32_t s = (int32_t)(t % S);
         int32_t inst = inst0 + (int32_t)(t / S);  /* inst = pat*R + rst */
         int32_t pat = inst / R;
-        const double *m = state + (size_t)inst * 2 * K * 4, *l = m + (size_t)K * 4;
-        double *zeta = (double *)malloc(sizeof(double) * K * 4);
-        double *eps = eps_all + (size_t)t * K * 4;
+        const double *m = state + (size_t)inst * 2 * K * C, *l = m + (size_t)K * C;
+        double *zeta = (double *)malloc(sizeof(double) * K * C);
+        double *eps = eps_all + (size_t)t * K * C;
         for (int32_t k = 0; k < K; ++k) {
-            orc_eps(seed, iteration, (uint32_t)inst, (uint32_t)s, (uint32_t)k, eps + 4 * k);
-            for (int c = 0; c < 4; ++c) zeta[4 * k + c] = m[4 * k + c] + exp(l[4 * k + c]) * eps[4 * k + c];
+            double e4[4];
+            orc_eps(seed, iteration, (uint32_t)inst, (uint32_t)s, (uint32_t)k, e4);
+            for (int c = 0; c < 4; ++c) eps[C * k + c] = e4[c];
+            if (C == 5) eps[C * k + 4] = orc_eps_alpha(seed, iteration, (uint32_t)inst, (uint32_t)s, (uint32_t)k);
+            for (int c = 0; c < C; ++c) zeta[C * k + c] = m[C * k + c] + exp(l[C * k + c]) * eps[C * k + c];
         }
         double *fbuf = (f_out && t < n_f) ? f_out + (size_t)t * N : NULL;
-        orc_logjoint_grad(q, pat, zeta, &lj_all[2 * t], &lj_all[2 * t + 1], gz_all + (size_t)t * K * 4, fbuf);
+        orc_logjoint_grad(q, pat, zeta, &lj_all[2 * t], &lj_all[2 * t + 1], gz_all + (size_t)t * K * C, fbuf);
         if (ll_out) ll_out[t] = lj_all[2 * t];
         free(zeta);
     }
     for (int32_t li = 0; li < n_inst; ++li) {
         const int32_t inst = inst0 + li;
-        const double *l = state + (size_t)inst * 2 * K * 4 + (size_t)K * 4;
-        double *gm = grad + (size_t)li * 2 * K * 4, *gl = gm + (size_t)K * 4;
+        const double *l = state + (size_t)inst * 2 * K * C + (size_t)K * C;
+        double *gm = grad + (size_t)li * 2 * K * C, *gl = gm + (size_t)K * C;
         double acc = 0.0;
-        for (int j = 0; j < 4 * K; ++j) { gm[j] = 0.0; gl[j] = 0.0; }
+        for (int j = 0; j < C * K; ++j) { gm[j] = 0.0; gl[j] = 0.0; }
         for (int32_t s = 0; s < S; ++s) {
             int64_t t = (int64_t)li * S + s;
             acc += lj_all[2 * t] + lj_all[2 * t + 1];
-            for (int j = 0; j < 4 * K; ++j) {
-                double gz = gz_all[(size_t)t * K * 4 + j];
+            for (int j = 0; j < C * K; ++j) {
+                double gz = gz_all[(size_t)t * K * C + j];
                 gm[j] += gz;
-                gl[j] += gz * eps_all[(size_t)t * K * 4 + j] * exp(l[j]);
+                gl[j] += gz * eps_all[(size_t)t * K * C + j] * exp(l[j]);
             }
         }
         double ent = 0.0;
-        for (int j = 0; j < 4 * K; ++j) {
+        for (int j = 0; j < C * K; ++j) {
             gm[j] /= (double)S;
             gl[j] = gl[j] / (double)S + 1.0;
             ent += l[j] + 0.5 * log(2.0 * M_PI * M_E);
@@ -431,7 +495,7 @@ void orc_elbo_grad(const orc_problem *q, const double *state, int32_t S, uint64_
 void orc_adam_step(const orc_problem *q, double *state, const double *grad, double *mom1, double *mom2,
                    int64_t step) {
     const orc_hyper *hy = &q->hy;
-    const int64_t per = 2 * (int64_t)q->K * 4, total = per * q->P * q->R;
+    const int64_t per = 2 * (int64_t)q->K * q->C, total = per * q->P * q->R;
     double bc1 = 1.0 - pow(hy->beta1, (double)step), bc2 = 1.0 - pow(hy->beta2, (double)step);
     for (int64_t j = 0; j < total; ++j) {
         mom1[j] = hy->beta1 * mom1[j] + (1.0 - hy->beta1) * grad[j];
@@ -451,7 +515,7 @@ void orc_adam_step(const orc_problem *q, double *state, const double *grad, doub
  *     m <- m + lr sigma^2 dELBO/dm,     l <- l + lr (dELBO/dl) / 2,   l clamped to [-12, 2],
  * with sigma taken BEFORE the step.  No moments, no bias correction. */
 void orc_natgrad_step(const orc_problem *q, double *state, const double *grad) {
-    const int64_t half = (int64_t)q->K * 4, per = 2 * half;
+    const int64_t half = (int64_t)q->K * q->C, per = 2 * half;
     for (int32_t inst = 0; inst < q->P * q->R; ++inst) {
         double *m = state + (size_t)inst * per, *l = m + half;
         const double *gm = grad + (size_t)inst * per, *gl = gm + half;
@@ -470,15 +534,16 @@ void orc_natgrad_step(const orc_problem *q, double *state, const double *grad) {
  * ctr = (0xFFFFFFFF, r, k, pat) under the given seed. */
 void orc_init_state(const orc_problem *q, uint64_t seed, double *state) {
     const int32_t K = q->K;
+    const int C = q->C;
     static const double jit[4] = {0.5, 0.01, 0.2, 0.5};
     for (int32_t pat = 0; pat < q->P; ++pat)
         for (int32_t rst = 0; rst < q->R; ++rst) {
-            double *m = state + (size_t)(pat * q->R + rst) * 2 * K * 4, *l = m + (size_t)K * 4;
+            double *m = state + (size_t)(pat * q->R + rst) * 2 * K * C, *l = m + (size_t)K * C;
             for (int32_t k = 0; k < K; ++k) {
-                m[4 * k + 0] = log(q->eta_h[pat] / (double)K);
-                m[4 * k + 1] = 0.0;
-                m[4 * k + 2] = log(q->hy.w_shape / q->hy.w_rate);
-                m[4 * k + 3] = 0.0;
+                m[C * k + 0] = log(q->eta_h[pat] / (double)K);
+                m[C * k + 1] = 0.0;
+                m[C * k + 2] = log(q->hy.w_shape / q->hy.w_rate);
+                m[C * k + 3] = 0.0;
                 if (rst > 0) {
                     double e[4];
                     uint32_t ctr[4] = {0xFFFFFFFFu, (uint32_t)rst, (uint32_t)k, (uint32_t)pat};
@@ -489,9 +554,20 @@ void orc_init_state(const orc_problem *q, uint64_t seed, double *state) {
                     double r0 = sqrt(-2.0 * log(u0)), r1 = sqrt(-2.0 * log(u2));
                     e[0] = r0 * cos(2.0 * M_PI * u1); e[1] = r0 * sin(2.0 * M_PI * u1);
                     e[2] = r1 * cos(2.0 * M_PI * u3); e[3] = r1 * sin(2.0 * M_PI * u3);
-                    for (int c = 0; c < 4; ++c) m[4 * k + c] += jit[c] * e[c];
+                    for (int c = 0; c < 4; ++c) m[C * k + c] += jit[c] * e[c];
                 }
-                for (int c = 0; c < 4; ++c) l[4 * k + c] = q->hy.init_log_sigma;
+                if (C == 5) {      /* R30: alpha starts at 1 (symmetric peaks); restart jitter 0.05 eps from a second
+                                      Philox call with bit 31 of the phase word set */
+                    m[C * k + 4] = 0.0;
+                    if (rst > 0) {
+                        uint32_t ctr[4] = {0xFFFFFFFFu, (uint32_t)rst, (uint32_t)k | 0x80000000u, (uint32_t)pat};
+                        uint32_t key[2] = {(uint32_t)seed, (uint32_t)(seed >> 32)};
+                        uint32_t wd[4];
+                        orc_philox4x32_10(ctr, key, wd);
+                        m[C * k + 4] += 0.05 * sqrt(-2.0 * log(uniform23(wd[0]))) * cos(2.0 * M_PI * uniform23(wd[1]));
+                    }
+                }
+                for (int c = 0; c < C; ++c) l[C * k + c] = q->hy.init_log_sigma;
             }
         }
 }
@@ -500,7 +576,7 @@ void orc_init_state(const orc_problem *q, uint64_t seed, double *state) {
  * first_step >= 1.  mom1/mom2 carried by the caller (zeros at first_step == 1). */
 void orc_fit(const orc_problem *q, double *state, double *mom1, double *mom2, int32_t iterations,
              int32_t S, uint64_t seed, int64_t first_step, double *elbo_trace /*[iterations][P][R] or NULL*/) {
-    const int64_t per = 2 * (int64_t)q->K * 4, total = per * q->P * q->R;
+    const int64_t per = 2 * (int64_t)q->K * q->C, total = per * q->P * q->R;
     double *grad = (double *)malloc(sizeof(double) * total);
     double *elbo = (double *)malloc(sizeof(double) * q->P * q->R);
     for (int32_t it = 0; it < iterations; ++it) {
@@ -521,22 +597,28 @@ static double normal_cdf(double z) { return 0.5 * erfc(-z / sqrt(2.0)); }
 void orc_inclusion(const orc_problem *q, const double *state, double *incl /*[P][R][K]*/,
                    double *area_ratio /*[P][R][K] or NULL*/) {
     const int32_t K = q->K;
+    const int C = q->C;
     for (int32_t inst = 0; inst < q->P * q->R; ++inst) {
-        const double *m = state + (size_t)inst * 2 * K * 4, *l = m + (size_t)K * 4;
+        const double *m = state + (size_t)inst * 2 * K * C, *l = m + (size_t)K * C;
         double Tbar = 0.0;
+        double *Ak = (double *)malloc(sizeof(double) * K);
         for (int32_t k = 0; k < K; ++k) {
             double A = 0.0;
             for (int64_t mm = q->ofs[k]; mm < q->ofs[k + 1]; ++mm) A += q->inten[mm];
-            double s = exp(l[4 * k]);
-            Tbar += A * exp(m[4 * k] + 0.5 * s * s);
+            if (C == 5) {            /* R30: a split peak has area (1 + alpha) / 2; alpha at its mean under q */
+                double sa = exp(l[C * k + 4]);
+                A *= 0.5 * (1.0 + exp(m[C * k + 4] + 0.5 * sa * sa));
+            }
+            Ak[k] = A;
+            double s = exp(l[C * k]);
+            Tbar += A * exp(m[C * k] + 0.5 * s * s);
         }
         for (int32_t k = 0; k < K; ++k) {
-            double A = 0.0;
-            for (int64_t mm = q->ofs[k]; mm < q->ofs[k + 1]; ++mm) A += q->inten[mm];
-            double s = exp(l[4 * k]);
-            incl[(size_t)inst * K + k] = normal_cdf((m[4 * k] - log(q->hy.incl_tau * Tbar / A)) / s);
-            if (area_ratio) area_ratio[(size_t)inst * K + k] = A * exp(m[4 * k] + 0.5 * s * s) / Tbar;
+            double s = exp(l[C * k]);
+            incl[(size_t)inst * K + k] = normal_cdf((m[C * k] - log(q->hy.incl_tau * Tbar / Ak[k])) / s);
+            if (area_ratio) area_ratio[(size_t)inst * K + k] = Ak[k] * exp(m[C * k] + 0.5 * s * s) / Tbar;
         }
+        free(Ak);
     }
 }
 
@@ -559,18 +641,19 @@ static double normal_quantile_bisect(double p) {
 
 static double sigmoid_d(double x) { return 1.0 / (1.0 + exp(-x)); }
 
-void orc_posterior_summary(const orc_problem *q, const double *state, double *out /*[P][R][K][4][5]*/) {
+void orc_posterior_summary(const orc_problem *q, const double *state, double *out /*[P][R][K][C][5]*/) {
     const int32_t K = q->K;
+    const int C = q->C;
     const double zq[3] = {normal_quantile_bisect(0.025), 0.0, normal_quantile_bisect(0.975)};
     const int nint = 48000;                      /* Simpson intervals (even) */
     const double za = -12.0, zb = 12.0, dz = (zb - za) / nint;
     for (int32_t inst = 0; inst < q->P * q->R; ++inst) {
-        const double *m = state + (size_t)inst * 2 * K * 4, *l = m + (size_t)K * 4;
+        const double *m = state + (size_t)inst * 2 * K * C, *l = m + (size_t)K * C;
         for (int32_t k = 0; k < K; ++k)
-            for (int c = 0; c < 4; ++c) {
-                const double mm = m[4 * k + c], s = exp(l[4 * k + c]);
-                double *o = out + (((size_t)inst * K + k) * 4 + c) * 5;
-                if (c == 0 || c == 2) {          /* log-normal */
+            for (int c = 0; c < C; ++c) {
+                const double mm = m[C * k + c], s = exp(l[C * k + c]);
+                double *o = out + (((size_t)inst * K + k) * C + c) * 5;
+                if (c == 0 || c == 2 || c == 4) { /* log-normal (h, w, alpha) */
                     o[0] = exp(mm + 0.5 * s * s);
                     o[1] = sqrt(expm1(s * s)) * exp(mm + 0.5 * s * s);
                     for (int j = 0; j < 3; ++j) o[2 + j] = exp(mm + s * zq[j]);

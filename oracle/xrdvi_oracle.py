@@ -31,12 +31,15 @@ class OrcHyper(C.Structure):
         ("init_log_sigma", C.c_double),
         ("n_patterns", C.c_int32), ("n_restarts", C.c_int32),
         ("likelihood", C.c_int32), ("optimizer", C.c_int32),
+        ("asymmetry", C.c_int32), ("width_sec", C.c_int32),
+        ("alpha_mu", C.c_double), ("alpha_sigma", C.c_double),
     ]
 
 
 DEFAULTS = dict(lambda_h=0.0, mu_sigma=0.03, w_shape=3.0, w_rate=100.0, noise_sigma=0.0,
                 window_W=10.0, fwhm_ref=0.15, incl_tau=0.01, lr=0.1, beta1=0.9, beta2=0.999,
-                adam_eps=1e-8, init_log_sigma=float(np.log(0.1)), n_patterns=1, n_restarts=1, likelihood=0, optimizer=0)
+                adam_eps=1e-8, init_log_sigma=float(np.log(0.1)), n_patterns=1, n_restarts=1, likelihood=0, optimizer=0,
+                asymmetry=0, width_sec=0, alpha_mu=1.0, alpha_sigma=0.2)
 
 _lib = None
 
@@ -65,6 +68,12 @@ def lib():
             getattr(L, name).argtypes = [C.c_double] * 3
         L.orc_pseudo_voigt.restype = C.c_double
         L.orc_pseudo_voigt.argtypes = [C.c_double] * 4
+        L.orc_pseudo_voigt_asym.restype = C.c_double
+        L.orc_pseudo_voigt_asym.argtypes = [C.c_double] * 5
+        L.orc_eps_alpha.restype = C.c_double
+        L.orc_eps_alpha.argtypes = [C.c_uint64, C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32]
+        L.orc_classes.restype = C.c_int32
+        L.orc_classes.argtypes = [C.c_void_p]
         L.orc_profile.argtypes = [C.c_void_p, C.c_int32, dp, dp]
         L.orc_loglik.restype = C.c_double
         L.orc_loglik.argtypes = [C.c_void_p, C.c_int32, dp]
@@ -119,6 +128,14 @@ def pseudo_voigt(x, rho, w, r):
     return lib().orc_pseudo_voigt(float(x), float(rho), float(w), float(r))
 
 
+def pseudo_voigt_asym(x, rho, w, r, alpha):
+    return lib().orc_pseudo_voigt_asym(float(x), float(rho), float(w), float(r), float(alpha))
+
+
+def eps_alpha(seed, iteration, inst, s, k):
+    return float(lib().orc_eps_alpha(int(seed), int(iteration), int(inst), int(s), int(k)))
+
+
 def num_threads():
     return int(lib().orc_num_threads())
 
@@ -149,6 +166,7 @@ class Oracle:
         self._h = L.orc_create(_dp(self.x), self.N, _dp(self.y), _dp(self.B), self.K,
                                self.ofs.ctypes.data_as(C.POINTER(C.c_int64)), _dp(self.pos),
                                _dp(self.inten), C.byref(self._hs))
+        self.C = int(L.orc_classes(self._h))        # latent classes per phase: 4, or 5 with the asymmetry (R30)
         self._mom = None
         self.step = 0
 
@@ -176,7 +194,7 @@ class Oracle:
 
     # ---- model pieces ------------------------------------------------------
     def _zeta(self, zeta):
-        z = np.ascontiguousarray(zeta, dtype=np.float64).reshape(self.K, 4)
+        z = np.ascontiguousarray(zeta, dtype=np.float64).reshape(self.K, self.C)
         return z
 
     def profile(self, zeta, pat=0):
@@ -196,13 +214,13 @@ class Oracle:
     def logjoint_grad(self, zeta, pat=0):
         z = self._zeta(zeta)
         ll, lpj = C.c_double(), C.c_double()
-        g = np.empty((self.K, 4), dtype=np.float64)
+        g = np.empty((self.K, self.C), dtype=np.float64)
         lib().orc_logjoint_grad(self._h, pat, _dp(z), C.byref(ll), C.byref(lpj), _dp(g), None)
         return ll.value, lpj.value, g
 
     # ---- ELBO --------------------------------------------------------------
     def _state(self, state):
-        st = np.ascontiguousarray(state, dtype=np.float64).reshape(self.P, self.R, 2, self.K, 4)
+        st = np.ascontiguousarray(state, dtype=np.float64).reshape(self.P, self.R, 2, self.K, self.C)
         return st
 
     def elbo_grad(self, state, S, seed, iteration, want_ll=False, n_profiles=0):
@@ -224,14 +242,14 @@ class Oracle:
         """ELBO / gradient (/ ll per draw) of instances inst0 .. inst0+n_inst-1 only (inst = pat*R + rst)."""
         st = self._state(state)
         elbo = np.empty(n_inst, dtype=np.float64)
-        grad = np.empty((n_inst, 2, self.K, 4), dtype=np.float64)
+        grad = np.empty((n_inst, 2, self.K, self.C), dtype=np.float64)
         ll = np.empty((n_inst, S), dtype=np.float64) if want_ll else None
         lib().orc_elbo_grad_range(self._h, _dp(st), int(S), int(seed), int(iteration), int(inst0), int(n_inst),
                                   _dp(elbo), _dp(grad), _dp(ll), None, 0)
         return (elbo, grad, ll) if want_ll else (elbo, grad)
 
     def init_state(self, seed=0):
-        st = np.empty((self.P, self.R, 2, self.K, 4), dtype=np.float64)
+        st = np.empty((self.P, self.R, 2, self.K, self.C), dtype=np.float64)
         lib().orc_init_state(self._h, int(seed), _dp(st))
         return st
 
@@ -300,7 +318,7 @@ class Oracle:
     def posterior_summary(self, state):
         """Marginals of q in (h, mu, w, r): [P][R][K][4][5] = (mean, sd, q2.5, q50, q97.5) (reading R28)."""
         st = self._state(state)
-        out = np.empty((self.P, self.R, self.K, 4, 5), dtype=np.float64)
+        out = np.empty((self.P, self.R, self.K, self.C, 5), dtype=np.float64)
         lib().orc_posterior_summary(self._h, _dp(st), _dp(out))
         return out
 

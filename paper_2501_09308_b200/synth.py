@@ -70,13 +70,16 @@ class Workload:
         return int(self.hyper.get("n_restarts", 1))
 
 
-def _pseudo_voigt_pattern(x, pos, inten, h, shift, fwhm, mix):
-    """Dense instrument response of one phase (plain numpy, fp64)."""
+def _pseudo_voigt_pattern(x, pos, inten, h, shift, fwhm, mix, alpha=1.0):
+    """Dense instrument response of one phase (plain numpy, fp64).  alpha != 1: split peaks, the high-angle side
+    alpha times wider at the same height (A9/A10)."""
     out = np.zeros_like(x)
     # chunk the (peak x point) plane to bound memory
     for a in range(0, pos.shape[0], 64):
         p = pos[a:a + 64, None] + shift
         t = (x[None, :] - p) / fwhm
+        if alpha != 1.0:
+            t = np.where(t >= 0.0, t / alpha, t)
         g = (_A_G / fwhm) * np.exp(-4.0 * math.log(2.0) * t * t)
         l = (_A_L / fwhm) / (1.0 + 4.0 * t * t)
         out += (inten[a:a + 64, None] * ((1.0 - mix) * g + mix * l)).sum(axis=0)
@@ -96,7 +99,7 @@ _SPEC = {
 def make_workload(cfg: int, n_patterns: int | None = None, n_restarts: int | None = None,
                   S: int | None = None, K: int | None = None, seed: int | None = None,
                   peak_counts: float | None = None, grid: tuple | None = None,
-                  noise_frac: float = 0.01) -> Workload:
+                  noise_frac: float = 0.01, asym: tuple | None = None) -> Workload:
     """Build config ``cfg`` (0..4).  Optional overrides shrink a config for tests
     (e.g. ``n_patterns=4`` for cfg 3) without changing its per-pattern recipe.
 
@@ -106,7 +109,9 @@ def make_workload(cfg: int, n_patterns: int | None = None, n_restarts: int | Non
 
     ``grid = (lo, hi, N)`` replaces the config's 2theta range and point count (same recipe otherwise), e.g. config 0
     on a 0.02 deg grid that resolves its peaks: ``grid=(10.0, 80.0, 3501)``.  ``noise_frac``: Gaussian noise sigma as a
-    fraction of the maximum signal (the configs' 1 %)."""
+    fraction of the maximum signal (the configs' 1 %).  ``asym = (lo, hi)``: every planted phase gets a peak asymmetry
+    alpha ~ U(lo, hi) (split peaks); ``true_params`` entries then carry alpha as a fifth value and
+    ``hyper['asymmetry'] = 1``."""
     if cfg not in _SPEC:
         raise ValueError(f"unknown config {cfg}")
     (K0, (mlo, mhi), N, lo, hi, P0, R0, S0, its, W, fwhm_ref, (fw_lo, fw_hi), (w_shape, w_rate)) = _SPEC[cfg]
@@ -149,6 +154,8 @@ def make_workload(cfg: int, n_patterns: int | None = None, n_restarts: int | Non
         for k in ids:
             prm[int(k)] = (float(rng.uniform(0.5, 2.0)), float(rng.normal(0.0, 0.02)),
                            float(rng.uniform(fw_lo, fw_hi)), float(rng.uniform(0.2, 0.8)))
+            if asym is not None:
+                prm[int(k)] = prm[int(k)] + (float(rng.uniform(asym[0], asym[1])),)
         true_params.append(prm)
 
     # ---- confusers: absent phases shadowing true phases of pattern 0 --------
@@ -171,8 +178,8 @@ def make_workload(cfg: int, n_patterns: int | None = None, n_restarts: int | Non
     bg = np.empty((P, N), dtype=np.float64)
     for pat in range(P):
         sig = np.zeros(N, dtype=np.float64)
-        for k, (h, sh, fw, mix) in true_params[pat].items():
-            sig += _pseudo_voigt_pattern(x, pos_list[k], int_list[k], h, sh, fw, mix)
+        for k, prm in true_params[pat].items():
+            sig += _pseudo_voigt_pattern(x, pos_list[k], int_list[k], *prm)
         smax = float(sig.max())
         b0 = 0.02 * smax
         b1 = rng.uniform(-0.5, 0.5) * b0 / (hi - lo)
@@ -184,25 +191,31 @@ def make_workload(cfg: int, n_patterns: int | None = None, n_restarts: int | Non
             c = float(peak_counts) / float((sig + bg[pat]).max())
             bg[pat] *= c
             y[pat] = rng.poisson(c * sig + bg[pat]).astype(np.float64)
-            true_params[pat] = {k: (h * c, sh, fw, mix) for k, (h, sh, fw, mix) in true_params[pat].items()}
+            true_params[pat] = {k: (prm[0] * c,) + tuple(prm[1:]) for k, prm in true_params[pat].items()}
 
     hyper = dict(window_W=W, fwhm_ref=fwhm_ref, w_shape=w_shape, w_rate=w_rate,
                  n_patterns=P, n_restarts=R)
     if peak_counts is not None:
         hyper["likelihood"] = 1
+    if asym is not None:
+        hyper["asymmetry"] = 1
     return Workload(cfg=cfg, two_theta=x, y=y, background=bg, peak_ofs=peak_ofs,
                     peak_pos=peak_pos, peak_int=peak_int, hyper=hyper, S=S, iterations=its,
                     true_phases=true_phases, true_params=true_params)
 
 
-def random_state(K: int, P: int, R: int, seed: int, spread: float = 0.3) -> np.ndarray:
-    """A seeded float32 variational state [P][R][2][K][4] near a plausible fit
-    (used by parity tests to probe ELBO/gradient away from the initial state)."""
+def random_state(K: int, P: int, R: int, seed: int, spread: float = 0.3, classes: int = 4) -> np.ndarray:
+    """A seeded float32 variational state [P][R][2][K][classes] near a plausible fit
+    (used by parity tests to probe ELBO/gradient away from the initial state); classes = 5 adds the
+    asymmetry latent ln alpha ~ N(0, 0.15)."""
     rng = np.random.default_rng(seed)
-    st = np.zeros((P, R, 2, K, 4), dtype=np.float32)
+    st = np.zeros((P, R, 2, K, classes), dtype=np.float32)
     st[:, :, 0, :, 0] = rng.normal(-3.0, 1.5 * spread + 0.5, size=(P, R, K))
     st[:, :, 0, :, 1] = rng.normal(0.0, 0.02, size=(P, R, K))
     st[:, :, 0, :, 2] = np.log(0.1) + rng.normal(0.0, spread, size=(P, R, K))
     st[:, :, 0, :, 3] = rng.normal(0.0, 1.0, size=(P, R, K))
-    st[:, :, 1] = np.log(0.1) + rng.normal(0.0, spread, size=(P, R, K, 4))
+    st[:, :, 1, :, :4] = np.log(0.1) + rng.normal(0.0, spread, size=(P, R, K, 4))
+    if classes == 5:
+        st[:, :, 0, :, 4] = rng.normal(0.0, 0.15, size=(P, R, K))
+        st[:, :, 1, :, 4] = np.log(0.05) + rng.normal(0.0, spread, size=(P, R, K))
     return st
