@@ -27,7 +27,8 @@
  *  - Results are bitwise reproducible for equal inputs (all reductions have a fixed order).
  *
  * Layout of variational parameters ("state"): float [P][R][2][K][4]; [..][0] = m (mean), [..][1] =
- * l = log sigma; the last axis is the latent class (h, mu, w, r).  An "instance" is inst = pat*R + rst.
+ * l = log sigma; the last axis is the latent class (h, mu, w, r) -- (h, mu, w, r, alpha), i.e. [K][5], when
+ * hyper.asymmetry = 1 (R30).  An "instance" is inst = pat*R + rst.
  */
 #ifndef XRDVI_H
 #define XRDVI_H
@@ -76,6 +77,14 @@ typedef struct {
     int32_t optimizer;     /* 0 Adam ascent (R10); 1 natural-gradient ascent of the mean-field Gaussian:
                               m += lr sigma^2 dELBO/dm, l += lr (dELBO/dl)/2, l clamped to [-12, 2] (R25);
                               plain steps, no trust region: needs a small lr (0.01 at config 0)             */
+    int32_t asymmetry;     /* 1: the paper's peak asymmetry (A9/A10; R30): a FIFTH latent per phase,
+                              alpha_k = exp(zeta_alpha) ~ Norm(alpha_mu, alpha_sigma); the high-angle side of every peak
+                              (x >= p_m + mu_k) is alpha_k times wider at unchanged height (area (1 + alpha_k)/2).
+                              Every [..][K][4] array of this header becomes [..][K][5] (class order h, mu, w, r, alpha);
+                              xrdvi_latent_classes() returns the count.  0 (default): the four-latent model          */
+    int32_t width_sec;     /* 1: angle-dependent width w_k sec(p_m / 2) per peak (the sec of; R30)      */
+    double alpha_mu;       /* 1.00 (B.2)                                                          */
+    double alpha_sigma;    /* 0.20 (B.2)                                                                        */
 } xrdvi_hyper;
 
 void xrdvi_default_hyper(xrdvi_hyper* hyp);
@@ -111,6 +120,9 @@ void xrdvi_destroy(xrdvi* h);
 
 /* In-window (m,i) pairs per sample-instance: the unit of the throughput metric.                    */
 int64_t xrdvi_pair_count(const xrdvi* h);
+/* Latent classes per phase C: 4 (h, mu, w, r), or 5 with hyper.asymmetry (+ alpha).  Wherever this header writes
+ * [K][4] (states, gradients, moments, zeta, summaries) the last axis has C entries.                   */
+int32_t xrdvi_latent_classes(const xrdvi* h);
 /* Window half-width n_c in grid points (N for dense).                                              */
 int64_t xrdvi_window_halfwidth(const xrdvi* h);
 

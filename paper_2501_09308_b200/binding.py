@@ -16,7 +16,7 @@ _LIB_PATH = _PKG / "libxrdvi.so"
 
 EXPORTS = (            # include/xrdvi.h: the product boundary
     "xrdvi_default_hyper", "xrdvi_workspace_bytes", "xrdvi_create", "xrdvi_destroy", "xrdvi_pair_count",
-    "xrdvi_window_halfwidth", "xrdvi_set_phase_windows", "xrdvi_get_phase_windows", "xrdvi_adapt_windows",
+    "xrdvi_latent_classes", "xrdvi_window_halfwidth", "xrdvi_set_phase_windows", "xrdvi_get_phase_windows", "xrdvi_adapt_windows",
     "xrdvi_fit_adaptive", "xrdvi_reset_state", "xrdvi_reset_state_restart", "xrdvi_get_state", "xrdvi_set_state",
     "xrdvi_get_optimizer_state", "xrdvi_set_optimizer_state", "xrdvi_elbo_grad",
     "xrdvi_fit", "xrdvi_inclusion", "xrdvi_posterior_summary", "xrdvi_logjoint_grad", "xrdvi_last_error",
@@ -41,6 +41,7 @@ class Hyper(C.Structure):
         ("incl_tau", C.c_double), ("lr", C.c_double), ("beta1", C.c_double), ("beta2", C.c_double),
         ("adam_eps", C.c_double), ("init_log_sigma", C.c_double),
         ("n_patterns", C.c_int32), ("n_restarts", C.c_int32), ("likelihood", C.c_int32), ("optimizer", C.c_int32),
+        ("asymmetry", C.c_int32), ("width_sec", C.c_int32), ("alpha_mu", C.c_double), ("alpha_sigma", C.c_double),
     ]
 
 
@@ -69,6 +70,8 @@ def load_library():
     L.xrdvi_pair_count.restype = C.c_int64
     L.xrdvi_window_halfwidth.argtypes = [vp]
     L.xrdvi_window_halfwidth.restype = C.c_int64
+    L.xrdvi_latent_classes.argtypes = [vp]
+    L.xrdvi_latent_classes.restype = C.c_int32
     ip = C.POINTER(C.c_int32)
     L.xrdvi_set_phase_windows.argtypes = [vp, ip]
     L.xrdvi_get_phase_windows.argtypes = [vp, ip]
@@ -172,6 +175,7 @@ class Xrdvi:
                               C.c_void_p(self.stream.cuda_stream if self.stream is not None else 0),
                               C.c_void_p(self.workspace.data_ptr()), nbytes, C.byref(self._h)))
         self.workspace_bytes = nbytes
+        self.C = int(L.xrdvi_latent_classes(self._h))       # latent classes per phase: 4, or 5 with the asymmetry
 
     @classmethod
     def from_workload(cls, wl, S_max=None, device=0, library_stream=False, **overrides):
@@ -202,7 +206,7 @@ class Xrdvi:
         return int(load_library().xrdvi_window_halfwidth(self._h))
 
     def _state_shape(self):
-        return (self.P, self.R, 2, self.K, 4)
+        return (self.P, self.R, 2, self.K, self.C)
 
     # ---- state -----------------------------------------------------------------
     def reset_state(self, seed=0, restart_offset=0):
@@ -275,11 +279,11 @@ class Xrdvi:
 
     def logjoint_grad(self, zeta, pattern=0):
         """ll [n], log prior + log Jacobian [n], gradient [n][K][4] at the points zeta [n][K][4] (xrdvi_logjoint_grad)."""
-        z = np.ascontiguousarray(zeta, dtype=np.float32).reshape(-1, self.K, 4)
+        z = np.ascontiguousarray(zeta, dtype=np.float32).reshape(-1, self.K, self.C)
         n = int(z.shape[0])
         ll = np.empty(n, dtype=np.float64)
         lpj = np.empty(n, dtype=np.float64)
-        g = np.empty((n, self.K, 4), dtype=np.float32)
+        g = np.empty((n, self.K, self.C), dtype=np.float32)
         _check(load_library().xrdvi_logjoint_grad(self._h, _f(z), n, int(pattern), _d(ll), _d(lpj), _f(g)))
         return ll, lpj, g
 
@@ -290,7 +294,7 @@ class Xrdvi:
         return inc, ar
 
     def posterior_summary(self):
-        out = np.empty((self.P, self.R, self.K, 4, 5), dtype=np.float64)
+        out = np.empty((self.P, self.R, self.K, self.C, 5), dtype=np.float64)
         _check(load_library().xrdvi_posterior_summary(self._h, _d(out)))
         return out
 

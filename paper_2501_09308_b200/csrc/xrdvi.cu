@@ -45,7 +45,7 @@ struct Plan {   // workspace carve; identical arithmetic in workspace_bytes and 
     size_t o_var, o_vartmp, o_mom1, o_mom2, o_grad, o_elbo, o_elbok, o_llt, o_trace, o_ctl;
     size_t o_lat, o_eps, o_rr, o_ng, o_llpart, o_part8, o_dbg;
     size_t o_pd, o_lpk, o_zeta, o_gradz, o_lls, o_partial, o_tcnt, o_summ;
-    size_t o_trng;
+    size_t o_trng, o_ia, o_epsa, o_parta, o_pksec, o_secmax;
     int pd_groups;     // groups one launch of the log-joint gradient service handles
 };
 
@@ -106,7 +106,7 @@ bool make_plan(int64_t N, int32_t K, int64_t M, int32_t S_max, double step, cons
     if (p.tile_cap > (1ll << 31) - 1 || p.slots_cap > (1ll << 31) - 1) return false;
     size_t o = 0;
     auto take = [&](size_t bytes) { size_t r = o; o = align_up(o + bytes); return r; };
-    const size_t var_b = sizeof(float) * p.PR * 8 * static_cast<size_t>(K);
+    const size_t var_b = sizeof(float) * p.PR * 10 * static_cast<size_t>(K);   // [PR][2][K][4], then [PR][2][K] for alpha (R30)
     const size_t gk32 = static_cast<size_t>(p.G_max) * K * 32;
     p.o_yb = take(sizeof(float) * p.P * N);
     p.o_bg = take(sizeof(float) * p.P * N);
@@ -135,29 +135,36 @@ bool make_plan(int64_t N, int32_t K, int64_t M, int32_t S_max, double step, cons
     p.o_llpart = take(sizeof(float) * static_cast<size_t>(p.G_max) * p.n_seg * 32);
     p.o_part8 = take(sizeof(float) * static_cast<size_t>(p.G_max) * std::max<long long>(p.slots_cap, 1) * 8);
     p.o_dbg = take(sizeof(double) * (2 * static_cast<size_t>(p.PR) * K + 64));
-    p.o_summ = take(sizeof(double) * 20 * static_cast<size_t>(p.PR) * K);   // marginal summaries (R28)
+    p.o_summ = take(sizeof(double) * 25 * static_cast<size_t>(p.PR) * K);   // marginal summaries (R28; 5 classes with R30)
     // log-joint gradient service: per-draw partials of at most 64 MiB worth of groups (at least one)
-    const size_t pd_group_bytes = sizeof(float) * 128 * static_cast<size_t>(std::max<long long>(p.slots_cap, 1));
+    const size_t pd_group_bytes = sizeof(float) * 160 * static_cast<size_t>(std::max<long long>(p.slots_cap, 1));
     p.pd_groups = static_cast<int>(std::min<size_t>(p.gpi_max, std::max<size_t>(1, (size_t(64) << 20) / pd_group_bytes)));
     p.o_pd = take(pd_group_bytes * p.pd_groups);
     p.o_lpk = take(sizeof(float) * 32 * static_cast<size_t>(K) * p.pd_groups);
-    p.o_zeta = take(sizeof(float4) * static_cast<size_t>(p.S_pad) * K);
-    p.o_gradz = take(sizeof(float4) * static_cast<size_t>(p.S_pad) * K);
+    p.o_zeta = take(sizeof(float) * 5 * static_cast<size_t>(p.S_pad) * K);    // float4 [S_pad][K], then float [S_pad][K] (alpha)
+    p.o_gradz = take(sizeof(float) * 5 * static_cast<size_t>(p.S_pad) * K);
     p.o_lls = take(sizeof(double) * 2 * p.S_pad);
     // split kernel (PS > 1): partial profiles of every (group, tile, share) and two counters per (group, tile)
     p.o_partial = take(p.PS > 1 ? sizeof(float) * kPT * 32 * static_cast<size_t>(p.G_max) * p.n_tile * p.PS : 0);
     p.o_tcnt = take(sizeof(unsigned int) * 2 * static_cast<size_t>(p.G_max) * p.n_tile);
     p.o_trng = take(sizeof(int2) * (static_cast<size_t>(p.n_tile) + 1));
+    const bool model = hyp->asymmetry || hyp->width_sec;    // R30 buffers only when the extension is on
+    p.o_ia = take(model ? sizeof(float) * gk32 : 0);
+    p.o_epsa = take(model ? sizeof(float) * gk32 : 0);
+    p.o_parta = take(model ? sizeof(float) * 2 * static_cast<size_t>(p.G_max) * std::max<long long>(p.slots_cap, 1) : 0);
+    p.o_pksec = take(hyp->width_sec ? sizeof(float) * (p.tile_cap + 1) : 0);
+    p.o_secmax = take(sizeof(float) * K);
     p.total = o;
     *pl = p;
     return true;
 }
 
 // ---- static tables (R16, R27) -----------------------------------------------------------------------
-struct HostPeak { long long j; double d; double I; int k; };   // nearest grid index, p_m - x_j, intensity, phase
+struct HostPeak { long long j; double d; double I; int k; double inv_s; };   // nearest grid index, p_m - x_j, intensity, phase, cos(p_m / 2) (R30)
 
 struct Tables {
     std::vector<PeakRec> pk_tile;     // per-tile phase-major peak lists (+1 padding record)
+    std::vector<float> pk_sec;        // cos(p_m / 2) of every record's peak (sec width term, R30)
     std::vector<int4> run_tab;        // (m0, m1, phase, slot) per phase run (+1 padding header)
     std::vector<int2> share_rng;      // [n_tile][PS] run ranges of the shares
     std::vector<int> seg_order, slot_ofs;
@@ -207,6 +214,7 @@ const char* build_tables(const Plan& pl, int64_t N, int K, const std::vector<Hos
     const int n_runs = run_base[n_tile];
     if (n_ent > pl.tile_cap || n_runs > pl.slots_cap) return "internal: table bound exceeded";
     // pass 2: fill the lists, the run headers (m0, m1, phase, 0) and the clipped pair count of every run
+    T->pk_sec.assign(static_cast<size_t>(n_ent) + 1, 1.0f);
     T->pk_tile.assign(static_cast<size_t>(n_ent) + 1, PeakRec{0, 0.f, 0.f, 0});   // +1: the kernel prefetches one
     T->run_tab.assign(static_cast<size_t>(n_runs) + 1, make_int4(0, 0, 0, 0));    // record / header past the end
     T->share_rng.assign(static_cast<size_t>(n_tile) * PSn, make_int2(0, 0));
@@ -227,6 +235,7 @@ const char* build_tables(const Plan& pl, int64_t N, int K, const std::vector<Hos
             const long long e = ent_cur[t]++;
             T->pk_tile[e] = PeakRec{static_cast<int>(dj), static_cast<float>(p.d), static_cast<float>(p.I),
                                     static_cast<int>(n << 1) | (full ? 1 : 0)};
+            T->pk_sec[e] = static_cast<float>(p.inv_s);
             if (last_k[t] != p.k) {
                 last_k[t] = p.k;
                 T->run_tab[run_cur[t]++] = make_int4(static_cast<int>(e), static_cast<int>(e), p.k, 0);
@@ -337,6 +346,8 @@ int install_tables(xrdvi* h, const Tables& T, const std::vector<long long>& nck,
     CU(cudaMemcpyAsync(w + pl.o_sord, T.seg_order.data(), sizeof(int) * T.seg_order.size(), cudaMemcpyHostToDevice, st));
     CU(cudaMemcpyAsync(w + pl.o_sofs, T.slot_ofs.data(), sizeof(int) * T.slot_ofs.size(), cudaMemcpyHostToDevice, st));
     CU(cudaMemcpyAsync(w + pl.o_trng, T.tile_rng.data(), sizeof(int2) * T.tile_rng.size(), cudaMemcpyHostToDevice, st));
+    if (h->hyp.width_sec)
+        CU(cudaMemcpyAsync(w + pl.o_pksec, T.pk_sec.data(), sizeof(float) * T.pk_sec.size(), cudaMemcpyHostToDevice, st));
     if (at_create) {
         d.n_slots = std::max(T.n_slots, 1);
         d.split = T.pairs / (static_cast<long long>(pl.n_tile) * pl.PS * kPT) >= 512 ? 1 : 0;   // peaks per work item
@@ -382,32 +393,49 @@ bool use_split(const Dev& d) {
     return d.TW == 1 && d.PS > 1 && d.split;
 }
 
+// one CTA shape: the staged variant when the tile lists fit (TW = 1), the R30 model variant when the asymmetry or the
+// sec term is on (instantiated for TW = 1 only; make_plan never selects another TW for them)
+template <int TW, int PS, bool BWD>
+void launch_tile_shape(const Dev& d, dim3 grid, cudaStream_t st, bool pdl, float* f_dbg, long long n_dbg) {
+    const dim3 block(32 * TW * PS);
+    if constexpr (TW == 1) {
+        if (d.model) {
+            if (d.stage) launch_k(elbo_tile_kernel<1, PS, BWD, true, 1>, grid, block, st, pdl, d, f_dbg, n_dbg);
+            else launch_k(elbo_tile_kernel<1, PS, BWD, false, 1>, grid, block, st, pdl, d, f_dbg, n_dbg);
+            return;
+        }
+        if (d.stage) { launch_k(elbo_tile_kernel<1, PS, BWD, true, 0>, grid, block, st, pdl, d, f_dbg, n_dbg); return; }
+    }
+    launch_k(elbo_tile_kernel<TW, PS, BWD, false, 0>, grid, block, st, pdl, d, f_dbg, n_dbg);
+}
+
+template <int PS, bool BWD>
+void launch_split_shape(const Dev& d, dim3 grid, cudaStream_t st, bool pdl, float* f_dbg, long long n_dbg) {
+    if (d.model) launch_k(elbo_split_kernel<PS, BWD, 1>, grid, dim3(32), st, pdl, d, f_dbg, n_dbg);
+    else launch_k(elbo_split_kernel<PS, BWD, 0>, grid, dim3(32), st, pdl, d, f_dbg, n_dbg);
+}
+
 template <bool BWD>
 void launch_tile(const Dev& d, cudaStream_t st, float* f_dbg, long long n_dbg, bool pdl = false) {
     if (BWD && use_split(d)) {   // forward-only launches (debug, timing) always take the fused kernel
         const unsigned items = static_cast<unsigned>(d.n_tile) * d.PS * d.G;
-        const unsigned grid = BWD ? 2 * items : items + static_cast<unsigned>(d.n_tile) * d.G;
+        const dim3 grid(BWD ? 2 * items : items + static_cast<unsigned>(d.n_tile) * d.G);
         switch (d.PS) {
-            case 4: launch_k(elbo_split_kernel<4, BWD>, dim3(grid), dim3(32), st, pdl, d, f_dbg, n_dbg); break;
+            case 4: launch_split_shape<4, BWD>(d, grid, st, pdl, f_dbg, n_dbg); break;
 #ifdef XRDVI_TUNING
-            case 3: launch_k(elbo_split_kernel<3, BWD>, dim3(grid), dim3(32), st, pdl, d, f_dbg, n_dbg); break;
-            case 2: launch_k(elbo_split_kernel<2, BWD>, dim3(grid), dim3(32), st, pdl, d, f_dbg, n_dbg); break;
-            case 5: launch_k(elbo_split_kernel<5, BWD>, dim3(grid), dim3(32), st, pdl, d, f_dbg, n_dbg); break;
-            case 6: launch_k(elbo_split_kernel<6, BWD>, dim3(grid), dim3(32), st, pdl, d, f_dbg, n_dbg); break;
-            case 8: launch_k(elbo_split_kernel<8, BWD>, dim3(grid), dim3(32), st, pdl, d, f_dbg, n_dbg); break;
+            case 3: launch_split_shape<3, BWD>(d, grid, st, pdl, f_dbg, n_dbg); break;
+            case 2: launch_split_shape<2, BWD>(d, grid, st, pdl, f_dbg, n_dbg); break;
+            case 5: launch_split_shape<5, BWD>(d, grid, st, pdl, f_dbg, n_dbg); break;
+            case 6: launch_split_shape<6, BWD>(d, grid, st, pdl, f_dbg, n_dbg); break;
+            case 8: launch_split_shape<8, BWD>(d, grid, st, pdl, f_dbg, n_dbg); break;
 #endif
             default: break;
         }
         return;
     }
     const dim3 grid(d.G, d.n_seg);   // x = draw group (dispatched fastest), y = position in seg_order
-#define XRDVI_TILE_CASE(TW_, PS_)                                                                                \
-    case TW_ * 16 + PS_:                                                                                        \
-        if (TW_ == 1 && d.stage)                                                                                \
-            launch_k(elbo_tile_kernel<1, PS_, BWD, true>, grid, dim3(32 * PS_), st, pdl, d, f_dbg, n_dbg);       \
-        else                                                                                                    \
-            launch_k(elbo_tile_kernel<TW_, PS_, BWD, false>, grid, dim3(32 * TW_ * PS_), st, pdl, d, f_dbg, n_dbg); \
-        break;
+#define XRDVI_TILE_CASE(TW_, PS_) \
+    case TW_ * 16 + PS_: launch_tile_shape<TW_, PS_, BWD>(d, grid, st, pdl, f_dbg, n_dbg); break;
     switch (d.TW * 16 + d.PS) {
         XRDVI_TILE_CASE(1, 1) XRDVI_TILE_CASE(1, 4)      // the shapes choose_shape selects
 #ifdef XRDVI_TUNING
@@ -532,6 +560,48 @@ int begin_steps(xrdvi* h, int S, uint64_t seed) {
     return XRDVI_OK;
 }
 
+// External <-> device layout of a state-shaped array.  External (include/xrdvi.h): float [PR][2][K][C], C = 4 or 5
+// (hyper.asymmetry, R30).  Device: the [PR][2][K][4] block of the four base classes, followed by [PR][2][K] for alpha.
+size_t block_floats(const xrdvi* h) { return static_cast<size_t>(h->plan.PR) * (h->hyp.asymmetry ? 10 : 8) * h->K; }
+
+int download_block(xrdvi* h, const float* dev, float* out) {   // synchronises the stream
+    const size_t n = block_floats(h);
+    if (!h->hyp.asymmetry) {
+        CU(cudaMemcpyAsync(out, dev, sizeof(float) * n, cudaMemcpyDeviceToHost, h->stream));
+        CU(cudaStreamSynchronize(h->stream));
+        return XRDVI_OK;
+    }
+    std::vector<float> tmp(n);
+    CU(cudaMemcpyAsync(tmp.data(), dev, sizeof(float) * n, cudaMemcpyDeviceToHost, h->stream));
+    CU(cudaStreamSynchronize(h->stream));
+    const size_t rows = static_cast<size_t>(h->plan.PR) * 2 * h->K;   // (inst, m | l, k)
+    const float* a = tmp.data() + rows * 4;
+    for (size_t r = 0; r < rows; ++r) {
+        for (int c = 0; c < 4; ++c) out[r * 5 + c] = tmp[r * 4 + c];
+        out[r * 5 + 4] = a[r];
+    }
+    return XRDVI_OK;
+}
+
+int upload_block(xrdvi* h, const float* in, float* dev) {      // synchronises the stream
+    const size_t n = block_floats(h);
+    if (!h->hyp.asymmetry) {
+        CU(cudaMemcpyAsync(dev, in, sizeof(float) * n, cudaMemcpyHostToDevice, h->stream));
+        CU(cudaStreamSynchronize(h->stream));
+        return XRDVI_OK;
+    }
+    std::vector<float> tmp(n);
+    const size_t rows = static_cast<size_t>(h->plan.PR) * 2 * h->K;
+    float* a = tmp.data() + rows * 4;
+    for (size_t r = 0; r < rows; ++r) {
+        for (int c = 0; c < 4; ++c) tmp[r * 4 + c] = in[r * 5 + c];
+        a[r] = in[r * 5 + 4];
+    }
+    CU(cudaMemcpyAsync(dev, tmp.data(), sizeof(float) * n, cudaMemcpyHostToDevice, h->stream));
+    CU(cudaStreamSynchronize(h->stream));
+    return XRDVI_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -559,6 +629,10 @@ void xrdvi_default_hyper(xrdvi_hyper* hy) {
     hy->n_restarts = 1;
     hy->likelihood = 0;
     hy->optimizer = 0;
+    hy->asymmetry = 0;
+    hy->width_sec = 0;
+    hy->alpha_mu = 1.0;        // B.2
+    hy->alpha_sigma = 0.2;
 }
 
 size_t xrdvi_workspace_bytes(int64_t N, int32_t K, int64_t M, int32_t S_max, double two_theta_step,
@@ -580,6 +654,9 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
         return fail(XRDVI_E_INVALID_ARG, "likelihood must be 0 (Gaussian) or 1 (Poisson)");
     if (hyp->optimizer != 0 && hyp->optimizer != 1)
         return fail(XRDVI_E_INVALID_ARG, "optimizer must be 0 (Adam) or 1 (natural gradient)");
+    if ((hyp->asymmetry != 0 && hyp->asymmetry != 1) || (hyp->width_sec != 0 && hyp->width_sec != 1))
+        return fail(XRDVI_E_INVALID_ARG, "asymmetry and width_sec must be 0 or 1");
+    if (hyp->asymmetry && !(hyp->alpha_sigma > 0)) return fail(XRDVI_E_INVALID_ARG, "non-positive alpha_sigma");
     if (N < 2 || K < 1 || S_max < 1) return fail(XRDVI_E_INVALID_ARG, "N >= 2, K >= 1, S_max >= 1 required");
     if (hyp->n_patterns < 1 || hyp->n_restarts < 1) return fail(XRDVI_E_INVALID_ARG, "P, R >= 1 required");
     if (!(hyp->mu_sigma > 0) || !(hyp->w_shape > 0) || !(hyp->w_rate > 0) || !(hyp->fwhm_ref > 0) ||
@@ -628,6 +705,7 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
     std::vector<HostPeak> all_peaks;
     all_peaks.reserve(M);
     std::vector<double> area(K, 0.0);
+    std::vector<float> sec_max(K, 1.0f);
     double imax = 0.0;
     for (int k = 0; k < K; ++k)
         for (int64_t m = ofs[k]; m < ofs[k + 1]; ++m) {
@@ -635,7 +713,10 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
             imax = std::max(imax, inten[m]);
             const long long j = static_cast<long long>(std::floor((pos[m] - x[0]) / delta + 0.5));
             const double xj = (j >= 0 && j < N) ? x[j] : x[0] + delta * static_cast<double>(j);
-            all_peaks.push_back({j, pos[m] - xj, inten[m], k});
+            const double inv_s = hyp->width_sec ? std::cos(0.5 * pos[m] * M_PI / 180.0) : 1.0;   // R30: 1 / sec(p_m / 2)
+            if (!(inv_s > 1e-3)) return fail(XRDVI_E_INVALID_ARG, "width_sec needs peak positions below 180 deg");
+            sec_max[k] = std::max(sec_max[k], static_cast<float>(1.0 / inv_s));
+            all_peaks.push_back({j, pos[m] - xj, inten[m], k, inv_s});
         }
     for (int k = 0; k < K; ++k)
         if (!(area[k] > 0.0)) return fail(XRDVI_E_EMPTY_PHASE, "phase " + std::to_string(k) + " has zero total intensity");
@@ -747,6 +828,22 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
     d.tile_cnt2 = d.tile_cnt + static_cast<size_t>(pl.G_max) * pl.n_tile;
     d.tile_rng = reinterpret_cast<int2*>(w + pl.o_trng);
     d.stage = 0;
+    d.asym = hyp->asymmetry;
+    d.sec = hyp->width_sec;
+    d.model = (hyp->asymmetry || hyp->width_sec) ? 1 : 0;
+    d.alpha_mu = static_cast<float>(hyp->alpha_mu);
+    d.alpha_inv_var = static_cast<float>(1.0 / (hyp->alpha_sigma * hyp->alpha_sigma));
+    d.alpha_logc = static_cast<float>(-std::log(hyp->alpha_sigma * std::sqrt(2.0 * M_PI)));
+    d.pk_sec = reinterpret_cast<float*>(w + pl.o_pksec);
+    d.sec_max = reinterpret_cast<float*>(w + pl.o_secmax);
+    const size_t a_ofs = static_cast<size_t>(pl.PR) * 8 * K;      // the alpha companion sits behind every [PR][2][K][4] block
+    d.var_a = d.var + a_ofs;
+    d.mom1_a = d.mom1 + a_ofs;
+    d.mom2_a = d.mom2 + a_ofs;
+    d.grad_a = d.grad + a_ofs;
+    d.ia = reinterpret_cast<float*>(w + pl.o_ia);
+    d.eps_a = reinterpret_cast<float*>(w + pl.o_epsa);
+    d.parta = reinterpret_cast<float*>(w + pl.o_parta);
     set_S(h, S_max);
 
     cudaStream_t st = h->stream;
@@ -759,6 +856,7 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
     chk(up(pl.o_bg, bgf.data(), sizeof(float) * bgf.size()));
     chk(up(pl.o_pat, pat.data(), sizeof(PatConst) * pat.size()));
     chk(up(pl.o_area, area.data(), sizeof(double) * area.size()));
+    chk(up(pl.o_secmax, sec_max.data(), sizeof(float) * sec_max.size()));
     chk(up(pl.o_mh0, m_h0.data(), sizeof(float) * m_h0.size()));
     chk(cudaMemsetAsync(w + pl.o_tcnt, 0, sizeof(unsigned int) * 2 * static_cast<size_t>(pl.G_max) * pl.n_tile, st));
     chk(cudaMemsetAsync(w + pl.o_trace, 0xFF, sizeof(double) * kTraceCap * pl.PR, st));
@@ -787,6 +885,7 @@ void xrdvi_destroy(xrdvi* h) {
 
 int64_t xrdvi_pair_count(const xrdvi* h) { return h ? h->pairs : -1; }
 int64_t xrdvi_window_halfwidth(const xrdvi* h) { return h ? h->n_c : -1; }
+int32_t xrdvi_latent_classes(const xrdvi* h) { return h ? (h->hyp.asymmetry ? 5 : 4) : -1; }
 
 // ---- per-phase (adaptive) windows, R27 ---------------------------------------------------------------
 int xrdvi_set_phase_windows(xrdvi* h, const int32_t* n_ck) {
@@ -818,21 +917,30 @@ int xrdvi_adapt_windows(xrdvi* h, double W, int32_t* n_ck_out) {
     if (!(W > 0.0) || !std::isfinite(W)) return fail(XRDVI_E_INVALID_ARG, "W must be positive");
     CU(cudaSetDevice(h->device));
     const int K = h->K, PR = h->plan.PR;
-    std::vector<float> var(static_cast<size_t>(PR) * 8 * K);
-    CU(cudaMemcpyAsync(var.data(), h->dev.var, sizeof(float) * var.size(), cudaMemcpyDeviceToHost, h->stream));
+    std::vector<float> var(static_cast<size_t>(PR) * 10 * K);
+    CU(cudaMemcpyAsync(var.data(), h->dev.var, sizeof(float) * block_floats(h), cudaMemcpyDeviceToHost, h->stream));
     CU(cudaStreamSynchronize(h->stream));
+    const float* var_a = var.data() + static_cast<size_t>(PR) * 8 * K;   // alpha companion (R30)
     // the rule, in fp64 on the host from the fp32 state (this is table preprocessing, like create):
     // cutoff_k = max over instances of W E_q[w_k] + |E_q[mu_k]|, E_q[w] = exp(m_w + sigma_w^2 / 2)
     const long long n_min = static_cast<long long>(std::ceil(2.0 * W - 1e-9));
     std::vector<int32_t> nck(K);
     for (int k = 0; k < K; ++k) {
         double cut = 0.0;
+        double smax = 1.0;      // R30: the widest peak of the phase under the sec term
+        if (h->hyp.width_sec)
+            for (const HostPeak& p : h->peaks) if (p.k == k) smax = std::max(smax, 1.0 / p.inv_s);
         for (int i = 0; i < PR; ++i) {
             const float* m = var.data() + static_cast<size_t>(i) * 8 * K;
             const float* l = m + 4 * static_cast<size_t>(K);
             const double sw = std::exp(static_cast<double>(l[4 * k + 2]));
-            const double ci = W * std::exp(static_cast<double>(m[4 * k + 2]) + 0.5 * sw * sw) +
-                              std::fabs(static_cast<double>(m[4 * k + 1]));
+            double wbar = std::exp(static_cast<double>(m[4 * k + 2]) + 0.5 * sw * sw) * smax;
+            if (h->hyp.asymmetry) {   // R30: the high-angle side is alpha times wider
+                const double sa = std::exp(static_cast<double>(var_a[static_cast<size_t>(i) * 2 * K + K + k]));
+                const double abar = std::exp(static_cast<double>(var_a[static_cast<size_t>(i) * 2 * K + k]) + 0.5 * sa * sa);
+                if (abar > 1.0) wbar *= abar;
+            }
+            const double ci = W * wbar + std::fabs(static_cast<double>(m[4 * k + 1]));
             if (!std::isfinite(ci)) return fail(XRDVI_E_INVALID_ARG, "non-finite variational state");
             cut = std::max(cut, ci);
         }
@@ -884,10 +992,8 @@ int xrdvi_reset_state_restart(xrdvi* h, uint64_t seed, int32_t restart_offset) {
 int xrdvi_get_state(xrdvi* h, float* var_params, int64_t* step) {
     if (!h) return fail(XRDVI_E_INVALID_ARG, "null handle");
     CU(cudaSetDevice(h->device));
-    if (var_params) {
-        CU(cudaMemcpyAsync(var_params, h->dev.var, sizeof(float) * h->plan.PR * 8 * h->K, cudaMemcpyDeviceToHost, h->stream));
-        CU(cudaStreamSynchronize(h->stream));
-    }
+    if (var_params)
+        if (int rc = download_block(h, h->dev.var, var_params)) return rc;
     if (step) *step = h->step_host;
     return XRDVI_OK;
 }
@@ -895,8 +1001,8 @@ int xrdvi_get_state(xrdvi* h, float* var_params, int64_t* step) {
 int xrdvi_set_state(xrdvi* h, const float* var_params, int64_t step) {
     if (!h || !var_params || step < 0) return fail(XRDVI_E_INVALID_ARG, "null handle/state or negative step");
     CU(cudaSetDevice(h->device));
-    const size_t b = sizeof(float) * h->plan.PR * 8 * h->K;
-    CU(cudaMemcpyAsync(h->dev.var, var_params, b, cudaMemcpyHostToDevice, h->stream));
+    const size_t b = sizeof(float) * block_floats(h);
+    if (int rc = upload_block(h, var_params, h->dev.var)) return rc;
     CU(cudaMemsetAsync(h->dev.mom1, 0, b, h->stream));
     CU(cudaMemsetAsync(h->dev.mom2, 0, b, h->stream));
     h->step_host = step;
@@ -907,10 +1013,8 @@ int xrdvi_set_state(xrdvi* h, const float* var_params, int64_t step) {
 int xrdvi_get_optimizer_state(xrdvi* h, float* mom1, float* mom2, int64_t* adam_steps) {
     if (!h) return fail(XRDVI_E_INVALID_ARG, "null handle");
     CU(cudaSetDevice(h->device));
-    const size_t b = sizeof(float) * h->plan.PR * 8 * h->K;
-    if (mom1) CU(cudaMemcpyAsync(mom1, h->dev.mom1, b, cudaMemcpyDeviceToHost, h->stream));
-    if (mom2) CU(cudaMemcpyAsync(mom2, h->dev.mom2, b, cudaMemcpyDeviceToHost, h->stream));
-    CU(cudaStreamSynchronize(h->stream));
+    if (mom1) if (int rc = download_block(h, h->dev.mom1, mom1)) return rc;
+    if (mom2) if (int rc = download_block(h, h->dev.mom2, mom2)) return rc;
     if (adam_steps) *adam_steps = h->step_host - h->adam_t0;
     return XRDVI_OK;
 }
@@ -919,9 +1023,8 @@ int xrdvi_set_optimizer_state(xrdvi* h, const float* mom1, const float* mom2, in
     if (!h || !mom1 || !mom2) return fail(XRDVI_E_INVALID_ARG, "null handle/moments");
     if (adam_steps < 0 || adam_steps > h->step_host) return fail(XRDVI_E_INVALID_ARG, "adam_steps outside [0, step]");
     CU(cudaSetDevice(h->device));
-    const size_t b = sizeof(float) * h->plan.PR * 8 * h->K;
-    CU(cudaMemcpyAsync(h->dev.mom1, mom1, b, cudaMemcpyHostToDevice, h->stream));
-    CU(cudaMemcpyAsync(h->dev.mom2, mom2, b, cudaMemcpyHostToDevice, h->stream));
+    if (int rc = upload_block(h, mom1, h->dev.mom1)) return rc;
+    if (int rc = upload_block(h, mom2, h->dev.mom2)) return rc;
     h->adam_t0 = h->step_host - adam_steps;
     return write_ctl(h, 0, h->step_host, h->step_host, -1);   // synchronises: the host buffers may go
 }
@@ -935,7 +1038,7 @@ static int begin_eval(xrdvi* h, const float* var_params, int32_t S, uint64_t see
     *var = h->dev.var;
     if (var_params) {
         float* tmp = reinterpret_cast<float*>(h->ws + h->plan.o_vartmp);
-        CU(cudaMemcpyAsync(tmp, var_params, sizeof(float) * h->plan.PR * 8 * h->K, cudaMemcpyHostToDevice, h->stream));
+        if (int urc = upload_block(h, var_params, tmp)) return urc;
         *var = tmp;
     }
     rc = set_S(h, S);
@@ -950,14 +1053,13 @@ int xrdvi_elbo_grad(xrdvi* h, const float* var_params, int32_t S, uint64_t seed,
     if (rc) return rc;
     rc = enqueue_eval(h, var, nullptr, 0, false);
     if (rc) return rc;
-    const size_t b = sizeof(float) * h->plan.PR * 8 * h->K;
     std::vector<double> el(elbo ? h->plan.PR : 0);
-    std::vector<float> gr(grad ? h->plan.PR * 8 * static_cast<size_t>(h->K) : 0);
+    std::vector<float> gr(grad ? block_floats(h) : 0);
     if (elbo) CU(cudaMemcpyAsync(el.data(), h->dev.elbo, sizeof(double) * h->plan.PR, cudaMemcpyDeviceToHost, h->stream));
-    if (grad) CU(cudaMemcpyAsync(gr.data(), h->dev.grad, b, cudaMemcpyDeviceToHost, h->stream));
+    if (grad) { if (int drc = download_block(h, h->dev.grad, gr.data())) return drc; }
     CU(cudaStreamSynchronize(h->stream));
     if (elbo) std::memcpy(elbo, el.data(), sizeof(double) * el.size());
-    if (grad) std::memcpy(grad, gr.data(), b);
+    if (grad) std::memcpy(grad, gr.data(), sizeof(float) * gr.size());
     return XRDVI_OK;
 }
 
@@ -976,10 +1078,10 @@ int xrdvi_fit(xrdvi* h, int32_t iterations, int32_t S, uint64_t seed, float* var
         h->step_host += iterations;
     }
     const int PR = h->plan.PR;
-    std::vector<float> vo(var_out ? PR * 8 * static_cast<size_t>(h->K) : 0);
+    std::vector<float> vo(var_out ? block_floats(h) : 0);
     std::vector<double> inc(incl ? PR * static_cast<size_t>(h->K) : 0);
     std::vector<double> tr;
-    if (var_out) CU(cudaMemcpyAsync(vo.data(), h->dev.var, sizeof(float) * vo.size(), cudaMemcpyDeviceToHost, h->stream));
+    if (var_out) { if (int drc = download_block(h, h->dev.var, vo.data())) return drc; }
     if (incl) {
         double* dbg = reinterpret_cast<double*>(h->ws + h->plan.o_dbg);
         inclusion_kernel<<<PR, 128, 0, h->stream>>>(h->dev, h->hyp.incl_tau, dbg, dbg + static_cast<size_t>(PR) * h->K);
@@ -1024,7 +1126,7 @@ int xrdvi_posterior_summary(xrdvi* h, double* summary) {
     if (!h) return fail(XRDVI_E_INVALID_ARG, "null handle");
     if (!summary) return fail(XRDVI_E_INVALID_ARG, "summary is NULL");
     CU(cudaSetDevice(h->device));
-    const size_t n = 20 * static_cast<size_t>(h->plan.PR) * h->K;
+    const size_t n = (h->hyp.asymmetry ? 25 : 20) * static_cast<size_t>(h->plan.PR) * h->K;
     double* dev = reinterpret_cast<double*>(h->ws + h->plan.o_summ);
     posterior_summary_kernel<<<dim3((h->K + 3) / 4, h->plan.PR), 128, 0, h->stream>>>(h->dev, dev);
     CU(cudaGetLastError());
@@ -1101,14 +1203,31 @@ int xrdvi_logjoint_grad(xrdvi* h, const float* zeta, int64_t n, int32_t pattern,
     if (pattern < 0 || pattern >= h->plan.P) return fail(XRDVI_E_INVALID_ARG, "pattern out of range");
     CU(cudaSetDevice(h->device));
     const int K = h->K;
-    const size_t zb = sizeof(float4) * static_cast<size_t>(n) * K;
-    float4* zeta_dev = reinterpret_cast<float4*>(h->ws + h->plan.o_zeta);
-    float4* grad_dev = reinterpret_cast<float4*>(h->ws + h->plan.o_gradz);
+    const bool asym = h->hyp.asymmetry != 0;
+    const size_t nk = static_cast<size_t>(n) * K;
+    // device layout: float4 [n][K] for the four base classes, then float [n][K] for alpha (R30); the caller's arrays are
+    // [n][K][C]
+    float* zeta_dev = reinterpret_cast<float*>(h->ws + h->plan.o_zeta);
+    float* grad_dev = reinterpret_cast<float*>(h->ws + h->plan.o_gradz);
+    float* zeta_a = zeta_dev + 4 * static_cast<size_t>(h->plan.S_pad) * K;
+    float* grad_a = grad_dev + 4 * static_cast<size_t>(h->plan.S_pad) * K;
     double* ll_dev = reinterpret_cast<double*>(h->ws + h->plan.o_lls);
     double* lpj_dev = ll_dev + h->plan.S_pad;
     float* lpk = reinterpret_cast<float*>(h->ws + h->plan.o_lpk);
     cudaStream_t st = h->stream;
-    CU(cudaMemcpyAsync(zeta_dev, zeta, zb, cudaMemcpyHostToDevice, st));
+    std::vector<float> z4, za;
+    if (asym) {
+        z4.resize(nk * 4);
+        za.resize(nk);
+        for (size_t r = 0; r < nk; ++r) {
+            for (int c = 0; c < 4; ++c) z4[r * 4 + c] = zeta[r * 5 + c];
+            za[r] = zeta[r * 5 + 4];
+        }
+        CU(cudaMemcpyAsync(zeta_dev, z4.data(), sizeof(float) * 4 * nk, cudaMemcpyHostToDevice, st));
+        CU(cudaMemcpyAsync(zeta_a, za.data(), sizeof(float) * nk, cudaMemcpyHostToDevice, st));
+    } else {
+        CU(cudaMemcpyAsync(zeta_dev, zeta, sizeof(float) * 4 * nk, cudaMemcpyHostToDevice, st));
+    }
     set_S(h, static_cast<int>(n));                    // the n points take the place of the draws of one instance
     const int gpi = h->dev.gpi;
     const int inst = pattern * h->plan.R;             // restart 0 of the pattern: only its buffers are used
@@ -1118,21 +1237,32 @@ int xrdvi_logjoint_grad(xrdvi* h, const float* zeta, int64_t n, int32_t pattern,
         dd.g_base = inst * gpi + c0;
         dd.G = ng;
         dd.pd = reinterpret_cast<float*>(h->ws + h->plan.o_pd);
-        zeta_latent_kernel<<<dim3((K + 3) / 4, ng), 128, 0, st>>>(dd, zeta_dev, static_cast<int>(n), c0);
+        zeta_latent_kernel<<<dim3((K + 3) / 4, ng), 128, 0, st>>>(dd, reinterpret_cast<const float4*>(zeta_dev), zeta_a,
+                                                                 static_cast<int>(n), c0);
         launch_tile<true>(dd, st, nullptr, 0);
-        logjoint_grad_kernel<<<dim3(K, ng), 32, 0, st>>>(dd, zeta_dev, static_cast<int>(n), c0, pattern, grad_dev, lpk);
+        logjoint_grad_kernel<<<dim3(K, ng), 32, 0, st>>>(dd, reinterpret_cast<const float4*>(zeta_dev), zeta_a,
+                                                        static_cast<int>(n), c0, pattern,
+                                                        reinterpret_cast<float4*>(grad_dev), grad_a, lpk);
         logjoint_scalar_kernel<<<ng, 32, 0, st>>>(dd, static_cast<int>(n), c0, pattern, lpk, ll_dev, lpj_dev);
         CU(cudaGetLastError());
     }
     std::vector<double> llh(ll ? n : 0), lph(lpj ? n : 0);
-    std::vector<float> gh(grad ? static_cast<size_t>(n) * K * 4 : 0);
+    std::vector<float> gh(grad ? nk * 4 : 0), ga(grad && asym ? nk : 0);
     if (ll) CU(cudaMemcpyAsync(llh.data(), ll_dev, sizeof(double) * n, cudaMemcpyDeviceToHost, st));
     if (lpj) CU(cudaMemcpyAsync(lph.data(), lpj_dev, sizeof(double) * n, cudaMemcpyDeviceToHost, st));
-    if (grad) CU(cudaMemcpyAsync(gh.data(), grad_dev, zb, cudaMemcpyDeviceToHost, st));
+    if (grad) CU(cudaMemcpyAsync(gh.data(), grad_dev, sizeof(float) * 4 * nk, cudaMemcpyDeviceToHost, st));
+    if (grad && asym) CU(cudaMemcpyAsync(ga.data(), grad_a, sizeof(float) * nk, cudaMemcpyDeviceToHost, st));
     CU(cudaStreamSynchronize(st));
     if (ll) std::memcpy(ll, llh.data(), sizeof(double) * n);
     if (lpj) std::memcpy(lpj, lph.data(), sizeof(double) * n);
-    if (grad) std::memcpy(grad, gh.data(), zb);
+    if (grad) {
+        if (!asym) std::memcpy(grad, gh.data(), sizeof(float) * 4 * nk);
+        else
+            for (size_t r = 0; r < nk; ++r) {
+                for (int c = 0; c < 4; ++c) grad[r * 5 + c] = gh[r * 4 + c];
+                grad[r * 5 + 4] = ga[r];
+            }
+    }
     return XRDVI_OK;
 }
 

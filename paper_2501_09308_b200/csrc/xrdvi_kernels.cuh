@@ -130,6 +130,20 @@ struct Dev {
     int g_base;               // group of blockIdx.x = 0 in elbo_tile_kernel (0 except in the service)
     const int2* tile_rng;     // [n_tile + 1] (first run, first record) of every tile's lists
     int stage;                // 1: elbo_tile_kernel copies the tile's lists into shared memory (they fit: host check)
+    // peak asymmetry and the sec width term (reading R30; hyper.asymmetry / hyper.width_sec).  asym = 1: a fifth latent
+    // alpha_k per phase; every state array has a companion for it ([PR][2][K]: m_alpha, l_alpha)
+    int asym, sec;
+    int model;                // 1: asym or sec is on: the tile kernels run tile_phase*_asym (per-draw rows of 160 floats)
+    float alpha_mu, alpha_inv_var, alpha_logc;   // prior Norm(alpha_mu, alpha_sigma): mean, 1/sigma^2, -ln(sigma sqrt(2 pi))
+    const float* pk_sec;      // [records] cos(p_m / 2) = 1 / sec factor of the record's peak (sec = 1 only)
+    const float* sec_max;     // [K] largest sec factor of the phase's peaks (1 without the sec term)
+    float* var_a;             // [PR][2][K]
+    float* mom1_a;
+    float* mom2_a;
+    float* grad_a;
+    float* ia;                // [G][K][32] 1 / alpha of the draw
+    float* eps_a;             // [G][K][32]
+    float* parta;             // [G][n_slots][2] (g_alpha, g_alpha eps_alpha) summed over the 32 draws
     // measurement (xrdvi_debug_timeline): nullptr, or [warps of the launch][4] = (start, end of phase 1, end, SM id | records << 32)
     unsigned long long* tl;
 };
@@ -218,7 +232,8 @@ __device__ __forceinline__ long long philox_iteration(const Ctl* ctl) {
 // a-2, second half: latent record, eps, r and the group's Gaussian-core half-width of phase k for the lane's
 // draw.  Must be called by all 32 lanes of a warp whose lanes hold consecutive draws of group g (the core
 // half-width n_g is a warp maximum); `valid` = false for padding lanes, which contribute nothing.
-__device__ __forceinline__ void emit_latent(const Dev& d, int g, int k, bool valid, const Phys& q, const float4 ep) {
+__device__ __forceinline__ void emit_latent(const Dev& d, int g, int k, bool valid, const Phys& q, const float4 ep,
+                                            float alpha = 1.0f, float ep_a = 0.0f) {
     const int lane = threadIdx.x & 31;
     // 1/w is capped at 5e7 (w >= 2e-8 deg: far outside the model's regime) so that the shared reciprocal
     // rcp(ua ub) of two points can never see an overflowed product
@@ -227,7 +242,11 @@ __device__ __forceinline__ void emit_latent(const Dev& d, int g, int k, bool val
     float4 lt = make_float4(iw2, -q.mu * iw2, q.h * (1.0f - q.r) * kAG * iw, q.h * q.r * kAL * iw);
     // Gaussian core half-width in grid points for this draw: |t'| <= kGaussCut  <=>
     // |i - j| <= kGaussCut w / (2 Delta) + |delta_m + mu| / Delta; |delta_m| <= Delta/2, +1 for rounding
-    float reach = fmaf(d.gcut, q.w, fabsf(q.mu) * d.inv_delta) + 1.5f;
+    // (R30: the high-angle side is alpha times wider, the widest peak of the phase sec_max times)
+    float wide = q.w;
+    if (d.asym) wide *= fmaxf(alpha, 1.0f);
+    if (d.sec) wide *= d.sec_max[k];
+    float reach = fmaf(d.gcut, wide, fabsf(q.mu) * d.inv_delta) + 1.5f;
     if (!valid) {
         lt = make_float4(1.0f, 0.0f, 0.0f, 0.0f);
         reach = 0.0f;
@@ -239,19 +258,39 @@ __device__ __forceinline__ void emit_latent(const Dev& d, int g, int k, bool val
     d.lat[o] = lt;
     d.eps[o] = ep;
     d.rr[o] = q.r;
+    if (d.asym) {
+        d.ia[o] = valid ? fminf(1.0f / alpha, 1.0e6f) : 1.0f;
+        d.eps_a[o] = ep_a;
+    }
     if (lane == 0) d.ng[static_cast<size_t>(g) * d.K + k] = static_cast<int>(reach) + 1;
+}
+
+// R30: the normal of the fifth latent: first Box-Muller output of a second Philox call, bit 31 of the phase word set.
+__device__ __forceinline__ float normal_alpha(unsigned it, unsigned s, unsigned k, unsigned inst, unsigned long long seed) {
+    const uint4 w = philox4x32_10(make_uint4(it, s, k | 0x80000000u, inst),
+                                  make_uint2(static_cast<unsigned>(seed), static_cast<unsigned>(seed >> 32)));
+    const float u0 = uniform23(w.x), u1 = uniform23(w.y);
+    float sn, cs;
+    sincospif(2.0f * u1, &sn, &cs);
+    return sqrtf(-2.0f * logf(u0)) * cs;
 }
 
 // a-1 + a-2 for one (instance, phase k, draw s): Philox draw, transform, latent record (all 32 lanes of a warp).
 __device__ __forceinline__ void draw_one(const Dev& d, int inst, int k, int s, unsigned it, unsigned long long seed,
-                                         const float4 m, const float4 l, uint4* __restrict__ raw_out) {
+                                         const float4 m, const float4 l, uint4* __restrict__ raw_out,
+                                         float m_a = 0.0f, float l_a = 0.0f) {
     const int g = inst * d.gpi + (s >> 5);
     const uint4 words = philox4x32_10(make_uint4(it, static_cast<unsigned>(s), static_cast<unsigned>(k),
                                                  static_cast<unsigned>(inst)),
                                       make_uint2(static_cast<unsigned>(seed), static_cast<unsigned>(seed >> 32)));
     const float4 ep = normals_from_words(words);
     const float4 sg = make_float4(expf(l.x), expf(l.y), expf(l.z), expf(l.w));
-    emit_latent(d, g, k, s < d.S, transform(m, sg, ep), ep);
+    float alpha = 1.0f, ep_a = 0.0f;
+    if (d.asym) {
+        ep_a = normal_alpha(it, static_cast<unsigned>(s), static_cast<unsigned>(k), static_cast<unsigned>(inst), seed);
+        alpha = expf(fmaf(expf(l_a), ep_a, m_a));
+    }
+    emit_latent(d, g, k, s < d.S, transform(m, sg, ep), ep, alpha, ep_a);
     if (raw_out) raw_out[(static_cast<size_t>(g) * d.K + k) * 32 + (threadIdx.x & 31)] = words;
 }
 
@@ -266,7 +305,13 @@ __global__ void __launch_bounds__(128) draw_transform_kernel(const Dev d, const 
     const int s = (g - inst * d.gpi) * 32 + lane;
     const float4 m = *reinterpret_cast<const float4*>(var + (static_cast<size_t>(inst) * 2 * d.K + k) * 4);
     const float4 l = *reinterpret_cast<const float4*>(var + (static_cast<size_t>(inst) * 2 * d.K + d.K + k) * 4);
-    draw_one(d, inst, k, s, static_cast<unsigned>(philox_iteration(d.ctl)), d.ctl->seed, m, l, raw_out);
+    float m_a = 0.0f, l_a = 0.0f;
+    if (d.asym) {   // the companion of `var` for alpha sits right behind it: var_a = var + PR * 8 * K (host layout)
+        const float* va = var + static_cast<size_t>(d.PR) * 8 * d.K;
+        m_a = va[static_cast<size_t>(inst) * 2 * d.K + k];
+        l_a = va[static_cast<size_t>(inst) * 2 * d.K + d.K + k];
+    }
+    draw_one(d, inst, k, s, static_cast<unsigned>(philox_iteration(d.ctl)), d.ctl->seed, m, l, raw_out, m_a, l_a);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -850,6 +895,230 @@ __device__ __forceinline__ void tile_phase2(const Dev& d, const Src& src, const 
     }
 }
 
+// ------------------------------------------------------------------------------------------------
+// Peak asymmetry and sec width term (reading R30; A9/A10 PAPER.md:234-239, prior PAPER.md:274,
+// the sec of).  t'' = t' / A, A = alpha for t' >= 0 (x >= rho), 1 below; heights unchanged.  With
+// ia = 1 / alpha and mx = max(t', 0):   t'' = t' + mx (ia - 1),   d t''/d mu = -(2/w) (1 on the low, ia on the high side)
+// so that  sum e L^2 t'' (d t''/d mu factor) = sum e L^2 [t' + mx (ia^2 - 1)],  and  d t''/d alpha = -t''/alpha on the high
+// side only:  alpha d f/d alpha = I [2 c_L t''^2 L^2 + 2 ln2 c_G t''^2 G]_high,  t''_high = mx ia.
+// The sec term multiplies the width of the record's peak by sec(p_m / 2): t', the step and both heights get the factor
+// inv_s = cos(p_m / 2), the mu chain one more.
+// Records whose 16 points are in-window and outside the Gaussian core lie wholly on ONE side of the peak for all 32
+// draws (the core half-width covers the largest sampled shift), so they keep the packed bodies with (t0, step) scaled
+// by ia on the high side; core and window-edge records take the scalar per-point bodies below.
+template <int Q>
+__device__ __forceinline__ void fwd_quad_asym(const PeakGeo& g, float t0, float step, float iam1, float cg2, float cl,
+                                              f32x2& accX, f32x2& accY) {
+    const int lo = max(g.p_lo, 4 * Q), hi = min(g.p_hi, 4 * Q + 3);
+    if (lo > hi) return;                                   // quad outside the window
+    const unsigned span = static_cast<unsigned>(hi - lo);
+    float u[4], m[4], a[4];
+    unpack2(accX, a[0], a[2]);
+    unpack2(accY, a[1], a[3]);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        float t = fmaf(static_cast<float>(4 * Q + i), step, t0);
+        t = fmaf(fmaxf(t, 0.0f), iam1, t);                 // high-angle side: t' / alpha
+        u[i] = fmaf(t, t, 1.0f);
+        m[i] = static_cast<unsigned>(4 * Q + i - lo) <= span ? 1.0f : 0.0f;
+    }
+    const float r01 = rcp_approx(u[0] * u[1]) * cl, r23 = rcp_approx(u[2] * u[3]) * cl;
+    a[0] = fmaf(r01 * u[1], m[0], a[0]);
+    a[1] = fmaf(r01 * u[0], m[1], a[1]);
+    a[2] = fmaf(r23 * u[3], m[2], a[2]);
+    a[3] = fmaf(r23 * u[2], m[3], a[3]);
+    if (g.c_hi >= 4 * Q && g.c_lo <= 4 * Q + 3) {
+#pragma unroll
+        for (int i = 0; i < 4; ++i) a[i] = fmaf(cg2 * m[i], ex2_approx(-u[i]), a[i]);
+    }
+    accX = pack2(a[0], a[2]);
+    accY = pack2(a[1], a[3]);
+}
+
+// a1 = sum e L, a5 = sum e L^2, a2 = sum e g, a6u = sum e u g (g = 2^-u = G/2, u = 1 + t''^2) as in Acc6;
+// a3m = sum e L^2 tm, a4m = sum e g tm with tm = t' + mx (ia^2 - 1) (the mu chain); h1 = sum e mx^2 L^2, h2 = sum e mx^2 g.
+struct Acc8 { float a1, a2, a5, a6u, a3m, a4m, h1, h2; };
+
+template <int Q>
+__device__ __forceinline__ void bwd_quad_asym(const PeakGeo& g, float t0, float step, float iam1, float ia2m1, f32x2 eX,
+                                              f32x2 eY, Acc8& a) {
+    const int lo = max(g.p_lo, 4 * Q), hi = min(g.p_hi, 4 * Q + 3);
+    if (lo > hi) return;
+    const unsigned span = static_cast<unsigned>(hi - lo);
+    float u[4], ev[4], tm[4], em[4];
+    unpack2(eX, ev[0], ev[2]);
+    unpack2(eY, ev[1], ev[3]);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const float tp = fmaf(static_cast<float>(4 * Q + i), step, t0);
+        const float mx = fmaxf(tp, 0.0f);
+        const float t = fmaf(mx, iam1, tp);
+        tm[i] = fmaf(mx, ia2m1, tp);
+        u[i] = fmaf(t, t, 1.0f);
+        const bool in = static_cast<unsigned>(4 * Q + i - lo) <= span;   // out-of-window points: zero residual
+        ev[i] = in ? ev[i] : 0.0f;
+        em[i] = ev[i] * mx * mx;
+    }
+    const float r01 = rcp_approx(u[0] * u[1]), r23 = rcp_approx(u[2] * u[3]);
+    const float L[4] = {r01 * u[1], r01 * u[0], r23 * u[3], r23 * u[2]};
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const float L2 = L[i] * L[i];
+        a.a1 = fmaf(ev[i], L[i], a.a1);
+        a.a5 = fmaf(ev[i], L2, a.a5);
+        a.a3m = fmaf(ev[i] * tm[i], L2, a.a3m);
+        a.h1 = fmaf(em[i], L2, a.h1);
+    }
+    if (g.c_hi >= 4 * Q && g.c_lo <= 4 * Q + 3) {
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const float gg = ex2_approx(-u[i]);
+            a.a2 = fmaf(ev[i], gg, a.a2);
+            a.a6u = fmaf(ev[i] * u[i], gg, a.a6u);
+            a.a4m = fmaf(ev[i] * tm[i], gg, a.a4m);
+            a.h2 = fmaf(em[i], gg, a.h2);
+        }
+    }
+}
+
+// Phase 1 with the asymmetry / sec term (R30).  ia_g: 1 / alpha of the group's draws, already offset by the lane.
+template <class Src>
+__device__ __forceinline__ void tile_phase1_asym(const Dev& d, const Src& src, const TileCtx& c, int2 rng, float (&acc)[kPT]) {
+    f32x2 acc2[kPT / 2];
+#pragma unroll
+    for (int i = 0; i < kPT / 2; ++i) acc2[i] = 0ull;
+    const float* __restrict__ iag = d.ia + static_cast<size_t>(c.g) * d.K * 32 + (threadIdx.x & 31);
+    for (int r = rng.x; r < rng.y; ++r) {
+        const int4 run = src.run(r);
+        const float4 lt = c.lat[static_cast<size_t>(run.z) * 32];
+        const int ngc = c.ngk[run.z];
+        const float ia = d.asym ? iag[static_cast<size_t>(run.z) * 32] : 1.0f;
+        const float iam1 = ia - 1.0f;
+        const float step_k = d.delta * lt.x;
+        const unsigned core_span = static_cast<unsigned>(kPT - 1 + 2 * ngc);
+#pragma unroll 1
+        for (int m = run.x; m < run.y; ++m) {
+            const PeakRec pk = src.rec(m);
+            const float inv_s = d.sec ? d.pk_sec[m] : 1.0f;
+            float step = step_k * inv_s;
+            float t0 = fmaf(static_cast<float>(-pk.dj), step_k, fmaf(-pk.delta, lt.x, lt.y)) * inv_s;
+            const float cl = pk.inten * lt.w * inv_s;
+            const bool core = static_cast<unsigned>(pk.dj + ngc) <= core_span;
+            if ((pk.full & 1) && !core) {                   // one side of the peak for every draw: packed body
+                if (pk.dj < 0) { t0 *= ia; step *= ia; }    // the tile lies above the peak: high-angle side
+                fwd_tile2<false>(t0, step, 0.0f, cl, acc2);
+            } else {
+                const PeakGeo geo = edge_geo(pk.dj, ngc, pk.full >> 1, c.plim);
+                const float cg2 = 2.0f * pk.inten * lt.z * inv_s;
+                fwd_quad_asym<0>(geo, t0, step, iam1, cg2, cl, acc2[0], acc2[1]);
+                fwd_quad_asym<1>(geo, t0, step, iam1, cg2, cl, acc2[2], acc2[3]);
+                fwd_quad_asym<2>(geo, t0, step, iam1, cg2, cl, acc2[4], acc2[5]);
+                fwd_quad_asym<3>(geo, t0, step, iam1, cg2, cl, acc2[6], acc2[7]);
+            }
+        }
+    }
+#pragma unroll
+    for (int Q = 0; Q < kPT / 4; ++Q) {
+        unpack2(acc2[2 * Q], acc[4 * Q], acc[4 * Q + 2]);
+        unpack2(acc2[2 * Q + 1], acc[4 * Q + 1], acc[4 * Q + 3]);
+    }
+}
+
+// Phase 2 with the asymmetry / sec term: ten values per run, (g_h, g_mu, g_w, g_r, g (x) eps) into part8 and
+// (g_alpha, g_alpha eps_alpha) into parta; per-draw mode: five classes per run.
+template <class Src>
+__device__ __forceinline__ void tile_phase2_asym(const Dev& d, const Src& src, const TileCtx& c, int2 rng, const float (&e)[kPT],
+                                                 int pd_row) {
+    if (rng.x >= rng.y) return;
+    const int lane = threadIdx.x & 31;
+    f32x2 e2[kPT / 2], pe2[kPT / 2];
+#pragma unroll
+    for (int Q = 0; Q < kPT / 4; ++Q) {
+        e2[2 * Q] = pack2(e[4 * Q], e[4 * Q + 2]);
+        e2[2 * Q + 1] = pack2(e[4 * Q + 1], e[4 * Q + 3]);
+        pe2[2 * Q] = pack2(static_cast<float>(4 * Q) * e[4 * Q], static_cast<float>(4 * Q + 2) * e[4 * Q + 2]);
+        pe2[2 * Q + 1] = pack2(static_cast<float>(4 * Q + 1) * e[4 * Q + 1], static_cast<float>(4 * Q + 3) * e[4 * Q + 3]);
+    }
+    const size_t gk = static_cast<size_t>(c.g) * d.K * 32 + lane;
+    for (int r = rng.x; r < rng.y; ++r) {
+        const int4 run = src.run(r);
+        const size_t o = gk + static_cast<size_t>(run.z) * 32;
+        const float4 lt = c.lat[static_cast<size_t>(run.z) * 32];
+        const int ngc = c.ngk[run.z];
+        const float4 ep = d.eps[o];
+        const float rmix = d.rr[o];
+        const float ia = d.asym ? d.ia[o] : 1.0f;
+        const float ep_a = d.asym ? d.eps_a[o] : 0.0f;
+        const float iam1 = ia - 1.0f, ia2 = ia * ia, ia2m1 = ia2 - 1.0f;
+        const float step_k = d.delta * lt.x;
+        const unsigned core_span = static_cast<unsigned>(kPT - 1 + 2 * ngc);
+        // per run, I_m / s_m folded in: B1 = sum e L, B5 = sum e L^2, B2 = sum e G, B6 = sum e G t''^2,
+        // B3 = sum e L^2 t'' (mu-chain factor), B4 = sum e G t'' (same), H1 = sum_high e L^2 t''^2, H2 = sum_high e G t''^2
+        float B1 = 0.f, B2 = 0.f, B3 = 0.f, B4 = 0.f, B5 = 0.f, B6 = 0.f, H1 = 0.f, H2 = 0.f;
+#pragma unroll 1
+        for (int m = run.x; m < run.y; ++m) {
+            const PeakRec pk = src.rec(m);
+            const float inv_s = d.sec ? d.pk_sec[m] : 1.0f;
+            float step = step_k * inv_s;
+            float t0 = fmaf(static_cast<float>(-pk.dj), step_k, fmaf(-pk.delta, lt.x, lt.y)) * inv_s;
+            const float wI = pk.inten * inv_s;              // height factor of the record
+            const bool core = static_cast<unsigned>(pk.dj + ngc) <= core_span;
+            if ((pk.full & 1) && !core) {
+                const bool high = pk.dj < 0;
+                if (high) { t0 *= ia; step *= ia; }
+                Acc6x2 a2 = {0ull, 0ull, 0ull, 0ull, 0ull, 0ull};
+                bwd_tile2<false>(t0, step, e2, pe2, a2);
+                const float a1 = hsum2(a2.a1), a5 = hsum2(a2.a5), a3p = hsum2(a2.a3p);
+                const float m3 = fmaf(t0, a5, step * a3p);  // sum e L^2 t''
+                B1 = fmaf(wI, a1, B1);
+                B5 = fmaf(wI, a5, B5);
+                B3 = fmaf(wI * inv_s * (high ? ia : 1.0f), m3, B3);
+                if (high) H1 = fmaf(wI, a1 - a5, H1);       // t''^2 L^2 = L - L^2
+            } else {
+                const PeakGeo geo = edge_geo(pk.dj, ngc, pk.full >> 1, c.plim);
+                Acc8 a = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+                bwd_quad_asym<0>(geo, t0, step, iam1, ia2m1, e2[0], e2[1], a);
+                bwd_quad_asym<1>(geo, t0, step, iam1, ia2m1, e2[2], e2[3], a);
+                bwd_quad_asym<2>(geo, t0, step, iam1, ia2m1, e2[4], e2[5], a);
+                bwd_quad_asym<3>(geo, t0, step, iam1, ia2m1, e2[6], e2[7], a);
+                const float i2 = 2.0f * wI;                 // g = G/2 in the Gaussian sums
+                B1 = fmaf(wI, a.a1, B1);
+                B2 = fmaf(i2, a.a2, B2);
+                B5 = fmaf(wI, a.a5, B5);
+                B6 = fmaf(i2, a.a6u - a.a2, B6);
+                B3 = fmaf(wI * inv_s, a.a3m, B3);
+                B4 = fmaf(i2 * inv_s, a.a4m, B4);
+                H1 = fmaf(wI * ia2, a.h1, H1);
+                H2 = fmaf(i2 * ia2, a.h2, H2);
+            }
+        }
+        const float cG = lt.z, cL = lt.w;
+        float v[8];
+        v[0] = fmaf(cL, B1, cG * B2);
+        v[1] = lt.x * (2.0f * cL * B3 + (2.0f * kLn2) * cG * B4);
+        v[2] = -(cL * (2.0f * B5 - B1) + cG * (B2 - (2.0f * kLn2) * B6));
+        v[3] = (1.0f - rmix) * cL * B1 - rmix * cG * B2;
+        const float va = d.asym ? 2.0f * cL * H1 + (2.0f * kLn2) * cG * H2 : 0.0f;   // alpha d ll / d alpha
+        if (d.pd) {   // gradient service: keep the draws apart, five classes per run
+            float* __restrict__ o5 = d.pd + (static_cast<size_t>(pd_row) * d.n_slots + run.w) * 160 + lane;
+            o5[0] = v[0]; o5[32] = v[1]; o5[64] = v[2]; o5[96] = v[3]; o5[128] = va;
+            continue;
+        }
+        v[4] = v[0] * ep.x; v[5] = v[1] * ep.y; v[6] = v[2] * ep.z; v[7] = v[3] * ep.w;
+        const float tot = warp_reduce8(v);
+        float* __restrict__ part = d.part8 + static_cast<size_t>(c.g) * d.n_slots * 8;
+        if (lane < 8) part[static_cast<size_t>(run.w) * 8 + lane] = tot;
+        float s0 = va, s1 = va * ep_a;
+#pragma unroll
+        for (int of = 16; of > 0; of >>= 1) {               // fixed butterfly: every lane ends with the totals
+            s0 += __shfl_xor_sync(0xffffffffu, s0, of);
+            s1 += __shfl_xor_sync(0xffffffffu, s1, of);
+        }
+        if (lane == 0)
+            *reinterpret_cast<float2*>(d.parta + (static_cast<size_t>(c.g) * d.n_slots + run.w) * 2) = make_float2(s0, s1);
+    }
+}
+
 // Fused variant: grid (G, n_seg), block 32*TW*PS; segment = TW consecutive tiles.  Warp w owns tile (w % TW) of the
 // segment and share (w / TW) of that tile's runs; the PS partial profiles meet in shared memory.  Used when the
 // launch has enough tile-warps without splitting (PS = 1: no barrier is ever waited on) and for forward-only runs.
@@ -872,7 +1141,8 @@ constexpr int tile_ctas_per_sm(int TW, int PS) {
 // copies completed on an mbarrier (north_star: "per-tile peak windows ... staged through shared memory/TMA"); the
 // tables are static, so the copies are issued BEFORE griddepcontrol.wait and overlap the predecessor kernel's drain.
 // All PS shares of the CTA then read records and run headers with LDS.128 broadcasts in both phases.
-template <int TW, int PS, bool BWD, bool STAGE>
+// MODEL 0: the base profile (A3-A8); MODEL 1: with the peak asymmetry / sec width term of R30 (tile_phase*_asym).
+template <int TW, int PS, bool BWD, bool STAGE, int MODEL>
 __global__ void __launch_bounds__(32 * TW * PS, tile_ctas_per_sm(TW, PS))
 elbo_tile_kernel(const Dev d, float* __restrict__ f_dbg, long long n_dbg) {
     static_assert(!STAGE || TW == 1, "staging holds one tile list per CTA");
@@ -923,7 +1193,8 @@ elbo_tile_kernel(const Dev d, float* __restrict__ f_dbg, long long n_dbg) {
     float acc[kPT];
 #pragma unroll
     for (int p = 0; p < kPT; ++p) acc[p] = 0.0f;
-    tile_phase1(d, src, c, rng, acc);
+    if constexpr (MODEL == 1) tile_phase1_asym(d, src, c, rng, acc);
+    else tile_phase1(d, src, c, rng, acc);
 
     if (PS > 1) {   // sum the PS partial profiles of the tile: shares 1.. in order onto share 0
         if (ps > 0) {
@@ -965,7 +1236,8 @@ elbo_tile_kernel(const Dev d, float* __restrict__ f_dbg, long long n_dbg) {
         const float4 t = e_s[tw][v][lane];
         e[4 * v] = t.x; e[4 * v + 1] = t.y; e[4 * v + 2] = t.z; e[4 * v + 3] = t.w;
     }
-    tile_phase2(d, src, c, rng, e, blockIdx.x);
+    if constexpr (MODEL == 1) tile_phase2_asym(d, src, c, rng, e, blockIdx.x);
+    else tile_phase2(d, src, c, rng, e, blockIdx.x);
     tl_stamp(d.tl, tl_row, 2);
 }
 
@@ -979,7 +1251,7 @@ elbo_tile_kernel(const Dev d, float* __restrict__ f_dbg, long long n_dbg) {
 // No barrier inside a CTA, items half as long as a fused CTA, phase-2 work fills the tail of phase 1.  All sums keep
 // a fixed order, so results do not depend on the schedule.  grid: n_items * 2 (BWD) or n_items + n_tile * G CTAs
 // (a persistent variant, 3552 CTAs looping over tickets, measured 3 % slower).
-template <int PS, bool BWD>
+template <int PS, bool BWD, int MODEL>
 __global__ void __launch_bounds__(32, XRDVI_TILE_WARPS_PER_SM) elbo_split_kernel(const Dev d, float* __restrict__ f_dbg, long long n_dbg) {
     const int lane = threadIdx.x;
     griddep_launch_dependents();
@@ -1015,7 +1287,8 @@ __global__ void __launch_bounds__(32, XRDVI_TILE_WARPS_PER_SM) elbo_split_kernel
         float acc[kPT];
 #pragma unroll
         for (int p = 0; p < kPT; ++p) acc[p] = 0.0f;
-        tile_phase1(d, SrcGlobal{d.pk_tile, d.run_tab}, c, rng, acc);
+        if constexpr (MODEL == 1) tile_phase1_asym(d, SrcGlobal{d.pk_tile, d.run_tab}, c, rng, acc);
+        else tile_phase1(d, SrcGlobal{d.pk_tile, d.run_tab}, c, rng, acc);
 #pragma unroll
         for (int p = 0; p < kPT; ++p) __stcg(partial + (ps * kPT + p) * 32, acc[p]);
         __threadfence();
@@ -1041,7 +1314,10 @@ __global__ void __launch_bounds__(32, XRDVI_TILE_WARPS_PER_SM) elbo_split_kernel
             d.llpart[(static_cast<size_t>(c.g) * d.n_seg + tile) * 32 + lane] = ss;
             if (f_dbg) tile_debug_profile(d, c, acc, f_dbg, n_dbg);
         }
-        if (BWD) tile_phase2(d, SrcGlobal{d.pk_tile, d.run_tab}, c, rng, ev, gi);
+        if (BWD) {
+            if constexpr (MODEL == 1) tile_phase2_asym(d, SrcGlobal{d.pk_tile, d.run_tab}, c, rng, ev, gi);
+            else tile_phase2(d, SrcGlobal{d.pk_tile, d.run_tab}, c, rng, ev, gi);
+        }
         __syncwarp();
         if (lane == 0) {   // the last phase-2 item of the (tile, group) re-arms its counters for the next launch
             const unsigned n_second = BWD ? PS : 1;
@@ -1093,9 +1369,9 @@ __device__ __forceinline__ void block_reduce(double (&v)[NV], double* smem /* [N
 //  The ELBO is assembled, and the step counted, by finish_step (next tile kernel, or finish_step_kernel).
 __global__ void __launch_bounds__(kUpdThreads) update_draw_kernel(const Dev d, const float* __restrict__ var_in,
                                                                   int do_update) {
-    __shared__ double red[(kUpdThreads / 32) * 9];
-    __shared__ float new_ml[8];
-    __shared__ double tot_s[8];
+    __shared__ double red[(kUpdThreads / 32) * 11];
+    __shared__ float new_ml[10];
+    __shared__ double tot_s[10];
     const int k = blockIdx.x, inst = blockIdx.y;
     const int pat = inst / d.R;
     const PatConst pc = d.pat[pat];
@@ -1136,9 +1412,13 @@ __global__ void __launch_bounds__(kUpdThreads) update_draw_kernel(const Dev d, c
         const float4 m = *reinterpret_cast<const float4*>(var_in + (static_cast<size_t>(inst) * 2 * d.K + k) * 4);
         const float4 l = *reinterpret_cast<const float4*>(var_in + (static_cast<size_t>(inst) * 2 * d.K + d.K + k) * 4);
         const float4 sg = make_float4(expf(l.x), expf(l.y), expf(l.z), expf(l.w));
-        double v[9];
+        // R30: the fifth latent's parameters sit behind the [PR][2][K][4] block of every state array
+        const float* __restrict__ va_in = var_in + static_cast<size_t>(d.PR) * 8 * d.K + static_cast<size_t>(inst) * 2 * d.K;
+        const float m_a = d.asym ? va_in[k] : 0.0f, l_a = d.asym ? va_in[d.K + k] : 0.0f;
+        const float sg_a = expf(l_a);
+        double v[11];   // [0..3] sum g, [4..7] sum g eps, [8] sum log prior + log Jacobian, [9] sum g_alpha, [10] sum g_alpha eps_alpha
 #pragma unroll
-        for (int i = 0; i < 9; ++i) v[i] = 0.0;
+        for (int i = 0; i < 11; ++i) v[i] = 0.0;
         // likelihood part: partials of phase k, all groups of the instance
         const int s0 = d.slot_ofs[k], s1 = d.slot_ofs[k + 1];
         const int n_sl = s1 - s0;
@@ -1165,6 +1445,15 @@ __global__ void __launch_bounds__(kUpdThreads) update_draw_kernel(const Dev d, c
                 }
             }
         }
+        if (d.asym) {
+            for (int idx = threadIdx.x; idx < n_part; idx += kUpdThreads) {
+                const int gi = idx / n_sl, sl = s0 + (idx - gi * n_sl);
+                const float2 pa = *reinterpret_cast<const float2*>(
+                    d.parta + (static_cast<size_t>(inst * d.gpi + gi) * d.n_slots + sl) * 2);
+                v[9] += pa.x;
+                v[10] += pa.y;
+            }
+        }
         // prior + Jacobian part, per draw
         for (int s = threadIdx.x; s < d.S; s += kUpdThreads) {
             const int g = inst * d.gpi + (s >> 5), lane = s & 31;
@@ -1184,11 +1473,21 @@ __global__ void __launch_bounds__(kUpdThreads) update_draw_kernel(const Dev d, c
                 v[4 + c] += static_cast<double>(gz[c] * e4[c]);
             }
             v[8] += static_cast<double>(lp);
+            if (d.asym) {      // alpha = exp(zeta) ~ Norm(alpha_mu, alpha_sigma) (B.2 PAPER.md:274) + log Jacobian (R30)
+                const float ea = d.eps_a[(static_cast<size_t>(g) * d.K + k) * 32 + lane];
+                const float za = fmaf(sg_a, ea, m_a), al = expf(za), da = al - d.alpha_mu;
+                const float ga = 1.0f - da * d.alpha_inv_var * al;
+                v[8] += static_cast<double>(-0.5f * da * da * d.alpha_inv_var + d.alpha_logc + za);
+                v[9] += static_cast<double>(ga);
+                v[10] += static_cast<double>(ga * ea);
+            }
         }
-        block_reduce<9, kUpdThreads / 32>(v, red);
+        block_reduce<11, kUpdThreads / 32>(v, red);
         if (threadIdx.x == 0) {
 #pragma unroll
             for (int i = 0; i < 8; ++i) tot_s[i] = v[i];
+            tot_s[8] = v[9];
+            tot_s[9] = v[10];
         }
         __syncthreads();
         if (threadIdx.x < 8) {
@@ -1218,18 +1517,45 @@ __global__ void __launch_bounds__(kUpdThreads) update_draw_kernel(const Dev d, c
                 d.var[o] = x;
             }
             new_ml[threadIdx.x] = x;
+        } else if (threadIdx.x < 10 && d.asym) {   // the two parameters of alpha: same update rules
+            const bool is_l = threadIdx.x == 9;
+            const double tot = tot_s[threadIdx.x];
+            const double gd = is_l ? tot * inv_s * static_cast<double>(sg_a) + 1.0 : tot * inv_s;
+            const float gj = static_cast<float>(gd);
+            const size_t o = static_cast<size_t>(inst) * 2 * d.K + (is_l ? d.K : 0) + k;
+            d.grad_a[o] = gj;
+            float x = is_l ? l_a : m_a;
+            if (do_update) {
+                if (d.optimizer == 1) {
+                    x += d.lr * (is_l ? 0.5f * gj : sg_a * sg_a * gj);
+                } else {
+                    const float stepf = static_cast<float>(step + 1 - d.ctl->adam_t0);
+                    const float bc1 = 1.0f - powf(d.beta1, stepf);
+                    const float bc2 = 1.0f - powf(d.beta2, stepf);
+                    const float m1 = d.beta1 * d.mom1_a[o] + (1.0f - d.beta1) * gj;
+                    const float m2 = d.beta2 * d.mom2_a[o] + (1.0f - d.beta2) * gj * gj;
+                    d.mom1_a[o] = m1;
+                    d.mom2_a[o] = m2;
+                    x += d.lr * (m1 / bc1) / (sqrtf(m2 / bc2) + d.adam_eps);
+                }
+                if (is_l) x = fminf(fmaxf(x, -12.0f), 2.0f);
+                d.var_a[o] = x;
+            }
+            new_ml[threadIdx.x] = x;
         }
         if (threadIdx.x == 0)  // mean log prior + Jacobian of the phase, plus its entropy sum_c (l_c + 1/2 ln 2 pi e)
             d.elbo_k[static_cast<size_t>(inst) * (d.K + 1) + k] =
                 v[8] * inv_s + (static_cast<double>(l.x) + static_cast<double>(l.y) + static_cast<double>(l.z) +
-                                static_cast<double>(l.w)) + 4.0 * 1.4189385332046727;
+                                static_cast<double>(l.w)) + 4.0 * 1.4189385332046727 +
+                (d.asym ? static_cast<double>(l_a) + 1.4189385332046727 : 0.0);
         if (do_update) {       // draws of the next step from the updated parameters
             __syncthreads();
             const float4 mn = make_float4(new_ml[0], new_ml[1], new_ml[2], new_ml[3]);
             const float4 ln = make_float4(new_ml[4], new_ml[5], new_ml[6], new_ml[7]);
             const unsigned it = static_cast<unsigned>(step + 2);
             const int s_pad = d.gpi * 32;
-            for (int s = threadIdx.x; s < s_pad; s += kUpdThreads) draw_one(d, inst, k, s, it, seed, mn, ln, nullptr);
+            const float mna = d.asym ? new_ml[8] : 0.0f, lna = d.asym ? new_ml[9] : 0.0f;
+            for (int s = threadIdx.x; s < s_pad; s += kUpdThreads) draw_one(d, inst, k, s, it, seed, mn, ln, nullptr, mna, lna);
         }
     }
 
@@ -1250,18 +1576,29 @@ __global__ void __launch_bounds__(128) inclusion_kernel(const Dev d, double tau,
     const int inst = blockIdx.x;
     const float* m = d.var + static_cast<size_t>(inst) * 8 * d.K;
     const float* l = m + 4 * d.K;
+    // R30: a split peak has area (1 + alpha) / 2, alpha at its mean under q
+    const float* ma = d.var_a + static_cast<size_t>(inst) * 2 * d.K;
+    auto area_of = [&](int k) {
+        double a = d.area[k];
+        if (d.asym) {
+            const double sa = exp(static_cast<double>(ma[d.K + k]));
+            a *= 0.5 * (1.0 + exp(static_cast<double>(ma[k]) + 0.5 * sa * sa));
+        }
+        return a;
+    };
     double v[1] = {0.0};
     for (int k = threadIdx.x; k < d.K; k += 128) {
         const double s = exp(static_cast<double>(l[4 * k]));
-        v[0] += d.area[k] * exp(static_cast<double>(m[4 * k]) + 0.5 * s * s);
+        v[0] += area_of(k) * exp(static_cast<double>(m[4 * k]) + 0.5 * s * s);
     }
     block_reduce<1, 4>(v, red);
     const double tbar = v[0];
     for (int k = threadIdx.x; k < d.K; k += 128) {
         const double s = exp(static_cast<double>(l[4 * k]));
-        const double z = (static_cast<double>(m[4 * k]) - log(tau * tbar / d.area[k])) / s;
+        const double ak = area_of(k);
+        const double z = (static_cast<double>(m[4 * k]) - log(tau * tbar / ak)) / s;
         incl[static_cast<size_t>(inst) * d.K + k] = 0.5 * erfc(-z * 0.70710678118654752440);
-        ratio[static_cast<size_t>(inst) * d.K + k] = d.area[k] * exp(static_cast<double>(m[4 * k]) + 0.5 * s * s) / tbar;
+        ratio[static_cast<size_t>(inst) * d.K + k] = ak * exp(static_cast<double>(m[4 * k]) + 0.5 * s * s) / tbar;
     }
 }
 
@@ -1278,7 +1615,16 @@ __global__ void __launch_bounds__(128) posterior_summary_kernel(const Dev d, dou
     const int inst = blockIdx.y;
     const float* mp = d.var + static_cast<size_t>(inst) * 8 * d.K + 4 * k;
     const double z975 = 1.95996398454005423552;
-    double* ok = out + (static_cast<size_t>(inst) * d.K + k) * 20;
+    const int C5 = d.asym ? 25 : 20;                       // classes x 5 values per phase
+    double* ok = out + (static_cast<size_t>(inst) * d.K + k) * C5;
+    if (lane == 4 && d.asym) {                             // alpha = exp(zeta): log-normal (R30)
+        const float* ma = d.var_a + static_cast<size_t>(inst) * 2 * d.K;
+        const double m = static_cast<double>(ma[k]), s = exp(static_cast<double>(ma[d.K + k]));
+        const double mean = exp(m + 0.5 * s * s);
+        double* o = ok + 20;
+        o[0] = mean; o[1] = sqrt(expm1(s * s)) * mean;
+        o[2] = exp(m - s * z975); o[3] = exp(m); o[4] = exp(m + s * z975);
+    }
     if (lane < 3) {
         const double m = static_cast<double>(mp[lane]);
         const double s = exp(static_cast<double>(mp[4 * d.K + lane]));
@@ -1334,12 +1680,25 @@ __global__ void __launch_bounds__(128) init_state_kernel(const Dev d, const floa
         o[0] = m.x; o[1] = m.y; o[2] = m.z; o[3] = m.w;
         float* ol = o + 4 * d.K;
         ol[0] = ol[1] = ol[2] = ol[3] = init_log_sigma;
+        if (d.asym) {   // R30: alpha starts at 1; restart jitter 0.05 eps from a second Philox call (bit 31 of the phase word)
+            float m_a = 0.0f;
+            if (rst > 0)
+                m_a = 0.05f * normal_alpha(0xFFFFFFFFu, static_cast<unsigned>(rst), static_cast<unsigned>(k),
+                                           static_cast<unsigned>(pat), seed);
+            d.var_a[static_cast<size_t>(inst) * 2 * d.K + k] = m_a;
+            d.var_a[static_cast<size_t>(inst) * 2 * d.K + d.K + k] = init_log_sigma;
+        }
     }
     const int per = 8 * d.K;
     for (int j = threadIdx.x; j < per; j += 128) {
         d.mom1[static_cast<size_t>(inst) * per + j] = 0.0f;
         d.mom2[static_cast<size_t>(inst) * per + j] = 0.0f;
     }
+    if (d.asym)
+        for (int j = threadIdx.x; j < 2 * d.K; j += 128) {
+            d.mom1_a[static_cast<size_t>(inst) * 2 * d.K + j] = 0.0f;
+            d.mom2_a[static_cast<size_t>(inst) * 2 * d.K + j] = 0.0f;
+        }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -1349,7 +1708,8 @@ __global__ void __launch_bounds__(128) init_state_kernel(const Dev d, const floa
 
 // a-2 for supplied points.  grid (ceil(K/4), groups of this launch), block 128.  Point of lane:
 // s = (s_group0 + blockIdx.y) * 32 + lane.
-__global__ void __launch_bounds__(128) zeta_latent_kernel(const Dev d, const float4* __restrict__ zeta, int n, int s_group0) {
+__global__ void __launch_bounds__(128) zeta_latent_kernel(const Dev d, const float4* __restrict__ zeta,
+                                                          const float* __restrict__ zeta_a, int n, int s_group0) {
     const int lane = threadIdx.x & 31;
     const int k = blockIdx.x * 4 + (threadIdx.x >> 5);
     if (k >= d.K) return;
@@ -1357,22 +1717,27 @@ __global__ void __launch_bounds__(128) zeta_latent_kernel(const Dev d, const flo
     const bool valid = s < n;
     const float4 z = valid ? zeta[static_cast<size_t>(s) * d.K + k] : make_float4(0.f, 0.f, 0.f, 0.f);
     const float4 zero = make_float4(0.f, 0.f, 0.f, 0.f);
-    emit_latent(d, d.g_base + blockIdx.y, k, valid, transform(z, zero, zero), zero);
+    const float alpha = (d.asym && valid) ? expf(zeta_a[static_cast<size_t>(s) * d.K + k]) : 1.0f;
+    emit_latent(d, d.g_base + blockIdx.y, k, valid, transform(z, zero, zero), zero, alpha, 0.0f);
 }
 
 // Sum of the per-run gradients of phase k over the tiles (fixed order) + prior and Jacobian part (a-6).
 // grid (K, groups of this launch), block 32 (lane = point).  Also the phase's log prior + log Jacobian -> lpk.
-__global__ void __launch_bounds__(32) logjoint_grad_kernel(const Dev d, const float4* __restrict__ zeta, int n, int s_group0,
-                                                           int pat, float4* __restrict__ grad, float* __restrict__ lpk) {
+__global__ void __launch_bounds__(32) logjoint_grad_kernel(const Dev d, const float4* __restrict__ zeta,
+                                                           const float* __restrict__ zeta_a, int n, int s_group0, int pat,
+                                                           float4* __restrict__ grad, float* __restrict__ grad_a,
+                                                           float* __restrict__ lpk) {
     const int lane = threadIdx.x, k = blockIdx.x, gi = blockIdx.y;
     const int s = (s_group0 + gi) * 32 + lane;
     if (s >= n) return;
     const PatConst pc = d.pat[pat];
-    double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+    const int row = d.model ? 160 : 128;                   // floats per (run, 32 points): 4 or 5 classes
+    double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0, a4 = 0.0;
     for (int j = d.slot_ofs[k]; j < d.slot_ofs[k + 1]; ++j) {
-        const float* __restrict__ o = d.pd + (static_cast<size_t>(gi) * d.n_slots + j) * 128 + lane;
+        const float* __restrict__ o = d.pd + (static_cast<size_t>(gi) * d.n_slots + j) * row + lane;
         a0 += static_cast<double>(o[0]); a1 += static_cast<double>(o[32]);
         a2 += static_cast<double>(o[64]); a3 += static_cast<double>(o[96]);
+        if (d.asym) a4 += static_cast<double>(o[128]);
     }
     const float4 zero = make_float4(0.f, 0.f, 0.f, 0.f);
     const Phys q = transform(zeta[static_cast<size_t>(s) * d.K + k], zero, zero);
@@ -1382,9 +1747,15 @@ __global__ void __launch_bounds__(32) logjoint_grad_kernel(const Dev d, const fl
                     static_cast<float>(a2 + static_cast<double>(d.w_shape - d.w_rate * q.w)),
                     static_cast<float>(a3 + static_cast<double>(1.0f - 2.0f * q.r)));
     const float az = fabsf(q.zr);
-    lpk[(static_cast<size_t>(gi) * d.K + k) * 32 + lane] =
-        (pc.log_lambda_h - pc.lambda_h * q.h + q.zh) + (-0.5f * q.mu * q.mu * d.mu_inv_var + d.mu_logc) +
-        (d.w_logc + d.w_shape * q.zw - d.w_rate * q.w) - (az + 2.0f * log1pf(expf(-az)));
+    float lp = (pc.log_lambda_h - pc.lambda_h * q.h + q.zh) + (-0.5f * q.mu * q.mu * d.mu_inv_var + d.mu_logc) +
+               (d.w_logc + d.w_shape * q.zw - d.w_rate * q.w) - (az + 2.0f * log1pf(expf(-az)));
+    if (d.asym) {
+        const float za = zeta_a[static_cast<size_t>(s) * d.K + k], al = expf(za), da = al - d.alpha_mu;
+        grad_a[static_cast<size_t>(s) * d.K + k] =
+            static_cast<float>(a4 + static_cast<double>(1.0f - da * d.alpha_inv_var * al));
+        lp += -0.5f * da * da * d.alpha_inv_var + d.alpha_logc + za;
+    }
+    lpk[(static_cast<size_t>(gi) * d.K + k) * 32 + lane] = lp;
 }
 
 // ll and log prior + log Jacobian per point.  grid (groups of this launch), block 32.
