@@ -14,11 +14,12 @@ extern "C" {
 #endif
 
 /* Debug read-back of the forward pass for parity tests: runs draw + forward at (var_params or
- * internal state, S, seed, iteration) and returns, for the first n sample-instances in
+ * internal state, S, seed, iteration) and returns, for the n sample-instances first .. first + n - 1 in
  * (pat, rst, s) order, the profile f float [n][N] (including B) and ll double [n]; f or ll may be NULL.
  * scratch: DEVICE buffer of at least n * N floats when f is wanted (XRDVI_E_WORKSPACE_TOO_SMALL otherwise). */
 int xrdvi_debug_profile(xrdvi* h, const float* var_params, int32_t S, uint64_t seed,
-                        uint64_t iteration, int64_t n, float* f, double* ll, void* scratch, size_t scratch_bytes);
+                        uint64_t iteration, int64_t first, int64_t n, float* f, double* ll, void* scratch,
+                        size_t scratch_bytes);
 
 /* Debug read-back of the draw kernel (a-1, a-2) at the internal state: eps float [n][K][4] for the first n
  * sample-instances; raw_words uint32 [n][K][4] (the Philox output) or NULL; core_halfwidth int32 [n][K]

@@ -88,7 +88,8 @@ def load_library():
     L.xrdvi_inclusion.argtypes = [vp, dp, dp]
     L.xrdvi_posterior_summary.argtypes = [vp, dp]
     L.xrdvi_logjoint_grad.argtypes = [vp, fp, C.c_int64, C.c_int32, dp, dp, fp]
-    L.xrdvi_debug_profile.argtypes = [vp, fp, C.c_int32, C.c_uint64, C.c_uint64, C.c_int64, fp, dp, vp, C.c_size_t]
+    L.xrdvi_debug_profile.argtypes = [vp, fp, C.c_int32, C.c_uint64, C.c_uint64, C.c_int64, C.c_int64, fp, dp, vp,
+                                      C.c_size_t]
     L.xrdvi_debug_draws.argtypes = [vp, C.c_int32, C.c_uint64, C.c_uint64, C.c_int64, fp, C.POINTER(C.c_uint32),
                                     C.POINTER(C.c_int32), vp, C.c_size_t]
     L.xrdvi_time_kernels.argtypes = [vp, C.c_int32, C.c_uint64, C.c_int32, fp]
@@ -307,14 +308,14 @@ class Xrdvi:
         t = torch.empty(int(nbytes), dtype=torch.uint8, device=self.device)
         return t, C.c_void_p(t.data_ptr()), int(nbytes)
 
-    def debug_profile(self, n, state=None, S=None, seed=0, iteration=0, want_f=True):
+    def debug_profile(self, n, state=None, S=None, seed=0, iteration=0, want_f=True, first=0):
         S = self.S_max if S is None else int(S)
         st = None if state is None else np.ascontiguousarray(state, dtype=np.float32).reshape(self._state_shape())
         f = np.empty((int(n), self.N), dtype=np.float32) if want_f else None
         ll = np.empty(int(n), dtype=np.float64)
         scratch, ptr, nb = self._scratch(4 * int(n) * self.N if want_f else 0)
-        _check(load_library().xrdvi_debug_profile(self._h, _f(st), S, int(seed), int(iteration), int(n), _f(f), _d(ll),
-                                                  ptr, nb))
+        _check(load_library().xrdvi_debug_profile(self._h, _f(st), S, int(seed), int(iteration), int(first), int(n),
+                                                  _f(f), _d(ll), ptr, nb))
         return f, ll
 
     def debug_draws(self, n, S=None, seed=0, iteration=0, want_core=False):

@@ -823,6 +823,7 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
     d.part8 = reinterpret_cast<float*>(w + pl.o_part8);
     d.pd = nullptr;
     d.g_base = 0;
+    d.dbg_first = 0;
     d.partial = reinterpret_cast<float*>(w + pl.o_partial);
     d.tile_cnt = reinterpret_cast<unsigned int*>(w + pl.o_tcnt);
     d.tile_cnt2 = d.tile_cnt + static_cast<size_t>(pl.G_max) * pl.n_tile;
@@ -1136,19 +1137,21 @@ int xrdvi_posterior_summary(xrdvi* h, double* summary) {
 }
 
 int xrdvi_debug_profile(xrdvi* h, const float* var_params, int32_t S, uint64_t seed, uint64_t iteration,
-                        int64_t n, float* f, double* ll, void* scratch, size_t scratch_bytes) {
+                        int64_t first, int64_t n, float* f, double* ll, void* scratch, size_t scratch_bytes) {
     const float* var = nullptr;
     int rc = begin_eval(h, var_params, S, seed, iteration, &var);
     if (rc) return rc;
     const long long T = static_cast<long long>(h->plan.PR) * S;
-    if (n < 0 || n > T) return fail(XRDVI_E_INVALID_ARG, "n out of range");
+    if (first < 0 || n < 0 || first + n > T) return fail(XRDVI_E_INVALID_ARG, "first / n out of range");
     float* f_dev = nullptr;
     if (f && n > 0) {
         if (!scratch || scratch_bytes < sizeof(float) * static_cast<size_t>(n) * h->N)
             return fail(XRDVI_E_WORKSPACE_TOO_SMALL, "debug_profile: scratch smaller than n * N floats");
         f_dev = static_cast<float*>(scratch);
     }
+    h->dev.dbg_first = first;
     rc = enqueue_eval(h, var, f_dev, n, true);
+    h->dev.dbg_first = 0;
     if (rc) return rc;
     std::vector<double> llh(static_cast<size_t>(h->plan.PR) * h->plan.S_pad);
     cudaError_t e = cudaMemcpyAsync(llh.data(), h->dev.ll_t, sizeof(double) * llh.size(), cudaMemcpyDeviceToHost, h->stream);
@@ -1157,7 +1160,7 @@ int xrdvi_debug_profile(xrdvi* h, const float* var_params, int32_t S, uint64_t s
     if (e != cudaSuccess) return fail(XRDVI_E_CUDA, std::string("debug_profile: ") + cudaGetErrorString(e));
     if (ll) {
         const int gpi32 = h->dev.gpi * 32;
-        for (long long t = 0; t < n; ++t) ll[t] = llh[static_cast<size_t>(t / S) * gpi32 + (t % S)];
+        for (long long t = 0; t < n; ++t) ll[t] = llh[static_cast<size_t>((first + t) / S) * gpi32 + ((first + t) % S)];
     }
     return XRDVI_OK;
 }

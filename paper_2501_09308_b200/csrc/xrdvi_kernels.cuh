@@ -128,6 +128,7 @@ struct Dev {
     unsigned int* tile_cnt2;  // [G][n_tile] phase-2 items that are done
     float* pd;                // nullptr, or [groups of the launch][n_slots][4][32] d ll / d zeta per (run, class, draw)
     int g_base;               // group of blockIdx.x = 0 in elbo_tile_kernel (0 except in the service)
+    long long dbg_first;      // first sample-instance of the debug profile read-back (xrdvi_debug_profile)
     const int2* tile_rng;     // [n_tile + 1] (first run, first record) of every tile's lists
     int stage;                // 1: elbo_tile_kernel copies the tile's lists into shared memory (they fit: host check)
     // peak asymmetry and the sec width term (reading R30; hyper.asymmetry / hyper.width_sec).  asym = 1: a fifth latent
@@ -796,8 +797,8 @@ __device__ __forceinline__ void tile_debug_profile(const Dev& d, const TileCtx& 
                                                    float* __restrict__ f_dbg, long long n_dbg) {
     const int inst = c.g / d.gpi;
     const int s = (c.g - inst * d.gpi) * 32 + (threadIdx.x & 31);
-    const long long t = static_cast<long long>(inst) * d.S + s;
-    if (s < d.S && t < n_dbg) {
+    const long long t = static_cast<long long>(inst) * d.S + s - d.dbg_first;   // row of the read-back buffer
+    if (s < d.S && t >= 0 && t < n_dbg) {
         const float* __restrict__ bg = d.bg + static_cast<size_t>(c.pat) * d.N;
 #pragma unroll
         for (int p = 0; p < kPT; ++p)

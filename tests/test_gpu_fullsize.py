@@ -30,14 +30,30 @@ def class_err(g_gpu, g_ref):
     return float((err / ref).max())
 
 
-def ll_one_draw(o, state64, seed, iteration, inst, s):
-    """log-likelihood of ONE draw computed piece by piece with the oracle (eps -> zeta -> profile -> ll)."""
+def profile_one_draw(o, state64, seed, iteration, inst, s):
+    """profile of ONE draw computed piece by piece with the oracle (eps -> zeta -> profile)."""
     pat = inst // o.R
     st = state64.reshape(o.P * o.R, 2, o.K, 4)[inst]
     zeta = np.empty((o.K, 4))
     for k in range(o.K):
         zeta[k] = st[0, k] + np.exp(st[1, k]) * orc.eps(seed, iteration, inst, s, k)
-    return o.loglik(o.profile(zeta, pat), pat)
+    return o.profile(zeta, pat), pat
+
+
+def ll_one_draw(o, state64, seed, iteration, inst, s):
+    """log-likelihood of ONE draw computed piece by piece with the oracle (eps -> zeta -> profile -> ll)."""
+    f, pat = profile_one_draw(o, state64, seed, iteration, inst, s)
+    return o.loglik(f, pat)
+
+
+def check_profiles(gpu, o, st, S, seed, iteration, picks):
+    """element-wise profile of sampled draws (instance, s) at full size: first / last group of the launch, so that both
+    ends of the grid of CTAs (and, at config 4, of the ticket queue) are hit"""
+    st64 = st.astype(np.float64)
+    for inst, s in picks:
+        f_g, _ = gpu.debug_profile(1, state=st, S=S, seed=seed, iteration=iteration, first=inst * S + s)
+        f_r, _ = profile_one_draw(o, st64, seed, iteration, inst, s)
+        assert np.abs(f_g[0] - f_r).max() / np.abs(f_r).max() <= TOL_PROFILE, (inst, s)
 
 
 def test_config1_full_size_three_states():
@@ -83,6 +99,7 @@ def test_config2_full_size_sampled_restarts():
         np.testing.assert_allclose(ll_g[rst], ll_r[0], rtol=TOL_ELBO)
         np.testing.assert_allclose(elbo_g[0, rst], e_r[0], rtol=TOL_ELBO)
         assert class_err(grad_g[0, rst], g_r[0]) <= TOL_GRAD
+    check_profiles(gpu, o, st, wl.S, 2, 9, [(0, 0), (0, 31), (wl.R - 1, wl.S - 32), (wl.R - 1, wl.S - 1)])
     rng = np.random.default_rng(0)
     for _ in range(12):                                          # other restarts: sampled draws one by one
         rst, s = int(rng.integers(1, wl.R - 1)), int(rng.integers(0, wl.S))
@@ -106,6 +123,7 @@ def test_config3_full_size_sampled_patterns():
         np.testing.assert_allclose(ll_g[pat], ll_r[0], rtol=TOL_ELBO)
         np.testing.assert_allclose(elbo_g[pat, 0], e_r[0], rtol=TOL_ELBO)
         assert class_err(grad_g[pat, 0], g_r[0]) <= TOL_GRAD
+    check_profiles(gpu, o, st, wl.S, 4, 7, [(0, 0), (0, 31), (wl.P - 1, wl.S - 32), (wl.P - 1, wl.S - 1)])
     rng = np.random.default_rng(1)
     for _ in range(12):
         pat, s = int(rng.integers(0, wl.P)), int(rng.integers(0, wl.S))
@@ -125,6 +143,7 @@ def test_config4_full_size():
     assert np.isfinite(ll_g).all()
     for s in (0, 31, 32, 100, 255):
         assert ll_g[s] == pytest.approx(ll_one_draw(o, st64, 6, 5, 0, s), rel=TOL_ELBO)
+    check_profiles(gpu, o, st, wl.S, 6, 5, [(0, 0), (0, 31), (0, wl.S - 32), (0, wl.S - 1)])
     # whole evaluation: 3.6e10 pair evaluations in the fp64 oracle (about a minute on 16 host cores)
     elbo_g, grad_g = gpu.elbo_grad(state=st, S=wl.S, seed=6, iteration=5)
     e_r, g_r, ll_r = o.elbo_grad_range(st64, wl.S, 6, 5, 0, 1, want_ll=True)
@@ -133,11 +152,11 @@ def test_config4_full_size():
     assert class_err(grad_g[0, 0], g_r[0]) <= TOL_GRAD
 
 
-def _fit_parity(iterations):
-    """Fit config 1 at full size (K=50, S=256) on both sides with the same draws; compare what is unique (R22):
-    inclusion probabilities (north_star: 0.02 absolute), area ratios and the identified parameters of the planted
+def _fit_parity(iterations, S=None):
+    """Fit config 1 at full size (K=50, S=256 unless given) on both sides with the same draws; compare what is unique
+    (R22): inclusion probabilities (north_star: 0.02 absolute), area ratios and the identified parameters of the planted
     phases."""
-    wl = synth.make_workload(1)
+    wl = synth.make_workload(1) if S is None else synth.make_workload(1, S=S)
     o = orc.from_workload(wl)
     gpu = Xrdvi.from_workload(wl)
     st_g, inc_g, tr_g = gpu.fit(iterations, seed=1, want_trace=True)
@@ -163,6 +182,16 @@ def _fit_parity(iterations):
 
 def test_config1_full_size_fit_inclusion_parity_200_iterations():
     _fit_parity(200)
+
+
+def test_config1_whole_2000_iteration_fit_inclusion_parity_at_32_draws():
+    """The metric's own workload end to end -- the 2000-iteration K=50 (2^50 combination) fit -- against the oracle in
+    the default GPU suite: both sides with S = 32 draws per step (a minute of fp64 oracle instead of eight at S = 256,
+    which stays opt-in below)."""
+    d_inc, inc_g, inc_r, wl = _fit_parity(2000, S=32)
+    truth = wl.true_phases[0]
+    assert np.all(inc_g[0, 0, truth] > 0.99) and np.all(inc_r[0, 0, truth] > 0.99)
+    assert np.delete(inc_g[0, 0], truth).max() < 0.5              # no absent phase is read as present (R29: converged)
 
 
 @pytest.mark.skipif(not __import__("os").environ.get("XRDVI_LONG"), reason="8 min of fp64 oracle: set XRDVI_LONG=1")
