@@ -829,6 +829,13 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
     d.tile_cnt2 = d.tile_cnt + static_cast<size_t>(pl.G_max) * pl.n_tile;
     d.tile_rng = reinterpret_cast<int2*>(w + pl.o_trng);
     d.stage = 0;
+    {   // dispatch chunk: as many draw groups as keep their latent records (K x 32 x 36 B each, + alpha) within 16 MB of L2
+        const long long per_group = static_cast<long long>(K) * 32 * 44;
+        d.g_block = static_cast<int>(std::min<long long>(std::max<long long>((16ll << 20) / per_group, 8), 65535));
+#ifdef XRDVI_TUNING
+        if (const char* e = std::getenv("XRDVI_G_BLOCK")) d.g_block = std::max(1, std::atoi(e));   // A/B knob
+#endif
+    }
     d.asym = hyp->asymmetry;
     d.sec = hyp->width_sec;
     d.model = (hyp->asymmetry || hyp->width_sec) ? 1 : 0;

@@ -131,6 +131,7 @@ struct Dev {
     long long dbg_first;      // first sample-instance of the debug profile read-back (xrdvi_debug_profile)
     const int2* tile_rng;     // [n_tile + 1] (first run, first record) of every tile's lists
     int stage;                // 1: elbo_tile_kernel copies the tile's lists into shared memory (they fit: host check)
+    int g_block;              // draw groups per dispatch chunk of elbo_tile_kernel (their latent records stay in L2)
     // peak asymmetry and the sec width term (reading R30; hyper.asymmetry / hyper.width_sec).  asym = 1: a fifth latent
     // alpha_k per phase; every state array has a companion for it ([PR][2][K]: m_alpha, l_alpha)
     int asym, sec;
@@ -1156,9 +1157,18 @@ elbo_tile_kernel(const Dev d, float* __restrict__ f_dbg, long long n_dbg) {
     griddep_launch_dependents();
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const int tw = w % TW, ps = w / TW;
-    // grid (G, n_seg): CTAs are dispatched blockIdx.x fastest, i.e. TILE-major: all draw groups of the heaviest tile
-    // first, the lightest tiles last (config 1: -1.6 % against group-major, configs 2/3: -0.4 %)
-    const int seg = d.seg_order[blockIdx.y];                // static tables: may be read before the predecessor is done
+    // grid (G, n_seg), dispatched blockIdx.x fastest.  The dispatch order is cut into chunks of g_block draw groups; inside a
+    // chunk the CTAs run TILE-major (all groups of the chunk on the heaviest tile first, the lightest tiles last), so the
+    // latent records of a chunk (g_block x K x 1.2 KB, sized to stay in L2) are read from DRAM once, not once per tile:
+    // with every group in one chunk, config 2 streamed all 241 MB of latents through DRAM for each of its 251 tiles
+    // (79 GB per launch, ncu; profiles/r2_*).  Config 1 (8 groups) is one chunk.
+    const unsigned lin = blockIdx.y * gridDim.x + blockIdx.x;
+    const unsigned per_chunk = static_cast<unsigned>(d.g_block) * gridDim.y;
+    const unsigned chunk = lin / per_chunk, rem = lin - chunk * per_chunk;
+    const unsigned gb = (chunk + 1) * d.g_block <= gridDim.x ? d.g_block : gridDim.x - chunk * d.g_block;
+    const unsigned seg_pos = rem / gb;
+    const int group = static_cast<int>(chunk * d.g_block + (rem - seg_pos * gb));
+    const int seg = d.seg_order[seg_pos];                   // static tables: may be read before the predecessor is done
     const int tile = seg * TW + tw;
     const bool live = tile < d.n_tile;                      // the last segment may have fewer than TW tiles
     typename TileSrc<STAGE>::type src;
@@ -1178,7 +1188,7 @@ elbo_tile_kernel(const Dev d, float* __restrict__ f_dbg, long long n_dbg) {
     } else {
         src = SrcGlobal{d.pk_tile, d.run_tab};
     }
-    const TileCtx c = tile_ctx(d, d.g_base + blockIdx.x, tile);
+    const TileCtx c = tile_ctx(d, d.g_base + group, tile);
     int2 rng = make_int2(0, 0);
     if (live) rng = d.share_rng[tile * PS + ps];
     if constexpr (STAGE) {
@@ -1187,7 +1197,7 @@ elbo_tile_kernel(const Dev d, float* __restrict__ f_dbg, long long n_dbg) {
     }
     griddep_wait();                                         // latents, control block: written by the predecessor
     if (blockIdx.x == gridDim.x - 1 && blockIdx.y == gridDim.y - 1) finish_step(d);   // previous step's ELBO / count
-    const unsigned tl_row = (blockIdx.y * gridDim.x + blockIdx.x) * (TW * PS) + w;
+    const unsigned tl_row = lin * (TW * PS) + w;
     tl_stamp(d.tl, tl_row, 0);
     if (d.tl) tl_tag(d.tl, tl_row, rng.x < rng.y ? d.run_tab[rng.y - 1].y - d.run_tab[rng.x].x : 0);
 
@@ -1237,8 +1247,8 @@ elbo_tile_kernel(const Dev d, float* __restrict__ f_dbg, long long n_dbg) {
         const float4 t = e_s[tw][v][lane];
         e[4 * v] = t.x; e[4 * v + 1] = t.y; e[4 * v + 2] = t.z; e[4 * v + 3] = t.w;
     }
-    if constexpr (MODEL == 1) tile_phase2_asym(d, src, c, rng, e, blockIdx.x);
-    else tile_phase2(d, src, c, rng, e, blockIdx.x);
+    if constexpr (MODEL == 1) tile_phase2_asym(d, src, c, rng, e, group);
+    else tile_phase2(d, src, c, rng, e, group);
     tl_stamp(d.tl, tl_row, 2);
 }
 
@@ -1424,27 +1434,13 @@ __global__ void __launch_bounds__(kUpdThreads) update_draw_kernel(const Dev d, c
         const int s0 = d.slot_ofs[k], s1 = d.slot_ofs[k + 1];
         const int n_sl = s1 - s0;
         const int n_part = n_sl * d.gpi;
-        for (int idx0 = threadIdx.x; idx0 < n_part; idx0 += 4 * kUpdThreads) {   // four slots in flight per thread,
-            float4 a[4], b[4];                                                    // added in increasing slot order
-#pragma unroll
-            for (int u = 0; u < 4; ++u) {
-                const int idx = idx0 + u * kUpdThreads;
-                a[u] = b[u] = make_float4(0.f, 0.f, 0.f, 0.f);
-                if (idx < n_part) {
-                    const int gi = idx / n_sl, sl = s0 + (idx - gi * n_sl);
-                    const float4* __restrict__ pp = reinterpret_cast<const float4*>(
-                        d.part8 + (static_cast<size_t>(inst * d.gpi + gi) * d.n_slots + sl) * 8);
-                    a[u] = pp[0];
-                    b[u] = pp[1];
-                }
-            }
-#pragma unroll
-            for (int u = 0; u < 4; ++u) {
-                if (idx0 + u * kUpdThreads < n_part) {
-                    v[0] += a[u].x; v[1] += a[u].y; v[2] += a[u].z; v[3] += a[u].w;
-                    v[4] += b[u].x; v[5] += b[u].y; v[6] += b[u].z; v[7] += b[u].w;
-                }
-            }
+        for (int idx = threadIdx.x; idx < n_part; idx += kUpdThreads) {
+            const int gi = idx / n_sl, sl = s0 + (idx - gi * n_sl);
+            const float4* __restrict__ pp = reinterpret_cast<const float4*>(
+                d.part8 + (static_cast<size_t>(inst * d.gpi + gi) * d.n_slots + sl) * 8);
+            const float4 a = pp[0], b = pp[1];
+            v[0] += a.x; v[1] += a.y; v[2] += a.z; v[3] += a.w;
+            v[4] += b.x; v[5] += b.y; v[6] += b.z; v[7] += b.w;
         }
         if (d.asym) {
             for (int idx = threadIdx.x; idx < n_part; idx += kUpdThreads) {
