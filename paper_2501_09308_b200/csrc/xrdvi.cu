@@ -38,7 +38,7 @@ size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
 
 struct Plan {   // workspace carve; identical arithmetic in workspace_bytes and create
     int P, R, PR, S_pad, gpi_max, G_max, K;
-    int TW, PS, NW, SP, n_seg, n_tile;
+    int TW, PS, split, NW, SP, n_seg, n_tile;
     long long M, n_c, tile_cap, slots_cap;
     size_t total;
     size_t o_yb, o_bg, o_pkt, o_runs, o_srng, o_sord, o_sofs, o_pat, o_area, o_mh0;
@@ -102,7 +102,11 @@ bool make_plan(int64_t N, int32_t K, int64_t M, int32_t S_max, double step, cons
     // entries of the per-tile phase-major lists: a peak appears once per 16-point tile its window touches
     const long long per_peak = p.n_c < 0 ? p.n_tile : std::min<long long>(p.n_tile, (2 * p.n_c + kPT) / kPT + 1);
     p.tile_cap = M * per_peak;
-    p.slots_cap = std::min<long long>(static_cast<long long>(p.n_tile) * K, p.tile_cap);   // one slot per (tile, phase)
+    // long work items (an upper bound of the records of one of PS shares of a tile >= 512; config 4): one-warp items on a
+    // ticket queue (elbo_split_kernel) instead of PS-warp CTAs
+    p.split = (p.PS > 1 && p.TW == 1 && p.tile_cap / (static_cast<long long>(p.n_tile) * p.PS) >= 512) ? 1 : 0;
+    // one output slot per (tile, phase present in the tile), plus one per run a share boundary cuts
+    p.slots_cap = std::min<long long>(static_cast<long long>(p.n_tile) * K, p.tile_cap) + static_cast<long long>(p.n_tile) * (p.PS - 1);
     if (p.tile_cap > (1ll << 31) - 1 || p.slots_cap > (1ll << 31) - 1) return false;
     size_t o = 0;
     auto take = [&](size_t bytes) { size_t r = o; o = align_up(o + bytes); return r; };
@@ -145,7 +149,7 @@ bool make_plan(int64_t N, int32_t K, int64_t M, int32_t S_max, double step, cons
     p.o_gradz = take(sizeof(float) * 5 * static_cast<size_t>(p.S_pad) * K);
     p.o_lls = take(sizeof(double) * 2 * p.S_pad);
     // split kernel (PS > 1): partial profiles of every (group, tile, share) and two counters per (group, tile)
-    p.o_partial = take(p.PS > 1 ? sizeof(float) * kPT * 32 * static_cast<size_t>(p.G_max) * p.n_tile * p.PS : 0);
+    p.o_partial = take(p.split ? sizeof(float) * kPT * 32 * static_cast<size_t>(p.G_max) * p.n_tile * p.PS : 0);
     p.o_tcnt = take(sizeof(unsigned int) * 2 * static_cast<size_t>(p.G_max) * p.n_tile);
     p.o_trng = take(sizeof(int2) * (static_cast<size_t>(p.n_tile) + 1));
     const bool model = hyp->asymmetry || hyp->width_sec;    // R30 buffers only when the extension is on
@@ -218,7 +222,8 @@ const char* build_tables(const Plan& pl, int64_t N, int K, const std::vector<Hos
     T->pk_tile.assign(static_cast<size_t>(n_ent) + 1, PeakRec{0, 0.f, 0.f, 0});   // +1: the kernel prefetches one
     T->run_tab.assign(static_cast<size_t>(n_runs) + 1, make_int4(0, 0, 0, 0));    // record / header past the end
     T->share_rng.assign(static_cast<size_t>(n_tile) * PSn, make_int2(0, 0));
-    std::vector<long long> run_w(n_runs, 0), seg_work(pl.n_seg, 0);
+    std::vector<long long> seg_work(pl.n_seg, 0);
+    std::vector<int> rec_w(static_cast<size_t>(n_ent), 0);   // in-window points of every record (share balance)
     std::vector<long long> ent_cur(ent_base.begin(), ent_base.end() - 1);
     std::vector<int> run_cur(run_base.begin(), run_base.end() - 1);
     std::fill(last_k.begin(), last_k.end(), -1);
@@ -242,29 +247,62 @@ const char* build_tables(const Plan& pl, int64_t N, int K, const std::vector<Hos
             }
             const int r = run_cur[t] - 1;
             T->run_tab[r].y = static_cast<int>(e) + 1;
-            run_w[r] += wq;
+            rec_w[e] = static_cast<int>(wq);
             seg_work[t / TWn] += wq;
             pairs_check += wq;
         }
     }
-    // pass 3: PS contiguous shares per tile, split at phase boundaries, balanced by clipped pair count
-    std::vector<int> slot_phase(n_runs);
-    for (int r = 0; r < n_runs; ++r) slot_phase[r] = T->run_tab[r].z;
-    for (int t = 0; t < n_tile; ++t) {
-        long long tot = 0;
-        for (int r = run_base[t]; r < run_base[t + 1]; ++r) tot += run_w[r];
-        int run = run_base[t];
-        long long cum = 0;
-        for (int w = 0; w < PSn; ++w) {
-            const int run0 = run;
-            const long long goal = tot * (w + 1) / PSn;
-            if (w == PSn - 1) run = run_base[t + 1];
-            else while (run < run_base[t + 1] && cum + run_w[run] <= goal) { cum += run_w[run]; ++run; }
-            T->share_rng[static_cast<size_t>(t) * PSn + w] = make_int2(run0, run);
+    // pass 3: PS contiguous shares per tile, balanced by in-window pair count at RECORD granularity: a share boundary
+    // that falls inside a phase run cuts the run in two (two headers, two output slots of the same phase: the reduction
+    // over the slots of a phase does not care), so that the shares of a tile -- which meet at a barrier -- carry equal
+    // work whatever the sizes of the phases.  Rebuilds run_tab / run_base with the cut runs.
+    {
+        std::vector<int4> runs2;
+        runs2.reserve(static_cast<size_t>(n_runs) + static_cast<size_t>(n_tile) * PSn);
+        std::vector<int> run_base2(n_tile + 1, 0);
+        for (int t = 0; t < n_tile; ++t) {
+            run_base2[t] = static_cast<int>(runs2.size());
+            const long long e0 = ent_base[t], e1 = ent_base[t + 1];
+            long long tot = 0;
+            for (long long e = e0; e < e1; ++e) tot += rec_w[e];
+            std::vector<long long> cuts(PSn + 1, e1);        // share w = records [cuts[w], cuts[w + 1])
+            cuts[0] = e0;
+            {
+                long long cum = 0, e = e0;
+                for (int w = 1; w < PSn; ++w) {
+                    const long long goal = tot * w / PSn;
+                    while (e < e1 && cum + rec_w[e] <= goal) { cum += rec_w[e]; ++e; }
+                    cuts[w] = e;
+                }
+            }
+            int w = 0;
+            std::vector<int> share_first(PSn + 1, 0);
+            for (int r = run_base[t]; r < run_base[t + 1]; ++r) {
+                long long m0 = T->run_tab[r].x;
+                const long long m1 = T->run_tab[r].y;
+                while (m0 < m1) {
+                    while (w < PSn && cuts[w + 1] <= m0) { ++w; share_first[w] = static_cast<int>(runs2.size()); }
+                    const long long stop = std::min(m1, w < PSn ? cuts[w + 1] : m1);
+                    runs2.push_back(make_int4(static_cast<int>(m0), static_cast<int>(stop), T->run_tab[r].z, 0));
+                    m0 = stop;
+                }
+            }
+            while (w < PSn) { ++w; share_first[w] = static_cast<int>(runs2.size()); }
+            for (int q = 0; q < PSn; ++q)
+                T->share_rng[static_cast<size_t>(t) * PSn + q] = make_int2(std::max(share_first[q], run_base2[t]), share_first[q + 1]);
+            T->share_rng[static_cast<size_t>(t) * PSn].x = run_base2[t];
         }
+        run_base2[n_tile] = static_cast<int>(runs2.size());
+        if (static_cast<long long>(runs2.size()) > pl.slots_cap) return "internal: table bound exceeded (cut runs)";
+        runs2.push_back(make_int4(0, 0, 0, 0));              // the header past the end
+        T->run_tab.swap(runs2);
+        run_base.swap(run_base2);
     }
+    const int n_runs2 = static_cast<int>(T->run_tab.size()) - 1;
+    std::vector<int> slot_phase(n_runs2);
+    for (int r = 0; r < n_runs2; ++r) slot_phase[r] = T->run_tab[r].z;
     if (pairs_check != pairs) return "internal: tile tables do not cover every pair once";
-    const int n_slots = n_runs;
+    const int n_slots = n_runs2;
     // output slots numbered phase-major (the reduction over the tiles of a phase reads one contiguous range);
     // within a phase in increasing tile order
     T->slot_ofs.assign(K + 1, 0);
@@ -350,7 +388,7 @@ int install_tables(xrdvi* h, const Tables& T, const std::vector<long long>& nck,
         CU(cudaMemcpyAsync(w + pl.o_pksec, T.pk_sec.data(), sizeof(float) * T.pk_sec.size(), cudaMemcpyHostToDevice, st));
     if (at_create) {
         d.n_slots = std::max(T.n_slots, 1);
-        d.split = T.pairs / (static_cast<long long>(pl.n_tile) * pl.PS * kPT) >= 512 ? 1 : 0;   // peaks per work item
+        d.split = pl.split;
         // bulk-copy staging (TW = 1) needs every tile list to fit the shared-memory buffers; decided once (the per-phase
         // windows of R27 only ever shrink the lists), because the Dev block is held by value in the captured graphs
         d.stage = (pl.TW == 1 && T.max_tile_rec <= kStageRec && T.max_tile_runs <= kStageRun - 1) ? 1 : 0;

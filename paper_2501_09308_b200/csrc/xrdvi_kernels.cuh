@@ -664,7 +664,7 @@ struct SrcShared {   // shared-window byte addresses of record 0 / run 0 (i.e. a
 
 // Bulk asynchronous copy global -> shared memory completed on an mbarrier (cp.async.bulk; SASS UBLKCP).
 constexpr int kStageRec = 224;   // records / run headers (incl. the one after the last run) a staged tile list may hold
-constexpr int kStageRun = 56;
+constexpr int kStageRun = 64;
 __device__ __forceinline__ unsigned smem_u32(const void* p) { return static_cast<unsigned>(__cvta_generic_to_shared(p)); }
 __device__ __forceinline__ void mbar_init(unsigned mbar, unsigned count) {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(mbar), "r"(count) : "memory");
