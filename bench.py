@@ -95,18 +95,17 @@ def measured_peaks() -> dict:
 CAPTURE_FILE = "profiles/r2_capture_counters.txt"
 
 
-def captured_counters(kernel: str, cfg: int):
-    """(DRAM bytes per launch, warp instructions per launch) of `kernel` at config `cfg` from the committed
-    `ncu --set full` capture of THIS build (profiles/r2_capture_counters.txt: kernel, config, dram bytes, warp
-    instructions; written from the capture named in its header), or (None, None) when no capture exists."""
+def captured_counters(cfg: int):
+    """(kernel, DRAM bytes per launch, warp instructions per launch) of the dominant kernel at config `cfg` from the
+    committed `ncu --set full` capture of THIS build (profiles/r2_capture_counters.txt: kernel, config, dram bytes, warp
+    instructions; written from the capture named in its header), or (DOM_KERNEL, None, None) when no capture exists."""
     p = ROOT / CAPTURE_FILE
-    if not p.exists():
-        return None, None
-    for ln in p.read_text().splitlines():
-        t = ln.split()
-        if len(t) == 4 and not ln.startswith("#") and t[0] == kernel and t[1] == str(cfg):
-            return int(t[2]), int(t[3])
-    return None, None
+    if p.exists():
+        for ln in p.read_text().splitlines():
+            t = ln.split()
+            if len(t) == 4 and not ln.startswith("#") and t[1] == str(cfg):
+                return t[0], int(t[2]), int(t[3])
+    return DOM_KERNEL, None, None
 
 
 def run_reference(args, rank: int) -> None:
@@ -224,6 +223,10 @@ def run_ours(args, rank: int, local_rank: int, world: int) -> None:
         t0 = time.perf_counter()
         gpu3.fit(wl.iterations, S=S, seed=seeds["draw_seed"])           # the same fit on the existing handle (no create)
         full["fit_wall_s_full_existing_handle"] = replicas.max_over_ranks(time.perf_counter() - t0, dist, "cuda")
+        # the steps of a fit are not equally expensive (the Gaussian-core extent follows the sampled widths and shifts:
+        # the first steps, which the --steps region times from a fresh state, are the slowest): mean over the whole fit
+        full["ms_per_step_whole_fit"] = 1e3 * full["fit_wall_s_full_existing_handle"] / wl.iterations
+        full["pair_evals_per_s_whole_fit"] = pairs * T * wl.iterations / full["fit_wall_s_full_existing_handle"]
         truth = set(wl.true_phases[0])
         full["planted_phases_recovered"] = bool(
             set(int(k) for k in np.nonzero(inc_full[0, 0] > 0.5)[0]) == truth)
@@ -264,9 +267,9 @@ def run_ours(args, rank: int, local_rank: int, world: int) -> None:
     dom_ms = tk["ms_tile"]
     achieved = pairs * T / (dom_ms * 1e-3)
     r_plain = n_sm * f_max * 16.0 / 4.0          # plain formulation: 4 MUFU per pair (2 per pass), 16 MUFU lanes/SM/clk
-    traffic, warp_instr = captured_counters(DOM_KERNEL, args.config)
+    dom_kernel, traffic, warp_instr = captured_counters(args.config)
     roofline = {
-        "bound": "alu", "kernel": DOM_KERNEL, "achieved": achieved / 1e9, "peak": r_plain / 1e9,
+        "bound": "alu", "kernel": dom_kernel, "achieved": achieved / 1e9, "peak": r_plain / 1e9,
         "unit": "Gpair/s", "frac": achieved / r_plain, "traffic": traffic,
         "traffic_source": (f"{CAPTURE_FILE} (ncu --set full capture of this build: dram read + write bytes per launch)"
                            if traffic is not None else f"null: no ncu capture of this build at config {args.config} "
