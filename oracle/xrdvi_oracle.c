@@ -159,6 +159,18 @@ static void *dup_mem(const void *src, size_t bytes) {
     return p;
 }
 
+/* R31: index of the grid point nearest to p on a strictly increasing grid (the lower one on a tie); positions beyond
+ * the grid are continued with the mean step, as the uniform formula does. */
+int64_t orc_nearest_index(const double *x, int64_t N, double p) {
+    double step = (x[N - 1] - x[0]) / (double)(N - 1);
+    if (p <= x[0]) return -(int64_t)floor((x[0] - p) / step + 0.5);
+    if (p >= x[N - 1]) return N - 1 + (int64_t)floor((p - x[N - 1]) / step + 0.5);
+    int64_t best = 0;
+    for (int64_t i = 1; i < N; ++i)                            /* plain scan: this is the oracle */
+        if (fabs(x[i] - p) < fabs(x[best] - p)) best = i;
+    return best;
+}
+
 orc_problem *orc_create(const double *x, int64_t N, const double *y, const double *B, int32_t K,
                         const int64_t *ofs, const double *pos, const double *inten,
                         const orc_hyper *hy) {
@@ -176,10 +188,16 @@ orc_problem *orc_create(const double *x, int64_t N, const double *y, const doubl
     q->pos = (double *)dup_mem(pos, sizeof(double) * q->M);
     q->inten = (double *)dup_mem(inten, sizeof(double) * q->M);
     q->jm = (int64_t *)malloc(sizeof(int64_t) * (q->M ? q->M : 1));
-    q->delta = (x[N - 1] - x[0]) / (double)(N - 1);
+    q->delta = (x[N - 1] - x[0]) / (double)(N - 1);            /* the (mean) grid step */
     /* R16: j_m = floor((p_m - x_0)/Delta + 1/2); n_c = ceil(W fwhm_ref / Delta - 1e-9)
-     * (the 1e-9 keeps an exact ratio such as 1.5/0.02 = 75 from rounding up to 76) */
-    for (int64_t m = 0; m < q->M; ++m) q->jm[m] = (int64_t)floor((pos[m] - x[0]) / q->delta + 0.5);
+     * (the 1e-9 keeps an exact ratio such as 1.5/0.02 = 75 from rounding up to 76).
+     * R31: on a grid that is not uniform (some x_i off x_0 + i Delta by more than 1e-6 Delta) j_m is the index of the
+     * grid point nearest to p_m and Delta the mean step; the window stays the integer rule |i - j_m| <= n_c. */
+    int uniform = 1;
+    for (int64_t i = 0; i < N; ++i)
+        if (fabs(x[i] - (x[0] + q->delta * (double)i)) > 1e-6 * q->delta) { uniform = 0; break; }
+    for (int64_t m = 0; m < q->M; ++m)
+        q->jm[m] = uniform ? (int64_t)floor((pos[m] - x[0]) / q->delta + 0.5) : orc_nearest_index(x, N, pos[m]);
     if (hy->window_W > 0.0) q->n_c = (int64_t)ceil(hy->window_W * hy->fwhm_ref / q->delta - 1e-9);
     else q->n_c = -1;
     q->sigma_n = (double *)malloc(sizeof(double) * q->P);

@@ -72,6 +72,8 @@ def lib():
         L.orc_pseudo_voigt_asym.argtypes = [C.c_double] * 5
         L.orc_eps_alpha.restype = C.c_double
         L.orc_eps_alpha.argtypes = [C.c_uint64, C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32]
+        L.orc_nearest_index.restype = C.c_int64
+        L.orc_nearest_index.argtypes = [dp, C.c_int64, C.c_double]
         L.orc_classes.restype = C.c_int32
         L.orc_classes.argtypes = [C.c_void_p]
         L.orc_profile.argtypes = [C.c_void_p, C.c_int32, dp, dp]
@@ -134,6 +136,11 @@ def pseudo_voigt_asym(x, rho, w, r, alpha):
 
 def eps_alpha(seed, iteration, inst, s, k):
     return float(lib().orc_eps_alpha(int(seed), int(iteration), int(inst), int(s), int(k)))
+
+
+def nearest_index(x, p):
+    x = np.ascontiguousarray(x, dtype=np.float64)
+    return int(lib().orc_nearest_index(_dp(x), int(x.shape[0]), float(p)))
 
 
 def num_threads():
