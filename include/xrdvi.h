@@ -46,7 +46,8 @@ enum {
     XRDVI_OK = 0,
     XRDVI_E_INVALID_ARG = -1,
     XRDVI_E_UNSORTED_GRID = -2,      /* 2theta not strictly increasing                      */
-    XRDVI_E_NONUNIFORM_GRID = -3,    /* 2theta not uniform to 1e-6 of the step (R16: see xrdvi_create) */
+    XRDVI_E_NONUNIFORM_GRID = -3,    /* 2theta not uniform to 1e-6 of the step and hyper.general_grid = 0, or its steps
+                                        differ by more than a factor 16 (R16, R31: see xrdvi_create)         */
     XRDVI_E_EMPTY_PHASE = -4,        /* a phase with M_k = 0                                 */
     XRDVI_E_WORKSPACE_TOO_SMALL = -5,
     XRDVI_E_CUDA = -6,
@@ -85,6 +86,13 @@ typedef struct {
     int32_t width_sec;     /* 1: angle-dependent width w_k sec(p_m / 2) per peak (the sec of; R30)      */
     double alpha_mu;       /* 1.00 (B.2)                                                          */
     double alpha_sigma;    /* 0.20 (B.2)                                                                        */
+    int32_t general_grid;  /* 0 (default): two_theta must be uniform (the fast path).  1: any strictly increasing grid whose
+                              steps differ by at most a factor 16 (R31): j_m = the grid point nearest to p_m, the window stays
+                              |i - j_m| <= n_c with n_c from the MEAN step; the kernels read per-tile point offsets and
+                              per-record bases (x_{i0} - p_m, fp64-computed) instead of (i - j_m) Delta, every record takes
+                              the per-point bodies (about half the speed).  The flag sizes the workspace, so it is part
+                              of xrdvi_workspace_bytes' input; a uniform grid is accepted with it as well               */
+    int32_t _pad2;
 } xrdvi_hyper;
 
 void xrdvi_default_hyper(xrdvi_hyper* hyp);
@@ -97,10 +105,10 @@ size_t xrdvi_workspace_bytes(int64_t N, int32_t K, int64_t M, int32_t S_max, dou
                              const xrdvi_hyper* hyp);
 
 /* Build a problem.
- *  two_theta [N]     strictly increasing, uniform grid (deg): the peak encoding (nearest grid index + fp64 offset,
- *                    R16) and the integer window need a constant step; a grid that departs from uniform by more
- *                    than 1e-6 of the step is rejected with XRDVI_E_NONUNIFORM_GRID (the paper's grid is uniform,
- *                    PAPER.md:84)
+ *  two_theta [N]     strictly increasing (deg).  Uniform (the paper's grid) is the fast path: the peak
+ *                    encoding (nearest grid index + fp64 offset, R16) and the packed bodies use the constant step.  A
+ *                    grid that departs from uniform by more than 1e-6 of the step needs hyper.general_grid = 1 (R31),
+ *                    else XRDVI_E_NONUNIFORM_GRID
  *  y [P][N]          observed intensities;  background [P][N] or NULL (-> 0) (R5: B is an input)
  *  peak_ofs [K+1]    CSR offsets into peak_pos / peak_int ([M], M = peak_ofs[K]); any order inside
  *                    a phase; peaks with no in-window grid point are dropped (R16)

@@ -42,6 +42,7 @@ class Hyper(C.Structure):
         ("adam_eps", C.c_double), ("init_log_sigma", C.c_double),
         ("n_patterns", C.c_int32), ("n_restarts", C.c_int32), ("likelihood", C.c_int32), ("optimizer", C.c_int32),
         ("asymmetry", C.c_int32), ("width_sec", C.c_int32), ("alpha_mu", C.c_double), ("alpha_sigma", C.c_double),
+        ("general_grid", C.c_int32), ("_pad2", C.c_int32),
     ]
 
 

@@ -45,7 +45,7 @@ struct Plan {   // workspace carve; identical arithmetic in workspace_bytes and 
     size_t o_var, o_vartmp, o_mom1, o_mom2, o_grad, o_elbo, o_elbok, o_llt, o_trace, o_ctl;
     size_t o_lat, o_eps, o_rr, o_ng, o_llpart, o_part8, o_dbg;
     size_t o_pd, o_lpk, o_zeta, o_gradz, o_lls, o_partial, o_tcnt, o_summ;
-    size_t o_trng, o_ia, o_epsa, o_parta, o_pksec, o_secmax;
+    size_t o_trng, o_ia, o_epsa, o_parta, o_pksec, o_secmax, o_tileoff, o_pkbase;
     int pd_groups;     // groups one launch of the log-joint gradient service handles
 };
 
@@ -152,23 +152,26 @@ bool make_plan(int64_t N, int32_t K, int64_t M, int32_t S_max, double step, cons
     p.o_partial = take(p.split ? sizeof(float) * kPT * 32 * static_cast<size_t>(p.G_max) * p.n_tile * p.PS : 0);
     p.o_tcnt = take(sizeof(unsigned int) * 2 * static_cast<size_t>(p.G_max) * p.n_tile);
     p.o_trng = take(sizeof(int2) * (static_cast<size_t>(p.n_tile) + 1));
-    const bool model = hyp->asymmetry || hyp->width_sec;    // R30 buffers only when the extension is on
+    const bool model = hyp->asymmetry || hyp->width_sec || hyp->general_grid;    // R30 / R31 buffers only when in use
     p.o_ia = take(model ? sizeof(float) * gk32 : 0);
     p.o_epsa = take(model ? sizeof(float) * gk32 : 0);
     p.o_parta = take(model ? sizeof(float) * 2 * static_cast<size_t>(p.G_max) * std::max<long long>(p.slots_cap, 1) : 0);
     p.o_pksec = take(hyp->width_sec ? sizeof(float) * (p.tile_cap + 1) : 0);
     p.o_secmax = take(sizeof(float) * K);
+    p.o_tileoff = take(hyp->general_grid ? sizeof(float) * kPT * static_cast<size_t>(p.n_tile) : 0);
+    p.o_pkbase = take(hyp->general_grid ? sizeof(float) * (p.tile_cap + 1) : 0);
     p.total = o;
     *pl = p;
     return true;
 }
 
 // ---- static tables (R16, R27) -----------------------------------------------------------------------
-struct HostPeak { long long j; double d; double I; int k; double inv_s; };   // nearest grid index, p_m - x_j, intensity, phase, cos(p_m / 2) (R30)
+struct HostPeak { long long j; double d; double I; int k; double inv_s; double pos; };   // nearest grid index, p_m - x_j, intensity, phase, cos(p_m / 2) (R30)
 
 struct Tables {
     std::vector<PeakRec> pk_tile;     // per-tile phase-major peak lists (+1 padding record)
     std::vector<float> pk_sec;        // cos(p_m / 2) of every record's peak (sec width term, R30)
+    std::vector<float> pk_base;       // x_{i0} - p_m of every record (general grid, R31)
     std::vector<int4> run_tab;        // (m0, m1, phase, slot) per phase run (+1 padding header)
     std::vector<int2> share_rng;      // [n_tile][PS] run ranges of the shares
     std::vector<int> seg_order, slot_ofs;
@@ -183,7 +186,7 @@ struct Tables {
 // tile).  `nck[k]` is the window half-width of phase k in points (the static n_c for every phase at create; per
 // phase after xrdvi_set_phase_windows, R27); peaks with no in-range grid point are dropped.  All in integers.
 const char* build_tables(const Plan& pl, int64_t N, int K, const std::vector<HostPeak>& all,
-                         const std::vector<long long>& nck, Tables* T) {
+                         const std::vector<long long>& nck, const std::vector<double>& xgrid, Tables* T) {
     std::vector<HostPeak> fw;
     fw.reserve(all.size());
     long long pairs = 0;
@@ -219,6 +222,7 @@ const char* build_tables(const Plan& pl, int64_t N, int K, const std::vector<Hos
     if (n_ent > pl.tile_cap || n_runs > pl.slots_cap) return "internal: table bound exceeded";
     // pass 2: fill the lists, the run headers (m0, m1, phase, 0) and the clipped pair count of every run
     T->pk_sec.assign(static_cast<size_t>(n_ent) + 1, 1.0f);
+    T->pk_base.assign(xgrid.empty() ? 0 : static_cast<size_t>(n_ent) + 1, 0.0f);
     T->pk_tile.assign(static_cast<size_t>(n_ent) + 1, PeakRec{0, 0.f, 0.f, 0});   // +1: the kernel prefetches one
     T->run_tab.assign(static_cast<size_t>(n_runs) + 1, make_int4(0, 0, 0, 0));    // record / header past the end
     T->share_rng.assign(static_cast<size_t>(n_tile) * PSn, make_int2(0, 0));
@@ -241,6 +245,7 @@ const char* build_tables(const Plan& pl, int64_t N, int K, const std::vector<Hos
             T->pk_tile[e] = PeakRec{static_cast<int>(dj), static_cast<float>(p.d), static_cast<float>(p.I),
                                     static_cast<int>(n << 1) | (full ? 1 : 0)};
             T->pk_sec[e] = static_cast<float>(p.inv_s);
+            if (!xgrid.empty()) T->pk_base[e] = static_cast<float>(xgrid[i0] - p.pos);   // fp64 difference (R31)
             if (last_k[t] != p.k) {
                 last_k[t] = p.k;
                 T->run_tab[run_cur[t]++] = make_int4(static_cast<int>(e), static_cast<int>(e), p.k, 0);
@@ -344,6 +349,7 @@ struct xrdvi {
     bool windowed = false;     // hyper.window_W > 0
     double delta = 0.0;        // grid step
     std::vector<HostPeak> peaks;   // every input peak, CSR order (xrdvi_set_phase_windows rebuilds the tables from it)
+    std::vector<double> xgrid;     // the grid, kept only for hyper.general_grid (R31: per-record bases x_{i0} - p_m)
     std::vector<long long> n_ck;   // [K] half-width per phase in force (R27); all n_c after create
     std::vector<float> m_h0;   // per pattern initial m_h
     float m_w0 = 0.f;
@@ -384,6 +390,8 @@ int install_tables(xrdvi* h, const Tables& T, const std::vector<long long>& nck,
     CU(cudaMemcpyAsync(w + pl.o_sord, T.seg_order.data(), sizeof(int) * T.seg_order.size(), cudaMemcpyHostToDevice, st));
     CU(cudaMemcpyAsync(w + pl.o_sofs, T.slot_ofs.data(), sizeof(int) * T.slot_ofs.size(), cudaMemcpyHostToDevice, st));
     CU(cudaMemcpyAsync(w + pl.o_trng, T.tile_rng.data(), sizeof(int2) * T.tile_rng.size(), cudaMemcpyHostToDevice, st));
+    if (h->hyp.general_grid)
+        CU(cudaMemcpyAsync(w + pl.o_pkbase, T.pk_base.data(), sizeof(float) * T.pk_base.size(), cudaMemcpyHostToDevice, st));
     if (h->hyp.width_sec)
         CU(cudaMemcpyAsync(w + pl.o_pksec, T.pk_sec.data(), sizeof(float) * T.pk_sec.size(), cudaMemcpyHostToDevice, st));
     if (at_create) {
@@ -671,6 +679,7 @@ void xrdvi_default_hyper(xrdvi_hyper* hy) {
     hy->width_sec = 0;
     hy->alpha_mu = 1.0;        // B.2
     hy->alpha_sigma = 0.2;
+    hy->general_grid = 0;
 }
 
 size_t xrdvi_workspace_bytes(int64_t N, int32_t K, int64_t M, int32_t S_max, double two_theta_step,
@@ -708,10 +717,27 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
     const int64_t M = ofs[K];
     for (int64_t i = 1; i < N; ++i)
         if (!(x[i] > x[i - 1])) return fail(XRDVI_E_UNSORTED_GRID, "two_theta not strictly increasing");
-    const double delta = (x[N - 1] - x[0]) / static_cast<double>(N - 1);
-    for (int64_t i = 0; i < N; ++i)
-        if (std::fabs(x[i] - (x[0] + delta * static_cast<double>(i))) > 1e-6 * delta)
-            return fail(XRDVI_E_NONUNIFORM_GRID, "two_theta is not a uniform grid (this build needs one)");
+    const double delta = (x[N - 1] - x[0]) / static_cast<double>(N - 1);   // the (mean) step
+    bool uniform = true;
+    double step_min = x[1] - x[0], step_max = step_min;
+    for (int64_t i = 0; i < N; ++i) {
+        if (std::fabs(x[i] - (x[0] + delta * static_cast<double>(i))) > 1e-6 * delta) uniform = false;
+        if (i > 0) { step_min = std::min(step_min, x[i] - x[i - 1]); step_max = std::max(step_max, x[i] - x[i - 1]); }
+    }
+    if (!uniform && !hyp->general_grid)
+        return fail(XRDVI_E_NONUNIFORM_GRID, "two_theta is not a uniform grid (set hyper.general_grid = 1 for the general path)");
+    if (!uniform && step_max > 16.0 * step_min)
+        return fail(XRDVI_E_NONUNIFORM_GRID, "two_theta steps differ by more than a factor 16");
+    const bool general = hyp->general_grid != 0;          // the general path also takes a uniform grid
+    // R31: nearest grid point of p (the lower one on a tie); beyond the grid continued with the mean step
+    auto nearest = [&](double p) -> long long {
+        if (uniform) return static_cast<long long>(std::floor((p - x[0]) / delta + 0.5));
+        if (p <= x[0]) return -static_cast<long long>(std::floor((x[0] - p) / delta + 0.5));
+        if (p >= x[N - 1]) return N - 1 + static_cast<long long>(std::floor((p - x[N - 1]) / delta + 0.5));
+        const double* hi = std::lower_bound(x, x + N, p);  // first x_i >= p; 0 < hi - x < N here
+        const long long i1 = hi - x, i0 = i1 - 1;
+        return (x[i1] - p) < (p - x[i0]) ? i1 : i0;
+    };
     for (int64_t m = 0; m < M; ++m)
         if (!std::isfinite(pos[m]) || !std::isfinite(inten[m]) || inten[m] < 0.0)
             return fail(XRDVI_E_INVALID_ARG, "peak position/intensity not finite or negative intensity");
@@ -735,7 +761,7 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
     if (n_c < 0) {     // dense: every point is inside every window, wherever the peak lies
         n_c = N;
         for (int64_t m = 0; m < M; ++m) {
-            const long long j = static_cast<long long>(std::floor((pos[m] - x[0]) / delta + 0.5));
+            const long long j = nearest(pos[m]);
             n_c = std::max<long long>(n_c, std::max<long long>(std::llabs(j), std::llabs(N - 1 - j)) + 1);
         }
     }
@@ -749,18 +775,19 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
         for (int64_t m = ofs[k]; m < ofs[k + 1]; ++m) {
             area[k] += inten[m];
             imax = std::max(imax, inten[m]);
-            const long long j = static_cast<long long>(std::floor((pos[m] - x[0]) / delta + 0.5));
+            const long long j = nearest(pos[m]);
             const double xj = (j >= 0 && j < N) ? x[j] : x[0] + delta * static_cast<double>(j);
             const double inv_s = hyp->width_sec ? std::cos(0.5 * pos[m] * M_PI / 180.0) : 1.0;   // R30: 1 / sec(p_m / 2)
             if (!(inv_s > 1e-3)) return fail(XRDVI_E_INVALID_ARG, "width_sec needs peak positions below 180 deg");
             sec_max[k] = std::max(sec_max[k], static_cast<float>(1.0 / inv_s));
-            all_peaks.push_back({j, pos[m] - xj, inten[m], k, inv_s});
+            all_peaks.push_back({j, pos[m] - xj, inten[m], k, inv_s, pos[m]});
         }
     for (int k = 0; k < K; ++k)
         if (!(area[k] > 0.0)) return fail(XRDVI_E_EMPTY_PHASE, "phase " + std::to_string(k) + " has zero total intensity");
     const std::vector<long long> nck0(K, n_c);
     Tables tabs;
-    if (const char* terr = build_tables(pl, N, K, all_peaks, nck0, &tabs)) return fail(XRDVI_E_INVALID_ARG, terr);
+    const std::vector<double> xgrid = general ? std::vector<double>(x, x + N) : std::vector<double>();
+    if (const char* terr = build_tables(pl, N, K, all_peaks, nck0, xgrid, &tabs)) return fail(XRDVI_E_INVALID_ARG, terr);
 
     // observed data and per-pattern constants
     std::vector<float> yb(static_cast<size_t>(P) * N), bgf(static_cast<size_t>(P) * N);
@@ -817,6 +844,7 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
     h->windowed = pl.n_c >= 0;
     h->delta = delta;
     h->peaks = std::move(all_peaks);
+    h->xgrid = xgrid;
     h->m_h0 = m_h0;
     h->m_w0 = static_cast<float>(std::log(hyp->w_shape / hyp->w_rate));
     Dev& d = h->dev;
@@ -826,8 +854,15 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
     d.likelihood = hyp->likelihood;
     d.optimizer = hyp->optimizer;
     d.delta = static_cast<float>(delta);
-    d.gcut = static_cast<float>(static_cast<double>(kGaussCut) / (2.0 * delta));
-    d.inv_delta = static_cast<float>(1.0 / delta);
+    // Gaussian-core half-width in POINTS: with the smallest step on a general grid (R31), and a slack that covers
+    // |p_m - x_{j_m}| <= step_max / 2 in units of that step
+    const double core_step = general ? step_min : delta;
+    d.gcut = static_cast<float>(static_cast<double>(kGaussCut) / (2.0 * core_step));
+    d.inv_delta = static_cast<float>(1.0 / core_step);
+    d.general = general ? 1 : 0;
+    d.reach_pad = general ? static_cast<float>(1.0 + 0.5 * step_max / step_min + 1e-3) : 1.5f;
+    d.tile_off = reinterpret_cast<float*>(w + pl.o_tileoff);
+    d.pk_base = reinterpret_cast<float*>(w + pl.o_pkbase);
     d.mu_inv_var = static_cast<float>(1.0 / (hyp->mu_sigma * hyp->mu_sigma));
     d.mu_logc = static_cast<float>(-std::log(hyp->mu_sigma * std::sqrt(2.0 * M_PI)));
     d.w_shape = static_cast<float>(hyp->w_shape);
@@ -876,7 +911,7 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
     }
     d.asym = hyp->asymmetry;
     d.sec = hyp->width_sec;
-    d.model = (hyp->asymmetry || hyp->width_sec) ? 1 : 0;
+    d.model = (hyp->asymmetry || hyp->width_sec || hyp->general_grid) ? 1 : 0;
     d.alpha_mu = static_cast<float>(hyp->alpha_mu);
     d.alpha_inv_var = static_cast<float>(1.0 / (hyp->alpha_sigma * hyp->alpha_sigma));
     d.alpha_logc = static_cast<float>(-std::log(hyp->alpha_sigma * std::sqrt(2.0 * M_PI)));
@@ -903,6 +938,13 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
     chk(up(pl.o_pat, pat.data(), sizeof(PatConst) * pat.size()));
     chk(up(pl.o_area, area.data(), sizeof(double) * area.size()));
     chk(up(pl.o_secmax, sec_max.data(), sizeof(float) * sec_max.size()));
+    std::vector<float> tile_off;
+    if (general) {   // R31: offsets of every tile's points from its first one, fp64 differences
+        tile_off.assign(static_cast<size_t>(pl.n_tile) * kPT, 0.0f);
+        for (int64_t i = 0; i < N; ++i) tile_off[i] = static_cast<float>(x[i] - x[i / kPT * kPT]);
+        for (size_t i = N; i < tile_off.size(); ++i) tile_off[i] = tile_off[N - 1] + static_cast<float>(delta * (i - (N - 1)));
+        chk(up(pl.o_tileoff, tile_off.data(), sizeof(float) * tile_off.size()));
+    }
     chk(up(pl.o_mh0, m_h0.data(), sizeof(float) * m_h0.size()));
     chk(cudaMemsetAsync(w + pl.o_tcnt, 0, sizeof(unsigned int) * 2 * static_cast<size_t>(pl.G_max) * pl.n_tile, st));
     chk(cudaMemsetAsync(w + pl.o_trace, 0xFF, sizeof(double) * kTraceCap * pl.PR, st));
@@ -947,7 +989,7 @@ int xrdvi_set_phase_windows(xrdvi* h, const int32_t* n_ck) {
     if (nck == h->n_ck) return XRDVI_OK;
     CU(cudaSetDevice(h->device));
     Tables tabs;
-    if (const char* terr = build_tables(h->plan, h->N, h->K, h->peaks, nck, &tabs)) return fail(XRDVI_E_INVALID_ARG, terr);
+    if (const char* terr = build_tables(h->plan, h->N, h->K, h->peaks, nck, h->xgrid, &tabs)) return fail(XRDVI_E_INVALID_ARG, terr);
     return install_tables(h, tabs, nck, false);
 }
 

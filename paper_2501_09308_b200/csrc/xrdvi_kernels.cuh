@@ -135,7 +135,11 @@ struct Dev {
     // peak asymmetry and the sec width term (reading R30; hyper.asymmetry / hyper.width_sec).  asym = 1: a fifth latent
     // alpha_k per phase; every state array has a companion for it ([PR][2][K]: m_alpha, l_alpha)
     int asym, sec;
-    int model;                // 1: asym or sec is on: the tile kernels run tile_phase*_asym (per-draw rows of 160 floats)
+    int general;              // 1: non-uniform 2theta grid (R31): per-tile point offsets and per-record bases instead of (i - j) Delta
+    float reach_pad;          // slack of the Gaussian-core half-width in points: 1.5 on a uniform grid (|delta_m| <= Delta/2, rounding)
+    const float* tile_off;    // [n_tile][16] x_{i0 + p} - x_{i0} (general = 1)
+    const float* pk_base;     // [records] x_{i0} - p_m of the record's tile and peak, fp64-computed (general = 1)
+    int model;                // 1: asym, sec or general is on: the tile kernels run tile_phase*_asym (per-draw rows of 160 floats)
     float alpha_mu, alpha_inv_var, alpha_logc;   // prior Norm(alpha_mu, alpha_sigma): mean, 1/sigma^2, -ln(sigma sqrt(2 pi))
     const float* pk_sec;      // [records] cos(p_m / 2) = 1 / sec factor of the record's peak (sec = 1 only)
     const float* sec_max;     // [K] largest sec factor of the phase's peaks (1 without the sec term)
@@ -248,7 +252,7 @@ __device__ __forceinline__ void emit_latent(const Dev& d, int g, int k, bool val
     float wide = q.w;
     if (d.asym) wide *= fmaxf(alpha, 1.0f);
     if (d.sec) wide *= d.sec_max[k];
-    float reach = fmaf(d.gcut, wide, fabsf(q.mu) * d.inv_delta) + 1.5f;
+    float reach = fmaf(d.gcut, wide, fabsf(q.mu) * d.inv_delta) + d.reach_pad;
     if (!valid) {
         lt = make_float4(1.0f, 0.0f, 0.0f, 0.0f);
         reach = 0.0f;
@@ -909,8 +913,8 @@ __device__ __forceinline__ void tile_phase2(const Dev& d, const Src& src, const 
 // draws (the core half-width covers the largest sampled shift), so they keep the packed bodies with (t0, step) scaled
 // by ia on the high side; core and window-edge records take the scalar per-point bodies below.
 template <int Q>
-__device__ __forceinline__ void fwd_quad_asym(const PeakGeo& g, float t0, float step, float iam1, float cg2, float cl,
-                                              f32x2& accX, f32x2& accY) {
+__device__ __forceinline__ void fwd_quad_asym(const PeakGeo& g, const float (&o)[kPT], float t0, float sx, float iam1,
+                                              float cg2, float cl, f32x2& accX, f32x2& accY) {
     const int lo = max(g.p_lo, 4 * Q), hi = min(g.p_hi, 4 * Q + 3);
     if (lo > hi) return;                                   // quad outside the window
     const unsigned span = static_cast<unsigned>(hi - lo);
@@ -919,7 +923,7 @@ __device__ __forceinline__ void fwd_quad_asym(const PeakGeo& g, float t0, float 
     unpack2(accY, a[1], a[3]);
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
-        float t = fmaf(static_cast<float>(4 * Q + i), step, t0);
+        float t = fmaf(o[4 * Q + i], sx, t0);              // o_p = x_{i0+p} - x_{i0} (p Delta on a uniform grid), sx = 2 / w_m
         t = fmaf(fmaxf(t, 0.0f), iam1, t);                 // high-angle side: t' / alpha
         u[i] = fmaf(t, t, 1.0f);
         m[i] = static_cast<unsigned>(4 * Q + i - lo) <= span ? 1.0f : 0.0f;
@@ -942,8 +946,8 @@ __device__ __forceinline__ void fwd_quad_asym(const PeakGeo& g, float t0, float 
 struct Acc8 { float a1, a2, a5, a6u, a3m, a4m, h1, h2; };
 
 template <int Q>
-__device__ __forceinline__ void bwd_quad_asym(const PeakGeo& g, float t0, float step, float iam1, float ia2m1, f32x2 eX,
-                                              f32x2 eY, Acc8& a) {
+__device__ __forceinline__ void bwd_quad_asym(const PeakGeo& g, const float (&o)[kPT], float t0, float sx, float iam1,
+                                              float ia2m1, f32x2 eX, f32x2 eY, Acc8& a) {
     const int lo = max(g.p_lo, 4 * Q), hi = min(g.p_hi, 4 * Q + 3);
     if (lo > hi) return;
     const unsigned span = static_cast<unsigned>(hi - lo);
@@ -952,7 +956,7 @@ __device__ __forceinline__ void bwd_quad_asym(const PeakGeo& g, float t0, float 
     unpack2(eY, ev[1], ev[3]);
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
-        const float tp = fmaf(static_cast<float>(4 * Q + i), step, t0);
+        const float tp = fmaf(o[4 * Q + i], sx, t0);
         const float mx = fmaxf(tp, 0.0f);
         const float t = fmaf(mx, iam1, tp);
         tm[i] = fmaf(mx, ia2m1, tp);
@@ -983,6 +987,21 @@ __device__ __forceinline__ void bwd_quad_asym(const PeakGeo& g, float t0, float 
     }
 }
 
+// Offsets of the tile's 16 points from its first one: p Delta on a uniform grid, the table of R31 otherwise.
+__device__ __forceinline__ void tile_offsets(const Dev& d, const TileCtx& c, float (&o)[kPT]) {
+    if (d.general) {
+        const float4* __restrict__ t = reinterpret_cast<const float4*>(d.tile_off + static_cast<size_t>(c.i0));   // i0 = 16 tile
+#pragma unroll
+        for (int v = 0; v < kPT / 4; ++v) {
+            const float4 q = t[v];
+            o[4 * v] = q.x; o[4 * v + 1] = q.y; o[4 * v + 2] = q.z; o[4 * v + 3] = q.w;
+        }
+    } else {
+#pragma unroll
+        for (int p = 0; p < kPT; ++p) o[p] = static_cast<float>(p) * d.delta;
+    }
+}
+
 // Phase 1 with the asymmetry / sec term (R30).  ia_g: 1 / alpha of the group's draws, already offset by the lane.
 template <class Src>
 __device__ __forceinline__ void tile_phase1_asym(const Dev& d, const Src& src, const TileCtx& c, int2 rng, float (&acc)[kPT]) {
@@ -990,6 +1009,8 @@ __device__ __forceinline__ void tile_phase1_asym(const Dev& d, const Src& src, c
 #pragma unroll
     for (int i = 0; i < kPT / 2; ++i) acc2[i] = 0ull;
     const float* __restrict__ iag = d.ia + static_cast<size_t>(c.g) * d.K * 32 + (threadIdx.x & 31);
+    float o[kPT];                                           // point offsets of the tile from its first point
+    tile_offsets(d, c, o);
     for (int r = rng.x; r < rng.y; ++r) {
         const int4 run = src.run(r);
         const float4 lt = c.lat[static_cast<size_t>(run.z) * 32];
@@ -1003,19 +1024,22 @@ __device__ __forceinline__ void tile_phase1_asym(const Dev& d, const Src& src, c
             const PeakRec pk = src.rec(m);
             const float inv_s = d.sec ? d.pk_sec[m] : 1.0f;
             float step = step_k * inv_s;
-            float t0 = fmaf(static_cast<float>(-pk.dj), step_k, fmaf(-pk.delta, lt.x, lt.y)) * inv_s;
+            // t' at the first point of the tile: grid-index form on a uniform grid, x_{i0} - p_m from the table otherwise
+            float t0 = (d.general ? fmaf(d.pk_base[m], lt.x, lt.y)
+                                  : fmaf(static_cast<float>(-pk.dj), step_k, fmaf(-pk.delta, lt.x, lt.y))) * inv_s;
             const float cl = pk.inten * lt.w * inv_s;
             const bool core = static_cast<unsigned>(pk.dj + ngc) <= core_span;
-            if ((pk.full & 1) && !core) {                   // one side of the peak for every draw: packed body
+            if ((pk.full & 1) && !core && !d.general) {     // one side of the peak for every draw: packed body
                 if (pk.dj < 0) { t0 *= ia; step *= ia; }    // the tile lies above the peak: high-angle side
                 fwd_tile2<false>(t0, step, 0.0f, cl, acc2);
             } else {
                 const PeakGeo geo = edge_geo(pk.dj, ngc, pk.full >> 1, c.plim);
                 const float cg2 = 2.0f * pk.inten * lt.z * inv_s;
-                fwd_quad_asym<0>(geo, t0, step, iam1, cg2, cl, acc2[0], acc2[1]);
-                fwd_quad_asym<1>(geo, t0, step, iam1, cg2, cl, acc2[2], acc2[3]);
-                fwd_quad_asym<2>(geo, t0, step, iam1, cg2, cl, acc2[4], acc2[5]);
-                fwd_quad_asym<3>(geo, t0, step, iam1, cg2, cl, acc2[6], acc2[7]);
+                const float sx = lt.x * inv_s;
+                fwd_quad_asym<0>(geo, o, t0, sx, iam1, cg2, cl, acc2[0], acc2[1]);
+                fwd_quad_asym<1>(geo, o, t0, sx, iam1, cg2, cl, acc2[2], acc2[3]);
+                fwd_quad_asym<2>(geo, o, t0, sx, iam1, cg2, cl, acc2[4], acc2[5]);
+                fwd_quad_asym<3>(geo, o, t0, sx, iam1, cg2, cl, acc2[6], acc2[7]);
             }
         }
     }
@@ -1042,6 +1066,8 @@ __device__ __forceinline__ void tile_phase2_asym(const Dev& d, const Src& src, c
         pe2[2 * Q + 1] = pack2(static_cast<float>(4 * Q + 1) * e[4 * Q + 1], static_cast<float>(4 * Q + 3) * e[4 * Q + 3]);
     }
     const size_t gk = static_cast<size_t>(c.g) * d.K * 32 + lane;
+    float off[kPT];
+    tile_offsets(d, c, off);
     for (int r = rng.x; r < rng.y; ++r) {
         const int4 run = src.run(r);
         const size_t o = gk + static_cast<size_t>(run.z) * 32;
@@ -1062,10 +1088,11 @@ __device__ __forceinline__ void tile_phase2_asym(const Dev& d, const Src& src, c
             const PeakRec pk = src.rec(m);
             const float inv_s = d.sec ? d.pk_sec[m] : 1.0f;
             float step = step_k * inv_s;
-            float t0 = fmaf(static_cast<float>(-pk.dj), step_k, fmaf(-pk.delta, lt.x, lt.y)) * inv_s;
+            float t0 = (d.general ? fmaf(d.pk_base[m], lt.x, lt.y)
+                                  : fmaf(static_cast<float>(-pk.dj), step_k, fmaf(-pk.delta, lt.x, lt.y))) * inv_s;
             const float wI = pk.inten * inv_s;              // height factor of the record
             const bool core = static_cast<unsigned>(pk.dj + ngc) <= core_span;
-            if ((pk.full & 1) && !core) {
+            if ((pk.full & 1) && !core && !d.general) {
                 const bool high = pk.dj < 0;
                 if (high) { t0 *= ia; step *= ia; }
                 Acc6x2 a2 = {0ull, 0ull, 0ull, 0ull, 0ull, 0ull};
@@ -1079,10 +1106,11 @@ __device__ __forceinline__ void tile_phase2_asym(const Dev& d, const Src& src, c
             } else {
                 const PeakGeo geo = edge_geo(pk.dj, ngc, pk.full >> 1, c.plim);
                 Acc8 a = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-                bwd_quad_asym<0>(geo, t0, step, iam1, ia2m1, e2[0], e2[1], a);
-                bwd_quad_asym<1>(geo, t0, step, iam1, ia2m1, e2[2], e2[3], a);
-                bwd_quad_asym<2>(geo, t0, step, iam1, ia2m1, e2[4], e2[5], a);
-                bwd_quad_asym<3>(geo, t0, step, iam1, ia2m1, e2[6], e2[7], a);
+                const float sx = lt.x * inv_s;
+                bwd_quad_asym<0>(geo, off, t0, sx, iam1, ia2m1, e2[0], e2[1], a);
+                bwd_quad_asym<1>(geo, off, t0, sx, iam1, ia2m1, e2[2], e2[3], a);
+                bwd_quad_asym<2>(geo, off, t0, sx, iam1, ia2m1, e2[4], e2[5], a);
+                bwd_quad_asym<3>(geo, off, t0, sx, iam1, ia2m1, e2[6], e2[7], a);
                 const float i2 = 2.0f * wI;                 // g = G/2 in the Gaussian sums
                 B1 = fmaf(wI, a.a1, B1);
                 B2 = fmaf(i2, a.a2, B2);
