@@ -44,7 +44,7 @@ def test_measure_library_builds_and_exports_its_symbol():
 def test_product_library_reads_no_environment_knob():
     """The tuning knobs (kernel shape, fused / split, PDL, staging) exist only under -DXRDVI_TUNING."""
     blob = (ROOT / "paper_2501_09308_b200" / "libxrdvi.so").read_bytes()
-    for knob in (b"XRDVI_TILE_SHAPE", b"XRDVI_FUSED", b"XRDVI_SPLIT", b"XRDVI_NO_PDL", b"XRDVI_NO_UNROLL", b"XRDVI_NO_STAGE"):
+    for knob in (b"XRDVI_TILE_SHAPE", b"XRDVI_FUSED", b"XRDVI_SPLIT", b"XRDVI_NO_PDL", b"XRDVI_NO_UNROLL", b"XRDVI_NO_STAGE", b"XRDVI_G_BLOCK"):
         assert knob not in blob, knob
 
 
