@@ -745,13 +745,14 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
     int dev_count = 0;
     CU(cudaGetDeviceCount(&dev_count));
     if (device < 0 || device >= dev_count) return fail(XRDVI_E_CUDA, "no such CUDA device");
-    cudaDeviceProp prop;
-    CU(cudaGetDeviceProperties(&prop, device));
-    if (prop.major != 10) return fail(XRDVI_E_NOT_SM100, "device is not compute capability 10.x (sm_100a build)");
+    int cc_major = 0, n_sm = 0;   // two attribute queries: cudaGetDeviceProperties costs ~1 ms per call
+    CU(cudaDeviceGetAttribute(&cc_major, cudaDevAttrComputeCapabilityMajor, device));
+    CU(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, device));
+    if (cc_major != 10) return fail(XRDVI_E_NOT_SM100, "device is not compute capability 10.x (sm_100a build)");
     CU(cudaSetDevice(device));
 
     Plan pl;
-    if (!make_plan(N, K, M, S_max, delta, hyp, prop.multiProcessorCount, &pl)) return fail(XRDVI_E_INVALID_ARG, "sizes out of range");
+    if (!make_plan(N, K, M, S_max, delta, hyp, n_sm, &pl)) return fail(XRDVI_E_INVALID_ARG, "sizes out of range");
     if (workspace_bytes < pl.total) return fail(XRDVI_E_WORKSPACE_TOO_SMALL, "workspace too small: need " + std::to_string(pl.total));
     if (reinterpret_cast<uintptr_t>(workspace) % 256) return fail(XRDVI_E_INVALID_ARG, "workspace not 256-byte aligned");
 
