@@ -397,11 +397,12 @@ __device__ __forceinline__ void fwd_tile2(float t0, float step, float cg2, float
     }
 }
 
-// Phase 2, full tile: the six sums of bwd_pair, each as a pair of partial sums (X points, Y points).
-struct Acc6x2 { f32x2 a1, a2, a3p, a4p, a5, a6u; };
+// Phase 2, full tile: the six sums of Acc6, each as a pair of partial sums (X points, Y points).  e t' is formed per
+// quad: two more packed multiplications per quad than weights p e_p held in registers would need (sum e L^2 t' =
+// t0 a5 + step sum p e L^2), but sixteen registers fewer, which measures faster (profiles/r2_dead_ends.md, "kept").
+struct Acc6x2 { f32x2 a1, a2, a3t, a4t, a5, a6t; };
 template <bool CORE>
-__device__ __forceinline__ void bwd_tile2(float t0, float step, const f32x2 (&e2)[kPT / 2], const f32x2 (&pe2)[kPT / 2],
-                                          Acc6x2& a) {
+__device__ __forceinline__ void bwd_tile2(float t0, float step, const f32x2 (&e2)[kPT / 2], Acc6x2& a) {
     Quad2 q = quad2_begin(t0, step);
     const f32x2 one2 = pack2(1.0f, 1.0f);
 #pragma unroll
@@ -410,14 +411,15 @@ __device__ __forceinline__ void bwd_tile2(float t0, float step, const f32x2 (&e2
         const f32x2 r = rcp2(mul2(uX, uY));
         const f32x2 LX = mul2(r, uY), LY = mul2(r, uX);
         const f32x2 L2X = mul2(LX, LX), L2Y = mul2(LY, LY);
+        const f32x2 etX = mul2(e2[2 * Q], q.tX), etY = mul2(e2[2 * Q + 1], q.tY);
         a.a1 = fma2(e2[2 * Q], LX, fma2(e2[2 * Q + 1], LY, a.a1));
         a.a5 = fma2(e2[2 * Q], L2X, fma2(e2[2 * Q + 1], L2Y, a.a5));
-        a.a3p = fma2(pe2[2 * Q], L2X, fma2(pe2[2 * Q + 1], L2Y, a.a3p));
+        a.a3t = fma2(etX, L2X, fma2(etY, L2Y, a.a3t));
         if (CORE) {
             const f32x2 gX = ex2neg2(uX), gY = ex2neg2(uY);
             a.a2 = fma2(e2[2 * Q], gX, fma2(e2[2 * Q + 1], gY, a.a2));
-            a.a4p = fma2(pe2[2 * Q], gX, fma2(pe2[2 * Q + 1], gY, a.a4p));
-            a.a6u = fma2(mul2(e2[2 * Q], uX), gX, fma2(mul2(e2[2 * Q + 1], uY), gY, a.a6u));
+            a.a4t = fma2(etX, gX, fma2(etY, gY, a.a4t));
+            a.a6t = fma2(mul2(etX, q.tX), gX, fma2(mul2(etY, q.tY), gY, a.a6t));
         }
         if (Q + 1 < kPT / 4) {
             q.tX = add2(q.tX, q.step4);
@@ -483,49 +485,29 @@ __device__ __forceinline__ void fwd_quad_generic(const PeakGeo& g, float t0, flo
 }
 
 // ------------------------------------------------------------------------------------------------
-// Phase-2 building blocks.  Per (peak, tile) with t'_p = t0 + p step, e_p the residual and pe_p = p e_p:
-//   a1 = sum e L, a5 = sum e L^2, a3p = sum pe L^2      (Lorentz part, every in-window point)
-//   a2 = sum e g, a4p = sum pe g, a6u = sum e u g       (Gaussian part, core points only; g = 2^(-u) = G/2,
-//                                                        u = 1 + t'^2)
-// and then  sum e L^2 t' = t0 a5 + step a3p,  sum e G = 2 a2,  sum e G t' = 2 (t0 a2 + step a4p),
-// sum e G t'^2 = 2 (a6u - a2).
-struct Acc6 { float a1, a2, a3p, a4p, a5, a6u; };
-
-template <bool CORE>
-__device__ __forceinline__ void bwd_pair(float ea, float eb, float pea, float peb, float ta, float tb, Acc6& a) {
-    const float ua = fmaf(ta, ta, 1.0f), ub = fmaf(tb, tb, 1.0f);
-    const float r = rcp_approx(ua * ub);
-    const float La = r * ub, Lb = r * ua;
-    const float La2 = La * La, Lb2 = Lb * Lb;
-    a.a1 = fmaf(ea, La, fmaf(eb, Lb, a.a1));
-    a.a5 = fmaf(ea, La2, fmaf(eb, Lb2, a.a5));
-    a.a3p = fmaf(pea, La2, fmaf(peb, Lb2, a.a3p));
-    if (CORE) {
-        const float ga = ex2_approx(-ua), gb = ex2_approx(-ub);
-        a.a2 = fmaf(ea, ga, fmaf(eb, gb, a.a2));
-        a.a4p = fmaf(pea, ga, fmaf(peb, gb, a.a4p));
-        a.a6u = fmaf(ea * ua, ga, fmaf(eb * ub, gb, a.a6u));
-    }
-}
+// Phase-2 building blocks.  Per (peak, tile) with t'_p = t0 + p step and e_p the residual:
+//   a1 = sum e L, a5 = sum e L^2, a3t = sum e L^2 t'       (Lorentz part, every in-window point)
+//   a2 = sum e g, a4t = sum e g t', a6t = sum e g t'^2     (Gaussian part, core points only; g = 2^(-u) = G/2,
+//                                                           u = 1 + t'^2)
+struct Acc6 { float a1, a2, a3t, a4t, a5, a6t; };
 
 template <int Q>
-__device__ __forceinline__ void bwd_quad_generic(const PeakGeo& g, float t0, float step, f32x2 eX, f32x2 eY, f32x2 peX,
-                                                 f32x2 peY, Acc6& a) {
+__device__ __forceinline__ void bwd_quad_generic(const PeakGeo& g, float t0, float step, f32x2 eX, f32x2 eY,
+                                                 Acc6& a) {
     const int lo = max(g.p_lo, 4 * Q), hi = min(g.p_hi, 4 * Q + 3);
     if (lo > hi) return;
     const unsigned span = static_cast<unsigned>(hi - lo);
-    float u[4], ev[4], qv[4];
+    float u[4], ev[4], qv[4], tv[4];
     unpack2(eX, ev[0], ev[2]);
     unpack2(eY, ev[1], ev[3]);
-    unpack2(peX, qv[0], qv[2]);
-    unpack2(peY, qv[1], qv[3]);
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
         const float t = fmaf(static_cast<float>(4 * Q + i), step, t0);
+        tv[i] = t;
         u[i] = fmaf(t, t, 1.0f);
         const bool in = static_cast<unsigned>(4 * Q + i - lo) <= span;   // out-of-window points: zero residual
         ev[i] = in ? ev[i] : 0.0f;
-        qv[i] = in ? qv[i] : 0.0f;
+        qv[i] = ev[i] * t;
     }
     const float r01 = rcp_approx(u[0] * u[1]), r23 = rcp_approx(u[2] * u[3]);
     const float L[4] = {r01 * u[1], r01 * u[0], r23 * u[3], r23 * u[2]};
@@ -534,15 +516,15 @@ __device__ __forceinline__ void bwd_quad_generic(const PeakGeo& g, float t0, flo
         const float L2 = L[i] * L[i];
         a.a1 = fmaf(ev[i], L[i], a.a1);
         a.a5 = fmaf(ev[i], L2, a.a5);
-        a.a3p = fmaf(qv[i], L2, a.a3p);
+        a.a3t = fmaf(qv[i], L2, a.a3t);
     }
     if (g.c_hi >= 4 * Q && g.c_lo <= 4 * Q + 3) {
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
             const float gg = ex2_approx(-u[i]);
             a.a2 = fmaf(ev[i], gg, a.a2);
-            a.a4p = fmaf(qv[i], gg, a.a4p);
-            a.a6u = fmaf(ev[i] * u[i], gg, a.a6u);
+            a.a4t = fmaf(qv[i], gg, a.a4t);
+            a.a6t = fmaf(qv[i] * tv[i], gg, a.a6t);
         }
     }
 }
@@ -818,13 +800,11 @@ __device__ __forceinline__ void tile_phase2(const Dev& d, const Src& src, const 
                                             int pd_row) {
     if (rng.x >= rng.y) return;
     const int lane = threadIdx.x & 31;
-    f32x2 e2[kPT / 2], pe2[kPT / 2];     // packed like the accumulators of phase 1; pe_p = p e_p
+    f32x2 e2[kPT / 2];                   // packed like the accumulators of phase 1
 #pragma unroll
     for (int Q = 0; Q < kPT / 4; ++Q) {
         e2[2 * Q] = pack2(e[4 * Q], e[4 * Q + 2]);
         e2[2 * Q + 1] = pack2(e[4 * Q + 1], e[4 * Q + 3]);
-        pe2[2 * Q] = pack2(static_cast<float>(4 * Q) * e[4 * Q], static_cast<float>(4 * Q + 2) * e[4 * Q + 2]);
-        pe2[2 * Q + 1] = pack2(static_cast<float>(4 * Q + 1) * e[4 * Q + 1], static_cast<float>(4 * Q + 3) * e[4 * Q + 3]);
     }
     const float4* __restrict__ epsg = d.eps + static_cast<size_t>(c.g) * d.K * 32 + lane;
     const float* __restrict__ rrg = d.rr + static_cast<size_t>(c.g) * d.K * 32 + lane;
@@ -855,32 +835,32 @@ __device__ __forceinline__ void tile_phase2(const Dev& d, const Src& src, const 
             const bool core = static_cast<unsigned>(pk.dj + ngc) <= core_span;
             if ((pk.full & 1) && !core) {
                 Acc6x2 a2 = {0ull, 0ull, 0ull, 0ull, 0ull, 0ull};
-                bwd_tile2<false>(t0, step, e2, pe2, a2);
-                const float a1 = hsum2(a2.a1), a5 = hsum2(a2.a5), a3p = hsum2(a2.a3p);
+                bwd_tile2<false>(t0, step, e2, a2);
+                const float a1 = hsum2(a2.a1), a5 = hsum2(a2.a5);
+                B3 = fmaf(pk.inten, hsum2(a2.a3t), B3);
                 B1 = fmaf(pk.inten, a1, B1);
-                B3 = fmaf(pk.inten, fmaf(t0, a5, step * a3p), B3);
                 B5 = fmaf(pk.inten, a5, B5);
             } else {
                 Acc6 a = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
                 if (pk.full & 1) {
                     Acc6x2 a2 = {0ull, 0ull, 0ull, 0ull, 0ull, 0ull};
-                    bwd_tile2<true>(t0, step, e2, pe2, a2);
-                    a.a1 = hsum2(a2.a1); a.a2 = hsum2(a2.a2); a.a3p = hsum2(a2.a3p);
-                    a.a4p = hsum2(a2.a4p); a.a5 = hsum2(a2.a5); a.a6u = hsum2(a2.a6u);
+                    bwd_tile2<true>(t0, step, e2, a2);
+                    a.a1 = hsum2(a2.a1); a.a2 = hsum2(a2.a2); a.a3t = hsum2(a2.a3t);
+                    a.a4t = hsum2(a2.a4t); a.a5 = hsum2(a2.a5); a.a6t = hsum2(a2.a6t);
                 } else {
                     const PeakGeo geo = edge_geo(pk.dj, ngc, pk.full >> 1, c.plim);
-                    bwd_quad_generic<0>(geo, t0, step, e2[0], e2[1], pe2[0], pe2[1], a);
-                    bwd_quad_generic<1>(geo, t0, step, e2[2], e2[3], pe2[2], pe2[3], a);
-                    bwd_quad_generic<2>(geo, t0, step, e2[4], e2[5], pe2[4], pe2[5], a);
-                    bwd_quad_generic<3>(geo, t0, step, e2[6], e2[7], pe2[6], pe2[7], a);
+                    bwd_quad_generic<0>(geo, t0, step, e2[0], e2[1], a);
+                    bwd_quad_generic<1>(geo, t0, step, e2[2], e2[3], a);
+                    bwd_quad_generic<2>(geo, t0, step, e2[4], e2[5], a);
+                    bwd_quad_generic<3>(geo, t0, step, e2[6], e2[7], a);
                 }
                 const float i2 = 2.0f * pk.inten;           // g = G/2 in the Gaussian sums
                 B1 = fmaf(pk.inten, a.a1, B1);
                 B2 = fmaf(i2, a.a2, B2);
-                B3 = fmaf(pk.inten, fmaf(t0, a.a5, step * a.a3p), B3);
-                B4 = fmaf(i2, fmaf(t0, a.a2, step * a.a4p), B4);
                 B5 = fmaf(pk.inten, a.a5, B5);
-                B6 = fmaf(i2, a.a6u - a.a2, B6);
+                B3 = fmaf(pk.inten, a.a3t, B3);
+                B4 = fmaf(i2, a.a4t, B4);
+                B6 = fmaf(i2, a.a6t, B6);
             }
         }
         // chain rule for the likelihood part (per draw), then sum over the 32 draws of the group
@@ -941,7 +921,7 @@ __device__ __forceinline__ void fwd_quad_asym(const PeakGeo& g, const float (&o)
     accY = pack2(a[1], a[3]);
 }
 
-// a1 = sum e L, a5 = sum e L^2, a2 = sum e g, a6u = sum e u g (g = 2^-u = G/2, u = 1 + t''^2) as in Acc6;
+// a1 = sum e L, a5 = sum e L^2, a2 = sum e g as in Acc6, a6u = sum e u g (g = 2^-u = G/2, u = 1 + t''^2);
 // a3m = sum e L^2 tm, a4m = sum e g tm with tm = t' + mx (ia^2 - 1) (the mu chain); h1 = sum e mx^2 L^2, h2 = sum e mx^2 g.
 struct Acc8 { float a1, a2, a5, a6u, a3m, a4m, h1, h2; };
 
@@ -1057,13 +1037,11 @@ __device__ __forceinline__ void tile_phase2_asym(const Dev& d, const Src& src, c
                                                  int pd_row) {
     if (rng.x >= rng.y) return;
     const int lane = threadIdx.x & 31;
-    f32x2 e2[kPT / 2], pe2[kPT / 2];
+    f32x2 e2[kPT / 2];
 #pragma unroll
     for (int Q = 0; Q < kPT / 4; ++Q) {
         e2[2 * Q] = pack2(e[4 * Q], e[4 * Q + 2]);
         e2[2 * Q + 1] = pack2(e[4 * Q + 1], e[4 * Q + 3]);
-        pe2[2 * Q] = pack2(static_cast<float>(4 * Q) * e[4 * Q], static_cast<float>(4 * Q + 2) * e[4 * Q + 2]);
-        pe2[2 * Q + 1] = pack2(static_cast<float>(4 * Q + 1) * e[4 * Q + 1], static_cast<float>(4 * Q + 3) * e[4 * Q + 3]);
     }
     const size_t gk = static_cast<size_t>(c.g) * d.K * 32 + lane;
     float off[kPT];
@@ -1096,9 +1074,8 @@ __device__ __forceinline__ void tile_phase2_asym(const Dev& d, const Src& src, c
                 const bool high = pk.dj < 0;
                 if (high) { t0 *= ia; step *= ia; }
                 Acc6x2 a2 = {0ull, 0ull, 0ull, 0ull, 0ull, 0ull};
-                bwd_tile2<false>(t0, step, e2, pe2, a2);
-                const float a1 = hsum2(a2.a1), a5 = hsum2(a2.a5), a3p = hsum2(a2.a3p);
-                const float m3 = fmaf(t0, a5, step * a3p);  // sum e L^2 t''
+                bwd_tile2<false>(t0, step, e2, a2);
+                const float a1 = hsum2(a2.a1), a5 = hsum2(a2.a5), m3 = hsum2(a2.a3t);   // m3 = sum e L^2 t''
                 B1 = fmaf(wI, a1, B1);
                 B5 = fmaf(wI, a5, B5);
                 B3 = fmaf(wI * inv_s * (high ? ia : 1.0f), m3, B3);
