@@ -779,6 +779,38 @@ __device__ __forceinline__ float tile_residual(const Dev& d, const TileCtx& c, c
     return ss;
 }
 
+// a-4 on one quad (points 4 Q .. 4 Q + 3) of the tile: the PS = 4 warps of a CTA take one quad each.
+__device__ __forceinline__ float quad_residual(const Dev& d, const TileCtx& c, int Q, const float4 acc, float4& ev) {
+    const PatConst pc = d.pat[c.pat];
+    const float* __restrict__ yb = d.yb + static_cast<size_t>(c.pat) * d.N + c.i0 + 4 * Q;
+    const float a[4] = {acc.x, acc.y, acc.z, acc.w};
+    float e[4];
+    float ss = 0.0f;
+    if (d.likelihood == 0) {
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            float r = 0.0f;
+            if (4 * Q + i <= c.plim) r = yb[i] - a[i];
+            const float z = r * pc.inv_sn;
+            ss = fmaf(z, z, ss);
+            e[i] = r * pc.inv_sn2;
+        }
+    } else {
+        const float* __restrict__ bgp = d.bg + static_cast<size_t>(c.pat) * d.N + c.i0 + 4 * Q;
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            e[i] = 0.0f;
+            if (4 * Q + i <= c.plim) {
+                const float2 ed = poisson_point(yb[i], bgp[i], a[i]);
+                e[i] = ed.x;
+                ss += ed.y;
+            }
+        }
+    }
+    ev = make_float4(e[0], e[1], e[2], e[3]);
+    return ss;
+}
+
 // debug read-back of the profile f = S_F + B of the first n_dbg sample-instances (parity tests)
 __device__ __forceinline__ void tile_debug_profile(const Dev& d, const TileCtx& c, const float (&acc)[kPT],
                                                    float* __restrict__ f_dbg, long long n_dbg) {
@@ -1154,8 +1186,9 @@ __global__ void __launch_bounds__(32 * TW * PS, tile_ctas_per_sm(TW, PS))
 elbo_tile_kernel(const Dev d, float* __restrict__ f_dbg, long long n_dbg) {
     static_assert(!STAGE || TW == 1, "staging holds one tile list per CTA");
     __shared__ float4 e_s[TW][kPT / 4][32];
-    __shared__ float ss_s[TW][32];
-    __shared__ float acc_s[PS > 1 ? (PS - 1) * TW * kPT : 1][32];
+    constexpr bool kQuadShare = (PS == 4 && TW == 1);       // residual formed by four warps, one quad each
+    __shared__ float ss_s[kQuadShare ? 4 : TW][32];
+    __shared__ __align__(16) float acc_s[PS > 1 ? (kQuadShare ? PS : PS - 1) * TW * kPT : 1][32];
     __shared__ __align__(128) PeakRec rec_s[STAGE ? kStageRec : 1];
     __shared__ __align__(16) int4 run_s[STAGE ? kStageRun : 1];
     __shared__ __align__(8) unsigned long long mbar_s;
@@ -1212,6 +1245,41 @@ elbo_tile_kernel(const Dev d, float* __restrict__ f_dbg, long long n_dbg) {
     if constexpr (MODEL == 1) tile_phase1_asym(d, src, c, rng, acc);
     else tile_phase1(d, src, c, rng, acc);
 
+    if constexpr (kQuadShare) {
+        // every share leaves its partial profile in shared memory as one float4 per quad; warp q then sums quad q over the
+        // shares in share order, forms its residual and its part of ll: a quarter of the serial section per warp
+        float4* __restrict__ aq = reinterpret_cast<float4*>(&acc_s[0][0]);     // [share][quad][lane]
+#pragma unroll
+        for (int v = 0; v < kPT / 4; ++v)
+            aq[(ps * 4 + v) * 32 + lane] = make_float4(acc[4 * v], acc[4 * v + 1], acc[4 * v + 2], acc[4 * v + 3]);
+        __syncthreads();
+        float4 a = aq[ps * 32 + lane];
+#pragma unroll
+        for (int q = 1; q < PS; ++q) {
+            const float4 b = aq[(q * 4 + ps) * 32 + lane];
+            a.x += b.x; a.y += b.y; a.z += b.z; a.w += b.w;
+        }
+        float4 ev;
+        const float ss = quad_residual(d, c, ps, a, ev);
+        if (BWD) e_s[0][ps][lane] = ev;
+        ss_s[ps][lane] = ss;
+        if (f_dbg) {
+            const int inst = c.g / d.gpi;
+            const int sd = (c.g - inst * d.gpi) * 32 + lane;
+            const long long t = static_cast<long long>(inst) * d.S + sd - d.dbg_first;
+            if (sd < d.S && t >= 0 && t < n_dbg) {
+                const float* __restrict__ bg = d.bg + static_cast<size_t>(c.pat) * d.N + c.i0 + 4 * ps;
+                const float av[4] = {a.x, a.y, a.z, a.w};
+#pragma unroll
+                for (int i = 0; i < 4; ++i)
+                    if (4 * ps + i <= c.plim) f_dbg[t * d.N + c.i0 + 4 * ps + i] = av[i] + bg[i];
+            }
+        }
+        __syncthreads();
+        if (w == 0)
+            d.llpart[(static_cast<size_t>(c.g) * d.n_seg + seg) * 32 + lane] =
+                ((ss_s[0][lane] + ss_s[1][lane]) + ss_s[2][lane]) + ss_s[3][lane];
+    } else {
     if (PS > 1) {   // sum the PS partial profiles of the tile: shares 1.. in order onto share 0
         if (ps > 0) {
 #pragma unroll
@@ -1242,6 +1310,7 @@ elbo_tile_kernel(const Dev d, float* __restrict__ f_dbg, long long n_dbg) {
 #pragma unroll
         for (int v = 1; v < TW; ++v) ss += ss_s[v][lane];
         d.llpart[(static_cast<size_t>(c.g) * d.n_seg + seg) * 32 + lane] = ss;
+    }
     }
     tl_stamp(d.tl, tl_row, 1);
     if (!BWD) return;
