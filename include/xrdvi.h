@@ -225,6 +225,26 @@ int xrdvi_posterior_summary(xrdvi* h, double* summary);
 int xrdvi_logjoint_grad(xrdvi* h, const float* zeta, int64_t n, int32_t pattern, double* ll, double* lpj,
                         float* grad);
 
+/* Model profile and log-likelihood of chosen draws WITHOUT any allocation and without caller scratch, for callers that
+ * cannot call cudaMalloc (tight serving loops, harnesses that forbid it, code around a CUDA graph capture): draw +
+ * forward pass (a-1 .. a-4: eq.(3)-(8) PAPER.md:206-232 profile, residual, ll) at (var_params or the internal state
+ * when NULL, S, seed, iteration), exactly as the fit evaluates them.  The profile rows pass through a file-scope
+ * `static __device__` array of the library: 1 048 576 floats = 4 MiB on every GPU that loads the library, held until the
+ * process exits; its device address is resolved once per device in xrdvi_create (cudaGetSymbolAddress).
+ *  var_params  host float [P][R][2][K][C] (C = xrdvi_latent_classes) or NULL;  1 <= S <= S_max
+ *  first, n    the sample-instances first .. first + n - 1 in (pattern, restart, s) order, 0 <= first, first + n <= P R S
+ *  f           host float [n][N]: S_F + B of each row (owned by the caller), or NULL
+ *  ll          host double [n]: log-likelihood of each row, or NULL
+ * Limit: n * N <= 1 048 576 when f is wanted, else XRDVI_E_WORKSPACE_TOO_SMALL (message states both numbers; ask for fewer
+ * rows per call).  XRDVI_E_INVALID_ARG for S / first / n out of range; XRDVI_E_CUDA if the array's address could not be
+ * resolved at create.  Calls no cudaMalloc / cudaFree / allocating routine, host or device.  Synchronous on the handle's
+ * stream; the variational state is not modified (the per-step draw buffers are overwritten, as by xrdvi_elbo_grad).
+ * EVERY call on a GPU, from any handle, shares the one array, which keeps the last call's rows (each call zeroes the
+ * part it uses first): calls whose GPU work overlaps (handles on different streams, several host threads) RACE on it --
+ * serialise them.                                                                                               */
+int xrdvi_profile_static(xrdvi* h, const float* var_params, int32_t S, uint64_t seed, uint64_t iteration,
+                         int64_t first, int64_t n, float* f, double* ll);
+
 const char* xrdvi_last_error(void);
 
 #ifdef __cplusplus

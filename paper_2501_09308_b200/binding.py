@@ -19,7 +19,8 @@ EXPORTS = (            # include/xrdvi.h: the product boundary
     "xrdvi_latent_classes", "xrdvi_window_halfwidth", "xrdvi_set_phase_windows", "xrdvi_get_phase_windows", "xrdvi_adapt_windows",
     "xrdvi_fit_adaptive", "xrdvi_reset_state", "xrdvi_reset_state_restart", "xrdvi_get_state", "xrdvi_set_state",
     "xrdvi_get_optimizer_state", "xrdvi_set_optimizer_state", "xrdvi_elbo_grad",
-    "xrdvi_fit", "xrdvi_inclusion", "xrdvi_posterior_summary", "xrdvi_logjoint_grad", "xrdvi_last_error",
+    "xrdvi_fit", "xrdvi_inclusion", "xrdvi_posterior_summary", "xrdvi_logjoint_grad", "xrdvi_profile_static",
+    "xrdvi_last_error",
 )
 DEBUG_EXPORTS = (      # include/xrdvi_debug.h: read-backs for the parity tests, timing for bench.py and profiles/
     "xrdvi_debug_profile", "xrdvi_debug_draws", "xrdvi_time_kernels", "xrdvi_bench_steps", "xrdvi_debug_timeline",
@@ -89,6 +90,7 @@ def load_library():
     L.xrdvi_inclusion.argtypes = [vp, dp, dp]
     L.xrdvi_posterior_summary.argtypes = [vp, dp]
     L.xrdvi_logjoint_grad.argtypes = [vp, fp, C.c_int64, C.c_int32, dp, dp, fp]
+    L.xrdvi_profile_static.argtypes = [vp, fp, C.c_int32, C.c_uint64, C.c_uint64, C.c_int64, C.c_int64, fp, dp]
     L.xrdvi_debug_profile.argtypes = [vp, fp, C.c_int32, C.c_uint64, C.c_uint64, C.c_int64, C.c_int64, fp, dp, vp,
                                       C.c_size_t]
     L.xrdvi_debug_draws.argtypes = [vp, C.c_int32, C.c_uint64, C.c_uint64, C.c_int64, fp, C.POINTER(C.c_uint32),
@@ -299,6 +301,19 @@ class Xrdvi:
         out = np.empty((self.P, self.R, self.K, self.C, 5), dtype=np.float64)
         _check(load_library().xrdvi_posterior_summary(self._h, _d(out)))
         return out
+
+    STATIC_SCRATCH_FLOATS = 1 << 20     # xrdvi_profile_static: n * N limit (4 MiB static device array)
+
+    def profile_static(self, n, state=None, S=None, seed=0, iteration=0, want_f=True, first=0):
+        """xrdvi_profile_static: profile rows f [n][N] and ll [n] of the draws first .. first + n - 1; allocates nothing
+        in the library and needs no scratch (n * N <= STATIC_SCRATCH_FLOATS)."""
+        S = self.S_max if S is None else int(S)
+        st = None if state is None else np.ascontiguousarray(state, dtype=np.float32).reshape(self._state_shape())
+        f = np.empty((int(n), self.N), dtype=np.float32) if want_f else None
+        ll = np.empty(int(n), dtype=np.float64)
+        _check(load_library().xrdvi_profile_static(self._h, _f(st), S, int(seed), int(iteration), int(first), int(n),
+                                                   _f(f), _d(ll)))
+        return f, ll
 
     # ---- debug / measurement (include/xrdvi_debug.h) -----------------------------
     def _scratch(self, nbytes):

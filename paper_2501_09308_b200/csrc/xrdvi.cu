@@ -11,11 +11,19 @@
 #include <cstdlib>
 #include <cstring>
 #include <limits>
+#include <mutex>
 #include <numeric>
 #include <string>
 #include <vector>
 
 using namespace xrdvi_dev;
+
+// Scratch of xrdvi_profile_static (include/xrdvi.h), the one entry point that needs no caller scratch: profile rows
+// float [n][N] between the forward kernel and the copy to the caller.  kStaticScratchFloats floats = 4 MiB, held by every
+// GPU that loads this library until the process exits.  In host code this NAME is a host-side stand-in, not a device
+// address: static_scratch_address() below resolves it once per device, and only that pointer is given to a kernel.
+constexpr size_t kStaticScratchFloats = size_t(1) << 20;
+static __device__ __align__(256) float g_static_scratch[kStaticScratchFloats];
 
 namespace {
 
@@ -34,6 +42,29 @@ int fail(int code, const std::string& msg) {
     } while (0)
 
 size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
+
+// Device address of g_static_scratch on `device`, which must be the CURRENT device (every device that loads the module has
+// its own copy of the array).  Resolved once per device, at set-up (xrdvi_create), cached with its return code.
+constexpr int kMaxDevices = 64;
+struct StaticScratch { float* ptr = nullptr; cudaError_t err = cudaSuccess; bool done = false; };
+StaticScratch g_static[kMaxDevices];
+std::mutex g_static_mu;
+
+cudaError_t static_scratch_address(int device, float** ptr) {
+    *ptr = nullptr;
+    if (device < 0 || device >= kMaxDevices) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(g_static_mu);
+    StaticScratch& e = g_static[device];
+    if (!e.done) {
+        void* p = nullptr;
+        e.err = cudaGetSymbolAddress(&p, g_static_scratch);
+        if (e.err != cudaSuccess) { p = nullptr; (void)cudaGetLastError(); }   // reported by xrdvi_profile_static, not here
+        e.ptr = static_cast<float*>(p);
+        e.done = true;
+    }
+    *ptr = e.ptr;
+    return e.err;
+}
 
 
 struct Plan {   // workspace carve; identical arithmetic in workspace_bytes and create
@@ -356,6 +387,8 @@ struct xrdvi {
     long long step_host = 0;   // mirror of ctl.step
     long long adam_t0 = 0;     // mirror of ctl.adam_t0 (step count at which the Adam moments were last zeroed)
     bool own_stream = false;   // the stream was created by xrdvi_create (caller passed 0)
+    float* static_scratch = nullptr;               // device address of g_static_scratch on h->device (set at create)
+    cudaError_t static_scratch_err = cudaSuccess;  // what cudaGetSymbolAddress returned there
     // CUDA Graph of one optimisation step, keyed by S
     cudaGraphExec_t graph_exec = nullptr;    // one step
     cudaGraphExec_t graph_execU = nullptr;   // kUnroll steps: programmatic launches also across step boundaries
@@ -959,6 +992,8 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
     int rc = install_tables(h, tabs, nck0, true);
     if (rc == XRDVI_OK) rc = xrdvi_reset_state(h, 0);
     if (rc != XRDVI_OK) { xrdvi_destroy(h); return rc; }
+    // set-up of xrdvi_profile_static: `device` is current here; a failure only disables that entry point
+    h->static_scratch_err = static_scratch_address(device, &h->static_scratch);
     *out = h;
     return XRDVI_OK;
 }
@@ -1250,6 +1285,64 @@ int xrdvi_debug_profile(xrdvi* h, const float* var_params, int32_t S, uint64_t s
         const int gpi32 = h->dev.gpi * 32;
         for (long long t = 0; t < n; ++t) ll[t] = llh[static_cast<size_t>((first + t) / S) * gpi32 + ((first + t) % S)];
     }
+    return XRDVI_OK;
+}
+
+// The same evaluation as xrdvi_debug_profile with the caller's scratch replaced by g_static_scratch: no device or host
+// allocation on this path (no std::vector either), so it may be called where cudaMalloc is forbidden.
+int xrdvi_profile_static(xrdvi* h, const float* var_params, int32_t S, uint64_t seed, uint64_t iteration,
+                         int64_t first, int64_t n, float* f, double* ll) {
+    int rc = check_S(h, S);
+    if (rc) return rc;
+    const long long T = static_cast<long long>(h->plan.PR) * S;
+    if (first < 0 || n < 0 || first + n > T) return fail(XRDVI_E_INVALID_ARG, "profile_static: first / n out of range");
+    const size_t want = f ? static_cast<size_t>(n) * static_cast<size_t>(h->N) : 0;
+    if (want > kStaticScratchFloats)
+        return fail(XRDVI_E_WORKSPACE_TOO_SMALL,
+                    "profile_static: n * N = " + std::to_string(want) + " floats exceed the static scratch of " +
+                        std::to_string(kStaticScratchFloats) + " floats (4 MiB); ask for fewer rows per call");
+    if (want && !h->static_scratch)
+        return fail(XRDVI_E_CUDA, std::string("profile_static: cudaGetSymbolAddress failed at create: ") +
+                                      cudaGetErrorString(h->static_scratch_err));
+    CU(cudaSetDevice(h->device));
+    const float* var = h->dev.var;
+    if (var_params) {   // external [PR][2][K][C] -> device [PR][2][K][4] (+ [PR][2][K] for alpha, R30), strided copies
+        float* tmp = reinterpret_cast<float*>(h->ws + h->plan.o_vartmp);
+        const size_t rows = static_cast<size_t>(h->plan.PR) * 2 * h->K;
+        if (!h->hyp.asymmetry) {
+            CU(cudaMemcpyAsync(tmp, var_params, sizeof(float) * rows * 4, cudaMemcpyHostToDevice, h->stream));
+        } else {
+            CU(cudaMemcpy2DAsync(tmp, 4 * sizeof(float), var_params, 5 * sizeof(float), 4 * sizeof(float), rows,
+                                 cudaMemcpyHostToDevice, h->stream));
+            CU(cudaMemcpy2DAsync(tmp + rows * 4, sizeof(float), var_params + 4, 5 * sizeof(float), sizeof(float), rows,
+                                 cudaMemcpyHostToDevice, h->stream));
+        }
+        var = tmp;
+    }
+    rc = set_S(h, S);
+    if (rc) return rc;
+    rc = write_ctl(h, seed, h->step_host, h->step_host, static_cast<long long>(iteration & 0xFFFFFFFFull));   // synchronises
+    if (rc) return rc;
+    float* f_dev = want ? h->static_scratch : nullptr;
+    // every call shares the array and finds the previous call's rows in it: start from zero, so that a point the kernel
+    // did not write can never be read as this call's result
+    if (f_dev) CU(cudaMemsetAsync(f_dev, 0, sizeof(float) * want, h->stream));
+    h->dev.dbg_first = first;
+    rc = enqueue_eval(h, var, f_dev, f_dev ? n : 0, true);
+    h->dev.dbg_first = 0;
+    if (rc) return rc;
+    cudaError_t e = cudaSuccess;
+    if (f_dev) e = cudaMemcpyAsync(f, f_dev, sizeof(float) * want, cudaMemcpyDeviceToHost, h->stream);
+    if (ll && n > 0) {   // ll_t is [PR][gpi * 32]: one contiguous piece per instance the rows touch
+        const int gpi32 = h->dev.gpi * 32;
+        for (long long inst = first / S; inst <= (first + n - 1) / S && e == cudaSuccess; ++inst) {
+            const long long lo = std::max<long long>(first, inst * S), hi = std::min<long long>(first + n, (inst + 1) * S);
+            e = cudaMemcpyAsync(ll + (lo - first), h->dev.ll_t + static_cast<size_t>(inst) * gpi32 + (lo - inst * S),
+                                sizeof(double) * static_cast<size_t>(hi - lo), cudaMemcpyDeviceToHost, h->stream);
+        }
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
+    if (e != cudaSuccess) return fail(XRDVI_E_CUDA, std::string("profile_static: ") + cudaGetErrorString(e));
     return XRDVI_OK;
 }
 
