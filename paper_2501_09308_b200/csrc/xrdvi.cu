@@ -73,7 +73,7 @@ struct Plan {   // workspace carve; identical arithmetic in workspace_bytes and 
     long long M, n_c, tile_cap, slots_cap;
     size_t total;
     size_t o_yb, o_bg, o_pkt, o_runs, o_srng, o_sord, o_sofs, o_pat, o_area, o_mh0;
-    size_t o_var, o_vartmp, o_mom1, o_mom2, o_grad, o_elbo, o_elbok, o_llt, o_trace, o_ctl;
+    size_t o_var, o_vartmp, o_mom1, o_mom2, o_grad, o_elbo, o_elbok, o_llt, o_llg, o_trace, o_ctl;
     size_t o_lat, o_eps, o_rr, o_ng, o_llpart, o_part8, o_dbg;
     size_t o_pd, o_lpk, o_zeta, o_gradz, o_lls, o_partial, o_tcnt, o_summ;
     size_t o_trng, o_ia, o_epsa, o_parta, o_pksec, o_secmax, o_tileoff, o_pkbase;
@@ -161,6 +161,7 @@ bool make_plan(int64_t N, int32_t K, int64_t M, int32_t S_max, double step, cons
     p.o_elbo = take(sizeof(double) * p.PR);
     p.o_elbok = take(sizeof(double) * p.PR * (K + 1));
     p.o_llt = take(sizeof(double) * p.PR * p.S_pad);
+    p.o_llg = take(sizeof(double) * p.G_max);
     p.o_trace = take(sizeof(double) * kTraceCap * p.PR);
     p.o_ctl = take(sizeof(Ctl));
     p.o_lat = take(sizeof(float4) * gk32);
@@ -393,15 +394,22 @@ struct xrdvi {
     cudaGraphExec_t graph_exec = nullptr;    // one step
     cudaGraphExec_t graph_execU = nullptr;   // kUnroll steps: programmatic launches also across step boundaries
     int graph_S = -1;
+    int max_phase_slots = 0;   // output slots of the widest phase at create
     cudaEvent_t ev[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
 };
 
 namespace {
 
+// Dynamic shared memory of update_draw_kernel: room for the slot rows (32 bytes each) of the widest phase over all
+// groups of an instance, if every draw of an instance has a thread of its own and the rows fit; else 0 (its long path).
+constexpr int kUpdSmemCap = 96 * 1024;
+
 int set_S(xrdvi* h, int S) {
     h->dev.S = S;
     h->dev.gpi = (S + 31) / 32;
     h->dev.G = h->plan.PR * h->dev.gpi;
+    const long long rows = static_cast<long long>(h->max_phase_slots) * h->dev.gpi * 32;
+    h->dev.upd_smem = (h->dev.gpi * 32 <= kUpdThreads && rows <= kUpdSmemCap) ? static_cast<int>(rows) : 0;
     return XRDVI_OK;
 }
 
@@ -428,6 +436,10 @@ int install_tables(xrdvi* h, const Tables& T, const std::vector<long long>& nck,
     if (h->hyp.width_sec)
         CU(cudaMemcpyAsync(w + pl.o_pksec, T.pk_sec.data(), sizeof(float) * T.pk_sec.size(), cudaMemcpyHostToDevice, st));
     if (at_create) {
+        // widest phase in output slots (per-phase windows only ever shrink it): sizes update_draw_kernel's staging buffer
+        h->max_phase_slots = 0;
+        for (size_t k = 0; k + 1 < T.slot_ofs.size(); ++k)
+            h->max_phase_slots = std::max(h->max_phase_slots, T.slot_ofs[k + 1] - T.slot_ofs[k]);
         d.n_slots = std::max(T.n_slots, 1);
         d.split = pl.split;
         // bulk-copy staging (TW = 1) needs every tile list to fit the shared-memory buffers; decided once (the per-phase
@@ -450,11 +462,11 @@ int install_tables(xrdvi* h, const Tables& T, const std::vector<long long>& nck,
 // Launch with the programmatic-stream-serialization attribute (the kernel may begin while its predecessor drains; it
 // calls griddep_wait() before touching the predecessor's data).  pdl = false: a plain launch.
 template <typename... KArgs, typename... Args>
-void launch_k(void (*kernel)(KArgs...), dim3 grid, dim3 block, cudaStream_t st, bool pdl, Args... args) {
+void launch_k(void (*kernel)(KArgs...), dim3 grid, dim3 block, cudaStream_t st, bool pdl, size_t smem, Args... args) {
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = grid;
     cfg.blockDim = block;
-    cfg.dynamicSmemBytes = 0;
+    cfg.dynamicSmemBytes = smem;
     cfg.stream = st;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
@@ -479,19 +491,19 @@ void launch_tile_shape(const Dev& d, dim3 grid, cudaStream_t st, bool pdl, float
     const dim3 block(32 * TW * PS);
     if constexpr (TW == 1) {
         if (d.model) {
-            if (d.stage) launch_k(elbo_tile_kernel<1, PS, BWD, true, 1>, grid, block, st, pdl, d, f_dbg, n_dbg);
-            else launch_k(elbo_tile_kernel<1, PS, BWD, false, 1>, grid, block, st, pdl, d, f_dbg, n_dbg);
+            if (d.stage) launch_k(elbo_tile_kernel<1, PS, BWD, true, 1>, grid, block, st, pdl, size_t(0), d, f_dbg, n_dbg);
+            else launch_k(elbo_tile_kernel<1, PS, BWD, false, 1>, grid, block, st, pdl, size_t(0), d, f_dbg, n_dbg);
             return;
         }
-        if (d.stage) { launch_k(elbo_tile_kernel<1, PS, BWD, true, 0>, grid, block, st, pdl, d, f_dbg, n_dbg); return; }
+        if (d.stage) { launch_k(elbo_tile_kernel<1, PS, BWD, true, 0>, grid, block, st, pdl, size_t(0), d, f_dbg, n_dbg); return; }
     }
-    launch_k(elbo_tile_kernel<TW, PS, BWD, false, 0>, grid, block, st, pdl, d, f_dbg, n_dbg);
+    launch_k(elbo_tile_kernel<TW, PS, BWD, false, 0>, grid, block, st, pdl, size_t(0), d, f_dbg, n_dbg);
 }
 
 template <int PS, bool BWD>
 void launch_split_shape(const Dev& d, dim3 grid, cudaStream_t st, bool pdl, float* f_dbg, long long n_dbg) {
-    if (d.model) launch_k(elbo_split_kernel<PS, BWD, 1>, grid, dim3(32), st, pdl, d, f_dbg, n_dbg);
-    else launch_k(elbo_split_kernel<PS, BWD, 0>, grid, dim3(32), st, pdl, d, f_dbg, n_dbg);
+    if (d.model) launch_k(elbo_split_kernel<PS, BWD, 1>, grid, dim3(32), st, pdl, size_t(0), d, f_dbg, n_dbg);
+    else launch_k(elbo_split_kernel<PS, BWD, 0>, grid, dim3(32), st, pdl, size_t(0), d, f_dbg, n_dbg);
 }
 
 template <bool BWD>
@@ -543,7 +555,8 @@ int enqueue_step(xrdvi* h) {
     // both kernels may start while their predecessor drains (programmatic dependent launch); each waits with
     // griddep_wait() before it touches the predecessor's data
     launch_tile<true>(d, h->stream, nullptr, 0, pdl);                  // also finishes the previous step (ELBO, count)
-    launch_k(update_draw_kernel, dim3(d.K + 1, d.PR), dim3(kUpdThreads), h->stream, pdl, d, static_cast<const float*>(d.var), 1);
+    launch_k(update_draw_kernel, dim3(d.K + d.gpi, d.PR), dim3(kUpdThreads), h->stream, pdl, static_cast<size_t>(d.upd_smem), d,
+             static_cast<const float*>(d.var), 1);
     CU(cudaGetLastError());
     return XRDVI_OK;
 }
@@ -562,7 +575,7 @@ int enqueue_eval(xrdvi* h, const float* var, float* f_dbg, long long n_dbg, bool
     if (forward_only) launch_tile<false>(d, h->stream, f_dbg, n_dbg);
     else launch_tile<true>(d, h->stream, f_dbg, n_dbg);
     // forward_only leaves stale partials in part8: the gradient output of this launch is not used then
-    update_draw_kernel<<<dim3(d.K + 1, d.PR), kUpdThreads, 0, h->stream>>>(d, var, 0);
+    update_draw_kernel<<<dim3(d.K + d.gpi, d.PR), kUpdThreads, d.upd_smem, h->stream>>>(d, var, 0);
     CU(cudaGetLastError());
     return enqueue_finish(h);
 }
@@ -571,6 +584,7 @@ int write_ctl(xrdvi* h, uint64_t seed, long long step, long long trace_base, lon
     Ctl c{};
     c.seed = seed;
     c.step = step;
+    c.u_step = step;
     c.trace_base = trace_base;
     c.iteration_override = it_override;
     c.adam_t0 = h->adam_t0;
@@ -920,6 +934,7 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
     d.elbo = reinterpret_cast<double*>(w + pl.o_elbo);
     d.elbo_k = reinterpret_cast<double*>(w + pl.o_elbok);
     d.ll_t = reinterpret_cast<double*>(w + pl.o_llt);
+    d.ll_g = reinterpret_cast<double*>(w + pl.o_llg);
     d.trace = reinterpret_cast<double*>(w + pl.o_trace);
     d.ctl = reinterpret_cast<Ctl*>(w + pl.o_ctl);
     d.lat = reinterpret_cast<float4*>(w + pl.o_lat);
@@ -990,6 +1005,11 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
         return fail(XRDVI_E_CUDA, std::string("upload: ") + cudaGetErrorString(ce));
     }
     int rc = install_tables(h, tabs, nck0, true);
+    if (rc == XRDVI_OK) {      // the update kernel's staging buffer: up to kUpdSmemCap of dynamic shared memory, sized by set_S
+        set_S(h, S_max);
+        cudaError_t e = cudaFuncSetAttribute(update_draw_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kUpdSmemCap);
+        if (e != cudaSuccess) rc = fail(XRDVI_E_CUDA, std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e));
+    }
     if (rc == XRDVI_OK) rc = xrdvi_reset_state(h, 0);
     if (rc != XRDVI_OK) { xrdvi_destroy(h); return rc; }
     // set-up of xrdvi_profile_static: `device` is current here; a failure only disables that entry point
@@ -1468,7 +1488,7 @@ int xrdvi_time_kernels(xrdvi* h, int32_t S, uint64_t seed, int32_t reps, float* 
         CU(cudaEventRecord(h->ev[1], st));
         launch_tile<true>(d, st, nullptr, 0);
         CU(cudaEventRecord(h->ev[2], st));
-        update_draw_kernel<<<dim3(d.K + 1, d.PR), kUpdThreads, 0, st>>>(d, d.var, 0);
+        update_draw_kernel<<<dim3(d.K + d.gpi, d.PR), kUpdThreads, d.upd_smem, st>>>(d, d.var, 0);
         CU(cudaEventRecord(h->ev[3], st));
         launch_tile<false>(d, st, nullptr, 0);
         CU(cudaEventRecord(h->ev[4], st));
@@ -1512,7 +1532,7 @@ int xrdvi_debug_timeline(xrdvi* h, int32_t S, uint64_t seed, int64_t capacity, u
         d.tl = pass == 2 ? buf : nullptr;
         if (pass == 2) e = cudaMemsetAsync(buf, 0, sizeof(unsigned long long) * 4 * warps, st);
         launch_tile<true>(d, st, nullptr, 0);
-        update_draw_kernel<<<dim3(d.K + 1, d.PR), kUpdThreads, 0, st>>>(h->dev, h->dev.var, 0);
+        update_draw_kernel<<<dim3(d.K + d.gpi, d.PR), kUpdThreads, h->dev.upd_smem, st>>>(h->dev, h->dev.var, 0);
         if (e == cudaSuccess) e = cudaGetLastError();
     }
     if (e == cudaSuccess) e = cudaMemcpyAsync(rows, buf, sizeof(unsigned long long) * 4 * warps, cudaMemcpyDeviceToHost, st);

@@ -79,6 +79,8 @@ struct Ctl {       // device-resident control block (so that graph replays need 
     unsigned int ticket;           // next work item of elbo_split_kernel (re-armed by the launch's last CTA)
     unsigned int finished;         // CTAs of the current elbo_split_kernel launch that are done
     unsigned int pad;
+    long long u_step;              // `step` as the next update_draw_kernel will see it: kept by update_draw_kernel itself
+                                   // (and set with `step` by the host), so that it may be read before griddep_wait
 };
 
 struct Dev {
@@ -111,8 +113,9 @@ struct Dev {
     float* mom2;
     float* grad;              // [PR][2][K][4]
     double* elbo;             // [PR]
-    double* elbo_k;           // [PR][K+1]  per-phase ELBO terms; [K] = mean log-likelihood
+    double* elbo_k;           // [PR][K+1]  per-phase ELBO terms ([K] unused)
     double* ll_t;             // [PR][S_pad]
+    double* ll_g;             // [G] sum of ll_t over the 32 draws of a group
     double* trace;            // [kTraceCap][PR]
     Ctl* ctl;
     // per-iteration buffers
@@ -132,6 +135,7 @@ struct Dev {
     const int2* tile_rng;     // [n_tile + 1] (first run, first record) of every tile's lists
     int stage;                // 1: elbo_tile_kernel copies the tile's lists into shared memory (they fit: host check)
     int g_block;              // draw groups per dispatch chunk of elbo_tile_kernel (their latent records stay in L2)
+    int upd_smem;             // dynamic shared memory of update_draw_kernel launches (bytes; its short path stages slot rows there)
     // peak asymmetry and the sec width term (reading R30; hyper.asymmetry / hyper.width_sec).  asym = 1: a fifth latent
     // alpha_k per phase; every state array has a companion for it ([PR][2][K]: m_alpha, l_alpha)
     int asym, sec;
@@ -163,7 +167,9 @@ __device__ __forceinline__ float ex2_approx(float x) {
 // Programmatic dependent launch (sm_90+): a kernel launched with the programmatic-serialization attribute may start
 // before its predecessor in the stream has finished; griddep_wait() blocks until the predecessor has completed and
 // its writes are visible (a no-op for a normal launch), griddep_launch_dependents() lets the successor start
-// launching.  Everything that reads or overwrites data of the predecessor comes after griddep_wait().
+// launching.  Everything that reads or overwrites data of the predecessor comes after griddep_wait().  The tile kernels
+// call griddep_launch_dependents() AFTER their griddep_wait(): their successor, update_draw_kernel, may then read
+// before its own wait whatever the kernels before the tile kernel wrote (they have completed).
 __device__ __forceinline__ void griddep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 // Per-warp timeline stamps of the tile kernels (xrdvi_debug_timeline; d.tl == nullptr in every other launch, a
 // warp-uniform test on a kernel parameter).  Each stamp is stored at once, nothing stays live across the phases.
@@ -607,7 +613,9 @@ __device__ __forceinline__ void finish_step(const Dev& d) {
     const long long step = d.ctl->step;
     for (int inst = threadIdx.x; inst < d.PR; inst += blockDim.x) {
         const double* __restrict__ ek = d.elbo_k + static_cast<size_t>(inst) * (d.K + 1);
-        double el = ek[d.K];
+        double llsum = 0.0;                                    // groups in order
+        for (int gi = 0; gi < d.gpi; ++gi) llsum += d.ll_g[static_cast<size_t>(inst) * d.gpi + gi];
+        double el = llsum * (1.0 / static_cast<double>(d.S));
         for (int kk = 0; kk < d.K; ++kk) el += ek[kk];
         d.elbo[inst] = el;
         if (pending == 2u) {
@@ -1192,7 +1200,6 @@ elbo_tile_kernel(const Dev d, float* __restrict__ f_dbg, long long n_dbg) {
     __shared__ __align__(128) PeakRec rec_s[STAGE ? kStageRec : 1];
     __shared__ __align__(16) int4 run_s[STAGE ? kStageRun : 1];
     __shared__ __align__(8) unsigned long long mbar_s;
-    griddep_launch_dependents();
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const int tw = w % TW, ps = w / TW;
     // grid (G, n_seg), dispatched blockIdx.x fastest.  The dispatch order is cut into chunks of g_block draw groups; inside a
@@ -1234,6 +1241,9 @@ elbo_tile_kernel(const Dev d, float* __restrict__ f_dbg, long long n_dbg) {
         mbar_wait(smem_u32(&mbar_s), 0u);
     }
     griddep_wait();                                         // latents, control block: written by the predecessor
+    // Only now may the successor (update_draw_kernel) begin: whatever it reads BEFORE its own griddep_wait was written
+    // by the update_draw_kernel before this launch, which has completed once any CTA here is past the wait.
+    griddep_launch_dependents();
     if (blockIdx.x == gridDim.x - 1 && blockIdx.y == gridDim.y - 1) finish_step(d);   // previous step's ELBO / count
     const unsigned tl_row = lin * (TW * PS) + w;
     tl_stamp(d.tl, tl_row, 0);
@@ -1339,8 +1349,8 @@ elbo_tile_kernel(const Dev d, float* __restrict__ f_dbg, long long n_dbg) {
 template <int PS, bool BWD, int MODEL>
 __global__ void __launch_bounds__(32, XRDVI_TILE_WARPS_PER_SM) elbo_split_kernel(const Dev d, float* __restrict__ f_dbg, long long n_dbg) {
     const int lane = threadIdx.x;
-    griddep_launch_dependents();
     griddep_wait();
+    griddep_launch_dependents();                           // after the wait: see elbo_tile_kernel
     if (blockIdx.x == gridDim.x - 1) finish_step(d);       // previous step's ELBO / count
     const unsigned n_items = static_cast<unsigned>(d.n_tile) * PS * d.G;
     unsigned ticket = 0;
@@ -1446,68 +1456,213 @@ __device__ __forceinline__ void block_reduce(double (&v)[NV], double* smem /* [N
     __syncthreads();
 }
 
-// a-6 (prior part) + a-7 + a-8 + next a-1/a-2.  grid (K + 1, PR), block 256.
-//  blockIdx.x = k < K : reduce the part8 slots of phase k and the per-draw prior/Jacobian terms over the S
-//                       draws of instance blockIdx.y -> grad; Adam ascent on the 8 parameters of (inst, k);
-//                       draws + transform of the next step for (inst, k, all s)          (do_update)
-//  blockIdx.x = K     : log-likelihood per draw (sum of llpart over the segments) and its mean
+// a-6 (prior part) + a-7 + a-8 + next a-1/a-2.  grid (K + gpi, PR), block 256.  This kernel is the serial section
+// between two tile kernels, so it is written for latency: every load a thread needs is issued before the first
+// dependent instruction, and the work that does not depend on the reduced gradient (the prior and Jacobian terms of
+// the own draw, the bias corrections, the Philox normals of the next step) runs while the output slots arrive.
+//  blockIdx.x = k < K       : reduce the part8 slots of phase k and the per-draw prior/Jacobian terms over the S
+//                             draws of instance blockIdx.y -> grad; Adam ascent on the 8 (10) parameters of (inst, k);
+//                             draws + transform of the next step for (inst, k, all s)          (do_update)
+//  blockIdx.x = K + gi      : log-likelihood of the 32 draws of group gi of the instance (sum of llpart over the
+//                             segments: warp w sums the segments t = w mod 8 in increasing order, the eight sums are
+//                             combined in a fixed tree) and their sum ll_g
+//  Short path (at most one draw per thread, and the phase's slot rows of all groups of the instance fit the dynamic
+//  shared memory of the launch, d.upd_smem: configs 0, 1, 3): thread 0 requests the rows with one bulk asynchronous
+//  copy per group right after the wait (cp.async.bulk on an mbarrier: no registers in flight, no address arithmetic),
+//  and every thread reads its rows from shared memory.  Long path: the loops over global memory.  Both add in the same
+//  order (slots in index order, then the draws, fixed shuffle tree, warps in order): results do not depend on the path.
 //  The ELBO is assembled, and the step counted, by finish_step (next tile kernel, or finish_step_kernel).
-__global__ void __launch_bounds__(kUpdThreads) update_draw_kernel(const Dev d, const float* __restrict__ var_in,
+constexpr int kLlBatch = 32;    // llpart loads a thread of a log-likelihood CTA keeps in flight
+
+__device__ __forceinline__ void prior_terms(const Dev& d, const PatConst& pc, const float4 m, const float4 sg, const float4 ep,
+                                            float (&gz)[4], float& lp) {
+    const Phys q = transform(m, sg, ep);
+    gz[0] = 1.0f - pc.lambda_h * q.h;
+    gz[1] = -q.mu * d.mu_inv_var;
+    gz[2] = d.w_shape - d.w_rate * q.w;
+    gz[3] = 1.0f - 2.0f * q.r;
+    const float az = fabsf(q.zr);
+    lp = (pc.log_lambda_h - pc.lambda_h * q.h + q.zh)
+       + (-0.5f * q.mu * q.mu * d.mu_inv_var + d.mu_logc)
+       + (d.w_logc + d.w_shape * q.zw - d.w_rate * q.w)
+       - (az + 2.0f * log1pf(expf(-az)));
+}
+// alpha = exp(zeta) ~ Norm(alpha_mu, alpha_sigma) (B.2 PAPER.md:274) + log Jacobian (R30): (log term, g_alpha)
+__device__ __forceinline__ float2 prior_alpha(const Dev& d, float m_a, float sg_a, float ea) {
+    const float za = fmaf(sg_a, ea, m_a), al = expf(za), da = al - d.alpha_mu;
+    return make_float2(-0.5f * da * da * d.alpha_inv_var + d.alpha_logc + za, 1.0f - da * d.alpha_inv_var * al);
+}
+
+__global__ void __launch_bounds__(kUpdThreads, 2) update_draw_kernel(const Dev d, const float* __restrict__ var_in,
                                                                   int do_update) {
-    __shared__ double red[(kUpdThreads / 32) * 11];
+    constexpr int kW = kUpdThreads / 32;
+    __shared__ double red[kW * 11];
+    __shared__ double ll_s[kW][32];
     __shared__ float new_ml[10];
-    __shared__ double tot_s[10];
-    const int k = blockIdx.x, inst = blockIdx.y;
+    const int inst = blockIdx.y;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int pat = inst / d.R;
     const PatConst pc = d.pat[pat];
-    griddep_launch_dependents();
-    griddep_wait();                               // partials and step counter: written by the tile kernel
-    const long long step = d.ctl->step;           // completed steps; this is step + 1
+    // static tables: the slot range of the phase, before the wait
+    extern __shared__ __align__(128) float rows_s[];           // short path: [gpi][n_sl][8] slot rows of the phase
+    __shared__ __align__(8) unsigned long long mbar_s;
+    const int k = blockIdx.x;
+    int s0 = 0, n_sl = 0;
+    if (k < d.K) { s0 = d.slot_ofs[k]; n_sl = d.slot_ofs[k + 1] - s0; }
+    const int n_part = n_sl * d.gpi;
+    const int s_pad = d.gpi * 32;
+    const bool fast = k < d.K && s_pad <= kUpdThreads && static_cast<long long>(n_part) * 32 <= d.upd_smem;
+    if (fast && n_part > 0) {
+        if (threadIdx.x == 0) {
+            mbar_init(smem_u32(&mbar_s), 1);
+            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        }
+        __syncthreads();                                        // the mbarrier is initialised before anybody polls it
+    }
+    // Also before the wait: everything the previous update_draw_kernel (or the host) wrote -- the variational parameters,
+    // the moments, the normals of this step's draws, the step counter u_step.  That kernel has completed: the tile kernel
+    // between the two lets this one start only after its own griddep_wait.  What the tile kernel writes (the output
+    // slots, llpart, ctl->step / pending through finish_step) is read after the wait.
+    const long long step = d.ctl->u_step;         // completed steps; this is step + 1
     const unsigned long long seed = d.ctl->seed;
     const double inv_s = 1.0 / static_cast<double>(d.S);
-
-    if (k == d.K) {
-        double v[1] = {0.0};
-        for (int s = threadIdx.x; s < d.S; s += kUpdThreads) {
-            const int g = inst * d.gpi + (s >> 5), lane = s & 31;
-            const float* __restrict__ lp = d.llpart + static_cast<size_t>(g) * d.n_seg * 32 + lane;
-            // eight interleaved partial sums (independent load/add chains), combined in a fixed order
-            double a8[8] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
-            int t = 0;
-            for (; t + 32 <= d.n_seg; t += 32) {           // 32 loads in flight, added in the order of the loop below
-                float x[32];
-#pragma unroll
-                for (int j = 0; j < 32; ++j) x[j] = lp[static_cast<size_t>(t + j) * 32];
-#pragma unroll
-                for (int j = 0; j < 32; ++j) a8[j & 7] += static_cast<double>(x[j]);
-            }
-            for (; t + 8 <= d.n_seg; t += 8) {
-#pragma unroll
-                for (int j = 0; j < 8; ++j) a8[j] += static_cast<double>(lp[static_cast<size_t>(t + j) * 32]);
-            }
-            for (int j = 0; t < d.n_seg; ++t, ++j) a8[j] += static_cast<double>(lp[static_cast<size_t>(t) * 32]);
-            const double a = ((a8[0] + a8[1]) + (a8[2] + a8[3])) + ((a8[4] + a8[5]) + (a8[6] + a8[7]));
-            const double ll = static_cast<double>(pc.ll_scale) * a + pc.ll_const;
-            d.ll_t[static_cast<size_t>(inst) * d.gpi * 32 + s] = ll;
-            v[0] += ll;
-        }
-        block_reduce<1, kUpdThreads / 32>(v, red);
-        if (threadIdx.x == 0) d.elbo_k[static_cast<size_t>(inst) * (d.K + 1) + d.K] = v[0] * inv_s;
-    } else {
-        const float4 m = *reinterpret_cast<const float4*>(var_in + (static_cast<size_t>(inst) * 2 * d.K + k) * 4);
-        const float4 l = *reinterpret_cast<const float4*>(var_in + (static_cast<size_t>(inst) * 2 * d.K + d.K + k) * 4);
-        const float4 sg = make_float4(expf(l.x), expf(l.y), expf(l.z), expf(l.w));
+    const unsigned it_n = static_cast<unsigned>(step + 2);
+    float4 m = make_float4(0.f, 0.f, 0.f, 0.f), l = m;
+    float m_a = 0.0f, l_a = 0.0f;
+    // the parameter this thread updates (threads 0..7: (m, l) x 4 classes; 8, 9: alpha), its moments, the bias corrections
+    const bool upd_thread = k < d.K && (threadIdx.x < 8 || (threadIdx.x < 10 && d.asym));
+    const bool is_l = threadIdx.x < 8 ? threadIdx.x >= 4 : threadIdx.x == 9;
+    const size_t o_par = threadIdx.x < 8
+        ? (static_cast<size_t>(inst) * 2 * d.K + (is_l ? d.K : 0) + k) * 4 + (threadIdx.x & 3)
+        : static_cast<size_t>(inst) * 2 * d.K + (is_l ? d.K : 0) + k;
+    float x_par = 0.0f, m1_par = 0.0f, m2_par = 0.0f;
+    float bc1 = 1.0f, bc2 = 1.0f;                    // Adam bias corrections of this step
+    if (k < d.K) {
+        m = *reinterpret_cast<const float4*>(var_in + (static_cast<size_t>(inst) * 2 * d.K + k) * 4);
+        l = *reinterpret_cast<const float4*>(var_in + (static_cast<size_t>(inst) * 2 * d.K + d.K + k) * 4);
         // R30: the fifth latent's parameters sit behind the [PR][2][K][4] block of every state array
         const float* __restrict__ va_in = var_in + static_cast<size_t>(d.PR) * 8 * d.K + static_cast<size_t>(inst) * 2 * d.K;
-        const float m_a = d.asym ? va_in[k] : 0.0f, l_a = d.asym ? va_in[d.K + k] : 0.0f;
-        const float sg_a = expf(l_a);
-        double v[11];   // [0..3] sum g, [4..7] sum g eps, [8] sum log prior + log Jacobian, [9] sum g_alpha, [10] sum g_alpha eps_alpha
+        if (d.asym) { m_a = va_in[k]; l_a = va_in[d.K + k]; }
+        if (upd_thread) {
+            x_par = threadIdx.x < 8 ? var_in[o_par] : (is_l ? l_a : m_a);
+            if (do_update && d.optimizer != 1) {
+                m1_par = threadIdx.x < 8 ? d.mom1[o_par] : d.mom1_a[o_par];
+                m2_par = threadIdx.x < 8 ? d.mom2[o_par] : d.mom2_a[o_par];
+                const float stepf = static_cast<float>(step + 1 - d.ctl->adam_t0);
+                bc1 = 1.0f - powf(d.beta1, stepf);
+                bc2 = 1.0f - powf(d.beta2, stepf);
+            }
+        }
+    }
+    // short path: prior + Jacobian terms of the thread's draw and the Philox normals of its next draw
+    const bool has_draw = fast && static_cast<int>(threadIdx.x) < d.S;
+    float4 ep = make_float4(0.f, 0.f, 0.f, 0.f), ep_n = ep;
+    float ea = 0.0f, epa_n = 0.0f;
+    float gz[4] = {0.f, 0.f, 0.f, 0.f}, lp = 0.0f;
+    float2 pr_a = make_float2(0.f, 0.f);
+    if (fast) {
+        const int s = threadIdx.x;
+        if (has_draw) {
+            const size_t o_draw = (static_cast<size_t>(inst * d.gpi + (s >> 5)) * d.K + k) * 32 + lane;
+            ep = d.eps[o_draw];
+            if (d.asym) ea = d.eps_a[o_draw];
+            const float4 sg = make_float4(expf(l.x), expf(l.y), expf(l.z), expf(l.w));
+            prior_terms(d, pc, m, sg, ep, gz, lp);
+            if (d.asym) pr_a = prior_alpha(d, m_a, expf(l_a), ea);
+        }
+        if (do_update && s < s_pad) {
+            const uint2 key = make_uint2(static_cast<unsigned>(seed), static_cast<unsigned>(seed >> 32));
+            ep_n = normals_from_words(philox4x32_10(
+                make_uint4(it_n, static_cast<unsigned>(s), static_cast<unsigned>(k), static_cast<unsigned>(inst)), key));
+            if (d.asym) epa_n = normal_alpha(it_n, static_cast<unsigned>(s), static_cast<unsigned>(k), static_cast<unsigned>(inst), seed);
+        }
+    }
+    griddep_launch_dependents();
+    griddep_wait();                               // output slots, llpart: written by the tile kernel
+    if (fast && n_part > 0 && threadIdx.x == 0) {               // the slot rows of the phase, one contiguous piece per group
+        const unsigned mb = smem_u32(&mbar_s), piece = 32u * static_cast<unsigned>(n_sl);
+        mbar_expect_tx(mb, piece * static_cast<unsigned>(d.gpi));
+        const float* __restrict__ src = d.part8 + (static_cast<size_t>(inst) * d.gpi * d.n_slots + s0) * 8;
+        for (int gi = 0; gi < d.gpi; ++gi)
+            bulk_g2s(smem_u32(rows_s) + piece * gi, src + static_cast<size_t>(gi) * d.n_slots * 8, piece, mb);
+    }
+
+    if (k >= d.K) {
+        const int gi = k - d.K;
+        const int g = inst * d.gpi + gi;
+        const float* __restrict__ lp_g = d.llpart + static_cast<size_t>(g) * d.n_seg * 32 + lane;
+        const int n_i = warp < d.n_seg ? (d.n_seg - warp + kW - 1) / kW : 0;   // segments warp, warp + 8, ...
+        double a = 0.0;
+        for (int i = 0; i < n_i; i += kLlBatch) {      // kLlBatch loads in flight, added in segment order
+            float x[kLlBatch];
 #pragma unroll
-        for (int i = 0; i < 11; ++i) v[i] = 0.0;
+            for (int j = 0; j < kLlBatch; ++j) x[j] = i + j < n_i ? lp_g[static_cast<size_t>(warp + kW * (i + j)) * 32] : 0.0f;
+#pragma unroll
+            for (int j = 0; j < kLlBatch; ++j)
+                if (i + j < n_i) a += static_cast<double>(x[j]);
+        }
+        ll_s[warp][lane] = a;
+        __syncthreads();
+        if (warp == 0) {
+            const double a8 = ((ll_s[0][lane] + ll_s[1][lane]) + (ll_s[2][lane] + ll_s[3][lane])) +
+                              ((ll_s[4][lane] + ll_s[5][lane]) + (ll_s[6][lane] + ll_s[7][lane]));
+            const int s = gi * 32 + lane;
+            double ll = 0.0;
+            if (s < d.S) {
+                ll = static_cast<double>(pc.ll_scale) * a8 + pc.ll_const;
+                d.ll_t[static_cast<size_t>(inst) * s_pad + s] = ll;
+            }
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) ll += __shfl_xor_sync(0xffffffffu, ll, o);
+            if (lane == 0) d.ll_g[g] = ll;
+        }
+        if (k == d.K && inst == 0 && threadIdx.x == 0) {
+            d.ctl->pending = do_update ? 2u : 1u;
+            d.ctl->u_step = step + (do_update ? 1 : 0);        // what finish_step will make of ctl->step
+        }
+        return;
+    }
+
+    double v[11];   // [0..3] sum g, [4..7] sum g eps, [8] sum log prior + log Jacobian, [9] sum g_alpha, [10] sum g_alpha eps_alpha
+#pragma unroll
+    for (int i = 0; i < 11; ++i) v[i] = 0.0;
+
+    if (fast) {
+        if (d.asym) {     // the alpha pair of every slot (R30 only): from global memory, under the bulk copies
+            for (int idx = threadIdx.x; idx < n_part; idx += kUpdThreads) {
+                const int gi = idx / n_sl, sl = s0 + (idx - gi * n_sl);
+                const float2 pa = *reinterpret_cast<const float2*>(
+                    d.parta + (static_cast<size_t>(inst * d.gpi + gi) * d.n_slots + sl) * 2);
+                v[9] += pa.x;
+                v[10] += pa.y;
+            }
+        }
+        // likelihood part, slots in index order (row idx of the staged block = group gi, slot s0 + idx - gi n_sl)
+        if (n_part > 0) {
+            mbar_wait(smem_u32(&mbar_s), 0u);
+            for (int idx = threadIdx.x; idx < n_part; idx += kUpdThreads) {
+                const float4 a = *reinterpret_cast<const float4*>(rows_s + static_cast<size_t>(idx) * 8);
+                const float4 b = *reinterpret_cast<const float4*>(rows_s + static_cast<size_t>(idx) * 8 + 4);
+                v[0] += a.x; v[1] += a.y; v[2] += a.z; v[3] += a.w;
+                v[4] += b.x; v[5] += b.y; v[6] += b.z; v[7] += b.w;
+            }
+        }
+        if (has_draw) {
+            const float e4[4] = {ep.x, ep.y, ep.z, ep.w};
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+                v[c] += static_cast<double>(gz[c]);
+                v[4 + c] += static_cast<double>(gz[c] * e4[c]);
+            }
+            v[8] += static_cast<double>(lp);
+            if (d.asym) {
+                v[8] += static_cast<double>(pr_a.x);
+                v[9] += static_cast<double>(pr_a.y);
+                v[10] += static_cast<double>(pr_a.y * ea);
+            }
+        }
+    } else {
         // likelihood part: partials of phase k, all groups of the instance
-        const int s0 = d.slot_ofs[k], s1 = d.slot_ofs[k + 1];
-        const int n_sl = s1 - s0;
-        const int n_part = n_sl * d.gpi;
         for (int idx = threadIdx.x; idx < n_part; idx += kUpdThreads) {
             const int gi = idx / n_sl, sl = s0 + (idx - gi * n_sl);
             const float4* __restrict__ pp = reinterpret_cast<const float4*>(
@@ -1526,17 +1681,13 @@ __global__ void __launch_bounds__(kUpdThreads) update_draw_kernel(const Dev d, c
             }
         }
         // prior + Jacobian part, per draw
+        const float4 sg = make_float4(expf(l.x), expf(l.y), expf(l.z), expf(l.w));
+        const float sg_a = expf(l_a);
         for (int s = threadIdx.x; s < d.S; s += kUpdThreads) {
-            const int g = inst * d.gpi + (s >> 5), lane = s & 31;
+            const int g = inst * d.gpi + (s >> 5);
             const float4 ep = d.eps[(static_cast<size_t>(g) * d.K + k) * 32 + lane];
-            const Phys q = transform(m, sg, ep);
-            const float gz[4] = {1.0f - pc.lambda_h * q.h, -q.mu * d.mu_inv_var,
-                                 d.w_shape - d.w_rate * q.w, 1.0f - 2.0f * q.r};
-            const float az = fabsf(q.zr);
-            const float lp = (pc.log_lambda_h - pc.lambda_h * q.h + q.zh)
-                           + (-0.5f * q.mu * q.mu * d.mu_inv_var + d.mu_logc)
-                           + (d.w_logc + d.w_shape * q.zw - d.w_rate * q.w)
-                           - (az + 2.0f * log1pf(expf(-az)));
+            float gz[4], lp;
+            prior_terms(d, pc, m, sg, ep, gz, lp);
             const float e4[4] = {ep.x, ep.y, ep.z, ep.w};
 #pragma unroll
             for (int c = 0; c < 4; ++c) {
@@ -1544,95 +1695,85 @@ __global__ void __launch_bounds__(kUpdThreads) update_draw_kernel(const Dev d, c
                 v[4 + c] += static_cast<double>(gz[c] * e4[c]);
             }
             v[8] += static_cast<double>(lp);
-            if (d.asym) {      // alpha = exp(zeta) ~ Norm(alpha_mu, alpha_sigma) (B.2 PAPER.md:274) + log Jacobian (R30)
+            if (d.asym) {
                 const float ea = d.eps_a[(static_cast<size_t>(g) * d.K + k) * 32 + lane];
-                const float za = fmaf(sg_a, ea, m_a), al = expf(za), da = al - d.alpha_mu;
-                const float ga = 1.0f - da * d.alpha_inv_var * al;
-                v[8] += static_cast<double>(-0.5f * da * da * d.alpha_inv_var + d.alpha_logc + za);
-                v[9] += static_cast<double>(ga);
-                v[10] += static_cast<double>(ga * ea);
+                const float2 pr_a = prior_alpha(d, m_a, sg_a, ea);
+                v[8] += static_cast<double>(pr_a.x);
+                v[9] += static_cast<double>(pr_a.y);
+                v[10] += static_cast<double>(pr_a.y * ea);
             }
         }
-        block_reduce<11, kUpdThreads / 32>(v, red);
-        if (threadIdx.x == 0) {
+    }
+
+    // deterministic block reduction: fixed shuffle tree inside a warp, then thread i < 11 adds the warps' sums of
+    // value i in warp order.  Thread i < 8 owns parameter i, threads 8 / 9 the alpha pair (sums 9 / 10), thread 10 sum 8.
+    const int n_red = d.asym ? 11 : 9;
 #pragma unroll
-            for (int i = 0; i < 8; ++i) tot_s[i] = v[i];
-            tot_s[8] = v[9];
-            tot_s[9] = v[10];
+    for (int i = 0; i < 11; ++i) {
+        if (i < n_red) {
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) v[i] += __shfl_xor_sync(0xffffffffu, v[i], o);
         }
-        __syncthreads();
-        if (threadIdx.x < 8) {
+    }
+    if (lane == 0) {
+#pragma unroll
+        for (int i = 0; i < 11; ++i) red[warp * 11 + i] = v[i];
+    }
+    __syncthreads();
+    if (threadIdx.x < 11) {
+        const int col = threadIdx.x < 8 ? threadIdx.x : threadIdx.x == 10 ? 8 : threadIdx.x + 1;
+        double tot = 0.0;
+#pragma unroll
+        for (int w = 0; w < kW; ++w) tot += red[w * 11 + col];
+        if (threadIdx.x == 10) {
+            // mean log prior + Jacobian of the phase, plus its entropy sum_c (l_c + 1/2 ln 2 pi e)
+            d.elbo_k[static_cast<size_t>(inst) * (d.K + 1) + k] =
+                tot * inv_s + (static_cast<double>(l.x) + static_cast<double>(l.y) + static_cast<double>(l.z) +
+                               static_cast<double>(l.w)) + 4.0 * 1.4189385332046727 +
+                (d.asym ? static_cast<double>(l_a) + 1.4189385332046727 : 0.0);
+        } else if (upd_thread) {
             const int c = threadIdx.x & 3;
-            const bool is_l = threadIdx.x >= 4;
-            const float sgc = c == 0 ? sg.x : c == 1 ? sg.y : c == 2 ? sg.z : sg.w;
-            const double tot = tot_s[threadIdx.x];
+            const float lc = threadIdx.x >= 8 ? l_a : c == 0 ? l.x : c == 1 ? l.y : c == 2 ? l.z : l.w;
+            const float sgc = expf(lc);
             const double gd = is_l ? tot * inv_s * static_cast<double>(sgc) + 1.0 : tot * inv_s;
             const float gj = static_cast<float>(gd);
-            const size_t o = (static_cast<size_t>(inst) * 2 * d.K + (is_l ? d.K : 0) + k) * 4 + c;
-            d.grad[o] = gj;
-            float x = var_in[o];
+            (threadIdx.x < 8 ? d.grad : d.grad_a)[o_par] = gj;
+            float x = x_par;
             if (do_update) {   // l clamped to [-12, 2]
                 if (d.optimizer == 1) {   // natural-gradient ascent: Fisher metric diag(1/sigma^2, 2) (R25)
                     x += d.lr * (is_l ? 0.5f * gj : sgc * sgc * gj);
                 } else {                  // Adam ascent, bias-corrected (R10)
-                    const float stepf = static_cast<float>(step + 1 - d.ctl->adam_t0);
-                    const float bc1 = 1.0f - powf(d.beta1, stepf);
-                    const float bc2 = 1.0f - powf(d.beta2, stepf);
-                    const float m1 = d.beta1 * d.mom1[o] + (1.0f - d.beta1) * gj;
-                    const float m2 = d.beta2 * d.mom2[o] + (1.0f - d.beta2) * gj * gj;
-                    d.mom1[o] = m1;
-                    d.mom2[o] = m2;
+                    // the roundings are written out (one product rounded, the other fused), so that the moments do
+                    // not depend on how a compiler version contracts the two-term sums
+                    const float m1 = __fmaf_rn(gj, 1.0f - d.beta1, __fmul_rn(d.beta1, m1_par));
+                    const float m2 = __fmaf_rn(m2_par, d.beta2, __fmul_rn(__fmul_rn(1.0f - d.beta2, gj), gj));
+                    (threadIdx.x < 8 ? d.mom1 : d.mom1_a)[o_par] = m1;
+                    (threadIdx.x < 8 ? d.mom2 : d.mom2_a)[o_par] = m2;
                     x += d.lr * (m1 / bc1) / (sqrtf(m2 / bc2) + d.adam_eps);
                 }
                 if (is_l) x = fminf(fmaxf(x, -12.0f), 2.0f);
-                d.var[o] = x;
+                (threadIdx.x < 8 ? d.var : d.var_a)[o_par] = x;
             }
             new_ml[threadIdx.x] = x;
-        } else if (threadIdx.x < 10 && d.asym) {   // the two parameters of alpha: same update rules
-            const bool is_l = threadIdx.x == 9;
-            const double tot = tot_s[threadIdx.x];
-            const double gd = is_l ? tot * inv_s * static_cast<double>(sg_a) + 1.0 : tot * inv_s;
-            const float gj = static_cast<float>(gd);
-            const size_t o = static_cast<size_t>(inst) * 2 * d.K + (is_l ? d.K : 0) + k;
-            d.grad_a[o] = gj;
-            float x = is_l ? l_a : m_a;
-            if (do_update) {
-                if (d.optimizer == 1) {
-                    x += d.lr * (is_l ? 0.5f * gj : sg_a * sg_a * gj);
-                } else {
-                    const float stepf = static_cast<float>(step + 1 - d.ctl->adam_t0);
-                    const float bc1 = 1.0f - powf(d.beta1, stepf);
-                    const float bc2 = 1.0f - powf(d.beta2, stepf);
-                    const float m1 = d.beta1 * d.mom1_a[o] + (1.0f - d.beta1) * gj;
-                    const float m2 = d.beta2 * d.mom2_a[o] + (1.0f - d.beta2) * gj * gj;
-                    d.mom1_a[o] = m1;
-                    d.mom2_a[o] = m2;
-                    x += d.lr * (m1 / bc1) / (sqrtf(m2 / bc2) + d.adam_eps);
-                }
-                if (is_l) x = fminf(fmaxf(x, -12.0f), 2.0f);
-                d.var_a[o] = x;
-            }
-            new_ml[threadIdx.x] = x;
-        }
-        if (threadIdx.x == 0)  // mean log prior + Jacobian of the phase, plus its entropy sum_c (l_c + 1/2 ln 2 pi e)
-            d.elbo_k[static_cast<size_t>(inst) * (d.K + 1) + k] =
-                v[8] * inv_s + (static_cast<double>(l.x) + static_cast<double>(l.y) + static_cast<double>(l.z) +
-                                static_cast<double>(l.w)) + 4.0 * 1.4189385332046727 +
-                (d.asym ? static_cast<double>(l_a) + 1.4189385332046727 : 0.0);
-        if (do_update) {       // draws of the next step from the updated parameters
-            __syncthreads();
-            const float4 mn = make_float4(new_ml[0], new_ml[1], new_ml[2], new_ml[3]);
-            const float4 ln = make_float4(new_ml[4], new_ml[5], new_ml[6], new_ml[7]);
-            const unsigned it = static_cast<unsigned>(step + 2);
-            const int s_pad = d.gpi * 32;
-            const float mna = d.asym ? new_ml[8] : 0.0f, lna = d.asym ? new_ml[9] : 0.0f;
-            for (int s = threadIdx.x; s < s_pad; s += kUpdThreads) draw_one(d, inst, k, s, it, seed, mn, ln, nullptr, mna, lna);
         }
     }
-
-    // The ELBO of the step is assembled from elbo_k by finish_step, which also counts the step: the NEXT step's
-    // tile kernel runs it, so this kernel ends without fences, tickets or a serial tail.
-    if (k == d.K && inst == 0 && threadIdx.x == 0) d.ctl->pending = do_update ? 2u : 1u;
+    if (do_update) {       // draws of the next step from the updated parameters
+        __syncthreads();
+        const float4 mn = make_float4(new_ml[0], new_ml[1], new_ml[2], new_ml[3]);
+        const float4 ln = make_float4(new_ml[4], new_ml[5], new_ml[6], new_ml[7]);
+        const float mna = d.asym ? new_ml[8] : 0.0f, lna = d.asym ? new_ml[9] : 0.0f;
+        if (fast) {
+            const int s = threadIdx.x;
+            if (s < s_pad) {   // whole warps
+                const float4 sgn = make_float4(expf(ln.x), expf(ln.y), expf(ln.z), expf(ln.w));
+                float alpha = 1.0f;
+                if (d.asym) alpha = expf(fmaf(expf(lna), epa_n, mna));
+                emit_latent(d, inst * d.gpi + (s >> 5), k, s < d.S, transform(mn, sgn, ep_n), ep_n, alpha, epa_n);
+            }
+        } else {
+            for (int s = threadIdx.x; s < s_pad; s += kUpdThreads) draw_one(d, inst, k, s, it_n, seed, mn, ln, nullptr, mna, lna);
+        }
+    }
 }
 
 // a-7 (last part): ELBO of every instance = mean log-likelihood + sum over the phases of (mean log prior + log
