@@ -228,9 +228,20 @@ const char* build_tables(const Plan& pl, int64_t N, int K, const std::vector<Hos
         pairs += hi - lo + 1;
         fw.push_back(p);
     }
-    // (phase, grid index, input order) order: the order of the entries inside every tile list
-    std::stable_sort(fw.begin(), fw.end(), [](const HostPeak& a, const HostPeak& b) { return a.j < b.j; });
-    std::stable_sort(fw.begin(), fw.end(), [](const HostPeak& a, const HostPeak& b) { return a.k < b.k; });
+    // (phase, grid index, input order) order: the order of the entries inside every tile list.  The callers hand the peaks
+    // over phase by phase, so one stable sort by grid index inside every phase's range does it (two stable sorts of the
+    // whole list otherwise: 0.34 of the 0.86 ms of a config-1 table build).
+    if (std::is_sorted(fw.begin(), fw.end(), [](const HostPeak& a, const HostPeak& b) { return a.k < b.k; })) {
+        for (size_t b = 0; b < fw.size();) {
+            size_t e = b + 1;
+            while (e < fw.size() && fw[e].k == fw[b].k) ++e;
+            std::stable_sort(fw.begin() + b, fw.begin() + e, [](const HostPeak& a, const HostPeak& b2) { return a.j < b2.j; });
+            b = e;
+        }
+    } else {
+        std::stable_sort(fw.begin(), fw.end(), [](const HostPeak& a, const HostPeak& b) { return a.j < b.j; });
+        std::stable_sort(fw.begin(), fw.end(), [](const HostPeak& a, const HostPeak& b) { return a.k < b.k; });
+    }
     const int PSn = pl.PS, TWn = pl.TW, n_tile = pl.n_tile;
     auto tiles_of = [&](const HostPeak& p, int* t0, int* t1) {
         const long long lo = std::max<long long>(0, p.j - nck[p.k]), hi = std::min<long long>(N - 1, p.j + nck[p.k]);
