@@ -1523,8 +1523,9 @@ __global__ void __launch_bounds__(kUpdThreads, 2) update_draw_kernel(const Dev d
     // the moments, the normals of this step's draws, the step counter u_step.  That kernel has completed: the tile kernel
     // between the two lets this one start only after its own griddep_wait.  What the tile kernel writes (the output
     // slots, llpart, ctl->step / pending through finish_step) is read after the wait.
-    const long long step = d.ctl->u_step;         // completed steps; this is step + 1
-    const unsigned long long seed = d.ctl->seed;
+    // These loads bypass L1 (ld.global.cg): the SM may still hold lines the previous launches of this kernel read.
+    const long long step = __ldcg(&d.ctl->u_step);         // completed steps; this is step + 1
+    const unsigned long long seed = __ldcg(&d.ctl->seed);
     const double inv_s = 1.0 / static_cast<double>(d.S);
     const unsigned it_n = static_cast<unsigned>(step + 2);
     float4 m = make_float4(0.f, 0.f, 0.f, 0.f), l = m;
@@ -1538,17 +1539,17 @@ __global__ void __launch_bounds__(kUpdThreads, 2) update_draw_kernel(const Dev d
     float x_par = 0.0f, m1_par = 0.0f, m2_par = 0.0f;
     float bc1 = 1.0f, bc2 = 1.0f;                    // Adam bias corrections of this step
     if (k < d.K) {
-        m = *reinterpret_cast<const float4*>(var_in + (static_cast<size_t>(inst) * 2 * d.K + k) * 4);
-        l = *reinterpret_cast<const float4*>(var_in + (static_cast<size_t>(inst) * 2 * d.K + d.K + k) * 4);
+        m = __ldcg(reinterpret_cast<const float4*>(var_in + (static_cast<size_t>(inst) * 2 * d.K + k) * 4));
+        l = __ldcg(reinterpret_cast<const float4*>(var_in + (static_cast<size_t>(inst) * 2 * d.K + d.K + k) * 4));
         // R30: the fifth latent's parameters sit behind the [PR][2][K][4] block of every state array
         const float* __restrict__ va_in = var_in + static_cast<size_t>(d.PR) * 8 * d.K + static_cast<size_t>(inst) * 2 * d.K;
-        if (d.asym) { m_a = va_in[k]; l_a = va_in[d.K + k]; }
+        if (d.asym) { m_a = __ldcg(va_in + k); l_a = __ldcg(va_in + d.K + k); }
         if (upd_thread) {
-            x_par = threadIdx.x < 8 ? var_in[o_par] : (is_l ? l_a : m_a);
+            x_par = threadIdx.x < 8 ? __ldcg(var_in + o_par) : (is_l ? l_a : m_a);
             if (do_update && d.optimizer != 1) {
-                m1_par = threadIdx.x < 8 ? d.mom1[o_par] : d.mom1_a[o_par];
-                m2_par = threadIdx.x < 8 ? d.mom2[o_par] : d.mom2_a[o_par];
-                const float stepf = static_cast<float>(step + 1 - d.ctl->adam_t0);
+                m1_par = __ldcg((threadIdx.x < 8 ? d.mom1 : d.mom1_a) + o_par);
+                m2_par = __ldcg((threadIdx.x < 8 ? d.mom2 : d.mom2_a) + o_par);
+                const float stepf = static_cast<float>(step + 1 - __ldcg(&d.ctl->adam_t0));
                 bc1 = 1.0f - powf(d.beta1, stepf);
                 bc2 = 1.0f - powf(d.beta2, stepf);
             }
@@ -1564,8 +1565,8 @@ __global__ void __launch_bounds__(kUpdThreads, 2) update_draw_kernel(const Dev d
         const int s = threadIdx.x;
         if (has_draw) {
             const size_t o_draw = (static_cast<size_t>(inst * d.gpi + (s >> 5)) * d.K + k) * 32 + lane;
-            ep = d.eps[o_draw];
-            if (d.asym) ea = d.eps_a[o_draw];
+            ep = __ldcg(d.eps + o_draw);
+            if (d.asym) ea = __ldcg(d.eps_a + o_draw);
             const float4 sg = make_float4(expf(l.x), expf(l.y), expf(l.z), expf(l.w));
             prior_terms(d, pc, m, sg, ep, gz, lp);
             if (d.asym) pr_a = prior_alpha(d, m_a, expf(l_a), ea);
