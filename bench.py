@@ -96,16 +96,19 @@ CAPTURE_FILE = "profiles/r2_capture_counters.txt"
 
 
 def captured_counters(cfg: int):
-    """(kernel, DRAM bytes per launch, warp instructions per launch) of the dominant kernel at config `cfg` from the
-    committed `ncu --set full` capture of THIS build (profiles/r2_capture_counters.txt: kernel, config, dram bytes, warp
-    instructions; written from the capture named in its header), or (DOM_KERNEL, None, None) when no capture exists."""
+    """(kernel, DRAM bytes per launch, warp instructions per launch, pipe utilisation) of the dominant kernel at config
+    `cfg` from the committed `ncu --set full` capture of THIS build (profiles/r2_capture_counters.txt: kernel, config,
+    dram bytes, warp instructions, then issue / XU / FMA pipe activity in per cent of the active cycles; written from the
+    capture named in its header), or (DOM_KERNEL, None, None, None) when no capture exists."""
     p = ROOT / CAPTURE_FILE
     if p.exists():
         for ln in p.read_text().splitlines():
             t = ln.split()
-            if len(t) == 4 and not ln.startswith("#") and t[1] == str(cfg):
-                return t[0], int(t[2]), int(t[3])
-    return DOM_KERNEL, None, None
+            if len(t) in (4, 7) and not ln.startswith("#") and t[1] == str(cfg):
+                util = ({"issue_active_pct": float(t[4]), "xu_pipe_pct": float(t[5]), "fma_pipe_pct": float(t[6])}
+                        if len(t) == 7 else None)
+                return t[0], int(t[2]), int(t[3]), util
+    return DOM_KERNEL, None, None, None
 
 
 def run_reference(args, rank: int) -> None:
@@ -267,7 +270,7 @@ def run_ours(args, rank: int, local_rank: int, world: int) -> None:
     dom_ms = tk["ms_tile"]
     achieved = pairs * T / (dom_ms * 1e-3)
     r_plain = n_sm * f_max * 16.0 / 4.0          # plain formulation: 4 MUFU per pair (2 per pass), 16 MUFU lanes/SM/clk
-    dom_kernel, traffic, warp_instr = captured_counters(args.config)
+    dom_kernel, traffic, warp_instr, pipe_util = captured_counters(args.config)
     roofline = {
         "bound": "alu", "kernel": dom_kernel, "achieved": achieved / 1e9, "peak": r_plain / 1e9,
         "unit": "Gpair/s", "frac": achieved / r_plain, "traffic": traffic,
@@ -278,6 +281,9 @@ def run_ours(args, rank: int, local_rank: int, world: int) -> None:
         # warp instructions per launch (same capture) / (SMs x 4 issue slots per clock x f_clk x kernel time)
         "issue_frac": (warp_instr / (n_sm * 4.0 * f_max * dom_ms * 1e-3) if warp_instr else None),
         "warp_instructions_per_launch": warp_instr,
+        # how busy the kernel keeps the pipes its own formulation uses (same capture, one launch under ncu: sm__
+        # inst_executed_pipe_xu, sm__pipe_fma_cycles_active, smsp__issue_active in % of the active cycles)
+        "pipe_util_captured": pipe_util,
         "peak_source": f"derived: {n_sm} SMs x {f_max / 1e6:.0f} MHz (MEASURED_PEAKS sm_max_mhz) x 16 MUFU lanes / "
                        f"4 MUFU per pair (plain forward+backward formulation, DESIGN.md Roofline)",
         "ms_tile": tk["ms_tile"], "ms_tile_forward_only": tk["ms_tile_forward_only"], "ms_update": tk["ms_update"],
