@@ -81,6 +81,8 @@ struct Ctl {       // device-resident control block (so that graph replays need 
     unsigned int pad;
     long long u_step;              // `step` as the next update_draw_kernel will see it: kept by update_draw_kernel itself
                                    // (and set with `step` by the host), so that it may be read before griddep_wait
+    unsigned int upd_done;         // CTAs of the current update_draw_kernel launch that are done (the last one moves u_step)
+    unsigned int pad2;
 };
 
 struct Dev {
@@ -1493,6 +1495,20 @@ __device__ __forceinline__ float2 prior_alpha(const Dev& d, float m_a, float sg_
     return make_float2(-0.5f * da * da * d.alpha_inv_var + d.alpha_logc + za, 1.0f - da * d.alpha_inv_var * al);
 }
 
+// End of a CTA of update_draw_kernel.  The step counter u_step is read by every CTA of a launch BEFORE its wait, so it may
+// move only when no CTA of the launch can still be about to read it: the last CTA to finish moves it (a grid with many
+// instances runs in several waves; the CTA that owns the log-likelihood of instance 0 is long gone when the last wave starts).
+__device__ __forceinline__ void upd_cta_done(const Dev& d, long long next_step) {
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        const unsigned n_cta = gridDim.x * gridDim.y;
+        if (atomicAdd(&d.ctl->upd_done, 1u) == n_cta - 1) {
+            d.ctl->upd_done = 0u;
+            d.ctl->u_step = next_step;                         // what finish_step will make of ctl->step
+        }
+    }
+}
+
 __global__ void __launch_bounds__(kUpdThreads, 2) update_draw_kernel(const Dev d, const float* __restrict__ var_in,
                                                                   int do_update) {
     constexpr int kW = kUpdThreads / 32;
@@ -1617,10 +1633,8 @@ __global__ void __launch_bounds__(kUpdThreads, 2) update_draw_kernel(const Dev d
             for (int o = 16; o > 0; o >>= 1) ll += __shfl_xor_sync(0xffffffffu, ll, o);
             if (lane == 0) d.ll_g[g] = ll;
         }
-        if (k == d.K && inst == 0 && threadIdx.x == 0) {
-            d.ctl->pending = do_update ? 2u : 1u;
-            d.ctl->u_step = step + (do_update ? 1 : 0);        // what finish_step will make of ctl->step
-        }
+        if (k == d.K && inst == 0 && threadIdx.x == 0) d.ctl->pending = do_update ? 2u : 1u;
+        upd_cta_done(d, step + (do_update ? 1 : 0));
         return;
     }
 
@@ -1775,6 +1789,7 @@ __global__ void __launch_bounds__(kUpdThreads, 2) update_draw_kernel(const Dev d
             for (int s = threadIdx.x; s < s_pad; s += kUpdThreads) draw_one(d, inst, k, s, it_n, seed, mn, ln, nullptr, mna, lna);
         }
     }
+    upd_cta_done(d, step + (do_update ? 1 : 0));
 }
 
 // a-7 (last part): ELBO of every instance = mean log-likelihood + sum over the phases of (mean log prior + log
