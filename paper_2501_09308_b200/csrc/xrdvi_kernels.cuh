@@ -79,10 +79,13 @@ struct Ctl {       // device-resident control block (so that graph replays need 
     unsigned int ticket;           // next work item of elbo_split_kernel (re-armed by the launch's last CTA)
     unsigned int finished;         // CTAs of the current elbo_split_kernel launch that are done
     unsigned int pad;
-    long long u_step;              // `step` as the next update_draw_kernel will see it: kept by update_draw_kernel itself
-                                   // (and set with `step` by the host), so that it may be read before griddep_wait
-    unsigned int upd_done;         // CTAs of the current update_draw_kernel launch that are done (the last one moves u_step)
-    unsigned int pad2;
+    // The step as update_draw_kernel sees it, kept by that kernel itself so that it may be read BEFORE griddep_wait
+    // (finish_step of the tile kernel moves `step`): step = u_step + u_acc / (CTAs of a launch).  The host sets u_step =
+    // step and u_acc = 0 at the start of a run; every CTA of an optimisation step adds 1 to u_acc when it is done
+    // (fire and forget).  A CTA of a later wave of the same launch reads u_acc with some of that launch's additions
+    // in it, but never all of them (its own is missing), so the quotient is the same for every CTA of a launch.
+    long long u_step;
+    unsigned long long u_acc;
 };
 
 struct Dev {
@@ -1495,20 +1498,6 @@ __device__ __forceinline__ float2 prior_alpha(const Dev& d, float m_a, float sg_
     return make_float2(-0.5f * da * da * d.alpha_inv_var + d.alpha_logc + za, 1.0f - da * d.alpha_inv_var * al);
 }
 
-// End of a CTA of update_draw_kernel.  The step counter u_step is read by every CTA of a launch BEFORE its wait, so it may
-// move only when no CTA of the launch can still be about to read it: the last CTA to finish moves it (a grid with many
-// instances runs in several waves; the CTA that owns the log-likelihood of instance 0 is long gone when the last wave starts).
-__device__ __forceinline__ void upd_cta_done(const Dev& d, long long next_step) {
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        const unsigned n_cta = gridDim.x * gridDim.y;
-        if (atomicAdd(&d.ctl->upd_done, 1u) == n_cta - 1) {
-            d.ctl->upd_done = 0u;
-            d.ctl->u_step = next_step;                         // what finish_step will make of ctl->step
-        }
-    }
-}
-
 __global__ void __launch_bounds__(kUpdThreads, 2) update_draw_kernel(const Dev d, const float* __restrict__ var_in,
                                                                   int do_update) {
     constexpr int kW = kUpdThreads / 32;
@@ -1540,7 +1529,8 @@ __global__ void __launch_bounds__(kUpdThreads, 2) update_draw_kernel(const Dev d
     // between the two lets this one start only after its own griddep_wait.  What the tile kernel writes (the output
     // slots, llpart, ctl->step / pending through finish_step) is read after the wait.
     // These loads bypass L1 (ld.global.cg): the SM may still hold lines the previous launches of this kernel read.
-    const long long step = __ldcg(&d.ctl->u_step);         // completed steps; this is step + 1
+    const long long step = __ldcg(&d.ctl->u_step) +        // completed steps; this is step + 1
+        static_cast<long long>(__ldcg(&d.ctl->u_acc) / (static_cast<unsigned long long>(gridDim.x) * gridDim.y));
     const unsigned long long seed = __ldcg(&d.ctl->seed);
     const double inv_s = 1.0 / static_cast<double>(d.S);
     const unsigned it_n = static_cast<unsigned>(step + 2);
@@ -1634,7 +1624,7 @@ __global__ void __launch_bounds__(kUpdThreads, 2) update_draw_kernel(const Dev d
             if (lane == 0) d.ll_g[g] = ll;
         }
         if (k == d.K && inst == 0 && threadIdx.x == 0) d.ctl->pending = do_update ? 2u : 1u;
-        upd_cta_done(d, step + (do_update ? 1 : 0));
+        if (do_update && threadIdx.x == 0) atomicAdd(&d.ctl->u_acc, 1ull);    // this CTA is done (result unused: a reduction)
         return;
     }
 
@@ -1789,7 +1779,7 @@ __global__ void __launch_bounds__(kUpdThreads, 2) update_draw_kernel(const Dev d
             for (int s = threadIdx.x; s < s_pad; s += kUpdThreads) draw_one(d, inst, k, s, it_n, seed, mn, ln, nullptr, mna, lna);
         }
     }
-    upd_cta_done(d, step + (do_update ? 1 : 0));
+    if (do_update && threadIdx.x == 0) atomicAdd(&d.ctl->u_acc, 1ull);        // this CTA is done (result unused: a reduction)
 }
 
 // a-7 (last part): ELBO of every instance = mean log-likelihood + sum over the phases of (mean log prior + log
