@@ -46,6 +46,24 @@ int xrdvi_time_kernels(xrdvi* h, int32_t S, uint64_t seed, int32_t reps, float* 
 int xrdvi_debug_timeline(xrdvi* h, int32_t S, uint64_t seed, int64_t capacity, uint64_t* rows, int64_t* n_rows,
                          void* scratch, size_t scratch_bytes);
 
+/* Measurement: timeline of ONE launch of update_draw_kernel (a-6 prior part, a-7, a-8 and the next a-1 / a-2), the serial
+ * section between two tile kernels.  Runs `steps` >= 2 optimisation steps from the internal state (the state advances) as
+ * xrdvi_fit enqueues them (programmatic dependent launches, outside a graph); in the last step but one thread 0 of every CTA of
+ * update_draw_kernel (an instantiation with the stamps compiled in; the product launches have none) writes eight
+ * %globaltimer words (ns):
+ *   [0] the CTA is resident, [1] it is done with everything that needs no output of the tile kernel (parameters, moments,
+ *   prior terms, bias corrections, Philox normals of the next draws), [2] its griddepcontrol.wait returned, [3] the output
+ *   slots (log-likelihood CTAs: the tiles) are added, [4] shuffle trees and barrier of the block reduction, [5] the
+ *   parameter of thread 0 is updated, [6] all parameters of the phase are (0 for log-likelihood CTAs and evaluations),
+ *   [7] the CTA is done.
+ * Rows are CTAs in launch order (instance-major: K phase CTAs, then the log-likelihood CTAs of the instance); one more row
+ * follows whose word [0] is the time at which the first warp of the NEXT step's tile kernel was past its
+ * griddepcontrol.wait (the earliest start stamp of xrdvi_debug_timeline's rows, taken in the last step).
+ * rows uint64 [capacity][8] (host), *n_rows = CTAs + 1; XRDVI_E_INVALID_ARG if capacity is smaller; scratch: DEVICE
+ * buffer of 64 bytes per CTA of update_draw_kernel + 32 bytes per warp of the tile kernel's launch.              */
+int xrdvi_debug_update_timeline(xrdvi* h, int32_t steps, int32_t S, uint64_t seed, int64_t capacity, uint64_t* rows,
+                                int64_t* n_rows, void* scratch, size_t scratch_bytes);
+
 /* Measurement: `steps` optimisation steps (graph replays, exactly as xrdvi_fit runs them), each one
  * bracketed by its own pair of CUDA events on the handle's stream; between two steps, outside the
  * brackets, the DEVICE buffer l2_flush (l2_flush_bytes; NULL / 0 = no flush) is overwritten so that every step

@@ -24,6 +24,7 @@ EXPORTS = (            # include/xrdvi.h: the product boundary
 )
 DEBUG_EXPORTS = (      # include/xrdvi_debug.h: read-backs for the parity tests, timing for bench.py and profiles/
     "xrdvi_debug_profile", "xrdvi_debug_draws", "xrdvi_time_kernels", "xrdvi_bench_steps", "xrdvi_debug_timeline",
+    "xrdvi_debug_update_timeline",
 )
 
 
@@ -99,6 +100,8 @@ def load_library():
     L.xrdvi_bench_steps.argtypes = [vp, C.c_int32, C.c_int32, C.c_uint64, vp, C.c_size_t, fp]
     L.xrdvi_debug_timeline.argtypes = [vp, C.c_int32, C.c_uint64, C.c_int64, C.POINTER(C.c_uint64), C.POINTER(C.c_int64),
                                        vp, C.c_size_t]
+    L.xrdvi_debug_update_timeline.argtypes = [vp, C.c_int32, C.c_int32, C.c_uint64, C.c_int64, C.POINTER(C.c_uint64),
+                                              C.POINTER(C.c_int64), vp, C.c_size_t]
     L.xrdvi_last_error.restype = C.c_char_p
     _lib = L
     return L
@@ -361,6 +364,40 @@ class Xrdvi:
         _check(load_library().xrdvi_debug_timeline(self._h, S, int(seed), int(capacity),
                                                    rows.ctypes.data_as(C.POINTER(C.c_uint64)), C.byref(n), ptr, nb))
         return rows[: n.value]
+
+    def debug_update_timeline(self, steps=40, S=None, seed=0, tile_warps=1 << 22):
+        """[CTAs + 1][8] %globaltimer stamps of one update_draw_kernel launch inside a run of `steps` steps
+        (xrdvi_debug_update_timeline); the last row's first word is the next tile kernel's start.  `tile_warps`: an upper
+        bound of the warps of one tile-kernel launch (sizes the scratch)."""
+        S = self.S_max if S is None else int(S)
+        cap = (self.K + (S + 31) // 32) * self.P * self.R + 1
+        rows = np.zeros((cap, 8), dtype=np.uint64)
+        n = C.c_int64(0)
+        scratch, ptr, nb = self._scratch(64 * cap + 32 * int(tile_warps))
+        _check(load_library().xrdvi_debug_update_timeline(self._h, int(steps), S, int(seed), cap,
+                                                          rows.ctypes.data_as(C.POINTER(C.c_uint64)), C.byref(n), ptr, nb))
+        return rows[: n.value]
+
+    def update_timeline_summary(self, steps=40, S=None, seed=0):
+        """Segment durations (ns; mean and max over the phase CTAs) of one update_draw_kernel launch, from
+        debug_update_timeline: the numbers of profiles/r2_update_kernel.md."""
+        S = self.S_max if S is None else int(S)
+        r = self.debug_update_timeline(steps=steps, S=S, seed=seed).astype(np.int64)
+        per_inst = self.K + (S + 31) // 32
+        u = r[:-1]
+        ph = u[[i for i in range(u.shape[0]) if i % per_inst < self.K]]
+        ll = u[[i for i in range(u.shape[0]) if i % per_inst >= self.K]]
+        t0 = int(u[:, 2].min())                                   # the first CTA's wait returned
+        d = np.diff(ph, axis=1)
+        names = ("before_the_wait", "waiting", "slots_and_prior_added", "shuffles_and_barrier", "own_parameter",
+                 "all_parameters", "draws_and_exit")
+        out = {"ctas": int(u.shape[0]),
+               "resident_before_wait_returned_ns": (int(t0 - u[:, 0].max()), int(t0 - u[:, 0].min())),
+               "segments_ns_mean_max": {n: (int(d[:, i].mean()), int(d[:, i].max())) for i, n in enumerate(names)},
+               "last_phase_cta_done_ns": int(ph[:, 7].max() - t0), "mean_phase_cta_done_ns": int((ph[:, 7] - t0).mean()),
+               "last_loglik_cta_done_ns": int(ll[:, 7].max() - t0),
+               "next_tile_kernel_past_its_wait_ns": int(r[-1, 0] - t0)}
+        return out
 
     def bench_steps(self, steps, S=None, seed=0, l2_flush_bytes=0):
         S = self.S_max if S is None else int(S)

@@ -566,8 +566,12 @@ int enqueue_step(xrdvi* h) {
     // both kernels may start while their predecessor drains (programmatic dependent launch); each waits with
     // griddep_wait() before it touches the predecessor's data
     launch_tile<true>(d, h->stream, nullptr, 0, pdl);                  // also finishes the previous step (ELBO, count)
-    launch_k(update_draw_kernel, dim3(d.K + d.gpi, d.PR), dim3(kUpdThreads), h->stream, pdl, static_cast<size_t>(d.upd_smem), d,
-             static_cast<const float*>(d.var), 1);
+    if (d.tlu)   // xrdvi_debug_update_timeline: the stamped instantiation
+        launch_k(update_draw_kernel<true>, dim3(d.K + d.gpi, d.PR), dim3(kUpdThreads), h->stream, pdl, static_cast<size_t>(d.upd_smem), d,
+                 static_cast<const float*>(d.var), 1);
+    else
+        launch_k(update_draw_kernel<false>, dim3(d.K + d.gpi, d.PR), dim3(kUpdThreads), h->stream, pdl, static_cast<size_t>(d.upd_smem), d,
+                 static_cast<const float*>(d.var), 1);
     CU(cudaGetLastError());
     return XRDVI_OK;
 }
@@ -586,7 +590,7 @@ int enqueue_eval(xrdvi* h, const float* var, float* f_dbg, long long n_dbg, bool
     if (forward_only) launch_tile<false>(d, h->stream, f_dbg, n_dbg);
     else launch_tile<true>(d, h->stream, f_dbg, n_dbg);
     // forward_only leaves stale partials in part8: the gradient output of this launch is not used then
-    update_draw_kernel<<<dim3(d.K + d.gpi, d.PR), kUpdThreads, d.upd_smem, h->stream>>>(d, var, 0);
+    update_draw_kernel<false><<<dim3(d.K + d.gpi, d.PR), kUpdThreads, d.upd_smem, h->stream>>>(d, var, 0);
     CU(cudaGetLastError());
     return enqueue_finish(h);
 }
@@ -1018,7 +1022,9 @@ int xrdvi_create(const double* x, int64_t N, const double* y, const double* bgin
     int rc = install_tables(h, tabs, nck0, true);
     if (rc == XRDVI_OK) {      // the update kernel's staging buffer: up to kUpdSmemCap of dynamic shared memory, sized by set_S
         set_S(h, S_max);
-        cudaError_t e = cudaFuncSetAttribute(update_draw_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kUpdSmemCap);
+        cudaError_t e = cudaFuncSetAttribute(update_draw_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kUpdSmemCap);
+        if (e == cudaSuccess)
+            e = cudaFuncSetAttribute(update_draw_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kUpdSmemCap);
         if (e != cudaSuccess) rc = fail(XRDVI_E_CUDA, std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e));
     }
     if (rc == XRDVI_OK) rc = xrdvi_reset_state(h, 0);
@@ -1499,7 +1505,7 @@ int xrdvi_time_kernels(xrdvi* h, int32_t S, uint64_t seed, int32_t reps, float* 
         CU(cudaEventRecord(h->ev[1], st));
         launch_tile<true>(d, st, nullptr, 0);
         CU(cudaEventRecord(h->ev[2], st));
-        update_draw_kernel<<<dim3(d.K + d.gpi, d.PR), kUpdThreads, d.upd_smem, st>>>(d, d.var, 0);
+        update_draw_kernel<false><<<dim3(d.K + d.gpi, d.PR), kUpdThreads, d.upd_smem, st>>>(d, d.var, 0);
         CU(cudaEventRecord(h->ev[3], st));
         launch_tile<false>(d, st, nullptr, 0);
         CU(cudaEventRecord(h->ev[4], st));
@@ -1543,7 +1549,7 @@ int xrdvi_debug_timeline(xrdvi* h, int32_t S, uint64_t seed, int64_t capacity, u
         d.tl = pass == 2 ? buf : nullptr;
         if (pass == 2) e = cudaMemsetAsync(buf, 0, sizeof(unsigned long long) * 4 * warps, st);
         launch_tile<true>(d, st, nullptr, 0);
-        update_draw_kernel<<<dim3(d.K + d.gpi, d.PR), kUpdThreads, h->dev.upd_smem, st>>>(h->dev, h->dev.var, 0);
+        update_draw_kernel<false><<<dim3(d.K + d.gpi, d.PR), kUpdThreads, h->dev.upd_smem, st>>>(h->dev, h->dev.var, 0);
         if (e == cudaSuccess) e = cudaGetLastError();
     }
     if (e == cudaSuccess) e = cudaMemcpyAsync(rows, buf, sizeof(unsigned long long) * 4 * warps, cudaMemcpyDeviceToHost, st);
@@ -1551,6 +1557,53 @@ int xrdvi_debug_timeline(xrdvi* h, int32_t S, uint64_t seed, int64_t capacity, u
     if (e != cudaSuccess) return fail(XRDVI_E_CUDA, std::string("debug_timeline: ") + cudaGetErrorString(e));
     *n_rows = warps;
     return enqueue_finish(h) ? XRDVI_E_CUDA : XRDVI_OK;
+}
+
+int xrdvi_debug_update_timeline(xrdvi* h, int32_t steps, int32_t S, uint64_t seed, int64_t capacity, uint64_t* rows,
+                                int64_t* n_rows, void* scratch, size_t scratch_bytes) {
+    int rc = check_S(h, S);
+    if (rc) return rc;
+    if (steps < 2 || !rows || !n_rows) return fail(XRDVI_E_INVALID_ARG, "steps < 2 or NULL output");
+    CU(cudaSetDevice(h->device));
+    rc = begin_steps(h, S, seed);
+    if (rc) return rc;
+    const Dev& d = h->dev;
+    const long long n_cta = static_cast<long long>(d.K + d.gpi) * d.PR;
+    if (n_cta + 1 > capacity) return fail(XRDVI_E_INVALID_ARG, "capacity < CTAs of update_draw_kernel + 1");
+    // the tile kernel of the step after the stamped one leaves its per-warp stamps (as in xrdvi_debug_timeline) behind the
+    // update kernel's rows: the earliest of them is the time at which the next step could begin
+    const long long warps = use_split(d) ? 2ll * d.n_tile * d.PS * d.G : static_cast<long long>(d.n_seg) * d.G * d.TW * d.PS;
+    const size_t u_bytes = sizeof(unsigned long long) * 8 * static_cast<size_t>(n_cta);
+    const size_t t_bytes = sizeof(unsigned long long) * 4 * static_cast<size_t>(warps);
+    if (!scratch || scratch_bytes < u_bytes + t_bytes)
+        return fail(XRDVI_E_WORKSPACE_TOO_SMALL,
+                    "debug_update_timeline: scratch smaller than 64 bytes per CTA of the update kernel + 32 per warp of the tile kernel");
+    unsigned long long* buf = static_cast<unsigned long long*>(scratch);
+    unsigned long long* buf_t = buf + 8 * n_cta;
+    cudaStream_t st = h->stream;
+    cudaError_t e = cudaMemsetAsync(buf, 0, u_bytes + t_bytes, st);
+    // the steps as xrdvi_fit enqueues them (programmatic launches), outside a graph
+    for (int i = 0; i < steps && e == cudaSuccess && rc == XRDVI_OK; ++i) {
+        h->dev.tlu = i == steps - 2 ? buf : nullptr;
+        h->dev.tl = i == steps - 1 ? buf_t : nullptr;
+        rc = enqueue_step(h);
+    }
+    h->dev.tlu = nullptr;
+    h->dev.tl = nullptr;
+    if (rc == XRDVI_OK) rc = enqueue_finish(h);
+    if (rc == XRDVI_OK) h->step_host += steps;
+    std::vector<unsigned long long> tl(static_cast<size_t>(warps) * 4);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(rows, buf, u_bytes, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(tl.data(), buf_t, t_bytes, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) return fail(XRDVI_E_CUDA, std::string("debug_update_timeline: ") + cudaGetErrorString(e));
+    if (rc != XRDVI_OK) return rc;
+    unsigned long long first = 0;
+    for (long long w = 0; w < warps; ++w)
+        if (tl[4 * w] && (!first || tl[4 * w] < first)) first = tl[4 * w];
+    for (int c = 0; c < 8; ++c) rows[8 * n_cta + c] = c == 0 ? first : 0;
+    *n_rows = n_cta + 1;
+    return XRDVI_OK;
 }
 
 int xrdvi_bench_steps(xrdvi* h, int32_t steps, int32_t S, uint64_t seed, void* flush, size_t flush_bytes, float* ms_steps) {

@@ -161,6 +161,9 @@ struct Dev {
     float* parta;             // [G][n_slots][2] (g_alpha, g_alpha eps_alpha) summed over the 32 draws
     // measurement (xrdvi_debug_timeline): nullptr, or [warps of the launch][4] = (start, end of phase 1, end, SM id | records << 32)
     unsigned long long* tl;
+    // measurement (xrdvi_debug_update_timeline): nullptr, or [CTAs of update_draw_kernel][8] %globaltimer stamps of
+    // thread 0 of every CTA of update_draw_kernel<true>
+    unsigned long long* tlu;
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -183,6 +186,13 @@ __device__ __forceinline__ void tl_stamp(unsigned long long* tl, unsigned row, i
         unsigned long long t;
         asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
         tl[static_cast<size_t>(row) * 4 + col] = t;
+    }
+}
+__device__ __forceinline__ void tlu_stamp(unsigned long long* tlu, unsigned row, int col) {   // thread 0 of a CTA
+    if (tlu && threadIdx.x == 0) {
+        unsigned long long t;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+        tlu[static_cast<size_t>(row) * 8 + col] = t;
     }
 }
 __device__ __forceinline__ void tl_tag(unsigned long long* tl, unsigned row, int records) {
@@ -1498,6 +1508,9 @@ __device__ __forceinline__ float2 prior_alpha(const Dev& d, float m_a, float sg_
     return make_float2(-0.5f * da * da * d.alpha_inv_var + d.alpha_logc + za, 1.0f - da * d.alpha_inv_var * al);
 }
 
+// STAMP: the instantiation xrdvi_debug_update_timeline launches (thread 0 of every CTA leaves %globaltimer stamps in d.tlu);
+// every other launch takes STAMP = false, which has none of that code.
+template <bool STAMP>
 __global__ void __launch_bounds__(kUpdThreads, 2) update_draw_kernel(const Dev d, const float* __restrict__ var_in,
                                                                   int do_update) {
     constexpr int kW = kUpdThreads / 32;
@@ -1529,6 +1542,8 @@ __global__ void __launch_bounds__(kUpdThreads, 2) update_draw_kernel(const Dev d
     // between the two lets this one start only after its own griddep_wait.  What the tile kernel writes (the output
     // slots, llpart, ctl->step / pending through finish_step) is read after the wait.
     // These loads bypass L1 (ld.global.cg): the SM may still hold lines the previous launches of this kernel read.
+    const unsigned tlu_row = blockIdx.y * gridDim.x + blockIdx.x;
+    if constexpr (STAMP) tlu_stamp(d.tlu, tlu_row, 0);                          // [0] the CTA is resident
     const long long step = __ldcg(&d.ctl->u_step) +        // completed steps; this is step + 1
         static_cast<long long>(__ldcg(&d.ctl->u_acc) / (static_cast<unsigned long long>(gridDim.x) * gridDim.y));
     const unsigned long long seed = __ldcg(&d.ctl->seed);
@@ -1584,8 +1599,10 @@ __global__ void __launch_bounds__(kUpdThreads, 2) update_draw_kernel(const Dev d
             if (d.asym) epa_n = normal_alpha(it_n, static_cast<unsigned>(s), static_cast<unsigned>(k), static_cast<unsigned>(inst), seed);
         }
     }
+    if constexpr (STAMP) tlu_stamp(d.tlu, tlu_row, 1);                          // [1] done with what needs no output of the tile kernel
     griddep_launch_dependents();
     griddep_wait();                               // output slots, llpart: written by the tile kernel
+    if constexpr (STAMP) tlu_stamp(d.tlu, tlu_row, 2);                          // [2] the wait returned
     if (fast && n_part > 0 && threadIdx.x == 0) {               // the slot rows of the phase, one contiguous piece per group
         const unsigned mb = smem_u32(&mbar_s), piece = 32u * static_cast<unsigned>(n_sl);
         mbar_expect_tx(mb, piece * static_cast<unsigned>(d.gpi));
@@ -1608,6 +1625,7 @@ __global__ void __launch_bounds__(kUpdThreads, 2) update_draw_kernel(const Dev d
             for (int j = 0; j < kLlBatch; ++j)
                 if (i + j < n_i) a += static_cast<double>(x[j]);
         }
+        if constexpr (STAMP) tlu_stamp(d.tlu, tlu_row, 3);                      // [3] log-likelihood CTA: the tiles are added
         ll_s[warp][lane] = a;
         __syncthreads();
         if (warp == 0) {
@@ -1625,6 +1643,7 @@ __global__ void __launch_bounds__(kUpdThreads, 2) update_draw_kernel(const Dev d
         }
         if (k == d.K && inst == 0 && threadIdx.x == 0) d.ctl->pending = do_update ? 2u : 1u;
         if (do_update && threadIdx.x == 0) atomicAdd(&d.ctl->u_acc, 1ull);    // this CTA is done (result unused: a reduction)
+        if constexpr (STAMP) tlu_stamp(d.tlu, tlu_row, 7);
         return;
     }
 
@@ -1710,6 +1729,7 @@ __global__ void __launch_bounds__(kUpdThreads, 2) update_draw_kernel(const Dev d
         }
     }
 
+    if constexpr (STAMP) tlu_stamp(d.tlu, tlu_row, 3);                          // [3] phase CTA: slots and prior terms are added
     // deterministic block reduction: fixed shuffle tree inside a warp, then thread i < 11 adds the warps' sums of
     // value i in warp order.  Thread i < 8 owns parameter i, threads 8 / 9 the alpha pair (sums 9 / 10), thread 10 sum 8.
     const int n_red = d.asym ? 11 : 9;
@@ -1725,6 +1745,7 @@ __global__ void __launch_bounds__(kUpdThreads, 2) update_draw_kernel(const Dev d
         for (int i = 0; i < 11; ++i) red[warp * 11 + i] = v[i];
     }
     __syncthreads();
+    if constexpr (STAMP) tlu_stamp(d.tlu, tlu_row, 4);                          // [4] shuffle trees and the barrier
     if (threadIdx.x < 11) {
         const int col = threadIdx.x < 8 ? threadIdx.x : threadIdx.x == 10 ? 8 : threadIdx.x + 1;
         double tot = 0.0;
@@ -1762,8 +1783,10 @@ __global__ void __launch_bounds__(kUpdThreads, 2) update_draw_kernel(const Dev d
             new_ml[threadIdx.x] = x;
         }
     }
+    if constexpr (STAMP) tlu_stamp(d.tlu, tlu_row, 5);                          // [5] the parameter of thread 0 is updated
     if (do_update) {       // draws of the next step from the updated parameters
         __syncthreads();
+        if constexpr (STAMP) tlu_stamp(d.tlu, tlu_row, 6);                      // [6] all parameters of the phase are updated
         const float4 mn = make_float4(new_ml[0], new_ml[1], new_ml[2], new_ml[3]);
         const float4 ln = make_float4(new_ml[4], new_ml[5], new_ml[6], new_ml[7]);
         const float mna = d.asym ? new_ml[8] : 0.0f, lna = d.asym ? new_ml[9] : 0.0f;
@@ -1780,6 +1803,7 @@ __global__ void __launch_bounds__(kUpdThreads, 2) update_draw_kernel(const Dev d
         }
     }
     if (do_update && threadIdx.x == 0) atomicAdd(&d.ctl->u_acc, 1ull);        // this CTA is done (result unused: a reduction)
+    if constexpr (STAMP) tlu_stamp(d.tlu, tlu_row, 7);                          // [7] done
 }
 
 // a-7 (last part): ELBO of every instance = mean log-likelihood + sum over the phases of (mean log prior + log

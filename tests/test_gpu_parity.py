@@ -496,3 +496,29 @@ def test_debug_timeline_rows_are_consistent():
     with pytest.raises(XrdviError):
         g.debug_timeline(capacity=8)
     g.close()
+
+
+def test_debug_update_timeline_rows_are_consistent():
+    """xrdvi_debug_update_timeline: one row per CTA of update_draw_kernel plus the next tile kernel's start; the stamps of
+    a CTA are ordered, every CTA is resident before its wait returns, the next step begins after the last CTA is done, and
+    the stamped run is the same fit as an unstamped one."""
+    wl = synth.make_workload(1, S=64)
+    g = Xrdvi.from_workload(wl)
+    rows = g.debug_update_timeline(steps=12, seed=3).astype(np.int64)
+    n_cta = wl.K + 2
+    assert rows.shape == (n_cta + 1, 8)
+    u = rows[:n_cta]
+    phase, ll = u[:wl.K], u[wl.K:]
+    assert (np.diff(phase, axis=1) >= 0).all()
+    assert (np.diff(ll[:, [0, 1, 2, 3, 7]], axis=1) >= 0).all() and (ll[:, 4:7] == 0).all()
+    assert rows[n_cta, 0] >= u[:, 7].max()                   # the next tile kernel waits for the whole launch
+    assert (u[:, 7].max() - u[:, 2].min()) < 50_000          # ns: the serial section is a few microseconds
+    h = Xrdvi.from_workload(wl)
+    st_h, _, _ = h.fit(12, seed=3)
+    st_g, _ = g.get_state()
+    assert np.array_equal(st_g, st_h)
+    summ = h.update_timeline_summary(steps=6, seed=3)
+    assert summ["ctas"] == n_cta and 0 < summ["last_phase_cta_done_ns"] <= summ["next_tile_kernel_past_its_wait_ns"] < 50_000
+    from paper_2501_09308_b200 import XrdviError
+    with pytest.raises(XrdviError):
+        g.debug_update_timeline(steps=1)                     # needs a stamped step and a step after it

@@ -82,3 +82,9 @@ def test_random_problem(seed):
     st2, inc, _ = gpu.fit(3, S=S, seed=5)
     assert np.isfinite(st2).all() and np.isfinite(inc).all()
     gpu.close()
+    # the same three steps on a second handle: bit for bit (fixed summation orders, no race between the kernels of a step)
+    gpu_b = Xrdvi(x, y, bg, ofs, pos, inten, S_max=S, **hp)
+    gpu_b.reset_state(seed=seed)
+    st2_b, inc_b, _ = gpu_b.fit(3, S=S, seed=5)
+    assert np.array_equal(st2, st2_b) and np.array_equal(inc, inc_b)
+    gpu_b.close()
