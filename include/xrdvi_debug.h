@@ -58,9 +58,11 @@ int xrdvi_debug_timeline(xrdvi* h, int32_t S, uint64_t seed, int64_t capacity, u
  *   [7] the CTA is done.
  * Rows are CTAs in launch order (instance-major: K phase CTAs, then the log-likelihood CTAs of the instance); one more row
  * follows whose word [0] is the time at which the first warp of the NEXT step's tile kernel was past its
- * griddepcontrol.wait (the earliest start stamp of xrdvi_debug_timeline's rows, taken in the last step).
+ * griddepcontrol.wait (the earliest start stamp of xrdvi_debug_timeline's rows, taken in the last step) and whose
+ * word [1] is the time at which the last warp of the SAME step's tile kernel was done (its stamps slow that launch by
+ * about 5 %, not the hand-over).
  * rows uint64 [capacity][8] (host), *n_rows = CTAs + 1; XRDVI_E_INVALID_ARG if capacity is smaller; scratch: DEVICE
- * buffer of 64 bytes per CTA of update_draw_kernel + 32 bytes per warp of the tile kernel's launch.              */
+ * buffer of 64 bytes per CTA of update_draw_kernel + 64 bytes per warp of the tile kernel's launch.              */
 int xrdvi_debug_update_timeline(xrdvi* h, int32_t steps, int32_t S, uint64_t seed, int64_t capacity, uint64_t* rows,
                                 int64_t* n_rows, void* scratch, size_t scratch_bytes);
 

@@ -373,7 +373,7 @@ class Xrdvi:
         cap = (self.K + (S + 31) // 32) * self.P * self.R + 1
         rows = np.zeros((cap, 8), dtype=np.uint64)
         n = C.c_int64(0)
-        scratch, ptr, nb = self._scratch(64 * cap + 32 * int(tile_warps))
+        scratch, ptr, nb = self._scratch(64 * cap + 64 * int(tile_warps))
         _check(load_library().xrdvi_debug_update_timeline(self._h, int(steps), S, int(seed), cap,
                                                           rows.ctypes.data_as(C.POINTER(C.c_uint64)), C.byref(n), ptr, nb))
         return rows[: n.value]
@@ -396,7 +396,8 @@ class Xrdvi:
                "segments_ns_mean_max": {n: (int(d[:, i].mean()), int(d[:, i].max())) for i, n in enumerate(names)},
                "last_phase_cta_done_ns": int(ph[:, 7].max() - t0), "mean_phase_cta_done_ns": int((ph[:, 7] - t0).mean()),
                "last_loglik_cta_done_ns": int(ll[:, 7].max() - t0),
-               "next_tile_kernel_past_its_wait_ns": int(r[-1, 0] - t0)}
+               "next_tile_kernel_past_its_wait_ns": int(r[-1, 0] - t0),
+               "tile_kernel_last_warp_done_ns": int(r[-1, 1] - t0)}
         return out
 
     def bench_steps(self, steps, S=None, seed=0, l2_flush_bytes=0):

@@ -1575,33 +1575,36 @@ int xrdvi_debug_update_timeline(xrdvi* h, int32_t steps, int32_t S, uint64_t see
     const long long warps = use_split(d) ? 2ll * d.n_tile * d.PS * d.G : static_cast<long long>(d.n_seg) * d.G * d.TW * d.PS;
     const size_t u_bytes = sizeof(unsigned long long) * 8 * static_cast<size_t>(n_cta);
     const size_t t_bytes = sizeof(unsigned long long) * 4 * static_cast<size_t>(warps);
-    if (!scratch || scratch_bytes < u_bytes + t_bytes)
+    if (!scratch || scratch_bytes < u_bytes + 2 * t_bytes)
         return fail(XRDVI_E_WORKSPACE_TOO_SMALL,
-                    "debug_update_timeline: scratch smaller than 64 bytes per CTA of the update kernel + 32 per warp of the tile kernel");
+                    "debug_update_timeline: scratch smaller than 64 bytes per CTA of the update kernel + 64 per warp of the tile kernel");
     unsigned long long* buf = static_cast<unsigned long long*>(scratch);
-    unsigned long long* buf_t = buf + 8 * n_cta;
+    unsigned long long* buf_t = buf + 8 * n_cta;            // tile kernel of the step after the stamped update kernel
+    unsigned long long* buf_t0 = buf_t + 4 * warps;         // tile kernel of the same step
     cudaStream_t st = h->stream;
-    cudaError_t e = cudaMemsetAsync(buf, 0, u_bytes + t_bytes, st);
+    cudaError_t e = cudaMemsetAsync(buf, 0, u_bytes + 2 * t_bytes, st);
     // the steps as xrdvi_fit enqueues them (programmatic launches), outside a graph
     for (int i = 0; i < steps && e == cudaSuccess && rc == XRDVI_OK; ++i) {
         h->dev.tlu = i == steps - 2 ? buf : nullptr;
-        h->dev.tl = i == steps - 1 ? buf_t : nullptr;
+        h->dev.tl = i == steps - 1 ? buf_t : i == steps - 2 ? buf_t0 : nullptr;
         rc = enqueue_step(h);
     }
     h->dev.tlu = nullptr;
     h->dev.tl = nullptr;
     if (rc == XRDVI_OK) rc = enqueue_finish(h);
     if (rc == XRDVI_OK) h->step_host += steps;
-    std::vector<unsigned long long> tl(static_cast<size_t>(warps) * 4);
+    std::vector<unsigned long long> tl(static_cast<size_t>(warps) * 8);
     if (e == cudaSuccess) e = cudaMemcpyAsync(rows, buf, u_bytes, cudaMemcpyDeviceToHost, st);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(tl.data(), buf_t, t_bytes, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(tl.data(), buf_t, 2 * t_bytes, cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
     if (e != cudaSuccess) return fail(XRDVI_E_CUDA, std::string("debug_update_timeline: ") + cudaGetErrorString(e));
     if (rc != XRDVI_OK) return rc;
-    unsigned long long first = 0;
-    for (long long w = 0; w < warps; ++w)
+    unsigned long long first = 0, last_end = 0;              // next tile kernel's first start; this step's tile kernel's last end
+    for (long long w = 0; w < warps; ++w) {
         if (tl[4 * w] && (!first || tl[4 * w] < first)) first = tl[4 * w];
-    for (int c = 0; c < 8; ++c) rows[8 * n_cta + c] = c == 0 ? first : 0;
+        last_end = std::max(last_end, tl[4 * (warps + w) + 2]);
+    }
+    for (int c = 0; c < 8; ++c) rows[8 * n_cta + c] = c == 0 ? first : c == 1 ? last_end : 0;
     *n_rows = n_cta + 1;
     return XRDVI_OK;
 }

@@ -512,6 +512,7 @@ def test_debug_update_timeline_rows_are_consistent():
     assert (np.diff(phase, axis=1) >= 0).all()
     assert (np.diff(ll[:, [0, 1, 2, 3, 7]], axis=1) >= 0).all() and (ll[:, 4:7] == 0).all()
     assert rows[n_cta, 0] >= u[:, 7].max()                   # the next tile kernel waits for the whole launch
+    assert 0 < rows[n_cta, 1] <= u[:, 2].min()               # and this launch for the whole tile kernel of its step
     assert (u[:, 7].max() - u[:, 2].min()) < 50_000          # ns: the serial section is a few microseconds
     h = Xrdvi.from_workload(wl)
     st_h, _, _ = h.fit(12, seed=3)
