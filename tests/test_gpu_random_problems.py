@@ -88,3 +88,36 @@ def test_random_problem(seed):
     st2_b, inc_b, _ = gpu_b.fit(3, S=S, seed=5)
     assert np.array_equal(st2, st2_b) and np.array_equal(inc, inc_b)
     gpu_b.close()
+
+
+@pytest.mark.parametrize("seed", list(range(16)))
+def test_random_problem_many_instances_fit_is_repeatable(seed):
+    """The same generator with up to 72 instances and up to 300 draws: a 30-step fit on two handles, the second in two
+    pieces, bit for bit (summation orders are fixed; the kernels of consecutive steps overlap only where it is safe)."""
+    x, y, bg, ofs, pos, inten, hp, S = random_problem(5000 + seed)
+    rng = np.random.default_rng(seed)
+    P, R = int(rng.choice([1, 2, 5, 9])), int(rng.choice([1, 3, 8]))
+    y = np.tile(y[:1], (P, 1)) * rng.uniform(0.5, 1.5, (P, 1))
+    bg = np.tile(bg[:1], (P, 1))
+    if hp["likelihood"]:
+        y = np.round(y)
+    hp["n_patterns"], hp["n_restarts"] = P, R
+    S = int(rng.choice([1, 5, 32, 33, 70, 256, 300]))
+    a = Xrdvi(x, y, bg, ofs, pos, inten, S_max=S, **hp)
+    st_a, inc_a, _ = a.fit(30, S=S, seed=9)
+    b = Xrdvi(x, y, bg, ofs, pos, inten, S_max=S, **hp)
+    b.fit(17, S=S, seed=9)
+    st_b, inc_b, _ = b.fit(13, S=S, seed=9)
+    assert np.isfinite(st_a).all() and np.isfinite(inc_a).all()
+    assert np.array_equal(st_a, st_b) and np.array_equal(inc_a, inc_b)
+    # and the ELBO / gradient at the fitted state against the oracle
+    o = orc.Oracle(x, y, bg, ofs, pos, inten, **{k: v for k, v in hp.items() if k != "general_grid"})
+    Se = min(S, 33)
+    elbo_r, grad_r = o.elbo_grad(st_a.astype(np.float64), Se, 7, 3)[:2]
+    elbo_g, grad_g = a.elbo_grad(state=st_a, S=Se, seed=7, iteration=3)
+    tol = TOL_ELBO if not hp["likelihood"] else 3e-4
+    np.testing.assert_allclose(elbo_g, elbo_r, rtol=tol, atol=1e-3)
+    err = np.abs(grad_g.astype(np.float64) - grad_r).max(axis=(0, 1, 3))
+    ref = np.maximum(np.abs(grad_r).max(axis=(0, 1, 3)), 1e-3)
+    assert (err / ref).max() <= TOL_GRAD, (hp, err / ref)
+    a.close(); b.close()
